@@ -1,0 +1,162 @@
+/*
+ * hsma.h -- C-ABI of the B200-native hot path of the harmonic surface mapping algorithm
+ * (HSMA, arXiv 1806.04801).  Citations are PAPER.md line numbers;
+ * "reading Sx/Gx" refers to DESIGN.md "Readings of the paper".
+ *
+ * The library computes, entirely in CUDA kernels for sm_100a (there is no CPU fallback):
+ *   (a) Phi_in at the monitoring (check) points, summed over the near image cells   Eq.(5)
+ *   (-) the least-squares fit of the harmonic coefficients A_nm                     Eq.(7)
+ *   (-) the harmonic surface mapping A_nm -> surface charge + dipole per node       Eq.(10),(11) PAPER.md:99-105
+ *   (b) Phi_in at all N sources over the near image cells, self excluded
+ *   (c) Phi_out at all N sources from the M sphere nodes (charge + dipole)          Eq.(10), Eq.(16)
+ *   (-) U = 1/2 sum q_i phi_i
+ *
+ * Conventions
+ *   - every call returns an hsma_status; nothing throws or aborts; out-params are untouched on error.
+ *   - "dev" pointers are CUDA device pointers owned by the caller; "host" pointers are host memory.
+ *   - Gaussian units, G = 1/r (Eq.1).  Coordinates are box coordinates in [0, L_a];
+ *     the library centres them (reading G10).
+ *   - periodic kinds: phi is in the gauge A_00 = 0 (reading S2); U is gauge free for neutral input.
+ *   - hsma_evaluate* are asynchronous on the plan's stream and perform no host synchronisation
+ *     (hsma_evaluate_host synchronises because it returns host data).
+ *   - preconditions not checked: particles inside the box, no coincident particles, no particle on
+ *     a check point (reading S13).
+ */
+#ifndef HSMA_H_
+#define HSMA_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct hsma_plan hsma_plan; /* opaque, library-owned */
+
+typedef enum {
+    HSMA_OK = 0,
+    HSMA_ERR_INVALID_ARG = -1,
+    HSMA_ERR_GEOMETRY = -2,       /* R_aux outside (R0, min_a (s_a+1/2) L_a]  (reading S7) */
+    HSMA_ERR_NOT_NEUTRAL = -3,    /* periodic axes need sum q = 0             (reading S17) */
+    HSMA_ERR_CUDA = -4,
+    HSMA_ERR_ALLOC = -5,
+    HSMA_ERR_RANK_DEFICIENT = -6  /* fitting matrix lost rank in the Householder QR */
+} hsma_status;
+
+typedef enum {
+    HSMA_BC_PERIODIC = 0,                  /* Eq.(3): all axes periodic             */
+    HSMA_BC_MIRROR_CAVITY = 1,             /* Eq.(4): all axes reflecting, gamma^|k| */
+    HSMA_BC_SLAB_XY_PERIODIC_Z_MIRROR = 2  /* x,y periodic, z reflecting (readings G11, S16)       */
+} hsma_boundary_kind;
+
+typedef enum {
+    HSMA_CLOSURE_BOUNDARY = 0, /* residual of the boundary condition at the check points */
+    HSMA_CLOSURE_FAR_DATA = 1  /* rhs = direct sum over the far cell table (reading S16, config 4)       */
+} hsma_closure;
+
+typedef enum {
+    HSMA_QUAD_SPIRAL = 0, /* exactly M nodes, Hannay-Nye warp on a golden-angle spiral (reading S10) */
+    HSMA_QUAD_LATTICE = 1 /* the paper's F1/F2 lattice, M = 2(F2+1), PAPER.md:124-126 (reading G4)   */
+} hsma_quad_rule;
+
+/* Plan descriptor (full form).  Set struct_size = sizeof(hsma_plan_desc); zero the rest first. */
+typedef struct {
+    size_t struct_size;
+    int kind;             /* hsma_boundary_kind */
+    double L[3];          /* box sides */
+    int near_shell[3];    /* near cells |k_a| <= near_shell[a]; whole cells (reading S7) */
+    double gamma;         /* reflection factor per mirror reflection (-1 = grounded metal) */
+    double R_aux;         /* radius of the auxiliary sphere */
+    int p;                /* harmonic degrees n = 0..p-1, p*p unknowns (reading S1); 1 <= p <= 32 */
+    int M;                /* integration nodes on the sphere; M >= 8 */
+    int K;                /* check points (periodic: K points + their K wrapped partners) */
+    const double* check_xyz; /* host [K,3] CENTRED coordinates, or NULL: the library's rule
+                                (periodic: Fibonacci grid on the circumsphere PAPER.md:82;
+                                 otherwise a deterministic low-discrepancy set on the faces) */
+    int closure;          /* hsma_closure */
+    int far_shell[3];     /* HSMA_CLOSURE_FAR_DATA only: far table = cells within far_shell minus near */
+    int quad_rule;        /* hsma_quad_rule */
+    int rsqrt_refine;     /* refinement of the MUFU.RSQ64H seed in the source near sum (b):
+                             1 = one mean-centred Newton step (|err| <= 1.2e-12 per pair, 10 FP64 instr/pair),
+                             2 = one cubic (Halley) step (|err| <= 5e-16, 12 instr/pair),
+                             0 = library default: 2 while N*N*cells < 2^32 pairs (latency-bound), else 1.
+                             Steps (a) and (c) always use the cubic step. */
+} hsma_plan_desc;
+
+/*
+ * north_star form: cubic box of side L, same shell on all axes, K = 2 p^2 check points (PAPER.md:163
+ * N_m = 2P^2), gamma = -1 for mirror kinds, spiral nodes, boundary closure.
+ * `cuda_stream` is a cudaStream_t (NULL = default stream); all work of the plan runs on it.
+ * Preparation step of PAPER.md:140: cell table, check points, nodes, fitting matrix, its Householder
+ * QR (device, single block).  Synchronises the stream before returning.
+ */
+hsma_status hsma_plan_create(double L, int boundary_kind, int near_shell, double R_aux, int p,
+                             int M_fib, void* cuda_stream, hsma_plan** plan_out);
+hsma_status hsma_plan_create_ex(const hsma_plan_desc* desc, void* cuda_stream, hsma_plan** plan_out);
+hsma_status hsma_plan_destroy(hsma_plan* plan);
+
+/*
+ * Update step of PAPER.md:142 for N sources.
+ *   xyz      dev [N,3] row-major box coordinates; q dev [N]
+ *   phi_out  dev [N]   potential at every source (near images + sphere nodes, bare self term excluded)
+ *   energy_out dev [1] U = 1/2 sum q_i phi_i, or NULL
+ */
+hsma_status hsma_evaluate(hsma_plan* plan, const double* xyz, const double* q, long long N,
+                          double* phi_out, double* energy_out);
+/*
+ * Target-sharded form (multi-GPU): phi only at sources t0 <= i < t1;
+ * phi_out dev [t1-t0]; energy_out dev [1] = 1/2 sum_{t0<=i<t1} q_i phi_i.  Step (a) and the fit are
+ * computed in full (they need all sources).
+ */
+hsma_status hsma_evaluate_shard(hsma_plan* plan, const double* xyz, const double* q, long long N,
+                                long long t0, long long t1, double* phi_out, double* energy_out);
+/*
+ * End-to-end form with HOST buffers: copies xyz,q to the device, evaluates, copies phi (and U) back,
+ * synchronises.  phi_host [N] may be NULL (energy only); energy_host [1] may be NULL.
+ */
+hsma_status hsma_evaluate_host(hsma_plan* plan, const double* xyz_host, const double* q_host,
+                               long long N, double* phi_host, double* energy_host);
+
+/* Synchronise the plan's stream and return the sticky status of the evaluations since the last
+ * call (HSMA_ERR_NOT_NEUTRAL, HSMA_ERR_CUDA, ...), then clear it. */
+hsma_status hsma_plan_sync(hsma_plan* plan);
+
+const char* hsma_status_string(int status);
+
+/* ---- introspection / test and bench hooks ------------------------------------------------------- */
+/* sizes: what[0]=rows of the fit, [1]=columns, [2]=check targets K_t, [3]=near cells, [4]=rhs cells,
+ * [5]=M nodes, [6]=p, [7]=kernels launched by the last evaluate.  host out [8]. */
+hsma_status hsma_plan_info(hsma_plan* plan, long long* what_out);
+/* copies of plan/evaluate state into caller DEVICE buffers (valid after an evaluate on the stream) */
+hsma_status hsma_get_coeffs(hsma_plan* plan, double* A_out /* dev [p*p], R0-scaled basis */);
+hsma_status hsma_get_rhs(hsma_plan* plan, double* rhs_out /* dev [rows] */);
+hsma_status hsma_get_check_targets(hsma_plan* plan, double* xyz_out /* dev [K_t,3] centred */);
+hsma_status hsma_get_nodes(hsma_plan* plan, double* xyz_out /* dev [M,3] */, double* w_out /* dev [M] */);
+hsma_status hsma_get_surface(hsma_plan* plan, double* Q_out /* dev [M] */, double* P_out /* dev [M,3] dipole vectors */);
+hsma_status hsma_get_fit_residual(hsma_plan* plan, double* rms_out /* host [1]; synchronises */);
+
+/*
+ * Raw kernel (a)/(b): phi[t] = sum_c w_c sum_j q_j / | tgt_t - (sign_c o src_j + shift_c) |  Eq.(5) PAPER.md:64.
+ *   tgt dev [T,3], src dev [N,3] (both centred), q dev [N]; shift, sign HOST [C,3] (sign = +-1), w HOST [C].
+ *   self_offset >= 0: target t is source self_offset+t, skipped in cell `central_cell` (-1: none).
+ *   refine: 1 Newton / 2 cubic.  Runs on `cuda_stream`; synchronises it before returning (it frees its scratch).
+ */
+hsma_status hsma_direct_sum(const double* tgt, long long T, const double* src, const double* q,
+                            long long N, const double* shift_host, const double* sign_host,
+                            const double* w_host, int C, int central_cell, long long self_offset,
+                            int refine, double* phi_out, void* cuda_stream);
+/* Raw kernel (c): phi[t] = sum_j Q_j/rho - P_j.(t - R_j)/rho^3.  All dev pointers; R [M,3], P [M,3]. */
+hsma_status hsma_node_sum(const double* tgt, long long T, const double* R, const double* Q,
+                          const double* P, long long M, double* phi_out, void* cuda_stream);
+
+/* DFMA-only microbenchmark on the current device: sustained FP64 FMA TFLOP/s over ~`seconds`
+ * (the roofline denominator).  host out; synchronises. */
+hsma_status hsma_fp64_peak(double seconds, double* tflops_out, double* sm_clock_mhz_out);
+
+/* total number of kernels this library has launched in this process */
+long long hsma_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HSMA_H_ */

@@ -1,0 +1,255 @@
+"""ctypes binding of include/hsma.h -- argument marshalling only.
+
+Every function has the name of the C entry point it calls; torch tensors are used for device
+memory (their data_ptr() is passed through) and for the CUDA stream.  Nothing of the method is
+computed here, and nothing here imports oracle/.  If libhsma_b200.so is missing and cannot be
+built the import fails loudly: there is no CPU fallback."""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+import torch
+
+from . import build as _build
+
+c_double_p = ctypes.POINTER(ctypes.c_double)
+
+HSMA_OK = 0
+HSMA_ERR_INVALID_ARG, HSMA_ERR_GEOMETRY, HSMA_ERR_NOT_NEUTRAL = -1, -2, -3
+HSMA_ERR_CUDA, HSMA_ERR_ALLOC, HSMA_ERR_RANK_DEFICIENT = -4, -5, -6
+HSMA_BC_PERIODIC, HSMA_BC_MIRROR_CAVITY, HSMA_BC_SLAB_XY_PERIODIC_Z_MIRROR = 0, 1, 2
+HSMA_CLOSURE_BOUNDARY, HSMA_CLOSURE_FAR_DATA = 0, 1
+HSMA_QUAD_SPIRAL, HSMA_QUAD_LATTICE = 0, 1
+
+
+class hsma_plan_desc(ctypes.Structure):
+    _fields_ = [("struct_size", ctypes.c_size_t), ("kind", ctypes.c_int), ("L", ctypes.c_double * 3),
+                ("near_shell", ctypes.c_int * 3), ("gamma", ctypes.c_double), ("R_aux", ctypes.c_double),
+                ("p", ctypes.c_int), ("M", ctypes.c_int), ("K", ctypes.c_int), ("check_xyz", c_double_p),
+                ("closure", ctypes.c_int), ("far_shell", ctypes.c_int * 3), ("quad_rule", ctypes.c_int),
+                ("rsqrt_refine", ctypes.c_int)]
+
+
+class HsmaError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        super().__init__(f"{where}: {hsma_status_string(status)} ({status})")
+
+
+_lib = None
+
+_SIGNATURES = {
+    "hsma_plan_create": (ctypes.c_int, [ctypes.c_double, ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_int,
+                                        ctypes.c_int, ctypes.c_void_p, ctypes.POINTER(ctypes.c_void_p)]),
+    "hsma_plan_create_ex": (ctypes.c_int, [ctypes.POINTER(hsma_plan_desc), ctypes.c_void_p,
+                                           ctypes.POINTER(ctypes.c_void_p)]),
+    "hsma_plan_destroy": (ctypes.c_int, [ctypes.c_void_p]),
+    "hsma_evaluate": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_longlong,
+                                     ctypes.c_void_p, ctypes.c_void_p]),
+    "hsma_evaluate_shard": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_longlong,
+                                           ctypes.c_longlong, ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p]),
+    "hsma_evaluate_host": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_longlong,
+                                          ctypes.c_void_p, ctypes.c_void_p]),
+    "hsma_plan_sync": (ctypes.c_int, [ctypes.c_void_p]),
+    "hsma_status_string": (ctypes.c_char_p, [ctypes.c_int]),
+    "hsma_plan_info": (ctypes.c_int, [ctypes.c_void_p, ctypes.POINTER(ctypes.c_longlong)]),
+    "hsma_get_coeffs": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p]),
+    "hsma_get_rhs": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p]),
+    "hsma_get_check_targets": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p]),
+    "hsma_get_nodes": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]),
+    "hsma_get_surface": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]),
+    "hsma_get_fit_residual": (ctypes.c_int, [ctypes.c_void_p, c_double_p]),
+    "hsma_direct_sum": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p,
+                                       ctypes.c_longlong, c_double_p, c_double_p, c_double_p, ctypes.c_int,
+                                       ctypes.c_int, ctypes.c_longlong, ctypes.c_int, ctypes.c_void_p,
+                                       ctypes.c_void_p]),
+    "hsma_node_sum": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p,
+                                     ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p]),
+    "hsma_fp64_peak": (ctypes.c_int, [ctypes.c_double, c_double_p, c_double_p]),
+    "hsma_launch_count": (ctypes.c_longlong, []),
+}
+EXPORTS = tuple(_SIGNATURES)
+
+
+def library_path() -> str:
+    return _build.LIB
+
+
+def load_library() -> ctypes.CDLL:
+    """Load (building first if stale) libhsma_b200.so.  Raises if it cannot be had."""
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        if not os.path.exists(path):
+            raise RuntimeError("libhsma_b200.so missing: the CUDA extension is required (no CPU fallback)")
+        lib = ctypes.CDLL(path)
+        for name, (res, args) in _SIGNATURES.items():
+            fn = getattr(lib, name)
+            fn.restype, fn.argtypes = res, args
+        _lib = lib
+    return _lib
+
+
+def hsma_status_string(status: int) -> str:
+    return load_library().hsma_status_string(int(status)).decode()
+
+
+def _check(status: int, where: str):
+    if status != HSMA_OK:
+        raise HsmaError(status, where)
+
+
+def _dev(t: Optional[torch.Tensor], n: Optional[int] = None, name: str = "tensor") -> Optional[int]:
+    if t is None:
+        return None
+    if not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+        raise TypeError(f"{name}: need a contiguous float64 CUDA tensor")
+    if n is not None and t.numel() < n:
+        raise ValueError(f"{name}: {t.numel()} elements, need {n}")
+    return t.data_ptr()
+
+
+def _host(a, name="array") -> np.ndarray:
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    return a
+
+
+def _hp(a: np.ndarray):
+    return a.ctypes.data_as(c_double_p)
+
+
+def _stream_ptr(stream) -> Optional[int]:
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return stream.cuda_stream or None
+
+
+def hsma_plan_create(L: float, boundary_kind: int, near_shell: int, R_aux: float, p: int, M_fib: int,
+                     stream=None) -> int:
+    h = ctypes.c_void_p()
+    _check(load_library().hsma_plan_create(L, boundary_kind, near_shell, R_aux, p, M_fib, _stream_ptr(stream),
+                                           ctypes.byref(h)), "hsma_plan_create")
+    return h.value
+
+
+def hsma_plan_create_ex(*, kind: int, L: Sequence[float], near_shell: Sequence[int], gamma: float, R_aux: float,
+                        p: int, M: int, K: int, check_xyz=None, closure: int = 0, far_shell=(0, 0, 0),
+                        quad_rule: int = 0, rsqrt_refine: int = 0, stream=None) -> int:
+    d = hsma_plan_desc()
+    d.struct_size = ctypes.sizeof(hsma_plan_desc)
+    d.kind = kind
+    d.L[:] = [float(v) for v in L]
+    d.near_shell[:] = [int(v) for v in near_shell]
+    d.gamma, d.R_aux, d.p, d.M, d.K = float(gamma), float(R_aux), int(p), int(M), int(K)
+    keep = None
+    if check_xyz is not None:
+        keep = _host(check_xyz)
+        if keep.shape != (K, 3):
+            raise ValueError("check_xyz must be [K,3]")
+        d.check_xyz = _hp(keep)
+    d.closure = closure
+    d.far_shell[:] = [int(v) for v in far_shell]
+    d.quad_rule, d.rsqrt_refine = int(quad_rule), int(rsqrt_refine)
+    h = ctypes.c_void_p()
+    _check(load_library().hsma_plan_create_ex(ctypes.byref(d), _stream_ptr(stream), ctypes.byref(h)),
+           "hsma_plan_create_ex")
+    return h.value
+
+
+def hsma_plan_destroy(plan: int):
+    _check(load_library().hsma_plan_destroy(plan), "hsma_plan_destroy")
+
+
+def hsma_evaluate(plan: int, xyz: torch.Tensor, q: torch.Tensor, phi_out: torch.Tensor,
+                  energy_out: Optional[torch.Tensor] = None):
+    N = q.numel()
+    _check(load_library().hsma_evaluate(plan, _dev(xyz, 3 * N, "xyz"), _dev(q, N, "q"), N, _dev(phi_out, N, "phi_out"),
+                                        _dev(energy_out, 1, "energy_out")), "hsma_evaluate")
+
+
+def hsma_evaluate_shard(plan: int, xyz: torch.Tensor, q: torch.Tensor, t0: int, t1: int, phi_out: torch.Tensor,
+                        energy_out: Optional[torch.Tensor] = None):
+    N = q.numel()
+    _check(load_library().hsma_evaluate_shard(plan, _dev(xyz, 3 * N, "xyz"), _dev(q, N, "q"), N, t0, t1,
+                                              _dev(phi_out, max(t1 - t0, 0), "phi_out"),
+                                              _dev(energy_out, 1, "energy_out")), "hsma_evaluate_shard")
+
+
+def hsma_evaluate_host(plan: int, xyz: np.ndarray, q: np.ndarray, phi_out: Optional[np.ndarray],
+                       energy_out: Optional[np.ndarray]):
+    """xyz [N,3], q [N], phi_out [N], energy_out [1]: C-contiguous float64 HOST arrays (pinned or not)."""
+    for a in (xyz, q, phi_out, energy_out):
+        if a is not None and not (a.dtype == np.float64 and a.flags.c_contiguous):
+            raise TypeError("host buffers must be C-contiguous float64")
+    N = q.shape[0]
+    _check(load_library().hsma_evaluate_host(plan, xyz.ctypes.data, q.ctypes.data, N,
+                                             None if phi_out is None else phi_out.ctypes.data,
+                                             None if energy_out is None else energy_out.ctypes.data),
+           "hsma_evaluate_host")
+
+
+def hsma_plan_sync(plan: int):
+    _check(load_library().hsma_plan_sync(plan), "hsma_plan_sync")
+
+
+def hsma_plan_info(plan: int) -> dict:
+    w = (ctypes.c_longlong * 8)()
+    _check(load_library().hsma_plan_info(plan, w), "hsma_plan_info")
+    keys = ("rows", "cols", "check_targets", "near_cells", "rhs_cells", "M", "p", "launches_last_evaluate")
+    return dict(zip(keys, [int(v) for v in w]))
+
+
+def hsma_get_coeffs(plan: int, A_out: torch.Tensor):
+    _check(load_library().hsma_get_coeffs(plan, _dev(A_out)), "hsma_get_coeffs")
+
+
+def hsma_get_rhs(plan: int, rhs_out: torch.Tensor):
+    _check(load_library().hsma_get_rhs(plan, _dev(rhs_out)), "hsma_get_rhs")
+
+
+def hsma_get_check_targets(plan: int, xyz_out: torch.Tensor):
+    _check(load_library().hsma_get_check_targets(plan, _dev(xyz_out)), "hsma_get_check_targets")
+
+
+def hsma_get_nodes(plan: int, xyz_out: Optional[torch.Tensor], w_out: Optional[torch.Tensor]):
+    _check(load_library().hsma_get_nodes(plan, _dev(xyz_out), _dev(w_out)), "hsma_get_nodes")
+
+
+def hsma_get_surface(plan: int, Q_out: Optional[torch.Tensor], P_out: Optional[torch.Tensor]):
+    _check(load_library().hsma_get_surface(plan, _dev(Q_out), _dev(P_out)), "hsma_get_surface")
+
+
+def hsma_get_fit_residual(plan: int) -> float:
+    v = ctypes.c_double()
+    _check(load_library().hsma_get_fit_residual(plan, ctypes.byref(v)), "hsma_get_fit_residual")
+    return v.value
+
+
+def hsma_direct_sum(tgt: torch.Tensor, src: torch.Tensor, q: torch.Tensor, shift, sign, w, central_cell: int,
+                    self_offset: int, refine: int, phi_out: torch.Tensor, stream=None):
+    shift, sign, w = _host(shift), _host(sign), _host(w)
+    T, N, C = tgt.shape[0], q.numel(), w.shape[0]
+    _check(load_library().hsma_direct_sum(_dev(tgt, 3 * T, "tgt"), T, _dev(src, 3 * N, "src"), _dev(q, N, "q"), N,
+                                          _hp(shift), _hp(sign), _hp(w), C, central_cell, self_offset, refine,
+                                          _dev(phi_out, T, "phi_out"), _stream_ptr(stream)), "hsma_direct_sum")
+
+
+def hsma_node_sum(tgt: torch.Tensor, R: torch.Tensor, Q: torch.Tensor, P: torch.Tensor, phi_out: torch.Tensor,
+                  stream=None):
+    T, M = tgt.shape[0], Q.numel()
+    _check(load_library().hsma_node_sum(_dev(tgt, 3 * T, "tgt"), T, _dev(R, 3 * M, "R"), _dev(Q, M, "Q"),
+                                        _dev(P, 3 * M, "P"), M, _dev(phi_out, T, "phi_out"), _stream_ptr(stream)),
+           "hsma_node_sum")
+
+
+def hsma_fp64_peak(seconds: float = 1.0):
+    t, c = ctypes.c_double(), ctypes.c_double()
+    _check(load_library().hsma_fp64_peak(seconds, ctypes.byref(t), ctypes.byref(c)), "hsma_fp64_peak")
+    return t.value, c.value
+
+
+def hsma_launch_count() -> int:
+    return int(load_library().hsma_launch_count())

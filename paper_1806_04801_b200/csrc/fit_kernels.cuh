@@ -1,0 +1,232 @@
+// The small dense steps that connect the pair sums: fitting matrix, Householder QR (plan time),
+// Q^T b + back-substitution (H3), harmonic-to-surface mapping (H4).  DESIGN.md "Kernels".
+#pragma once
+#include "common.cuh"
+
+namespace hsma {
+
+constexpr int kMaxP = 32;
+constexpr double kInv4Pi = 0.07957747154594767280;   // 1/(4 pi)
+constexpr double kSqrtInv4Pi = 0.28209479177387814347;  // sqrt(1/(4 pi))
+
+// Real orthonormal solid harmonics (r/a)^n Y_nm, n < p (Eq.6; real form PAPER.md:140;
+// reading S4), evaluated without trigonometry or division by rho:
+//   xi = (x + i y)/a, zeta = z/a, rho2 = |r|^2/a^2
+//   V_m^m     = K_m xi^m,  K_0 = sqrt(1/4pi), K_m = K_{m-1} sqrt((2m+1)/(2m))
+//   V_{m+1}^m = sqrt(2m+3) zeta V_m^m
+//   V_n^m     = a_nm (zeta V_{n-1}^m - b_nm rho2 V_{n-2}^m),
+//               a_nm = sqrt((4n^2-1)/(n^2-m^2)),  b_nm = sqrt(((n-1)^2-m^2)/(4(n-1)^2-1))
+// (the fully normalised associated-Legendre recurrences with (r/a)^n folded in).  Column n^2+n+m:
+// m = 0: Re V_n^0;  m > 0: sqrt2 Re V_n^m (cos);  -m: sqrt2 Im V_n^m (sin).
+// f(n, m, vc, vs) is called once per (n, m >= 0) with vc/vs the cos/sin members already scaled.
+template <class F>
+__device__ __forceinline__ void solid_harmonics(double x, double y, double z, double inv_a, int p, F f) {
+    const double xr = x * inv_a, xi = y * inv_a, zeta = z * inv_a;
+    const double rho2 = xr * xr + xi * xi + zeta * zeta;
+    double er = kSqrtInv4Pi, ei = 0.0;  // K_m xi^m
+    for (int m = 0; m < p; ++m) {
+        if (m > 0) {
+            const double k = sqrt((2.0 * m + 1.0) / (2.0 * m));
+            const double nr = k * (er * xr - ei * xi), ni = k * (er * xi + ei * xr);
+            er = nr; ei = ni;
+        }
+        const double s = m == 0 ? 1.0 : 1.4142135623730951;
+        double c2 = 0.0, s2 = 0.0;            // V_{n-2}^m
+        double c1 = er, s1 = ei;              // V_{n-1}^m (starts at n-1 = m)
+        f(m, m, s * c1, s * s1);
+        for (int n = m + 1; n < p; ++n) {
+            const double nn = (double)n, mm = (double)m;
+            const double anm = sqrt((4.0 * nn * nn - 1.0) / (nn * nn - mm * mm));
+            const double bnm = n == m + 1 ? 0.0 : sqrt(((nn - 1.0) * (nn - 1.0) - mm * mm) / (4.0 * (nn - 1.0) * (nn - 1.0) - 1.0));
+            const double c0 = anm * (zeta * c1 - bnm * rho2 * c2);
+            const double s0 = anm * (zeta * s1 - bnm * rho2 * s2);
+            f(n, m, s * c0, s * s0);
+            c2 = c1; s2 = s1; c1 = c0; s1 = s0;
+        }
+    }
+}
+
+// Fitting matrix, column-major [rows x ncol] (ld = rows).  PAPER.md:72-82.
+//   periodic (pairs = 1): row_i = B(x_i) - B(x~_i), constant column dropped (reading S2): col = idx - 1
+//   otherwise:            row_i = B(x_i)
+// chk: [K_t,3] centred check targets, x_i = chk[i], x~_i = chk[rows + i].
+__global__ void build_fit_matrix_kernel(const double* __restrict__ chk, int rows, int pairs, int p, double inv_R0,
+                                        double* __restrict__ Fm) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= rows) return;
+    const int drop = pairs ? 1 : 0;
+    const double* a = chk + 3 * (size_t)i;
+    solid_harmonics(a[0], a[1], a[2], inv_R0, p, [&](int n, int m, double vc, double vs) {
+        const int cc = n * n + n + m - drop, cs = n * n + n - m - drop;
+        if (cc >= 0) Fm[(size_t)cc * rows + i] = vc;
+        if (m > 0) Fm[(size_t)cs * rows + i] = vs;
+    });
+    if (pairs) {
+        const double* b = chk + 3 * (size_t)(rows + i);
+        solid_harmonics(b[0], b[1], b[2], inv_R0, p, [&](int n, int m, double vc, double vs) {
+            const int cc = n * n + n + m - drop, cs = n * n + n - m - drop;
+            if (cc >= 0) Fm[(size_t)cc * rows + i] -= vc;
+            if (m > 0) Fm[(size_t)cs * rows + i] -= vs;
+        });
+    }
+}
+
+// ---- block-wide helpers (blockDim.x = 1024) --------------------------------------------------
+__device__ __forceinline__ double warp_sum(double a) {
+    for (int o = 16; o; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
+    return a;
+}
+__device__ __forceinline__ double block_sum(double a, double* sh /* [32] */) {
+    a = warp_sum(a);
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    __syncthreads();
+    if (l == 0) sh[w] = a;
+    __syncthreads();
+    double b = l < (int)(blockDim.x >> 5) ? sh[l] : 0.0;
+    return warp_sum(b);  // every thread gets the same value, same order
+}
+
+// apply H = I - tau v v^T (v[0] = 1 implicit, v stored in col k of A below the diagonal) to the
+// columns j0..j1-1 of B (rows k..m-1); one warp per column.
+__device__ __forceinline__ void apply_reflector(const double* __restrict__ v, double tau, int k, int m, double* B,
+                                                int ldb, int j0, int j1) {
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31, nw = blockDim.x >> 5;
+    for (int j = j0 + w; j < j1; j += nw) {
+        double* col = B + (size_t)j * ldb;
+        double s = 0.0;
+        for (int i = k + 1 + l; i < m; i += 32) s += v[i] * col[i];
+        s = warp_sum(s) + col[k];
+        const double ts = tau * s;
+        for (int i = k + 1 + l; i < m; i += 32) col[i] -= ts * v[i];
+        __syncwarp();
+        if (l == 0) col[k] -= ts;
+    }
+}
+
+// Householder QR of A [m x n] column-major in place (LAPACK dgeqr2 convention): R in the upper
+// triangle, reflector vectors below the diagonal, tau[n].  Then the thin Q [m x n] is formed
+// explicitly in Qm (dorg2r) and R copied to Rm [n x n] column-major.  Single block.  Eq.(7) PAPER.md:76-78,
+// preparation step PAPER.md:140.  flag[0] = 1 if |R_kk| <= 1e-13 max|R_jj| (rank deficient).
+__global__ void __launch_bounds__(1024) householder_qr_kernel(double* __restrict__ A, int m, int n,
+                                                              double* __restrict__ tau, double* __restrict__ Qm,
+                                                              double* __restrict__ Rm, int* __restrict__ flag) {
+    __shared__ double sh[32];
+    __shared__ double s_tau;
+    for (int k = 0; k < n; ++k) {
+        double* x = A + (size_t)k * m;
+        double ss = 0.0;
+        for (int i = k + 1 + threadIdx.x; i < m; i += blockDim.x) ss += x[i] * x[i];
+        ss = block_sum(ss, sh);
+        const double alpha = x[k];
+        __syncthreads();
+        const double beta = -copysign(sqrt(alpha * alpha + ss), alpha);
+        const double t = (ss == 0.0) ? 0.0 : (beta - alpha) / beta;
+        const double inv = (ss == 0.0) ? 0.0 : 1.0 / (alpha - beta);
+        for (int i = k + 1 + threadIdx.x; i < m; i += blockDim.x) x[i] *= inv;
+        if (threadIdx.x == 0) { x[k] = (ss == 0.0) ? alpha : beta; tau[k] = t; s_tau = t; }
+        __syncthreads();
+        apply_reflector(x, s_tau, k, m, A, m, k + 1, n);
+        __syncthreads();
+    }
+    // R, rank check
+    for (int idx = threadIdx.x; idx < n * n; idx += blockDim.x) {
+        const int i = idx % n, j = idx / n;
+        Rm[idx] = i <= j ? A[(size_t)j * m + i] : 0.0;
+    }
+    if (threadIdx.x == 0) {
+        double mx = 0.0, mn = 1e300;
+        for (int k = 0; k < n; ++k) { const double d = fabs(A[(size_t)k * m + k]); mx = fmax(mx, d); mn = fmin(mn, d); }
+        flag[0] = (mn <= 1e-13 * mx) ? 1 : 0;
+    }
+    // thin Q = H_0 ... H_{n-1} [I; 0]
+    for (size_t idx = threadIdx.x; idx < (size_t)m * n; idx += blockDim.x) {
+        const int i = (int)(idx % m), j = (int)(idx / m);
+        Qm[idx] = i == j ? 1.0 : 0.0;
+    }
+    __syncthreads();
+    for (int k = n - 1; k >= 0; --k) {
+        apply_reflector(A + (size_t)k * m, tau[k], k, m, Qm, m, k, n);
+        __syncthreads();
+    }
+}
+
+// H3: rhs from the check-point sums, c = Q^T rhs, back-substitution R A = c.  Single block.
+//   pc [K_t] check-point potentials; pairs: rhs_i = sgn (pc[i] - pc[rows+i]); else rhs_i = sgn pc[i]
+//   A_full [p*p] in the R0-scaled basis (A_00 = 0 when the constant column was dropped)
+__global__ void __launch_bounds__(1024) ls_solve_kernel(const double* __restrict__ pc, int rows, int ncol, int pairs,
+                                                        double sgn, const double* __restrict__ Qm,
+                                                        const double* __restrict__ Rm, double* __restrict__ rhs,
+                                                        double* __restrict__ cvec, double* __restrict__ A_full) {
+    extern __shared__ double c[];  // [ncol]
+    for (int i = threadIdx.x; i < rows; i += blockDim.x) rhs[i] = sgn * (pairs ? pc[i] - pc[rows + i] : pc[i]);
+    __syncthreads();
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31, nw = blockDim.x >> 5;
+    for (int j = w; j < ncol; j += nw) {
+        const double* col = Qm + (size_t)j * rows;
+        double s = 0.0;
+        for (int i = l; i < rows; i += 32) s += col[i] * rhs[i];
+        s = warp_sum(s);
+        if (l == 0) { c[j] = s; cvec[j] = s; }
+    }
+    __syncthreads();
+    for (int k = ncol - 1; k >= 0; --k) {
+        const double ak = c[k] / Rm[(size_t)k * ncol + k];
+        __syncthreads();
+        for (int i = threadIdx.x; i < k; i += blockDim.x) c[i] -= Rm[(size_t)k * ncol + i] * ak;
+        if (threadIdx.x == 0) c[k] = ak;
+        __syncthreads();
+    }
+    const int drop = pairs ? 1 : 0;
+    if (threadIdx.x == 0 && drop) A_full[0] = 0.0;
+    for (int j = threadIdx.x; j < ncol; j += blockDim.x) A_full[j + drop] = c[j];
+}
+
+// residual of the fit: out[0] = || rhs - Q c ||_2 / sqrt(rows).  Single block.
+__global__ void __launch_bounds__(1024) fit_residual_kernel(const double* __restrict__ rhs, int rows, int ncol,
+                                                            const double* __restrict__ Qm,
+                                                            const double* __restrict__ cvec, double* __restrict__ out) {
+    __shared__ double sh[32];
+    double ss = 0.0;
+    for (int i = threadIdx.x; i < rows; i += blockDim.x) {
+        double r = rhs[i];
+        for (int j = 0; j < ncol; ++j) r -= Qm[(size_t)j * rows + i] * cvec[j];
+        ss += r * r;
+    }
+    ss = block_sum(ss, sh);
+    if (threadIdx.x == 0) out[0] = sqrt(ss / rows);
+}
+
+// H4: harmonic surface mapping, Eq.(10),(11) PAPER.md:99-105.  One thread per node j:
+//   S_j = sum A'_nm Y_nm(n_j)        (= Phi_out on the sphere),  A'_nm = A_nm (R_aux/R0)^n
+//   N_j = (1/R_aux) sum n A'_nm Y_nm (= sigma = d/dr Phi_out, Eq.11)
+//   Q_j = w_j N_j / 4pi,  P_j = (w_j S_j / 4pi) n_j   (exact normal dipole, reading S9)
+// Writes the packed record (R_j, Q_j | P_j, 0) read by node_sum_kernel.
+__global__ void surface_mapping_kernel(const double* __restrict__ A_full, int p, double ratio /* R_aux/R0 */,
+                                       double R_aux, const double* __restrict__ nrm /* [M,3] */,
+                                       const double* __restrict__ wq /* [M] */, int M, Node8* __restrict__ nodes) {
+    __shared__ double As[kMaxP * kMaxP];
+    for (int idx = threadIdx.x; idx < p * p; idx += blockDim.x) {
+        int n = 0;
+        while ((n + 1) * (n + 1) <= idx) ++n;
+        As[idx] = A_full[idx] * pow(ratio, (double)n);
+    }
+    __syncthreads();
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= M) return;
+    const double nx = nrm[3 * j], ny = nrm[3 * j + 1], nz = nrm[3 * j + 2];
+    double S = 0.0, Nn = 0.0;
+    solid_harmonics(nx, ny, nz, 1.0, p, [&](int n, int m, double vc, double vs) {
+        double t = As[n * n + n + m] * vc;
+        if (m > 0) t += As[n * n + n - m] * vs;
+        S += t;
+        Nn += n * t;
+    });
+    const double w = wq[j] * kInv4Pi;
+    const double D = w * S;
+    Node8 o;
+    o.x = R_aux * nx; o.y = R_aux * ny; o.z = R_aux * nz; o.q = w * Nn / R_aux;
+    o.px = D * nx; o.py = D * ny; o.pz = D * nz; o.pad = 0.0;
+    nodes[j] = o;
+}
+
+}  // namespace hsma

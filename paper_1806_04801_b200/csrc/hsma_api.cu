@@ -1,0 +1,620 @@
+// C-ABI of include/hsma.h: plan (preparation step) and evaluate (update step,
+// PAPER.md:142).  Host orchestration only; every arithmetic step of the path is a kernel in
+// sum_kernels.cuh / fit_kernels.cuh.  No CPU fallback exists.
+#include <algorithm>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "common.cuh"
+#include "fit_kernels.cuh"
+#include "geometry.h"
+#include "hsma.h"
+#include "peak.cuh"
+#include "sum_kernels.cuh"
+
+namespace hsma {
+long long g_launches = 0;
+
+#define CU(x)                                     \
+    do {                                          \
+        if ((x) != cudaSuccess) return HSMA_ERR_CUDA; \
+    } while (0)
+
+template <class T>
+struct DevBuf {  // growable device buffer owned by the plan
+    T* p = nullptr;
+    size_t cap = 0;
+    cudaError_t reserve(size_t n) {
+        if (n <= cap) return cudaSuccess;
+        if (p) cudaFree(p);
+        p = nullptr; cap = 0;
+        cudaError_t e = cudaMalloc(&p, n * sizeof(T));
+        if (e == cudaSuccess) cap = n;
+        return e;
+    }
+    void release() { if (p) cudaFree(p); p = nullptr; cap = 0; }
+};
+
+struct Split {  // decomposition of one pair-kernel launch
+    int R, ntb, nss, tiles_per_split, ncg, cells_per_group, ny;
+};
+
+static int g_num_sm = 0;
+static int num_sm() {
+    if (!g_num_sm) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        if (cudaDeviceGetAttribute(&g_num_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || g_num_sm <= 0)
+            g_num_sm = 148;
+    }
+    return g_num_sm;
+}
+
+// Grid sizing: CTAs = ntb x ny with ny splits over (source tiles x cell groups),
+// aiming at >= 16 waves of 2 CTAs/SM when there is enough work, never below 4 (tile,cell) units per CTA.
+static Split choose_split(long long T, long long n_tiles, int C) {
+    Split s;
+    const long long slots = 2LL * num_sm();
+    s.R = T >= slots * kThreads * 4 / 2 ? 4 : (T >= slots * kThreads ? 2 : 1);
+    s.ntb = (int)((T + (long long)kThreads * s.R - 1) / ((long long)kThreads * s.R));
+    const long long units = n_tiles * C;
+    long long want = (16 * slots + s.ntb - 1) / s.ntb;
+    want = std::max(1LL, std::min(want, std::max(1LL, units / 4)));
+    want = std::min(want, 32768LL);
+    long long nss = std::min(want, n_tiles);
+    s.tiles_per_split = (int)((n_tiles + nss - 1) / nss);
+    s.nss = (int)((n_tiles + s.tiles_per_split - 1) / s.tiles_per_split);
+    long long ncg = std::max(1LL, std::min((long long)C, want / s.nss));
+    s.cells_per_group = (int)((C + ncg - 1) / ncg);
+    s.ncg = (C + s.cells_per_group - 1) / s.cells_per_group;
+    s.ny = s.nss * s.ncg;
+    return s;
+}
+
+template <int REFINE>
+static void launch_near_r(const Split& s, const NearArgs& a, cudaStream_t st) {
+    dim3 grid(s.ntb, s.ny);
+    if (s.R == 4) near_sum_kernel<4, REFINE><<<grid, kThreads, 0, st>>>(a);
+    else if (s.R == 2) near_sum_kernel<2, REFINE><<<grid, kThreads, 0, st>>>(a);
+    else near_sum_kernel<1, REFINE><<<grid, kThreads, 0, st>>>(a);
+    HSMA_COUNT_LAUNCH();
+}
+
+// part must hold s.ny * T doubles
+static void launch_near(const Split& s, const double* tgt, int tstride, long long T, long long t_first, const Src4* src,
+                        long long n_tiles, const Cell* cells, int C, long long self_offset, int refine, double* part,
+                        cudaStream_t st) {
+    NearArgs a;
+    a.tgt = tgt; a.tstride = tstride; a.T = T; a.t_first = t_first; a.src = src; a.n_tiles = n_tiles;
+    a.cells = cells; a.C = C; a.n_src_split = s.nss; a.tiles_per_split = s.tiles_per_split;
+    a.cells_per_group = s.cells_per_group; a.self_offset = self_offset;
+    a.scale = refine == 1 ? 0.5 : 1.0; a.part = part;
+    if (refine == 1) launch_near_r<1>(s, a, st); else launch_near_r<2>(s, a, st);
+}
+
+struct NodeSplit { int R, ntb, ny, tiles_per_split; };
+static NodeSplit choose_node_split(long long T, long long n_tiles) {
+    NodeSplit s;
+    const long long slots = 2LL * num_sm();
+    s.R = T >= slots * kThreads * 4 / 2 ? 4 : (T >= slots * kThreads ? 2 : 1);
+    s.ntb = (int)((T + (long long)kThreads * s.R - 1) / ((long long)kThreads * s.R));
+    long long want = (4 * slots + s.ntb - 1) / s.ntb;
+    want = std::max(1LL, std::min(want, std::max(1LL, n_tiles / 2)));
+    s.tiles_per_split = (int)((n_tiles + want - 1) / want);
+    s.ny = (int)((n_tiles + s.tiles_per_split - 1) / s.tiles_per_split);
+    return s;
+}
+static void launch_node(const NodeSplit& s, const double* tgt, int tstride, long long T, long long t_first,
+                        const Node8* nodes, long long n_tiles, double* part, cudaStream_t st) {
+    NodeArgs a;
+    a.tgt = tgt; a.tstride = tstride; a.T = T; a.t_first = t_first; a.nodes = nodes; a.n_tiles = n_tiles;
+    a.tiles_per_split = s.tiles_per_split; a.part = part;
+    dim3 grid(s.ntb, s.ny);
+    if (s.R == 4) node_sum_kernel<4><<<grid, kThreads, 0, st>>>(a);
+    else if (s.R == 2) node_sum_kernel<2><<<grid, kThreads, 0, st>>>(a);
+    else node_sum_kernel<1><<<grid, kThreads, 0, st>>>(a);
+    HSMA_COUNT_LAUNCH();
+}
+
+}  // namespace hsma
+
+using namespace hsma;
+
+struct hsma_plan {
+    hsma_plan_desc d;
+    cudaStream_t stream = nullptr;
+    double R0 = 0.0, half[3] = {0, 0, 0};
+    bool pairs = false;       // periodic: rows are differences x_i / x~_i
+    bool need_neutral = false;
+    int rows = 0, ncol = 0, Kt = 0, C_near = 0, C_rhs = 0, refine = 1;
+    long long node_tiles = 0;
+    double rhs_sign = -1.0;
+    // plan-owned device data
+    Cell* cells_near = nullptr;
+    Cell* cells_rhs = nullptr;   // == cells_near for the boundary closure
+    double* chk = nullptr;       // [Kt,3]
+    double* nrm = nullptr;       // [M,3]
+    double* wq = nullptr;        // [M]
+    Node8* nodes = nullptr;      // packed, padded
+    double *Fm = nullptr, *tau = nullptr, *Qm = nullptr, *Rm = nullptr;
+    double *pc = nullptr, *rhs = nullptr, *cvec = nullptr, *A_full = nullptr, *scalars = nullptr;  // scalars[8]
+    int* flags = nullptr;        // [0] rank deficient, [1] not neutral
+    // scratch grown to the largest N seen
+    DevBuf<Src4> src;
+    DevBuf<double> part_a, part_b, part_c, red, xyz_in, q_in, phi_dev;
+    long long last_launches = 0;
+    hsma_status sticky = HSMA_OK;
+};
+
+// ------------------------------------------------------------------------------------------------
+// plan
+// ------------------------------------------------------------------------------------------------
+static void plan_free(hsma_plan* p) {
+    if (!p) return;
+    if (p->cells_rhs && p->cells_rhs != p->cells_near) cudaFree(p->cells_rhs);
+    void* ptrs[] = {p->cells_near, p->chk, p->nrm, p->wq, p->nodes, p->Fm, p->tau, p->Qm, p->Rm,
+                    p->pc, p->rhs, p->cvec, p->A_full, p->scalars, p->flags};
+    for (void* q : ptrs) if (q) cudaFree(q);
+    p->src.release(); p->part_a.release(); p->part_b.release(); p->part_c.release(); p->red.release();
+    p->xyz_in.release(); p->q_in.release(); p->phi_dev.release();
+    delete p;
+}
+
+template <class T>
+static cudaError_t upload(T** dst, const std::vector<T>& v, cudaStream_t st) {
+    cudaError_t e = cudaMalloc(dst, std::max<size_t>(1, v.size()) * sizeof(T));
+    if (e != cudaSuccess) return e;
+    return cudaMemcpyAsync(*dst, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice, st);
+}
+
+extern "C" hsma_status hsma_plan_create_ex(const hsma_plan_desc* desc, void* cuda_stream, hsma_plan** plan_out) {
+    if (!desc || !plan_out || desc->struct_size != sizeof(hsma_plan_desc)) return HSMA_ERR_INVALID_ARG;
+    const hsma_plan_desc& d = *desc;
+    if (d.kind < 0 || d.kind > 2 || d.p < 1 || d.p > kMaxP || d.M < 8 || d.K < 1) return HSMA_ERR_INVALID_ARG;
+    if (d.closure != HSMA_CLOSURE_BOUNDARY && d.closure != HSMA_CLOSURE_FAR_DATA) return HSMA_ERR_INVALID_ARG;
+    if (d.rsqrt_refine < 0 || d.rsqrt_refine > 2) return HSMA_ERR_INVALID_ARG;
+    for (int a = 0; a < 3; ++a)
+        if (!(d.L[a] > 0.0) || d.near_shell[a] < 0 || d.near_shell[a] > 8) return HSMA_ERR_INVALID_ARG;
+    if (d.kind == HSMA_BC_PERIODIC && d.closure != HSMA_CLOSURE_BOUNDARY) return HSMA_ERR_INVALID_ARG;
+    if (d.kind == HSMA_BC_SLAB_XY_PERIODIC_Z_MIRROR && d.closure != HSMA_CLOSURE_FAR_DATA)
+        return HSMA_ERR_INVALID_ARG;  // reading S16: the slab is defined only with the far-data closure
+    // reading S7: whole-cell near set is valid iff R0 < R_aux <= min_a (s_a + 1/2) L_a
+    const double R0 = 0.5 * std::sqrt(d.L[0] * d.L[0] + d.L[1] * d.L[1] + d.L[2] * d.L[2]);
+    double bound = 1e300;
+    for (int a = 0; a < 3; ++a) bound = std::min(bound, (d.near_shell[a] + 0.5) * d.L[a]);
+    if (!(d.R_aux > R0 && d.R_aux <= bound * (1 + 1e-14))) return HSMA_ERR_GEOMETRY;
+
+    hsma_plan* p = new (std::nothrow) hsma_plan;
+    if (!p) return HSMA_ERR_ALLOC;
+    p->d = d; p->d.check_xyz = nullptr;
+    p->stream = (cudaStream_t)cuda_stream;
+    p->R0 = R0;
+    for (int a = 0; a < 3; ++a) p->half[a] = 0.5 * d.L[a];
+    p->pairs = d.kind == HSMA_BC_PERIODIC;
+    p->need_neutral = d.kind != HSMA_BC_MIRROR_CAVITY;
+    p->refine = d.rsqrt_refine;  // 0 = by size, see evaluate_impl
+    p->rhs_sign = d.closure == HSMA_CLOSURE_FAR_DATA ? 1.0 : -1.0;
+    cudaStream_t st = p->stream;
+#define PCU(x) do { if ((x) != cudaSuccess) { plan_free(p); return HSMA_ERR_CUDA; } } while (0)
+
+    // cell tables
+    std::vector<Cell> near = make_cells(d.kind, d.L, d.near_shell, d.gamma, nullptr);
+    std::vector<Cell> rhsc;
+    if (d.closure == HSMA_CLOSURE_FAR_DATA) {
+        for (int a = 0; a < 3; ++a) if (d.far_shell[a] < d.near_shell[a] || d.far_shell[a] > 16) { plan_free(p); return HSMA_ERR_INVALID_ARG; }
+        rhsc = make_cells(d.kind, d.L, d.far_shell, d.gamma, d.near_shell);
+        if (rhsc.empty()) { plan_free(p); return HSMA_ERR_INVALID_ARG; }
+    }
+    if ((int)near.size() > kMaxCells || (int)rhsc.size() > kMaxCells) { plan_free(p); return HSMA_ERR_INVALID_ARG; }
+    p->C_near = (int)near.size();
+    PCU(upload(&p->cells_near, near, st));
+    if (rhsc.empty()) { p->cells_rhs = p->cells_near; p->C_rhs = p->C_near; }
+    else { p->C_rhs = (int)rhsc.size(); PCU(upload(&p->cells_rhs, rhsc, st)); }
+
+    // monitoring points
+    std::vector<double> x;
+    if (d.check_xyz) x.assign(d.check_xyz, d.check_xyz + 3 * (size_t)d.K);
+    else if (p->pairs) x = fibonacci_checkpoints(d.K, R0);
+    else {
+        bool use[3] = {true, true, true};
+        x = default_face_points(d.K, d.L, use);
+    }
+    std::vector<double> chk;
+    if (p->pairs) {  // x~ = x - L round(x/L); rows with x~ = x carry no information
+        std::vector<double> a, b;
+        for (int i = 0; i < d.K; ++i) {
+            double w[3]; bool moved = false;
+            for (int c = 0; c < 3; ++c) {
+                const double v = x[3 * (size_t)i + c];
+                w[c] = v - d.L[c] * std::nearbyint(v / d.L[c]);
+                moved = moved || std::fabs(v - w[c]) > 0.0;
+            }
+            if (!moved) continue;
+            for (int c = 0; c < 3; ++c) { a.push_back(x[3 * (size_t)i + c]); b.push_back(w[c]); }
+        }
+        p->rows = (int)(a.size() / 3);
+        chk = a; chk.insert(chk.end(), b.begin(), b.end());
+        p->Kt = 2 * p->rows;
+        p->ncol = d.p * d.p - 1;
+    } else {
+        chk = x; p->rows = d.K; p->Kt = d.K; p->ncol = d.p * d.p;
+    }
+    if (p->rows < p->ncol || p->ncol < 1) { plan_free(p); return HSMA_ERR_RANK_DEFICIENT; }
+    PCU(upload(&p->chk, chk, st));
+
+    // integration nodes
+    std::vector<double> nrm, wq;
+    if (!make_nodes(d.M, d.R_aux, d.quad_rule, nrm, wq)) { plan_free(p); return HSMA_ERR_INVALID_ARG; }
+    PCU(upload(&p->nrm, nrm, st));
+    PCU(upload(&p->wq, wq, st));
+    constexpr int kNT = kTile / 2;
+    p->node_tiles = (d.M + kNT - 1) / kNT;
+    {
+        std::vector<Node8> pad((size_t)p->node_tiles * kNT);
+        for (auto& n : pad) { n.x = n.y = n.z = kFar; n.q = n.px = n.py = n.pz = n.pad = 0.0; }
+        PCU(upload(&p->nodes, pad, st));
+    }
+
+    // fitting matrix and its QR (device)
+    const size_t mn = (size_t)p->rows * p->ncol;
+    PCU(cudaMalloc(&p->Fm, mn * sizeof(double)));
+    PCU(cudaMalloc(&p->Qm, mn * sizeof(double)));
+    PCU(cudaMalloc(&p->Rm, (size_t)p->ncol * p->ncol * sizeof(double)));
+    PCU(cudaMalloc(&p->tau, p->ncol * sizeof(double)));
+    PCU(cudaMalloc(&p->pc, p->Kt * sizeof(double)));
+    PCU(cudaMalloc(&p->rhs, p->rows * sizeof(double)));
+    PCU(cudaMalloc(&p->cvec, p->ncol * sizeof(double)));
+    PCU(cudaMalloc(&p->A_full, d.p * d.p * sizeof(double)));
+    PCU(cudaMalloc(&p->scalars, 8 * sizeof(double)));
+    PCU(cudaMalloc(&p->flags, 4 * sizeof(int)));
+    PCU(cudaMemsetAsync(p->flags, 0, 4 * sizeof(int), st));
+    PCU(cudaMemsetAsync(p->A_full, 0, d.p * d.p * sizeof(double), st));
+    build_fit_matrix_kernel<<<(p->rows + 127) / 128, 128, 0, st>>>(p->chk, p->rows, p->pairs ? 1 : 0, d.p, 1.0 / R0, p->Fm);
+    HSMA_COUNT_LAUNCH();
+    householder_qr_kernel<<<1, 1024, 0, st>>>(p->Fm, p->rows, p->ncol, p->tau, p->Qm, p->Rm, p->flags);
+    HSMA_COUNT_LAUNCH();
+    int hflags[4] = {0, 0, 0, 0};
+    PCU(cudaMemcpyAsync(hflags, p->flags, sizeof(hflags), cudaMemcpyDeviceToHost, st));
+    PCU(cudaStreamSynchronize(st));
+    PCU(cudaGetLastError());
+    if (hflags[0]) { plan_free(p); return HSMA_ERR_RANK_DEFICIENT; }
+#undef PCU
+    *plan_out = p;
+    return HSMA_OK;
+}
+
+extern "C" hsma_status hsma_plan_create(double L, int boundary_kind, int near_shell, double R_aux, int p, int M_fib,
+                                        void* cuda_stream, hsma_plan** plan_out) {
+    hsma_plan_desc d;
+    std::memset(&d, 0, sizeof(d));
+    d.struct_size = sizeof(d);
+    d.kind = boundary_kind;
+    for (int a = 0; a < 3; ++a) { d.L[a] = L; d.near_shell[a] = near_shell; }
+    d.gamma = boundary_kind == HSMA_BC_PERIODIC ? 1.0 : -1.0;
+    d.R_aux = R_aux; d.p = p; d.M = M_fib;
+    d.K = 2 * p * p;  // PAPER.md:163 N_m = 2 P^2
+    d.closure = HSMA_CLOSURE_BOUNDARY;
+    d.quad_rule = HSMA_QUAD_SPIRAL;
+    if (boundary_kind == HSMA_BC_SLAB_XY_PERIODIC_Z_MIRROR) return HSMA_ERR_INVALID_ARG;  // needs far_shell: use _ex
+    return hsma_plan_create_ex(&d, cuda_stream, plan_out);
+}
+
+extern "C" hsma_status hsma_plan_destroy(hsma_plan* plan) {
+    if (!plan) return HSMA_ERR_INVALID_ARG;
+    cudaStreamSynchronize(plan->stream);
+    plan_free(plan);
+    return HSMA_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// evaluate (update step; Table I)
+// ------------------------------------------------------------------------------------------------
+namespace hsma {
+// flags[1] = 1 if |sum q| > 1e-12 sum |q|  (reading S17); s = {sum q, sum |q|}
+__global__ void neutrality_kernel(const double* __restrict__ s, int* __restrict__ flags) {
+    if (fabs(s[0]) > 1e-12 * s[1]) flags[1] = 1;
+}
+__global__ void unpack_nodes_kernel(const Node8* __restrict__ n, int M, double* __restrict__ Q, double* __restrict__ P) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= M) return;
+    if (Q) Q[j] = n[j].q;
+    if (P) { P[3 * j] = n[j].px; P[3 * j + 1] = n[j].py; P[3 * j + 2] = n[j].pz; }
+}
+__global__ void node_positions_kernel(const double* __restrict__ nrm, double R, int M, double* __restrict__ xyz) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j < 3 * M) xyz[j] = R * nrm[j];
+}
+}  // namespace hsma
+
+static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* q, long long N, long long t0,
+                                 long long t1, double* phi_out, double* energy_out) {
+    if (!p || !xyz || !q || N < 1 || t0 < 0 || t1 > N || t0 > t1 || (!phi_out && t1 > t0)) return HSMA_ERR_INVALID_ARG;
+    cudaStream_t st = p->stream;
+    const long long before = g_launches;
+    const long long n_tiles = (N + kTile - 1) / kTile, Npad = n_tiles * kTile;
+    const hsma_plan_desc& d = p->d;
+
+    // H1 pre-pass: centre + pack, neutrality flag
+    const int pb = 256;
+    const long long pack_blocks = (Npad + pb - 1) / pb;
+    if (p->src.reserve((size_t)Npad) != cudaSuccess) return HSMA_ERR_ALLOC;
+    if (p->red.reserve((size_t)std::max(2 * pack_blocks, (t1 - t0 + 255) / 256 + 1)) != cudaSuccess) return HSMA_ERR_ALLOC;
+    pack_sources_kernel<<<(unsigned)pack_blocks, pb, 0, st>>>(xyz, q, N, Npad, p->half[0], p->half[1], p->half[2],
+                                                             p->src.p, p->need_neutral ? p->red.p : nullptr);
+    HSMA_COUNT_LAUNCH();
+    if (p->need_neutral) {
+        reduce_rows_kernel<<<1, 1024, 0, st>>>(p->red.p, pack_blocks, 2, 2, 1.0, p->scalars + 2);
+        neutrality_kernel<<<1, 1, 0, st>>>(p->scalars + 2, p->flags);
+        HSMA_COUNT_LAUNCH(); HSMA_COUNT_LAUNCH();
+    }
+
+    // H2 (a): Phi_in (or the far-cell data) at the monitoring points -> pc [Kt]
+    {
+        const Split s = choose_split(p->Kt, n_tiles, p->C_rhs);
+        if (p->part_a.reserve((size_t)s.ny * p->Kt) != cudaSuccess) return HSMA_ERR_ALLOC;
+        launch_near(s, p->chk, 3, p->Kt, 0, p->src.p, n_tiles, p->cells_rhs, p->C_rhs, -1, 2, p->part_a.p, st);  // (a) always cubic: it feeds the fit
+        finish_phi_kernel<<<(p->Kt + 255) / 256, 256, 0, st>>>(p->part_a.p, s.ny, nullptr, 0, p->Kt, nullptr, 0, p->pc, nullptr);
+        HSMA_COUNT_LAUNCH();
+    }
+    // H3: least squares, Eq.(7)
+    ls_solve_kernel<<<1, 1024, p->ncol * sizeof(double), st>>>(p->pc, p->rows, p->ncol, p->pairs ? 1 : 0, p->rhs_sign,
+                                                               p->Qm, p->Rm, p->rhs, p->cvec, p->A_full);
+    HSMA_COUNT_LAUNCH();
+    // H4: harmonic surface mapping, Eq.(10),(11) PAPER.md:99-105
+    surface_mapping_kernel<<<(d.M + 127) / 128, 128, 0, st>>>(p->A_full, d.p, d.R_aux / p->R0, d.R_aux, p->nrm, p->wq,
+                                                              d.M, p->nodes);
+    HSMA_COUNT_LAUNCH();
+
+    const long long T = t1 - t0;
+    if (T > 0) {
+        // H5 (b): near images at the sources, self excluded
+        const Split sb = choose_split(T, n_tiles, p->C_near);
+        if (p->part_b.reserve((size_t)sb.ny * T) != cudaSuccess) return HSMA_ERR_ALLOC;
+        // rsqrt_refine = 0: the cubic step while (b) is latency-bound anyway (< 2^32 pairs), Newton above
+        const int refine = p->refine ? p->refine : ((double)N * (double)N * p->C_near < 4294967296.0 ? 2 : 1);
+        launch_near(sb, reinterpret_cast<const double*>(p->src.p), 4, T, t0, p->src.p, n_tiles, p->cells_near, p->C_near,
+                    t0, refine, p->part_b.p, st);
+        // H6 (c): sphere nodes, charge + dipole
+        const NodeSplit sc = choose_node_split(T, p->node_tiles);
+        if (p->part_c.reserve((size_t)sc.ny * T) != cudaSuccess) return HSMA_ERR_ALLOC;
+        launch_node(sc, reinterpret_cast<const double*>(p->src.p), 4, T, t0, p->nodes, p->node_tiles, p->part_c.p, st);
+        // H7: phi and U
+        const long long fb = (T + 255) / 256;
+        finish_phi_kernel<<<(unsigned)fb, 256, 0, st>>>(p->part_b.p, sb.ny, p->part_c.p, sc.ny, T, p->src.p, t0, phi_out,
+                                                        energy_out ? p->red.p : nullptr);
+        HSMA_COUNT_LAUNCH();
+        if (energy_out) {
+            reduce_rows_kernel<<<1, 1024, 0, st>>>(p->red.p, fb, 1, 1, 0.5, energy_out);
+            HSMA_COUNT_LAUNCH();
+        }
+    } else if (energy_out) {
+        if (cudaMemsetAsync(energy_out, 0, sizeof(double), st) != cudaSuccess) return HSMA_ERR_CUDA;
+    }
+    p->last_launches = g_launches - before;
+    if (cudaPeekAtLastError() != cudaSuccess) { cudaGetLastError(); p->sticky = HSMA_ERR_CUDA; return HSMA_ERR_CUDA; }
+    return HSMA_OK;
+}
+
+extern "C" hsma_status hsma_evaluate(hsma_plan* plan, const double* xyz, const double* q, long long N, double* phi_out,
+                                     double* energy_out) {
+    return evaluate_impl(plan, xyz, q, N, 0, N, phi_out, energy_out);
+}
+
+extern "C" hsma_status hsma_evaluate_shard(hsma_plan* plan, const double* xyz, const double* q, long long N,
+                                           long long t0, long long t1, double* phi_out, double* energy_out) {
+    return evaluate_impl(plan, xyz, q, N, t0, t1, phi_out, energy_out);
+}
+
+extern "C" hsma_status hsma_plan_sync(hsma_plan* plan) {
+    if (!plan) return HSMA_ERR_INVALID_ARG;
+    int hf[4] = {0, 0, 0, 0};
+    cudaError_t e = cudaMemcpyAsync(hf, plan->flags, sizeof(hf), cudaMemcpyDeviceToHost, plan->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(plan->stream);
+    hsma_status s = plan->sticky;
+    plan->sticky = HSMA_OK;
+    if (e != cudaSuccess) { cudaGetLastError(); return HSMA_ERR_CUDA; }
+    if (hf[1]) {
+        cudaMemsetAsync(plan->flags + 1, 0, sizeof(int), plan->stream);
+        if (s == HSMA_OK) s = HSMA_ERR_NOT_NEUTRAL;
+    }
+    return s;
+}
+
+extern "C" hsma_status hsma_evaluate_host(hsma_plan* p, const double* xyz_host, const double* q_host, long long N,
+                                          double* phi_host, double* energy_host) {
+    if (!p || !xyz_host || !q_host || N < 1) return HSMA_ERR_INVALID_ARG;
+    if (p->xyz_in.reserve(3 * (size_t)N) != cudaSuccess || p->q_in.reserve((size_t)N) != cudaSuccess ||
+        p->phi_dev.reserve((size_t)N) != cudaSuccess)
+        return HSMA_ERR_ALLOC;
+    cudaStream_t st = p->stream;
+    CU(cudaMemcpyAsync(p->xyz_in.p, xyz_host, 3 * (size_t)N * sizeof(double), cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(p->q_in.p, q_host, (size_t)N * sizeof(double), cudaMemcpyHostToDevice, st));
+    hsma_status s = evaluate_impl(p, p->xyz_in.p, p->q_in.p, N, 0, N, p->phi_dev.p, p->scalars);
+    if (s != HSMA_OK) return s;
+    if (phi_host) CU(cudaMemcpyAsync(phi_host, p->phi_dev.p, (size_t)N * sizeof(double), cudaMemcpyDeviceToHost, st));
+    if (energy_host) CU(cudaMemcpyAsync(energy_host, p->scalars, sizeof(double), cudaMemcpyDeviceToHost, st));
+    return hsma_plan_sync(p);
+}
+
+// ------------------------------------------------------------------------------------------------
+// introspection, raw kernels, microbenchmark
+// ------------------------------------------------------------------------------------------------
+extern "C" const char* hsma_status_string(int s) {
+    switch (s) {
+        case HSMA_OK: return "HSMA_OK";
+        case HSMA_ERR_INVALID_ARG: return "HSMA_ERR_INVALID_ARG";
+        case HSMA_ERR_GEOMETRY: return "HSMA_ERR_GEOMETRY: R_aux must lie in (R0, min_a (shell_a + 1/2) L_a]";
+        case HSMA_ERR_NOT_NEUTRAL: return "HSMA_ERR_NOT_NEUTRAL: periodic axes need sum q = 0";
+        case HSMA_ERR_CUDA: return "HSMA_ERR_CUDA";
+        case HSMA_ERR_ALLOC: return "HSMA_ERR_ALLOC";
+        case HSMA_ERR_RANK_DEFICIENT: return "HSMA_ERR_RANK_DEFICIENT";
+        default: return "HSMA_ERR_UNKNOWN";
+    }
+}
+
+extern "C" hsma_status hsma_plan_info(hsma_plan* p, long long* w) {
+    if (!p || !w) return HSMA_ERR_INVALID_ARG;
+    w[0] = p->rows; w[1] = p->ncol; w[2] = p->Kt; w[3] = p->C_near; w[4] = p->C_rhs; w[5] = p->d.M; w[6] = p->d.p;
+    w[7] = p->last_launches;
+    return HSMA_OK;
+}
+
+static hsma_status d2d(hsma_plan* p, void* dst, const void* src, size_t bytes) {
+    if (!p || !dst) return HSMA_ERR_INVALID_ARG;
+    CU(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToDevice, p->stream));
+    return HSMA_OK;
+}
+extern "C" hsma_status hsma_get_coeffs(hsma_plan* p, double* A_out) {
+    return p ? d2d(p, A_out, p->A_full, (size_t)p->d.p * p->d.p * sizeof(double)) : HSMA_ERR_INVALID_ARG;
+}
+extern "C" hsma_status hsma_get_rhs(hsma_plan* p, double* rhs_out) {
+    return p ? d2d(p, rhs_out, p->rhs, (size_t)p->rows * sizeof(double)) : HSMA_ERR_INVALID_ARG;
+}
+extern "C" hsma_status hsma_get_check_targets(hsma_plan* p, double* xyz_out) {
+    return p ? d2d(p, xyz_out, p->chk, 3 * (size_t)p->Kt * sizeof(double)) : HSMA_ERR_INVALID_ARG;
+}
+extern "C" hsma_status hsma_get_nodes(hsma_plan* p, double* xyz_out, double* w_out) {
+    if (!p) return HSMA_ERR_INVALID_ARG;
+    if (xyz_out) {
+        node_positions_kernel<<<(3 * p->d.M + 255) / 256, 256, 0, p->stream>>>(p->nrm, p->d.R_aux, p->d.M, xyz_out);
+        HSMA_COUNT_LAUNCH();
+    }
+    if (w_out) return d2d(p, w_out, p->wq, (size_t)p->d.M * sizeof(double));
+    return HSMA_OK;
+}
+extern "C" hsma_status hsma_get_surface(hsma_plan* p, double* Q_out, double* P_out) {
+    if (!p) return HSMA_ERR_INVALID_ARG;
+    unpack_nodes_kernel<<<(p->d.M + 255) / 256, 256, 0, p->stream>>>(p->nodes, p->d.M, Q_out, P_out);
+    HSMA_COUNT_LAUNCH();
+    return HSMA_OK;
+}
+extern "C" hsma_status hsma_get_fit_residual(hsma_plan* p, double* rms_out) {
+    if (!p || !rms_out) return HSMA_ERR_INVALID_ARG;
+    fit_residual_kernel<<<1, 1024, 0, p->stream>>>(p->rhs, p->rows, p->ncol, p->Qm, p->cvec, p->scalars + 4);
+    HSMA_COUNT_LAUNCH();
+    CU(cudaMemcpyAsync(rms_out, p->scalars + 4, sizeof(double), cudaMemcpyDeviceToHost, p->stream));
+    CU(cudaStreamSynchronize(p->stream));
+    return HSMA_OK;
+}
+
+namespace hsma {
+__global__ void pack_plain_kernel(const double* __restrict__ xyz, const double* __restrict__ q, long long N,
+                                  long long Npad, Src4* __restrict__ out) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= Npad) return;
+    Src4 s;
+    if (i < N) { s.x = xyz[3 * i]; s.y = xyz[3 * i + 1]; s.z = xyz[3 * i + 2]; s.q = q[i]; }
+    else { s.x = s.y = s.z = kFar; s.q = 0.0; }
+    out[i] = s;
+}
+__global__ void pack_nodes_kernel(const double* __restrict__ R, const double* __restrict__ Q, const double* __restrict__ P,
+                                  long long M, long long Mpad, Node8* __restrict__ out) {
+    const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= Mpad) return;
+    Node8 n;
+    if (j < M) { n.x = R[3 * j]; n.y = R[3 * j + 1]; n.z = R[3 * j + 2]; n.q = Q[j]; n.px = P[3 * j]; n.py = P[3 * j + 1]; n.pz = P[3 * j + 2]; }
+    else { n.x = n.y = n.z = kFar; n.q = n.px = n.py = n.pz = 0.0; }
+    n.pad = 0.0;
+    out[j] = n;
+}
+}  // namespace hsma
+
+extern "C" hsma_status hsma_direct_sum(const double* tgt, long long T, const double* src, const double* q, long long N,
+                                       const double* shift_host, const double* sign_host, const double* w_host, int C,
+                                       int central_cell, long long self_offset, int refine, double* phi_out,
+                                       void* cuda_stream) {
+    if (!tgt || !src || !q || !shift_host || !sign_host || !w_host || !phi_out) return HSMA_ERR_INVALID_ARG;
+    if (T < 1 || N < 1 || C < 1 || C > kMaxCells || (refine != 1 && refine != 2)) return HSMA_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    std::vector<Cell> cells(C);
+    for (int c = 0; c < C; ++c) {
+        cells[c].sx = shift_host[3 * c]; cells[c].sy = shift_host[3 * c + 1]; cells[c].sz = shift_host[3 * c + 2];
+        cells[c].w = w_host[c];
+        cells[c].fx = sign_host[3 * c] < 0; cells[c].fy = sign_host[3 * c + 1] < 0; cells[c].fz = sign_host[3 * c + 2] < 0;
+        cells[c].central = (c == central_cell);
+    }
+    const long long n_tiles = (N + kTile - 1) / kTile, Npad = n_tiles * kTile;
+    const Split s = choose_split(T, n_tiles, C);
+    Cell* dc = nullptr; Src4* ds = nullptr; double* part = nullptr;
+    hsma_status rc = HSMA_OK;
+    if (cudaMalloc(&dc, C * sizeof(Cell)) != cudaSuccess || cudaMalloc(&ds, Npad * sizeof(Src4)) != cudaSuccess ||
+        cudaMalloc(&part, (size_t)s.ny * T * sizeof(double)) != cudaSuccess) {
+        rc = HSMA_ERR_ALLOC;
+    } else {
+        cudaMemcpyAsync(dc, cells.data(), C * sizeof(Cell), cudaMemcpyHostToDevice, st);
+        pack_plain_kernel<<<(unsigned)((Npad + 255) / 256), 256, 0, st>>>(src, q, N, Npad, ds);
+        HSMA_COUNT_LAUNCH();
+        launch_near(s, tgt, 3, T, 0, ds, n_tiles, dc, C, central_cell >= 0 ? self_offset : -1, refine, part, st);
+        finish_phi_kernel<<<(unsigned)((T + 255) / 256), 256, 0, st>>>(part, s.ny, nullptr, 0, T, nullptr, 0, phi_out, nullptr);
+        HSMA_COUNT_LAUNCH();
+        if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) rc = HSMA_ERR_CUDA;
+    }
+    if (dc) cudaFree(dc);
+    if (ds) cudaFree(ds);
+    if (part) cudaFree(part);
+    return rc;
+}
+
+extern "C" hsma_status hsma_node_sum(const double* tgt, long long T, const double* R, const double* Q, const double* P,
+                                     long long M, double* phi_out, void* cuda_stream) {
+    if (!tgt || !R || !Q || !P || !phi_out || T < 1 || M < 1) return HSMA_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    constexpr int kNT = kTile / 2;
+    const long long n_tiles = (M + kNT - 1) / kNT, Mpad = n_tiles * kNT;
+    const NodeSplit s = choose_node_split(T, n_tiles);
+    Node8* dn = nullptr; double* part = nullptr;
+    hsma_status rc = HSMA_OK;
+    if (cudaMalloc(&dn, Mpad * sizeof(Node8)) != cudaSuccess || cudaMalloc(&part, (size_t)s.ny * T * sizeof(double)) != cudaSuccess) {
+        rc = HSMA_ERR_ALLOC;
+    } else {
+        pack_nodes_kernel<<<(unsigned)((Mpad + 255) / 256), 256, 0, st>>>(R, Q, P, M, Mpad, dn);
+        HSMA_COUNT_LAUNCH();
+        launch_node(s, tgt, 3, T, 0, dn, n_tiles, part, st);
+        finish_phi_kernel<<<(unsigned)((T + 255) / 256), 256, 0, st>>>(nullptr, 0, part, s.ny, T, nullptr, 0, phi_out, nullptr);
+        HSMA_COUNT_LAUNCH();
+        if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) rc = HSMA_ERR_CUDA;
+    }
+    if (dn) cudaFree(dn);
+    if (part) cudaFree(part);
+    return rc;
+}
+
+extern "C" hsma_status hsma_fp64_peak(double seconds, double* tflops_out, double* sm_clock_mhz_out) {
+    if (!tflops_out || !(seconds > 0.0) || seconds > 30.0) return HSMA_ERR_INVALID_ARG;
+    int dev = 0, khz = 0;
+    CU(cudaGetDevice(&dev));
+    cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, dev);
+    double* out = nullptr;
+    CU(cudaMalloc(&out, sizeof(double)));
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const int blocks = num_sm() * 8;
+    int iters = 2000;
+    float ms = 0.f;
+    hsma_status rc = HSMA_OK;
+    for (int pass = 0; pass < 3 && rc == HSMA_OK; ++pass) {  // calibrate, then one long timed launch
+        cudaEventRecord(e0);
+        dfma_peak_kernel<<<blocks, 256>>>(out, iters, 0.999999, 1e-9);
+        HSMA_COUNT_LAUNCH();
+        cudaEventRecord(e1);
+        if (cudaEventSynchronize(e1) != cudaSuccess) { rc = HSMA_ERR_CUDA; break; }
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (pass < 2) {
+            const double scale = seconds * 1e3 / std::max(1e-3, (double)ms) * (pass == 0 ? 0.1 : 1.0);
+            iters = (int)std::max(100.0, std::min(2.0e8, iters * scale * (pass == 0 ? 1.0 : 1.0)));
+            if (pass == 1) iters = (int)std::max(100.0, std::min(2.0e8, (double)iters));
+        }
+    }
+    if (rc == HSMA_OK) {
+        const double fma = (double)blocks * 256.0 * (double)iters * (double)kPeakFmaPerThreadIter;
+        *tflops_out = 2.0 * fma / (ms * 1e-3) * 1e-12;
+        if (sm_clock_mhz_out) *sm_clock_mhz_out = khz * 1e-3;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(out);
+    return rc;
+}
+
+extern "C" long long hsma_launch_count(void) { return g_launches; }

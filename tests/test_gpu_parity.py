@@ -1,0 +1,268 @@
+"""Parity of the CUDA path (through the C-ABI, via the ctypes binding) against the CPU oracle, element
+by element on the same seeded inputs.  Bars (BASELINE.json north_star): max|dphi|/max|phi| <= 1e-10,
+|dU|/|U| <= 1e-11.  All `-m gpu`."""
+import math
+import os
+
+import numpy as np
+import pytest
+
+import hsma_workloads as W
+from oracle import hsma_oracle as O
+
+pytestmark = pytest.mark.gpu
+
+PHI_TOL = 1e-10
+U_TOL = 1e-11
+
+
+@pytest.fixture(scope="module")
+def H():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    import paper_1806_04801_b200 as H
+    H.binding.load_library()   # fails loudly if the extension is missing
+    return H
+
+
+def dev(a):
+    import torch
+    return torch.as_tensor(np.ascontiguousarray(a, dtype=np.float64), device="cuda")
+
+
+def rel_inf(a, b):
+    return float(np.max(np.abs(a - b)) / np.max(np.abs(b)))
+
+
+def report(line):
+    """Achieved errors, appended to gpurun_out/parity_errors.log when that folder exists (GPU box)."""
+    d = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out")
+    if os.path.isdir(d):
+        with open(os.path.join(d, "parity_errors.log"), "a") as f:
+            f.write(line + "\n")
+
+
+# ------------------------------------------------------------------ raw kernels (a)/(b)
+@pytest.mark.parametrize("kind,L,shell,gamma", [
+    (W.BC_PERIODIC, (1.0, 1.0, 1.0), (1, 1, 1), 1.0),
+    (W.BC_MIRROR_CAVITY, (1.0, 1.5, 0.7), (1, 1, 1), -1.0),
+    (W.BC_SLAB_XY_PERIODIC_Z_MIRROR, (1.0, 1.0, 0.5), (1, 1, 2), 0.5),
+])
+@pytest.mark.parametrize("refine", [1, 2])
+@pytest.mark.parametrize("N,T", [(1, 1), (7, 300), (255, 257), (256, 256), (1000, 1029), (2311, 77)])
+def test_direct_sum_matches_oracle(H, kind, L, shell, gamma, refine, N, T):
+    import torch
+    rng = np.random.default_rng(100 + N + T)
+    Lh = np.asarray(L)
+    src = (rng.random((N, 3)) - 0.5) * Lh
+    q = rng.standard_normal(N)
+    tgt = (rng.random((T, 3)) - 0.5) * Lh * 1.2
+    cells = O.cell_table(kind, L, shell, gamma)
+    ref = O.near_sum(tgt, src, q, cells)
+    out = torch.empty(T, dtype=torch.float64, device="cuda")
+    H.hsma_direct_sum(dev(tgt), dev(src), dev(q), cells.shift, cells.sign, cells.w, cells.central, -1, refine, out)
+    assert rel_inf(out.cpu().numpy(), ref) < 1e-12
+
+
+@pytest.mark.parametrize("refine", [1, 2])
+@pytest.mark.parametrize("N,t0,T", [(300, 0, 300), (1500, 0, 1500), (1500, 700, 555), (5000, 4990, 10)])
+def test_direct_sum_self_exclusion(H, refine, N, t0, T):
+    """Targets are sources t0..t0+T-1; only the bare self term of the central cell is skipped
+    (PAPER.md:142): self images in the other cells are kept."""
+    import torch
+    rng = np.random.default_rng(7 + N)
+    src = rng.random((N, 3)) - 0.5
+    q = W.alternating_charges(N)
+    cells = O.cell_table(W.BC_PERIODIC, (1.0, 1.0, 1.0), (1, 1, 1), 1.0)
+    ref = O.near_sum(src[t0:t0 + T], src, q, cells, self_offset=t0)
+    out = torch.empty(T, dtype=torch.float64, device="cuda")
+    H.hsma_direct_sum(dev(src[t0:t0 + T]), dev(src), dev(q), cells.shift, cells.sign, cells.w, cells.central, t0,
+                      refine, out)
+    assert np.all(np.isfinite(out.cpu().numpy()))
+    assert rel_inf(out.cpu().numpy(), ref) < 1e-12
+
+
+def test_rsqrt_refinement_error(H):
+    """One source, one cell: phi = q / r.  Measures the relative error of the two refinements of the
+    MUFU.RSQ64H seed over distances spanning 12 decades."""
+    import torch
+    rng = np.random.default_rng(5)
+    T = 200000
+    r = 10.0 ** rng.uniform(-6, 6, T)
+    u = rng.standard_normal((T, 3))
+    u /= np.linalg.norm(u, axis=1)[:, None]
+    tgt = u * r[:, None]
+    exact = 1.0 / np.sqrt((tgt * tgt).sum(1))
+    z3 = np.zeros((1, 3))
+    for refine, bound, mean_bound in ((1, 1.3e-12, 2e-14), (2, 6e-16, 1e-16)):
+        out = torch.empty(T, dtype=torch.float64, device="cuda")
+        H.hsma_direct_sum(dev(tgt), dev(z3), dev(np.ones(1)), z3, np.ones((1, 3)), np.ones(1), 0, -1, refine, out)
+        err = out.cpu().numpy() / exact - 1.0
+        report(f"rsqrt refine={refine}: max|err|={np.abs(err).max():.3e} mean={err.mean():.3e} rms={np.sqrt((err**2).mean()):.3e}")
+        assert np.abs(err).max() < bound, (refine, np.abs(err).max())
+        assert abs(err.mean()) < mean_bound, (refine, err.mean())
+
+
+# ------------------------------------------------------------------ raw kernel (c)
+@pytest.mark.parametrize("T,M", [(1, 8), (300, 127), (1029, 128), (513, 2000)])
+def test_node_sum_matches_oracle(H, T, M):
+    import torch
+    rng = np.random.default_rng(T + M)
+    nodes, nrm, w = O.nodes_spiral(M, 1.3)
+    Q, D = rng.standard_normal(M), rng.standard_normal(M)
+    tgt = rng.random((T, 3)) - 0.5
+    ref = O.node_sum(tgt, nodes, nrm, Q, D)
+    out = torch.empty(T, dtype=torch.float64, device="cuda")
+    H.hsma_node_sum(dev(tgt), dev(nodes), dev(Q), dev(D[:, None] * nrm), out)
+    assert rel_inf(out.cpu().numpy(), ref) < 1e-13
+
+
+# ------------------------------------------------------------------ full path, BASELINE.json configs
+def run_both(H, w, sl=None, **plan_kw):
+    import torch
+    r = O.hsma(w, targets_slice=sl)
+    with H.Plan.from_workload(w, **plan_kw) as plan:
+        xyz, q = dev(w.xyz), dev(w.q)
+        if sl is None:
+            phi, U = plan.evaluate(xyz, q, sync=True)
+        else:
+            i0, i1, _ = sl.indices(w.N)
+            phi, U = plan.evaluate_shard(xyz, q, i0, i1, sync=True)
+        torch.cuda.synchronize()
+        extra = dict(A=plan.coeffs().cpu().numpy(), rhs=plan.rhs().cpu().numpy(),
+                     chk=plan.check_targets().cpu().numpy(), nodes=plan.nodes()[0].cpu().numpy(),
+                     Q=plan.surface()[0].cpu().numpy(), P=plan.surface()[1].cpu().numpy(),
+                     rms=plan.fit_residual(), info=plan.info, launches=plan.launches_last_evaluate())
+    return r, phi.cpu().numpy(), float(U.cpu().numpy()[0]), extra
+
+
+def check_parity(r, phi, U, extra, tag=""):
+    report(f"{tag}: phi {rel_inf(phi, r.phi):.3e} U {abs(U - r.U) / abs(r.U):.3e} rhs {rel_inf(extra['rhs'], r.rhs):.3e} "
+           f"A {rel_inf(extra['A'], r.A):.3e} Q {rel_inf(extra['Q'], r.Q):.3e} cond {r.cond:.3g} fit_rms {r.fit_rms:.3e}")
+    assert np.allclose(extra["chk"], r.check_targets, rtol=0, atol=1e-14)
+    assert np.allclose(extra["nodes"], r.nodes, rtol=0, atol=1e-14)
+    assert rel_inf(extra["rhs"], r.rhs) < 1e-11
+    assert rel_inf(extra["A"], r.A) < 1e-9          # cond * eps * modest factor; phi is what is judged
+    assert rel_inf(extra["Q"], r.Q) < 1e-9
+    assert rel_inf(extra["P"], r.D[:, None] * r.normals) < 1e-9
+    assert abs(extra["rms"] - r.fit_rms) <= 1e-6 * r.fit_rms + 1e-13
+    assert rel_inf(phi, r.phi) <= PHI_TOL
+    assert abs(U - r.U) <= U_TOL * abs(r.U)
+    assert extra["launches"] >= 7
+
+
+@pytest.mark.parametrize("refine", [0, 1, 2])
+@pytest.mark.parametrize("idx", [1, 2, 3, 4])
+def test_config_full(H, idx, refine):
+    """BASELINE.json configs 1-4 at full size, every potential compared; library default (0) and both
+    explicit refinements of the near-sum kernel."""
+    w = W.config(idx)
+    r, phi, U, extra = run_both(H, w, rsqrt_refine=refine)
+    check_parity(r, phi, U, extra, f"cfg{idx} refine={refine}")
+    if idx == 1:
+        M = O.madelung_constant(U, w.N, w.meta["a_nn"])
+        assert abs(M - 1.7475645946) < 5e-8
+
+
+def test_paper_example2(H):
+    r, phi, U, extra = run_both(H, W.paper_example2())
+    check_parity(r, phi, U, extra, "paper_example2")
+
+
+def test_config5_reduced(H):
+    """Config 5 recipe at N = 20,011 (odd tile tail; neutral needs even N -> 20,012)."""
+    w = W.config(5, N=20012)
+    r, phi, U, extra = run_both(H, w)
+    check_parity(r, phi, U, extra, "cfg5_N20012")
+
+
+def test_config5_full_size_sampled(H):
+    """Config 5 at N = 262,144 in the launch configuration bench.py times: a contiguous slice of 96
+    targets straddling a tile boundary is compared with the oracle potential by potential; the oracle
+    needs the full (a) step (2.8e10 pairs) for the fit."""
+    import torch
+    w = W.config(5)
+    sl = slice(131072 - 40, 131072 + 56)
+    r = O.hsma(w, targets_slice=sl)
+    with H.Plan.from_workload(w) as plan:
+        phi, U = plan.evaluate(dev(w.xyz), dev(w.q), sync=True)
+        phi = phi.cpu().numpy()
+        A = plan.coeffs().cpu().numpy()
+    assert rel_inf(A, r.A) < 1e-9
+    scale = np.max(np.abs(phi))
+    report(f"cfg5 full sampled: phi {np.max(np.abs(phi[sl] - r.phi)) / scale:.3e} A {rel_inf(A, r.A):.3e} max|phi| {scale:.4g}")
+    assert np.max(np.abs(phi[sl] - r.phi)) <= PHI_TOL * scale
+    # properties that hold at any size: finite, U = 1/2 sum q phi in extended precision
+    assert np.all(np.isfinite(phi))
+    Uref = 0.5 * float(np.sum(np.asarray(w.q, dtype=np.longdouble) * phi.astype(np.longdouble)))
+    assert abs(float(U.cpu().numpy()[0]) - Uref) <= U_TOL * abs(Uref)
+
+
+# ------------------------------------------------------------------ API behaviour
+def test_shards_and_host_path_agree(H):
+    import torch
+    w = W.config(2)
+    with H.Plan.from_workload(w) as plan:
+        xyz, q = dev(w.xyz), dev(w.q)
+        phi, U = plan.evaluate(xyz, q, sync=True)
+        cuts = [0, 1, 257, 700, 1000]
+        parts, Us = [], 0.0
+        for a, b in zip(cuts[:-1], cuts[1:]):
+            ph, u = plan.evaluate_shard(xyz, q, a, b, sync=True)
+            parts.append(ph.cpu().numpy())
+            Us += float(u.cpu().numpy()[0])
+        assert np.array_equal(np.concatenate(parts), phi.cpu().numpy())
+        assert abs(Us - float(U.cpu().numpy()[0])) < 1e-12 * abs(Us)
+        ph_h, U_h = plan.evaluate_host(np.ascontiguousarray(w.xyz), np.ascontiguousarray(w.q))
+        assert np.array_equal(ph_h, phi.cpu().numpy())
+        assert U_h == float(U.cpu().numpy()[0])
+        ph_e, u_e = plan.evaluate_shard(xyz, q, 5, 5, sync=True)   # empty shard
+        assert ph_e.numel() == 0 and float(u_e.cpu().numpy()[0]) == 0.0
+
+
+def test_deterministic(H):
+    w = W.config(3)
+    with H.Plan.from_workload(w) as plan:
+        a, ua = plan.evaluate(dev(w.xyz), dev(w.q), sync=True)
+        b, ub = plan.evaluate(dev(w.xyz), dev(w.q), sync=True)
+        assert np.array_equal(a.cpu().numpy(), b.cpu().numpy()) and float(ua) == float(ub)
+
+
+def test_error_statuses(H):
+    s3 = math.sqrt(3.0)
+    with pytest.raises(H.HsmaError) as e:       # config 1 as literally written: 3^3 cells with R = sqrt3 L (reading S7)
+        H.hsma_plan_create(2.0, H.HSMA_BC_PERIODIC, 1, s3 * 2.0, 8, 400)
+    assert e.value.status == H.HSMA_ERR_GEOMETRY
+    with pytest.raises(H.HsmaError) as e:
+        H.hsma_plan_create(1.0, H.HSMA_BC_PERIODIC, 1, 0.5, 8, 400)          # R_aux inside the circumsphere
+    assert e.value.status == H.HSMA_ERR_GEOMETRY
+    with pytest.raises(H.HsmaError) as e:
+        H.hsma_plan_create(1.0, H.HSMA_BC_PERIODIC, 1, 1.2, 0, 400)
+    assert e.value.status == H.HSMA_ERR_INVALID_ARG
+    with pytest.raises(H.HsmaError) as e:       # fewer rows than unknowns
+        H.Plan(kind=0, L=(1, 1, 1), near_shell=(1, 1, 1), R_aux=1.2, p=10, M=500, K=50)
+    assert e.value.status == H.HSMA_ERR_RANK_DEFICIENT
+    w = W.config(2, N=101)                      # odd N: not neutral
+    with H.Plan.from_workload(w) as plan:
+        with pytest.raises(H.HsmaError) as e:
+            plan.evaluate(dev(w.xyz), dev(w.q), sync=True)
+        assert e.value.status == H.HSMA_ERR_NOT_NEUTRAL
+        w2 = W.config(2, N=100)
+        plan.evaluate(dev(w2.xyz), dev(w2.q), sync=True)   # the sticky status was cleared
+
+
+def test_north_star_create_form(H):
+    """hsma_plan_create(L, kind, shell, R_aux, p, M, stream): K = 2 p^2 Fibonacci check points."""
+    import torch
+    w = W.config(2).with_(K=200)
+    h = H.hsma_plan_create(1.0, H.HSMA_BC_PERIODIC, 1, w.R_aux, w.p, w.M)
+    try:
+        phi = torch.empty(w.N, dtype=torch.float64, device="cuda")
+        U = torch.empty(1, dtype=torch.float64, device="cuda")
+        H.hsma_evaluate(h, dev(w.xyz), dev(w.q), phi, U)
+        H.hsma_plan_sync(h)
+        r = O.hsma(w)
+        assert rel_inf(phi.cpu().numpy(), r.phi) <= PHI_TOL
+        assert abs(float(U) - r.U) <= U_TOL * abs(r.U)
+    finally:
+        H.hsma_plan_destroy(h)
