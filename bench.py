@@ -1,0 +1,374 @@
+#!/usr/bin/env python
+"""bench.py -- BASELINE.json's metric on BASELINE.json's configs: fp64 pair interactions per second and
+ms per full HSMA evaluation, with the FP64 roofline of the dominant kernel and the CPU oracle timed
+beside it.  One JSON line on stdout (rank 0).  DESIGN.md "Measurement" explains every field.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 5] [--impl b200|reference]
+  N > 1: python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 \
+         --master-port P bench.py --gpus N --steps K --warmup W
+
+A "step" is one pass of the whole hot path (H1..H7: pre-pass, (a) check-point sums, fit, mapping,
+(b) near sums at the sources, (c) node sums, energy) over one synthetic configuration.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import hsma_workloads as W  # noqa: E402
+
+METRIC = "fp64 pair interactions/sec"
+UNIT = "pairs/s"
+
+# Algorithmic work per pair, SURVEY.md 8(d) / DESIGN.md "Roofline": flops with add/mul = 1, fma = 2
+FLOPS_PAIR_CHARGE = 18.0      # 3 DADD + (DMUL + 2 DFMA) + cubic rsqrt refinement (2 DMUL + 3 DFMA) + DFMA
+FLOPS_PAIR_DIPOLE = 26.0      # + P.d (DMUL + 2 DFMA) + y^2 (DMUL) + DFMA
+# what near_sum_kernel<R, REFINE> executes per pair (FP64-pipe instructions, flops), DESIGN.md "rsqrt"
+EXEC_PAIR = {1: (10.0, 14.0), 2: (12.0, 18.0)}
+# FP64 peak derived from unit counts and clocks: SMs x 64 DFMA lanes x 2 x clock
+FP64_LANES_PER_SM = 64
+
+
+def pair_counts(info: dict, N: int, T: int) -> dict:
+    """Pairs per step for a rank that owns T of the N targets (step (a) is computed in full)."""
+    return {"a": info["check_targets"] * N * info["rhs_cells"], "b": T * N * info["near_cells"], "c": T * info["M"]}
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.gpu = gpu_index
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+
+    def start(self):
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu), f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "200"], stdout=self.f,
+                                      stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self) -> dict:
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for line in self.f.read().splitlines():
+            t = [x.strip() for x in line.split(",")]
+            if len(t) < 9:
+                continue
+            try:
+                sm.append(float(t[1])); mx.append(float(t[2])); pw.append(float(t[3]))
+            except ValueError:
+                continue
+            for name, v in zip(names, t[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        try:
+            os.unlink(self.f.name)
+        except OSError:
+            pass
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": statistics.median(sm), "sm_min_mhz": min(sm), "sm_max_mhz": max(mx),
+                "power_w_max": max(pw), "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ---------------------------------------------------------------------------------------------------
+# CPU oracle arm (cpu_baseline leg and --impl reference): the only place bench.py executes oracle/
+# ---------------------------------------------------------------------------------------------------
+class OracleSample:
+    """A bounded sample of one HSMA step of workload `w`, run by the oracle as it stands
+    (oracle/direct_sum.c, OpenMP over targets): the three direct sums at T_b of the N source targets
+    and at the same fraction of the check targets.  The fit and the mapping (O(1e6) flops) are not in
+    the sample; the node strengths are fixed numbers of the right size (their values do not change the
+    cost of a sum)."""
+
+    def __init__(self, w):
+        from oracle import hsma_oracle as O
+        self.O, self.w = O, w
+        L = np.asarray(w.L, dtype=np.float64)
+        self.src = np.ascontiguousarray(np.asarray(w.xyz, dtype=np.float64) - 0.5 * L)
+        self.q = np.ascontiguousarray(w.q, dtype=np.float64)
+        self.near = O.cell_table(w.kind, L, w.near_shell, w.gamma)
+        self.rhs_cells = (O.cell_table(w.kind, L, w.far_shell, w.gamma, exclude_shell=w.near_shell)
+                          if w.closure == W.CLOSURE_FAR_DATA else self.near)
+        R0 = 0.5 * float(np.linalg.norm(L))
+        if w.kind == W.BC_PERIODIC:
+            x = O.fibonacci_sphere_checkpoints(w.K, R0)
+            self.chk = np.concatenate([x, O.wrap_into_box(x, L)], axis=0)
+        else:
+            self.chk = np.asarray(w.check_xyz, dtype=np.float64)
+        self.nodes, self.nrm, wq = O.make_nodes(w.M, w.R_aux, w.quad_rule)
+        self.Q = wq / (4 * np.pi)
+        self.D = wq / (4 * np.pi)
+        self.cores = O.num_threads()
+
+    def run(self, T_b: int):
+        """Returns (seconds, pairs).  T_b source targets taken from the middle of the index range."""
+        w, O = self.w, self.O
+        N = w.N
+        T_b = max(1, min(N, T_b))
+        T_a = max(1, min(self.chk.shape[0], int(round(self.chk.shape[0] * T_b / N))))
+        i0 = (N - T_b) // 2
+        t0 = time.perf_counter()
+        O.near_sum(self.chk[:T_a], self.src, self.q, self.rhs_cells)
+        O.near_sum(self.src[i0:i0 + T_b], self.src, self.q, self.near, self_offset=i0)
+        O.node_sum(self.src[i0:i0 + T_b], self.nodes, self.nrm, self.Q, self.D)
+        dt = time.perf_counter() - t0
+        pairs = (T_a * N * self.rhs_cells.w.shape[0] + T_b * N * self.near.w.shape[0] + T_b * w.M)
+        return dt, pairs, T_a
+
+    def calibrate(self, seconds: float) -> int:
+        """Number of source targets whose sample takes about `seconds` on this host."""
+        T = max(1, min(self.w.N, self.cores))
+        dt, pairs, _ = self.run(T)
+        while dt < 0.2 and T < self.w.N:
+            T = min(self.w.N, T * 4)
+            dt, pairs, _ = self.run(T)
+        return max(1, min(self.w.N, int(T * seconds / max(dt, 1e-6))))
+
+
+def cpu_baseline(w, seconds: float) -> dict:
+    s = OracleSample(w)
+    T = s.calibrate(seconds)
+    dt, pairs, T_a = s.run(T)
+    return {"value": pairs / dt, "unit": UNIT, "cores": s.cores, "kind": "oracle", "seconds": dt,
+            "sample": f"{w.name}: oracle direct sums (a)+(b)+(c) at {T} of {w.N} source targets and {T_a} of "
+                      f"{s.chk.shape[0]} check targets against all {w.N} sources x cells ({pairs:.3e} pairs); "
+                      f"fit and mapping not in the sample"}
+
+
+def run_reference(args, w) -> dict:
+    """--impl reference: the oracle, as it stands, on the host cores; each step is a bounded sample."""
+    s = OracleSample(w)
+    T = s.calibrate(args.ref_step_seconds)
+    for _ in range(args.warmup):
+        s.run(T)
+    tot_t, tot_p, T_a = 0.0, 0, 0
+    for _ in range(args.steps):
+        dt, pairs, T_a = s.run(T)
+        tot_t += dt
+        tot_p += pairs
+    value = tot_p / tot_t
+    sample = (f"{w.name}: per step the oracle direct sums (a)+(b)+(c) at {T} of {w.N} source targets and {T_a} check "
+              f"targets against all sources x cells ({tot_p / args.steps:.3e} pairs/step); fit and mapping not in the sample")
+    return {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps,
+            "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": w.name, "N": w.N, "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": s.cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+
+
+# ---------------------------------------------------------------------------------------------------
+# CUDA arm
+# ---------------------------------------------------------------------------------------------------
+def run_b200(args, w) -> dict:
+    import torch
+    import torch.distributed as dist
+
+    import paper_1806_04801_b200 as H
+    from paper_1806_04801_b200 import shard
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the CUDA path has no CPU fallback")
+    H.binding.load_library()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != args.gpus:
+        raise RuntimeError(f"--gpus {args.gpus} but WORLD_SIZE={world}: launch with torch.distributed.run")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    N = w.N
+    t0, t1 = shard.shard_bounds(N, world)[rank]
+    T = t1 - t0
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    plan = H.Plan.from_workload(w, rsqrt_refine=args.refine)
+    info = plan.info
+    refine = args.refine if args.refine else (2 if float(N) * N * info["near_cells"] < 2.0 ** 32 else 1)
+    xyz = torch.as_tensor(np.ascontiguousarray(w.xyz), device=dev)
+    q = torch.as_tensor(np.ascontiguousarray(w.q), device=dev)
+    phi = torch.empty(T, dtype=torch.float64, device=dev)
+    U = torch.empty(1, dtype=torch.float64, device=dev)
+    flush = torch.empty(256 * 1024 * 1024 // 8, dtype=torch.float64, device=dev)   # 256 MiB > 126 MB L2
+
+    def step():
+        flush.zero_()                                     # L2 flush between iterations (torch memset, not counted)
+        H.hsma_evaluate_shard(plan.handle, xyz, q, t0, t1, phi, U)
+        if world > 1:                                     # the exchange step: assemble phi and U on every rank
+            full = shard.all_gather_phi(phi, N)
+            shard.all_reduce_energy(U)
+            return full
+        return phi
+
+    # peak FP64 (DFMA microbenchmark) before the run: the measured roofline denominator
+    dfma_tflops, _ = H.hsma_fp64_peak(args.peak_seconds)
+
+    for _ in range(args.warmup):
+        step()
+    plan.sync()
+    plan.set_timing(True)
+    stage_ms = {k: 0.0 for k in H.binding.TIMING_KEYS}
+    sampler = ClockSampler(local)
+    barrier()
+    sampler.start()
+    launches0 = H.hsma_launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+        for k, v in plan.timing().items():               # synchronises the stream once per step
+            stage_ms[k] += v
+    e1.record()
+    barrier()
+    launches = H.hsma_launch_count() - launches0
+    clocks = sampler.stop()
+    ms = e0.elapsed_time(e1) / args.steps
+    plan.set_timing(False)
+    U_val = float(U.cpu()[0])
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t[0])
+    stage_ms = {k: v / args.steps for k, v in stage_ms.items()}
+
+    # whole-job pairs per step: (a) once (computed redundantly by every rank, counted once), (b), (c) over all N
+    pc_all = pair_counts(info, N, N)
+    pairs_step = pc_all["a"] + pc_all["b"] + pc_all["c"]
+    value = pairs_step / (ms * 1e-3)
+
+    # end to end through the C-ABI with HOST buffers (pinned): H2D of xyz,q and D2H of phi,U inside the timed region
+    xyz_h = torch.as_tensor(np.ascontiguousarray(w.xyz)).pin_memory()
+    q_h = torch.as_tensor(np.ascontiguousarray(w.q)).pin_memory()
+    phi_h = torch.empty(max(T, 1), dtype=torch.float64).pin_memory()
+    U_h = torch.empty(1, dtype=torch.float64).pin_memory()
+    xyz_n, q_n, phi_n, U_n = xyz_h.numpy(), q_h.numpy(), phi_h.numpy(), U_h.numpy()
+
+    def step_e2e():
+        flush.zero_()
+        H.hsma_evaluate_shard_host(plan.handle, xyz_n, q_n, t0, t1, phi_n, U_n)   # synchronises (returns host data)
+
+    n_e2e = max(1, min(args.steps, args.e2e_steps))
+    step_e2e()
+    barrier()
+    tw = time.perf_counter()
+    for _ in range(n_e2e):
+        step_e2e()
+    barrier()
+    ms_e2e = 1e3 * (time.perf_counter() - tw) / n_e2e
+    if world > 1:
+        t = torch.tensor([ms_e2e], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_e2e = float(t[0])
+    e2e = {"value": pairs_step / (ms_e2e * 1e-3), "unit": UNIT, "ms_per_step": ms_e2e, "steps": n_e2e,
+           "h2d_bytes_per_step": int(xyz_n.nbytes + q_n.nbytes), "d2h_bytes_per_step": int(8 * T + 8),
+           "api": "hsma_evaluate_shard_host (pinned host buffers; per rank: all sources in, its phi shard and U out)"}
+
+    # roofline of the dominant kernel: near_sum_kernel over the sources, step (b)
+    pc_rank = pair_counts(info, N, T)
+    k_ms = stage_ms["near_source_kernel"]
+    sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except (OSError, ValueError):
+        pass
+    sm_max_mhz = float(peaks.get("sm_max_mhz") or clocks.get("sm_max_mhz") or 1965.0)
+    peak_tf = sm_count * FP64_LANES_PER_SM * 2 * sm_max_mhz * 1e6 * 1e-12
+    ach_tf = pc_rank["b"] * FLOPS_PAIR_CHARGE / (k_ms * 1e-3) * 1e-12 if k_ms > 0 else 0.0
+    ex_instr, ex_flops = EXEC_PAIR[refine]
+    issue_peak = sm_count * FP64_LANES_PER_SM * sm_max_mhz * 1e6          # FP64-pipe thread-instructions/s
+    roofline = {"bound": "alu", "kernel": f"near_sum_kernel<R,{refine}> step (b)", "achieved": ach_tf, "peak": peak_tf,
+                "unit": "TFLOP/s", "frac": ach_tf / peak_tf, "traffic": None,
+                "peak_source": f"derived: {sm_count} SMs x {FP64_LANES_PER_SM} FP64 lanes x 2 x {sm_max_mhz:.0f} MHz "
+                               f"(no FP64 entry in MEASURED_PEAKS.json)",
+                "flops_per_pair_algorithmic": FLOPS_PAIR_CHARGE, "pairs_per_launch": pc_rank["b"],
+                "kernel_ms": k_ms, "kernel_pairs_per_s": pc_rank["b"] / (k_ms * 1e-3) if k_ms > 0 else 0.0,
+                "kernel_share_of_step": k_ms / stage_ms["total"] if stage_ms["total"] > 0 else None,
+                "flops_per_pair_executed": ex_flops, "fp64_instr_per_pair_executed": ex_instr,
+                "frac_executed_flops": pc_rank["b"] * ex_flops / (k_ms * 1e-3) * 1e-12 / peak_tf if k_ms > 0 else 0.0,
+                "fp64_pipe_issue_util": pc_rank["b"] * ex_instr / (k_ms * 1e-3) / issue_peak if k_ms > 0 else 0.0,
+                "dfma_microbench_tflops": dfma_tflops, "frac_of_dfma_microbench": ach_tf / dfma_tflops if dfma_tflops else None}
+
+    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+           "ms_per_step": ms, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64",
+           "data": "synthetic",
+           "config": {"workload": w.name, "N": N, "near_cells": info["near_cells"], "p": info["p"], "M": info["M"],
+                      "check_targets": info["check_targets"], "pairs_per_step": pc_all, "rsqrt_refine": refine,
+                      "parallelism": f"targets sharded over {world} rank(s), sources replicated",
+                      "l2": "256 MiB flush written between iterations"},
+           "energy": U_val, "stage_ms": stage_ms, "e2e": e2e, "gpu_launches": int(launches),
+           "launches_per_step": plan.launches_last_evaluate(), "clocks": clocks, "roofline": roofline}
+    plan.close()
+    if world > 1:
+        dist.destroy_process_group()
+    return out if rank == 0 else {}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--config", type=int, default=5, help="BASELINE.json configs[config-1]; 5 = the metric's workload")
+    ap.add_argument("--size", type=int, default=None, help="override N (same generator and seed)")
+    ap.add_argument("--refine", type=int, default=0, choices=[0, 1, 2], help="hsma_plan_desc.rsqrt_refine")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--peak-seconds", type=float, default=1.0)
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="size of the cpu_baseline sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--ref-step-seconds", type=float, default=5.0, help="--impl reference: oracle sample per step")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "b200":
+        print(f"note: --warmup {args.warmup} < 3 (timing rules ask for >= 3)", file=sys.stderr)
+    w = W.config(args.config, N=args.size)
+    rank = int(os.environ.get("RANK", "0"))
+    if args.impl == "reference":
+        if rank == 0:
+            print(json.dumps(run_reference(args, w)), flush=True)
+        return
+    out = run_b200(args, w)
+    if rank == 0:
+        if args.gpus == 1 and not args.no_cpu_baseline:
+            out["cpu_baseline"] = cpu_baseline(w, args.cpu_seconds)
+        print(json.dumps(out), flush=True)
+
+
+if __name__ == "__main__":
+    main()

@@ -116,6 +116,11 @@ hsma_status hsma_evaluate_shard(hsma_plan* plan, const double* xyz, const double
  */
 hsma_status hsma_evaluate_host(hsma_plan* plan, const double* xyz_host, const double* q_host,
                                long long N, double* phi_host, double* energy_host);
+/* Target-sharded end-to-end form: all N sources are copied in, phi_host [t1-t0] and the shard's
+ * energy_host [1] are copied out.  hsma_evaluate_host is this with t0 = 0, t1 = N. */
+hsma_status hsma_evaluate_shard_host(hsma_plan* plan, const double* xyz_host, const double* q_host,
+                                     long long N, long long t0, long long t1, double* phi_host,
+                                     double* energy_host);
 
 /* Synchronise the plan's stream and return the sticky status of the evaluations since the last
  * call (HSMA_ERR_NOT_NEUTRAL, HSMA_ERR_CUDA, ...), then clear it. */
@@ -152,6 +157,18 @@ hsma_status hsma_node_sum(const double* tgt, long long T, const double* R, const
 /* DFMA-only microbenchmark on the current device: sustained FP64 FMA TFLOP/s over ~`seconds`
  * (the roofline denominator).  host out; synchronises. */
 hsma_status hsma_fp64_peak(double seconds, double* tflops_out, double* sm_clock_mhz_out);
+
+/*
+ * Per-stage device timing (bench.py "roofline").  While enabled, every evaluate
+ * records CUDA events on the plan's stream around its stages (no host synchronisation is added).
+ * hsma_plan_get_timing synchronises the stream and writes the stage durations of the LAST evaluate in
+ * milliseconds to host ms_out [8]:
+ *   [0] H1 pre-pass (+ neutrality)   [1] H2 near_sum_kernel over the check targets, kernel only
+ *   [2] H2 finish + H3 fit + H4 map  [3] H5 near_sum_kernel over the sources, kernel only (the hot loop)
+ *   [4] H6 node_sum_kernel, kernel only   [5] H7 finish + energy   [6] whole evaluate   [7] 0
+ */
+hsma_status hsma_plan_set_timing(hsma_plan* plan, int enable);
+hsma_status hsma_plan_get_timing(hsma_plan* plan, double* ms_out);
 
 /* total number of kernels this library has launched in this process */
 long long hsma_launch_count(void);

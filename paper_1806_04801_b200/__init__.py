@@ -87,6 +87,12 @@ class Plan:
     def sync(self):
         binding.hsma_plan_sync(self.handle)
 
+    def set_timing(self, enable: bool = True):
+        binding.hsma_plan_set_timing(self.handle, enable)
+
+    def timing(self) -> dict:
+        return binding.hsma_plan_get_timing(self.handle)
+
     # -- introspection (device tensors) ----------------------------------------------------------
     def _new(self, *shape):
         return torch.empty(*shape, dtype=torch.float64, device="cuda")

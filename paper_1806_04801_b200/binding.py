@@ -53,6 +53,9 @@ _SIGNATURES = {
                                            ctypes.c_longlong, ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p]),
     "hsma_evaluate_host": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_longlong,
                                           ctypes.c_void_p, ctypes.c_void_p]),
+    "hsma_evaluate_shard_host": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_longlong,
+                                                ctypes.c_longlong, ctypes.c_longlong, ctypes.c_void_p,
+                                                ctypes.c_void_p]),
     "hsma_plan_sync": (ctypes.c_int, [ctypes.c_void_p]),
     "hsma_status_string": (ctypes.c_char_p, [ctypes.c_int]),
     "hsma_plan_info": (ctypes.c_int, [ctypes.c_void_p, ctypes.POINTER(ctypes.c_longlong)]),
@@ -69,6 +72,8 @@ _SIGNATURES = {
     "hsma_node_sum": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p,
                                      ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p]),
     "hsma_fp64_peak": (ctypes.c_int, [ctypes.c_double, c_double_p, c_double_p]),
+    "hsma_plan_set_timing": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int]),
+    "hsma_plan_get_timing": (ctypes.c_int, [ctypes.c_void_p, c_double_p]),
     "hsma_launch_count": (ctypes.c_longlong, []),
 }
 EXPORTS = tuple(_SIGNATURES)
@@ -191,6 +196,21 @@ def hsma_evaluate_host(plan: int, xyz: np.ndarray, q: np.ndarray, phi_out: Optio
            "hsma_evaluate_host")
 
 
+def hsma_evaluate_shard_host(plan: int, xyz: np.ndarray, q: np.ndarray, t0: int, t1: int,
+                             phi_out: Optional[np.ndarray], energy_out: Optional[np.ndarray]):
+    """As hsma_evaluate_host for the targets t0 <= i < t1: phi_out [t1-t0]."""
+    for a in (xyz, q, phi_out, energy_out):
+        if a is not None and not (a.dtype == np.float64 and a.flags.c_contiguous):
+            raise TypeError("host buffers must be C-contiguous float64")
+    if phi_out is not None and phi_out.shape[0] < t1 - t0:
+        raise ValueError("phi_out too small")
+    N = q.shape[0]
+    _check(load_library().hsma_evaluate_shard_host(plan, xyz.ctypes.data, q.ctypes.data, N, t0, t1,
+                                                   None if phi_out is None else phi_out.ctypes.data,
+                                                   None if energy_out is None else energy_out.ctypes.data),
+           "hsma_evaluate_shard_host")
+
+
 def hsma_plan_sync(plan: int):
     _check(load_library().hsma_plan_sync(plan), "hsma_plan_sync")
 
@@ -249,6 +269,20 @@ def hsma_fp64_peak(seconds: float = 1.0):
     t, c = ctypes.c_double(), ctypes.c_double()
     _check(load_library().hsma_fp64_peak(seconds, ctypes.byref(t), ctypes.byref(c)), "hsma_fp64_peak")
     return t.value, c.value
+
+
+TIMING_KEYS = ("prepass", "near_check_kernel", "fit_map", "near_source_kernel", "node_kernel", "finish", "total")
+
+
+def hsma_plan_set_timing(plan: int, enable: bool):
+    _check(load_library().hsma_plan_set_timing(plan, 1 if enable else 0), "hsma_plan_set_timing")
+
+
+def hsma_plan_get_timing(plan: int) -> dict:
+    """Stage durations (ms) of the last evaluate; synchronises the plan's stream."""
+    ms = (ctypes.c_double * 8)()
+    _check(load_library().hsma_plan_get_timing(plan, ms), "hsma_plan_get_timing")
+    return dict(zip(TIMING_KEYS, [float(v) for v in ms]))
 
 
 def hsma_launch_count() -> int:

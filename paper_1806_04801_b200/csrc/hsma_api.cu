@@ -146,6 +146,10 @@ struct hsma_plan {
     DevBuf<double> part_a, part_b, part_c, red, xyz_in, q_in, phi_dev;
     long long last_launches = 0;
     hsma_status sticky = HSMA_OK;
+    // stage timing (hsma_plan_set_timing): events ev[0..7] bracket the stages of one evaluate
+    bool timing = false;
+    cudaEvent_t ev[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    bool ev_valid = false;
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -159,6 +163,7 @@ static void plan_free(hsma_plan* p) {
     for (void* q : ptrs) if (q) cudaFree(q);
     p->src.release(); p->part_a.release(); p->part_b.release(); p->part_c.release(); p->red.release();
     p->xyz_in.release(); p->q_in.release(); p->phi_dev.release();
+    for (cudaEvent_t e : p->ev) if (e) cudaEventDestroy(e);
     delete p;
 }
 
@@ -336,6 +341,9 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
     const long long n_tiles = (N + kTile - 1) / kTile, Npad = n_tiles * kTile;
     const hsma_plan_desc& d = p->d;
 
+#define MARK(i) do { if (p->timing) cudaEventRecord(p->ev[i], st); } while (0)
+    p->ev_valid = false;
+    MARK(0);
     // H1 pre-pass: centre + pack, neutrality flag
     const int pb = 256;
     const long long pack_blocks = (Npad + pb - 1) / pb;
@@ -354,7 +362,9 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
     {
         const Split s = choose_split(p->Kt, n_tiles, p->C_rhs);
         if (p->part_a.reserve((size_t)s.ny * p->Kt) != cudaSuccess) return HSMA_ERR_ALLOC;
+        MARK(1);
         launch_near(s, p->chk, 3, p->Kt, 0, p->src.p, n_tiles, p->cells_rhs, p->C_rhs, -1, 2, p->part_a.p, st);  // (a) always cubic: it feeds the fit
+        MARK(2);
         finish_phi_kernel<<<(p->Kt + 255) / 256, 256, 0, st>>>(p->part_a.p, s.ny, nullptr, 0, p->Kt, nullptr, 0, p->pc, nullptr);
         HSMA_COUNT_LAUNCH();
     }
@@ -374,12 +384,15 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
         if (p->part_b.reserve((size_t)sb.ny * T) != cudaSuccess) return HSMA_ERR_ALLOC;
         // rsqrt_refine = 0: the cubic step while (b) is latency-bound anyway (< 2^32 pairs), Newton above
         const int refine = p->refine ? p->refine : ((double)N * (double)N * p->C_near < 4294967296.0 ? 2 : 1);
-        launch_near(sb, reinterpret_cast<const double*>(p->src.p), 4, T, t0, p->src.p, n_tiles, p->cells_near, p->C_near,
-                    t0, refine, p->part_b.p, st);
-        // H6 (c): sphere nodes, charge + dipole
         const NodeSplit sc = choose_node_split(T, p->node_tiles);
         if (p->part_c.reserve((size_t)sc.ny * T) != cudaSuccess) return HSMA_ERR_ALLOC;
+        MARK(3);
+        launch_near(sb, reinterpret_cast<const double*>(p->src.p), 4, T, t0, p->src.p, n_tiles, p->cells_near, p->C_near,
+                    t0, refine, p->part_b.p, st);
+        MARK(4);
+        // H6 (c): sphere nodes, charge + dipole
         launch_node(sc, reinterpret_cast<const double*>(p->src.p), 4, T, t0, p->nodes, p->node_tiles, p->part_c.p, st);
+        MARK(5);
         // H7: phi and U
         const long long fb = (T + 255) / 256;
         finish_phi_kernel<<<(unsigned)fb, 256, 0, st>>>(p->part_b.p, sb.ny, p->part_c.p, sc.ny, T, p->src.p, t0, phi_out,
@@ -389,9 +402,13 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
             reduce_rows_kernel<<<1, 1024, 0, st>>>(p->red.p, fb, 1, 1, 0.5, energy_out);
             HSMA_COUNT_LAUNCH();
         }
-    } else if (energy_out) {
-        if (cudaMemsetAsync(energy_out, 0, sizeof(double), st) != cudaSuccess) return HSMA_ERR_CUDA;
+    } else {
+        MARK(3); MARK(4); MARK(5);
+        if (energy_out && cudaMemsetAsync(energy_out, 0, sizeof(double), st) != cudaSuccess) return HSMA_ERR_CUDA;
     }
+    MARK(6);
+#undef MARK
+    p->ev_valid = p->timing;
     p->last_launches = g_launches - before;
     if (cudaPeekAtLastError() != cudaSuccess) { cudaGetLastError(); p->sticky = HSMA_ERR_CUDA; return HSMA_ERR_CUDA; }
     return HSMA_OK;
@@ -422,20 +439,28 @@ extern "C" hsma_status hsma_plan_sync(hsma_plan* plan) {
     return s;
 }
 
-extern "C" hsma_status hsma_evaluate_host(hsma_plan* p, const double* xyz_host, const double* q_host, long long N,
-                                          double* phi_host, double* energy_host) {
-    if (!p || !xyz_host || !q_host || N < 1) return HSMA_ERR_INVALID_ARG;
+extern "C" hsma_status hsma_evaluate_shard_host(hsma_plan* p, const double* xyz_host, const double* q_host,
+                                                long long N, long long t0, long long t1, double* phi_host,
+                                                double* energy_host) {
+    if (!p || !xyz_host || !q_host || N < 1 || t0 < 0 || t1 > N || t0 > t1) return HSMA_ERR_INVALID_ARG;
+    const long long T = t1 - t0;
     if (p->xyz_in.reserve(3 * (size_t)N) != cudaSuccess || p->q_in.reserve((size_t)N) != cudaSuccess ||
-        p->phi_dev.reserve((size_t)N) != cudaSuccess)
+        p->phi_dev.reserve((size_t)std::max(1LL, T)) != cudaSuccess)
         return HSMA_ERR_ALLOC;
     cudaStream_t st = p->stream;
     CU(cudaMemcpyAsync(p->xyz_in.p, xyz_host, 3 * (size_t)N * sizeof(double), cudaMemcpyHostToDevice, st));
     CU(cudaMemcpyAsync(p->q_in.p, q_host, (size_t)N * sizeof(double), cudaMemcpyHostToDevice, st));
-    hsma_status s = evaluate_impl(p, p->xyz_in.p, p->q_in.p, N, 0, N, p->phi_dev.p, p->scalars);
+    hsma_status s = evaluate_impl(p, p->xyz_in.p, p->q_in.p, N, t0, t1, p->phi_dev.p, p->scalars);
     if (s != HSMA_OK) return s;
-    if (phi_host) CU(cudaMemcpyAsync(phi_host, p->phi_dev.p, (size_t)N * sizeof(double), cudaMemcpyDeviceToHost, st));
+    if (phi_host && T > 0)
+        CU(cudaMemcpyAsync(phi_host, p->phi_dev.p, (size_t)T * sizeof(double), cudaMemcpyDeviceToHost, st));
     if (energy_host) CU(cudaMemcpyAsync(energy_host, p->scalars, sizeof(double), cudaMemcpyDeviceToHost, st));
     return hsma_plan_sync(p);
+}
+
+extern "C" hsma_status hsma_evaluate_host(hsma_plan* p, const double* xyz_host, const double* q_host, long long N,
+                                          double* phi_host, double* energy_host) {
+    return hsma_evaluate_shard_host(p, xyz_host, q_host, N, 0, N, phi_host, energy_host);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -615,6 +640,32 @@ extern "C" hsma_status hsma_fp64_peak(double seconds, double* tflops_out, double
     cudaEventDestroy(e0); cudaEventDestroy(e1);
     cudaFree(out);
     return rc;
+}
+
+extern "C" hsma_status hsma_plan_set_timing(hsma_plan* p, int enable) {
+    if (!p) return HSMA_ERR_INVALID_ARG;
+    if (enable)
+        for (cudaEvent_t& e : p->ev)
+            if (!e) CU(cudaEventCreate(&e));
+    p->timing = enable != 0;
+    p->ev_valid = false;
+    return HSMA_OK;
+}
+
+extern "C" hsma_status hsma_plan_get_timing(hsma_plan* p, double* ms_out) {
+    if (!p || !ms_out || !p->timing || !p->ev_valid) return HSMA_ERR_INVALID_ARG;
+    CU(cudaEventSynchronize(p->ev[6]));
+    double ms[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    for (int i = 0; i < 6; ++i) {
+        float f = 0.f;
+        CU(cudaEventElapsedTime(&f, p->ev[i], p->ev[i + 1]));
+        ms[i] = f;
+    }
+    float tot = 0.f;
+    CU(cudaEventElapsedTime(&tot, p->ev[0], p->ev[6]));
+    ms[6] = tot;
+    for (int i = 0; i < 8; ++i) ms_out[i] = ms[i];
+    return HSMA_OK;
 }
 
 extern "C" long long hsma_launch_count(void) { return g_launches; }

@@ -1,0 +1,68 @@
+"""The N > 1 path on CPU: world_size-2 `gloo` processes run the host-side sharding of DESIGN.md
+"Multi-GPU" (contiguous target shards, replicated sources, all-gather of phi, all-reduce of U), with the
+oracle standing in for the per-rank evaluation (tests may call oracle/).  `-m "not gpu"`."""
+import os
+import sys
+
+import numpy as np
+import pytest
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1806_04801_b200 import shard  # noqa: E402
+
+
+@pytest.mark.parametrize("N,world", [(0, 1), (1, 2), (5, 8), (255, 2), (1000, 2), (1000, 3), (262144, 8), (262145, 7)])
+def test_shard_bounds_cover_exactly_once(N, world):
+    b = shard.shard_bounds(N, world)
+    assert len(b) == world and b[0][0] == 0 and b[-1][1] == N
+    for (a0, a1), (b0, b1) in zip(b[:-1], b[1:]):
+        assert a1 == b0 and a0 <= a1
+    sizes = [y - x for x, y in b]
+    assert max(sizes) - min(sizes) <= (shard.ALIGN if N >= shard.ALIGN * world else 1)
+    if N >= shard.ALIGN * world:
+        assert all(x % shard.ALIGN == 0 for x, _ in b)
+
+
+def _worker(rank, world, port, N, out_dir):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        import hsma_workloads as W
+        from oracle import hsma_oracle as O
+        w = W.config(2, N=N)
+        t0, t1 = shard.shard_bounds(N, world)[rank]
+        r = O.hsma(w, targets_slice=slice(t0, t1))      # this rank's shard: phi[t0:t1], U over the shard
+        phi = shard.all_gather_phi(torch.from_numpy(r.phi.copy()), N)
+        U = shard.all_reduce_energy(torch.tensor([r.U], dtype=torch.float64))
+        np.save(os.path.join(out_dir, f"phi{rank}.npy"), phi.numpy())
+        np.save(os.path.join(out_dir, f"U{rank}.npy"), U.numpy())
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("N", [600, 257 * 2])
+def test_two_ranks_assemble_the_single_rank_result(tmp_path, N):
+    import hsma_workloads as W
+    from oracle import hsma_oracle as O
+    world, port = 2, 29500 + (os.getpid() + N) % 2000
+    mp.spawn(_worker, args=(world, port, N, str(tmp_path)), nprocs=world, join=True)
+    ref = O.hsma(W.config(2, N=N))
+    for r in range(world):
+        phi = np.load(tmp_path / f"phi{r}.npy")
+        U = float(np.load(tmp_path / f"U{r}.npy")[0])
+        assert phi.shape == (N,)
+        assert np.array_equal(phi, ref.phi)             # same per-target arithmetic: bit-identical
+        assert abs(U - ref.U) <= 1e-14 * abs(ref.U)
+
+
+def test_single_process_is_a_no_op():
+    x = torch.arange(5, dtype=torch.float64)
+    assert shard.all_gather_phi(x, 5) is x
+    u = torch.tensor([1.5], dtype=torch.float64)
+    assert shard.all_reduce_energy(u) is u
