@@ -37,10 +37,6 @@ struct DevBuf {  // growable device buffer owned by the plan
     void release() { if (p) cudaFree(p); p = nullptr; cap = 0; }
 };
 
-struct Split {  // decomposition of one pair-kernel launch
-    int R, ntb, nss, tiles_per_split, ncg, cells_per_group, ny;
-};
-
 static int g_num_sm = 0;
 static int num_sm() {
     if (!g_num_sm) {
@@ -52,69 +48,92 @@ static int num_sm() {
     return g_num_sm;
 }
 
-// Grid sizing: CTAs = ntb x ny with ny splits over (source tiles x cell groups),
-// aiming at >= 16 waves of 2 CTAs/SM when there is enough work, never below 4 (tile,cell) units per CTA.
-static Split choose_split(long long T, long long n_tiles, int C) {
-    Split s;
-    const long long slots = 2LL * num_sm();
-    s.R = T >= slots * kThreads * 4 / 2 ? 4 : (T >= slots * kThreads ? 2 : 1);
-    s.ntb = (int)((T + (long long)kThreads * s.R - 1) / ((long long)kThreads * s.R));
-    const long long units = n_tiles * C;
-    long long want = (16 * slots + s.ntb - 1) / s.ntb;
-    want = std::max(1LL, std::min(want, std::max(1LL, units / 4)));
-    want = std::min(want, 32768LL);
-    long long nss = std::min(want, n_tiles);
-    s.tiles_per_split = (int)((n_tiles + nss - 1) / nss);
-    s.nss = (int)((n_tiles + s.tiles_per_split - 1) / s.tiles_per_split);
-    long long ncg = std::max(1LL, std::min((long long)C, want / s.nss));
-    s.cells_per_group = (int)((C + ncg - 1) / ncg);
-    s.ncg = (C + s.cells_per_group - 1) / s.cells_per_group;
-    s.ny = s.nss * s.ncg;
-    return s;
+// Persistent launch shape of one pair kernel (sum_kernels.cuh "work decomposition").
+struct Launch {
+    int R;            // targets per thread
+    int ntb;          // target blocks of kThreads * R
+    long long Ub, U;  // units per block / in all
+    int G;            // CTAs = min(resident CTAs, U)
+    int rows;         // rows of the partial-sum buffer
+    PartLayout layout(const double* part) const { return PartLayout{part, U, Ub, G, kThreads * R}; }
+};
+
+template <class K>
+static int resident_ctas(K kernel) {
+    int per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, kThreads, 0) != cudaSuccess || per_sm < 1) {
+        cudaGetLastError();
+        per_sm = 1;
+    }
+    return per_sm * num_sm();
+}
+static int near_resident(int R, int refine) {
+    static int cache[3][2] = {{0, 0}, {0, 0}, {0, 0}};
+    const int i = R == 4 ? 2 : (R == 2 ? 1 : 0), j = refine == 1 ? 0 : 1;
+    if (!cache[i][j]) {
+        if (refine == 1) cache[i][j] = R == 4 ? resident_ctas(near_sum_kernel<4, 1>) : R == 2 ? resident_ctas(near_sum_kernel<2, 1>) : resident_ctas(near_sum_kernel<1, 1>);
+        else cache[i][j] = R == 4 ? resident_ctas(near_sum_kernel<4, 2>) : R == 2 ? resident_ctas(near_sum_kernel<2, 2>) : resident_ctas(near_sum_kernel<1, 2>);
+    }
+    return cache[i][j];
+}
+static int node_resident(int R) {
+    static int cache[3] = {0, 0, 0};
+    const int i = R == 4 ? 2 : (R == 2 ? 1 : 0);
+    if (!cache[i]) cache[i] = R == 4 ? resident_ctas(node_sum_kernel<4>) : R == 2 ? resident_ctas(node_sum_kernel<2>) : resident_ctas(node_sum_kernel<1>);
+    return cache[i];
 }
 
-template <int REFINE>
-static void launch_near_r(const Split& s, const NearArgs& a, cudaStream_t st) {
-    dim3 grid(s.ntb, s.ny);
-    if (s.R == 4) near_sum_kernel<4, REFINE><<<grid, kThreads, 0, st>>>(a);
-    else if (s.R == 2) near_sum_kernel<2, REFINE><<<grid, kThreads, 0, st>>>(a);
-    else near_sum_kernel<1, REFINE><<<grid, kThreads, 0, st>>>(a);
-    HSMA_COUNT_LAUNCH();
+// The largest R in {4, 2, 1} that still leaves every resident CTA at least 4 units; R = 1 otherwise.
+template <class Resident>
+static Launch choose_launch(long long T, long long units_per_block, Resident resident) {
+    Launch L;
+    for (int R : {4, 2, 1}) {
+        L.R = R;
+        L.ntb = (int)((T + (long long)kThreads * R - 1) / ((long long)kThreads * R));
+        L.Ub = units_per_block;
+        L.U = L.ntb * L.Ub;
+        const int res = resident(R);
+        L.G = (int)std::min<long long>(res, L.U);
+        if (L.U >= 4LL * res) break;
+    }
+    L.rows = part_rows(L.U, L.Ub, L.G);
+    return L;
 }
 
-// part must hold s.ny * T doubles
-static void launch_near(const Split& s, const double* tgt, int tstride, long long T, long long t_first, const Src4* src,
+// part must hold L.rows * T doubles
+static void launch_near(const Launch& L, const double* tgt, int tstride, long long T, long long t_first, const Src4* src,
                         long long n_tiles, const Cell* cells, int C, long long self_offset, int refine, double* part,
                         cudaStream_t st) {
     NearArgs a;
     a.tgt = tgt; a.tstride = tstride; a.T = T; a.t_first = t_first; a.src = src; a.n_tiles = n_tiles;
-    a.cells = cells; a.C = C; a.n_src_split = s.nss; a.tiles_per_split = s.tiles_per_split;
-    a.cells_per_group = s.cells_per_group; a.self_offset = self_offset;
+    a.cells = cells; a.C = C; a.units = L.U; a.self_offset = self_offset;
     a.scale = refine == 1 ? 0.5 : 1.0; a.part = part;
-    if (refine == 1) launch_near_r<1>(s, a, st); else launch_near_r<2>(s, a, st);
+    if (refine == 1) {
+        if (L.R == 4) near_sum_kernel<4, 1><<<L.G, kThreads, 0, st>>>(a);
+        else if (L.R == 2) near_sum_kernel<2, 1><<<L.G, kThreads, 0, st>>>(a);
+        else near_sum_kernel<1, 1><<<L.G, kThreads, 0, st>>>(a);
+    } else {
+        if (L.R == 4) near_sum_kernel<4, 2><<<L.G, kThreads, 0, st>>>(a);
+        else if (L.R == 2) near_sum_kernel<2, 2><<<L.G, kThreads, 0, st>>>(a);
+        else near_sum_kernel<1, 2><<<L.G, kThreads, 0, st>>>(a);
+    }
+    HSMA_COUNT_LAUNCH();
+}
+static Launch choose_near(long long T, long long n_tiles, int C, int refine) {
+    return choose_launch(T, n_tiles * C, [refine](int R) { return near_resident(R, refine); });
 }
 
-struct NodeSplit { int R, ntb, ny, tiles_per_split; };
-static NodeSplit choose_node_split(long long T, long long n_tiles) {
-    NodeSplit s;
-    const long long slots = 2LL * num_sm();
-    s.R = T >= slots * kThreads * 4 / 2 ? 4 : (T >= slots * kThreads ? 2 : 1);
-    s.ntb = (int)((T + (long long)kThreads * s.R - 1) / ((long long)kThreads * s.R));
-    long long want = (4 * slots + s.ntb - 1) / s.ntb;
-    want = std::max(1LL, std::min(want, std::max(1LL, n_tiles / 2)));
-    s.tiles_per_split = (int)((n_tiles + want - 1) / want);
-    s.ny = (int)((n_tiles + s.tiles_per_split - 1) / s.tiles_per_split);
-    return s;
+static Launch choose_node(long long T, long long n_tiles) {
+    return choose_launch(T, n_tiles, [](int R) { return node_resident(R); });
 }
-static void launch_node(const NodeSplit& s, const double* tgt, int tstride, long long T, long long t_first,
+static void launch_node(const Launch& L, const double* tgt, int tstride, long long T, long long t_first,
                         const Node8* nodes, long long n_tiles, double* part, cudaStream_t st) {
     NodeArgs a;
     a.tgt = tgt; a.tstride = tstride; a.T = T; a.t_first = t_first; a.nodes = nodes; a.n_tiles = n_tiles;
-    a.tiles_per_split = s.tiles_per_split; a.part = part;
-    dim3 grid(s.ntb, s.ny);
-    if (s.R == 4) node_sum_kernel<4><<<grid, kThreads, 0, st>>>(a);
-    else if (s.R == 2) node_sum_kernel<2><<<grid, kThreads, 0, st>>>(a);
-    else node_sum_kernel<1><<<grid, kThreads, 0, st>>>(a);
+    a.units = L.U; a.part = part;
+    if (L.R == 4) node_sum_kernel<4><<<L.G, kThreads, 0, st>>>(a);
+    else if (L.R == 2) node_sum_kernel<2><<<L.G, kThreads, 0, st>>>(a);
+    else node_sum_kernel<1><<<L.G, kThreads, 0, st>>>(a);
     HSMA_COUNT_LAUNCH();
 }
 
@@ -360,12 +379,12 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
 
     // H2 (a): Phi_in (or the far-cell data) at the monitoring points -> pc [Kt]
     {
-        const Split s = choose_split(p->Kt, n_tiles, p->C_rhs);
-        if (p->part_a.reserve((size_t)s.ny * p->Kt) != cudaSuccess) return HSMA_ERR_ALLOC;
+        const Launch s = choose_near(p->Kt, n_tiles, p->C_rhs, 2);
+        if (p->part_a.reserve((size_t)s.rows * p->Kt) != cudaSuccess) return HSMA_ERR_ALLOC;
         MARK(1);
         launch_near(s, p->chk, 3, p->Kt, 0, p->src.p, n_tiles, p->cells_rhs, p->C_rhs, -1, 2, p->part_a.p, st);  // (a) always cubic: it feeds the fit
         MARK(2);
-        finish_phi_kernel<<<(p->Kt + 255) / 256, 256, 0, st>>>(p->part_a.p, s.ny, nullptr, 0, p->Kt, nullptr, 0, p->pc, nullptr);
+        finish_phi_kernel<<<(p->Kt + 255) / 256, 256, 0, st>>>(s.layout(p->part_a.p), PartLayout{nullptr, 1, 1, 1, 1}, p->Kt, nullptr, 0, p->pc, nullptr);
         HSMA_COUNT_LAUNCH();
     }
     // H3: least squares, Eq.(7)
@@ -380,12 +399,12 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
     const long long T = t1 - t0;
     if (T > 0) {
         // H5 (b): near images at the sources, self excluded
-        const Split sb = choose_split(T, n_tiles, p->C_near);
-        if (p->part_b.reserve((size_t)sb.ny * T) != cudaSuccess) return HSMA_ERR_ALLOC;
-        // rsqrt_refine = 0: the cubic step while (b) is latency-bound anyway (< 2^32 pairs), Newton above
         const int refine = p->refine ? p->refine : ((double)N * (double)N * p->C_near < 4294967296.0 ? 2 : 1);
-        const NodeSplit sc = choose_node_split(T, p->node_tiles);
-        if (p->part_c.reserve((size_t)sc.ny * T) != cudaSuccess) return HSMA_ERR_ALLOC;
+        const Launch sb = choose_near(T, n_tiles, p->C_near, refine);
+        if (p->part_b.reserve((size_t)sb.rows * T) != cudaSuccess) return HSMA_ERR_ALLOC;
+        // rsqrt_refine = 0: the cubic step while (b) is latency-bound anyway (< 2^32 pairs), Newton above
+        const Launch sc = choose_node(T, p->node_tiles);
+        if (p->part_c.reserve((size_t)sc.rows * T) != cudaSuccess) return HSMA_ERR_ALLOC;
         MARK(3);
         launch_near(sb, reinterpret_cast<const double*>(p->src.p), 4, T, t0, p->src.p, n_tiles, p->cells_near, p->C_near,
                     t0, refine, p->part_b.p, st);
@@ -395,7 +414,7 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
         MARK(5);
         // H7: phi and U
         const long long fb = (T + 255) / 256;
-        finish_phi_kernel<<<(unsigned)fb, 256, 0, st>>>(p->part_b.p, sb.ny, p->part_c.p, sc.ny, T, p->src.p, t0, phi_out,
+        finish_phi_kernel<<<(unsigned)fb, 256, 0, st>>>(sb.layout(p->part_b.p), sc.layout(p->part_c.p), T, p->src.p, t0, phi_out,
                                                         energy_out ? p->red.p : nullptr);
         HSMA_COUNT_LAUNCH();
         if (energy_out) {
@@ -561,18 +580,18 @@ extern "C" hsma_status hsma_direct_sum(const double* tgt, long long T, const dou
         cells[c].central = (c == central_cell);
     }
     const long long n_tiles = (N + kTile - 1) / kTile, Npad = n_tiles * kTile;
-    const Split s = choose_split(T, n_tiles, C);
+    const Launch s = choose_near(T, n_tiles, C, refine);
     Cell* dc = nullptr; Src4* ds = nullptr; double* part = nullptr;
     hsma_status rc = HSMA_OK;
     if (cudaMalloc(&dc, C * sizeof(Cell)) != cudaSuccess || cudaMalloc(&ds, Npad * sizeof(Src4)) != cudaSuccess ||
-        cudaMalloc(&part, (size_t)s.ny * T * sizeof(double)) != cudaSuccess) {
+        cudaMalloc(&part, (size_t)s.rows * T * sizeof(double)) != cudaSuccess) {
         rc = HSMA_ERR_ALLOC;
     } else {
         cudaMemcpyAsync(dc, cells.data(), C * sizeof(Cell), cudaMemcpyHostToDevice, st);
         pack_plain_kernel<<<(unsigned)((Npad + 255) / 256), 256, 0, st>>>(src, q, N, Npad, ds);
         HSMA_COUNT_LAUNCH();
         launch_near(s, tgt, 3, T, 0, ds, n_tiles, dc, C, central_cell >= 0 ? self_offset : -1, refine, part, st);
-        finish_phi_kernel<<<(unsigned)((T + 255) / 256), 256, 0, st>>>(part, s.ny, nullptr, 0, T, nullptr, 0, phi_out, nullptr);
+        finish_phi_kernel<<<(unsigned)((T + 255) / 256), 256, 0, st>>>(s.layout(part), PartLayout{nullptr, 1, 1, 1, 1}, T, nullptr, 0, phi_out, nullptr);
         HSMA_COUNT_LAUNCH();
         if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) rc = HSMA_ERR_CUDA;
     }
@@ -588,16 +607,16 @@ extern "C" hsma_status hsma_node_sum(const double* tgt, long long T, const doubl
     cudaStream_t st = (cudaStream_t)cuda_stream;
     constexpr int kNT = kTile / 2;
     const long long n_tiles = (M + kNT - 1) / kNT, Mpad = n_tiles * kNT;
-    const NodeSplit s = choose_node_split(T, n_tiles);
+    const Launch s = choose_node(T, n_tiles);
     Node8* dn = nullptr; double* part = nullptr;
     hsma_status rc = HSMA_OK;
-    if (cudaMalloc(&dn, Mpad * sizeof(Node8)) != cudaSuccess || cudaMalloc(&part, (size_t)s.ny * T * sizeof(double)) != cudaSuccess) {
+    if (cudaMalloc(&dn, Mpad * sizeof(Node8)) != cudaSuccess || cudaMalloc(&part, (size_t)s.rows * T * sizeof(double)) != cudaSuccess) {
         rc = HSMA_ERR_ALLOC;
     } else {
         pack_nodes_kernel<<<(unsigned)((Mpad + 255) / 256), 256, 0, st>>>(R, Q, P, M, Mpad, dn);
         HSMA_COUNT_LAUNCH();
         launch_node(s, tgt, 3, T, 0, dn, n_tiles, part, st);
-        finish_phi_kernel<<<(unsigned)((T + 255) / 256), 256, 0, st>>>(nullptr, 0, part, s.ny, T, nullptr, 0, phi_out, nullptr);
+        finish_phi_kernel<<<(unsigned)((T + 255) / 256), 256, 0, st>>>(PartLayout{nullptr, 1, 1, 1, 1}, s.layout(part), T, nullptr, 0, phi_out, nullptr);
         HSMA_COUNT_LAUNCH();
         if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) rc = HSMA_ERR_CUDA;
     }

@@ -11,6 +11,33 @@
 
 namespace hsma {
 
+// ---- persistent work decomposition ------------------------------------------
+// The work of one launch is the linear sequence of units u = (target block b, source tile t, cell c),
+// cell fastest: u = (b * n_tiles + t) * C + c, U units in all.  The grid is persistent: G CTAs (one
+// wave: resident CTAs per SM x SMs), CTA k owns the contiguous range [unit_start(k), unit_start(k+1)),
+// so every CTA gets U/G units to within one unit and there is no tail wave.  A target block is covered by
+// a few consecutive CTAs; each writes its partial sums to row (k - first CTA of the block) of `part`,
+// and finish_phi_kernel adds the rows in that fixed order (no atomics: bit-reproducible).
+__host__ __device__ inline long long unit_start(long long k, long long U, int G) { return (k * U) / G; }
+__host__ __device__ inline int cta_of_unit(long long u, long long U, int G) {
+    long long k = (u * G) / U;
+    while (k + 1 < G && unit_start(k + 1, U, G) <= u) ++k;
+    while (k > 0 && unit_start(k, U, G) > u) --k;
+    return (int)k;
+}
+// rows of `part` that are enough for any block: CTAs overlapping an interval of Ub units
+__host__ __device__ inline int part_rows(long long U, long long Ub, int G) {
+    const long long per = U / G > 0 ? U / G : 1;
+    return (int)(Ub / per + 2);
+}
+
+struct PartLayout {      // how finish_phi_kernel finds the partial rows of one pair kernel
+    const double* part;  // [rows][T], or nullptr
+    long long U, Ub;     // units in all / per target block
+    int G;               // CTAs of the launch
+    int block_targets;   // targets per block (kThreads * R)
+};
+
 struct NearArgs {
     const double* tgt;   // targets, `tstride` doubles apart (3 = xyz rows, 4 = packed Src4 rows)
     int tstride;
@@ -20,17 +47,15 @@ struct NearArgs {
     long long n_tiles;   // padded source count / kTile
     const Cell* cells;   // [C]
     int C;
-    int n_src_split;     // blockIdx.y = cell_group * n_src_split + src_split
-    int tiles_per_split;
-    int cells_per_group;
+    long long units;     // U = ntb * n_tiles * C
     long long self_offset;  // >= 0: target t is source (self_offset + t); its bare term is skipped
     double scale;        // applied to the cell weights (0.5 for the Newton form, see below)
-    double* part;        // [gridDim.y][T] partial sums
+    double* part;        // [part_rows][T] partial sums
 };
 
 // One pair: acc += q / |d|.
 //  REFINE 1: y0 = seed; q*y = (q*y0) * (kNewton3 - r2*y0^2) / 2  (one Newton step; the 1/2 lives in `scale`)
-//            -> 3 DADD + DMUL + 2 DFMA (r2) + MUFU + DMUL + DFMA + DMUL + DFMA = 10 FP64-pipe instructions
+//            -> 3 DADD + DMUL + 2 DFMA (r2) + MUFU + DMUL + DMUL + DFMA + DFMA = 10 FP64-pipe instructions
 //            Plain Newton (constant 3) always lands below 1/sqrt: relative error -1.5 eps^2 for a seed
 //            error eps; measured on B200 (MUFU.RSQ64H): |eps| <= 9.2e-7 (2^-20), mean eps^2 = 7.6e-14, i.e.
 //            error in [-1.27e-12, 0] with mean -1.14e-13.  kNewton3 = 3 + 2.28e-13 shifts the mean to zero
@@ -57,60 +82,78 @@ __device__ __forceinline__ void pair(double tx, double ty, double tz, double sx,
     }
 }
 
+constexpr int near_min_ctas(int R) { return R == 4 ? 2 : (R == 2 ? 3 : 4); }
+
 template <int R, int REFINE>
-__global__ void __launch_bounds__(kThreads) near_sum_kernel(const NearArgs a) {
+__global__ void __launch_bounds__(kThreads, near_min_ctas(R)) near_sum_kernel(const NearArgs a) {
     __shared__ __align__(128) Src4 tile[kStages][kTile];
     __shared__ __align__(8) uint64_t full[kStages];
     __shared__ Cell cells[kMaxCells];
 
     const int tid = threadIdx.x;
-    const int split = blockIdx.y % a.n_src_split;
-    const int group = blockIdx.y / a.n_src_split;
-    const int c0 = group * a.cells_per_group;
-    const int c1 = min(a.C, c0 + a.cells_per_group);
-    const long long tile0 = (long long)split * a.tiles_per_split;
-    const long long tile1 = min(a.n_tiles, tile0 + a.tiles_per_split);
-    const int nt = (int)(tile1 - tile0);
+    const int G = gridDim.x, k = blockIdx.x;
+    const long long u0 = unit_start(k, a.units, G), u1 = unit_start(k + 1, a.units, G);
+    if (u1 <= u0) return;  // (never: the host launches G <= U CTAs)
+    const long long Ub = a.n_tiles * a.C;
+    const long long V0 = u0 / a.C, V1 = (u1 - 1) / a.C;  // visits v = b * n_tiles + t of this CTA
 
-    for (int c = c0 + tid; c < c1; c += kThreads) cells[c - c0] = a.cells[c];
+    for (int c = tid; c < a.C; c += kThreads) cells[c] = a.cells[c];
     if (tid == 0) {
         for (int s = 0; s < kStages; ++s) mbar_init(&full[s], 1);
         mbar_fence_init();
     }
     __syncthreads();
-    if (tid == 0 && nt > 0) {
+    if (tid == 0) {
         mbar_expect_tx(&full[0], kTile * sizeof(Src4));
-        bulk_g2s(tile[0], a.src + tile0 * kTile, kTile * sizeof(Src4), &full[0]);
+        bulk_g2s(tile[0], a.src + (V0 % a.n_tiles) * kTile, kTile * sizeof(Src4), &full[0]);
     }
 
-    // targets owned by this thread (tail threads recompute target T-1 and do not store)
-    const long long tb = (long long)blockIdx.x * (kThreads * R);
     double ox[R], oy[R], oz[R], tot[R];
-    long long ti[R];
+    // visits are walked with 32-bit state: block b, tile tl inside the block
+    const int nvis = (int)(V1 - V0) + 1;
+    const int nt = (int)a.n_tiles;
+    int b = (int)(V0 / a.n_tiles), tl = (int)(V0 - (long long)b * a.n_tiles);
+    const int c_first = (int)(u0 - V0 * a.C), c_last = (int)(u1 - 1 - V1 * a.C) + 1;
+    bool fresh = true;  // targets of block b not loaded yet
+    // partial sums of block b go to row (k - first CTA that works on b)
+    auto store_block = [&](int blk) {
+        const int row = k - cta_of_unit(blk * Ub, a.units, G);
 #pragma unroll
-    for (int r = 0; r < R; ++r) {
-        long long t = tb + r * kThreads + tid;
-        ti[r] = t < a.T ? t : a.T - 1;
-        const double* p = a.tgt + (a.t_first + ti[r]) * a.tstride;
-        ox[r] = p[0]; oy[r] = p[1]; oz[r] = p[2];
-        tot[r] = 0.0;
-    }
-    // block-uniform range of source indices that can be "self" for this block's targets
-    const long long self_lo = a.self_offset + tb;
-    const long long self_hi = a.self_offset + min(a.T, tb + (long long)kThreads * R);  // exclusive
+        for (int r = 0; r < R; ++r) {
+            const long long t = (long long)blk * (kThreads * R) + r * kThreads + tid;
+            if (t < a.T) a.part[(long long)row * a.T + t] = tot[r];
+        }
+    };
 
-    for (int it = 0; it < nt; ++it) {
+    for (int it = 0; it < nvis; ++it) {
         const int st = it & 1;
-        if (tid == 0 && it + 1 < nt) {  // buffer st^1 was released by the barrier that ended iteration it-1
+        if (tid == 0 && it + 1 < nvis) {  // buffer st^1 was released by the barrier that ended the previous visit
+            const int tn = tl + 1 == nt ? 0 : tl + 1;
             mbar_expect_tx(&full[st ^ 1], kTile * sizeof(Src4));
-            bulk_g2s(tile[st ^ 1], a.src + (tile0 + it + 1) * kTile, kTile * sizeof(Src4), &full[st ^ 1]);
+            bulk_g2s(tile[st ^ 1], a.src + (long long)tn * kTile, kTile * sizeof(Src4), &full[st ^ 1]);
+        }
+        const long long tb = (long long)b * (kThreads * R);
+        if (fresh) {
+            fresh = false;
+            // targets owned by this thread (tail threads recompute target T-1 and do not store)
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const long long t = min(tb + r * kThreads + tid, a.T - 1);
+                const double* p = a.tgt + (a.t_first + t) * a.tstride;
+                ox[r] = p[0]; oy[r] = p[1]; oz[r] = p[2];
+                tot[r] = 0.0;
+            }
         }
         mbar_wait(&full[st], (it >> 1) & 1);
         const Src4* __restrict__ s = tile[st];
-        const long long j0 = (tile0 + it) * kTile;
+        // self: target t is source self_offset + t.  Block-uniform test whether this tile holds any of
+        // the block's own sources; sj0 + (local target index) is then the in-tile index of "self".
+        const long long j0 = (long long)tl * kTile;
+        const long long self_lo = a.self_offset + tb, self_hi = a.self_offset + min(a.T, tb + (long long)kThreads * R);
         const bool tile_has_self = a.self_offset >= 0 && j0 < self_hi && j0 + kTile > self_lo;
-
-        for (int c = 0; c < c1 - c0; ++c) {
+        const int c_lo = it == 0 ? c_first : 0;
+        const int c_hi = it == nvis - 1 ? c_last : a.C;
+        for (int c = c_lo; c < c_hi; ++c) {
             const Cell cell = cells[c];
             double tx[R], ty[R], tz[R], acc[R];
 #pragma unroll
@@ -122,12 +165,16 @@ __global__ void __launch_bounds__(kThreads) near_sum_kernel(const NearArgs a) {
             }
             if (cell.central && tile_has_self) {
                 // masked path: the pair (t, j = self_offset + t) has r2 = 0; give it r2 = 1, q = 0
+                int sj[R];
+#pragma unroll
+                for (int r = 0; r < R; ++r)
+                    sj[r] = (int)max(-1LL, min((long long)kTile, a.self_offset + min(tb + r * kThreads + tid, a.T - 1) - j0));
                 for (int j = 0; j < kTile; ++j) {
                     const double2 xy = *reinterpret_cast<const double2*>(&s[j].x);
                     const double2 zq = *reinterpret_cast<const double2*>(&s[j].z);
 #pragma unroll
                     for (int r = 0; r < R; ++r) {
-                        const bool self = (j0 + j) == (a.self_offset + ti[r]);
+                        const bool self = j == sj[r];
                         pair<REFINE>(tx[r], ty[r], tz[r], self ? tx[r] + 1.0 : xy.x, self ? ty[r] : xy.y,
                                      self ? tz[r] : zq.x, self ? 0.0 : zq.y, acc[r]);
                     }
@@ -146,12 +193,12 @@ __global__ void __launch_bounds__(kThreads) near_sum_kernel(const NearArgs a) {
             for (int r = 0; r < R; ++r) tot[r] = fma(w, acc[r], tot[r]);
         }
         __syncthreads();  // everyone is done with tile[st] before it is refilled
+        if (++tl == nt) {   // next visit starts the next target block
+            store_block(b);
+            tl = 0; ++b; fresh = true;
+        }
     }
-#pragma unroll
-    for (int r = 0; r < R; ++r) {
-        const long long t = tb + r * kThreads + tid;
-        if (t < a.T) a.part[(long long)blockIdx.y * a.T + t] = tot[r];
-    }
+    if (!fresh) store_block(b);
 }
 
 struct NodeArgs {
@@ -161,46 +208,59 @@ struct NodeArgs {
     long long t_first;
     const Node8* nodes;  // padded to a multiple of kTile/2 with zero-strength records at kFar
     long long n_tiles;   // tiles of kTile/2 nodes (same 8 KB stage size)
-    int tiles_per_split; // blockIdx.y = split over node tiles
-    double* part;        // [gridDim.y][T]
+    long long units;     // U = ntb * n_tiles (the decomposition above with C = 1)
+    double* part;        // [part_rows][T]
 };
 
 // phi(t) = sum_j Q_j/rho - P_j.(t - R_j)/rho^3  = sum_j y (Q_j - (P_j.d) y^2),  y = 1/rho,
 // with the exact normal dipole P_j = D_j n_j (reading S9).  y by the cubic step (relative ~1e-19
 // before rounding).  3 DADD + 3 (r2) + 5 (rsqrt) + 3 (P.d) + DMUL (y^2) + DFMA + DFMA = 17 FP64 instructions.
 template <int R>
-__global__ void __launch_bounds__(kThreads) node_sum_kernel(const NodeArgs a) {
+__global__ void __launch_bounds__(kThreads, near_min_ctas(R)) node_sum_kernel(const NodeArgs a) {
     constexpr int kNT = kTile / 2;
     __shared__ __align__(128) Node8 tile[kStages][kNT];
     __shared__ __align__(8) uint64_t full[kStages];
     const int tid = threadIdx.x;
-    const long long tile0 = (long long)blockIdx.y * a.tiles_per_split;
-    const long long tile1 = min(a.n_tiles, tile0 + a.tiles_per_split);
-    const int nt = (int)(tile1 - tile0);
+    const int G = gridDim.x, k = blockIdx.x;
+    const long long V0 = unit_start(k, a.units, G), V1 = unit_start(k + 1, a.units, G) - 1;  // inclusive
+    if (V1 < V0) return;
     if (tid == 0) {
         for (int s = 0; s < kStages; ++s) mbar_init(&full[s], 1);
         mbar_fence_init();
     }
     __syncthreads();
-    if (tid == 0 && nt > 0) {
+    if (tid == 0) {
         mbar_expect_tx(&full[0], kNT * sizeof(Node8));
-        bulk_g2s(tile[0], a.nodes + tile0 * kNT, kNT * sizeof(Node8), &full[0]);
+        bulk_g2s(tile[0], a.nodes + (V0 % a.n_tiles) * kNT, kNT * sizeof(Node8), &full[0]);
     }
-    const long long tb = (long long)blockIdx.x * (kThreads * R);
     double tx[R], ty[R], tz[R], acc[R];
+    long long cur_b = -1;
+    auto store_block = [&](long long b) {
+        const int row = k - cta_of_unit(b * a.n_tiles, a.units, G);
 #pragma unroll
-    for (int r = 0; r < R; ++r) {
-        long long t = tb + r * kThreads + tid;
-        t = t < a.T ? t : a.T - 1;
-        const double* p = a.tgt + (a.t_first + t) * a.tstride;
-        tx[r] = p[0]; ty[r] = p[1]; tz[r] = p[2];
-        acc[r] = 0.0;
-    }
-    for (int it = 0; it < nt; ++it) {
-        const int st = it & 1;
-        if (tid == 0 && it + 1 < nt) {
+        for (int r = 0; r < R; ++r) {
+            const long long t = b * (kThreads * R) + r * kThreads + tid;
+            if (t < a.T) a.part[(long long)row * a.T + t] = acc[r];
+        }
+    };
+    for (long long v = V0; v <= V1; ++v) {
+        const int it = (int)(v - V0), st = it & 1;
+        const long long b = v / a.n_tiles;
+        if (tid == 0 && v < V1) {
             mbar_expect_tx(&full[st ^ 1], kNT * sizeof(Node8));
-            bulk_g2s(tile[st ^ 1], a.nodes + (tile0 + it + 1) * kNT, kNT * sizeof(Node8), &full[st ^ 1]);
+            bulk_g2s(tile[st ^ 1], a.nodes + ((v + 1) % a.n_tiles) * kNT, kNT * sizeof(Node8), &full[st ^ 1]);
+        }
+        if (b != cur_b) {
+            if (cur_b >= 0) store_block(cur_b);
+            cur_b = b;
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                long long t = b * (kThreads * R) + r * kThreads + tid;
+                t = t < a.T ? t : a.T - 1;
+                const double* p = a.tgt + (a.t_first + t) * a.tstride;
+                tx[r] = p[0]; ty[r] = p[1]; tz[r] = p[2];
+                acc[r] = 0.0;
+            }
         }
         mbar_wait(&full[st], (it >> 1) & 1);
         const Node8* __restrict__ s = tile[st];
@@ -222,11 +282,7 @@ __global__ void __launch_bounds__(kThreads) node_sum_kernel(const NodeArgs a) {
         }
         __syncthreads();
     }
-#pragma unroll
-    for (int r = 0; r < R; ++r) {
-        const long long t = tb + r * kThreads + tid;
-        if (t < a.T) a.part[(long long)blockIdx.y * a.T + t] = acc[r];
-    }
+    store_block(cur_b);
 }
 
 // ---- H1 pre-pass: centre the coordinates and pack (x,y,z,q); pad with q = 0 records ----------
@@ -263,17 +319,22 @@ __global__ void pack_sources_kernel(const double* __restrict__ xyz, const double
 }
 
 // ---- H7: phi = sum over partial rows (fixed order), U block partials --------------------------
-// part_b [nb][T], part_c [nc][T] (either may have 0 rows).  q read from the packed sources.
-__global__ void finish_phi_kernel(const double* __restrict__ part_b, int nb, const double* __restrict__ part_c,
-                                  int nc, long long T, const Src4* __restrict__ src, long long t_first,
-                                  double* __restrict__ phi, double* __restrict__ u_part /* [gridDim.x] or null */) {
+// The rows of a target block are those of the CTAs that worked on it, in CTA order (PartLayout).
+__device__ __forceinline__ double sum_part_rows(const PartLayout& L, long long t, long long T) {
+    if (!L.part) return 0.0;
+    const long long b = t / L.block_targets;
+    const int first = cta_of_unit(b * L.Ub, L.U, L.G), last = cta_of_unit((b + 1) * L.Ub - 1, L.U, L.G);
+    double s = 0.0;
+    for (int k = 0; k <= last - first; ++k) s += L.part[(long long)k * T + t];
+    return s;
+}
+__global__ void finish_phi_kernel(const PartLayout Lb, const PartLayout Lc, long long T,
+                                  const Src4* __restrict__ src, long long t_first, double* __restrict__ phi,
+                                  double* __restrict__ u_part /* [gridDim.x] or null */) {
     const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     double e = 0.0;
     if (t < T) {
-        double sb = 0.0, sc = 0.0;
-        for (int k = 0; k < nb; ++k) sb += part_b[(long long)k * T + t];
-        for (int k = 0; k < nc; ++k) sc += part_c[(long long)k * T + t];
-        const double v = sb + sc;
+        const double v = sum_part_rows(Lb, t, T) + sum_part_rows(Lc, t, T);
         phi[t] = v;
         if (src) e = src[t_first + t].q * v;
     }
