@@ -35,8 +35,9 @@ UNIT = "pairs/s"
 # Algorithmic work per pair, SURVEY.md 8(d) / DESIGN.md "Roofline": flops with add/mul = 1, fma = 2
 FLOPS_PAIR_CHARGE = 18.0      # 3 DADD + (DMUL + 2 DFMA) + cubic rsqrt refinement (2 DMUL + 3 DFMA) + DFMA
 FLOPS_PAIR_DIPOLE = 26.0      # + P.d (DMUL + 2 DFMA) + y^2 (DMUL) + DFMA
-# what near_sum_kernel<R, REFINE> executes per pair (FP64-pipe instructions, flops), DESIGN.md "rsqrt"
-EXEC_PAIR = {1: (10.0, 14.0), 2: (12.0, 18.0)}
+# what near_sum_kernel<R, REFINE> executes per pair (FP64-pipe instructions, flops), DESIGN.md 6.1/6.4:
+# (refine, all |q| equal) -> the uniform-|q| path drops the multiplication by q
+EXEC_PAIR = {(1, False): (10.0, 14.0), (2, False): (12.0, 18.0), (1, True): (9.0, 13.0), (2, True): (11.0, 17.0)}
 # FP64 peak derived from unit counts and clocks: SMs x 64 DFMA lanes x 2 x clock
 FP64_LANES_PER_SM = 64
 
@@ -311,9 +312,10 @@ def run_b200(args, w) -> dict:
     sm_max_mhz = float(peaks.get("sm_max_mhz") or clocks.get("sm_max_mhz") or 1965.0)
     peak_tf = sm_count * FP64_LANES_PER_SM * 2 * sm_max_mhz * 1e6 * 1e-12
     ach_tf = pc_rank["b"] * FLOPS_PAIR_CHARGE / (k_ms * 1e-3) * 1e-12 if k_ms > 0 else 0.0
-    ex_instr, ex_flops = EXEC_PAIR[refine]
+    uniform_q = bool(np.all(np.abs(w.q) == abs(w.q[0])))
+    ex_instr, ex_flops = EXEC_PAIR[(refine, uniform_q)]
     issue_peak = sm_count * FP64_LANES_PER_SM * sm_max_mhz * 1e6          # FP64-pipe thread-instructions/s
-    roofline = {"bound": "alu", "kernel": f"near_sum_kernel<R,{refine}> step (b)", "achieved": ach_tf, "peak": peak_tf,
+    roofline = {"bound": "alu", "kernel": f"near_sum_kernel<R,{refine}> step (b), {'uniform-|q|' if uniform_q else 'generic'} path", "achieved": ach_tf, "peak": peak_tf,
                 "unit": "TFLOP/s", "frac": ach_tf / peak_tf, "traffic": None,
                 "peak_source": f"derived: {sm_count} SMs x {FP64_LANES_PER_SM} FP64 lanes x 2 x {sm_max_mhz:.0f} MHz "
                                f"(no FP64 entry in MEASURED_PEAKS.json)",

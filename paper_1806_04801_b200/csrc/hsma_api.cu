@@ -68,11 +68,11 @@ static int resident_ctas(K kernel) {
     return per_sm * num_sm();
 }
 static int near_resident(int R, int refine) {
-    static int cache[3][2] = {{0, 0}, {0, 0}, {0, 0}};
-    const int i = R == 4 ? 2 : (R == 2 ? 1 : 0), j = refine == 1 ? 0 : 1;
+    static int cache[4][2] = {{0, 0}, {0, 0}, {0, 0}, {0, 0}};
+    const int i = R == 8 ? 3 : (R == 4 ? 2 : (R == 2 ? 1 : 0)), j = refine == 1 ? 0 : 1;
     if (!cache[i][j]) {
-        if (refine == 1) cache[i][j] = R == 4 ? resident_ctas(near_sum_kernel<4, 1>) : R == 2 ? resident_ctas(near_sum_kernel<2, 1>) : resident_ctas(near_sum_kernel<1, 1>);
-        else cache[i][j] = R == 4 ? resident_ctas(near_sum_kernel<4, 2>) : R == 2 ? resident_ctas(near_sum_kernel<2, 2>) : resident_ctas(near_sum_kernel<1, 2>);
+        if (refine == 1) cache[i][j] = R == 8 ? resident_ctas(near_sum_kernel<8, 1>) : R == 4 ? resident_ctas(near_sum_kernel<4, 1>) : R == 2 ? resident_ctas(near_sum_kernel<2, 1>) : resident_ctas(near_sum_kernel<1, 1>);
+        else cache[i][j] = R == 8 ? resident_ctas(near_sum_kernel<8, 2>) : R == 4 ? resident_ctas(near_sum_kernel<4, 2>) : R == 2 ? resident_ctas(near_sum_kernel<2, 2>) : resident_ctas(near_sum_kernel<1, 2>);
     }
     return cache[i][j];
 }
@@ -83,53 +83,71 @@ static int node_resident(int R) {
     return cache[i];
 }
 
-// The largest R in {4, 2, 1} that still leaves every resident CTA at least 4 units; R = 1 otherwise.
+// Targets per thread: the largest R in {Rmax, .., 2, 1} that (i) leaves every resident CTA at least 4 units
+// and (ii) wastes at most 6 % of its target slots on the padding of the last block; if none qualifies, the
+// R with the least padding among those that satisfy (i), else R = 1.
 template <class Resident>
-static Launch choose_launch(long long T, long long units_per_block, Resident resident) {
-    Launch L;
-    for (int R : {4, 2, 1}) {
+static Launch choose_launch(long long T, long long units_per_block, int Rmax, Resident resident) {
+    auto shape = [&](int R) {
+        Launch L;
         L.R = R;
         L.ntb = (int)((T + (long long)kThreads * R - 1) / ((long long)kThreads * R));
         L.Ub = units_per_block;
         L.U = L.ntb * L.Ub;
-        const int res = resident(R);
-        L.G = (int)std::min<long long>(res, L.U);
-        if (L.U >= 4LL * res) break;
+        L.G = (int)std::min<long long>(resident(R), L.U);
+        L.rows = part_rows(L.U, L.Ub, L.G);
+        return L;
+    };
+    int best = 1;
+    double best_fill = 0.0;
+    for (int R = Rmax; R >= 1; R /= 2) {
+        const Launch L = shape(R);
+        if (R > 1 && L.U < 4LL * resident(R)) continue;
+        const double fill = (double)T / ((double)L.ntb * kThreads * R);
+        if (fill >= 0.94) { best = R; break; }
+        if (fill > best_fill + 1e-9) { best_fill = fill; best = R; }
     }
-    L.rows = part_rows(L.U, L.Ub, L.G);
-    return L;
+    return shape(best);
 }
 
-// part must hold L.rows * T doubles
-static void launch_near(const Launch& L, const double* tgt, int tstride, long long T, long long t_first, const Src4* src,
-                        long long n_tiles, const Cell* cells, int C, long long self_offset, int refine, double* part,
+// The packed sources of one evaluate (pack_sources_kernel) as the pair kernels need them.
+struct Packed {
+    const Src4* src; long long n_src, n_tiles; const int* tile_np; const int* slot_of; const QInfo* qinfo;
+};
+
+// part must hold L.rows * T doubles.  tgt_index: null, or the row of each target inside tgt.
+static void launch_near(const Launch& L, const double* tgt, int tstride, const int* tgt_index, long long T, long long t_first,
+                        const Packed& P, const Cell* cells, int C, long long self_offset, int refine, double* part,
                         cudaStream_t st) {
     NearArgs a;
-    a.tgt = tgt; a.tstride = tstride; a.T = T; a.t_first = t_first; a.src = src; a.n_tiles = n_tiles;
+    a.tgt = tgt; a.tstride = tstride; a.tgt_index = tgt_index; a.T = T; a.t_first = t_first;
+    a.src = P.src; a.n_src = P.n_src; a.n_tiles = P.n_tiles; a.tile_np = P.tile_np; a.slot_of = P.slot_of; a.qinfo = P.qinfo;
     a.cells = cells; a.C = C; a.units = L.U; a.self_offset = self_offset;
     a.scale = refine == 1 ? 0.5 : 1.0; a.part = part;
     if (refine == 1) {
-        if (L.R == 4) near_sum_kernel<4, 1><<<L.G, kThreads, 0, st>>>(a);
+        if (L.R == 8) near_sum_kernel<8, 1><<<L.G, kThreads, 0, st>>>(a);
+        else if (L.R == 4) near_sum_kernel<4, 1><<<L.G, kThreads, 0, st>>>(a);
         else if (L.R == 2) near_sum_kernel<2, 1><<<L.G, kThreads, 0, st>>>(a);
         else near_sum_kernel<1, 1><<<L.G, kThreads, 0, st>>>(a);
     } else {
-        if (L.R == 4) near_sum_kernel<4, 2><<<L.G, kThreads, 0, st>>>(a);
+        if (L.R == 8) near_sum_kernel<8, 2><<<L.G, kThreads, 0, st>>>(a);
+        else if (L.R == 4) near_sum_kernel<4, 2><<<L.G, kThreads, 0, st>>>(a);
         else if (L.R == 2) near_sum_kernel<2, 2><<<L.G, kThreads, 0, st>>>(a);
         else near_sum_kernel<1, 2><<<L.G, kThreads, 0, st>>>(a);
     }
     HSMA_COUNT_LAUNCH();
 }
 static Launch choose_near(long long T, long long n_tiles, int C, int refine) {
-    return choose_launch(T, n_tiles * C, [refine](int R) { return near_resident(R, refine); });
+    return choose_launch(T, n_tiles * C, 8, [refine](int R) { return near_resident(R, refine); });
 }
 
 static Launch choose_node(long long T, long long n_tiles) {
-    return choose_launch(T, n_tiles, [](int R) { return node_resident(R); });
+    return choose_launch(T, n_tiles, 4, [](int R) { return node_resident(R); });
 }
-static void launch_node(const Launch& L, const double* tgt, int tstride, long long T, long long t_first,
+static void launch_node(const Launch& L, const double* tgt, int tstride, const int* tgt_index, long long T, long long t_first,
                         const Node8* nodes, long long n_tiles, double* part, cudaStream_t st) {
     NodeArgs a;
-    a.tgt = tgt; a.tstride = tstride; a.T = T; a.t_first = t_first; a.nodes = nodes; a.n_tiles = n_tiles;
+    a.tgt = tgt; a.tstride = tstride; a.tgt_index = tgt_index; a.T = T; a.t_first = t_first; a.nodes = nodes; a.n_tiles = n_tiles;
     a.units = L.U; a.part = part;
     if (L.R == 4) node_sum_kernel<4><<<L.G, kThreads, 0, st>>>(a);
     else if (L.R == 2) node_sum_kernel<2><<<L.G, kThreads, 0, st>>>(a);
@@ -162,6 +180,8 @@ struct hsma_plan {
     int* flags = nullptr;        // [0] rank deficient, [1] not neutral
     // scratch grown to the largest N seen
     DevBuf<Src4> src;
+    DevBuf<int> slot_of, tile_np;
+    QInfo* qinfo = nullptr;
     DevBuf<double> part_a, part_b, part_c, red, xyz_in, q_in, phi_dev;
     long long last_launches = 0;
     hsma_status sticky = HSMA_OK;
@@ -180,7 +200,8 @@ static void plan_free(hsma_plan* p) {
     void* ptrs[] = {p->cells_near, p->chk, p->nrm, p->wq, p->nodes, p->Fm, p->tau, p->Qm, p->Rm,
                     p->pc, p->rhs, p->cvec, p->A_full, p->scalars, p->flags};
     for (void* q : ptrs) if (q) cudaFree(q);
-    p->src.release(); p->part_a.release(); p->part_b.release(); p->part_c.release(); p->red.release();
+    p->src.release(); p->slot_of.release(); p->tile_np.release(); if (p->qinfo) cudaFree(p->qinfo);
+    p->part_a.release(); p->part_b.release(); p->part_c.release(); p->red.release();
     p->xyz_in.release(); p->q_in.release(); p->phi_dev.release();
     for (cudaEvent_t e : p->ev) if (e) cudaEventDestroy(e);
     delete p;
@@ -293,6 +314,7 @@ extern "C" hsma_status hsma_plan_create_ex(const hsma_plan_desc* desc, void* cud
     PCU(cudaMalloc(&p->A_full, d.p * d.p * sizeof(double)));
     PCU(cudaMalloc(&p->scalars, 8 * sizeof(double)));
     PCU(cudaMalloc(&p->flags, 4 * sizeof(int)));
+    PCU(cudaMalloc(&p->qinfo, sizeof(QInfo)));
     PCU(cudaMemsetAsync(p->flags, 0, 4 * sizeof(int), st));
     PCU(cudaMemsetAsync(p->A_full, 0, d.p * d.p * sizeof(double), st));
     build_fit_matrix_kernel<<<(p->rows + 127) / 128, 128, 0, st>>>(p->chk, p->rows, p->pairs ? 1 : 0, d.p, 1.0 / R0, p->Fm);
@@ -336,10 +358,6 @@ extern "C" hsma_status hsma_plan_destroy(hsma_plan* plan) {
 // evaluate (update step; Table I)
 // ------------------------------------------------------------------------------------------------
 namespace hsma {
-// flags[1] = 1 if |sum q| > 1e-12 sum |q|  (reading S17); s = {sum q, sum |q|}
-__global__ void neutrality_kernel(const double* __restrict__ s, int* __restrict__ flags) {
-    if (fabs(s[0]) > 1e-12 * s[1]) flags[1] = 1;
-}
 __global__ void unpack_nodes_kernel(const Node8* __restrict__ n, int M, double* __restrict__ Q, double* __restrict__ P) {
     const int j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= M) return;
@@ -363,28 +381,26 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
 #define MARK(i) do { if (p->timing) cudaEventRecord(p->ev[i], st); } while (0)
     p->ev_valid = false;
     MARK(0);
-    // H1 pre-pass: centre + pack, neutrality flag
-    const int pb = 256;
-    const long long pack_blocks = (Npad + pb - 1) / pb;
-    if (p->src.reserve((size_t)Npad) != cudaSuccess) return HSMA_ERR_ALLOC;
-    if (p->red.reserve((size_t)std::max(2 * pack_blocks, (t1 - t0 + 255) / 256 + 1)) != cudaSuccess) return HSMA_ERR_ALLOC;
-    pack_sources_kernel<<<(unsigned)pack_blocks, pb, 0, st>>>(xyz, q, N, Npad, p->half[0], p->half[1], p->half[2],
-                                                             p->src.p, p->need_neutral ? p->red.p : nullptr);
-    HSMA_COUNT_LAUNCH();
-    if (p->need_neutral) {
-        reduce_rows_kernel<<<1, 1024, 0, st>>>(p->red.p, pack_blocks, 2, 2, 1.0, p->scalars + 2);
-        neutrality_kernel<<<1, 1, 0, st>>>(p->scalars + 2, p->flags);
-        HSMA_COUNT_LAUNCH(); HSMA_COUNT_LAUNCH();
-    }
+    // H1 pre-pass: centre + pack + in-tile sign sort; charge statistics (neutrality flag, uniform |q|)
+    if (N > 2000000000LL) return HSMA_ERR_INVALID_ARG;  // packed indices are 32-bit
+    if (p->src.reserve((size_t)Npad) != cudaSuccess || p->slot_of.reserve((size_t)N) != cudaSuccess ||
+        p->tile_np.reserve((size_t)n_tiles) != cudaSuccess)
+        return HSMA_ERR_ALLOC;
+    if (p->red.reserve((size_t)std::max(4 * n_tiles, (t1 - t0 + 255) / 256 + 1)) != cudaSuccess) return HSMA_ERR_ALLOC;
+    pack_sources_kernel<<<(unsigned)n_tiles, kTile, 0, st>>>(xyz, q, N, p->half[0], p->half[1], p->half[2], p->src.p,
+                                                           p->slot_of.p, p->tile_np.p, p->red.p);
+    charge_stats_kernel<<<1, 1024, 0, st>>>(p->red.p, n_tiles, p->need_neutral ? 1 : 0, p->scalars + 2, p->qinfo, p->flags);
+    HSMA_COUNT_LAUNCH(); HSMA_COUNT_LAUNCH();
+    const Packed P{p->src.p, N, n_tiles, p->tile_np.p, p->slot_of.p, p->qinfo};
 
     // H2 (a): Phi_in (or the far-cell data) at the monitoring points -> pc [Kt]
     {
         const Launch s = choose_near(p->Kt, n_tiles, p->C_rhs, 2);
         if (p->part_a.reserve((size_t)s.rows * p->Kt) != cudaSuccess) return HSMA_ERR_ALLOC;
         MARK(1);
-        launch_near(s, p->chk, 3, p->Kt, 0, p->src.p, n_tiles, p->cells_rhs, p->C_rhs, -1, 2, p->part_a.p, st);  // (a) always cubic: it feeds the fit
+        launch_near(s, p->chk, 3, nullptr, p->Kt, 0, P, p->cells_rhs, p->C_rhs, -1, 2, p->part_a.p, st);  // (a) always cubic: it feeds the fit
         MARK(2);
-        finish_phi_kernel<<<(p->Kt + 255) / 256, 256, 0, st>>>(s.layout(p->part_a.p), PartLayout{nullptr, 1, 1, 1, 1}, p->Kt, nullptr, 0, p->pc, nullptr);
+        finish_phi_kernel<<<(p->Kt + 255) / 256, 256, 0, st>>>(s.layout(p->part_a.p), PartLayout{nullptr, 1, 1, 1, 1}, p->Kt, nullptr, nullptr, 0, p->pc, nullptr);
         HSMA_COUNT_LAUNCH();
     }
     // H3: least squares, Eq.(7)
@@ -406,15 +422,15 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
         const Launch sc = choose_node(T, p->node_tiles);
         if (p->part_c.reserve((size_t)sc.rows * T) != cudaSuccess) return HSMA_ERR_ALLOC;
         MARK(3);
-        launch_near(sb, reinterpret_cast<const double*>(p->src.p), 4, T, t0, p->src.p, n_tiles, p->cells_near, p->C_near,
+        launch_near(sb, reinterpret_cast<const double*>(p->src.p), 4, p->slot_of.p, T, t0, P, p->cells_near, p->C_near,
                     t0, refine, p->part_b.p, st);
         MARK(4);
         // H6 (c): sphere nodes, charge + dipole
-        launch_node(sc, reinterpret_cast<const double*>(p->src.p), 4, T, t0, p->nodes, p->node_tiles, p->part_c.p, st);
+        launch_node(sc, reinterpret_cast<const double*>(p->src.p), 4, p->slot_of.p, T, t0, p->nodes, p->node_tiles, p->part_c.p, st);
         MARK(5);
         // H7: phi and U
         const long long fb = (T + 255) / 256;
-        finish_phi_kernel<<<(unsigned)fb, 256, 0, st>>>(sb.layout(p->part_b.p), sc.layout(p->part_c.p), T, p->src.p, t0, phi_out,
+        finish_phi_kernel<<<(unsigned)fb, 256, 0, st>>>(sb.layout(p->part_b.p), sc.layout(p->part_c.p), T, p->src.p, p->slot_of.p, t0, phi_out,
                                                         energy_out ? p->red.p : nullptr);
         HSMA_COUNT_LAUNCH();
         if (energy_out) {
@@ -544,15 +560,6 @@ extern "C" hsma_status hsma_get_fit_residual(hsma_plan* p, double* rms_out) {
 }
 
 namespace hsma {
-__global__ void pack_plain_kernel(const double* __restrict__ xyz, const double* __restrict__ q, long long N,
-                                  long long Npad, Src4* __restrict__ out) {
-    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= Npad) return;
-    Src4 s;
-    if (i < N) { s.x = xyz[3 * i]; s.y = xyz[3 * i + 1]; s.z = xyz[3 * i + 2]; s.q = q[i]; }
-    else { s.x = s.y = s.z = kFar; s.q = 0.0; }
-    out[i] = s;
-}
 __global__ void pack_nodes_kernel(const double* __restrict__ R, const double* __restrict__ Q, const double* __restrict__ P,
                                   long long M, long long Mpad, Node8* __restrict__ out) {
     const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -581,23 +588,30 @@ extern "C" hsma_status hsma_direct_sum(const double* tgt, long long T, const dou
     }
     const long long n_tiles = (N + kTile - 1) / kTile, Npad = n_tiles * kTile;
     const Launch s = choose_near(T, n_tiles, C, refine);
-    Cell* dc = nullptr; Src4* ds = nullptr; double* part = nullptr;
+    if (N > 2000000000LL) return HSMA_ERR_INVALID_ARG;
+    Cell* dc = nullptr; Src4* ds = nullptr; double* part = nullptr; double* stats = nullptr; int* idx = nullptr;
+    QInfo* qi = nullptr; int* flags = nullptr;
     hsma_status rc = HSMA_OK;
+    // idx: slot_of [N] then tile_np [n_tiles]; stats: per tile [4] then scal [2]
     if (cudaMalloc(&dc, C * sizeof(Cell)) != cudaSuccess || cudaMalloc(&ds, Npad * sizeof(Src4)) != cudaSuccess ||
-        cudaMalloc(&part, (size_t)s.rows * T * sizeof(double)) != cudaSuccess) {
+        cudaMalloc(&part, (size_t)s.rows * T * sizeof(double)) != cudaSuccess ||
+        cudaMalloc(&stats, (size_t)(4 * n_tiles + 2) * sizeof(double)) != cudaSuccess ||
+        cudaMalloc(&idx, (size_t)(N + n_tiles) * sizeof(int)) != cudaSuccess || cudaMalloc(&qi, sizeof(QInfo)) != cudaSuccess ||
+        cudaMalloc(&flags, 4 * sizeof(int)) != cudaSuccess) {
         rc = HSMA_ERR_ALLOC;
     } else {
         cudaMemcpyAsync(dc, cells.data(), C * sizeof(Cell), cudaMemcpyHostToDevice, st);
-        pack_plain_kernel<<<(unsigned)((Npad + 255) / 256), 256, 0, st>>>(src, q, N, Npad, ds);
-        HSMA_COUNT_LAUNCH();
-        launch_near(s, tgt, 3, T, 0, ds, n_tiles, dc, C, central_cell >= 0 ? self_offset : -1, refine, part, st);
-        finish_phi_kernel<<<(unsigned)((T + 255) / 256), 256, 0, st>>>(s.layout(part), PartLayout{nullptr, 1, 1, 1, 1}, T, nullptr, 0, phi_out, nullptr);
+        pack_sources_kernel<<<(unsigned)n_tiles, kTile, 0, st>>>(src, q, N, 0.0, 0.0, 0.0, ds, idx, idx + N, stats);
+        charge_stats_kernel<<<1, 1024, 0, st>>>(stats, n_tiles, 0, stats + 4 * n_tiles, qi, flags);
+        HSMA_COUNT_LAUNCH(); HSMA_COUNT_LAUNCH();
+        const Packed P{ds, N, n_tiles, idx + N, idx, qi};
+        launch_near(s, tgt, 3, nullptr, T, 0, P, dc, C, central_cell >= 0 ? self_offset : -1, refine, part, st);
+        finish_phi_kernel<<<(unsigned)((T + 255) / 256), 256, 0, st>>>(s.layout(part), PartLayout{nullptr, 1, 1, 1, 1}, T, nullptr, nullptr, 0, phi_out, nullptr);
         HSMA_COUNT_LAUNCH();
         if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) rc = HSMA_ERR_CUDA;
     }
-    if (dc) cudaFree(dc);
-    if (ds) cudaFree(ds);
-    if (part) cudaFree(part);
+    for (void* ptr : {(void*)dc, (void*)ds, (void*)part, (void*)stats, (void*)idx, (void*)qi, (void*)flags})
+        if (ptr) cudaFree(ptr);
     return rc;
 }
 
@@ -615,8 +629,8 @@ extern "C" hsma_status hsma_node_sum(const double* tgt, long long T, const doubl
     } else {
         pack_nodes_kernel<<<(unsigned)((Mpad + 255) / 256), 256, 0, st>>>(R, Q, P, M, Mpad, dn);
         HSMA_COUNT_LAUNCH();
-        launch_node(s, tgt, 3, T, 0, dn, n_tiles, part, st);
-        finish_phi_kernel<<<(unsigned)((T + 255) / 256), 256, 0, st>>>(PartLayout{nullptr, 1, 1, 1, 1}, s.layout(part), T, nullptr, 0, phi_out, nullptr);
+        launch_node(s, tgt, 3, nullptr, T, 0, dn, n_tiles, part, st);
+        finish_phi_kernel<<<(unsigned)((T + 255) / 256), 256, 0, st>>>(PartLayout{nullptr, 1, 1, 1, 1}, s.layout(part), T, nullptr, nullptr, 0, phi_out, nullptr);
         HSMA_COUNT_LAUNCH();
         if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) rc = HSMA_ERR_CUDA;
     }

@@ -38,13 +38,20 @@ struct PartLayout {      // how finish_phi_kernel finds the partial rows of one 
     int block_targets;   // targets per block (kThreads * R)
 };
 
+struct QInfo { double qmag; int uniform; int pad; };  // all |q| equal to qmag (charge_stats_kernel)
+
 struct NearArgs {
     const double* tgt;   // targets, `tstride` doubles apart (3 = xyz rows, 4 = packed Src4 rows)
     int tstride;
     long long T;         // number of targets
-    long long t_first;   // index of the first target inside tgt (row offset)
-    const Src4* src;     // packed, padded to a multiple of kTile with q = 0 records at kFar
+    long long t_first;   // target t is row tgt_index[t_first + t] of tgt (row t_first + t if tgt_index is null)
+    const int* tgt_index;
+    const Src4* src;     // packed by pack_sources_kernel: tiles of kTile records, sign-sorted, padded with q = 0 at kFar
+    long long n_src;     // valid sources
     long long n_tiles;   // padded source count / kTile
+    const int* tile_np;  // [n_tiles] sources with q >= 0 at the front of each tile
+    const int* slot_of;  // [n_src] packed index of source i (needed only for the self exclusion)
+    const QInfo* qinfo;  // null: always multiply by q
     const Cell* cells;   // [C]
     int C;
     long long units;     // U = ntb * n_tiles * C
@@ -82,7 +89,27 @@ __device__ __forceinline__ void pair(double tx, double ty, double tz, double sx,
     }
 }
 
-constexpr int near_min_ctas(int R) { return R == 4 ? 2 : (R == 2 ? 3 : 4); }
+// The same pair with the charge factored out (all |q| equal, tiles sign-sorted): acc += y or acc -= y.
+//  REFINE 1: 3 DADD + DMUL + 2 DFMA + MUFU + DMUL + DFMA + DFMA = 9 FP64-pipe instructions (the negation is
+//  an operand modifier); REFINE 2: 11.
+template <int REFINE, bool NEG>
+__device__ __forceinline__ void pair_unit(double tx, double ty, double tz, double sx, double sy, double sz, double& acc) {
+    const double dx = tx - sx, dy = ty - sy, dz = tz - sz;
+    const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+    const double y0 = rsqrt_seed(r2);
+    const double t = y0 * y0;
+    if (REFINE == 1) {
+        const double g = fma(-r2, t, kNewton3);
+        acc = NEG ? fma(-y0, g, acc) : fma(y0, g, acc);
+    } else {
+        const double e = fma(-r2, t, 1.0);
+        const double h = fma(e, 0.375, 0.5);
+        const double k = fma(e, h, 1.0);
+        acc = NEG ? fma(-y0, k, acc) : fma(y0, k, acc);
+    }
+}
+
+constexpr int near_min_ctas(int R) { return R >= 8 ? 1 : (R == 4 ? 2 : (R == 2 ? 3 : 4)); }
 
 template <int R, int REFINE>
 __global__ void __launch_bounds__(kThreads, near_min_ctas(R)) near_sum_kernel(const NearArgs a) {
@@ -90,6 +117,7 @@ __global__ void __launch_bounds__(kThreads, near_min_ctas(R)) near_sum_kernel(co
     __shared__ __align__(8) uint64_t full[kStages];
     __shared__ Cell cells[kMaxCells];
 
+    constexpr int kUnroll = R >= 4 ? 2 : 4;  // sources per unrolled body (measured best on B200)
     const int tid = threadIdx.x;
     const int G = gridDim.x, k = blockIdx.x;
     const long long u0 = unit_start(k, a.units, G), u1 = unit_start(k + 1, a.units, G);
@@ -107,6 +135,8 @@ __global__ void __launch_bounds__(kThreads, near_min_ctas(R)) near_sum_kernel(co
         mbar_expect_tx(&full[0], kTile * sizeof(Src4));
         bulk_g2s(tile[0], a.src + (V0 % a.n_tiles) * kTile, kTile * sizeof(Src4), &full[0]);
     }
+    const bool uniform = a.qinfo != nullptr && a.qinfo->uniform != 0;
+    const double qmag = uniform ? a.qinfo->qmag : 1.0;
 
     double ox[R], oy[R], oz[R], tot[R];
     // visits are walked with 32-bit state: block b, tile tl inside the block
@@ -138,21 +168,25 @@ __global__ void __launch_bounds__(kThreads, near_min_ctas(R)) near_sum_kernel(co
             // targets owned by this thread (tail threads recompute target T-1 and do not store)
 #pragma unroll
             for (int r = 0; r < R; ++r) {
-                const long long t = min(tb + r * kThreads + tid, a.T - 1);
-                const double* p = a.tgt + (a.t_first + t) * a.tstride;
+                long long t = a.t_first + min(tb + r * kThreads + tid, a.T - 1);
+                if (a.tgt_index) t = a.tgt_index[t];
+                const double* p = a.tgt + t * a.tstride;
                 ox[r] = p[0]; oy[r] = p[1]; oz[r] = p[2];
                 tot[r] = 0.0;
             }
         }
+        const int np = a.tile_np[tl];
+        const int nv = (int)min((long long)kTile, a.n_src - (long long)tl * kTile);
         mbar_wait(&full[st], (it >> 1) & 1);
         const Src4* __restrict__ s = tile[st];
-        // self: target t is source self_offset + t.  Block-uniform test whether this tile holds any of
-        // the block's own sources; sj0 + (local target index) is then the in-tile index of "self".
+        // self: target t is source self_offset + t (same tile after the in-tile sort).  Block-uniform test
+        // whether this tile holds any of the block's own sources.
         const long long j0 = (long long)tl * kTile;
         const long long self_lo = a.self_offset + tb, self_hi = a.self_offset + min(a.T, tb + (long long)kThreads * R);
         const bool tile_has_self = a.self_offset >= 0 && j0 < self_hi && j0 + kTile > self_lo;
         const int c_lo = it == 0 ? c_first : 0;
         const int c_hi = it == nvis - 1 ? c_last : a.C;
+
         for (int c = c_lo; c < c_hi; ++c) {
             const Cell cell = cells[c];
             double tx[R], ty[R], tz[R], acc[R];
@@ -163,12 +197,17 @@ __global__ void __launch_bounds__(kThreads, near_min_ctas(R)) near_sum_kernel(co
                 tz[r] = flip(oz[r] - cell.sz, cell.fz);
                 acc[r] = 0.0;
             }
+            double w = cell.w * a.scale;
             if (cell.central && tile_has_self) {
-                // masked path: the pair (t, j = self_offset + t) has r2 = 0; give it r2 = 1, q = 0
+                // masked path: the pair (t, j = slot of source self_offset + t) has r2 = 0; give it r2 = 1, q = 0
                 int sj[R];
 #pragma unroll
-                for (int r = 0; r < R; ++r)
-                    sj[r] = (int)max(-1LL, min((long long)kTile, a.self_offset + min(tb + r * kThreads + tid, a.T - 1) - j0));
+                for (int r = 0; r < R; ++r) {
+                    const long long i = a.self_offset + min(tb + r * kThreads + tid, a.T - 1);
+                    const long long slot = a.slot_of ? (long long)a.slot_of[i] : i;
+                    sj[r] = (int)max(-1LL, min((long long)kTile, slot - j0));
+                }
+#pragma unroll 1
                 for (int j = 0; j < kTile; ++j) {
                     const double2 xy = *reinterpret_cast<const double2*>(&s[j].x);
                     const double2 zq = *reinterpret_cast<const double2*>(&s[j].z);
@@ -179,8 +218,24 @@ __global__ void __launch_bounds__(kThreads, near_min_ctas(R)) near_sum_kernel(co
                                      self ? tz[r] : zq.x, self ? 0.0 : zq.y, acc[r]);
                     }
                 }
+            } else if (uniform) {
+                w *= qmag;
+#pragma unroll kUnroll
+                for (int j = 0; j < np; ++j) {
+                    const double2 xy = *reinterpret_cast<const double2*>(&s[j].x);
+                    const double sz = s[j].z;
+#pragma unroll
+                    for (int r = 0; r < R; ++r) pair_unit<REFINE, false>(tx[r], ty[r], tz[r], xy.x, xy.y, sz, acc[r]);
+                }
+#pragma unroll kUnroll
+                for (int j = np; j < nv; ++j) {
+                    const double2 xy = *reinterpret_cast<const double2*>(&s[j].x);
+                    const double sz = s[j].z;
+#pragma unroll
+                    for (int r = 0; r < R; ++r) pair_unit<REFINE, true>(tx[r], ty[r], tz[r], xy.x, xy.y, sz, acc[r]);
+                }
             } else {
-#pragma unroll 4
+#pragma unroll kUnroll
                 for (int j = 0; j < kTile; ++j) {
                     const double2 xy = *reinterpret_cast<const double2*>(&s[j].x);
                     const double2 zq = *reinterpret_cast<const double2*>(&s[j].z);
@@ -188,7 +243,6 @@ __global__ void __launch_bounds__(kThreads, near_min_ctas(R)) near_sum_kernel(co
                     for (int r = 0; r < R; ++r) pair<REFINE>(tx[r], ty[r], tz[r], xy.x, xy.y, zq.x, zq.y, acc[r]);
                 }
             }
-            const double w = cell.w * a.scale;
 #pragma unroll
             for (int r = 0; r < R; ++r) tot[r] = fma(w, acc[r], tot[r]);
         }
@@ -205,7 +259,8 @@ struct NodeArgs {
     const double* tgt;
     int tstride;
     long long T;
-    long long t_first;
+    long long t_first;   // target t is row tgt_index[t_first + t] of tgt (row t_first + t if tgt_index is null)
+    const int* tgt_index;
     const Node8* nodes;  // padded to a multiple of kTile/2 with zero-strength records at kFar
     long long n_tiles;   // tiles of kTile/2 nodes (same 8 KB stage size)
     long long units;     // U = ntb * n_tiles (the decomposition above with C = 1)
@@ -256,8 +311,9 @@ __global__ void __launch_bounds__(kThreads, near_min_ctas(R)) node_sum_kernel(co
 #pragma unroll
             for (int r = 0; r < R; ++r) {
                 long long t = b * (kThreads * R) + r * kThreads + tid;
-                t = t < a.T ? t : a.T - 1;
-                const double* p = a.tgt + (a.t_first + t) * a.tstride;
+                t = a.t_first + (t < a.T ? t : a.T - 1);
+                if (a.tgt_index) t = a.tgt_index[t];
+                const double* p = a.tgt + t * a.tstride;
                 tx[r] = p[0]; ty[r] = p[1]; tz[r] = p[2];
                 acc[r] = 0.0;
             }
@@ -285,36 +341,82 @@ __global__ void __launch_bounds__(kThreads, near_min_ctas(R)) node_sum_kernel(co
     store_block(cur_b);
 }
 
-// ---- H1 pre-pass: centre the coordinates and pack (x,y,z,q); pad with q = 0 records ----------
-// Also accumulates sum q and sum |q| per block for the neutrality check (reading S17).
-__global__ void pack_sources_kernel(const double* __restrict__ xyz, const double* __restrict__ q, long long N,
-                                    long long Npad, double hx, double hy, double hz, Src4* __restrict__ out,
-                                    double* __restrict__ qsum_part /* [gridDim.x][2] or null */) {
-    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    double qi = 0.0;
-    if (i < Npad) {
-        Src4 s;
-        if (i < N) {
-            s.x = xyz[3 * i] - hx; s.y = xyz[3 * i + 1] - hy; s.z = xyz[3 * i + 2] - hz; s.q = q[i];
-            qi = s.q;
-        } else {
-            s.x = kFar; s.y = kFar; s.z = kFar; s.q = 0.0;
-        }
-        out[i] = s;
+// ---- H1 pre-pass: centre the coordinates, pack (x,y,z,q) and sort each tile by the sign of q ----
+// One block = one tile of kTile sources.  Inside a tile the records are stably partitioned: the n_pos
+// sources with q >= 0 first, then the negative ones (tile_np[tile] = n_pos); pads (q = 0 at kFar) stay
+// behind the valid records.  slot_of[i] = index of source i in the packed array (same tile, so the
+// "does this tile hold my own sources" test of the self exclusion is unchanged).  With all |q| equal
+// (QInfo.uniform, found by charge_stats_kernel) the sum kernels then never multiply by q: they add
+// over the positive part, subtract over the negative part and scale the cell weight by |q|.
+// Also writes per block [sum q, sum |q|, min |q|, max |q|] for charge_stats_kernel.
+__global__ void __launch_bounds__(kTile) pack_sources_kernel(const double* __restrict__ xyz, const double* __restrict__ q,
+                                                           long long N, double hx, double hy, double hz,
+                                                           Src4* __restrict__ out, int* __restrict__ slot_of,
+                                                           int* __restrict__ tile_np, double* __restrict__ stats /* [gridDim.x][4] */) {
+    __shared__ int wpos[kTile / 32], wneg[kTile / 32];
+    __shared__ double sh[4][kTile / 32];
+    const int tid = threadIdx.x, w = tid >> 5, l = tid & 31;
+    const long long i = (long long)blockIdx.x * kTile + tid;
+    const bool valid = i < N;
+    Src4 s;
+    if (valid) { s.x = xyz[3 * i] - hx; s.y = xyz[3 * i + 1] - hy; s.z = xyz[3 * i + 2] - hz; s.q = q[i]; }
+    else { s.x = kFar; s.y = kFar; s.z = kFar; s.q = 0.0; }
+    const bool pos = valid && !(s.q < 0.0), neg = valid && s.q < 0.0;
+    const unsigned bp = __ballot_sync(0xffffffffu, pos), bn = __ballot_sync(0xffffffffu, neg);
+    if (l == 0) { wpos[w] = __popc(bp); wneg[w] = __popc(bn); }
+    // block statistics of q
+    double a = valid ? s.q : 0.0, b = fabs(a), mn = valid ? b : 1e300, mx = valid ? b : 0.0;
+    for (int o = 16; o; o >>= 1) {
+        a += __shfl_down_sync(0xffffffffu, a, o); b += __shfl_down_sync(0xffffffffu, b, o);
+        mn = fmin(mn, __shfl_down_sync(0xffffffffu, mn, o)); mx = fmax(mx, __shfl_down_sync(0xffffffffu, mx, o));
     }
-    if (qsum_part) {
-        __shared__ double sh[2][32];
-        double a = qi, b = fabs(qi);
-        for (int o = 16; o; o >>= 1) { a += __shfl_down_sync(0xffffffffu, a, o); b += __shfl_down_sync(0xffffffffu, b, o); }
-        const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
-        if (l == 0) { sh[0][w] = a; sh[1][w] = b; }
-        __syncthreads();
-        if (w == 0) {
-            const int nw = blockDim.x >> 5;
-            a = l < nw ? sh[0][l] : 0.0; b = l < nw ? sh[1][l] : 0.0;
-            for (int o = 16; o; o >>= 1) { a += __shfl_down_sync(0xffffffffu, a, o); b += __shfl_down_sync(0xffffffffu, b, o); }
-            if (l == 0) { qsum_part[2 * blockIdx.x] = a; qsum_part[2 * blockIdx.x + 1] = b; }
-        }
+    if (l == 0) { sh[0][w] = a; sh[1][w] = b; sh[2][w] = mn; sh[3][w] = mx; }
+    __syncthreads();
+    int before_pos = 0, before_neg = 0, npos = 0, nneg = 0;
+#pragma unroll
+    for (int k = 0; k < kTile / 32; ++k) {
+        if (k < w) { before_pos += wpos[k]; before_neg += wneg[k]; }
+        npos += wpos[k]; nneg += wneg[k];
+    }
+    const unsigned lower = (1u << l) - 1u;
+    int slot;
+    if (pos) slot = before_pos + __popc(bp & lower);
+    else if (neg) slot = npos + before_neg + __popc(bn & lower);
+    else slot = tid;  // pads: the valid sources of a tile are its first threads, so pads keep their place
+    out[(long long)blockIdx.x * kTile + slot] = s;
+    if (valid) slot_of[i] = (int)(blockIdx.x * kTile + slot);
+    if (tid == 0) {
+        tile_np[blockIdx.x] = npos;
+        double A = 0.0, B = 0.0, MN = 1e300, MX = 0.0;
+        for (int k = 0; k < kTile / 32; ++k) { A += sh[0][k]; B += sh[1][k]; MN = fmin(MN, sh[2][k]); MX = fmax(MX, sh[3][k]); }
+        stats[4 * blockIdx.x] = A; stats[4 * blockIdx.x + 1] = B; stats[4 * blockIdx.x + 2] = MN; stats[4 * blockIdx.x + 3] = MX;
+    }
+}
+
+// Single block: sum q, sum |q| -> scal[0..1]; neutrality flag (reading S17); QInfo (all |q| equal, bit for bit).
+__global__ void __launch_bounds__(1024) charge_stats_kernel(const double* __restrict__ stats, long long nblocks,
+                                                            int need_neutral, double* __restrict__ scal,
+                                                            QInfo* __restrict__ qi, int* __restrict__ flags) {
+    __shared__ double sh[4][32];
+    double a = 0.0, b = 0.0, mn = 1e300, mx = 0.0;
+    for (long long i = threadIdx.x; i < nblocks; i += blockDim.x) {
+        a += stats[4 * i]; b += stats[4 * i + 1]; mn = fmin(mn, stats[4 * i + 2]); mx = fmax(mx, stats[4 * i + 3]);
+    }
+    for (int o = 16; o; o >>= 1) {
+        a += __shfl_down_sync(0xffffffffu, a, o); b += __shfl_down_sync(0xffffffffu, b, o);
+        mn = fmin(mn, __shfl_down_sync(0xffffffffu, mn, o)); mx = fmax(mx, __shfl_down_sync(0xffffffffu, mx, o));
+    }
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    if (l == 0) { sh[0][w] = a; sh[1][w] = b; sh[2][w] = mn; sh[3][w] = mx; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        a = 0.0; b = 0.0; mn = 1e300; mx = 0.0;
+        for (int k = 0; k < (int)(blockDim.x >> 5); ++k) { a += sh[0][k]; b += sh[1][k]; mn = fmin(mn, sh[2][k]); mx = fmax(mx, sh[3][k]); }
+        scal[0] = a; scal[1] = b;
+        qi->uniform = (mn == mx) ? 1 : 0;
+        qi->qmag = mx;
+        qi->pad = 0;
+        if (need_neutral && fabs(a) > 1e-12 * b) flags[1] = 1;
     }
 }
 
@@ -329,14 +431,14 @@ __device__ __forceinline__ double sum_part_rows(const PartLayout& L, long long t
     return s;
 }
 __global__ void finish_phi_kernel(const PartLayout Lb, const PartLayout Lc, long long T,
-                                  const Src4* __restrict__ src, long long t_first, double* __restrict__ phi,
-                                  double* __restrict__ u_part /* [gridDim.x] or null */) {
+                                  const Src4* __restrict__ src, const int* __restrict__ slot_of, long long t_first,
+                                  double* __restrict__ phi, double* __restrict__ u_part /* [gridDim.x] or null */) {
     const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     double e = 0.0;
     if (t < T) {
         const double v = sum_part_rows(Lb, t, T) + sum_part_rows(Lc, t, T);
         phi[t] = v;
-        if (src) e = src[t_first + t].q * v;
+        if (src) e = src[slot_of[t_first + t]].q * v;
     }
     if (u_part) {
         __shared__ double sh[32];

@@ -82,6 +82,40 @@ def test_direct_sum_self_exclusion(H, refine, N, t0, T):
     assert rel_inf(out.cpu().numpy(), ref) < 1e-12
 
 
+@pytest.mark.parametrize("refine", [1, 2])
+@pytest.mark.parametrize("charges", ["pm0.7", "all_plus", "all_minus", "blocks", "one_odd", "with_zero"])
+@pytest.mark.parametrize("N,t0,T", [(1, 0, 1), (300, 0, 300), (1500, 700, 555), (4100, 0, 4100)])
+def test_direct_sum_charge_patterns(H, refine, charges, N, t0, T):
+    """The in-tile sign sort and the uniform-|q| path: equal magnitudes with every sign
+    pattern (all one sign, long runs, alternating), magnitudes equal except one, and zero charges; with
+    self exclusion across tile boundaries."""
+    import torch
+    rng = np.random.default_rng(11 + N)
+    src = rng.random((N, 3)) - 0.5
+    if charges == "pm0.7":
+        q = 0.7 * W.alternating_charges(N)
+    elif charges == "all_plus":
+        q = np.full(N, 1.25)
+    elif charges == "all_minus":
+        q = np.full(N, -3.0)
+    elif charges == "blocks":
+        q = np.where((np.arange(N) // 173) % 2 == 0, 2.0, -2.0)
+    elif charges == "one_odd":
+        q = W.alternating_charges(N)
+        q[N // 2] = 1.0000000000000002
+    else:
+        q = W.alternating_charges(N)
+        q[::7] = 0.0
+    cells = O.cell_table(W.BC_MIRROR_CAVITY, (1.0, 1.0, 1.0), (1, 1, 1), -1.0)
+    ref = O.near_sum(src[t0:t0 + T], src, q, cells, self_offset=t0)
+    out = torch.empty(T, dtype=torch.float64, device="cuda")
+    H.hsma_direct_sum(dev(src[t0:t0 + T]), dev(src), dev(q), cells.shift, cells.sign, cells.w, cells.central, t0,
+                      refine, out)
+    got = out.cpu().numpy()
+    assert np.all(np.isfinite(got))
+    assert np.max(np.abs(got - ref)) <= 1e-12 * max(np.max(np.abs(ref)), 1e-300)
+
+
 def test_rsqrt_refinement_error(H):
     """One source, one cell: phi = q / r.  Measures the relative error of the two refinements of the
     MUFU.RSQ64H seed over distances spanning 12 decades."""
@@ -162,6 +196,25 @@ def test_config_full(H, idx, refine):
     if idx == 1:
         M = O.madelung_constant(U, w.N, w.meta["a_nn"])
         assert abs(M - 1.7475645946) < 5e-8
+
+
+@pytest.mark.parametrize("refine", [1, 2])
+def test_config2_scaled_uniform_charges(H, refine):
+    """Config 2 with every charge multiplied by 0.37: still neutral, |q| uniform but not 1."""
+    w = W.config(2)
+    w = w.with_(q=0.37 * w.q)
+    r, phi, U, extra = run_both(H, w, rsqrt_refine=refine)
+    check_parity(r, phi, U, extra, f"cfg2 q*0.37 refine={refine}")
+
+
+@pytest.mark.parametrize("refine", [1, 2])
+def test_config3_random_magnitudes(H, refine):
+    """Config 3 (metallic cavity: no neutrality needed) with charges of random sign AND magnitude:
+    the generic multiply-by-q path through the whole evaluate."""
+    w = W.config(3)
+    q = np.random.default_rng(33).standard_normal(w.N)
+    r, phi, U, extra = run_both(H, w.with_(q=q), rsqrt_refine=refine)
+    check_parity(r, phi, U, extra, f"cfg3 random q refine={refine}")
 
 
 def test_paper_example2(H):
