@@ -67,12 +67,17 @@ static int resident_ctas(K kernel) {
     }
     return per_sm * num_sm();
 }
+// resident CTAs of near_sum_kernel<R, REFINE, *>: the smaller of the two loop forms (they share one launch shape)
+template <int R, int REFINE>
+static int near_resident_of() {
+    return std::min(resident_ctas(near_sum_kernel<R, REFINE, false>), resident_ctas(near_sum_kernel<R, REFINE, true>));
+}
 static int near_resident(int R, int refine) {
     static int cache[4][2] = {{0, 0}, {0, 0}, {0, 0}, {0, 0}};
     const int i = R == 8 ? 3 : (R == 4 ? 2 : (R == 2 ? 1 : 0)), j = refine == 1 ? 0 : 1;
     if (!cache[i][j]) {
-        if (refine == 1) cache[i][j] = R == 8 ? resident_ctas(near_sum_kernel<8, 1>) : R == 4 ? resident_ctas(near_sum_kernel<4, 1>) : R == 2 ? resident_ctas(near_sum_kernel<2, 1>) : resident_ctas(near_sum_kernel<1, 1>);
-        else cache[i][j] = R == 8 ? resident_ctas(near_sum_kernel<8, 2>) : R == 4 ? resident_ctas(near_sum_kernel<4, 2>) : R == 2 ? resident_ctas(near_sum_kernel<2, 2>) : resident_ctas(near_sum_kernel<1, 2>);
+        if (refine == 1) cache[i][j] = R == 8 ? near_resident_of<8, 1>() : R == 4 ? near_resident_of<4, 1>() : R == 2 ? near_resident_of<2, 1>() : near_resident_of<1, 1>();
+        else cache[i][j] = R == 8 ? near_resident_of<8, 2>() : R == 4 ? near_resident_of<4, 2>() : R == 2 ? near_resident_of<2, 2>() : near_resident_of<1, 2>();
     }
     return cache[i][j];
 }
@@ -115,6 +120,22 @@ struct Packed {
     const Src4* src; long long n_src, n_tiles; const int* tile_np; const int* slot_of; const QInfo* qinfo;
 };
 
+template <bool UNIFORM>
+static void launch_near_form(const Launch& L, int refine, const NearArgs& a, cudaStream_t st) {
+    if (refine == 1) {
+        if (L.R == 8) near_sum_kernel<8, 1, UNIFORM><<<L.G, kThreads, 0, st>>>(a);
+        else if (L.R == 4) near_sum_kernel<4, 1, UNIFORM><<<L.G, kThreads, 0, st>>>(a);
+        else if (L.R == 2) near_sum_kernel<2, 1, UNIFORM><<<L.G, kThreads, 0, st>>>(a);
+        else near_sum_kernel<1, 1, UNIFORM><<<L.G, kThreads, 0, st>>>(a);
+    } else {
+        if (L.R == 8) near_sum_kernel<8, 2, UNIFORM><<<L.G, kThreads, 0, st>>>(a);
+        else if (L.R == 4) near_sum_kernel<4, 2, UNIFORM><<<L.G, kThreads, 0, st>>>(a);
+        else if (L.R == 2) near_sum_kernel<2, 2, UNIFORM><<<L.G, kThreads, 0, st>>>(a);
+        else near_sum_kernel<1, 2, UNIFORM><<<L.G, kThreads, 0, st>>>(a);
+    }
+    HSMA_COUNT_LAUNCH();
+}
+
 // part must hold L.rows * T doubles.  tgt_index: null, or the row of each target inside tgt.
 static void launch_near(const Launch& L, const double* tgt, int tstride, const int* tgt_index, long long T, long long t_first,
                         const Packed& P, const Cell* cells, int C, long long self_offset, int refine, double* part,
@@ -124,18 +145,10 @@ static void launch_near(const Launch& L, const double* tgt, int tstride, const i
     a.src = P.src; a.n_src = P.n_src; a.n_tiles = P.n_tiles; a.tile_np = P.tile_np; a.slot_of = P.slot_of; a.qinfo = P.qinfo;
     a.cells = cells; a.C = C; a.units = L.U; a.self_offset = self_offset;
     a.scale = refine == 1 ? 0.5 : 1.0; a.part = part;
-    if (refine == 1) {
-        if (L.R == 8) near_sum_kernel<8, 1><<<L.G, kThreads, 0, st>>>(a);
-        else if (L.R == 4) near_sum_kernel<4, 1><<<L.G, kThreads, 0, st>>>(a);
-        else if (L.R == 2) near_sum_kernel<2, 1><<<L.G, kThreads, 0, st>>>(a);
-        else near_sum_kernel<1, 1><<<L.G, kThreads, 0, st>>>(a);
-    } else {
-        if (L.R == 8) near_sum_kernel<8, 2><<<L.G, kThreads, 0, st>>>(a);
-        else if (L.R == 4) near_sum_kernel<4, 2><<<L.G, kThreads, 0, st>>>(a);
-        else if (L.R == 2) near_sum_kernel<2, 2><<<L.G, kThreads, 0, st>>>(a);
-        else near_sum_kernel<1, 2><<<L.G, kThreads, 0, st>>>(a);
-    }
-    HSMA_COUNT_LAUNCH();
+    // generic form always; the uniform-|q| form too when the charge statistics are available (each returns at
+    // once unless QInfo.uniform selects it)
+    launch_near_form<false>(L, refine, a, st);
+    if (a.qinfo) launch_near_form<true>(L, refine, a, st);
 }
 static Launch choose_near(long long T, long long n_tiles, int C, int refine) {
     return choose_launch(T, n_tiles * C, 8, [refine](int R) { return near_resident(R, refine); });

@@ -111,13 +111,17 @@ __device__ __forceinline__ void pair_unit(double tx, double ty, double tz, doubl
 
 constexpr int near_min_ctas(int R) { return R >= 8 ? 1 : (R == 4 ? 2 : (R == 2 ? 3 : 4)); }
 
-template <int R, int REFINE>
+// UNIFORM selects the loop form at compile time; the host launches both instantiations and the one that does
+// not match the device-side flag QInfo.uniform returns at once (no host synchronisation to pick a kernel,
+// and each instantiation keeps only its own loops: fewer live registers, better schedules).
+template <int R, int REFINE, bool UNIFORM>
 __global__ void __launch_bounds__(kThreads, near_min_ctas(R)) near_sum_kernel(const NearArgs a) {
     __shared__ __align__(128) Src4 tile[kStages][kTile];
     __shared__ __align__(8) uint64_t full[kStages];
     __shared__ Cell cells[kMaxCells];
 
     constexpr int kUnroll = R >= 4 ? 2 : 4;  // sources per unrolled body (measured best on B200)
+    if ((a.qinfo != nullptr && a.qinfo->uniform != 0) != UNIFORM) return;
     const int tid = threadIdx.x;
     const int G = gridDim.x, k = blockIdx.x;
     const long long u0 = unit_start(k, a.units, G), u1 = unit_start(k + 1, a.units, G);
@@ -135,8 +139,7 @@ __global__ void __launch_bounds__(kThreads, near_min_ctas(R)) near_sum_kernel(co
         mbar_expect_tx(&full[0], kTile * sizeof(Src4));
         bulk_g2s(tile[0], a.src + (V0 % a.n_tiles) * kTile, kTile * sizeof(Src4), &full[0]);
     }
-    const bool uniform = a.qinfo != nullptr && a.qinfo->uniform != 0;
-    const double qmag = uniform ? a.qinfo->qmag : 1.0;
+    const double qmag = UNIFORM ? a.qinfo->qmag : 1.0;
 
     double ox[R], oy[R], oz[R], tot[R];
     // visits are walked with 32-bit state: block b, tile tl inside the block
@@ -218,7 +221,7 @@ __global__ void __launch_bounds__(kThreads, near_min_ctas(R)) near_sum_kernel(co
                                      self ? tz[r] : zq.x, self ? 0.0 : zq.y, acc[r]);
                     }
                 }
-            } else if (uniform) {
+            } else if (UNIFORM) {
                 w *= qmag;
 #pragma unroll kUnroll
                 for (int j = 0; j < np; ++j) {
