@@ -116,6 +116,73 @@ void oracle_node_sum(const double *tgt, long T, const double *R, const double *n
     }
 }
 
+/*
+ * Gradients with respect to the TARGET position (Eq.(9): the force on source i is
+ * -q_i grad Phi(r_i)); same arguments and conventions as the two sums above, out [T,3].
+ *   d/dt  q/|p - t|                      =  q (p - t)/|p - t|^3                      (p = image position)
+ *   d/dt [Q/rho - D n.(t-R)/rho^3]       = -Q d/rho^3 - D n/rho^3 + 3 D (n.d) d/rho^5,   d = t - R
+ */
+void oracle_near_grad(const double *tgt, long T, const double *src, const double *q, long N,
+                      const double *shift, const double *sign, const double *w, long C,
+                      long central_cell, long self_offset, double *grad)
+{
+#pragma omp parallel for schedule(dynamic, 1)
+    for (long t = 0; t < T; ++t) {
+        const double tx = tgt[3 * t], ty = tgt[3 * t + 1], tz = tgt[3 * t + 2];
+        long double gx = 0.0L, gy = 0.0L, gz = 0.0L;
+        for (long c = 0; c < C; ++c) {
+            const double ax = sign[3 * c], ay = sign[3 * c + 1], az = sign[3 * c + 2];
+            const double bx = shift[3 * c], by = shift[3 * c + 1], bz = shift[3 * c + 2];
+            const long skip = (c == central_cell && self_offset >= 0) ? self_offset + t : -1;
+            long double cx = 0.0L, cy = 0.0L, cz = 0.0L;
+            for (long j0 = 0; j0 < N; j0 += ORACLE_BLOCK) {
+                const long j1 = (j0 + ORACLE_BLOCK < N) ? j0 + ORACLE_BLOCK : N;
+                double sx = 0.0, sy = 0.0, sz = 0.0;
+                for (long j = j0; j < j1; ++j) {
+                    if (j == skip) continue;
+                    const double dx = (ax * src[3 * j] + bx) - tx;
+                    const double dy = (ay * src[3 * j + 1] + by) - ty;
+                    const double dz = (az * src[3 * j + 2] + bz) - tz;
+                    const double r2 = dx * dx + dy * dy + dz * dz;
+                    const double f = q[j] / (r2 * sqrt(r2));
+                    sx += f * dx; sy += f * dy; sz += f * dz;
+                }
+                cx += (long double)sx; cy += (long double)sy; cz += (long double)sz;
+            }
+            gx += (long double)w[c] * cx; gy += (long double)w[c] * cy; gz += (long double)w[c] * cz;
+        }
+        grad[3 * t] = (double)gx; grad[3 * t + 1] = (double)gy; grad[3 * t + 2] = (double)gz;
+    }
+}
+
+void oracle_node_grad(const double *tgt, long T, const double *R, const double *nrm,
+                      const double *Q, const double *D, long M, double *grad)
+{
+#pragma omp parallel for schedule(static)
+    for (long t = 0; t < T; ++t) {
+        const double tx = tgt[3 * t], ty = tgt[3 * t + 1], tz = tgt[3 * t + 2];
+        long double gx = 0.0L, gy = 0.0L, gz = 0.0L;
+        for (long j0 = 0; j0 < M; j0 += ORACLE_BLOCK) {
+            const long j1 = (j0 + ORACLE_BLOCK < M) ? j0 + ORACLE_BLOCK : M;
+            double sx = 0.0, sy = 0.0, sz = 0.0;
+            for (long j = j0; j < j1; ++j) {
+                const double dx = tx - R[3 * j], dy = ty - R[3 * j + 1], dz = tz - R[3 * j + 2];
+                const double rho2 = dx * dx + dy * dy + dz * dz;
+                const double rho = sqrt(rho2);
+                const double i3 = 1.0 / (rho2 * rho), i5 = i3 / rho2;
+                const double nd = nrm[3 * j] * dx + nrm[3 * j + 1] * dy + nrm[3 * j + 2] * dz;
+                const double a = -Q[j] * i3 + 3.0 * D[j] * nd * i5;   /* multiplies d */
+                const double b = -D[j] * i3;                          /* multiplies n */
+                sx += a * dx + b * nrm[3 * j];
+                sy += a * dy + b * nrm[3 * j + 1];
+                sz += a * dz + b * nrm[3 * j + 2];
+            }
+            gx += (long double)sx; gy += (long double)sy; gz += (long double)sz;
+        }
+        grad[3 * t] = (double)gx; grad[3 * t + 1] = (double)gy; grad[3 * t + 2] = (double)gz;
+    }
+}
+
 /* U = 1/2 sum_i q_i phi_i, accumulated in long double. */
 double oracle_energy(const double *q, const double *phi, long N)
 {

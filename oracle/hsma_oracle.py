@@ -65,6 +65,10 @@ def _lib():
         lib.oracle_near_sum.restype = None
         lib.oracle_node_sum.argtypes = [dp, ctypes.c_long, dp, dp, dp, dp, ctypes.c_long, dp]
         lib.oracle_node_sum.restype = None
+        lib.oracle_near_grad.argtypes = lib.oracle_near_sum.argtypes
+        lib.oracle_near_grad.restype = None
+        lib.oracle_node_grad.argtypes = lib.oracle_node_sum.argtypes
+        lib.oracle_node_grad.restype = None
         lib.oracle_energy.argtypes = [dp, dp, ctypes.c_long]
         lib.oracle_energy.restype = ctypes.c_double
         lib.oracle_num_threads.restype = ctypes.c_int
@@ -151,6 +155,29 @@ def node_sum(tgt, R, nrm, Q, D) -> np.ndarray:
         return phi
     _lib().oracle_node_sum(_p(tgt), tgt.shape[0], _p(R), _p(nrm), _p(Q), _p(D), R.shape[0], _p(phi))
     return phi
+
+
+def near_grad(tgt, src, q, cells: CellTable, self_offset: int = -1) -> np.ndarray:
+    """Gradient of Phi_in (Eq.5) with respect to the target position, [T,3].
+    The force on source i is -q_i grad Phi(r_i)."""
+    tgt, src, q = _c(tgt), _c(src), _c(q)
+    g = np.zeros((tgt.shape[0], 3))
+    if tgt.shape[0] == 0:
+        return g
+    _lib().oracle_near_grad(_p(tgt), tgt.shape[0], _p(src), _p(q), src.shape[0], _p(cells.shift),
+                            _p(cells.sign), _p(cells.w), cells.w.shape[0], cells.central,
+                            self_offset, _p(g))
+    return g
+
+
+def node_grad(tgt, R, nrm, Q, D) -> np.ndarray:
+    """Gradient of Phi_out (Eq.10 PAPER.md:101 on the nodes, exact normal dipole) at the targets, [T,3]."""
+    tgt, R, nrm, Q, D = _c(tgt), _c(R), _c(nrm), _c(Q), _c(D)
+    g = np.zeros((tgt.shape[0], 3))
+    if tgt.shape[0] == 0:
+        return g
+    _lib().oracle_node_grad(_p(tgt), tgt.shape[0], _p(R), _p(nrm), _p(Q), _p(D), R.shape[0], _p(g))
+    return g
 
 
 def energy(q, phi) -> float:
@@ -342,6 +369,8 @@ class OracleResult:
     nodes: np.ndarray
     normals: np.ndarray
     pairs: dict                # pair counts per call site
+    grad: Optional[np.ndarray] = None   # [N,3] grad Phi at the sources (forces=True)
+    F: Optional[np.ndarray] = None      # [N,3] forces -q_i grad Phi(r_i)
 
 
 def validate_geometry(L, shell, R_aux):
@@ -355,7 +384,7 @@ def validate_geometry(L, shell, R_aux):
 
 
 def hsma(w, targets_slice: Optional[slice] = None, dipole: str = "exact", dr_rel: float = 1e-5,
-         p: Optional[int] = None, M: Optional[int] = None) -> OracleResult:
+         p: Optional[int] = None, M: Optional[int] = None, forces: bool = False) -> OracleResult:
     """One HSMA evaluation of workload `w` (an hsma_workloads.Workload).
     `targets_slice`: evaluate phi only at that slice of the sources (sampled parity at full size);
     U is then the partial sum over the slice.  `dipole`: "exact" (reading S9, primary) or "fd3"
@@ -451,8 +480,16 @@ def hsma(w, targets_slice: Optional[slice] = None, dipole: str = "exact", dr_rel
     pairs = {"a": int(check_targets.shape[0]) * N * int(n_check_cells),
              "b": int(i1 - i0) * N * int(near.w.shape[0]),
              "c": int(i1 - i0) * int(nodes.shape[0])}
-    return OracleResult(phi, U, A, rhs, fit_rms, float(sv[0] / sv[-1]), phi_near, phi_out,
-                        check_targets, phi_check, Q, D, nodes, nrm, pairs)
+    res = OracleResult(phi, U, A, rhs, fit_rms, float(sv[0] / sv[-1]), phi_near, phi_out,
+                       check_targets, phi_check, Q, D, nodes, nrm, pairs)
+    if forces:
+        # PAPER.md:89-93 (Eq.9): F_i = -q_i grad [Phi_in + Phi_out](r_i), bare self term excluded,
+        # coefficients A_nm held fixed; the image gradient uses the exact dipole layer (reading S9)
+        if dipole != "exact":
+            raise ValueError("forces are implemented for the exact dipole layer")
+        res.grad = near_grad(tg, src, q, near, self_offset=i0) + node_grad(tg, nodes, nrm, Q, D)
+        res.F = -q[i0:i1, None] * res.grad
+    return res
 
 
 def series_at(points_centred, A, p: int, R0: float) -> np.ndarray:

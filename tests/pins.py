@@ -46,6 +46,42 @@ def ewald_potentials(xyz, q, L, alpha, rcut_cells, kmax):
     return phi
 
 
+def ewald_forces(xyz, q, L, alpha, rcut_cells, kmax):
+    """F_i = -dU/dr_i of the same Ewald sum (tin-foil), textbook form:
+    real space  q_i q_j [erfc(a r)/r + 2a/sqrt(pi) exp(-a^2 r^2)] r_vec/r^2,
+    reciprocal  -q_i (4 pi/V) sum_k k exp(-k^2/4a^2)/k^2 Im[exp(-i k.r_i) S(k)] with S = sum q exp(i k.r)."""
+    xyz = np.asarray(xyz, float)
+    q = np.asarray(q, float)
+    L = np.asarray(L, float)
+    N = len(q)
+    V = float(np.prod(L))
+    F = np.zeros((N, 3))
+    d = xyz[:, None, :] - xyz[None, :, :]
+    rng = range(-rcut_cells, rcut_cells + 1)
+    for nx in rng:
+        for ny in rng:
+            for nz in rng:
+                dv = d + np.array([nx, ny, nz]) * L
+                r2 = (dv ** 2).sum(-1)
+                if nx == 0 and ny == 0 and nz == 0:
+                    np.fill_diagonal(r2, np.inf)
+                r = np.sqrt(r2)
+                c = (erfc(alpha * r) / r + 2 * alpha / math.sqrt(math.pi) * np.exp(-alpha * alpha * r2)) / r2
+                F += q[:, None] * np.einsum("ij,ijk->ik", c * q[None, :], dv)
+    ms = np.arange(-kmax, kmax + 1)
+    MX, MY, MZ = np.meshgrid(ms, ms, ms, indexing="ij")
+    m = np.stack([MX.ravel(), MY.ravel(), MZ.ravel()], 1)
+    m = m[(m != 0).any(1)]
+    k = 2 * math.pi * m / L
+    k2 = (k * k).sum(1)
+    ph = xyz @ k.T
+    S = (q[:, None] * np.exp(1j * ph)).sum(0)
+    coef = (4 * math.pi / V) * np.exp(-k2 / (4 * alpha * alpha)) / k2
+    im = (np.exp(-1j * ph) * S[None, :]).imag                  # [N, nk]
+    F += -q[:, None] * ((im * coef[None, :]) @ k)
+    return F
+
+
 def grounded_box_green(x, xp, box, nmax=80):
     """G(x, x') with G = 0 on the walls of [0,a]x[0,b]x[0,c], normalised so that
     G -> 1/|x-x'| near x' (Gaussian units).  Converges like exp(-K |z - z'|): use |z-z'| > 0."""
