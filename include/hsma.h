@@ -122,6 +122,21 @@ hsma_status hsma_evaluate_shard_host(hsma_plan* plan, const double* xyz_host, co
                                      long long N, long long t0, long long t1, double* phi_host,
                                      double* energy_host);
 
+/*
+ * Forces (Eq.(9); Appendix A): as hsma_evaluate*, and in addition
+ *   force_out dev [N,3] (shard: [t1-t0,3]) row-major,  F_i = -q_i grad [Phi_in + Phi_out](r_i),
+ * with the bare self term excluded and the coefficients A_nm held fixed.  Steps (b) and (c) run their
+ * potential+gradient kernels (16 / 26 FP64 instructions per pair instead of 10 / 17).  phi_out may be NULL.
+ */
+hsma_status hsma_evaluate_forces(hsma_plan* plan, const double* xyz, const double* q, long long N,
+                                 double* phi_out, double* force_out, double* energy_out);
+hsma_status hsma_evaluate_forces_shard(hsma_plan* plan, const double* xyz, const double* q, long long N,
+                                       long long t0, long long t1, double* phi_out, double* force_out,
+                                       double* energy_out);
+/* HOST buffers; force_host [N,3] required, phi_host / energy_host may be NULL; synchronises. */
+hsma_status hsma_evaluate_forces_host(hsma_plan* plan, const double* xyz_host, const double* q_host,
+                                      long long N, double* phi_host, double* force_host, double* energy_host);
+
 /* Synchronise the plan's stream and return the sticky status of the evaluations since the last
  * call (HSMA_ERR_NOT_NEUTRAL, HSMA_ERR_CUDA, ...), then clear it. */
 hsma_status hsma_plan_sync(hsma_plan* plan);
@@ -153,6 +168,15 @@ hsma_status hsma_direct_sum(const double* tgt, long long T, const double* src, c
 /* Raw kernel (c): phi[t] = sum_j Q_j/rho - P_j.(t - R_j)/rho^3.  All dev pointers; R [M,3], P [M,3]. */
 hsma_status hsma_node_sum(const double* tgt, long long T, const double* R, const double* Q,
                           const double* P, long long M, double* phi_out, void* cuda_stream);
+/* Raw potential+gradient kernels: as the two above, and grad_out dev [T,3] = d phi / d tgt_t.
+ * phi_out may be NULL. */
+hsma_status hsma_direct_field(const double* tgt, long long T, const double* src, const double* q,
+                              long long N, const double* shift_host, const double* sign_host,
+                              const double* w_host, int C, int central_cell, long long self_offset,
+                              int refine, double* phi_out, double* grad_out, void* cuda_stream);
+hsma_status hsma_node_field(const double* tgt, long long T, const double* R, const double* Q,
+                            const double* P, long long M, double* phi_out, double* grad_out,
+                            void* cuda_stream);
 
 /* DFMA-only microbenchmark on the current device: sustained FP64 FMA TFLOP/s over ~`seconds`
  * (the roofline denominator).  host out; synchronises. */

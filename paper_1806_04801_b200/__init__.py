@@ -68,6 +68,27 @@ class Plan:
             binding.hsma_plan_sync(self.handle)
         return phi, U
 
+    def evaluate_forces(self, xyz: torch.Tensor, q: torch.Tensor, sync: bool = False):
+        """phi [N], F [N,3] = -q grad Phi, U [1]."""
+        N = q.numel()
+        phi = torch.empty(N, dtype=torch.float64, device=q.device)
+        F = torch.empty(N, 3, dtype=torch.float64, device=q.device)
+        U = torch.empty(1, dtype=torch.float64, device=q.device)
+        binding.hsma_evaluate_forces(self.handle, xyz, q, phi, F, U)
+        if sync:
+            binding.hsma_plan_sync(self.handle)
+        return phi, F, U
+
+    def evaluate_forces_shard(self, xyz: torch.Tensor, q: torch.Tensor, t0: int, t1: int, sync: bool = False):
+        T = max(t1 - t0, 0)
+        phi = torch.empty(T, dtype=torch.float64, device=q.device)
+        F = torch.empty(T, 3, dtype=torch.float64, device=q.device)
+        U = torch.empty(1, dtype=torch.float64, device=q.device)
+        binding.hsma_evaluate_forces_shard(self.handle, xyz, q, t0, t1, phi, F, U)
+        if sync:
+            binding.hsma_plan_sync(self.handle)
+        return phi, F, U
+
     def evaluate_shard(self, xyz: torch.Tensor, q: torch.Tensor, t0: int, t1: int, sync: bool = False):
         phi = torch.empty(max(t1 - t0, 0), dtype=torch.float64, device=q.device)
         U = torch.empty(1, dtype=torch.float64, device=q.device)

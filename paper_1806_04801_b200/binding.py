@@ -56,6 +56,13 @@ _SIGNATURES = {
     "hsma_evaluate_shard_host": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_longlong,
                                                 ctypes.c_longlong, ctypes.c_longlong, ctypes.c_void_p,
                                                 ctypes.c_void_p]),
+    "hsma_evaluate_forces": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_longlong,
+                                            ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]),
+    "hsma_evaluate_forces_shard": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_longlong,
+                                                  ctypes.c_longlong, ctypes.c_longlong, ctypes.c_void_p,
+                                                  ctypes.c_void_p, ctypes.c_void_p]),
+    "hsma_evaluate_forces_host": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_longlong,
+                                                 ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]),
     "hsma_plan_sync": (ctypes.c_int, [ctypes.c_void_p]),
     "hsma_status_string": (ctypes.c_char_p, [ctypes.c_int]),
     "hsma_plan_info": (ctypes.c_int, [ctypes.c_void_p, ctypes.POINTER(ctypes.c_longlong)]),
@@ -71,6 +78,13 @@ _SIGNATURES = {
                                        ctypes.c_void_p]),
     "hsma_node_sum": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p,
                                      ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p]),
+    "hsma_direct_field": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p,
+                                         ctypes.c_longlong, c_double_p, c_double_p, c_double_p, ctypes.c_int,
+                                         ctypes.c_int, ctypes.c_longlong, ctypes.c_int, ctypes.c_void_p,
+                                         ctypes.c_void_p, ctypes.c_void_p]),
+    "hsma_node_field": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p,
+                                       ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p,
+                                       ctypes.c_void_p]),
     "hsma_fp64_peak": (ctypes.c_int, [ctypes.c_double, c_double_p, c_double_p]),
     "hsma_plan_set_timing": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int]),
     "hsma_plan_get_timing": (ctypes.c_int, [ctypes.c_void_p, c_double_p]),
@@ -211,6 +225,39 @@ def hsma_evaluate_shard_host(plan: int, xyz: np.ndarray, q: np.ndarray, t0: int,
            "hsma_evaluate_shard_host")
 
 
+def hsma_evaluate_forces(plan: int, xyz: torch.Tensor, q: torch.Tensor, phi_out: Optional[torch.Tensor],
+                         force_out: torch.Tensor, energy_out: Optional[torch.Tensor] = None):
+    N = q.numel()
+    _check(load_library().hsma_evaluate_forces(plan, _dev(xyz, 3 * N, "xyz"), _dev(q, N, "q"), N,
+                                               _dev(phi_out, N, "phi_out"), _dev(force_out, 3 * N, "force_out"),
+                                               _dev(energy_out, 1, "energy_out")), "hsma_evaluate_forces")
+
+
+def hsma_evaluate_forces_shard(plan: int, xyz: torch.Tensor, q: torch.Tensor, t0: int, t1: int,
+                               phi_out: Optional[torch.Tensor], force_out: torch.Tensor,
+                               energy_out: Optional[torch.Tensor] = None):
+    N, T = q.numel(), max(t1 - t0, 0)
+    _check(load_library().hsma_evaluate_forces_shard(plan, _dev(xyz, 3 * N, "xyz"), _dev(q, N, "q"), N, t0, t1,
+                                                     _dev(phi_out, T, "phi_out"), _dev(force_out, 3 * T, "force_out"),
+                                                     _dev(energy_out, 1, "energy_out")), "hsma_evaluate_forces_shard")
+
+
+def hsma_evaluate_forces_host(plan: int, xyz: np.ndarray, q: np.ndarray, phi_out: Optional[np.ndarray],
+                              force_out: np.ndarray, energy_out: Optional[np.ndarray]):
+    """HOST arrays: xyz [N,3], q [N], phi_out [N] or None, force_out [N,3], energy_out [1] or None."""
+    for a in (xyz, q, phi_out, force_out, energy_out):
+        if a is not None and not (a.dtype == np.float64 and a.flags.c_contiguous):
+            raise TypeError("host buffers must be C-contiguous float64")
+    N = q.shape[0]
+    if force_out.size < 3 * N:
+        raise ValueError("force_out too small")
+    _check(load_library().hsma_evaluate_forces_host(plan, xyz.ctypes.data, q.ctypes.data, N,
+                                                    None if phi_out is None else phi_out.ctypes.data,
+                                                    force_out.ctypes.data,
+                                                    None if energy_out is None else energy_out.ctypes.data),
+           "hsma_evaluate_forces_host")
+
+
 def hsma_plan_sync(plan: int):
     _check(load_library().hsma_plan_sync(plan), "hsma_plan_sync")
 
@@ -263,6 +310,24 @@ def hsma_node_sum(tgt: torch.Tensor, R: torch.Tensor, Q: torch.Tensor, P: torch.
     _check(load_library().hsma_node_sum(_dev(tgt, 3 * T, "tgt"), T, _dev(R, 3 * M, "R"), _dev(Q, M, "Q"),
                                         _dev(P, 3 * M, "P"), M, _dev(phi_out, T, "phi_out"), _stream_ptr(stream)),
            "hsma_node_sum")
+
+
+def hsma_direct_field(tgt: torch.Tensor, src: torch.Tensor, q: torch.Tensor, shift, sign, w, central_cell: int,
+                      self_offset: int, refine: int, phi_out: Optional[torch.Tensor], grad_out: torch.Tensor, stream=None):
+    shift, sign, w = _host(shift), _host(sign), _host(w)
+    T, N, C = tgt.shape[0], q.numel(), w.shape[0]
+    _check(load_library().hsma_direct_field(_dev(tgt, 3 * T, "tgt"), T, _dev(src, 3 * N, "src"), _dev(q, N, "q"), N,
+                                            _hp(shift), _hp(sign), _hp(w), C, central_cell, self_offset, refine,
+                                            _dev(phi_out, T, "phi_out"), _dev(grad_out, 3 * T, "grad_out"),
+                                            _stream_ptr(stream)), "hsma_direct_field")
+
+
+def hsma_node_field(tgt: torch.Tensor, R: torch.Tensor, Q: torch.Tensor, P: torch.Tensor,
+                    phi_out: Optional[torch.Tensor], grad_out: torch.Tensor, stream=None):
+    T, M = tgt.shape[0], Q.numel()
+    _check(load_library().hsma_node_field(_dev(tgt, 3 * T, "tgt"), T, _dev(R, 3 * M, "R"), _dev(Q, M, "Q"),
+                                          _dev(P, 3 * M, "P"), M, _dev(phi_out, T, "phi_out"),
+                                          _dev(grad_out, 3 * T, "grad_out"), _stream_ptr(stream)), "hsma_node_field")
 
 
 def hsma_fp64_peak(seconds: float = 1.0):

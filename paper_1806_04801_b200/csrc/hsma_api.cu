@@ -67,25 +67,34 @@ static int resident_ctas(K kernel) {
     }
     return per_sm * num_sm();
 }
-// resident CTAs of near_sum_kernel<R, REFINE, *>: the smaller of the two loop forms (they share one launch shape)
-template <int R, int REFINE>
+// resident CTAs of near_sum_kernel<R, REFINE, *, FIELD>: the smaller of the two loop forms (one launch shape)
+template <int R, int REFINE, bool FIELD>
 static int near_resident_of() {
-    return std::min(resident_ctas(near_sum_kernel<R, REFINE, false>), resident_ctas(near_sum_kernel<R, REFINE, true>));
+    return std::min(resident_ctas(near_sum_kernel<R, REFINE, false, FIELD>), resident_ctas(near_sum_kernel<R, REFINE, true, FIELD>));
 }
-static int near_resident(int R, int refine) {
-    static int cache[4][2] = {{0, 0}, {0, 0}, {0, 0}, {0, 0}};
-    const int i = R == 8 ? 3 : (R == 4 ? 2 : (R == 2 ? 1 : 0)), j = refine == 1 ? 0 : 1;
-    if (!cache[i][j]) {
-        if (refine == 1) cache[i][j] = R == 8 ? near_resident_of<8, 1>() : R == 4 ? near_resident_of<4, 1>() : R == 2 ? near_resident_of<2, 1>() : near_resident_of<1, 1>();
-        else cache[i][j] = R == 8 ? near_resident_of<8, 2>() : R == 4 ? near_resident_of<4, 2>() : R == 2 ? near_resident_of<2, 2>() : near_resident_of<1, 2>();
+static int near_resident(int R, int refine, bool field) {
+    static int cache[4][2][2] = {};
+    const int i = R == 8 ? 3 : (R == 4 ? 2 : (R == 2 ? 1 : 0)), j = refine == 1 ? 0 : 1, f = field ? 1 : 0;
+    int& c = cache[i][j][f];
+    if (!c) {
+        if (!field) {
+            if (refine == 1) c = R == 8 ? near_resident_of<8, 1, false>() : R == 4 ? near_resident_of<4, 1, false>() : R == 2 ? near_resident_of<2, 1, false>() : near_resident_of<1, 1, false>();
+            else c = R == 8 ? near_resident_of<8, 2, false>() : R == 4 ? near_resident_of<4, 2, false>() : R == 2 ? near_resident_of<2, 2, false>() : near_resident_of<1, 2, false>();
+        } else {  // FIELD: R <= 4
+            if (refine == 1) c = R == 4 ? near_resident_of<4, 1, true>() : R == 2 ? near_resident_of<2, 1, true>() : near_resident_of<1, 1, true>();
+            else c = R == 4 ? near_resident_of<4, 2, true>() : R == 2 ? near_resident_of<2, 2, true>() : near_resident_of<1, 2, true>();
+        }
     }
-    return cache[i][j];
+    return c;
 }
-static int node_resident(int R) {
-    static int cache[3] = {0, 0, 0};
-    const int i = R == 4 ? 2 : (R == 2 ? 1 : 0);
-    if (!cache[i]) cache[i] = R == 4 ? resident_ctas(node_sum_kernel<4>) : R == 2 ? resident_ctas(node_sum_kernel<2>) : resident_ctas(node_sum_kernel<1>);
-    return cache[i];
+static int node_resident(int R, bool field) {
+    static int cache[3][2] = {};
+    int& c = cache[R == 4 ? 2 : (R == 2 ? 1 : 0)][field ? 1 : 0];
+    if (!c) {
+        if (!field) c = R == 4 ? resident_ctas(node_sum_kernel<4, false>) : R == 2 ? resident_ctas(node_sum_kernel<2, false>) : resident_ctas(node_sum_kernel<1, false>);
+        else c = R == 4 ? resident_ctas(node_sum_kernel<4, true>) : R == 2 ? resident_ctas(node_sum_kernel<2, true>) : resident_ctas(node_sum_kernel<1, true>);
+    }
+    return c;
 }
 
 // Targets per thread: the largest R in {Rmax, .., 2, 1} that (i) leaves every resident CTA at least 4 units
@@ -120,51 +129,62 @@ struct Packed {
     const Src4* src; long long n_src, n_tiles; const int* tile_np; const int* slot_of; const QInfo* qinfo;
 };
 
-template <bool UNIFORM>
+template <bool UNIFORM, bool FIELD>
 static void launch_near_form(const Launch& L, int refine, const NearArgs& a, cudaStream_t st) {
     if (refine == 1) {
-        if (L.R == 8) near_sum_kernel<8, 1, UNIFORM><<<L.G, kThreads, 0, st>>>(a);
-        else if (L.R == 4) near_sum_kernel<4, 1, UNIFORM><<<L.G, kThreads, 0, st>>>(a);
-        else if (L.R == 2) near_sum_kernel<2, 1, UNIFORM><<<L.G, kThreads, 0, st>>>(a);
-        else near_sum_kernel<1, 1, UNIFORM><<<L.G, kThreads, 0, st>>>(a);
+        if (L.R == 8) { if (!FIELD) near_sum_kernel<8, 1, UNIFORM, false><<<L.G, kThreads, 0, st>>>(a); }
+        else if (L.R == 4) near_sum_kernel<4, 1, UNIFORM, FIELD><<<L.G, kThreads, 0, st>>>(a);
+        else if (L.R == 2) near_sum_kernel<2, 1, UNIFORM, FIELD><<<L.G, kThreads, 0, st>>>(a);
+        else near_sum_kernel<1, 1, UNIFORM, FIELD><<<L.G, kThreads, 0, st>>>(a);
     } else {
-        if (L.R == 8) near_sum_kernel<8, 2, UNIFORM><<<L.G, kThreads, 0, st>>>(a);
-        else if (L.R == 4) near_sum_kernel<4, 2, UNIFORM><<<L.G, kThreads, 0, st>>>(a);
-        else if (L.R == 2) near_sum_kernel<2, 2, UNIFORM><<<L.G, kThreads, 0, st>>>(a);
-        else near_sum_kernel<1, 2, UNIFORM><<<L.G, kThreads, 0, st>>>(a);
+        if (L.R == 8) { if (!FIELD) near_sum_kernel<8, 2, UNIFORM, false><<<L.G, kThreads, 0, st>>>(a); }
+        else if (L.R == 4) near_sum_kernel<4, 2, UNIFORM, FIELD><<<L.G, kThreads, 0, st>>>(a);
+        else if (L.R == 2) near_sum_kernel<2, 2, UNIFORM, FIELD><<<L.G, kThreads, 0, st>>>(a);
+        else near_sum_kernel<1, 2, UNIFORM, FIELD><<<L.G, kThreads, 0, st>>>(a);
     }
     HSMA_COUNT_LAUNCH();
 }
 
-// part must hold L.rows * T doubles.  tgt_index: null, or the row of each target inside tgt.
-static void launch_near(const Launch& L, const double* tgt, int tstride, const int* tgt_index, long long T, long long t_first,
-                        const Packed& P, const Cell* cells, int C, long long self_offset, int refine, double* part,
-                        cudaStream_t st) {
+// part must hold L.rows * T doubles (x 4 with field).  tgt_index: null, or the row of each target inside tgt.
+static void launch_near(const Launch& L, bool field, const double* tgt, int tstride, const int* tgt_index, long long T,
+                        long long t_first, const Packed& P, const Cell* cells, int C, long long self_offset, int refine,
+                        double* part, cudaStream_t st) {
     NearArgs a;
     a.tgt = tgt; a.tstride = tstride; a.tgt_index = tgt_index; a.T = T; a.t_first = t_first;
     a.src = P.src; a.n_src = P.n_src; a.n_tiles = P.n_tiles; a.tile_np = P.tile_np; a.slot_of = P.slot_of; a.qinfo = P.qinfo;
     a.cells = cells; a.C = C; a.units = L.U; a.self_offset = self_offset;
-    a.scale = refine == 1 ? 0.5 : 1.0; a.part = part;
+    a.scale = refine == 1 ? 0.5 : 1.0; a.scale_grad = refine == 1 ? -0.125 : -1.0; a.part = part;
     // generic form always; the uniform-|q| form too when the charge statistics are available (each returns at
     // once unless QInfo.uniform selects it)
-    launch_near_form<false>(L, refine, a, st);
-    if (a.qinfo) launch_near_form<true>(L, refine, a, st);
+    if (field) {
+        launch_near_form<false, true>(L, refine, a, st);
+        if (a.qinfo) launch_near_form<true, true>(L, refine, a, st);
+    } else {
+        launch_near_form<false, false>(L, refine, a, st);
+        if (a.qinfo) launch_near_form<true, false>(L, refine, a, st);
+    }
 }
-static Launch choose_near(long long T, long long n_tiles, int C, int refine) {
-    return choose_launch(T, n_tiles * C, 8, [refine](int R) { return near_resident(R, refine); });
+static Launch choose_near(long long T, long long n_tiles, int C, int refine, bool field = false) {
+    return choose_launch(T, n_tiles * C, field ? 4 : 8, [refine, field](int R) { return near_resident(R, refine, field); });
 }
 
-static Launch choose_node(long long T, long long n_tiles) {
-    return choose_launch(T, n_tiles, 4, [](int R) { return node_resident(R); });
+static Launch choose_node(long long T, long long n_tiles, bool field = false) {
+    return choose_launch(T, n_tiles, 4, [field](int R) { return node_resident(R, field); });
 }
-static void launch_node(const Launch& L, const double* tgt, int tstride, const int* tgt_index, long long T, long long t_first,
-                        const Node8* nodes, long long n_tiles, double* part, cudaStream_t st) {
+static void launch_node(const Launch& L, bool field, const double* tgt, int tstride, const int* tgt_index, long long T,
+                        long long t_first, const Node8* nodes, long long n_tiles, double* part, cudaStream_t st) {
     NodeArgs a;
     a.tgt = tgt; a.tstride = tstride; a.tgt_index = tgt_index; a.T = T; a.t_first = t_first; a.nodes = nodes; a.n_tiles = n_tiles;
     a.units = L.U; a.part = part;
-    if (L.R == 4) node_sum_kernel<4><<<L.G, kThreads, 0, st>>>(a);
-    else if (L.R == 2) node_sum_kernel<2><<<L.G, kThreads, 0, st>>>(a);
-    else node_sum_kernel<1><<<L.G, kThreads, 0, st>>>(a);
+    if (field) {
+        if (L.R == 4) node_sum_kernel<4, true><<<L.G, kThreads, 0, st>>>(a);
+        else if (L.R == 2) node_sum_kernel<2, true><<<L.G, kThreads, 0, st>>>(a);
+        else node_sum_kernel<1, true><<<L.G, kThreads, 0, st>>>(a);
+    } else {
+        if (L.R == 4) node_sum_kernel<4, false><<<L.G, kThreads, 0, st>>>(a);
+        else if (L.R == 2) node_sum_kernel<2, false><<<L.G, kThreads, 0, st>>>(a);
+        else node_sum_kernel<1, false><<<L.G, kThreads, 0, st>>>(a);
+    }
     HSMA_COUNT_LAUNCH();
 }
 
@@ -195,7 +215,7 @@ struct hsma_plan {
     DevBuf<Src4> src;
     DevBuf<int> slot_of, tile_np;
     QInfo* qinfo = nullptr;
-    DevBuf<double> part_a, part_b, part_c, red, xyz_in, q_in, phi_dev;
+    DevBuf<double> part_a, part_b, part_c, red, xyz_in, q_in, phi_dev, force_dev;
     long long last_launches = 0;
     hsma_status sticky = HSMA_OK;
     // stage timing (hsma_plan_set_timing): events ev[0..7] bracket the stages of one evaluate
@@ -215,7 +235,7 @@ static void plan_free(hsma_plan* p) {
     for (void* q : ptrs) if (q) cudaFree(q);
     p->src.release(); p->slot_of.release(); p->tile_np.release(); if (p->qinfo) cudaFree(p->qinfo);
     p->part_a.release(); p->part_b.release(); p->part_c.release(); p->red.release();
-    p->xyz_in.release(); p->q_in.release(); p->phi_dev.release();
+    p->xyz_in.release(); p->q_in.release(); p->phi_dev.release(); p->force_dev.release();
     for (cudaEvent_t e : p->ev) if (e) cudaEventDestroy(e);
     delete p;
 }
@@ -383,9 +403,11 @@ __global__ void node_positions_kernel(const double* __restrict__ nrm, double R, 
 }
 }  // namespace hsma
 
+// force_out non-null: the FIELD kernels also produce F_i = -q_i grad Phi(r_i)
 static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* q, long long N, long long t0,
-                                 long long t1, double* phi_out, double* energy_out) {
-    if (!p || !xyz || !q || N < 1 || t0 < 0 || t1 > N || t0 > t1 || (!phi_out && t1 > t0)) return HSMA_ERR_INVALID_ARG;
+                                 long long t1, double* phi_out, double* energy_out, double* force_out = nullptr) {
+    if (!p || !xyz || !q || N < 1 || t0 < 0 || t1 > N || t0 > t1 || (!phi_out && !force_out && t1 > t0)) return HSMA_ERR_INVALID_ARG;
+    const bool field = force_out != nullptr;
     cudaStream_t st = p->stream;
     const long long before = g_launches;
     const long long n_tiles = (N + kTile - 1) / kTile, Npad = n_tiles * kTile;
@@ -411,7 +433,7 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
         const Launch s = choose_near(p->Kt, n_tiles, p->C_rhs, 2);
         if (p->part_a.reserve((size_t)s.rows * p->Kt) != cudaSuccess) return HSMA_ERR_ALLOC;
         MARK(1);
-        launch_near(s, p->chk, 3, nullptr, p->Kt, 0, P, p->cells_rhs, p->C_rhs, -1, 2, p->part_a.p, st);  // (a) always cubic: it feeds the fit
+        launch_near(s, false, p->chk, 3, nullptr, p->Kt, 0, P, p->cells_rhs, p->C_rhs, -1, 2, p->part_a.p, st);  // (a) always cubic: it feeds the fit
         MARK(2);
         finish_phi_kernel<<<(p->Kt + 255) / 256, 256, 0, st>>>(s.layout(p->part_a.p), PartLayout{nullptr, 1, 1, 1, 1}, p->Kt, nullptr, nullptr, 0, p->pc, nullptr);
         HSMA_COUNT_LAUNCH();
@@ -429,22 +451,27 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
     if (T > 0) {
         // H5 (b): near images at the sources, self excluded
         const int refine = p->refine ? p->refine : ((double)N * (double)N * p->C_near < 4294967296.0 ? 2 : 1);
-        const Launch sb = choose_near(T, n_tiles, p->C_near, refine);
-        if (p->part_b.reserve((size_t)sb.rows * T) != cudaSuccess) return HSMA_ERR_ALLOC;
         // rsqrt_refine = 0: the cubic step while (b) is latency-bound anyway (< 2^32 pairs), Newton above
-        const Launch sc = choose_node(T, p->node_tiles);
-        if (p->part_c.reserve((size_t)sc.rows * T) != cudaSuccess) return HSMA_ERR_ALLOC;
+        const size_t comps = field ? 4 : 1;
+        const Launch sb = choose_near(T, n_tiles, p->C_near, refine, field);
+        if (p->part_b.reserve((size_t)sb.rows * T * comps) != cudaSuccess) return HSMA_ERR_ALLOC;
+        const Launch sc = choose_node(T, p->node_tiles, field);
+        if (p->part_c.reserve((size_t)sc.rows * T * comps) != cudaSuccess) return HSMA_ERR_ALLOC;
         MARK(3);
-        launch_near(sb, reinterpret_cast<const double*>(p->src.p), 4, p->slot_of.p, T, t0, P, p->cells_near, p->C_near,
+        launch_near(sb, field, reinterpret_cast<const double*>(p->src.p), 4, p->slot_of.p, T, t0, P, p->cells_near, p->C_near,
                     t0, refine, p->part_b.p, st);
         MARK(4);
         // H6 (c): sphere nodes, charge + dipole
-        launch_node(sc, reinterpret_cast<const double*>(p->src.p), 4, p->slot_of.p, T, t0, p->nodes, p->node_tiles, p->part_c.p, st);
+        launch_node(sc, field, reinterpret_cast<const double*>(p->src.p), 4, p->slot_of.p, T, t0, p->nodes, p->node_tiles, p->part_c.p, st);
         MARK(5);
-        // H7: phi and U
+        // H7: phi (forces) and U
         const long long fb = (T + 255) / 256;
-        finish_phi_kernel<<<(unsigned)fb, 256, 0, st>>>(sb.layout(p->part_b.p), sc.layout(p->part_c.p), T, p->src.p, p->slot_of.p, t0, phi_out,
-                                                        energy_out ? p->red.p : nullptr);
+        if (field)
+            finish_field_kernel<<<(unsigned)fb, 256, 0, st>>>(sb.layout(p->part_b.p), sc.layout(p->part_c.p), T, p->src.p, p->slot_of.p, t0,
+                                                              phi_out, force_out, energy_out ? p->red.p : nullptr);
+        else
+            finish_phi_kernel<<<(unsigned)fb, 256, 0, st>>>(sb.layout(p->part_b.p), sc.layout(p->part_c.p), T, p->src.p, p->slot_of.p, t0, phi_out,
+                                                            energy_out ? p->red.p : nullptr);
         HSMA_COUNT_LAUNCH();
         if (energy_out) {
             reduce_rows_kernel<<<1, 1024, 0, st>>>(p->red.p, fb, 1, 1, 0.5, energy_out);
@@ -472,6 +499,20 @@ extern "C" hsma_status hsma_evaluate_shard(hsma_plan* plan, const double* xyz, c
     return evaluate_impl(plan, xyz, q, N, t0, t1, phi_out, energy_out);
 }
 
+extern "C" hsma_status hsma_evaluate_forces(hsma_plan* plan, const double* xyz, const double* q, long long N,
+                                            double* phi_out, double* force_out, double* energy_out) {
+    if (!force_out) return HSMA_ERR_INVALID_ARG;
+    return evaluate_impl(plan, xyz, q, N, 0, N, phi_out, energy_out, force_out);
+}
+
+extern "C" hsma_status hsma_evaluate_forces_shard(hsma_plan* plan, const double* xyz, const double* q, long long N,
+                                                  long long t0, long long t1, double* phi_out, double* force_out,
+                                                  double* energy_out) {
+    if (!force_out && t1 > t0) return HSMA_ERR_INVALID_ARG;
+    if (t1 == t0) return evaluate_impl(plan, xyz, q, N, t0, t1, phi_out, energy_out);
+    return evaluate_impl(plan, xyz, q, N, t0, t1, phi_out, energy_out, force_out);
+}
+
 extern "C" hsma_status hsma_plan_sync(hsma_plan* plan) {
     if (!plan) return HSMA_ERR_INVALID_ARG;
     int hf[4] = {0, 0, 0, 0};
@@ -487,23 +528,37 @@ extern "C" hsma_status hsma_plan_sync(hsma_plan* plan) {
     return s;
 }
 
-extern "C" hsma_status hsma_evaluate_shard_host(hsma_plan* p, const double* xyz_host, const double* q_host,
-                                                long long N, long long t0, long long t1, double* phi_host,
-                                                double* energy_host) {
+static hsma_status host_impl(hsma_plan* p, const double* xyz_host, const double* q_host, long long N, long long t0,
+                             long long t1, double* phi_host, double* force_host, double* energy_host) {
     if (!p || !xyz_host || !q_host || N < 1 || t0 < 0 || t1 > N || t0 > t1) return HSMA_ERR_INVALID_ARG;
     const long long T = t1 - t0;
+    const bool field = force_host != nullptr && T > 0;
     if (p->xyz_in.reserve(3 * (size_t)N) != cudaSuccess || p->q_in.reserve((size_t)N) != cudaSuccess ||
-        p->phi_dev.reserve((size_t)std::max(1LL, T)) != cudaSuccess)
+        p->phi_dev.reserve((size_t)std::max(1LL, T)) != cudaSuccess ||
+        (field && p->force_dev.reserve(3 * (size_t)T) != cudaSuccess))
         return HSMA_ERR_ALLOC;
     cudaStream_t st = p->stream;
     CU(cudaMemcpyAsync(p->xyz_in.p, xyz_host, 3 * (size_t)N * sizeof(double), cudaMemcpyHostToDevice, st));
     CU(cudaMemcpyAsync(p->q_in.p, q_host, (size_t)N * sizeof(double), cudaMemcpyHostToDevice, st));
-    hsma_status s = evaluate_impl(p, p->xyz_in.p, p->q_in.p, N, t0, t1, p->phi_dev.p, p->scalars);
+    hsma_status s = evaluate_impl(p, p->xyz_in.p, p->q_in.p, N, t0, t1, p->phi_dev.p, p->scalars, field ? p->force_dev.p : nullptr);
     if (s != HSMA_OK) return s;
     if (phi_host && T > 0)
         CU(cudaMemcpyAsync(phi_host, p->phi_dev.p, (size_t)T * sizeof(double), cudaMemcpyDeviceToHost, st));
+    if (field) CU(cudaMemcpyAsync(force_host, p->force_dev.p, 3 * (size_t)T * sizeof(double), cudaMemcpyDeviceToHost, st));
     if (energy_host) CU(cudaMemcpyAsync(energy_host, p->scalars, sizeof(double), cudaMemcpyDeviceToHost, st));
     return hsma_plan_sync(p);
+}
+
+extern "C" hsma_status hsma_evaluate_shard_host(hsma_plan* p, const double* xyz_host, const double* q_host,
+                                                long long N, long long t0, long long t1, double* phi_host,
+                                                double* energy_host) {
+    return host_impl(p, xyz_host, q_host, N, t0, t1, phi_host, nullptr, energy_host);
+}
+
+extern "C" hsma_status hsma_evaluate_forces_host(hsma_plan* p, const double* xyz_host, const double* q_host, long long N,
+                                                 double* phi_host, double* force_host, double* energy_host) {
+    if (!force_host) return HSMA_ERR_INVALID_ARG;
+    return host_impl(p, xyz_host, q_host, N, 0, N, phi_host, force_host, energy_host);
 }
 
 extern "C" hsma_status hsma_evaluate_host(hsma_plan* p, const double* xyz_host, const double* q_host, long long N,
@@ -585,11 +640,12 @@ __global__ void pack_nodes_kernel(const double* __restrict__ R, const double* __
 }
 }  // namespace hsma
 
-extern "C" hsma_status hsma_direct_sum(const double* tgt, long long T, const double* src, const double* q, long long N,
-                                       const double* shift_host, const double* sign_host, const double* w_host, int C,
-                                       int central_cell, long long self_offset, int refine, double* phi_out,
-                                       void* cuda_stream) {
-    if (!tgt || !src || !q || !shift_host || !sign_host || !w_host || !phi_out) return HSMA_ERR_INVALID_ARG;
+static hsma_status direct_impl(const double* tgt, long long T, const double* src, const double* q, long long N,
+                               const double* shift_host, const double* sign_host, const double* w_host, int C,
+                               int central_cell, long long self_offset, int refine, double* phi_out, double* grad_out,
+                               void* cuda_stream) {
+    const bool field = grad_out != nullptr;
+    if (!tgt || !src || !q || !shift_host || !sign_host || !w_host || (!phi_out && !grad_out)) return HSMA_ERR_INVALID_ARG;
     if (T < 1 || N < 1 || C < 1 || C > kMaxCells || (refine != 1 && refine != 2)) return HSMA_ERR_INVALID_ARG;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     std::vector<Cell> cells(C);
@@ -600,14 +656,14 @@ extern "C" hsma_status hsma_direct_sum(const double* tgt, long long T, const dou
         cells[c].central = (c == central_cell);
     }
     const long long n_tiles = (N + kTile - 1) / kTile, Npad = n_tiles * kTile;
-    const Launch s = choose_near(T, n_tiles, C, refine);
+    const Launch s = choose_near(T, n_tiles, C, refine, field);
     if (N > 2000000000LL) return HSMA_ERR_INVALID_ARG;
     Cell* dc = nullptr; Src4* ds = nullptr; double* part = nullptr; double* stats = nullptr; int* idx = nullptr;
     QInfo* qi = nullptr; int* flags = nullptr;
     hsma_status rc = HSMA_OK;
     // idx: slot_of [N] then tile_np [n_tiles]; stats: per tile [4] then scal [2]
     if (cudaMalloc(&dc, C * sizeof(Cell)) != cudaSuccess || cudaMalloc(&ds, Npad * sizeof(Src4)) != cudaSuccess ||
-        cudaMalloc(&part, (size_t)s.rows * T * sizeof(double)) != cudaSuccess ||
+        cudaMalloc(&part, (size_t)s.rows * T * (field ? 4 : 1) * sizeof(double)) != cudaSuccess ||
         cudaMalloc(&stats, (size_t)(4 * n_tiles + 2) * sizeof(double)) != cudaSuccess ||
         cudaMalloc(&idx, (size_t)(N + n_tiles) * sizeof(int)) != cudaSuccess || cudaMalloc(&qi, sizeof(QInfo)) != cudaSuccess ||
         cudaMalloc(&flags, 4 * sizeof(int)) != cudaSuccess) {
@@ -618,8 +674,11 @@ extern "C" hsma_status hsma_direct_sum(const double* tgt, long long T, const dou
         charge_stats_kernel<<<1, 1024, 0, st>>>(stats, n_tiles, 0, stats + 4 * n_tiles, qi, flags);
         HSMA_COUNT_LAUNCH(); HSMA_COUNT_LAUNCH();
         const Packed P{ds, N, n_tiles, idx + N, idx, qi};
-        launch_near(s, tgt, 3, nullptr, T, 0, P, dc, C, central_cell >= 0 ? self_offset : -1, refine, part, st);
-        finish_phi_kernel<<<(unsigned)((T + 255) / 256), 256, 0, st>>>(s.layout(part), PartLayout{nullptr, 1, 1, 1, 1}, T, nullptr, nullptr, 0, phi_out, nullptr);
+        launch_near(s, field, tgt, 3, nullptr, T, 0, P, dc, C, central_cell >= 0 ? self_offset : -1, refine, part, st);
+        if (field)
+            finish_field_kernel<<<(unsigned)((T + 255) / 256), 256, 0, st>>>(s.layout(part), PartLayout{nullptr, 1, 1, 1, 1}, T, nullptr, nullptr, 0, phi_out, grad_out, nullptr);
+        else
+            finish_phi_kernel<<<(unsigned)((T + 255) / 256), 256, 0, st>>>(s.layout(part), PartLayout{nullptr, 1, 1, 1, 1}, T, nullptr, nullptr, 0, phi_out, nullptr);
         HSMA_COUNT_LAUNCH();
         if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) rc = HSMA_ERR_CUDA;
     }
@@ -628,28 +687,60 @@ extern "C" hsma_status hsma_direct_sum(const double* tgt, long long T, const dou
     return rc;
 }
 
-extern "C" hsma_status hsma_node_sum(const double* tgt, long long T, const double* R, const double* Q, const double* P,
-                                     long long M, double* phi_out, void* cuda_stream) {
-    if (!tgt || !R || !Q || !P || !phi_out || T < 1 || M < 1) return HSMA_ERR_INVALID_ARG;
+extern "C" hsma_status hsma_direct_sum(const double* tgt, long long T, const double* src, const double* q, long long N,
+                                       const double* shift_host, const double* sign_host, const double* w_host, int C,
+                                       int central_cell, long long self_offset, int refine, double* phi_out,
+                                       void* cuda_stream) {
+    if (!phi_out) return HSMA_ERR_INVALID_ARG;
+    return direct_impl(tgt, T, src, q, N, shift_host, sign_host, w_host, C, central_cell, self_offset, refine, phi_out,
+                       nullptr, cuda_stream);
+}
+extern "C" hsma_status hsma_direct_field(const double* tgt, long long T, const double* src, const double* q, long long N,
+                                         const double* shift_host, const double* sign_host, const double* w_host, int C,
+                                         int central_cell, long long self_offset, int refine, double* phi_out,
+                                         double* grad_out, void* cuda_stream) {
+    if (!grad_out) return HSMA_ERR_INVALID_ARG;
+    return direct_impl(tgt, T, src, q, N, shift_host, sign_host, w_host, C, central_cell, self_offset, refine, phi_out,
+                       grad_out, cuda_stream);
+}
+
+static hsma_status node_impl(const double* tgt, long long T, const double* R, const double* Q, const double* P,
+                             long long M, double* phi_out, double* grad_out, void* cuda_stream) {
+    const bool field = grad_out != nullptr;
+    if (!tgt || !R || !Q || !P || (!phi_out && !grad_out) || T < 1 || M < 1) return HSMA_ERR_INVALID_ARG;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     constexpr int kNT = kTile / 2;
     const long long n_tiles = (M + kNT - 1) / kNT, Mpad = n_tiles * kNT;
-    const Launch s = choose_node(T, n_tiles);
+    const Launch s = choose_node(T, n_tiles, field);
     Node8* dn = nullptr; double* part = nullptr;
     hsma_status rc = HSMA_OK;
-    if (cudaMalloc(&dn, Mpad * sizeof(Node8)) != cudaSuccess || cudaMalloc(&part, (size_t)s.rows * T * sizeof(double)) != cudaSuccess) {
+    if (cudaMalloc(&dn, Mpad * sizeof(Node8)) != cudaSuccess || cudaMalloc(&part, (size_t)s.rows * T * (field ? 4 : 1) * sizeof(double)) != cudaSuccess) {
         rc = HSMA_ERR_ALLOC;
     } else {
         pack_nodes_kernel<<<(unsigned)((Mpad + 255) / 256), 256, 0, st>>>(R, Q, P, M, Mpad, dn);
         HSMA_COUNT_LAUNCH();
-        launch_node(s, tgt, 3, nullptr, T, 0, dn, n_tiles, part, st);
-        finish_phi_kernel<<<(unsigned)((T + 255) / 256), 256, 0, st>>>(PartLayout{nullptr, 1, 1, 1, 1}, s.layout(part), T, nullptr, nullptr, 0, phi_out, nullptr);
+        launch_node(s, field, tgt, 3, nullptr, T, 0, dn, n_tiles, part, st);
+        if (field)
+            finish_field_kernel<<<(unsigned)((T + 255) / 256), 256, 0, st>>>(PartLayout{nullptr, 1, 1, 1, 1}, s.layout(part), T, nullptr, nullptr, 0, phi_out, grad_out, nullptr);
+        else
+            finish_phi_kernel<<<(unsigned)((T + 255) / 256), 256, 0, st>>>(PartLayout{nullptr, 1, 1, 1, 1}, s.layout(part), T, nullptr, nullptr, 0, phi_out, nullptr);
         HSMA_COUNT_LAUNCH();
         if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) rc = HSMA_ERR_CUDA;
     }
     if (dn) cudaFree(dn);
     if (part) cudaFree(part);
     return rc;
+}
+
+extern "C" hsma_status hsma_node_sum(const double* tgt, long long T, const double* R, const double* Q, const double* P,
+                                     long long M, double* phi_out, void* cuda_stream) {
+    if (!phi_out) return HSMA_ERR_INVALID_ARG;
+    return node_impl(tgt, T, R, Q, P, M, phi_out, nullptr, cuda_stream);
+}
+extern "C" hsma_status hsma_node_field(const double* tgt, long long T, const double* R, const double* Q, const double* P,
+                                       long long M, double* phi_out, double* grad_out, void* cuda_stream) {
+    if (!grad_out) return HSMA_ERR_INVALID_ARG;
+    return node_impl(tgt, T, R, Q, P, M, phi_out, grad_out, cuda_stream);
 }
 
 extern "C" hsma_status hsma_fp64_peak(double seconds, double* tflops_out, double* sm_clock_mhz_out) {

@@ -57,7 +57,8 @@ struct NearArgs {
     long long units;     // U = ntb * n_tiles * C
     long long self_offset;  // >= 0: target t is source (self_offset + t); its bare term is skipped
     double scale;        // applied to the cell weights (0.5 for the Newton form, see below)
-    double* part;        // [part_rows][T] partial sums
+    double scale_grad;   // FIELD: weight of the gradient sums (-1/8 Newton, -1 cubic)
+    double* part;        // [part_rows][T] partial sums ([part_rows][4][T] in the FIELD form)
 };
 
 // One pair: acc += q / |d|.
@@ -109,13 +110,46 @@ __device__ __forceinline__ void pair_unit(double tx, double ty, double tz, doubl
     }
 }
 
+// Potential AND gradient (forces, Eq.(9)): with a = 2y (Newton) or y (cubic),
+//   phi += s q a,   G += s q a^3 d   (d = t - source; grad_t q/|d| = -q d/|d|^3: the sign and the powers of 2
+//   live in the cell weights).  SIGN 0: multiply by q (generic), +1/-1: all |q| equal, sign from the tile half.
+//   FP64-pipe instructions per pair: generic 16 (Newton) / 18 (cubic); uniform 15 / 17.
+template <int REFINE, int SIGN>
+__device__ __forceinline__ void pair_field(double tx, double ty, double tz, double sx, double sy, double sz, double sq,
+                                           double& acc, double& gx, double& gy, double& gz) {
+    const double dx = tx - sx, dy = ty - sy, dz = tz - sz;
+    const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+    const double y0 = rsqrt_seed(r2);
+    const double t = y0 * y0;
+    double k;
+    if (REFINE == 1) {
+        k = fma(-r2, t, kNewton3);
+    } else {
+        const double e = fma(-r2, t, 1.0);
+        const double h = fma(e, 0.375, 0.5);
+        k = fma(e, h, 1.0);
+    }
+    const double a = y0 * k;
+    const double u = SIGN == 0 ? sq * a : a;
+    const double v = u * (a * a);
+    if (SIGN >= 0) {
+        acc += u;
+        gx = fma(v, dx, gx); gy = fma(v, dy, gy); gz = fma(v, dz, gz);
+    } else {
+        acc -= u;
+        gx = fma(-v, dx, gx); gy = fma(-v, dy, gy); gz = fma(-v, dz, gz);
+    }
+}
+
 constexpr int near_min_ctas(int R) { return R >= 8 ? 1 : (R == 4 ? 2 : (R == 2 ? 3 : 4)); }
 
 // UNIFORM selects the loop form at compile time; the host launches both instantiations and the one that does
 // not match the device-side flag QInfo.uniform returns at once (no host synchronisation to pick a kernel,
 // and each instantiation keeps only its own loops: fewer live registers, better schedules).
-template <int R, int REFINE, bool UNIFORM>
-__global__ void __launch_bounds__(kThreads, near_min_ctas(R)) near_sum_kernel(const NearArgs a) {
+// FIELD: also accumulate the gradient; partial rows then hold 4 components per target, part[(row*4 + comp)*T + t],
+// comp 0 = phi, 1..3 = grad phi (in the frame of the ORIGINAL target: a reflected axis flips its component back).
+template <int R, int REFINE, bool UNIFORM, bool FIELD = false>
+__global__ void __launch_bounds__(kThreads, near_min_ctas(FIELD ? 2 * R : R)) near_sum_kernel(const NearArgs a) {
     __shared__ __align__(128) Src4 tile[kStages][kTile];
     __shared__ __align__(8) uint64_t full[kStages];
     __shared__ Cell cells[kMaxCells];
@@ -141,7 +175,9 @@ __global__ void __launch_bounds__(kThreads, near_min_ctas(R)) near_sum_kernel(co
     }
     const double qmag = UNIFORM ? a.qinfo->qmag : 1.0;
 
+    constexpr int RG = FIELD ? R : 1;  // gradient accumulators exist only in the FIELD form
     double ox[R], oy[R], oz[R], tot[R];
+    double totx[RG], toty[RG], totz[RG];
     // visits are walked with 32-bit state: block b, tile tl inside the block
     const int nvis = (int)(V1 - V0) + 1;
     const int nt = (int)a.n_tiles;
@@ -154,7 +190,14 @@ __global__ void __launch_bounds__(kThreads, near_min_ctas(R)) near_sum_kernel(co
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const long long t = (long long)blk * (kThreads * R) + r * kThreads + tid;
-            if (t < a.T) a.part[(long long)row * a.T + t] = tot[r];
+            if (t < a.T) {
+                if (FIELD) {
+                    double* o = a.part + (long long)row * 4 * a.T + t;
+                    o[0] = tot[r]; o[a.T] = totx[r % RG]; o[2 * a.T] = toty[r % RG]; o[3 * a.T] = totz[r % RG];
+                } else {
+                    a.part[(long long)row * a.T + t] = tot[r];
+                }
+            }
         }
     };
 
@@ -176,6 +219,7 @@ __global__ void __launch_bounds__(kThreads, near_min_ctas(R)) near_sum_kernel(co
                 const double* p = a.tgt + t * a.tstride;
                 ox[r] = p[0]; oy[r] = p[1]; oz[r] = p[2];
                 tot[r] = 0.0;
+                if (FIELD) { totx[r % RG] = 0.0; toty[r % RG] = 0.0; totz[r % RG] = 0.0; }
             }
         }
         const int np = a.tile_np[tl];
@@ -193,14 +237,17 @@ __global__ void __launch_bounds__(kThreads, near_min_ctas(R)) near_sum_kernel(co
         for (int c = c_lo; c < c_hi; ++c) {
             const Cell cell = cells[c];
             double tx[R], ty[R], tz[R], acc[R];
+            double gx[RG], gy[RG], gz[RG];
 #pragma unroll
             for (int r = 0; r < R; ++r) {
                 tx[r] = flip(ox[r] - cell.sx, cell.fx);
                 ty[r] = flip(oy[r] - cell.sy, cell.fy);
                 tz[r] = flip(oz[r] - cell.sz, cell.fz);
                 acc[r] = 0.0;
+                if (FIELD) { gx[r % RG] = 0.0; gy[r % RG] = 0.0; gz[r % RG] = 0.0; }
             }
             double w = cell.w * a.scale;
+            double wg = cell.w * a.scale_grad;
             if (cell.central && tile_has_self) {
                 // masked path: the pair (t, j = slot of source self_offset + t) has r2 = 0; give it r2 = 1, q = 0
                 int sj[R];
@@ -217,25 +264,36 @@ __global__ void __launch_bounds__(kThreads, near_min_ctas(R)) near_sum_kernel(co
 #pragma unroll
                     for (int r = 0; r < R; ++r) {
                         const bool self = j == sj[r];
-                        pair<REFINE>(tx[r], ty[r], tz[r], self ? tx[r] + 1.0 : xy.x, self ? ty[r] : xy.y,
-                                     self ? tz[r] : zq.x, self ? 0.0 : zq.y, acc[r]);
+                        if (FIELD)
+                            pair_field<REFINE, 0>(tx[r], ty[r], tz[r], self ? tx[r] + 1.0 : xy.x, self ? ty[r] : xy.y,
+                                                  self ? tz[r] : zq.x, self ? 0.0 : zq.y, acc[r], gx[r % RG], gy[r % RG], gz[r % RG]);
+                        else
+                            pair<REFINE>(tx[r], ty[r], tz[r], self ? tx[r] + 1.0 : xy.x, self ? ty[r] : xy.y,
+                                         self ? tz[r] : zq.x, self ? 0.0 : zq.y, acc[r]);
                     }
                 }
             } else if (UNIFORM) {
                 w *= qmag;
+                wg *= qmag;
 #pragma unroll kUnroll
                 for (int j = 0; j < np; ++j) {
                     const double2 xy = *reinterpret_cast<const double2*>(&s[j].x);
                     const double sz = s[j].z;
 #pragma unroll
-                    for (int r = 0; r < R; ++r) pair_unit<REFINE, false>(tx[r], ty[r], tz[r], xy.x, xy.y, sz, acc[r]);
+                    for (int r = 0; r < R; ++r) {
+                        if (FIELD) pair_field<REFINE, 1>(tx[r], ty[r], tz[r], xy.x, xy.y, sz, 1.0, acc[r], gx[r % RG], gy[r % RG], gz[r % RG]);
+                        else pair_unit<REFINE, false>(tx[r], ty[r], tz[r], xy.x, xy.y, sz, acc[r]);
+                    }
                 }
 #pragma unroll kUnroll
                 for (int j = np; j < nv; ++j) {
                     const double2 xy = *reinterpret_cast<const double2*>(&s[j].x);
                     const double sz = s[j].z;
 #pragma unroll
-                    for (int r = 0; r < R; ++r) pair_unit<REFINE, true>(tx[r], ty[r], tz[r], xy.x, xy.y, sz, acc[r]);
+                    for (int r = 0; r < R; ++r) {
+                        if (FIELD) pair_field<REFINE, -1>(tx[r], ty[r], tz[r], xy.x, xy.y, sz, 1.0, acc[r], gx[r % RG], gy[r % RG], gz[r % RG]);
+                        else pair_unit<REFINE, true>(tx[r], ty[r], tz[r], xy.x, xy.y, sz, acc[r]);
+                    }
                 }
             } else {
 #pragma unroll kUnroll
@@ -243,11 +301,21 @@ __global__ void __launch_bounds__(kThreads, near_min_ctas(R)) near_sum_kernel(co
                     const double2 xy = *reinterpret_cast<const double2*>(&s[j].x);
                     const double2 zq = *reinterpret_cast<const double2*>(&s[j].z);
 #pragma unroll
-                    for (int r = 0; r < R; ++r) pair<REFINE>(tx[r], ty[r], tz[r], xy.x, xy.y, zq.x, zq.y, acc[r]);
+                    for (int r = 0; r < R; ++r) {
+                        if (FIELD) pair_field<REFINE, 0>(tx[r], ty[r], tz[r], xy.x, xy.y, zq.x, zq.y, acc[r], gx[r % RG], gy[r % RG], gz[r % RG]);
+                        else pair<REFINE>(tx[r], ty[r], tz[r], xy.x, xy.y, zq.x, zq.y, acc[r]);
+                    }
                 }
             }
 #pragma unroll
-            for (int r = 0; r < R; ++r) tot[r] = fma(w, acc[r], tot[r]);
+            for (int r = 0; r < R; ++r) {
+                tot[r] = fma(w, acc[r], tot[r]);
+                if (FIELD) {
+                    totx[r % RG] = fma(wg, flip(gx[r % RG], cell.fx), totx[r % RG]);
+                    toty[r % RG] = fma(wg, flip(gy[r % RG], cell.fy), toty[r % RG]);
+                    totz[r % RG] = fma(wg, flip(gz[r % RG], cell.fz), totz[r % RG]);
+                }
+            }
         }
         __syncthreads();  // everyone is done with tile[st] before it is refilled
         if (++tl == nt) {   // next visit starts the next target block
@@ -267,14 +335,15 @@ struct NodeArgs {
     const Node8* nodes;  // padded to a multiple of kTile/2 with zero-strength records at kFar
     long long n_tiles;   // tiles of kTile/2 nodes (same 8 KB stage size)
     long long units;     // U = ntb * n_tiles (the decomposition above with C = 1)
-    double* part;        // [part_rows][T]
+    double* part;        // [part_rows][T] ([part_rows][4][T] in the FIELD form)
 };
 
 // phi(t) = sum_j Q_j/rho - P_j.(t - R_j)/rho^3  = sum_j y (Q_j - (P_j.d) y^2),  y = 1/rho,
 // with the exact normal dipole P_j = D_j n_j (reading S9).  y by the cubic step (relative ~1e-19
 // before rounding).  3 DADD + 3 (r2) + 5 (rsqrt) + 3 (P.d) + DMUL (y^2) + DFMA + DFMA = 17 FP64 instructions.
-template <int R>
-__global__ void __launch_bounds__(kThreads, near_min_ctas(R)) node_sum_kernel(const NodeArgs a) {
+// FIELD: also grad phi = y^3 [ (3 (P.d) y^2 - Q) d - P ]  (+ DMUL y^3, DMUL 3 y^2, DFMA, 3 DFMA, 3 DFMA = 26).
+template <int R, bool FIELD = false>
+__global__ void __launch_bounds__(kThreads, near_min_ctas(FIELD ? 2 * R : R)) node_sum_kernel(const NodeArgs a) {
     constexpr int kNT = kTile / 2;
     __shared__ __align__(128) Node8 tile[kStages][kNT];
     __shared__ __align__(8) uint64_t full[kStages];
@@ -291,14 +360,23 @@ __global__ void __launch_bounds__(kThreads, near_min_ctas(R)) node_sum_kernel(co
         mbar_expect_tx(&full[0], kNT * sizeof(Node8));
         bulk_g2s(tile[0], a.nodes + (V0 % a.n_tiles) * kNT, kNT * sizeof(Node8), &full[0]);
     }
+    constexpr int RG = FIELD ? R : 1;
     double tx[R], ty[R], tz[R], acc[R];
+    double gx[RG], gy[RG], gz[RG];
     long long cur_b = -1;
     auto store_block = [&](long long b) {
         const int row = k - cta_of_unit(b * a.n_tiles, a.units, G);
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const long long t = b * (kThreads * R) + r * kThreads + tid;
-            if (t < a.T) a.part[(long long)row * a.T + t] = acc[r];
+            if (t < a.T) {
+                if (FIELD) {
+                    double* o = a.part + (long long)row * 4 * a.T + t;
+                    o[0] = acc[r]; o[a.T] = gx[r % RG]; o[2 * a.T] = gy[r % RG]; o[3 * a.T] = gz[r % RG];
+                } else {
+                    a.part[(long long)row * a.T + t] = acc[r];
+                }
+            }
         }
     };
     for (long long v = V0; v <= V1; ++v) {
@@ -319,6 +397,7 @@ __global__ void __launch_bounds__(kThreads, near_min_ctas(R)) node_sum_kernel(co
                 const double* p = a.tgt + t * a.tstride;
                 tx[r] = p[0]; ty[r] = p[1]; tz[r] = p[2];
                 acc[r] = 0.0;
+                if (FIELD) { gx[r % RG] = 0.0; gy[r % RG] = 0.0; gz[r % RG] = 0.0; }
             }
         }
         mbar_wait(&full[st], (it >> 1) & 1);
@@ -335,8 +414,16 @@ __global__ void __launch_bounds__(kThreads, near_min_ctas(R)) node_sum_kernel(co
                 const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
                 const double y = rsqrt_cubic(r2);
                 const double pd = fma(pz, dz, fma(pxy.y, dy, pxy.x * dx));
-                const double u = fma(-pd, y * y, zq.y);
+                const double y2 = y * y;
+                const double u = fma(-pd, y2, zq.y);
                 acc[r] = fma(y, u, acc[r]);
+                if (FIELD) {
+                    const double y3 = y2 * y;
+                    const double c = fma(3.0 * y2, pd, -zq.y);       // 3 (P.d) y^2 - Q
+                    gx[r % RG] = fma(y3, fma(c, dx, -pxy.x), gx[r % RG]);
+                    gy[r % RG] = fma(y3, fma(c, dy, -pxy.y), gy[r % RG]);
+                    gz[r % RG] = fma(y3, fma(c, dz, -pz), gz[r % RG]);
+                }
             }
         }
         __syncthreads();
@@ -433,6 +520,46 @@ __device__ __forceinline__ double sum_part_rows(const PartLayout& L, long long t
     for (int k = 0; k <= last - first; ++k) s += L.part[(long long)k * T + t];
     return s;
 }
+// FIELD form of the finish: phi, force F_i = -q_i grad phi(r_i) or, without charges, grad phi itself.
+__device__ __forceinline__ void sum_part_rows4(const PartLayout& L, long long t, long long T, double out[4]) {
+    if (!L.part) return;
+    const long long b = t / L.block_targets;
+    const int first = cta_of_unit(b * L.Ub, L.U, L.G), last = cta_of_unit((b + 1) * L.Ub - 1, L.U, L.G);
+    for (int k = 0; k <= last - first; ++k)
+#pragma unroll
+        for (int c = 0; c < 4; ++c) out[c] += L.part[((long long)k * 4 + c) * T + t];
+}
+__global__ void finish_field_kernel(const PartLayout Lb, const PartLayout Lc, long long T,
+                                    const Src4* __restrict__ src, const int* __restrict__ slot_of, long long t_first,
+                                    double* __restrict__ phi, double* __restrict__ vec /* [T,3] */,
+                                    double* __restrict__ u_part /* [gridDim.x] or null */) {
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    double e = 0.0;
+    if (t < T) {
+        double sb[4] = {0.0, 0.0, 0.0, 0.0}, sc[4] = {0.0, 0.0, 0.0, 0.0};
+        sum_part_rows4(Lb, t, T, sb);
+        sum_part_rows4(Lc, t, T, sc);
+        const double v = sb[0] + sc[0];
+        if (phi) phi[t] = v;
+        const double qi = src ? src[slot_of[t_first + t]].q : -1.0;   // no charges: write +grad
+        vec[3 * t] = -qi * (sb[1] + sc[1]); vec[3 * t + 1] = -qi * (sb[2] + sc[2]); vec[3 * t + 2] = -qi * (sb[3] + sc[3]);
+        if (src) e = qi * v;
+    }
+    if (u_part) {
+        __shared__ double sh[32];
+        for (int o = 16; o; o >>= 1) e += __shfl_down_sync(0xffffffffu, e, o);
+        const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+        if (l == 0) sh[w] = e;
+        __syncthreads();
+        if (w == 0) {
+            const int nw = blockDim.x >> 5;
+            e = l < nw ? sh[l] : 0.0;
+            for (int o = 16; o; o >>= 1) e += __shfl_down_sync(0xffffffffu, e, o);
+            if (l == 0) u_part[blockIdx.x] = e;
+        }
+    }
+}
+
 __global__ void finish_phi_kernel(const PartLayout Lb, const PartLayout Lc, long long T,
                                   const Src4* __restrict__ src, const int* __restrict__ slot_of, long long t_first,
                                   double* __restrict__ phi, double* __restrict__ u_part /* [gridDim.x] or null */) {

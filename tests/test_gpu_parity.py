@@ -264,7 +264,8 @@ def test_shards_and_host_path_agree(H):
             ph, u = plan.evaluate_shard(xyz, q, a, b, sync=True)
             parts.append(ph.cpu().numpy())
             Us += float(u.cpu().numpy()[0])
-        assert np.array_equal(np.concatenate(parts), phi.cpu().numpy())
+        # rounding only: the split points of the partial sums move with the shard
+        assert np.max(np.abs(np.concatenate(parts) - phi.cpu().numpy())) <= 1e-13 * float(phi.abs().max())
         assert abs(Us - float(U.cpu().numpy()[0])) < 1e-12 * abs(Us)
         ph_h, U_h = plan.evaluate_host(np.ascontiguousarray(w.xyz), np.ascontiguousarray(w.q))
         assert np.array_equal(ph_h, phi.cpu().numpy())
