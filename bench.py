@@ -38,6 +38,13 @@ FLOPS_PAIR_DIPOLE = 26.0      # + P.d (DMUL + 2 DFMA) + y^2 (DMUL) + DFMA
 # what near_sum_kernel<R, REFINE> executes per pair (FP64-pipe instructions, flops), DESIGN.md 6.1/6.4:
 # (refine, all |q| equal) -> the uniform-|q| path drops the multiplication by q
 EXEC_PAIR = {(1, False): (10.0, 14.0), (2, False): (12.0, 18.0), (1, True): (9.0, 13.0), (2, True): (11.0, 17.0)}
+# --forces: the potential+gradient form of the same kernel: (instructions, flops) executed per pair;
+# algorithmic: the charge pair (18) + q y^3 (2 mul) + 3 fma = 26 flops
+EXEC_PAIR_FIELD = {(1, False): (16.0, 22.0), (2, False): (18.0, 26.0), (1, True): (15.0, 21.0), (2, True): (17.0, 25.0)}
+FLOPS_PAIR_CHARGE_FIELD = 26.0
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel from the committed ncu --set full
+# capture (profiles/r01_ncu_near_sum_N262144.md): valid for config 5 at N = 262,144 on one GPU, potential only
+NCU_TRAFFIC_BYTES_CFG5 = 9555200
 # FP64 peak derived from unit counts and clocks: SMs x 64 DFMA lanes x 2 x clock
 FP64_LANES_PER_SM = 64
 
@@ -225,11 +232,15 @@ def run_b200(args, w) -> dict:
     q = torch.as_tensor(np.ascontiguousarray(w.q), device=dev)
     phi = torch.empty(T, dtype=torch.float64, device=dev)
     U = torch.empty(1, dtype=torch.float64, device=dev)
+    force = torch.empty(T, 3, dtype=torch.float64, device=dev) if args.forces else None
     flush = torch.empty(256 * 1024 * 1024 // 8, dtype=torch.float64, device=dev)   # 256 MiB > 126 MB L2
 
     def step():
         flush.zero_()                                     # L2 flush between iterations (torch memset, not counted)
-        H.hsma_evaluate_shard(plan.handle, xyz, q, t0, t1, phi, U)
+        if args.forces:
+            H.hsma_evaluate_forces_shard(plan.handle, xyz, q, t0, t1, phi, force, U)
+        else:
+            H.hsma_evaluate_shard(plan.handle, xyz, q, t0, t1, phi, U)
         if world > 1:                                     # the exchange step: assemble phi and U on every rank
             full = shard.all_gather_phi(phi, N)
             shard.all_reduce_energy(U)
@@ -279,10 +290,14 @@ def run_b200(args, w) -> dict:
     phi_h = torch.empty(max(T, 1), dtype=torch.float64).pin_memory()
     U_h = torch.empty(1, dtype=torch.float64).pin_memory()
     xyz_n, q_n, phi_n, U_n = xyz_h.numpy(), q_h.numpy(), phi_h.numpy(), U_h.numpy()
+    force_n = torch.empty(max(T, 1), 3, dtype=torch.float64).pin_memory().numpy() if args.forces else None
 
     def step_e2e():
         flush.zero_()
-        H.hsma_evaluate_shard_host(plan.handle, xyz_n, q_n, t0, t1, phi_n, U_n)   # synchronises (returns host data)
+        if args.forces and world == 1:
+            H.hsma_evaluate_forces_host(plan.handle, xyz_n, q_n, phi_n, force_n, U_n)
+        else:
+            H.hsma_evaluate_shard_host(plan.handle, xyz_n, q_n, t0, t1, phi_n, U_n)   # synchronises (returns host data)
 
     n_e2e = max(1, min(args.steps, args.e2e_steps))
     step_e2e()
@@ -297,8 +312,9 @@ def run_b200(args, w) -> dict:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         ms_e2e = float(t[0])
     e2e = {"value": pairs_step / (ms_e2e * 1e-3), "unit": UNIT, "ms_per_step": ms_e2e, "steps": n_e2e,
-           "h2d_bytes_per_step": int(xyz_n.nbytes + q_n.nbytes), "d2h_bytes_per_step": int(8 * T + 8),
-           "api": "hsma_evaluate_shard_host (pinned host buffers; per rank: all sources in, its phi shard and U out)"}
+           "h2d_bytes_per_step": int(xyz_n.nbytes + q_n.nbytes), "d2h_bytes_per_step": int(8 * T + 8 + (24 * T if args.forces and world == 1 else 0)),
+           "api": ("hsma_evaluate_forces_host" if args.forces and world == 1 else "hsma_evaluate_shard_host") +
+                  " (pinned host buffers; per rank: all sources in, its phi shard and U out)"}
 
     # roofline of the dominant kernel: near_sum_kernel over the sources, step (b)
     pc_rank = pair_counts(info, N, T)
@@ -311,15 +327,19 @@ def run_b200(args, w) -> dict:
         pass
     sm_max_mhz = float(peaks.get("sm_max_mhz") or clocks.get("sm_max_mhz") or 1965.0)
     peak_tf = sm_count * FP64_LANES_PER_SM * 2 * sm_max_mhz * 1e6 * 1e-12
-    ach_tf = pc_rank["b"] * FLOPS_PAIR_CHARGE / (k_ms * 1e-3) * 1e-12 if k_ms > 0 else 0.0
+    alg_flops_early = FLOPS_PAIR_CHARGE_FIELD if args.forces else FLOPS_PAIR_CHARGE
+    ach_tf = pc_rank["b"] * alg_flops_early / (k_ms * 1e-3) * 1e-12 if k_ms > 0 else 0.0
     uniform_q = bool(np.all(np.abs(w.q) == abs(w.q[0])))
-    ex_instr, ex_flops = EXEC_PAIR[(refine, uniform_q)]
+    ex_instr, ex_flops = (EXEC_PAIR_FIELD if args.forces else EXEC_PAIR)[(refine, uniform_q)]
+    alg_flops = FLOPS_PAIR_CHARGE_FIELD if args.forces else FLOPS_PAIR_CHARGE
+    traffic = NCU_TRAFFIC_BYTES_CFG5 if (args.config == 5 and args.size is None and world == 1 and not args.forces) else None
     issue_peak = sm_count * FP64_LANES_PER_SM * sm_max_mhz * 1e6          # FP64-pipe thread-instructions/s
-    roofline = {"bound": "alu", "kernel": f"near_sum_kernel<R,{refine}> step (b), {'uniform-|q|' if uniform_q else 'generic'} path", "achieved": ach_tf, "peak": peak_tf,
-                "unit": "TFLOP/s", "frac": ach_tf / peak_tf, "traffic": None,
+    roofline = {"bound": "alu", "kernel": f"near_sum_kernel<R,{refine},{'uniform-|q|' if uniform_q else 'generic'},{'field' if args.forces else 'potential'}> step (b)", "achieved": ach_tf, "peak": peak_tf,
+                "unit": "TFLOP/s", "frac": ach_tf / peak_tf, "traffic": traffic,
+                "traffic_source": "profiles/r01_ncu_near_sum_N262144.md (dram read+write bytes of one launch)" if traffic else None,
                 "peak_source": f"derived: {sm_count} SMs x {FP64_LANES_PER_SM} FP64 lanes x 2 x {sm_max_mhz:.0f} MHz "
                                f"(no FP64 entry in MEASURED_PEAKS.json)",
-                "flops_per_pair_algorithmic": FLOPS_PAIR_CHARGE, "pairs_per_launch": pc_rank["b"],
+                "flops_per_pair_algorithmic": alg_flops, "pairs_per_launch": pc_rank["b"],
                 "kernel_ms": k_ms, "kernel_pairs_per_s": pc_rank["b"] / (k_ms * 1e-3) if k_ms > 0 else 0.0,
                 "kernel_share_of_step": k_ms / stage_ms["total"] if stage_ms["total"] > 0 else None,
                 "flops_per_pair_executed": ex_flops, "fp64_instr_per_pair_executed": ex_instr,
@@ -331,7 +351,7 @@ def run_b200(args, w) -> dict:
            "ms_per_step": ms, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64",
            "data": "synthetic",
            "config": {"workload": w.name, "N": N, "near_cells": info["near_cells"], "p": info["p"], "M": info["M"],
-                      "check_targets": info["check_targets"], "pairs_per_step": pc_all, "rsqrt_refine": refine,
+                      "check_targets": info["check_targets"], "pairs_per_step": pc_all, "rsqrt_refine": refine, "forces": bool(args.forces),
                       "parallelism": f"targets sharded over {world} rank(s), sources replicated",
                       "l2": "256 MiB flush written between iterations"},
            "energy": U_val, "stage_ms": stage_ms, "e2e": e2e, "gpu_launches": int(launches),
@@ -350,6 +370,7 @@ def main():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--config", type=int, default=5, help="BASELINE.json configs[config-1]; 5 = the metric's workload")
     ap.add_argument("--size", type=int, default=None, help="override N (same generator and seed)")
+    ap.add_argument("--forces", action="store_true", help="time hsma_evaluate_forces (potential + forces) instead")
     ap.add_argument("--refine", type=int, default=0, choices=[0, 1, 2], help="hsma_plan_desc.rsqrt_refine")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--peak-seconds", type=float, default=1.0)
