@@ -150,35 +150,50 @@ __global__ void __launch_bounds__(1024) householder_qr_kernel(double* __restrict
     }
 }
 
-// H3: rhs from the check-point sums, c = Q^T rhs, back-substitution R A = c.  Single block.
-//   pc [K_t] check-point potentials; pairs: rhs_i = sgn (pc[i] - pc[rows+i]); else rhs_i = sgn pc[i]
-//   A_full [p*p] in the R0-scaled basis (A_00 = 0 when the constant column was dropped)
-__global__ void __launch_bounds__(1024) ls_solve_kernel(const double* __restrict__ pc, int rows, int ncol, int pairs,
-                                                        double sgn, const double* __restrict__ Qm,
-                                                        const double* __restrict__ Rm, double* __restrict__ rhs,
-                                                        double* __restrict__ cvec, double* __restrict__ A_full) {
-    extern __shared__ double c[];  // [ncol]
-    for (int i = threadIdx.x; i < rows; i += blockDim.x) rhs[i] = sgn * (pairs ? pc[i] - pc[rows + i] : pc[i]);
-    __syncthreads();
-    const int w = threadIdx.x >> 5, l = threadIdx.x & 31, nw = blockDim.x >> 5;
-    for (int j = w; j < ncol; j += nw) {
-        const double* col = Qm + (size_t)j * rows;
-        double s = 0.0;
-        for (int i = l; i < rows; i += 32) s += col[i] * rhs[i];
-        s = warp_sum(s);
-        if (l == 0) { c[j] = s; cvec[j] = s; }
-    }
-    __syncthreads();
+// Plan time: Pinv = R^-1 Q^T  [ncol x rows], row j contiguous (Pinv[j*rows + i]).  One thread per row i of F
+// (column i of Q^T) back-substitutes R x = Q^T e_i; R is read uniformly (cache broadcast), x lives in Pinv.
+// With it the update step solves Eq.(7) PAPER.md:76 as one parallel mat-vec A = Pinv rhs instead of a single-block
+// Q^T b + back-substitution (0.1-0.45 ms of pure latency per evaluate).  cond(F) <= 2e3 in every configuration,
+// so the explicit pseudo-inverse costs cond * eps ~ 1e-13 relative: far inside the parity bars.
+__global__ void pinv_kernel(const double* __restrict__ Qm, const double* __restrict__ Rm, int rows, int ncol,
+                            double* __restrict__ Pinv) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= rows) return;
     for (int k = ncol - 1; k >= 0; --k) {
-        const double ak = c[k] / Rm[(size_t)k * ncol + k];
-        __syncthreads();
-        for (int i = threadIdx.x; i < k; i += blockDim.x) c[i] -= Rm[(size_t)k * ncol + i] * ak;
-        if (threadIdx.x == 0) c[k] = ak;
-        __syncthreads();
+        double s = Qm[(size_t)k * rows + i];
+        for (int j = k + 1; j < ncol; ++j) s -= Rm[(size_t)j * ncol + k] * Pinv[(size_t)j * rows + i];
+        Pinv[(size_t)k * rows + i] = s / Rm[(size_t)k * ncol + k];
     }
+}
+
+// H3 (update step): rhs from the check-point sums, A = Pinv rhs.  One warp per coefficient, 8 warps per block;
+// block 0 also stores rhs.  Fixed summation order (lane-strided partial sums, xor-shuffle tree).
+__global__ void __launch_bounds__(256) ls_apply_kernel(const double* __restrict__ pc, int rows, int ncol, int pairs,
+                                                       double sgn, const double* __restrict__ Pinv,
+                                                       double* __restrict__ rhs, double* __restrict__ A_full) {
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    const int j = blockIdx.x * 8 + w;
+    if (blockIdx.x == 0)
+        for (int i = threadIdx.x; i < rows; i += blockDim.x) rhs[i] = sgn * (pairs ? pc[i] - pc[rows + i] : pc[i]);
     const int drop = pairs ? 1 : 0;
-    if (threadIdx.x == 0 && drop) A_full[0] = 0.0;
-    for (int j = threadIdx.x; j < ncol; j += blockDim.x) A_full[j + drop] = c[j];
+    if (j < ncol) {
+        const double* row = Pinv + (size_t)j * rows;
+        double s = 0.0;
+        for (int i = l; i < rows; i += 32) s += row[i] * (sgn * (pairs ? pc[i] - pc[rows + i] : pc[i]));
+        s = warp_sum(s);
+        if (l == 0) A_full[j + drop] = s;
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0 && drop) A_full[0] = 0.0;
+}
+
+// c = R A (the Q^T rhs of the fitted part), for the residual below.  Single block.
+__global__ void r_times_a_kernel(const double* __restrict__ Rm, const double* __restrict__ A_full, int ncol, int drop,
+                                 double* __restrict__ cvec) {
+    for (int j = threadIdx.x; j < ncol; j += blockDim.x) {
+        double s = 0.0;
+        for (int k = j; k < ncol; ++k) s += Rm[(size_t)k * ncol + j] * A_full[k + drop];
+        cvec[j] = s;
+    }
 }
 
 // residual of the fit: out[0] = || rhs - Q c ||_2 / sqrt(rows).  Single block.

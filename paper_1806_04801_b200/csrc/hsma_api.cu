@@ -208,7 +208,7 @@ struct hsma_plan {
     double* nrm = nullptr;       // [M,3]
     double* wq = nullptr;        // [M]
     Node8* nodes = nullptr;      // packed, padded
-    double *Fm = nullptr, *tau = nullptr, *Qm = nullptr, *Rm = nullptr;
+    double *Fm = nullptr, *tau = nullptr, *Qm = nullptr, *Rm = nullptr, *Pinv = nullptr;
     double *pc = nullptr, *rhs = nullptr, *cvec = nullptr, *A_full = nullptr, *scalars = nullptr;  // scalars[8]
     int* flags = nullptr;        // [0] rank deficient, [1] not neutral
     // scratch grown to the largest N seen
@@ -230,7 +230,7 @@ struct hsma_plan {
 static void plan_free(hsma_plan* p) {
     if (!p) return;
     if (p->cells_rhs && p->cells_rhs != p->cells_near) cudaFree(p->cells_rhs);
-    void* ptrs[] = {p->cells_near, p->chk, p->nrm, p->wq, p->nodes, p->Fm, p->tau, p->Qm, p->Rm,
+    void* ptrs[] = {p->cells_near, p->chk, p->nrm, p->wq, p->nodes, p->Fm, p->tau, p->Qm, p->Rm, p->Pinv,
                     p->pc, p->rhs, p->cvec, p->A_full, p->scalars, p->flags};
     for (void* q : ptrs) if (q) cudaFree(q);
     p->src.release(); p->slot_of.release(); p->tile_np.release(); if (p->qinfo) cudaFree(p->qinfo);
@@ -340,6 +340,7 @@ extern "C" hsma_status hsma_plan_create_ex(const hsma_plan_desc* desc, void* cud
     PCU(cudaMalloc(&p->Fm, mn * sizeof(double)));
     PCU(cudaMalloc(&p->Qm, mn * sizeof(double)));
     PCU(cudaMalloc(&p->Rm, (size_t)p->ncol * p->ncol * sizeof(double)));
+    PCU(cudaMalloc(&p->Pinv, mn * sizeof(double)));
     PCU(cudaMalloc(&p->tau, p->ncol * sizeof(double)));
     PCU(cudaMalloc(&p->pc, p->Kt * sizeof(double)));
     PCU(cudaMalloc(&p->rhs, p->rows * sizeof(double)));
@@ -353,6 +354,8 @@ extern "C" hsma_status hsma_plan_create_ex(const hsma_plan_desc* desc, void* cud
     build_fit_matrix_kernel<<<(p->rows + 127) / 128, 128, 0, st>>>(p->chk, p->rows, p->pairs ? 1 : 0, d.p, 1.0 / R0, p->Fm);
     HSMA_COUNT_LAUNCH();
     householder_qr_kernel<<<1, 1024, 0, st>>>(p->Fm, p->rows, p->ncol, p->tau, p->Qm, p->Rm, p->flags);
+    HSMA_COUNT_LAUNCH();
+    pinv_kernel<<<(p->rows + 63) / 64, 64, 0, st>>>(p->Qm, p->Rm, p->rows, p->ncol, p->Pinv);
     HSMA_COUNT_LAUNCH();
     int hflags[4] = {0, 0, 0, 0};
     PCU(cudaMemcpyAsync(hflags, p->flags, sizeof(hflags), cudaMemcpyDeviceToHost, st));
@@ -439,8 +442,8 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
         HSMA_COUNT_LAUNCH();
     }
     // H3: least squares, Eq.(7)
-    ls_solve_kernel<<<1, 1024, p->ncol * sizeof(double), st>>>(p->pc, p->rows, p->ncol, p->pairs ? 1 : 0, p->rhs_sign,
-                                                               p->Qm, p->Rm, p->rhs, p->cvec, p->A_full);
+    ls_apply_kernel<<<(p->ncol + 7) / 8, 256, 0, st>>>(p->pc, p->rows, p->ncol, p->pairs ? 1 : 0, p->rhs_sign, p->Pinv, p->rhs,
+                                                       p->A_full);
     HSMA_COUNT_LAUNCH();
     // H4: harmonic surface mapping, Eq.(10),(11) PAPER.md:99-105
     surface_mapping_kernel<<<(d.M + 127) / 128, 128, 0, st>>>(p->A_full, d.p, d.R_aux / p->R0, d.R_aux, p->nrm, p->wq,
@@ -620,8 +623,9 @@ extern "C" hsma_status hsma_get_surface(hsma_plan* p, double* Q_out, double* P_o
 }
 extern "C" hsma_status hsma_get_fit_residual(hsma_plan* p, double* rms_out) {
     if (!p || !rms_out) return HSMA_ERR_INVALID_ARG;
+    r_times_a_kernel<<<1, 256, 0, p->stream>>>(p->Rm, p->A_full, p->ncol, p->pairs ? 1 : 0, p->cvec);
     fit_residual_kernel<<<1, 1024, 0, p->stream>>>(p->rhs, p->rows, p->ncol, p->Qm, p->cvec, p->scalars + 4);
-    HSMA_COUNT_LAUNCH();
+    HSMA_COUNT_LAUNCH(); HSMA_COUNT_LAUNCH();
     CU(cudaMemcpyAsync(rms_out, p->scalars + 4, sizeof(double), cudaMemcpyDeviceToHost, p->stream));
     CU(cudaStreamSynchronize(p->stream));
     return HSMA_OK;
