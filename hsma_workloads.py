@@ -37,6 +37,14 @@ CLOSURE_FAR_DATA = 1   # explicit far-cell data at the check points (DESIGN.md r
 QUAD_SPIRAL = 0        # exactly M nodes (reading S10)
 QUAD_LATTICE = 1       # the paper's F1/F2 lattice, M = 2(F2+1)
 
+# near set (values match include/hsma.h)
+NEAR_WHOLE_CELLS = 0   # every image of the neighbour cells (reading S7, north_star)
+NEAR_SPHERE = 1        # paper-literal: only the images inside the auxiliary sphere
+
+# dipole layer (values match include/hsma.h)
+DIPOLE_EXACT = 0       # exact normal dipole on M nodes (reading S9)
+DIPOLE_FD3 = 1         # paper-literal: central difference over three spheres, 3M charges (Eq.12-14)
+
 
 @dataclass
 class Workload:
@@ -55,6 +63,9 @@ class Workload:
     far_shell: tuple = (0, 0, 0)
     closure: int = CLOSURE_BOUNDARY
     quad_rule: int = QUAD_SPIRAL
+    near_mode: int = NEAR_WHOLE_CELLS
+    dipole_mode: int = DIPOLE_EXACT
+    fd_dr_rel: float = 1e-5   # Delta r / R_s of the three-sphere form
     meta: dict = field(default_factory=dict)
 
     @property
@@ -143,6 +154,24 @@ def config(idx: int, N: Optional[int] = None, **overrides) -> Workload:
     if N is not None:
         w.name += f"_N{N}"
     return w.with_(**overrides) if overrides else w
+
+
+def paper_timing(N: int, seed: int = 5, alpha: float = 1.3, P: int = 25, F2: int = 987) -> Workload:
+    """The paper's timing workload: N unit charges of random sign on the sites of a uniformly
+    spaced lattice in the unit cube (neutral), PBC, alpha = 1.3, P = 25 (p = 26 degrees), N_o = 3 x 2(F2+1) = 5928
+    images on three spheres, N_m = 2 P^2 monitoring points, near set = the images inside the sphere.
+    N must be a perfect cube with an even number of sites."""
+    n = round(N ** (1.0 / 3.0))
+    if n ** 3 != N or N % 2:
+        raise ValueError("N must be an even perfect cube")
+    g = (np.arange(n) + 0.5) / n
+    X, Y, Z = np.meshgrid(g, g, g, indexing="ij")
+    xyz = np.stack([X.ravel(), Y.ravel(), Z.ravel()], axis=1)
+    q = np.ones(N)
+    q[np.random.default_rng(seed).permutation(N)[: N // 2]] = -1.0
+    return Workload(f"paper_timing_N{N}", BC_PERIODIC, (1.0, 1.0, 1.0), (1, 1, 1), 1.0, alpha * math.sqrt(3.0) / 2.0,
+                    P + 1, 2 * (F2 + 1), 2 * P * P, xyz, q, quad_rule=QUAD_LATTICE, near_mode=NEAR_SPHERE,
+                    dipole_mode=DIPOLE_FD3)
 
 
 def paper_example2() -> Workload:

@@ -32,6 +32,8 @@ _LIB = None
 BC_PERIODIC, BC_MIRROR_CAVITY, BC_SLAB = 0, 1, 2
 CLOSURE_BOUNDARY, CLOSURE_FAR_DATA = 0, 1
 QUAD_SPIRAL, QUAD_LATTICE = 0, 1
+NEAR_WHOLE_CELLS, NEAR_SPHERE = 0, 1
+DIPOLE_EXACT, DIPOLE_FD3 = 0, 1
 
 
 # --------------------------------------------------------------------------------------
@@ -178,6 +180,28 @@ def node_grad(tgt, R, nrm, Q, D) -> np.ndarray:
         return g
     _lib().oracle_node_grad(_p(tgt), tgt.shape[0], _p(R), _p(nrm), _p(Q), _p(D), R.shape[0], _p(g))
     return g
+
+
+def images_inside_sphere(src, q, cells: CellTable, R: float):
+    """Paper-literal near set: "the set of those charges within the sphere, where the first N
+    charges are the sources and the remaining N_s - N are the images near the central box".  Every image
+    sign o r_j + k L of the cell table with |image| <= R, carrying charge w_c q_j; the central cell comes first
+    and in source order (the box lies inside the sphere), so image i < N is source i."""
+    src, q = _c(src), _c(q)
+    order = [cells.central] + [c for c in range(cells.w.shape[0]) if c != cells.central]
+    pos, chg = [], []
+    for c in order:
+        p = cells.sign[c] * src + cells.shift[c]
+        keep = (p * p).sum(axis=1) <= R * R
+        if c == cells.central and not keep.all():
+            raise ValueError("a source lies outside the auxiliary sphere")
+        pos.append(p[keep])
+        chg.append(cells.w[c] * q[keep])
+    return np.concatenate(pos, axis=0), np.concatenate(chg)
+
+
+def identity_cell() -> CellTable:
+    return CellTable(np.zeros((1, 3), dtype=np.int64), np.zeros((1, 3)), np.ones((1, 3)), np.ones(1), 0)
 
 
 def energy(q, phi) -> float:
@@ -391,6 +415,8 @@ def hsma(w, targets_slice: Optional[slice] = None, dipole: str = "exact", dr_rel
     (the paper's three-sphere central difference, Eq.12-14, cross-check)."""
     p = int(p if p is not None else w.p)
     M = int(M if M is not None else w.M)
+    if getattr(w, "dipole_mode", DIPOLE_EXACT) == DIPOLE_FD3 and dipole == "exact":
+        dipole, dr_rel = "fd3", float(getattr(w, "fd_dr_rel", dr_rel))
     L = np.asarray(w.L, dtype=np.float64)
     R0 = validate_geometry(L, w.near_shell, w.R_aux)
     # -- centre the box at the origin (PAPER.md:62 "same center at the origin"; reading G10)
@@ -404,6 +430,15 @@ def hsma(w, targets_slice: Optional[slice] = None, dipole: str = "exact", dr_rel
 
     # -- preparation step, PAPER.md:140 ----------------------------------------------------
     near = cell_table(w.kind, L, w.near_shell, w.gamma)
+    # paper-literal near set: the images inside the sphere, as an explicit list summed with the
+    # identity cell; otherwise the whole cells of the table (reading S7)
+    sphere = getattr(w, "near_mode", NEAR_WHOLE_CELLS) == NEAR_SPHERE
+    if sphere:
+        if w.closure != CLOSURE_BOUNDARY:
+            raise ValueError("the sphere-culled near set is defined for the boundary closure")
+        near_src, near_q, near_cells = (*images_inside_sphere(src, q, near, w.R_aux), identity_cell())
+    else:
+        near_src, near_q, near_cells = src, q, near
     if periodic:
         if w.closure != CLOSURE_BOUNDARY:
             raise ValueError("periodic kind uses the boundary closure")
@@ -437,7 +472,7 @@ def hsma(w, targets_slice: Optional[slice] = None, dipole: str = "exact", dr_rel
         rhs = phi_check.copy()                            # Phi_out := field of the far cells (S16)
         n_check_cells = far.w.shape[0]
     else:
-        phi_check = near_sum(check_targets, src, q, near)
+        phi_check = near_sum(check_targets, near_src, near_q, near_cells)
         n_check_cells = near.w.shape[0]
         if periodic:
             K = x.shape[0]
@@ -462,7 +497,7 @@ def hsma(w, targets_slice: Optional[slice] = None, dipole: str = "exact", dr_rel
     sl = targets_slice if targets_slice is not None else slice(0, N)
     i0, i1, _ = sl.indices(N)
     tg = src[i0:i1]
-    phi_near = near_sum(tg, src, q, near, self_offset=i0)
+    phi_near = near_sum(tg, near_src, near_q, near_cells, self_offset=i0)
     if dipole == "exact":
         phi_out = node_sum(tg, nodes, nrm, Q, D)
     elif dipole == "fd3":
@@ -477,8 +512,9 @@ def hsma(w, targets_slice: Optional[slice] = None, dipole: str = "exact", dr_rel
         raise ValueError(dipole)
     phi = phi_near + phi_out
     U = energy(q[i0:i1], phi)
-    pairs = {"a": int(check_targets.shape[0]) * N * int(n_check_cells),
-             "b": int(i1 - i0) * N * int(near.w.shape[0]),
+    n_near = int(near_src.shape[0]) if sphere else N * int(near.w.shape[0])
+    pairs = {"a": int(check_targets.shape[0]) * (n_near if sphere else N * int(n_check_cells)),
+             "b": int(i1 - i0) * n_near,
              "c": int(i1 - i0) * int(nodes.shape[0])}
     res = OracleResult(phi, U, A, rhs, fit_rms, float(sv[0] / sv[-1]), phi_near, phi_out,
                        check_targets, phi_check, Q, D, nodes, nrm, pairs)
@@ -487,7 +523,7 @@ def hsma(w, targets_slice: Optional[slice] = None, dipole: str = "exact", dr_rel
         # coefficients A_nm held fixed; the image gradient uses the exact dipole layer (reading S9)
         if dipole != "exact":
             raise ValueError("forces are implemented for the exact dipole layer")
-        res.grad = near_grad(tg, src, q, near, self_offset=i0) + node_grad(tg, nodes, nrm, Q, D)
+        res.grad = near_grad(tg, near_src, near_q, near_cells, self_offset=i0) + node_grad(tg, nodes, nrm, Q, D)
         res.F = -q[i0:i1, None] * res.grad
     return res
 
