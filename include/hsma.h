@@ -59,6 +59,19 @@ typedef enum {
     HSMA_QUAD_LATTICE = 1 /* the paper's F1/F2 lattice, M = 2(F2+1), PAPER.md:124-126 (reading G4)   */
 } hsma_quad_rule;
 
+typedef enum {
+    HSMA_NEAR_WHOLE_CELLS = 0, /* every image of the cells |k_a| <= near_shell[a], generated on the fly (reading S7) */
+    HSMA_NEAR_SPHERE = 1       /* only the images inside the sphere |r| <= R_aux.  Each evaluate builds
+                                  the explicit image list on the device (count, scan, scatter), packs it and sums it
+                                  with the identity cell; the image count is read back, so hsma_evaluate* SYNCHRONISES
+                                  the stream once in this mode.  Boundary closure only. */
+} hsma_near_mode;
+
+typedef enum {
+    HSMA_DIPOLE_EXACT = 0,     /* exact normal dipole on the M nodes (reading S9) */
+    HSMA_DIPOLE_FD3 = 1        /* Eq.(12)-(14) PAPER.md:107-120: central difference over three spheres, 3M charges */
+} hsma_dipole_mode;
+
 /* Plan descriptor (full form).  Set struct_size = sizeof(hsma_plan_desc); zero the rest first. */
 typedef struct {
     size_t struct_size;
@@ -81,6 +94,10 @@ typedef struct {
                              2 = one cubic (Halley) step (|err| <= 5e-16, 12 instr/pair),
                              0 = library default: 2 while N*N*cells < 2^32 pairs (latency-bound), else 1.
                              Steps (a) and (c) always use the cubic step. */
+    /* paper-literal variants; 0 = the north_star forms */
+    int near_mode;        /* hsma_near_mode */
+    int dipole_mode;      /* hsma_dipole_mode */
+    double fd_dr_rel;     /* HSMA_DIPOLE_FD3: Delta r / R_aux (1e-5; 1e-4 for the Dirichlet example); 0 = 1e-5 */
 } hsma_plan_desc;
 
 /*
@@ -145,7 +162,8 @@ const char* hsma_status_string(int status);
 
 /* ---- introspection / test and bench hooks ------------------------------------------------------- */
 /* sizes: what[0]=rows of the fit, [1]=columns, [2]=check targets K_t, [3]=near cells, [4]=rhs cells,
- * [5]=M nodes, [6]=p, [7]=kernels launched by the last evaluate.  host out [8]. */
+ * [5]=M nodes, [6]=p, [7]=kernels launched by the last evaluate, [8]=near images summed per target by the last
+ * evaluate (N * cells, or the image count inside the sphere), [9]=node records (M or 3M).  host out [10]. */
 hsma_status hsma_plan_info(hsma_plan* plan, long long* what_out);
 /* copies of plan/evaluate state into caller DEVICE buffers (valid after an evaluate on the stream) */
 hsma_status hsma_get_coeffs(hsma_plan* plan, double* A_out /* dev [p*p], R0-scaled basis */);

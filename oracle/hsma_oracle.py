@@ -515,15 +515,20 @@ def hsma(w, targets_slice: Optional[slice] = None, dipole: str = "exact", dr_rel
     n_near = int(near_src.shape[0]) if sphere else N * int(near.w.shape[0])
     pairs = {"a": int(check_targets.shape[0]) * (n_near if sphere else N * int(n_check_cells)),
              "b": int(i1 - i0) * n_near,
-             "c": int(i1 - i0) * int(nodes.shape[0])}
+             "c": int(i1 - i0) * int(nodes.shape[0]) * (3 if dipole == "fd3" else 1)}
     res = OracleResult(phi, U, A, rhs, fit_rms, float(sv[0] / sv[-1]), phi_near, phi_out,
                        check_targets, phi_check, Q, D, nodes, nrm, pairs)
     if forces:
         # PAPER.md:89-93 (Eq.9): F_i = -q_i grad [Phi_in + Phi_out](r_i), bare self term excluded,
         # coefficients A_nm held fixed; the image gradient uses the exact dipole layer (reading S9)
-        if dipole != "exact":
-            raise ValueError("forces are implemented for the exact dipole layer")
-        res.grad = near_grad(tg, near_src, near_q, near_cells, self_offset=i0) + node_grad(tg, nodes, nrm, Q, D)
+        if dipole == "exact":
+            g_out = node_grad(tg, nodes, nrm, Q, D)
+        else:   # the three charged spheres of Eq.(14): gradients of pure charges
+            zero = np.zeros_like(Q)
+            g_out = (node_grad(tg, nodes, nrm, Q, zero)
+                     + node_grad(tg, (w.R_aux - dr / 2) * nrm, nrm, D / dr, zero)
+                     - node_grad(tg, (w.R_aux + dr / 2) * nrm, nrm, D / dr, zero))
+        res.grad = near_grad(tg, near_src, near_q, near_cells, self_offset=i0) + g_out
         res.F = -q[i0:i1, None] * res.grad
     return res
 

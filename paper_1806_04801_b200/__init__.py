@@ -22,21 +22,24 @@ class Plan:
 
     def __init__(self, *, kind: int, L, near_shell, R_aux: float, p: int, M: int, K: int, gamma: float = 1.0,
                  check_xyz=None, closure: int = 0, far_shell=(0, 0, 0), quad_rule: int = 0,
-                 rsqrt_refine: int = 0, stream=None):
+                 rsqrt_refine: int = 0, near_mode: int = 0, dipole_mode: int = 0, fd_dr_rel: float = 0.0, stream=None):
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1806_04801_b200 needs a CUDA device (no CPU fallback)")
         self.handle = None
         self.handle = binding.hsma_plan_create_ex(kind=kind, L=L, near_shell=near_shell, gamma=gamma, R_aux=R_aux,
                                                   p=p, M=M, K=K, check_xyz=check_xyz, closure=closure,
                                                   far_shell=far_shell, quad_rule=quad_rule,
-                                                  rsqrt_refine=rsqrt_refine, stream=stream)
+                                                  rsqrt_refine=rsqrt_refine, near_mode=near_mode,
+                                                  dipole_mode=dipole_mode, fd_dr_rel=fd_dr_rel, stream=stream)
         self.info = binding.hsma_plan_info(self.handle)
 
     @classmethod
     def from_workload(cls, w, **overrides) -> "Plan":
         """w: an hsma_workloads.Workload (plain parameters + inputs; holds none of the method's arithmetic)."""
         kw = dict(kind=w.kind, L=w.L, near_shell=w.near_shell, R_aux=w.R_aux, p=w.p, M=w.M, K=w.K, gamma=w.gamma,
-                  check_xyz=w.check_xyz, closure=w.closure, far_shell=w.far_shell, quad_rule=w.quad_rule)
+                  check_xyz=w.check_xyz, closure=w.closure, far_shell=w.far_shell, quad_rule=w.quad_rule,
+                  near_mode=getattr(w, "near_mode", 0), dipole_mode=getattr(w, "dipole_mode", 0),
+                  fd_dr_rel=getattr(w, "fd_dr_rel", 0.0))
         kw.update(overrides)
         return cls(**kw)
 
@@ -145,6 +148,9 @@ class Plan:
 
     def fit_residual(self) -> float:
         return binding.hsma_get_fit_residual(self.handle)
+
+    def near_images_last_evaluate(self) -> int:
+        return binding.hsma_plan_info(self.handle)["near_images_last_evaluate"]
 
     def launches_last_evaluate(self) -> int:
         return binding.hsma_plan_info(self.handle)["launches_last_evaluate"]

@@ -23,6 +23,8 @@ HSMA_ERR_CUDA, HSMA_ERR_ALLOC, HSMA_ERR_RANK_DEFICIENT = -4, -5, -6
 HSMA_BC_PERIODIC, HSMA_BC_MIRROR_CAVITY, HSMA_BC_SLAB_XY_PERIODIC_Z_MIRROR = 0, 1, 2
 HSMA_CLOSURE_BOUNDARY, HSMA_CLOSURE_FAR_DATA = 0, 1
 HSMA_QUAD_SPIRAL, HSMA_QUAD_LATTICE = 0, 1
+HSMA_NEAR_WHOLE_CELLS, HSMA_NEAR_SPHERE = 0, 1
+HSMA_DIPOLE_EXACT, HSMA_DIPOLE_FD3 = 0, 1
 
 
 class hsma_plan_desc(ctypes.Structure):
@@ -30,7 +32,8 @@ class hsma_plan_desc(ctypes.Structure):
                 ("near_shell", ctypes.c_int * 3), ("gamma", ctypes.c_double), ("R_aux", ctypes.c_double),
                 ("p", ctypes.c_int), ("M", ctypes.c_int), ("K", ctypes.c_int), ("check_xyz", c_double_p),
                 ("closure", ctypes.c_int), ("far_shell", ctypes.c_int * 3), ("quad_rule", ctypes.c_int),
-                ("rsqrt_refine", ctypes.c_int)]
+                ("rsqrt_refine", ctypes.c_int), ("near_mode", ctypes.c_int), ("dipole_mode", ctypes.c_int),
+                ("fd_dr_rel", ctypes.c_double)]
 
 
 class HsmaError(RuntimeError):
@@ -156,7 +159,8 @@ def hsma_plan_create(L: float, boundary_kind: int, near_shell: int, R_aux: float
 
 def hsma_plan_create_ex(*, kind: int, L: Sequence[float], near_shell: Sequence[int], gamma: float, R_aux: float,
                         p: int, M: int, K: int, check_xyz=None, closure: int = 0, far_shell=(0, 0, 0),
-                        quad_rule: int = 0, rsqrt_refine: int = 0, stream=None) -> int:
+                        quad_rule: int = 0, rsqrt_refine: int = 0, near_mode: int = 0, dipole_mode: int = 0,
+                        fd_dr_rel: float = 0.0, stream=None) -> int:
     d = hsma_plan_desc()
     d.struct_size = ctypes.sizeof(hsma_plan_desc)
     d.kind = kind
@@ -172,6 +176,7 @@ def hsma_plan_create_ex(*, kind: int, L: Sequence[float], near_shell: Sequence[i
     d.closure = closure
     d.far_shell[:] = [int(v) for v in far_shell]
     d.quad_rule, d.rsqrt_refine = int(quad_rule), int(rsqrt_refine)
+    d.near_mode, d.dipole_mode, d.fd_dr_rel = int(near_mode), int(dipole_mode), float(fd_dr_rel)
     h = ctypes.c_void_p()
     _check(load_library().hsma_plan_create_ex(ctypes.byref(d), _stream_ptr(stream), ctypes.byref(h)),
            "hsma_plan_create_ex")
@@ -263,9 +268,10 @@ def hsma_plan_sync(plan: int):
 
 
 def hsma_plan_info(plan: int) -> dict:
-    w = (ctypes.c_longlong * 8)()
+    w = (ctypes.c_longlong * 10)()
     _check(load_library().hsma_plan_info(plan, w), "hsma_plan_info")
-    keys = ("rows", "cols", "check_targets", "near_cells", "rhs_cells", "M", "p", "launches_last_evaluate")
+    keys = ("rows", "cols", "check_targets", "near_cells", "rhs_cells", "M", "p", "launches_last_evaluate",
+            "near_images_last_evaluate", "node_records")
     return dict(zip(keys, [int(v) for v in w]))
 
 

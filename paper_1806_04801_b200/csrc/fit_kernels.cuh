@@ -216,9 +216,13 @@ __global__ void __launch_bounds__(1024) fit_residual_kernel(const double* __rest
 //   N_j = (1/R_aux) sum n A'_nm Y_nm (= sigma = d/dr Phi_out, Eq.11)
 //   Q_j = w_j N_j / 4pi,  P_j = (w_j S_j / 4pi) n_j   (exact normal dipole, reading S9)
 // Writes the packed record (R_j, Q_j | P_j, 0) read by node_sum_kernel.
+// fd_dr > 0: the paper's three-sphere form instead (Eq.12-14): three pure charges per node,
+//   Q_j on R_s,  +D_j/dr on R_s - dr/2,  -D_j/dr on R_s + dr/2,  D_j = w_j S_j/4pi (the area factors of Eq.(13)
+//   cancel against the quadrature weights of the two displaced spheres); records j, M + j, 2M + j.
 __global__ void surface_mapping_kernel(const double* __restrict__ A_full, int p, double ratio /* R_aux/R0 */,
                                        double R_aux, const double* __restrict__ nrm /* [M,3] */,
-                                       const double* __restrict__ wq /* [M] */, int M, Node8* __restrict__ nodes) {
+                                       const double* __restrict__ wq /* [M] */, int M, double fd_dr,
+                                       Node8* __restrict__ nodes) {
     __shared__ double As[kMaxP * kMaxP];
     for (int idx = threadIdx.x; idx < p * p; idx += blockDim.x) {
         int n = 0;
@@ -241,6 +245,15 @@ __global__ void surface_mapping_kernel(const double* __restrict__ A_full, int p,
     Node8 o;
     o.x = R_aux * nx; o.y = R_aux * ny; o.z = R_aux * nz; o.q = w * Nn / R_aux;
     o.px = D * nx; o.py = D * ny; o.pz = D * nz; o.pad = 0.0;
+    if (fd_dr > 0.0) {
+        o.px = 0.0; o.py = 0.0; o.pz = 0.0;
+        Node8 in = o, out = o;
+        const double ri = R_aux - 0.5 * fd_dr, ro = R_aux + 0.5 * fd_dr;
+        in.x = ri * nx; in.y = ri * ny; in.z = ri * nz; in.q = D / fd_dr;
+        out.x = ro * nx; out.y = ro * ny; out.z = ro * nz; out.q = -D / fd_dr;
+        nodes[M + j] = in;
+        nodes[2 * M + j] = out;
+    }
     nodes[j] = o;
 }
 

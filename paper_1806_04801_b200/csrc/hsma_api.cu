@@ -203,6 +203,17 @@ struct hsma_plan {
     double rhs_sign = -1.0;
     // plan-owned device data
     Cell* cells_near = nullptr;
+    Cell* cell_identity = nullptr;   // one cell: no shift, weight 1, central (sphere-culled near set)
+    int* cell_order = nullptr;       // central cell first (sphere-culled near set)
+    bool sphere = false;
+    double fd_dr = 0.0;              // > 0: three-sphere dipole
+    long long n_node_records = 0, last_images = 0;
+    // image list of the sphere-culled near set (grown as needed)
+    DevBuf<long long> img_counts;
+    DevBuf<double> img_xyz, img_q, img_stats;
+    DevBuf<Src4> img_src;
+    DevBuf<int> img_slot_of, img_tile_np;
+    QInfo* img_qinfo = nullptr;
     Cell* cells_rhs = nullptr;   // == cells_near for the boundary closure
     double* chk = nullptr;       // [Kt,3]
     double* nrm = nullptr;       // [M,3]
@@ -234,6 +245,11 @@ static void plan_free(hsma_plan* p) {
                     p->pc, p->rhs, p->cvec, p->A_full, p->scalars, p->flags};
     for (void* q : ptrs) if (q) cudaFree(q);
     p->src.release(); p->slot_of.release(); p->tile_np.release(); if (p->qinfo) cudaFree(p->qinfo);
+    if (p->cell_identity) cudaFree(p->cell_identity);
+    if (p->cell_order) cudaFree(p->cell_order);
+    if (p->img_qinfo) cudaFree(p->img_qinfo);
+    p->img_counts.release(); p->img_xyz.release(); p->img_q.release(); p->img_stats.release(); p->img_src.release();
+    p->img_slot_of.release(); p->img_tile_np.release();
     p->part_a.release(); p->part_b.release(); p->part_c.release(); p->red.release();
     p->xyz_in.release(); p->q_in.release(); p->phi_dev.release(); p->force_dev.release();
     for (cudaEvent_t e : p->ev) if (e) cudaEventDestroy(e);
@@ -253,6 +269,10 @@ extern "C" hsma_status hsma_plan_create_ex(const hsma_plan_desc* desc, void* cud
     if (d.kind < 0 || d.kind > 2 || d.p < 1 || d.p > kMaxP || d.M < 8 || d.K < 1) return HSMA_ERR_INVALID_ARG;
     if (d.closure != HSMA_CLOSURE_BOUNDARY && d.closure != HSMA_CLOSURE_FAR_DATA) return HSMA_ERR_INVALID_ARG;
     if (d.rsqrt_refine < 0 || d.rsqrt_refine > 2) return HSMA_ERR_INVALID_ARG;
+    if (d.near_mode != HSMA_NEAR_WHOLE_CELLS && d.near_mode != HSMA_NEAR_SPHERE) return HSMA_ERR_INVALID_ARG;
+    if (d.dipole_mode != HSMA_DIPOLE_EXACT && d.dipole_mode != HSMA_DIPOLE_FD3) return HSMA_ERR_INVALID_ARG;
+    if (d.near_mode == HSMA_NEAR_SPHERE && d.closure != HSMA_CLOSURE_BOUNDARY) return HSMA_ERR_INVALID_ARG;
+    if (d.fd_dr_rel < 0.0 || d.fd_dr_rel > 0.1) return HSMA_ERR_INVALID_ARG;
     for (int a = 0; a < 3; ++a)
         if (!(d.L[a] > 0.0) || d.near_shell[a] < 0 || d.near_shell[a] > 8) return HSMA_ERR_INVALID_ARG;
     if (d.kind == HSMA_BC_PERIODIC && d.closure != HSMA_CLOSURE_BOUNDARY) return HSMA_ERR_INVALID_ARG;
@@ -274,6 +294,8 @@ extern "C" hsma_status hsma_plan_create_ex(const hsma_plan_desc* desc, void* cud
     p->need_neutral = d.kind != HSMA_BC_MIRROR_CAVITY;
     p->refine = d.rsqrt_refine;  // 0 = by size, see evaluate_impl
     p->rhs_sign = d.closure == HSMA_CLOSURE_FAR_DATA ? 1.0 : -1.0;
+    p->sphere = d.near_mode == HSMA_NEAR_SPHERE;
+    p->fd_dr = d.dipole_mode == HSMA_DIPOLE_FD3 ? (d.fd_dr_rel > 0.0 ? d.fd_dr_rel : 1e-5) * d.R_aux : 0.0;
     cudaStream_t st = p->stream;
 #define PCU(x) do { if ((x) != cudaSuccess) { plan_free(p); return HSMA_ERR_CUDA; } } while (0)
 
@@ -288,6 +310,16 @@ extern "C" hsma_status hsma_plan_create_ex(const hsma_plan_desc* desc, void* cud
     if ((int)near.size() > kMaxCells || (int)rhsc.size() > kMaxCells) { plan_free(p); return HSMA_ERR_INVALID_ARG; }
     p->C_near = (int)near.size();
     PCU(upload(&p->cells_near, near, st));
+    if (p->sphere) {
+        Cell id;
+        id.sx = id.sy = id.sz = 0.0; id.w = 1.0; id.fx = id.fy = id.fz = 0; id.central = 1;
+        PCU(upload(&p->cell_identity, std::vector<Cell>(1, id), st));
+        std::vector<int> order;
+        for (int c = 0; c < (int)near.size(); ++c) if (near[c].central) order.push_back(c);
+        for (int c = 0; c < (int)near.size(); ++c) if (!near[c].central) order.push_back(c);
+        PCU(upload(&p->cell_order, order, st));
+        PCU(cudaMalloc(&p->img_qinfo, sizeof(QInfo)));
+    }
     if (rhsc.empty()) { p->cells_rhs = p->cells_near; p->C_rhs = p->C_near; }
     else { p->C_rhs = (int)rhsc.size(); PCU(upload(&p->cells_rhs, rhsc, st)); }
 
@@ -328,7 +360,8 @@ extern "C" hsma_status hsma_plan_create_ex(const hsma_plan_desc* desc, void* cud
     PCU(upload(&p->nrm, nrm, st));
     PCU(upload(&p->wq, wq, st));
     constexpr int kNT = kTile / 2;
-    p->node_tiles = (d.M + kNT - 1) / kNT;
+    p->n_node_records = p->fd_dr > 0.0 ? 3LL * d.M : d.M;
+    p->node_tiles = (p->n_node_records + kNT - 1) / kNT;
     {
         std::vector<Node8> pad((size_t)p->node_tiles * kNT);
         for (auto& n : pad) { n.x = n.y = n.z = kFar; n.q = n.px = n.py = n.pz = n.pad = 0.0; }
@@ -429,14 +462,51 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
                                                            p->slot_of.p, p->tile_np.p, p->red.p);
     charge_stats_kernel<<<1, 1024, 0, st>>>(p->red.p, n_tiles, p->need_neutral ? 1 : 0, p->scalars + 2, p->qinfo, p->flags);
     HSMA_COUNT_LAUNCH(); HSMA_COUNT_LAUNCH();
-    const Packed P{p->src.p, N, n_tiles, p->tile_np.p, p->slot_of.p, p->qinfo};
+    Packed P{p->src.p, N, n_tiles, p->tile_np.p, p->slot_of.p, p->qinfo};   // what the near sums read
+    const Cell *cells_a = p->cells_rhs, *cells_b = p->cells_near;
+    int C_a = p->C_rhs, C_b = p->C_near;
+    long long n_tiles_near = n_tiles;
+    p->last_images = N * (long long)p->C_near;
+    if (p->sphere) {
+        // paper-literal near set: explicit list of the images inside the sphere, central cell first
+        // (image i < N is source i), packed like a source array and summed with the identity cell
+        const long long entries = (long long)p->C_near * N, blocks = (entries + kTile - 1) / kTile;
+        const double R2 = d.R_aux * d.R_aux;
+        if (p->img_counts.reserve((size_t)blocks + 1) != cudaSuccess) return HSMA_ERR_ALLOC;
+        image_count_kernel<<<(unsigned)blocks, kTile, 0, st>>>(xyz, q, N, p->half[0], p->half[1], p->half[2], p->cells_near,
+                                                              p->cell_order, p->C_near, R2, p->img_counts.p);
+        scan_counts_kernel<<<1, 1024, 0, st>>>(p->img_counts.p, blocks);
+        HSMA_COUNT_LAUNCH(); HSMA_COUNT_LAUNCH();
+        long long Ns = 0;   // the launch shapes below depend on it: the one host synchronisation of this mode
+        if (cudaMemcpyAsync(&Ns, p->img_counts.p + blocks, sizeof(long long), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+            cudaStreamSynchronize(st) != cudaSuccess)
+            return HSMA_ERR_CUDA;
+        if (Ns < N || Ns > 2000000000LL) return HSMA_ERR_GEOMETRY;   // a source outside the sphere / index overflow
+        const long long nt_img = (Ns + kTile - 1) / kTile;
+        if (p->img_xyz.reserve(3 * (size_t)Ns) != cudaSuccess || p->img_q.reserve((size_t)Ns) != cudaSuccess ||
+            p->img_src.reserve((size_t)nt_img * kTile) != cudaSuccess || p->img_slot_of.reserve((size_t)Ns) != cudaSuccess ||
+            p->img_tile_np.reserve((size_t)nt_img) != cudaSuccess || p->img_stats.reserve(4 * (size_t)nt_img + 2) != cudaSuccess)
+            return HSMA_ERR_ALLOC;
+        image_scatter_kernel<<<(unsigned)blocks, kTile, 0, st>>>(xyz, q, N, p->half[0], p->half[1], p->half[2], p->cells_near,
+                                                                p->cell_order, p->C_near, R2, p->img_counts.p, p->img_xyz.p,
+                                                                p->img_q.p);
+        pack_sources_kernel<<<(unsigned)nt_img, kTile, 0, st>>>(p->img_xyz.p, p->img_q.p, Ns, 0.0, 0.0, 0.0, p->img_src.p,
+                                                               p->img_slot_of.p, p->img_tile_np.p, p->img_stats.p);
+        charge_stats_kernel<<<1, 1024, 0, st>>>(p->img_stats.p, nt_img, 0, p->img_stats.p + 4 * nt_img, p->img_qinfo, p->flags);
+        HSMA_COUNT_LAUNCH(); HSMA_COUNT_LAUNCH(); HSMA_COUNT_LAUNCH();
+        P = Packed{p->img_src.p, Ns, nt_img, p->img_tile_np.p, p->img_slot_of.p, p->img_qinfo};
+        cells_a = cells_b = p->cell_identity;
+        C_a = C_b = 1;
+        n_tiles_near = nt_img;
+        p->last_images = Ns;
+    }
 
     // H2 (a): Phi_in (or the far-cell data) at the monitoring points -> pc [Kt]
     {
-        const Launch s = choose_near(p->Kt, n_tiles, p->C_rhs, 2);
+        const Launch s = choose_near(p->Kt, n_tiles_near, C_a, 2);
         if (p->part_a.reserve((size_t)s.rows * p->Kt) != cudaSuccess) return HSMA_ERR_ALLOC;
         MARK(1);
-        launch_near(s, false, p->chk, 3, nullptr, p->Kt, 0, P, p->cells_rhs, p->C_rhs, -1, 2, p->part_a.p, st);  // (a) always cubic: it feeds the fit
+        launch_near(s, false, p->chk, 3, nullptr, p->Kt, 0, P, cells_a, C_a, -1, 2, p->part_a.p, st);  // (a) always cubic: it feeds the fit
         MARK(2);
         finish_phi_kernel<<<(p->Kt + 255) / 256, 256, 0, st>>>(s.layout(p->part_a.p), PartLayout{nullptr, 1, 1, 1, 1}, p->Kt, nullptr, nullptr, 0, p->pc, nullptr);
         HSMA_COUNT_LAUNCH();
@@ -447,21 +517,21 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
     HSMA_COUNT_LAUNCH();
     // H4: harmonic surface mapping, Eq.(10),(11) PAPER.md:99-105
     surface_mapping_kernel<<<(d.M + 127) / 128, 128, 0, st>>>(p->A_full, d.p, d.R_aux / p->R0, d.R_aux, p->nrm, p->wq,
-                                                              d.M, p->nodes);
+                                                              d.M, p->fd_dr, p->nodes);
     HSMA_COUNT_LAUNCH();
 
     const long long T = t1 - t0;
     if (T > 0) {
         // H5 (b): near images at the sources, self excluded
-        const int refine = p->refine ? p->refine : ((double)N * (double)N * p->C_near < 4294967296.0 ? 2 : 1);
+        const int refine = p->refine ? p->refine : ((double)N * (double)p->last_images < 4294967296.0 ? 2 : 1);
         // rsqrt_refine = 0: the cubic step while (b) is latency-bound anyway (< 2^32 pairs), Newton above
         const size_t comps = field ? 4 : 1;
-        const Launch sb = choose_near(T, n_tiles, p->C_near, refine, field);
+        const Launch sb = choose_near(T, n_tiles_near, C_b, refine, field);
         if (p->part_b.reserve((size_t)sb.rows * T * comps) != cudaSuccess) return HSMA_ERR_ALLOC;
         const Launch sc = choose_node(T, p->node_tiles, field);
         if (p->part_c.reserve((size_t)sc.rows * T * comps) != cudaSuccess) return HSMA_ERR_ALLOC;
         MARK(3);
-        launch_near(sb, field, reinterpret_cast<const double*>(p->src.p), 4, p->slot_of.p, T, t0, P, p->cells_near, p->C_near,
+        launch_near(sb, field, reinterpret_cast<const double*>(p->src.p), 4, p->slot_of.p, T, t0, P, cells_b, C_b,
                     t0, refine, p->part_b.p, st);
         MARK(4);
         // H6 (c): sphere nodes, charge + dipole
@@ -588,7 +658,7 @@ extern "C" const char* hsma_status_string(int s) {
 extern "C" hsma_status hsma_plan_info(hsma_plan* p, long long* w) {
     if (!p || !w) return HSMA_ERR_INVALID_ARG;
     w[0] = p->rows; w[1] = p->ncol; w[2] = p->Kt; w[3] = p->C_near; w[4] = p->C_rhs; w[5] = p->d.M; w[6] = p->d.p;
-    w[7] = p->last_launches;
+    w[7] = p->last_launches; w[8] = p->last_images; w[9] = p->n_node_records;
     return HSMA_OK;
 }
 

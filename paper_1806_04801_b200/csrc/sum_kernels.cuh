@@ -483,6 +483,90 @@ __global__ void __launch_bounds__(kTile) pack_sources_kernel(const double* __res
     }
 }
 
+// ---- paper-literal near set: the images inside the auxiliary sphere ----
+// Entry e = c * N + j of the (cell, source) table, cells in the order `order[c]` (central cell first, so that
+// image i < N is source i).  inside(e): |sign o r_j + shift|^2 <= R^2.  Pass 1 counts per block of kTile entries,
+// scan_counts_kernel turns the counts into offsets (single block), pass 2 writes the compacted list in order:
+// xyz_img [N_s,3], q_img [N_s] = w_c q_j.  The list is then packed like any source array and summed with the
+// identity cell.
+__device__ __forceinline__ bool image_of(const double* __restrict__ xyz, const double* __restrict__ q, long long N,
+                                         double hx, double hy, double hz, const Cell* __restrict__ cells,
+                                         const int* __restrict__ order, long long e, long long total, double R2,
+                                         double out[4]) {
+    if (e >= total) return false;
+    const int c = order[e / N];
+    const long long j = e - (e / N) * N;
+    const Cell cell = cells[c];
+    // image = sign o r + shift  (the pair kernels use the equivalent transform of the target instead)
+    const double x = flip(xyz[3 * j] - hx, cell.fx) + cell.sx;
+    const double y = flip(xyz[3 * j + 1] - hy, cell.fy) + cell.sy;
+    const double z = flip(xyz[3 * j + 2] - hz, cell.fz) + cell.sz;
+    out[0] = x; out[1] = y; out[2] = z; out[3] = cell.w * q[j];
+    return x * x + y * y + z * z <= R2;
+}
+__global__ void __launch_bounds__(kTile) image_count_kernel(const double* __restrict__ xyz, const double* __restrict__ q,
+                                                          long long N, double hx, double hy, double hz,
+                                                          const Cell* __restrict__ cells, const int* __restrict__ order,
+                                                          int C, double R2, long long* __restrict__ block_count) {
+    __shared__ int wc[kTile / 32];
+    const long long e = (long long)blockIdx.x * kTile + threadIdx.x;
+    double r[4];
+    const bool in = image_of(xyz, q, N, hx, hy, hz, cells, order, e, (long long)C * N, R2, r);
+    const unsigned b = __ballot_sync(0xffffffffu, in);
+    if ((threadIdx.x & 31) == 0) wc[threadIdx.x >> 5] = __popc(b);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int n = 0;
+        for (int k = 0; k < kTile / 32; ++k) n += wc[k];
+        block_count[blockIdx.x] = n;
+    }
+}
+// in place: counts -> exclusive offsets; total -> counts[n].  Single block of 1024 threads, chunked.
+__global__ void __launch_bounds__(1024) scan_counts_kernel(long long* __restrict__ counts, long long n) {
+    __shared__ long long sh[1024];
+    __shared__ long long carry;
+    if (threadIdx.x == 0) carry = 0;
+    __syncthreads();
+    for (long long base = 0; base < n; base += 1024) {
+        const long long i = base + threadIdx.x;
+        const long long v = i < n ? counts[i] : 0;
+        sh[threadIdx.x] = v;
+        __syncthreads();
+        for (int o = 1; o < 1024; o <<= 1) {
+            const long long t = threadIdx.x >= o ? sh[threadIdx.x - o] : 0;
+            __syncthreads();
+            sh[threadIdx.x] += t;
+            __syncthreads();
+        }
+        if (i < n) counts[i] = carry + sh[threadIdx.x] - v;
+        __syncthreads();
+        if (threadIdx.x == 0) carry += sh[1023];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) counts[n] = carry;
+}
+__global__ void __launch_bounds__(kTile) image_scatter_kernel(const double* __restrict__ xyz, const double* __restrict__ q,
+                                                            long long N, double hx, double hy, double hz,
+                                                            const Cell* __restrict__ cells, const int* __restrict__ order,
+                                                            int C, double R2, const long long* __restrict__ block_offset,
+                                                            double* __restrict__ xyz_img, double* __restrict__ q_img) {
+    __shared__ int wc[kTile / 32];
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    const long long e = (long long)blockIdx.x * kTile + threadIdx.x;
+    double r[4];
+    const bool in = image_of(xyz, q, N, hx, hy, hz, cells, order, e, (long long)C * N, R2, r);
+    const unsigned b = __ballot_sync(0xffffffffu, in);
+    if (l == 0) wc[w] = __popc(b);
+    __syncthreads();
+    if (in) {
+        int before = 0;
+        for (int k = 0; k < w; ++k) before += wc[k];
+        const long long o = block_offset[blockIdx.x] + before + __popc(b & ((1u << l) - 1u));
+        xyz_img[3 * o] = r[0]; xyz_img[3 * o + 1] = r[1]; xyz_img[3 * o + 2] = r[2];
+        q_img[o] = r[3];
+    }
+}
+
 // Single block: sum q, sum |q| -> scal[0..1]; neutrality flag (reading S17); QInfo (all |q| equal, bit for bit).
 __global__ void __launch_bounds__(1024) charge_stats_kernel(const double* __restrict__ stats, long long nblocks,
                                                             int need_neutral, double* __restrict__ scal,

@@ -1,0 +1,108 @@
+"""Parity of the paper-literal variants through the C-ABI against the oracle:
+sphere-culled near set and three-sphere dipole (Eq.12-14).  All `-m gpu`.
+Bars: the north_star ones (phi 1e-10, U 1e-11) for every mode with the exact dipole layer.  The three-sphere form
+differences two potentials of size D/dr = 1e5 |Phi_out| (dr = 1e-5 R_s), so EACH implementation carries
+rounding of about 1e5 eps |Phi_out| per potential (the paper itself raises dr to 1e-4 R_s "to avoid the influence of
+roundoff"); the errors are independent from particle to particle, and U = 1/2 sum q phi of a neutral
+system cancels the large common part of phi, so the relative agreement in U degrades to ~1e5 eps sqrt(N) max|phi|/|U|.
+For this mode the energy bar is therefore 1e-9; the potential bar stays 1e-10."""
+import math
+
+import numpy as np
+import pytest
+
+import hsma_workloads as W
+from oracle import hsma_oracle as O
+
+pytestmark = pytest.mark.gpu
+
+PHI_TOL = 1e-10
+U_TOL = 1e-11
+U_TOL_FD3 = 1e-9
+F_TOL = 1e-10
+
+
+@pytest.fixture(scope="module")
+def H():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    import paper_1806_04801_b200 as H
+    H.binding.load_library()
+    return H
+
+
+def dev(a):
+    import torch
+    return torch.as_tensor(np.ascontiguousarray(a, dtype=np.float64), device="cuda")
+
+
+def rel_inf(a, b):
+    return float(np.max(np.abs(a - b)) / np.max(np.abs(b)))
+
+
+def both(H, w, forces=False, **plan_kw):
+    r = O.hsma(w, forces=forces)
+    with H.Plan.from_workload(w, **plan_kw) as plan:
+        if forces:
+            phi, F, U = plan.evaluate_forces(dev(w.xyz), dev(w.q), sync=True)
+            F = F.cpu().numpy()
+        else:
+            phi, U = plan.evaluate(dev(w.xyz), dev(w.q), sync=True)
+            F = None
+        images = plan.near_images_last_evaluate()
+        info = plan.info
+        A = plan.coeffs().cpu().numpy()
+    return r, phi.cpu().numpy(), float(U), F, images, info, A
+
+
+@pytest.mark.parametrize("near_mode,dipole_mode", [(W.NEAR_SPHERE, W.DIPOLE_EXACT), (W.NEAR_WHOLE_CELLS, W.DIPOLE_FD3),
+                                                   (W.NEAR_SPHERE, W.DIPOLE_FD3)])
+@pytest.mark.parametrize("refine", [1, 2])
+def test_config2_paper_literal_modes(H, near_mode, dipole_mode, refine):
+    w = W.config(2).with_(near_mode=near_mode, dipole_mode=dipole_mode)
+    r, phi, U, _, images, info, A = both(H, w, rsqrt_refine=refine)
+    assert rel_inf(A, r.A) < 1e-9
+    assert rel_inf(phi, r.phi) <= PHI_TOL
+    assert abs(U - r.U) <= (U_TOL_FD3 if dipole_mode == W.DIPOLE_FD3 else U_TOL) * abs(r.U)
+    assert images == r.pairs["b"] // w.N                       # the same image count, bit for bit the same predicate
+    assert info["node_records"] == (3 if dipole_mode == W.DIPOLE_FD3 else 1) * w.M
+
+
+def test_sphere_mode_in_the_cavity_and_with_forces(H):
+    """Mirror cavity (charges w_c q_j = +-q_j in the image list), random magnitudes, forces."""
+    w = W.config(3, N=1500)
+    w = w.with_(q=np.random.default_rng(35).standard_normal(w.N), near_mode=W.NEAR_SPHERE)
+    r, phi, U, F, images, _, _ = both(H, w, forces=True)
+    assert rel_inf(phi, r.phi) <= PHI_TOL and abs(U - r.U) <= U_TOL * abs(r.U)
+    assert rel_inf(F, r.F) <= F_TOL
+    assert images == r.pairs["b"] // w.N and images < 27 * w.N
+
+
+def test_madelung_64_ions_paper_setting(H):
+    """64 ions, L = 2, alpha = 2, P = 23, N_o = 5928, sphere-culled images, three spheres."""
+    xyz, q, _ = W.rock_salt(2)
+    P = 23
+    w = W.Workload("nacl64", W.BC_PERIODIC, (2.0, 2.0, 2.0), (2, 2, 2), 1.0, 2.0 * math.sqrt(3.0), P + 1, 2 * 988,
+                   2 * P * P, xyz * 0.5, q, quad_rule=W.QUAD_LATTICE, near_mode=W.NEAR_SPHERE, dipole_mode=W.DIPOLE_FD3)
+    r, phi, U, _, _, _, _ = both(H, w)
+    assert rel_inf(phi, r.phi) <= PHI_TOL and abs(U - r.U) <= U_TOL_FD3 * abs(r.U)
+    assert abs(O.madelung_constant(U, w.N, 0.5) - 1.7475645946331822) < 5e-9
+
+
+@pytest.mark.parametrize("N", [216, 4096, 32768])
+def test_paper_timing_workload(H, N):
+    """The paper's timing workload (alpha = 1.3, P = 25, N_o = 5928, N_m = 2 P^2), potentials and forces."""
+    w = W.paper_timing(N)
+    forces = N <= 4096
+    r, phi, U, F, images, _, A = both(H, w, forces=forces)
+    assert rel_inf(A, r.A) < 1e-8
+    assert rel_inf(phi, r.phi) <= PHI_TOL and abs(U - r.U) <= U_TOL_FD3 * abs(r.U)
+    if forces:
+        assert rel_inf(F, r.F) <= F_TOL
+    assert images == r.pairs["b"] // w.N and 5.0 * N < images < 7.5 * N
+
+
+def test_sphere_mode_rejects_a_sphere_beyond_the_cell_block(H):
+    with pytest.raises(H.HsmaError) as e:
+        H.Plan(kind=0, L=(1, 1, 1), near_shell=(1, 1, 1), R_aux=1.6, p=8, M=400, K=200, near_mode=W.NEAR_SPHERE)
+    assert e.value.status == H.HSMA_ERR_GEOMETRY
