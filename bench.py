@@ -50,8 +50,11 @@ FP64_LANES_PER_SM = 64
 
 
 def pair_counts(info: dict, N: int, T: int) -> dict:
-    """Pairs per step for a rank that owns T of the N targets (step (a) is computed in full)."""
-    return {"a": info["check_targets"] * N * info["rhs_cells"], "b": T * N * info["near_cells"], "c": T * info["M"]}
+    """Pairs per step for a rank that owns T of the N targets (step (a) is computed in full).  With the
+    sphere-culled near set the images per target are what the last evaluate counted on the device."""
+    images = info.get("near_images_last_evaluate") or N * info["near_cells"]
+    near_a = images if images != N * info["near_cells"] else N * info["rhs_cells"]
+    return {"a": info["check_targets"] * near_a, "b": T * images, "c": T * info.get("node_records", info["M"])}
 
 
 class ClockSampler:
@@ -227,7 +230,7 @@ def run_b200(args, w) -> dict:
 
     plan = H.Plan.from_workload(w, rsqrt_refine=args.refine)
     info = plan.info
-    refine = args.refine if args.refine else (2 if float(N) * N * info["near_cells"] < 2.0 ** 32 else 1)
+    refine = args.refine   # 0: resolved after the warm-up (the library decides by the pair count)
     xyz = torch.as_tensor(np.ascontiguousarray(w.xyz), device=dev)
     q = torch.as_tensor(np.ascontiguousarray(w.q), device=dev)
     phi = torch.empty(T, dtype=torch.float64, device=dev)
@@ -253,6 +256,7 @@ def run_b200(args, w) -> dict:
     for _ in range(args.warmup):
         step()
     plan.sync()
+    info = H.binding.hsma_plan_info(plan.handle)          # now with the image count of the last evaluate
     plan.set_timing(True)
     stage_ms = {k: 0.0 for k in H.binding.TIMING_KEYS}
     sampler = ClockSampler(local)
@@ -318,6 +322,8 @@ def run_b200(args, w) -> dict:
 
     # roofline of the dominant kernel: near_sum_kernel over the sources, step (b)
     pc_rank = pair_counts(info, N, T)
+    if not refine:
+        refine = 2 if float(N) * pc_rank["b"] / max(T, 1) < 2.0 ** 32 else 1
     k_ms = stage_ms["near_source_kernel"]
     sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
     peaks = {}
@@ -332,7 +338,8 @@ def run_b200(args, w) -> dict:
     uniform_q = bool(np.all(np.abs(w.q) == abs(w.q[0])))
     ex_instr, ex_flops = (EXEC_PAIR_FIELD if args.forces else EXEC_PAIR)[(refine, uniform_q)]
     alg_flops = FLOPS_PAIR_CHARGE_FIELD if args.forces else FLOPS_PAIR_CHARGE
-    traffic = NCU_TRAFFIC_BYTES_CFG5 if (args.config == 5 and args.size is None and world == 1 and not args.forces) else None
+    traffic = NCU_TRAFFIC_BYTES_CFG5 if (args.config == 5 and args.size is None and world == 1 and not args.forces
+                                         and not args.paper_timing) else None
     issue_peak = sm_count * FP64_LANES_PER_SM * sm_max_mhz * 1e6          # FP64-pipe thread-instructions/s
     roofline = {"bound": "alu", "kernel": f"near_sum_kernel<R,{refine},{'uniform-|q|' if uniform_q else 'generic'},{'field' if args.forces else 'potential'}> step (b)", "achieved": ach_tf, "peak": peak_tf,
                 "unit": "TFLOP/s", "frac": ach_tf / peak_tf, "traffic": traffic,
@@ -370,6 +377,9 @@ def main():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--config", type=int, default=5, help="BASELINE.json configs[config-1]; 5 = the metric's workload")
     ap.add_argument("--size", type=int, default=None, help="override N (same generator and seed)")
+    ap.add_argument("--paper-timing", type=int, default=0, metavar="N",
+                    help="the paper's own timing workload instead of a BASELINE.json config (PAPER.md:171,183: lattice "
+                         "sites, random signs, alpha=1.3, P=25, N_o=5928, images inside the sphere); N an even cube")
     ap.add_argument("--forces", action="store_true", help="time hsma_evaluate_forces (potential + forces) instead")
     ap.add_argument("--refine", type=int, default=0, choices=[0, 1, 2], help="hsma_plan_desc.rsqrt_refine")
     ap.add_argument("--e2e-steps", type=int, default=3)
@@ -380,7 +390,7 @@ def main():
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "b200":
         print(f"note: --warmup {args.warmup} < 3 (timing rules ask for >= 3)", file=sys.stderr)
-    w = W.config(args.config, N=args.size)
+    w = W.paper_timing(args.paper_timing) if args.paper_timing else W.config(args.config, N=args.size)
     rank = int(os.environ.get("RANK", "0"))
     if args.impl == "reference":
         if rank == 0:
@@ -388,7 +398,7 @@ def main():
         return
     out = run_b200(args, w)
     if rank == 0:
-        if args.gpus == 1 and not args.no_cpu_baseline:
+        if args.gpus == 1 and not args.no_cpu_baseline and not args.paper_timing:
             out["cpu_baseline"] = cpu_baseline(w, args.cpu_seconds)
         print(json.dumps(out), flush=True)
 
