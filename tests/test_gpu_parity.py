@@ -251,6 +251,66 @@ def test_config5_full_size_sampled(H):
     assert abs(float(U.cpu().numpy()[0]) - Uref) <= U_TOL * abs(Uref)
 
 
+# ------------------------------------------------------------------ maximum sizes and degenerate inputs
+def test_maximum_degree_p32(H):
+    """p = 32 (the library's maximum: 1023 fitted coefficients, 2048 rows), periodic, shell 2."""
+    w = W.config(2, N=400).with_(p=32, K=1100, M=6000, near_shell=(2, 2, 2), R_aux=2.4)
+    r, phi, U, extra = run_both(H, w)
+    # The coefficients of degree ~31 sit at the rounding level of the fit and the mapping multiplies them by
+    # (R_aux/R0)^31 = 5e13, so the node strengths Q_j are compared only through what they produce: phi and U.
+    report(f"p32: phi {rel_inf(phi, r.phi):.3e} U {abs(U - r.U) / abs(r.U):.3e} A {rel_inf(extra['A'], r.A):.3e} cond {r.cond:.3g}")
+    assert rel_inf(extra["A"], r.A) < 1e-9
+    assert rel_inf(phi, r.phi) <= PHI_TOL
+    assert abs(U - r.U) <= U_TOL * abs(r.U)
+    with pytest.raises(H.HsmaError) as e:
+        H.Plan(kind=0, L=(1, 1, 1), near_shell=(1, 1, 1), R_aux=1.2, p=33, M=500, K=3000)
+    assert e.value.status == H.HSMA_ERR_INVALID_ARG
+
+
+def test_largest_cell_tables(H):
+    """Cell tables at the shared-memory limit: 7x7x9 = 441 near cells (slab), and shell 3 periodic (343)."""
+    import torch
+    rng = np.random.default_rng(77)
+    for kind, L, shell, gamma in ((W.BC_SLAB_XY_PERIODIC_Z_MIRROR, (1.0, 1.0, 0.5), (3, 3, 4), 0.5),
+                                  (W.BC_PERIODIC, (1.0, 1.0, 1.0), (3, 3, 3), 1.0)):
+        N, T = 300, 130
+        src = (rng.random((N, 3)) - 0.5) * np.asarray(L)
+        q = rng.standard_normal(N)
+        tgt = (rng.random((T, 3)) - 0.5) * np.asarray(L)
+        cells = O.cell_table(kind, L, shell, gamma)
+        ref = O.near_sum(tgt, src, q, cells)
+        out = torch.empty(T, dtype=torch.float64, device="cuda")
+        H.hsma_direct_sum(dev(tgt), dev(src), dev(q), cells.shift, cells.sign, cells.w, cells.central, -1, 2, out)
+        assert rel_inf(out.cpu().numpy(), ref) < 1e-12
+    with pytest.raises(H.HsmaError):   # 9^3 = 729 cells do not fit
+        H.Plan(kind=0, L=(1, 1, 1), near_shell=(4, 4, 4), R_aux=1.2, p=4, M=100, K=100)
+
+
+def test_degenerate_inputs(H):
+    """N = 1 in a grounded cavity; two particles; all charges zero; a single target shard."""
+    import torch
+    L = (1.0, 1.0, 1.0)
+    chk = W.seeded_face_points(400, L, W.ALL_FACES, seed=5)
+    base = W.Workload("tiny", W.BC_MIRROR_CAVITY, L, (1, 1, 1), -1.0, 1.5 * math.sqrt(3) / 2, 8, 800, 400,
+                      np.array([[0.3, 0.6, 0.45]]), np.array([1.5]), check_xyz=chk)
+    r, phi, U, extra = run_both(H, base)
+    check_parity(r, phi, U, extra, "N=1 cavity")
+    two = base.with_(xyz=np.array([[0.3, 0.6, 0.45], [0.7, 0.2, 0.55]]), q=np.array([1.0, -2.5]))
+    r, phi, U, extra = run_both(H, two)
+    check_parity(r, phi, U, extra, "N=2 cavity")
+    zero = W.config(2, N=300)
+    with H.Plan.from_workload(zero) as plan:
+        phi0, U0 = plan.evaluate(dev(zero.xyz), dev(np.zeros(300)), sync=True)
+        assert float(phi0.abs().max()) == 0.0 and float(U0) == 0.0
+        ph1, u1 = plan.evaluate_shard(dev(zero.xyz), dev(zero.q), 299, 300, sync=True)
+        full, _ = plan.evaluate(dev(zero.xyz), dev(zero.q), sync=True)
+        assert abs(float(ph1[0]) - float(full[299])) <= 1e-13 * float(full.abs().max())
+    with pytest.raises(H.HsmaError) as e:       # N = 0 is rejected, nothing is launched
+        H.hsma_evaluate(H.hsma_plan_create(1.0, 0, 1, 1.2, 4, 100), torch.empty(0, 3, dtype=torch.float64, device="cuda"),
+                        torch.empty(0, dtype=torch.float64, device="cuda"), torch.empty(0, dtype=torch.float64, device="cuda"))
+    assert e.value.status == H.HSMA_ERR_INVALID_ARG
+
+
 # ------------------------------------------------------------------ API behaviour
 def test_shards_and_host_path_agree(H):
     import torch
