@@ -424,7 +424,11 @@ def hsma(w, targets_slice: Optional[slice] = None, dipole: str = "exact", dr_rel
     q = np.asarray(w.q, dtype=np.float64)
     N = src.shape[0]
     periodic = w.kind == BC_PERIODIC
-    if periodic or w.kind == BC_SLAB:
+    # grounded slab: x,y periodic, conducting plates at z = +-H/2
+    # (gamma = -1), closed by the boundary conditions themselves instead of far-cell data
+    slab_bc = w.kind == BC_SLAB and w.closure == CLOSURE_BOUNDARY
+    n_pair = 0
+    if periodic or (w.kind == BC_SLAB and not slab_bc):
         if abs(q.sum()) > 1e-12 * np.abs(q).sum():
             raise ValueError("periodic system must be neutral (reading S17)")
 
@@ -450,6 +454,24 @@ def hsma(w, targets_slice: Optional[slice] = None, dipole: str = "exact", dr_rel
         Bt = real_solid_harmonics(xt, p, R0)
         F = (Bx - Bt)[:, 1:]                              # reading S2: drop the constant, A00 = 0
         check_targets = np.concatenate([x, xt], axis=0)
+        n_pair = x.shape[0]
+    elif slab_bc:
+        # Two families of rows ("boundary conditions", 80-82 for the periodic directions):
+        #   pairs    K Fibonacci points on the circumsphere and their partners wrapped in x and y only,
+        #            Phi(x_i) - Phi(x~_i) = 0 (the image system is xy-periodic at every height, also beyond the plates);
+        #   plates   K points on the two faces z = +-H/2, Phi = 0 ("DBC").
+        # The constant harmonic is seen by the plate rows, so no column is dropped.
+        if w.gamma != -1.0:
+            raise ValueError("the boundary closure of the slab is defined for grounded plates, gamma = -1")
+        xs = fibonacci_sphere_checkpoints(w.K, R0)
+        xt = wrap_into_box(xs, L, periodic_axes=(True, True, False))
+        keep = np.any(np.abs(xs - xt) > 0, axis=1)
+        xs, xt = xs[keep], xt[keep]
+        xf = default_face_points(w.K, L, (2,)) if w.check_xyz is None else np.asarray(w.check_xyz, float)
+        F = np.concatenate([real_solid_harmonics(xs, p, R0) - real_solid_harmonics(xt, p, R0),
+                            real_solid_harmonics(xf, p, R0)], axis=0)
+        check_targets = np.concatenate([xs, xt, xf], axis=0)
+        n_pair = xs.shape[0]
     else:
         if w.check_xyz is not None:
             x = np.asarray(w.check_xyz, float)
@@ -477,6 +499,8 @@ def hsma(w, targets_slice: Optional[slice] = None, dipole: str = "exact", dr_rel
         if periodic:
             K = x.shape[0]
             rhs = -(phi_check[:K] - phi_check[K:])        # v_i = Phi(x_i) - Phi(x~_i) = 0
+        elif slab_bc:
+            rhs = np.concatenate([-(phi_check[:n_pair] - phi_check[n_pair:2 * n_pair]), -phi_check[2 * n_pair:]])
         else:
             rhs = -phi_check                              # grounded wall: Phi_in + Phi_out = 0
     # least squares, Eq.(7)

@@ -101,6 +101,27 @@ def grounded_box_green(x, xp, box, nmax=80):
     return 16 * math.pi / (a * b) * total
 
 
+def grounded_slab_green(x, xp, Lx, Ly, H, mmax=40):
+    """G(x, x') between two grounded plates z = 0 and z = H, periodic in x and y with cell Lx x Ly, normalised so
+    that G -> 1/|x - x'| near x' (Gaussian units): the in-plane Fourier series of the textbook parallel-plate
+    Green function,  G = (4 pi/A) [ z<(H - z>)/H + sum_{k != 0} cos(k.drho) sinh(k z<) sinh(k (H - z>)) / (k sinh kH) ].
+    Converges like exp(-k |z - z'|): use z != z'."""
+    A = Lx * Ly
+    zl, zg = (x[2], xp[2]) if x[2] < xp[2] else (xp[2], x[2])
+    total = zl * (H - zg) / H
+    dx, dy = x[0] - xp[0], x[1] - xp[1]
+    for m in range(-mmax, mmax + 1):
+        for n in range(-mmax, mmax + 1):
+            if m == 0 and n == 0:
+                continue
+            kx, ky = 2 * math.pi * m / Lx, 2 * math.pi * n / Ly
+            k = math.hypot(kx, ky)
+            num = (1 - math.exp(-2 * k * zl)) * (1 - math.exp(-2 * k * (H - zg)))
+            den = 1 - math.exp(-2 * k * H)
+            total += math.cos(kx * dx + ky * dy) * 0.5 * math.exp(-k * (zg - zl)) * num / den / k
+    return 4 * math.pi / A * total
+
+
 def brute_image_sum(targets, src_c, q, L, reflecting, shell, gamma, skip_self=False,
                     exclude_shell=None):
     """Explicit images, pure Python.  src_c: CENTRED source coordinates.  For every cell k with
