@@ -46,11 +46,15 @@ typedef enum {
 typedef enum {
     HSMA_BC_PERIODIC = 0,                  /* Eq.(3): all axes periodic             */
     HSMA_BC_MIRROR_CAVITY = 1,             /* Eq.(4): all axes reflecting, gamma^|k| */
-    HSMA_BC_SLAB_XY_PERIODIC_Z_MIRROR = 2  /* x,y periodic, z reflecting (readings G11, S16)       */
+    HSMA_BC_SLAB_XY_PERIODIC_Z_MIRROR = 2  /* x,y periodic, z reflecting (readings G11, S16): with the far-data closure for
+                                              any gamma; with the boundary closure for grounded plates, gamma = -1     */
 } hsma_boundary_kind;
 
 typedef enum {
-    HSMA_CLOSURE_BOUNDARY = 0, /* residual of the boundary condition at the check points */
+    HSMA_CLOSURE_BOUNDARY = 0, /* residual of the boundary condition at the check points.  Periodic:
+                                  K circumsphere points and their wrapped partners; cavity: K Dirichlet points on the
+                                  faces; grounded slab: K circumsphere points wrapped in x,y only PLUS K Dirichlet points
+                                  on the two plates (check_xyz, if given, are the plate points) -- DESIGN.md 6.8 */
     HSMA_CLOSURE_FAR_DATA = 1  /* rhs = direct sum over the far cell table (reading S16, config 4)       */
 } hsma_closure;
 

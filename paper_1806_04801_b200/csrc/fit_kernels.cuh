@@ -46,23 +46,24 @@ __device__ __forceinline__ void solid_harmonics(double x, double y, double z, do
     }
 }
 
-// Fitting matrix, column-major [rows x ncol] (ld = rows).  PAPER.md:72-82.
-//   periodic (pairs = 1): row_i = B(x_i) - B(x~_i), constant column dropped (reading S2): col = idx - 1
-//   otherwise:            row_i = B(x_i)
-// chk: [K_t,3] centred check targets, x_i = chk[i], x~_i = chk[rows + i].
-__global__ void build_fit_matrix_kernel(const double* __restrict__ chk, int rows, int pairs, int p, double inv_R0,
-                                        double* __restrict__ Fm) {
+// Fitting matrix, column-major [rows x ncol] (ld = rows), rows = n_pair + n_single.  PAPER.md:72-82.
+//   pair rows   (i < n_pair):  row_i = B(x_i) - B(x~_i),  x_i = chk[i], x~_i = chk[n_pair + i]   (periodic axes)
+//   single rows (the rest):    row_i = B(y_i),            y_i = chk[2 n_pair + (i - n_pair)]     (Dirichlet / data)
+//   drop = 1: the constant column is dropped (fully periodic kind, reading S2): col = idx - 1
+__global__ void build_fit_matrix_kernel(const double* __restrict__ chk, int n_pair, int n_single, int drop, int p,
+                                        double inv_R0, double* __restrict__ Fm) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int rows = n_pair + n_single;
     if (i >= rows) return;
-    const int drop = pairs ? 1 : 0;
-    const double* a = chk + 3 * (size_t)i;
+    const bool pairs = i < n_pair;
+    const double* a = chk + 3 * (size_t)(pairs ? i : n_pair + i);
     solid_harmonics(a[0], a[1], a[2], inv_R0, p, [&](int n, int m, double vc, double vs) {
         const int cc = n * n + n + m - drop, cs = n * n + n - m - drop;
         if (cc >= 0) Fm[(size_t)cc * rows + i] = vc;
         if (m > 0) Fm[(size_t)cs * rows + i] = vs;
     });
     if (pairs) {
-        const double* b = chk + 3 * (size_t)(rows + i);
+        const double* b = chk + 3 * (size_t)(n_pair + i);
         solid_harmonics(b[0], b[1], b[2], inv_R0, p, [&](int n, int m, double vc, double vs) {
             const int cc = n * n + n + m - drop, cs = n * n + n - m - drop;
             if (cc >= 0) Fm[(size_t)cc * rows + i] -= vc;
@@ -168,18 +169,20 @@ __global__ void pinv_kernel(const double* __restrict__ Qm, const double* __restr
 
 // H3 (update step): rhs from the check-point sums, A = Pinv rhs.  One warp per coefficient, 8 warps per block;
 // block 0 also stores rhs.  Fixed summation order (lane-strided partial sums, xor-shuffle tree).
-__global__ void __launch_bounds__(256) ls_apply_kernel(const double* __restrict__ pc, int rows, int ncol, int pairs,
-                                                       double sgn, const double* __restrict__ Pinv,
+__global__ void __launch_bounds__(256) ls_apply_kernel(const double* __restrict__ pc, int n_pair, int n_single, int ncol,
+                                                       int drop, double sgn, const double* __restrict__ Pinv,
                                                        double* __restrict__ rhs, double* __restrict__ A_full) {
     const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
     const int j = blockIdx.x * 8 + w;
+    const int rows = n_pair + n_single;
+    // residual of the boundary condition at row i: difference of the pair, or the value at the single point
+    auto rhs_of = [&](int i) { return sgn * (i < n_pair ? pc[i] - pc[n_pair + i] : pc[n_pair + i]); };
     if (blockIdx.x == 0)
-        for (int i = threadIdx.x; i < rows; i += blockDim.x) rhs[i] = sgn * (pairs ? pc[i] - pc[rows + i] : pc[i]);
-    const int drop = pairs ? 1 : 0;
+        for (int i = threadIdx.x; i < rows; i += blockDim.x) rhs[i] = rhs_of(i);
     if (j < ncol) {
         const double* row = Pinv + (size_t)j * rows;
         double s = 0.0;
-        for (int i = l; i < rows; i += 32) s += row[i] * (sgn * (pairs ? pc[i] - pc[rows + i] : pc[i]));
+        for (int i = l; i < rows; i += 32) s += row[i] * rhs_of(i);
         s = warp_sum(s);
         if (l == 0) A_full[j + drop] = s;
     }

@@ -196,7 +196,9 @@ struct hsma_plan {
     hsma_plan_desc d;
     cudaStream_t stream = nullptr;
     double R0 = 0.0, half[3] = {0, 0, 0};
-    bool pairs = false;       // periodic: rows are differences x_i / x~_i
+    bool pairs = false;       // fully periodic: all rows are differences x_i / x~_i, constant column dropped
+    bool slab_bc = false;     // grounded slab: pair rows wrapped in x,y + Dirichlet rows on the plates
+    int n_pair = 0, n_single = 0, drop = 0;
     bool need_neutral = false;
     int rows = 0, ncol = 0, Kt = 0, C_near = 0, C_rhs = 0, refine = 1;
     long long node_tiles = 0;
@@ -276,8 +278,9 @@ extern "C" hsma_status hsma_plan_create_ex(const hsma_plan_desc* desc, void* cud
     for (int a = 0; a < 3; ++a)
         if (!(d.L[a] > 0.0) || d.near_shell[a] < 0 || d.near_shell[a] > 8) return HSMA_ERR_INVALID_ARG;
     if (d.kind == HSMA_BC_PERIODIC && d.closure != HSMA_CLOSURE_BOUNDARY) return HSMA_ERR_INVALID_ARG;
-    if (d.kind == HSMA_BC_SLAB_XY_PERIODIC_Z_MIRROR && d.closure != HSMA_CLOSURE_FAR_DATA)
-        return HSMA_ERR_INVALID_ARG;  // reading S16: the slab is defined only with the far-data closure
+    if (d.kind == HSMA_BC_SLAB_XY_PERIODIC_Z_MIRROR && d.closure != HSMA_CLOSURE_FAR_DATA && d.gamma != -1.0)
+        return HSMA_ERR_INVALID_ARG;  // reading S16: a dielectric slab is defined only with the far-data closure;
+                                      // grounded plates (gamma = -1) also close by their boundary conditions
     // reading S7: whole-cell near set is valid iff R0 < R_aux <= min_a (s_a + 1/2) L_a
     const double R0 = 0.5 * std::sqrt(d.L[0] * d.L[0] + d.L[1] * d.L[1] + d.L[2] * d.L[2]);
     double bound = 1e300;
@@ -291,7 +294,8 @@ extern "C" hsma_status hsma_plan_create_ex(const hsma_plan_desc* desc, void* cud
     p->R0 = R0;
     for (int a = 0; a < 3; ++a) p->half[a] = 0.5 * d.L[a];
     p->pairs = d.kind == HSMA_BC_PERIODIC;
-    p->need_neutral = d.kind != HSMA_BC_MIRROR_CAVITY;
+    p->slab_bc = d.kind == HSMA_BC_SLAB_XY_PERIODIC_Z_MIRROR && d.closure == HSMA_CLOSURE_BOUNDARY;
+    p->need_neutral = d.kind != HSMA_BC_MIRROR_CAVITY && !p->slab_bc;   // grounded walls screen a net charge
     p->refine = d.rsqrt_refine;  // 0 = by size, see evaluate_impl
     p->rhs_sign = d.closure == HSMA_CLOSURE_FAR_DATA ? 1.0 : -1.0;
     p->sphere = d.near_mode == HSMA_NEAR_SPHERE;
@@ -328,29 +332,39 @@ extern "C" hsma_status hsma_plan_create_ex(const hsma_plan_desc* desc, void* cud
     if (d.check_xyz) x.assign(d.check_xyz, d.check_xyz + 3 * (size_t)d.K);
     else if (p->pairs) x = fibonacci_checkpoints(d.K, R0);
     else {
-        bool use[3] = {true, true, true};
+        bool use[3] = {!p->slab_bc, !p->slab_bc, true};   // grounded slab: points on the two plates only
         x = default_face_points(d.K, d.L, use);
     }
     std::vector<double> chk;
-    if (p->pairs) {  // x~ = x - L round(x/L); rows with x~ = x carry no information
+    if (p->pairs || p->slab_bc) {
+        // x~ = x - L round(x/L) on the periodic axes; rows with x~ = x carry no information
+        const std::vector<double> sph = p->pairs ? x : fibonacci_checkpoints(d.K, R0);
+        const int wrap_axes = p->pairs ? 3 : 2;
         std::vector<double> a, b;
         for (int i = 0; i < d.K; ++i) {
             double w[3]; bool moved = false;
             for (int c = 0; c < 3; ++c) {
-                const double v = x[3 * (size_t)i + c];
-                w[c] = v - d.L[c] * std::nearbyint(v / d.L[c]);
+                const double v = sph[3 * (size_t)i + c];
+                w[c] = c < wrap_axes ? v - d.L[c] * std::nearbyint(v / d.L[c]) : v;
                 moved = moved || std::fabs(v - w[c]) > 0.0;
             }
             if (!moved) continue;
-            for (int c = 0; c < 3; ++c) { a.push_back(x[3 * (size_t)i + c]); b.push_back(w[c]); }
+            for (int c = 0; c < 3; ++c) { a.push_back(sph[3 * (size_t)i + c]); b.push_back(w[c]); }
         }
-        p->rows = (int)(a.size() / 3);
+        p->n_pair = (int)(a.size() / 3);
         chk = a; chk.insert(chk.end(), b.begin(), b.end());
-        p->Kt = 2 * p->rows;
-        p->ncol = d.p * d.p - 1;
+        if (p->slab_bc) {   // + Dirichlet rows on the plates; the constant column stays
+            chk.insert(chk.end(), x.begin(), x.end());
+            p->n_single = d.K; p->drop = 0;
+        } else {
+            p->n_single = 0; p->drop = 1;
+        }
     } else {
-        chk = x; p->rows = d.K; p->Kt = d.K; p->ncol = d.p * d.p;
+        chk = x; p->n_pair = 0; p->n_single = d.K; p->drop = 0;
     }
+    p->rows = p->n_pair + p->n_single;
+    p->Kt = 2 * p->n_pair + p->n_single;
+    p->ncol = d.p * d.p - p->drop;
     if (p->rows < p->ncol || p->ncol < 1) { plan_free(p); return HSMA_ERR_RANK_DEFICIENT; }
     PCU(upload(&p->chk, chk, st));
 
@@ -384,7 +398,7 @@ extern "C" hsma_status hsma_plan_create_ex(const hsma_plan_desc* desc, void* cud
     PCU(cudaMalloc(&p->qinfo, sizeof(QInfo)));
     PCU(cudaMemsetAsync(p->flags, 0, 4 * sizeof(int), st));
     PCU(cudaMemsetAsync(p->A_full, 0, d.p * d.p * sizeof(double), st));
-    build_fit_matrix_kernel<<<(p->rows + 127) / 128, 128, 0, st>>>(p->chk, p->rows, p->pairs ? 1 : 0, d.p, 1.0 / R0, p->Fm);
+    build_fit_matrix_kernel<<<(p->rows + 127) / 128, 128, 0, st>>>(p->chk, p->n_pair, p->n_single, p->drop, d.p, 1.0 / R0, p->Fm);
     HSMA_COUNT_LAUNCH();
     householder_qr_kernel<<<1, 1024, 0, st>>>(p->Fm, p->rows, p->ncol, p->tau, p->Qm, p->Rm, p->flags);
     HSMA_COUNT_LAUNCH();
@@ -512,8 +526,8 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
         HSMA_COUNT_LAUNCH();
     }
     // H3: least squares, Eq.(7)
-    ls_apply_kernel<<<(p->ncol + 7) / 8, 256, 0, st>>>(p->pc, p->rows, p->ncol, p->pairs ? 1 : 0, p->rhs_sign, p->Pinv, p->rhs,
-                                                       p->A_full);
+    ls_apply_kernel<<<(p->ncol + 7) / 8, 256, 0, st>>>(p->pc, p->n_pair, p->n_single, p->ncol, p->drop, p->rhs_sign, p->Pinv,
+                                                       p->rhs, p->A_full);
     HSMA_COUNT_LAUNCH();
     // H4: harmonic surface mapping, Eq.(10),(11) PAPER.md:99-105
     surface_mapping_kernel<<<(d.M + 127) / 128, 128, 0, st>>>(p->A_full, d.p, d.R_aux / p->R0, d.R_aux, p->nrm, p->wq,
@@ -693,7 +707,7 @@ extern "C" hsma_status hsma_get_surface(hsma_plan* p, double* Q_out, double* P_o
 }
 extern "C" hsma_status hsma_get_fit_residual(hsma_plan* p, double* rms_out) {
     if (!p || !rms_out) return HSMA_ERR_INVALID_ARG;
-    r_times_a_kernel<<<1, 256, 0, p->stream>>>(p->Rm, p->A_full, p->ncol, p->pairs ? 1 : 0, p->cvec);
+    r_times_a_kernel<<<1, 256, 0, p->stream>>>(p->Rm, p->A_full, p->ncol, p->drop, p->cvec);
     fit_residual_kernel<<<1, 1024, 0, p->stream>>>(p->rhs, p->rows, p->ncol, p->Qm, p->cvec, p->scalars + 4);
     HSMA_COUNT_LAUNCH(); HSMA_COUNT_LAUNCH();
     CU(cudaMemcpyAsync(rms_out, p->scalars + 4, sizeof(double), cudaMemcpyDeviceToHost, p->stream));

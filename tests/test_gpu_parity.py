@@ -251,6 +251,31 @@ def test_config5_full_size_sampled(H):
     assert abs(float(U.cpu().numpy()[0]) - Uref) <= U_TOL * abs(Uref)
 
 
+# ------------------------------------------------------------------ grounded slab (first part)
+@pytest.mark.parametrize("refine", [1, 2])
+@pytest.mark.parametrize("neutral", [True, False])
+def test_grounded_slab_boundary_closure(H, refine, neutral):
+    """x,y periodic, conducting plates at z = 0, H (gamma = -1), closed by xy-wrapped circumsphere pairs plus
+    Dirichlet rows on the plates (mixed pair / single rows in one fit); also with a net charge."""
+    N = 3000
+    L = (1.0, 1.0, 0.5)
+    xyz = np.random.default_rng(3).random((N, 3)) * np.asarray(L)
+    xyz[:, 2] = 0.02 + 0.92 * xyz[:, 2]
+    q = W.alternating_charges(N) if neutral else np.random.default_rng(4).standard_normal(N) + 0.3
+    w = W.Workload("slab_grounded", W.BC_SLAB_XY_PERIODIC_Z_MIRROR, L, (1, 1, 2), -1.0, 1.1, 14, 8000, 1200, xyz, q,
+                   closure=W.CLOSURE_BOUNDARY)
+    r, phi, U, extra = run_both(H, w, rsqrt_refine=refine)
+    check_parity(r, phi, U, extra, f"grounded slab neutral={neutral} refine={refine}")
+    assert extra["info"]["rows"] == r.rhs.shape[0] and extra["info"]["cols"] == 14 * 14
+    rf = O.hsma(w, forces=True)
+    with H.Plan.from_workload(w, rsqrt_refine=refine) as plan:
+        _, F, _ = plan.evaluate_forces(dev(w.xyz), dev(w.q), sync=True)
+    assert rel_inf(F.cpu().numpy(), rf.F) <= 1e-10
+    with pytest.raises(H.HsmaError) as e:        # a dielectric slab has no boundary closure (reading S16)
+        H.Plan.from_workload(w.with_(gamma=0.5))
+    assert e.value.status == H.HSMA_ERR_INVALID_ARG
+
+
 # ------------------------------------------------------------------ maximum sizes and degenerate inputs
 def test_maximum_degree_p32(H):
     """p = 32 (the library's maximum: 1023 fitted coefficients, 2048 rows), periodic, shell 2."""
