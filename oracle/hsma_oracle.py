@@ -261,6 +261,59 @@ def real_solid_harmonics(xyz, p: int, a: float) -> np.ndarray:
     return B
 
 
+def real_solid_harmonics_grad(xyz, p: int, a: float) -> np.ndarray:
+    """Cartesian gradient of the same basis, G[t, n^2+n+m, :] = grad B_nm(r_t), written out in spherical
+    components and rotated (needed by the Neumann rows, d Phi/d n = 0):
+        d/dr      B = n B / r
+        d/dtheta  B = (r/a)^n N_nm dP_n^m/dtheta {cos, sin}(m phi),
+                      dP_n^m/dtheta = [n cos(th) P_n^m - (n+m) P_{n-1}^m] / sin(th)       (textbook identity)
+        d/dphi    B = m (r/a)^n N_nm P_n^m {-sin, cos}(m phi)
+        grad = r^ d/dr + th^ (1/r) d/dtheta + ph^ (1/(r sin th)) d/dphi.
+    Points on the z axis (sin th = 0) are refused: the formulas divide by sin th."""
+    xyz = np.atleast_2d(np.asarray(xyz, dtype=np.float64))
+    T = xyz.shape[0]
+    x, y, z = xyz[:, 0], xyz[:, 1], xyz[:, 2]
+    r = np.sqrt(x * x + y * y + z * z)
+    st = np.sqrt(x * x + y * y) / r
+    ct = z / r
+    if np.any(st < 1e-9):
+        raise ValueError("gradient of the basis requested on the z axis")
+    ph = np.arctan2(y, x)
+    cp, sp = np.cos(ph), np.sin(ph)
+    rhat = np.stack([st * cp, st * sp, ct], axis=1)
+    that = np.stack([ct * cp, ct * sp, -st], axis=1)
+    phat = np.stack([-sp, cp, np.zeros(T)], axis=1)
+    P = [[None] * (n + 1) for n in range(p)]
+    for m in range(p):
+        dfact = 1.0
+        for k in range(1, 2 * m, 2):
+            dfact *= k
+        P[m][m] = dfact * st ** m
+        if m + 1 < p:
+            P[m + 1][m] = (2 * m + 1) * ct * P[m][m]
+        for n in range(m + 2, p):
+            P[n][m] = ((2 * n - 1) * ct * P[n - 1][m] - (n + m - 1) * P[n - 2][m]) / (n - m)
+    G = np.zeros((T, p * p, 3))
+    rho = r / a
+    for n in range(1, p):
+        rn = rho ** n
+        for m in range(0, n + 1):
+            Nnm = math.sqrt((2 * n + 1) / (4 * math.pi) * math.factorial(n - m) / math.factorial(n + m))
+            Pnm = P[n][m]
+            Pn1m = P[n - 1][m] if m <= n - 1 else 0.0
+            dP = (n * ct * Pnm - (n + m) * Pn1m) / st
+            # members: m = 0 has the cosine one only (trig = 1); m > 0 has cos(m phi) [column +m] and sin(m phi) [column -m]
+            members = [(np.ones(T), np.zeros(T), 0)] if m == 0 else \
+                      [(np.cos(m * ph), -np.sin(m * ph), m), (np.sin(m * ph), np.cos(m * ph), -m)]
+            c = (1.0 if m == 0 else math.sqrt(2.0)) * Nnm * rn
+            for trig, dtrig, mm in members:
+                d_r = n * c * Pnm * trig / r
+                d_t = c * dP * trig / r
+                d_p = c * Pnm * m * dtrig / (r * st)
+                G[:, basis_index(n, mm), :] = d_r[:, None] * rhat + d_t[:, None] * that + d_p[:, None] * phat
+    return G
+
+
 def degree_of_column(p: int) -> np.ndarray:
     return np.array([n for n in range(p) for _ in range(2 * n + 1)], dtype=np.float64)
 
@@ -428,9 +481,24 @@ def hsma(w, targets_slice: Optional[slice] = None, dipole: str = "exact", dr_rel
     # (gamma = -1), closed by the boundary conditions themselves instead of far-cell data
     slab_bc = w.kind == BC_SLAB and w.closure == CLOSURE_BOUNDARY
     n_pair = 0
-    if periodic or (w.kind == BC_SLAB and not slab_bc):
+    # wall rows of the boundary closure on reflecting axes: gamma = -1 is a conductor, Phi = 0
+    # (Dirichlet rows); gamma = +1 is the insulating / symmetric wall, d Phi/d n = 0 (Neumann rows)
+    neumann = w.kind != BC_PERIODIC and w.closure == CLOSURE_BOUNDARY and w.gamma == 1.0
+    if w.kind != BC_PERIODIC and w.closure == CLOSURE_BOUNDARY and w.gamma not in (-1.0, 1.0):
+        raise ValueError("the boundary closure on reflecting walls is defined for gamma = -1 (Dirichlet) or +1 (Neumann)")
+    if periodic or (w.kind == BC_SLAB and not slab_bc) or neumann:
         if abs(q.sum()) > 1e-12 * np.abs(q).sum():
-            raise ValueError("periodic system must be neutral (reading S17)")
+            raise ValueError("periodic / Neumann system must be neutral (reading S17)")
+
+    def wall_rows(xf):
+        """Rows of the fitting matrix at wall points: B(x) (Dirichlet) or dB/dx_a (Neumann), a = the axis whose
+        face the point lies on; returns (rows, axes)."""
+        if not neumann:
+            return real_solid_harmonics(xf, p, R0), None
+        axes = np.argmax(np.isclose(np.abs(xf), 0.5 * L, rtol=0, atol=1e-12 * L.max()) &
+                         np.array([w.kind == BC_MIRROR_CAVITY, w.kind == BC_MIRROR_CAVITY, True]), axis=1)
+        G = real_solid_harmonics_grad(xf, p, R0)
+        return G[np.arange(xf.shape[0]), :, axes], axes
 
     # -- preparation step, PAPER.md:140 ----------------------------------------------------
     near = cell_table(w.kind, L, w.near_shell, w.gamma)
@@ -461,15 +529,15 @@ def hsma(w, targets_slice: Optional[slice] = None, dipole: str = "exact", dr_rel
         #            Phi(x_i) - Phi(x~_i) = 0 (the image system is xy-periodic at every height, also beyond the plates);
         #   plates   K points on the two faces z = +-H/2, Phi = 0 ("DBC").
         # The constant harmonic is seen by the plate rows, so no column is dropped.
-        if w.gamma != -1.0:
-            raise ValueError("the boundary closure of the slab is defined for grounded plates, gamma = -1")
         xs = fibonacci_sphere_checkpoints(w.K, R0)
         xt = wrap_into_box(xs, L, periodic_axes=(True, True, False))
         keep = np.any(np.abs(xs - xt) > 0, axis=1)
         xs, xt = xs[keep], xt[keep]
         xf = default_face_points(w.K, L, (2,)) if w.check_xyz is None else np.asarray(w.check_xyz, float)
-        F = np.concatenate([real_solid_harmonics(xs, p, R0) - real_solid_harmonics(xt, p, R0),
-                            real_solid_harmonics(xf, p, R0)], axis=0)
+        Fw, wall_axes = wall_rows(xf)
+        F = np.concatenate([real_solid_harmonics(xs, p, R0) - real_solid_harmonics(xt, p, R0), Fw], axis=0)
+        if neumann:
+            F = F[:, 1:]                                  # neither family of rows sees the constant: A00 = 0
         check_targets = np.concatenate([xs, xt, xf], axis=0)
         n_pair = xs.shape[0]
     else:
@@ -479,9 +547,12 @@ def hsma(w, targets_slice: Optional[slice] = None, dipole: str = "exact", dr_rel
             x = default_face_points(w.K, L, (0, 1, 2))
         else:
             x = default_face_points(w.K, L, (0, 1, 2) if w.kind == BC_MIRROR_CAVITY else (2,))
-        if w.kind == BC_SLAB and w.closure != CLOSURE_FAR_DATA:
-            raise ValueError("slab kind is defined only with the far-data closure (reading S16)")
-        F = real_solid_harmonics(x, p, R0)
+        if w.closure == CLOSURE_FAR_DATA:
+            F, wall_axes = real_solid_harmonics(x, p, R0), None
+        else:
+            F, wall_axes = wall_rows(x)
+            if neumann:
+                F = F[:, 1:]
         check_targets = x
     nodes, nrm, wq = make_nodes(M, w.R_aux, w.quad_rule)
     Ynodes = real_solid_harmonics(nodes, p, w.R_aux)      # = Y_nm at the node directions (r = a)
@@ -499,14 +570,18 @@ def hsma(w, targets_slice: Optional[slice] = None, dipole: str = "exact", dr_rel
         if periodic:
             K = x.shape[0]
             rhs = -(phi_check[:K] - phi_check[K:])        # v_i = Phi(x_i) - Phi(x~_i) = 0
-        elif slab_bc:
-            rhs = np.concatenate([-(phi_check[:n_pair] - phi_check[n_pair:2 * n_pair]), -phi_check[2 * n_pair:]])
         else:
-            rhs = -phi_check                              # grounded wall: Phi_in + Phi_out = 0
+            xw = check_targets[2 * n_pair:]               # the wall points (all of them in the cavity)
+            if neumann:                                   # d(Phi_in + Phi_out)/d x_a = 0 on the wall
+                gw = near_grad(xw, near_src, near_q, near_cells)
+                wall_rhs = -gw[np.arange(xw.shape[0]), wall_axes]
+            else:                                         # grounded wall: Phi_in + Phi_out = 0
+                wall_rhs = -phi_check[2 * n_pair:]
+            rhs = np.concatenate([-(phi_check[:n_pair] - phi_check[n_pair:2 * n_pair]), wall_rhs])
     # least squares, Eq.(7)
     sol, *_ = np.linalg.lstsq(F, rhs, rcond=None)
     sv = np.linalg.svd(F, compute_uv=False)
-    A = np.concatenate([[0.0], sol]) if periodic else sol
+    A = np.concatenate([[0.0], sol]) if (periodic or neumann) else sol
     fit_rms = float(np.linalg.norm(F @ sol - rhs) / math.sqrt(F.shape[0]))
 
     # harmonic surface mapping, Eq.(10),(11) PAPER.md:99-105: on |r'| = R_aux
