@@ -54,7 +54,10 @@ typedef enum {
     HSMA_CLOSURE_BOUNDARY = 0, /* residual of the boundary condition at the check points.  Periodic:
                                   K circumsphere points and their wrapped partners; cavity: K Dirichlet points on the
                                   faces; grounded slab: K circumsphere points wrapped in x,y only PLUS K Dirichlet points
-                                  on the two plates (check_xyz, if given, are the plate points) -- DESIGN.md 6.8 */
+                                  on the two plates (check_xyz, if given, are the plate points) -- DESIGN.md 6.8.
+                                  On reflecting walls gamma must be -1 (conductor: Dirichlet rows Phi = 0) or +1
+                                  (Neumann rows d Phi/d n = 0: wall points must lie exactly on a wall,
+                                  the input must be neutral and phi is in the gauge A_00 = 0) */
     HSMA_CLOSURE_FAR_DATA = 1  /* rhs = direct sum over the far cell table (reading S16, config 4)       */
 } hsma_closure;
 
@@ -82,7 +85,8 @@ typedef struct {
     int kind;             /* hsma_boundary_kind */
     double L[3];          /* box sides */
     int near_shell[3];    /* near cells |k_a| <= near_shell[a]; whole cells (reading S7) */
-    double gamma;         /* reflection factor per mirror reflection (-1 = grounded metal) */
+    double gamma;         /* reflection factor per mirror reflection (-1 = grounded metal; +1 = Neumann wall;
+                             other values only with HSMA_CLOSURE_FAR_DATA) */
     double R_aux;         /* radius of the auxiliary sphere */
     int p;                /* harmonic degrees n = 0..p-1, p*p unknowns (reading S1); 1 <= p <= 32 */
     int M;                /* integration nodes on the sphere; M >= 8 */

@@ -46,17 +46,64 @@ __device__ __forceinline__ void solid_harmonics(double x, double y, double z, do
     }
 }
 
+// The same recurrences carried in forward mode: value and Cartesian gradient of every basis function (plan time
+// only: the Neumann rows d Phi/d n = 0 of DESIGN.md 6.9).  g(n, m, vc, vs) receives the cos/sin members as D4.
+struct D4 { double v, x, y, z; };
+__device__ __forceinline__ D4 operator+(D4 a, D4 b) { return {a.v + b.v, a.x + b.x, a.y + b.y, a.z + b.z}; }
+__device__ __forceinline__ D4 operator-(D4 a, D4 b) { return {a.v - b.v, a.x - b.x, a.y - b.y, a.z - b.z}; }
+__device__ __forceinline__ D4 operator*(D4 a, D4 b) {
+    return {a.v * b.v, a.x * b.v + a.v * b.x, a.y * b.v + a.v * b.y, a.z * b.v + a.v * b.z};
+}
+__device__ __forceinline__ D4 operator*(double k, D4 a) { return {k * a.v, k * a.x, k * a.y, k * a.z}; }
+template <class F>
+__device__ __forceinline__ void solid_harmonics_grad(double x, double y, double z, double inv_a, int p, F f) {
+    const D4 xr{x * inv_a, inv_a, 0.0, 0.0}, xi{y * inv_a, 0.0, inv_a, 0.0}, zeta{z * inv_a, 0.0, 0.0, inv_a};
+    const D4 rho2 = xr * xr + xi * xi + zeta * zeta;
+    D4 er{kSqrtInv4Pi, 0.0, 0.0, 0.0}, ei{0.0, 0.0, 0.0, 0.0};
+    for (int m = 0; m < p; ++m) {
+        if (m > 0) {
+            const double k = sqrt((2.0 * m + 1.0) / (2.0 * m));
+            const D4 nr = k * (er * xr - ei * xi), ni = k * (er * xi + ei * xr);
+            er = nr; ei = ni;
+        }
+        const double s = m == 0 ? 1.0 : 1.4142135623730951;
+        D4 c2{0.0, 0.0, 0.0, 0.0}, s2{0.0, 0.0, 0.0, 0.0};
+        D4 c1 = er, s1 = ei;
+        f(m, m, s * c1, s * s1);
+        for (int n = m + 1; n < p; ++n) {
+            const double nn = (double)n, mm = (double)m;
+            const double anm = sqrt((4.0 * nn * nn - 1.0) / (nn * nn - mm * mm));
+            const double bnm = n == m + 1 ? 0.0 : sqrt(((nn - 1.0) * (nn - 1.0) - mm * mm) / (4.0 * (nn - 1.0) * (nn - 1.0) - 1.0));
+            const D4 c0 = anm * (zeta * c1 - bnm * (rho2 * c2));
+            const D4 s0 = anm * (zeta * s1 - bnm * (rho2 * s2));
+            f(n, m, s * c0, s * s0);
+            c2 = c1; s2 = s1; c1 = c0; s1 = s0;
+        }
+    }
+}
+
 // Fitting matrix, column-major [rows x ncol] (ld = rows), rows = n_pair + n_single.  PAPER.md:72-82.
 //   pair rows   (i < n_pair):  row_i = B(x_i) - B(x~_i),  x_i = chk[i], x~_i = chk[n_pair + i]   (periodic axes)
 //   single rows (the rest):    row_i = B(y_i),            y_i = chk[2 n_pair + (i - n_pair)]     (Dirichlet / data)
-//   drop = 1: the constant column is dropped (fully periodic kind, reading S2): col = idx - 1
+//   single rows with row_axis[i - n_pair] = a in {0,1,2}: row_i = dB/dx_a (y_i)  (Neumann wall)
+//   drop = 1: the constant column is dropped (no row sees it: fully periodic kind, reading S2; Neumann walls)
 __global__ void build_fit_matrix_kernel(const double* __restrict__ chk, int n_pair, int n_single, int drop, int p,
-                                        double inv_R0, double* __restrict__ Fm) {
+                                        double inv_R0, const int* __restrict__ row_axis /* [n_single] or null */,
+                                        double* __restrict__ Fm) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int rows = n_pair + n_single;
     if (i >= rows) return;
     const bool pairs = i < n_pair;
     const double* a = chk + 3 * (size_t)(pairs ? i : n_pair + i);
+    const int axis = (!pairs && row_axis) ? row_axis[i - n_pair] : -1;
+    if (axis >= 0) {
+        solid_harmonics_grad(a[0], a[1], a[2], inv_R0, p, [&](int n, int m, D4 vc, D4 vs) {
+            const int cc = n * n + n + m - drop, cs = n * n + n - m - drop;
+            if (cc >= 0) Fm[(size_t)cc * rows + i] = axis == 0 ? vc.x : (axis == 1 ? vc.y : vc.z);
+            if (m > 0) Fm[(size_t)cs * rows + i] = axis == 0 ? vs.x : (axis == 1 ? vs.y : vs.z);
+        });
+        return;
+    }
     solid_harmonics(a[0], a[1], a[2], inv_R0, p, [&](int n, int m, double vc, double vs) {
         const int cc = n * n + n + m - drop, cs = n * n + n - m - drop;
         if (cc >= 0) Fm[(size_t)cc * rows + i] = vc;
@@ -169,14 +216,20 @@ __global__ void pinv_kernel(const double* __restrict__ Qm, const double* __restr
 
 // H3 (update step): rhs from the check-point sums, A = Pinv rhs.  One warp per coefficient, 8 warps per block;
 // block 0 also stores rhs.  Fixed summation order (lane-strided partial sums, xor-shuffle tree).
-__global__ void __launch_bounds__(256) ls_apply_kernel(const double* __restrict__ pc, int n_pair, int n_single, int ncol,
-                                                       int drop, double sgn, const double* __restrict__ Pinv,
+__global__ void __launch_bounds__(256) ls_apply_kernel(const double* __restrict__ pc, const double* __restrict__ pcg,
+                                                       const int* __restrict__ row_axis, int n_pair, int n_single,
+                                                       int ncol, int drop, double sgn, const double* __restrict__ Pinv,
                                                        double* __restrict__ rhs, double* __restrict__ A_full) {
     const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
     const int j = blockIdx.x * 8 + w;
     const int rows = n_pair + n_single;
-    // residual of the boundary condition at row i: difference of the pair, or the value at the single point
-    auto rhs_of = [&](int i) { return sgn * (i < n_pair ? pc[i] - pc[n_pair + i] : pc[n_pair + i]); };
+    // residual of the boundary condition at row i: difference of the pair, the value at the single point, or
+    // (Neumann rows) the component row_axis of grad Phi_in there (pcg [K_t,3])
+    auto rhs_of = [&](int i) {
+        if (i < n_pair) return sgn * (pc[i] - pc[n_pair + i]);
+        if (row_axis && row_axis[i - n_pair] >= 0) return sgn * pcg[3 * (size_t)(n_pair + i) + row_axis[i - n_pair]];
+        return sgn * pc[n_pair + i];
+    };
     if (blockIdx.x == 0)
         for (int i = threadIdx.x; i < rows; i += blockDim.x) rhs[i] = rhs_of(i);
     if (j < ncol) {

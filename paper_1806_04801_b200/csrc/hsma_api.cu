@@ -199,6 +199,9 @@ struct hsma_plan {
     bool pairs = false;       // fully periodic: all rows are differences x_i / x~_i, constant column dropped
     bool slab_bc = false;     // grounded slab: pair rows wrapped in x,y + Dirichlet rows on the plates
     int n_pair = 0, n_single = 0, drop = 0;
+    bool neumann = false;     // gamma = +1 walls: derivative rows, step (a) also needs grad Phi_in
+    int* row_axis = nullptr;  // [n_single] axis of the wall of each single row (Neumann), else null
+    double* pcg = nullptr;    // [Kt,3] grad Phi_in at the check targets (Neumann)
     bool need_neutral = false;
     int rows = 0, ncol = 0, Kt = 0, C_near = 0, C_rhs = 0, refine = 1;
     long long node_tiles = 0;
@@ -248,6 +251,8 @@ static void plan_free(hsma_plan* p) {
     for (void* q : ptrs) if (q) cudaFree(q);
     p->src.release(); p->slot_of.release(); p->tile_np.release(); if (p->qinfo) cudaFree(p->qinfo);
     if (p->cell_identity) cudaFree(p->cell_identity);
+    if (p->row_axis) cudaFree(p->row_axis);
+    if (p->pcg) cudaFree(p->pcg);
     if (p->cell_order) cudaFree(p->cell_order);
     if (p->img_qinfo) cudaFree(p->img_qinfo);
     p->img_counts.release(); p->img_xyz.release(); p->img_q.release(); p->img_stats.release(); p->img_src.release();
@@ -278,9 +283,9 @@ extern "C" hsma_status hsma_plan_create_ex(const hsma_plan_desc* desc, void* cud
     for (int a = 0; a < 3; ++a)
         if (!(d.L[a] > 0.0) || d.near_shell[a] < 0 || d.near_shell[a] > 8) return HSMA_ERR_INVALID_ARG;
     if (d.kind == HSMA_BC_PERIODIC && d.closure != HSMA_CLOSURE_BOUNDARY) return HSMA_ERR_INVALID_ARG;
-    if (d.kind == HSMA_BC_SLAB_XY_PERIODIC_Z_MIRROR && d.closure != HSMA_CLOSURE_FAR_DATA && d.gamma != -1.0)
-        return HSMA_ERR_INVALID_ARG;  // reading S16: a dielectric slab is defined only with the far-data closure;
-                                      // grounded plates (gamma = -1) also close by their boundary conditions
+    if (d.kind != HSMA_BC_PERIODIC && d.closure == HSMA_CLOSURE_BOUNDARY && d.gamma != -1.0 && d.gamma != 1.0)
+        return HSMA_ERR_INVALID_ARG;  // reading S16: a dielectric wall has no boundary closure (far-data closure only);
+                                      // gamma = -1 closes by Dirichlet rows, gamma = +1 by Neumann rows
     // reading S7: whole-cell near set is valid iff R0 < R_aux <= min_a (s_a + 1/2) L_a
     const double R0 = 0.5 * std::sqrt(d.L[0] * d.L[0] + d.L[1] * d.L[1] + d.L[2] * d.L[2]);
     double bound = 1e300;
@@ -295,7 +300,8 @@ extern "C" hsma_status hsma_plan_create_ex(const hsma_plan_desc* desc, void* cud
     for (int a = 0; a < 3; ++a) p->half[a] = 0.5 * d.L[a];
     p->pairs = d.kind == HSMA_BC_PERIODIC;
     p->slab_bc = d.kind == HSMA_BC_SLAB_XY_PERIODIC_Z_MIRROR && d.closure == HSMA_CLOSURE_BOUNDARY;
-    p->need_neutral = d.kind != HSMA_BC_MIRROR_CAVITY && !p->slab_bc;   // grounded walls screen a net charge
+    p->neumann = d.kind != HSMA_BC_PERIODIC && d.closure == HSMA_CLOSURE_BOUNDARY && d.gamma == 1.0;
+    p->need_neutral = (d.kind != HSMA_BC_MIRROR_CAVITY && !p->slab_bc) || p->neumann;   // grounded walls screen a net charge
     p->refine = d.rsqrt_refine;  // 0 = by size, see evaluate_impl
     p->rhs_sign = d.closure == HSMA_CLOSURE_FAR_DATA ? 1.0 : -1.0;
     p->sphere = d.near_mode == HSMA_NEAR_SPHERE;
@@ -355,12 +361,24 @@ extern "C" hsma_status hsma_plan_create_ex(const hsma_plan_desc* desc, void* cud
         chk = a; chk.insert(chk.end(), b.begin(), b.end());
         if (p->slab_bc) {   // + Dirichlet rows on the plates; the constant column stays
             chk.insert(chk.end(), x.begin(), x.end());
-            p->n_single = d.K; p->drop = 0;
+            p->n_single = d.K; p->drop = p->neumann ? 1 : 0;
         } else {
             p->n_single = 0; p->drop = 1;
         }
     } else {
-        chk = x; p->n_pair = 0; p->n_single = d.K; p->drop = 0;
+        chk = x; p->n_pair = 0; p->n_single = d.K; p->drop = p->neumann ? 1 : 0;
+    }
+    if (p->neumann) {   // the wall each single point lies on: the reflecting axis with |x_a| = L_a/2
+        std::vector<int> axis(p->n_single, 2);
+        const int first_axis = d.kind == HSMA_BC_MIRROR_CAVITY ? 0 : 2;
+        for (int i = 0; i < p->n_single; ++i) {
+            int found = -1;
+            for (int a = first_axis; a < 3 && found < 0; ++a)
+                if (std::fabs(std::fabs(x[3 * (size_t)i + a]) - 0.5 * d.L[a]) <= 1e-12 * std::max({d.L[0], d.L[1], d.L[2]})) found = a;
+            if (found < 0) { plan_free(p); return HSMA_ERR_INVALID_ARG; }   // a wall point that is on no wall
+            axis[i] = found;
+        }
+        PCU(upload(&p->row_axis, axis, st));
     }
     p->rows = p->n_pair + p->n_single;
     p->Kt = 2 * p->n_pair + p->n_single;
@@ -390,6 +408,7 @@ extern "C" hsma_status hsma_plan_create_ex(const hsma_plan_desc* desc, void* cud
     PCU(cudaMalloc(&p->Pinv, mn * sizeof(double)));
     PCU(cudaMalloc(&p->tau, p->ncol * sizeof(double)));
     PCU(cudaMalloc(&p->pc, p->Kt * sizeof(double)));
+    if (p->neumann) PCU(cudaMalloc(&p->pcg, 3 * (size_t)p->Kt * sizeof(double)));
     PCU(cudaMalloc(&p->rhs, p->rows * sizeof(double)));
     PCU(cudaMalloc(&p->cvec, p->ncol * sizeof(double)));
     PCU(cudaMalloc(&p->A_full, d.p * d.p * sizeof(double)));
@@ -398,7 +417,7 @@ extern "C" hsma_status hsma_plan_create_ex(const hsma_plan_desc* desc, void* cud
     PCU(cudaMalloc(&p->qinfo, sizeof(QInfo)));
     PCU(cudaMemsetAsync(p->flags, 0, 4 * sizeof(int), st));
     PCU(cudaMemsetAsync(p->A_full, 0, d.p * d.p * sizeof(double), st));
-    build_fit_matrix_kernel<<<(p->rows + 127) / 128, 128, 0, st>>>(p->chk, p->n_pair, p->n_single, p->drop, d.p, 1.0 / R0, p->Fm);
+    build_fit_matrix_kernel<<<(p->rows + 127) / 128, 128, 0, st>>>(p->chk, p->n_pair, p->n_single, p->drop, d.p, 1.0 / R0, p->row_axis, p->Fm);
     HSMA_COUNT_LAUNCH();
     householder_qr_kernel<<<1, 1024, 0, st>>>(p->Fm, p->rows, p->ncol, p->tau, p->Qm, p->Rm, p->flags);
     HSMA_COUNT_LAUNCH();
@@ -517,17 +536,21 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
 
     // H2 (a): Phi_in (or the far-cell data) at the monitoring points -> pc [Kt]
     {
-        const Launch s = choose_near(p->Kt, n_tiles_near, C_a, 2);
-        if (p->part_a.reserve((size_t)s.rows * p->Kt) != cudaSuccess) return HSMA_ERR_ALLOC;
+        const bool fa = p->neumann;   // Neumann rows need grad Phi_in at the wall points: the FIELD form of (a)
+        const Launch s = choose_near(p->Kt, n_tiles_near, C_a, 2, fa);
+        if (p->part_a.reserve((size_t)s.rows * p->Kt * (fa ? 4 : 1)) != cudaSuccess) return HSMA_ERR_ALLOC;
         MARK(1);
-        launch_near(s, false, p->chk, 3, nullptr, p->Kt, 0, P, cells_a, C_a, -1, 2, p->part_a.p, st);  // (a) always cubic: it feeds the fit
+        launch_near(s, fa, p->chk, 3, nullptr, p->Kt, 0, P, cells_a, C_a, -1, 2, p->part_a.p, st);  // (a) always cubic: it feeds the fit
         MARK(2);
-        finish_phi_kernel<<<(p->Kt + 255) / 256, 256, 0, st>>>(s.layout(p->part_a.p), PartLayout{nullptr, 1, 1, 1, 1}, p->Kt, nullptr, nullptr, 0, p->pc, nullptr);
+        if (fa)
+            finish_field_kernel<<<(p->Kt + 255) / 256, 256, 0, st>>>(s.layout(p->part_a.p), PartLayout{nullptr, 1, 1, 1, 1}, p->Kt, nullptr, nullptr, 0, p->pc, p->pcg, nullptr);
+        else
+            finish_phi_kernel<<<(p->Kt + 255) / 256, 256, 0, st>>>(s.layout(p->part_a.p), PartLayout{nullptr, 1, 1, 1, 1}, p->Kt, nullptr, nullptr, 0, p->pc, nullptr);
         HSMA_COUNT_LAUNCH();
     }
     // H3: least squares, Eq.(7)
-    ls_apply_kernel<<<(p->ncol + 7) / 8, 256, 0, st>>>(p->pc, p->n_pair, p->n_single, p->ncol, p->drop, p->rhs_sign, p->Pinv,
-                                                       p->rhs, p->A_full);
+    ls_apply_kernel<<<(p->ncol + 7) / 8, 256, 0, st>>>(p->pc, p->pcg, p->row_axis, p->n_pair, p->n_single, p->ncol, p->drop,
+                                                       p->rhs_sign, p->Pinv, p->rhs, p->A_full);
     HSMA_COUNT_LAUNCH();
     // H4: harmonic surface mapping, Eq.(10),(11) PAPER.md:99-105
     surface_mapping_kernel<<<(d.M + 127) / 128, 128, 0, st>>>(p->A_full, d.p, d.R_aux / p->R0, d.R_aux, p->nrm, p->wq,

@@ -276,6 +276,42 @@ def test_grounded_slab_boundary_closure(H, refine, neutral):
     assert e.value.status == H.HSMA_ERR_INVALID_ARG
 
 
+# ------------------------------------------------------------------ Neumann walls
+@pytest.mark.parametrize("which", ["cavity", "slab"])
+@pytest.mark.parametrize("refine", [1, 2])
+def test_neumann_walls(H, which, refine):
+    """gamma = +1: d Phi/d n = 0 on the reflecting walls; derivative rows in the fit, grad Phi_in at the wall
+    points from the FIELD form of step (a), constant column dropped, neutral input required."""
+    rng = np.random.default_rng(21)
+    N = 2500
+    if which == "cavity":
+        L = (1.0, 1.0, 1.0)
+        xyz = 0.03 + 0.94 * rng.random((N, 3))
+        chk = W.seeded_face_points(1100, L, W.ALL_FACES, seed=31)
+        w = W.Workload("neumann_cavity", W.BC_MIRROR_CAVITY, L, (1, 1, 1), 1.0, 1.5 * math.sqrt(3) / 2, 14, 6000,
+                       1100, xyz, W.alternating_charges(N), check_xyz=chk)
+    else:
+        L = (1.0, 1.0, 0.5)
+        xyz = rng.random((N, 3)) * np.asarray(L)
+        xyz[:, 2] = 0.02 + 0.92 * xyz[:, 2]
+        q = rng.standard_normal(N)
+        q -= q.mean()
+        w = W.Workload("neumann_slab", W.BC_SLAB_XY_PERIODIC_Z_MIRROR, L, (1, 1, 2), 1.0, 1.1, 14, 8000, 1200, xyz, q,
+                       closure=W.CLOSURE_BOUNDARY)
+    r, phi, U, extra = run_both(H, w, rsqrt_refine=refine)
+    check_parity(r, phi, U, extra, f"neumann {which} refine={refine}")
+    assert extra["A"][0] == 0.0 and extra["info"]["cols"] == 14 * 14 - 1
+    rf = O.hsma(w, forces=True)
+    with H.Plan.from_workload(w, rsqrt_refine=refine) as plan:
+        _, F, _ = plan.evaluate_forces(dev(w.xyz), dev(w.q), sync=True)
+        assert rel_inf(F.cpu().numpy(), rf.F) <= 1e-10
+        bad = w.q.copy()
+        bad[0] += 0.5
+        with pytest.raises(H.HsmaError) as e:
+            plan.evaluate(dev(w.xyz), dev(bad), sync=True)
+        assert e.value.status == H.HSMA_ERR_NOT_NEUTRAL
+
+
 # ------------------------------------------------------------------ maximum sizes and degenerate inputs
 def test_maximum_degree_p32(H):
     """p = 32 (the library's maximum: 1023 fitted coefficients, 2048 rows), periodic, shell 2."""
