@@ -32,6 +32,8 @@ BC_SLAB_XY_PERIODIC_Z_MIRROR = 2
 # closures (values match include/hsma.h)
 CLOSURE_BOUNDARY = 0   # residual of the boundary condition at the check points
 CLOSURE_FAR_DATA = 1   # explicit far-cell data at the check points (reading S16)
+CLOSURE_FACE_PAIRS = 2 # periodic: value + normal-derivative pairs on opposite faces (reading S15)
+LOWER_FACES = [(0, -1), (1, -1), (2, -1)]   # the faces x_a = -L_a/2 (their partners are on the opposite faces)
 
 # quadrature rules (values match include/hsma.h)
 QUAD_SPIRAL = 0        # exactly M nodes (reading S10)

@@ -58,7 +58,11 @@ typedef enum {
                                   On reflecting walls gamma must be -1 (conductor: Dirichlet rows Phi = 0) or +1
                                   (Neumann rows d Phi/d n = 0: wall points must lie exactly on a wall,
                                   the input must be neutral and phi is in the gauge A_00 = 0) */
-    HSMA_CLOSURE_FAR_DATA = 1  /* rhs = direct sum over the far cell table (reading S16, config 4)       */
+    HSMA_CLOSURE_FAR_DATA = 1, /* rhs = direct sum over the far cell table (reading S16, config 4)       */
+    HSMA_CLOSURE_FACE_PAIRS = 2 /* periodic kind only -- BASELINE.json's "check-point pairs on opposite faces" made
+                                  well posed (reading S15): K points on the lower faces x_a = -L_a/2
+                                  (check_xyz, or the library's lattice) and their partners on the opposite faces;
+                                  each pair gives a value row AND a normal-derivative row (2K rows) */
 } hsma_closure;
 
 typedef enum {

@@ -30,7 +30,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB = None
 
 BC_PERIODIC, BC_MIRROR_CAVITY, BC_SLAB = 0, 1, 2
-CLOSURE_BOUNDARY, CLOSURE_FAR_DATA = 0, 1
+CLOSURE_BOUNDARY, CLOSURE_FAR_DATA, CLOSURE_FACE_PAIRS = 0, 1, 2
 QUAD_SPIRAL, QUAD_LATTICE = 0, 1
 NEAR_WHOLE_CELLS, NEAR_SPHERE = 0, 1
 DIPOLE_EXACT, DIPOLE_FD3 = 0, 1
@@ -375,6 +375,27 @@ def default_face_points(K: int, L, axes) -> np.ndarray:
 # --------------------------------------------------------------------------------------
 # Integration nodes on the auxiliary sphere
 # --------------------------------------------------------------------------------------
+def default_lower_face_points(K: int, L) -> np.ndarray:
+    """The face-pair closure's default points: the same lattice rule as default_face_points, on the three lower
+    faces x_a = -L_a/2 only (face f gets floor(K a_f / sum a) points, leftovers one each to the first faces)."""
+    L = np.asarray(L, dtype=np.float64)
+    areas = np.array([np.prod(np.delete(L, a)) for a in range(3)])
+    cnt = np.floor(K * areas / areas.sum()).astype(int)
+    for f in range(K - int(cnt.sum())):
+        cnt[f] += 1
+    g1, g2 = 1.0 / PLASTIC, 1.0 / (PLASTIC * PLASTIC)
+    pts = np.zeros((K, 3))
+    n = 0
+    for a in range(3):
+        u_ax, v_ax = [b for b in range(3) if b != a]
+        for _ in range(cnt[a]):
+            pts[n, a] = -0.5 * L[a]
+            pts[n, u_ax] = (math.fmod(0.5 + (n + 1) * g1, 1.0) - 0.5) * L[u_ax]
+            pts[n, v_ax] = (math.fmod(0.5 + (n + 1) * g2, 1.0) - 0.5) * L[v_ax]
+            n += 1
+    return pts
+
+
 def fibonacci_pair(F2: int):
     a, b = 1, 1
     while b < F2:
@@ -506,14 +527,34 @@ def hsma(w, targets_slice: Optional[slice] = None, dipole: str = "exact", dr_rel
     # identity cell; otherwise the whole cells of the table (reading S7)
     sphere = getattr(w, "near_mode", NEAR_WHOLE_CELLS) == NEAR_SPHERE
     if sphere:
-        if w.closure != CLOSURE_BOUNDARY:
-            raise ValueError("the sphere-culled near set is defined for the boundary closure")
+        if w.closure == CLOSURE_FAR_DATA:
+            raise ValueError("the sphere-culled near set is defined for the boundary closures")
         near_src, near_q, near_cells = (*images_inside_sphere(src, q, near, w.R_aux), identity_cell())
     else:
         near_src, near_q, near_cells = src, q, near
-    if periodic:
+    face_pairs = periodic and w.closure == CLOSURE_FACE_PAIRS
+    if face_pairs:
+        # BASELINE.json: "check-point pairs on opposite faces".  Matching the values alone is rank deficient (every
+        # harmonic even in x, y and z is invisible, reading S15); periodicity of Phi AND of its normal derivative
+        # across the faces is the complete condition: K points on the lower faces x_a = -L_a/2, partners x + L_a e_a,
+        # one value row and one derivative row per pair.  The constant is dropped (reading S2).
+        x = default_lower_face_points(w.K, L) if w.check_xyz is None else np.asarray(w.check_xyz, float)
+        on = np.isclose(x, -0.5 * L, rtol=0, atol=1e-12 * L.max())
+        if not on.any(axis=1).all():
+            raise ValueError("face-pair check points must lie on the lower faces x_a = -L_a/2")
+        pair_axes = np.argmax(on, axis=1)
+        xt = x.copy()
+        xt[np.arange(x.shape[0]), pair_axes] += L[pair_axes]
+        idx = np.arange(x.shape[0])
+        Fv = real_solid_harmonics(x, p, R0) - real_solid_harmonics(xt, p, R0)
+        Fd = (real_solid_harmonics_grad(x, p, R0)[idx, :, pair_axes]
+              - real_solid_harmonics_grad(xt, p, R0)[idx, :, pair_axes])
+        F = np.concatenate([Fv, Fd], axis=0)[:, 1:]
+        check_targets = np.concatenate([x, xt], axis=0)
+        n_pair = x.shape[0]
+    elif periodic:
         if w.closure != CLOSURE_BOUNDARY:
-            raise ValueError("periodic kind uses the boundary closure")
+            raise ValueError("periodic kind uses the boundary or the face-pair closure")
         x = fibonacci_sphere_checkpoints(w.K, R0) if w.check_xyz is None else np.asarray(w.check_xyz, float)
         xt = wrap_into_box(x, L)
         keep = np.any(np.abs(x - xt) > 0, axis=1)       # rows with x~ = x carry no information
@@ -567,7 +608,11 @@ def hsma(w, targets_slice: Optional[slice] = None, dipole: str = "exact", dr_rel
     else:
         phi_check = near_sum(check_targets, near_src, near_q, near_cells)
         n_check_cells = near.w.shape[0]
-        if periodic:
+        if face_pairs:
+            K = x.shape[0]
+            g = near_grad(check_targets, near_src, near_q, near_cells)[np.arange(2 * K), np.tile(pair_axes, 2)]
+            rhs = np.concatenate([-(phi_check[:K] - phi_check[K:]), -(g[:K] - g[K:])])
+        elif periodic:
             K = x.shape[0]
             rhs = -(phi_check[:K] - phi_check[K:])        # v_i = Phi(x_i) - Phi(x~_i) = 0
         else:

@@ -21,7 +21,7 @@ HSMA_OK = 0
 HSMA_ERR_INVALID_ARG, HSMA_ERR_GEOMETRY, HSMA_ERR_NOT_NEUTRAL = -1, -2, -3
 HSMA_ERR_CUDA, HSMA_ERR_ALLOC, HSMA_ERR_RANK_DEFICIENT = -4, -5, -6
 HSMA_BC_PERIODIC, HSMA_BC_MIRROR_CAVITY, HSMA_BC_SLAB_XY_PERIODIC_Z_MIRROR = 0, 1, 2
-HSMA_CLOSURE_BOUNDARY, HSMA_CLOSURE_FAR_DATA = 0, 1
+HSMA_CLOSURE_BOUNDARY, HSMA_CLOSURE_FAR_DATA, HSMA_CLOSURE_FACE_PAIRS = 0, 1, 2
 HSMA_QUAD_SPIRAL, HSMA_QUAD_LATTICE = 0, 1
 HSMA_NEAR_WHOLE_CELLS, HSMA_NEAR_SPHERE = 0, 1
 HSMA_DIPOLE_EXACT, HSMA_DIPOLE_FD3 = 0, 1

@@ -82,40 +82,40 @@ __device__ __forceinline__ void solid_harmonics_grad(double x, double y, double 
     }
 }
 
-// Fitting matrix, column-major [rows x ncol] (ld = rows), rows = n_pair + n_single.  PAPER.md:72-82.
-//   pair rows   (i < n_pair):  row_i = B(x_i) - B(x~_i),  x_i = chk[i], x~_i = chk[n_pair + i]   (periodic axes)
-//   single rows (the rest):    row_i = B(y_i),            y_i = chk[2 n_pair + (i - n_pair)]     (Dirichlet / data)
-//   single rows with row_axis[i - n_pair] = a in {0,1,2}: row_i = dB/dx_a (y_i)  (Neumann wall)
-//   drop = 1: the constant column is dropped (no row sees it: fully periodic kind, reading S2; Neumann walls)
-__global__ void build_fit_matrix_kernel(const double* __restrict__ chk, int n_pair, int n_single, int drop, int p,
-                                        double inv_R0, const int* __restrict__ row_axis /* [n_single] or null */,
-                                        double* __restrict__ Fm) {
+// One row of the least-squares problem: the residual of a boundary condition,
+//   row = D B(chk[i1]) - D B(chk[i2]),   rhs = -(D Phi_in(chk[i1]) - D Phi_in(chk[i2]))      (i2 < 0: no second point)
+// with D = identity (axis < 0) or d/dx_axis.  Pair rows express periodicity (and for the face-pair
+// closure also of the normal derivative); single value rows a grounded wall or given data; single derivative rows a
+// Neumann wall.
+struct RowDesc { int i1, i2, axis, pad; };
+
+// Fitting matrix, column-major [rows x ncol] (ld = rows).  drop = 1: the constant column is dropped because no row
+// sees it (periodic kinds, reading S2; Neumann walls): col = idx - 1.
+__global__ void build_fit_matrix_kernel(const double* __restrict__ chk, const RowDesc* __restrict__ desc, int rows,
+                                        int drop, int p, double inv_R0, double* __restrict__ Fm) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    const int rows = n_pair + n_single;
     if (i >= rows) return;
-    const bool pairs = i < n_pair;
-    const double* a = chk + 3 * (size_t)(pairs ? i : n_pair + i);
-    const int axis = (!pairs && row_axis) ? row_axis[i - n_pair] : -1;
-    if (axis >= 0) {
-        solid_harmonics_grad(a[0], a[1], a[2], inv_R0, p, [&](int n, int m, D4 vc, D4 vs) {
-            const int cc = n * n + n + m - drop, cs = n * n + n - m - drop;
-            if (cc >= 0) Fm[(size_t)cc * rows + i] = axis == 0 ? vc.x : (axis == 1 ? vc.y : vc.z);
-            if (m > 0) Fm[(size_t)cs * rows + i] = axis == 0 ? vs.x : (axis == 1 ? vs.y : vs.z);
-        });
-        return;
-    }
-    solid_harmonics(a[0], a[1], a[2], inv_R0, p, [&](int n, int m, double vc, double vs) {
-        const int cc = n * n + n + m - drop, cs = n * n + n - m - drop;
-        if (cc >= 0) Fm[(size_t)cc * rows + i] = vc;
-        if (m > 0) Fm[(size_t)cs * rows + i] = vs;
-    });
-    if (pairs) {
-        const double* b = chk + 3 * (size_t)(n_pair + i);
-        solid_harmonics(b[0], b[1], b[2], inv_R0, p, [&](int n, int m, double vc, double vs) {
-            const int cc = n * n + n + m - drop, cs = n * n + n - m - drop;
-            if (cc >= 0) Fm[(size_t)cc * rows + i] -= vc;
-            if (m > 0) Fm[(size_t)cs * rows + i] -= vs;
-        });
+    const RowDesc d = desc[i];
+    for (int k = 0; k < 2; ++k) {
+        const int idx = k == 0 ? d.i1 : d.i2;
+        if (idx < 0) continue;
+        const double sgn = k == 0 ? 1.0 : -1.0;
+        const double* a = chk + 3 * (size_t)idx;
+        if (d.axis >= 0) {
+            solid_harmonics_grad(a[0], a[1], a[2], inv_R0, p, [&](int n, int m, D4 vc, D4 vs) {
+                const int cc = n * n + n + m - drop, cs = n * n + n - m - drop;
+                const double gc = d.axis == 0 ? vc.x : (d.axis == 1 ? vc.y : vc.z);
+                const double gs = d.axis == 0 ? vs.x : (d.axis == 1 ? vs.y : vs.z);
+                if (cc >= 0) Fm[(size_t)cc * rows + i] = (k == 0 ? 0.0 : Fm[(size_t)cc * rows + i]) + sgn * gc;
+                if (m > 0) Fm[(size_t)cs * rows + i] = (k == 0 ? 0.0 : Fm[(size_t)cs * rows + i]) + sgn * gs;
+            });
+        } else {
+            solid_harmonics(a[0], a[1], a[2], inv_R0, p, [&](int n, int m, double vc, double vs) {
+                const int cc = n * n + n + m - drop, cs = n * n + n - m - drop;
+                if (cc >= 0) Fm[(size_t)cc * rows + i] = (k == 0 ? 0.0 : Fm[(size_t)cc * rows + i]) + sgn * vc;
+                if (m > 0) Fm[(size_t)cs * rows + i] = (k == 0 ? 0.0 : Fm[(size_t)cs * rows + i]) + sgn * vs;
+            });
+        }
     }
 }
 
@@ -217,18 +217,17 @@ __global__ void pinv_kernel(const double* __restrict__ Qm, const double* __restr
 // H3 (update step): rhs from the check-point sums, A = Pinv rhs.  One warp per coefficient, 8 warps per block;
 // block 0 also stores rhs.  Fixed summation order (lane-strided partial sums, xor-shuffle tree).
 __global__ void __launch_bounds__(256) ls_apply_kernel(const double* __restrict__ pc, const double* __restrict__ pcg,
-                                                       const int* __restrict__ row_axis, int n_pair, int n_single,
-                                                       int ncol, int drop, double sgn, const double* __restrict__ Pinv,
+                                                       const RowDesc* __restrict__ desc, int rows, int ncol, int drop,
+                                                       double sgn, const double* __restrict__ Pinv,
                                                        double* __restrict__ rhs, double* __restrict__ A_full) {
     const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
     const int j = blockIdx.x * 8 + w;
-    const int rows = n_pair + n_single;
-    // residual of the boundary condition at row i: difference of the pair, the value at the single point, or
-    // (Neumann rows) the component row_axis of grad Phi_in there (pcg [K_t,3])
+    // residual of the boundary condition of row i from Phi_in (pc [K_t]) or a component of grad Phi_in (pcg [K_t,3])
     auto rhs_of = [&](int i) {
-        if (i < n_pair) return sgn * (pc[i] - pc[n_pair + i]);
-        if (row_axis && row_axis[i - n_pair] >= 0) return sgn * pcg[3 * (size_t)(n_pair + i) + row_axis[i - n_pair]];
-        return sgn * pc[n_pair + i];
+        const RowDesc d = desc[i];
+        const double a = d.axis < 0 ? pc[d.i1] : pcg[3 * (size_t)d.i1 + d.axis];
+        const double b = d.i2 < 0 ? 0.0 : (d.axis < 0 ? pc[d.i2] : pcg[3 * (size_t)d.i2 + d.axis]);
+        return sgn * (a - b);
     };
     if (blockIdx.x == 0)
         for (int i = threadIdx.x; i < rows; i += blockDim.x) rhs[i] = rhs_of(i);

@@ -64,7 +64,8 @@ inline std::vector<double> fibonacci_checkpoints(int K, double R0) {
 // (reading S5b): faces ordered (-x,+x,-y,+y,-z,+z); face f gets floor(K a_f/sum a)
 // points, leftovers one each to the first faces; global point n has in-face coordinates
 // (frac(1/2 + (n+1) g1) - 1/2) L_u, (frac(1/2 + (n+1) g2) - 1/2) L_v, g = 1/rho, 1/rho^2 (plastic number).
-inline std::vector<double> default_face_points(int K, const double L[3], const bool use_axis[3]) {
+// lower_only: only the faces x_a = -L_a/2 (the face-pair closure).
+inline std::vector<double> default_face_points(int K, const double L[3], const bool use_axis[3], bool lower_only = false) {
     const double rho = 1.32471795724474602596;
     const double g1 = 1.0 / rho, g2 = 1.0 / (rho * rho);
     std::vector<int> fa, fs;
@@ -72,7 +73,7 @@ inline std::vector<double> default_face_points(int K, const double L[3], const b
     double asum = 0.0;
     for (int a = 0; a < 3; ++a)
         if (use_axis[a])
-            for (int s = -1; s <= 1; s += 2) {
+            for (int s = -1; s <= (lower_only ? -1 : 1); s += 2) {
                 fa.push_back(a); fs.push_back(s);
                 const double ar = L[(a + 1) % 3] * L[(a + 2) % 3];
                 area.push_back(ar); asum += ar;

@@ -198,10 +198,12 @@ struct hsma_plan {
     double R0 = 0.0, half[3] = {0, 0, 0};
     bool pairs = false;       // fully periodic: all rows are differences x_i / x~_i, constant column dropped
     bool slab_bc = false;     // grounded slab: pair rows wrapped in x,y + Dirichlet rows on the plates
-    int n_pair = 0, n_single = 0, drop = 0;
-    bool neumann = false;     // gamma = +1 walls: derivative rows, step (a) also needs grad Phi_in
-    int* row_axis = nullptr;  // [n_single] axis of the wall of each single row (Neumann), else null
-    double* pcg = nullptr;    // [Kt,3] grad Phi_in at the check targets (Neumann)
+    int drop = 0;             // 1: the constant column is dropped, A_00 = 0
+    bool neumann = false;     // gamma = +1 walls: derivative rows
+    bool face_pairs = false;  // periodic kind closed by value + normal-derivative pairs on opposite faces
+    bool need_grad = false;   // some row is a derivative row: step (a) runs its FIELD form
+    RowDesc* row_desc = nullptr;  // [rows]
+    double* pcg = nullptr;    // [Kt,3] grad Phi_in at the check targets (need_grad)
     bool need_neutral = false;
     int rows = 0, ncol = 0, Kt = 0, C_near = 0, C_rhs = 0, refine = 1;
     long long node_tiles = 0;
@@ -251,7 +253,7 @@ static void plan_free(hsma_plan* p) {
     for (void* q : ptrs) if (q) cudaFree(q);
     p->src.release(); p->slot_of.release(); p->tile_np.release(); if (p->qinfo) cudaFree(p->qinfo);
     if (p->cell_identity) cudaFree(p->cell_identity);
-    if (p->row_axis) cudaFree(p->row_axis);
+    if (p->row_desc) cudaFree(p->row_desc);
     if (p->pcg) cudaFree(p->pcg);
     if (p->cell_order) cudaFree(p->cell_order);
     if (p->img_qinfo) cudaFree(p->img_qinfo);
@@ -274,15 +276,17 @@ extern "C" hsma_status hsma_plan_create_ex(const hsma_plan_desc* desc, void* cud
     if (!desc || !plan_out || desc->struct_size != sizeof(hsma_plan_desc)) return HSMA_ERR_INVALID_ARG;
     const hsma_plan_desc& d = *desc;
     if (d.kind < 0 || d.kind > 2 || d.p < 1 || d.p > kMaxP || d.M < 8 || d.K < 1) return HSMA_ERR_INVALID_ARG;
-    if (d.closure != HSMA_CLOSURE_BOUNDARY && d.closure != HSMA_CLOSURE_FAR_DATA) return HSMA_ERR_INVALID_ARG;
+    if (d.closure != HSMA_CLOSURE_BOUNDARY && d.closure != HSMA_CLOSURE_FAR_DATA && d.closure != HSMA_CLOSURE_FACE_PAIRS)
+        return HSMA_ERR_INVALID_ARG;
+    if (d.closure == HSMA_CLOSURE_FACE_PAIRS && d.kind != HSMA_BC_PERIODIC) return HSMA_ERR_INVALID_ARG;
     if (d.rsqrt_refine < 0 || d.rsqrt_refine > 2) return HSMA_ERR_INVALID_ARG;
     if (d.near_mode != HSMA_NEAR_WHOLE_CELLS && d.near_mode != HSMA_NEAR_SPHERE) return HSMA_ERR_INVALID_ARG;
     if (d.dipole_mode != HSMA_DIPOLE_EXACT && d.dipole_mode != HSMA_DIPOLE_FD3) return HSMA_ERR_INVALID_ARG;
-    if (d.near_mode == HSMA_NEAR_SPHERE && d.closure != HSMA_CLOSURE_BOUNDARY) return HSMA_ERR_INVALID_ARG;
+    if (d.near_mode == HSMA_NEAR_SPHERE && d.closure == HSMA_CLOSURE_FAR_DATA) return HSMA_ERR_INVALID_ARG;
     if (d.fd_dr_rel < 0.0 || d.fd_dr_rel > 0.1) return HSMA_ERR_INVALID_ARG;
     for (int a = 0; a < 3; ++a)
         if (!(d.L[a] > 0.0) || d.near_shell[a] < 0 || d.near_shell[a] > 8) return HSMA_ERR_INVALID_ARG;
-    if (d.kind == HSMA_BC_PERIODIC && d.closure != HSMA_CLOSURE_BOUNDARY) return HSMA_ERR_INVALID_ARG;
+    if (d.kind == HSMA_BC_PERIODIC && d.closure == HSMA_CLOSURE_FAR_DATA) return HSMA_ERR_INVALID_ARG;
     if (d.kind != HSMA_BC_PERIODIC && d.closure == HSMA_CLOSURE_BOUNDARY && d.gamma != -1.0 && d.gamma != 1.0)
         return HSMA_ERR_INVALID_ARG;  // reading S16: a dielectric wall has no boundary closure (far-data closure only);
                                       // gamma = -1 closes by Dirichlet rows, gamma = +1 by Neumann rows
@@ -298,7 +302,8 @@ extern "C" hsma_status hsma_plan_create_ex(const hsma_plan_desc* desc, void* cud
     p->stream = (cudaStream_t)cuda_stream;
     p->R0 = R0;
     for (int a = 0; a < 3; ++a) p->half[a] = 0.5 * d.L[a];
-    p->pairs = d.kind == HSMA_BC_PERIODIC;
+    p->pairs = d.kind == HSMA_BC_PERIODIC && d.closure == HSMA_CLOSURE_BOUNDARY;
+    p->face_pairs = d.kind == HSMA_BC_PERIODIC && d.closure == HSMA_CLOSURE_FACE_PAIRS;
     p->slab_bc = d.kind == HSMA_BC_SLAB_XY_PERIODIC_Z_MIRROR && d.closure == HSMA_CLOSURE_BOUNDARY;
     p->neumann = d.kind != HSMA_BC_PERIODIC && d.closure == HSMA_CLOSURE_BOUNDARY && d.gamma == 1.0;
     p->need_neutral = (d.kind != HSMA_BC_MIRROR_CAVITY && !p->slab_bc) || p->neumann;   // grounded walls screen a net charge
@@ -333,58 +338,79 @@ extern "C" hsma_status hsma_plan_create_ex(const hsma_plan_desc* desc, void* cud
     if (rhsc.empty()) { p->cells_rhs = p->cells_near; p->C_rhs = p->C_near; }
     else { p->C_rhs = (int)rhsc.size(); PCU(upload(&p->cells_rhs, rhsc, st)); }
 
-    // monitoring points
-    std::vector<double> x;
-    if (d.check_xyz) x.assign(d.check_xyz, d.check_xyz + 3 * (size_t)d.K);
-    else if (p->pairs) x = fibonacci_checkpoints(d.K, R0);
-    else {
-        bool use[3] = {!p->slab_bc, !p->slab_bc, true};   // grounded slab: points on the two plates only
-        x = default_face_points(d.K, d.L, use);
-    }
+    // monitoring points and the rows of the least-squares problem, PAPER.md:74-82 (RowDesc in fit_kernels.cuh)
+    const double tol_wall = 1e-12 * std::max({d.L[0], d.L[1], d.L[2]});
     std::vector<double> chk;
-    if (p->pairs || p->slab_bc) {
-        // x~ = x - L round(x/L) on the periodic axes; rows with x~ = x carry no information
-        const std::vector<double> sph = p->pairs ? x : fibonacci_checkpoints(d.K, R0);
-        const int wrap_axes = p->pairs ? 3 : 2;
-        std::vector<double> a, b;
+    std::vector<RowDesc> rowd;
+    if (p->face_pairs) {
+        // K points on the lower faces x_a = -L_a/2 and their partners x + L_a e_a on the opposite
+        // faces; one value row and one normal-derivative row per pair (value rows alone are rank deficient, S15)
+        std::vector<double> x;
+        if (d.check_xyz) x.assign(d.check_xyz, d.check_xyz + 3 * (size_t)d.K);
+        else { bool use[3] = {true, true, true}; x = default_face_points(d.K, d.L, use, /*lower_only=*/true); }
+        std::vector<double> xp = x;
+        std::vector<int> axis(d.K, -1);
         for (int i = 0; i < d.K; ++i) {
-            double w[3]; bool moved = false;
-            for (int c = 0; c < 3; ++c) {
-                const double v = sph[3 * (size_t)i + c];
-                w[c] = c < wrap_axes ? v - d.L[c] * std::nearbyint(v / d.L[c]) : v;
-                moved = moved || std::fabs(v - w[c]) > 0.0;
-            }
-            if (!moved) continue;
-            for (int c = 0; c < 3; ++c) { a.push_back(sph[3 * (size_t)i + c]); b.push_back(w[c]); }
+            for (int a = 0; a < 3 && axis[i] < 0; ++a)
+                if (std::fabs(x[3 * (size_t)i + a] + 0.5 * d.L[a]) <= tol_wall) axis[i] = a;
+            if (axis[i] < 0) { plan_free(p); return HSMA_ERR_INVALID_ARG; }   // not on a lower face
+            xp[3 * (size_t)i + axis[i]] += d.L[axis[i]];
         }
-        p->n_pair = (int)(a.size() / 3);
-        chk = a; chk.insert(chk.end(), b.begin(), b.end());
-        if (p->slab_bc) {   // + Dirichlet rows on the plates; the constant column stays
-            chk.insert(chk.end(), x.begin(), x.end());
-            p->n_single = d.K; p->drop = p->neumann ? 1 : 0;
-        } else {
-            p->n_single = 0; p->drop = 1;
-        }
+        chk = x; chk.insert(chk.end(), xp.begin(), xp.end());
+        for (int i = 0; i < d.K; ++i) rowd.push_back(RowDesc{i, d.K + i, -1, 0});
+        for (int i = 0; i < d.K; ++i) rowd.push_back(RowDesc{i, d.K + i, axis[i], 0});
+        p->drop = 1;
+        p->need_grad = true;
     } else {
-        chk = x; p->n_pair = 0; p->n_single = d.K; p->drop = p->neumann ? 1 : 0;
-    }
-    if (p->neumann) {   // the wall each single point lies on: the reflecting axis with |x_a| = L_a/2
-        std::vector<int> axis(p->n_single, 2);
-        const int first_axis = d.kind == HSMA_BC_MIRROR_CAVITY ? 0 : 2;
-        for (int i = 0; i < p->n_single; ++i) {
-            int found = -1;
-            for (int a = first_axis; a < 3 && found < 0; ++a)
-                if (std::fabs(std::fabs(x[3 * (size_t)i + a]) - 0.5 * d.L[a]) <= 1e-12 * std::max({d.L[0], d.L[1], d.L[2]})) found = a;
-            if (found < 0) { plan_free(p); return HSMA_ERR_INVALID_ARG; }   // a wall point that is on no wall
-            axis[i] = found;
+        std::vector<double> x;   // the user's / default points: circumsphere points (periodic) or wall points
+        if (d.check_xyz) x.assign(d.check_xyz, d.check_xyz + 3 * (size_t)d.K);
+        else if (p->pairs) x = fibonacci_checkpoints(d.K, R0);
+        else {
+            bool use[3] = {!p->slab_bc, !p->slab_bc, true};   // slab: points on the two plates only
+            x = default_face_points(d.K, d.L, use);
         }
-        PCU(upload(&p->row_axis, axis, st));
+        int n_pair = 0;
+        if (p->pairs || p->slab_bc) {
+            // x~ = x - L round(x/L) on the periodic axes; rows with x~ = x carry no information
+            const std::vector<double> sph = p->pairs ? x : fibonacci_checkpoints(d.K, R0);
+            const int wrap_axes = p->pairs ? 3 : 2;
+            std::vector<double> a, b;
+            for (int i = 0; i < d.K; ++i) {
+                double w[3]; bool moved = false;
+                for (int c = 0; c < 3; ++c) {
+                    const double v = sph[3 * (size_t)i + c];
+                    w[c] = c < wrap_axes ? v - d.L[c] * std::nearbyint(v / d.L[c]) : v;
+                    moved = moved || std::fabs(v - w[c]) > 0.0;
+                }
+                if (!moved) continue;
+                for (int c = 0; c < 3; ++c) { a.push_back(sph[3 * (size_t)i + c]); b.push_back(w[c]); }
+            }
+            n_pair = (int)(a.size() / 3);
+            chk = a; chk.insert(chk.end(), b.begin(), b.end());
+            for (int i = 0; i < n_pair; ++i) rowd.push_back(RowDesc{i, n_pair + i, -1, 0});
+        }
+        if (!p->pairs) {   // wall rows (cavity, slab) or data rows (far-data closure)
+            const int first_axis = d.kind == HSMA_BC_MIRROR_CAVITY ? 0 : 2;
+            for (int i = 0; i < d.K; ++i) {
+                int axis = -1;
+                if (p->neumann) {   // the wall the point lies on: the reflecting axis with |x_a| = L_a/2
+                    for (int a = first_axis; a < 3 && axis < 0; ++a)
+                        if (std::fabs(std::fabs(x[3 * (size_t)i + a]) - 0.5 * d.L[a]) <= tol_wall) axis = a;
+                    if (axis < 0) { plan_free(p); return HSMA_ERR_INVALID_ARG; }   // a wall point that is on no wall
+                }
+                rowd.push_back(RowDesc{2 * n_pair + i, -1, axis, 0});
+            }
+            chk.insert(chk.end(), x.begin(), x.end());
+        }
+        p->drop = (p->pairs || p->neumann) ? 1 : 0;   // no row sees the constant harmonic
+        p->need_grad = p->neumann;
     }
-    p->rows = p->n_pair + p->n_single;
-    p->Kt = 2 * p->n_pair + p->n_single;
+    p->rows = (int)rowd.size();
+    p->Kt = (int)(chk.size() / 3);
     p->ncol = d.p * d.p - p->drop;
     if (p->rows < p->ncol || p->ncol < 1) { plan_free(p); return HSMA_ERR_RANK_DEFICIENT; }
     PCU(upload(&p->chk, chk, st));
+    PCU(upload(&p->row_desc, rowd, st));
 
     // integration nodes
     std::vector<double> nrm, wq;
@@ -408,7 +434,7 @@ extern "C" hsma_status hsma_plan_create_ex(const hsma_plan_desc* desc, void* cud
     PCU(cudaMalloc(&p->Pinv, mn * sizeof(double)));
     PCU(cudaMalloc(&p->tau, p->ncol * sizeof(double)));
     PCU(cudaMalloc(&p->pc, p->Kt * sizeof(double)));
-    if (p->neumann) PCU(cudaMalloc(&p->pcg, 3 * (size_t)p->Kt * sizeof(double)));
+    if (p->need_grad) PCU(cudaMalloc(&p->pcg, 3 * (size_t)p->Kt * sizeof(double)));
     PCU(cudaMalloc(&p->rhs, p->rows * sizeof(double)));
     PCU(cudaMalloc(&p->cvec, p->ncol * sizeof(double)));
     PCU(cudaMalloc(&p->A_full, d.p * d.p * sizeof(double)));
@@ -417,7 +443,7 @@ extern "C" hsma_status hsma_plan_create_ex(const hsma_plan_desc* desc, void* cud
     PCU(cudaMalloc(&p->qinfo, sizeof(QInfo)));
     PCU(cudaMemsetAsync(p->flags, 0, 4 * sizeof(int), st));
     PCU(cudaMemsetAsync(p->A_full, 0, d.p * d.p * sizeof(double), st));
-    build_fit_matrix_kernel<<<(p->rows + 127) / 128, 128, 0, st>>>(p->chk, p->n_pair, p->n_single, p->drop, d.p, 1.0 / R0, p->row_axis, p->Fm);
+    build_fit_matrix_kernel<<<(p->rows + 127) / 128, 128, 0, st>>>(p->chk, p->row_desc, p->rows, p->drop, d.p, 1.0 / R0, p->Fm);
     HSMA_COUNT_LAUNCH();
     householder_qr_kernel<<<1, 1024, 0, st>>>(p->Fm, p->rows, p->ncol, p->tau, p->Qm, p->Rm, p->flags);
     HSMA_COUNT_LAUNCH();
@@ -536,7 +562,7 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
 
     // H2 (a): Phi_in (or the far-cell data) at the monitoring points -> pc [Kt]
     {
-        const bool fa = p->neumann;   // Neumann rows need grad Phi_in at the wall points: the FIELD form of (a)
+        const bool fa = p->need_grad;   // derivative rows need grad Phi_in at the check targets: the FIELD form of (a)
         const Launch s = choose_near(p->Kt, n_tiles_near, C_a, 2, fa);
         if (p->part_a.reserve((size_t)s.rows * p->Kt * (fa ? 4 : 1)) != cudaSuccess) return HSMA_ERR_ALLOC;
         MARK(1);
@@ -549,8 +575,8 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
         HSMA_COUNT_LAUNCH();
     }
     // H3: least squares, Eq.(7)
-    ls_apply_kernel<<<(p->ncol + 7) / 8, 256, 0, st>>>(p->pc, p->pcg, p->row_axis, p->n_pair, p->n_single, p->ncol, p->drop,
-                                                       p->rhs_sign, p->Pinv, p->rhs, p->A_full);
+    ls_apply_kernel<<<(p->ncol + 7) / 8, 256, 0, st>>>(p->pc, p->pcg, p->row_desc, p->rows, p->ncol, p->drop, p->rhs_sign,
+                                                       p->Pinv, p->rhs, p->A_full);
     HSMA_COUNT_LAUNCH();
     // H4: harmonic surface mapping, Eq.(10),(11) PAPER.md:99-105
     surface_mapping_kernel<<<(d.M + 127) / 128, 128, 0, st>>>(p->A_full, d.p, d.R_aux / p->R0, d.R_aux, p->nrm, p->wq,
