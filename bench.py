@@ -380,6 +380,9 @@ def main():
     ap.add_argument("--paper-timing", type=int, default=0, metavar="N",
                     help="the paper's own timing workload instead of a BASELINE.json config (PAPER.md:171,183: lattice "
                          "sites, random signs, alpha=1.3, P=25, N_o=5928, images inside the sphere); N an even cube")
+    ap.add_argument("--face-pairs", action="store_true",
+                    help="periodic configs: close by seeded value+derivative pairs on opposite faces instead of the "
+                         "paper's circumsphere rule (DESIGN.md 6.10)")
     ap.add_argument("--forces", action="store_true", help="time hsma_evaluate_forces (potential + forces) instead")
     ap.add_argument("--refine", type=int, default=0, choices=[0, 1, 2], help="hsma_plan_desc.rsqrt_refine")
     ap.add_argument("--e2e-steps", type=int, default=3)
@@ -391,6 +394,8 @@ def main():
     if args.warmup < 3 and args.impl == "b200":
         print(f"note: --warmup {args.warmup} < 3 (timing rules ask for >= 3)", file=sys.stderr)
     w = W.paper_timing(args.paper_timing) if args.paper_timing else W.config(args.config, N=args.size)
+    if args.face_pairs:   # BASELINE.json's "check-point pairs on opposite faces", seeded
+        w = w.with_(closure=W.CLOSURE_FACE_PAIRS, check_xyz=W.seeded_face_points(w.K, w.L, W.LOWER_FACES, seed=args.config))
     rank = int(os.environ.get("RANK", "0"))
     if args.impl == "reference":
         if rank == 0:

@@ -276,6 +276,38 @@ def test_grounded_slab_boundary_closure(H, refine, neutral):
     assert e.value.status == H.HSMA_ERR_INVALID_ARG
 
 
+# ------------------------------------------------------------------ face-pair closure
+@pytest.mark.parametrize("idx,seed", [(1, 0), (2, 1)])
+@pytest.mark.parametrize("refine", [0, 1, 2])
+def test_face_pair_closure_configs_as_literally_written(H, idx, seed, refine):
+    """BASELINE.json configs 1 and 2 with their "random check-point pairs on opposite faces": seeded points on the
+    lower faces, partners on the opposite faces, value + normal-derivative rows (2K rows)."""
+    w = W.config(idx)
+    chk = W.seeded_face_points(w.K, w.L, W.LOWER_FACES, seed=seed)
+    w = w.with_(closure=W.CLOSURE_FACE_PAIRS, check_xyz=chk)
+    r, phi, U, extra = run_both(H, w, rsqrt_refine=refine)
+    check_parity(r, phi, U, extra, f"face pairs cfg{idx} refine={refine}")
+    assert extra["info"]["rows"] == 2 * w.K and extra["A"][0] == 0.0
+    if idx == 1:
+        assert abs(O.madelung_constant(U, w.N, 1.0) - 1.7475645946) < 5e-7
+
+
+def test_face_pair_closure_default_points_forces_and_sphere_mode(H):
+    """The library's own lattice on the lower faces (both sides build the same points), forces, and the
+    sphere-culled near set under this closure."""
+    w = W.config(5, N=6000).with_(closure=W.CLOSURE_FACE_PAIRS, K=900, p=12, M=6000)
+    r, phi, U, extra = run_both(H, w)
+    check_parity(r, phi, U, extra, "face pairs default points")
+    rf = O.hsma(w.with_(near_mode=W.NEAR_SPHERE), forces=True)
+    with H.Plan.from_workload(w.with_(near_mode=W.NEAR_SPHERE)) as plan:
+        ph, F, Uf = plan.evaluate_forces(dev(w.xyz), dev(w.q), sync=True)
+    assert rel_inf(ph.cpu().numpy(), rf.phi) <= PHI_TOL and abs(float(Uf) - rf.U) <= U_TOL * abs(rf.U)
+    assert rel_inf(F.cpu().numpy(), rf.F) <= 1e-10
+    with pytest.raises(H.HsmaError) as e:       # the closure belongs to the periodic kind
+        H.Plan(kind=1, L=(1, 1, 1), near_shell=(1, 1, 1), R_aux=1.2, p=6, M=500, K=300, gamma=-1.0, closure=2)
+    assert e.value.status == H.HSMA_ERR_INVALID_ARG
+
+
 # ------------------------------------------------------------------ Neumann walls (SURVEY.md 8(f) NEXT 3)
 @pytest.mark.parametrize("which", ["cavity", "slab"])
 @pytest.mark.parametrize("refine", [1, 2])
