@@ -240,14 +240,16 @@ def run_b200(args, w) -> dict:
 
     def step():
         flush.zero_()                                     # L2 flush between iterations (torch memset, not counted)
+        if world > 1:
+            # targets AND check-point sums sharded; exchanges: all-gather of the K_t check sums before the fit,
+            # all-gather of phi (F) and all-reduce of U at the end
+            full, _, Uall = shard.evaluate_distributed(plan, xyz, q, forces=args.forces)
+            U.copy_(Uall)
+            return full
         if args.forces:
             H.hsma_evaluate_forces_shard(plan.handle, xyz, q, t0, t1, phi, force, U)
         else:
             H.hsma_evaluate_shard(plan.handle, xyz, q, t0, t1, phi, U)
-        if world > 1:                                     # the exchange step: assemble phi and U on every rank
-            full = shard.all_gather_phi(phi, N)
-            shard.all_reduce_energy(U)
-            return full
         return phi
 
     # peak FP64 (DFMA microbenchmark) before the run: the measured roofline denominator
@@ -359,7 +361,8 @@ def run_b200(args, w) -> dict:
            "data": "synthetic",
            "config": {"workload": w.name, "N": N, "near_cells": info["near_cells"], "p": info["p"], "M": info["M"],
                       "check_targets": info["check_targets"], "pairs_per_step": pc_all, "rsqrt_refine": refine, "forces": bool(args.forces),
-                      "parallelism": f"targets sharded over {world} rank(s), sources replicated",
+                      "parallelism": f"targets and check-point sums sharded over {world} rank(s), sources replicated"
+                                     + ("" if world == 1 else "; stage_ms covers the second phase only (step (a) runs in its own call)"),
                       "l2": "256 MiB flush written between iterations"},
            "energy": U_val, "stage_ms": stage_ms, "e2e": e2e, "gpu_launches": int(launches),
            "launches_per_step": plan.launches_last_evaluate(), "clocks": clocks, "roofline": roofline}

@@ -166,6 +166,25 @@ hsma_status hsma_evaluate_forces_shard(hsma_plan* plan, const double* xyz, const
 hsma_status hsma_evaluate_forces_host(hsma_plan* plan, const double* xyz_host, const double* q_host,
                                       long long N, double* phi_host, double* force_host, double* energy_host);
 
+/*
+ * Multi-GPU with step (a) sharded as well.  Every rank holds all N sources and the same plan.
+ *   1. hsma_check_sums_shard      H1 + step (a) for the check targets c0 <= i < c1 (of K_t = plan_info[2]) only
+ *   2. hsma_get_check_sums        copy that slice out: pc_out dev [c1-c0] (and pcg_out dev [c1-c0,3] when the fit has
+ *                                 derivative rows -- Neumann walls, face-pair closure; else pcg_out may be NULL)
+ *      ... the caller all-gathers the slices (K_t doubles: one latency-bound message) ...
+ *   3. hsma_set_check_sums        copy the other ranks' slices in
+ *   4. hsma_evaluate_rest_shard   H1 + fit + mapping + (b) + (c) + finish for the targets t0 <= i < t1 with the check
+ *                                 sums as they now are; force_out may be NULL (potentials only)
+ * All asynchronous on the plan's stream.  Steps 1 and 4 together equal hsma_evaluate(_forces)_shard.
+ */
+hsma_status hsma_check_sums_shard(hsma_plan* plan, const double* xyz, const double* q, long long N,
+                                  long long c0, long long c1);
+hsma_status hsma_get_check_sums(hsma_plan* plan, long long c0, long long c1, double* pc_out, double* pcg_out);
+hsma_status hsma_set_check_sums(hsma_plan* plan, long long c0, long long c1, const double* pc_in, const double* pcg_in);
+hsma_status hsma_evaluate_rest_shard(hsma_plan* plan, const double* xyz, const double* q, long long N,
+                                     long long t0, long long t1, double* phi_out, double* force_out,
+                                     double* energy_out);
+
 /* Synchronise the plan's stream and return the sticky status of the evaluations since the last
  * call (HSMA_ERR_NOT_NEUTRAL, HSMA_ERR_CUDA, ...), then clear it. */
 hsma_status hsma_plan_sync(hsma_plan* plan);
@@ -175,7 +194,8 @@ const char* hsma_status_string(int status);
 /* ---- introspection / test and bench hooks ------------------------------------------------------- */
 /* sizes: what[0]=rows of the fit, [1]=columns, [2]=check targets K_t, [3]=near cells, [4]=rhs cells,
  * [5]=M nodes, [6]=p, [7]=kernels launched by the last evaluate, [8]=near images summed per target by the last
- * evaluate (N * cells, or the image count inside the sphere), [9]=node records (M or 3M).  host out [10]. */
+ * evaluate (N * cells, or the image count inside the sphere), [9]=node records (M or 3M), [10]=1 if the fit has derivative rows (step (a) then also
+ * produces grad Phi_in at the check targets).  host out [11]. */
 hsma_status hsma_plan_info(hsma_plan* plan, long long* what_out);
 /* copies of plan/evaluate state into caller DEVICE buffers (valid after an evaluate on the stream) */
 hsma_status hsma_get_coeffs(hsma_plan* plan, double* A_out /* dev [p*p], R0-scaled basis */);

@@ -66,6 +66,15 @@ _SIGNATURES = {
                                                   ctypes.c_void_p, ctypes.c_void_p]),
     "hsma_evaluate_forces_host": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_longlong,
                                                  ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]),
+    "hsma_check_sums_shard": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_longlong,
+                                             ctypes.c_longlong, ctypes.c_longlong]),
+    "hsma_get_check_sums": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_longlong, ctypes.c_longlong, ctypes.c_void_p,
+                                           ctypes.c_void_p]),
+    "hsma_set_check_sums": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_longlong, ctypes.c_longlong, ctypes.c_void_p,
+                                           ctypes.c_void_p]),
+    "hsma_evaluate_rest_shard": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_longlong,
+                                                ctypes.c_longlong, ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p,
+                                                ctypes.c_void_p]),
     "hsma_plan_sync": (ctypes.c_int, [ctypes.c_void_p]),
     "hsma_status_string": (ctypes.c_char_p, [ctypes.c_int]),
     "hsma_plan_info": (ctypes.c_int, [ctypes.c_void_p, ctypes.POINTER(ctypes.c_longlong)]),
@@ -263,16 +272,46 @@ def hsma_evaluate_forces_host(plan: int, xyz: np.ndarray, q: np.ndarray, phi_out
            "hsma_evaluate_forces_host")
 
 
+def hsma_check_sums_shard(plan: int, xyz: torch.Tensor, q: torch.Tensor, c0: int, c1: int):
+    N = q.numel()
+    _check(load_library().hsma_check_sums_shard(plan, _dev(xyz, 3 * N, "xyz"), _dev(q, N, "q"), N, c0, c1),
+           "hsma_check_sums_shard")
+
+
+def hsma_get_check_sums(plan: int, c0: int, c1: int, pc_out: torch.Tensor, pcg_out: Optional[torch.Tensor] = None):
+    _check(load_library().hsma_get_check_sums(plan, c0, c1, _dev(pc_out, c1 - c0, "pc_out"),
+                                              _dev(pcg_out, 3 * (c1 - c0), "pcg_out")), "hsma_get_check_sums")
+
+
+def hsma_set_check_sums(plan: int, c0: int, c1: int, pc_in: torch.Tensor, pcg_in: Optional[torch.Tensor] = None):
+    _check(load_library().hsma_set_check_sums(plan, c0, c1, _dev(pc_in, c1 - c0, "pc_in"),
+                                              _dev(pcg_in, 3 * (c1 - c0), "pcg_in")), "hsma_set_check_sums")
+
+
+def hsma_evaluate_rest_shard(plan: int, xyz: torch.Tensor, q: torch.Tensor, t0: int, t1: int,
+                             phi_out: Optional[torch.Tensor], force_out: Optional[torch.Tensor],
+                             energy_out: Optional[torch.Tensor] = None):
+    N, T = q.numel(), max(t1 - t0, 0)
+    _check(load_library().hsma_evaluate_rest_shard(plan, _dev(xyz, 3 * N, "xyz"), _dev(q, N, "q"), N, t0, t1,
+                                                   _dev(phi_out, T, "phi_out"), _dev(force_out, 3 * T, "force_out"),
+                                                   _dev(energy_out, 1, "energy_out")), "hsma_evaluate_rest_shard")
+
+
 def hsma_plan_sync(plan: int):
     _check(load_library().hsma_plan_sync(plan), "hsma_plan_sync")
 
 
 def hsma_plan_info(plan: int) -> dict:
-    w = (ctypes.c_longlong * 10)()
+    w = (ctypes.c_longlong * 11)()
     _check(load_library().hsma_plan_info(plan, w), "hsma_plan_info")
     keys = ("rows", "cols", "check_targets", "near_cells", "rhs_cells", "M", "p", "launches_last_evaluate",
-            "near_images_last_evaluate", "node_records")
+            "near_images_last_evaluate", "node_records", "check_gradient")
     return dict(zip(keys, [int(v) for v in w]))
+
+
+def hsma_plan_needs_check_gradient(plan: int) -> bool:
+    """True if the fit has derivative rows (Neumann walls, face-pair closure): hsma_get/set_check_sums then also move pcg."""
+    return bool(hsma_plan_info(plan)["check_gradient"])
 
 
 def hsma_get_coeffs(plan: int, A_out: torch.Tensor):

@@ -499,9 +499,19 @@ __global__ void node_positions_kernel(const double* __restrict__ nrm, double R, 
 }  // namespace hsma
 
 // force_out non-null: the FIELD kernels also produce F_i = -q_i grad Phi(r_i)
+// Phases of the update step (multi-GPU): the check-point sums of step (a) can be sharded over ranks too.
+//   kPhaseAll     the whole evaluate
+//   kPhaseCheck   H1 + step (a) for the check targets c0 <= i < c1 only, into the plan's pc (pcg); nothing else
+//   kPhaseRest    H1 + fit + mapping + (b) + (c) + finish with the plan's pc (pcg) AS THEY ARE (hsma_set_check_sums)
+enum { kPhaseAll = 0, kPhaseCheck = 1, kPhaseRest = 2 };
 static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* q, long long N, long long t0,
-                                 long long t1, double* phi_out, double* energy_out, double* force_out = nullptr) {
-    if (!p || !xyz || !q || N < 1 || t0 < 0 || t1 > N || t0 > t1 || (!phi_out && !force_out && t1 > t0)) return HSMA_ERR_INVALID_ARG;
+                                 long long t1, double* phi_out, double* energy_out, double* force_out = nullptr,
+                                 int phase = kPhaseAll, long long c0 = 0, long long c1 = -1) {
+    if (!p || !xyz || !q || N < 1 || t0 < 0 || t1 > N || t0 > t1 ||
+        (phase != kPhaseCheck && !phi_out && !force_out && t1 > t0))
+        return HSMA_ERR_INVALID_ARG;
+    if (phase == kPhaseAll) { c0 = 0; c1 = p->Kt; }
+    if (phase == kPhaseCheck && (c0 < 0 || c1 > p->Kt || c0 > c1)) return HSMA_ERR_INVALID_ARG;
     const bool field = force_out != nullptr;
     cudaStream_t st = p->stream;
     const long long before = g_launches;
@@ -560,19 +570,29 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
         p->last_images = Ns;
     }
 
-    // H2 (a): Phi_in (or the far-cell data) at the monitoring points -> pc [Kt]
-    {
+    // H2 (a): Phi_in (or the far-cell data) at the monitoring points c0..c1-1 -> pc [Kt]
+    if (phase != kPhaseRest && c1 > c0) {
+        const long long Tc = c1 - c0;
         const bool fa = p->need_grad;   // derivative rows need grad Phi_in at the check targets: the FIELD form of (a)
-        const Launch s = choose_near(p->Kt, n_tiles_near, C_a, 2, fa);
-        if (p->part_a.reserve((size_t)s.rows * p->Kt * (fa ? 4 : 1)) != cudaSuccess) return HSMA_ERR_ALLOC;
+        const Launch s = choose_near(Tc, n_tiles_near, C_a, 2, fa);
+        if (p->part_a.reserve((size_t)s.rows * Tc * (fa ? 4 : 1)) != cudaSuccess) return HSMA_ERR_ALLOC;
         MARK(1);
-        launch_near(s, fa, p->chk, 3, nullptr, p->Kt, 0, P, cells_a, C_a, -1, 2, p->part_a.p, st);  // (a) always cubic: it feeds the fit
+        launch_near(s, fa, p->chk, 3, nullptr, Tc, c0, P, cells_a, C_a, -1, 2, p->part_a.p, st);  // (a) always cubic: it feeds the fit
         MARK(2);
         if (fa)
-            finish_field_kernel<<<(p->Kt + 255) / 256, 256, 0, st>>>(s.layout(p->part_a.p), PartLayout{nullptr, 1, 1, 1, 1}, p->Kt, nullptr, nullptr, 0, p->pc, p->pcg, nullptr);
+            finish_field_kernel<<<(unsigned)((Tc + 255) / 256), 256, 0, st>>>(s.layout(p->part_a.p), PartLayout{nullptr, 1, 1, 1, 1}, Tc, nullptr, nullptr, 0, p->pc + c0, p->pcg + 3 * c0, nullptr);
         else
-            finish_phi_kernel<<<(p->Kt + 255) / 256, 256, 0, st>>>(s.layout(p->part_a.p), PartLayout{nullptr, 1, 1, 1, 1}, p->Kt, nullptr, nullptr, 0, p->pc, nullptr);
+            finish_phi_kernel<<<(unsigned)((Tc + 255) / 256), 256, 0, st>>>(s.layout(p->part_a.p), PartLayout{nullptr, 1, 1, 1, 1}, Tc, nullptr, nullptr, 0, p->pc + c0, nullptr);
         HSMA_COUNT_LAUNCH();
+    } else {
+        MARK(1); MARK(2);
+    }
+    if (phase == kPhaseCheck) {
+        MARK(3); MARK(4); MARK(5); MARK(6);
+        p->ev_valid = p->timing;
+        p->last_launches = g_launches - before;
+        if (cudaPeekAtLastError() != cudaSuccess) { cudaGetLastError(); p->sticky = HSMA_ERR_CUDA; return HSMA_ERR_CUDA; }
+        return HSMA_OK;
     }
     // H3: least squares, Eq.(7)
     ls_apply_kernel<<<(p->ncol + 7) / 8, 256, 0, st>>>(p->pc, p->pcg, p->row_desc, p->rows, p->ncol, p->drop, p->rhs_sign,
@@ -649,6 +669,31 @@ extern "C" hsma_status hsma_evaluate_forces_shard(hsma_plan* plan, const double*
     return evaluate_impl(plan, xyz, q, N, t0, t1, phi_out, energy_out, force_out);
 }
 
+// ---- multi-GPU: step (a) sharded over the check targets --------------------------------------------
+extern "C" hsma_status hsma_check_sums_shard(hsma_plan* plan, const double* xyz, const double* q, long long N,
+                                             long long c0, long long c1) {
+    return evaluate_impl(plan, xyz, q, N, 0, 0, nullptr, nullptr, nullptr, kPhaseCheck, c0, c1);
+}
+extern "C" hsma_status hsma_get_check_sums(hsma_plan* p, long long c0, long long c1, double* pc_out, double* pcg_out) {
+    if (!p || c0 < 0 || c1 > p->Kt || c0 > c1 || !pc_out || (p->need_grad && !pcg_out)) return HSMA_ERR_INVALID_ARG;
+    if (c1 == c0) return HSMA_OK;
+    CU(cudaMemcpyAsync(pc_out, p->pc + c0, (size_t)(c1 - c0) * sizeof(double), cudaMemcpyDeviceToDevice, p->stream));
+    if (p->need_grad) CU(cudaMemcpyAsync(pcg_out, p->pcg + 3 * c0, 3 * (size_t)(c1 - c0) * sizeof(double), cudaMemcpyDeviceToDevice, p->stream));
+    return HSMA_OK;
+}
+extern "C" hsma_status hsma_set_check_sums(hsma_plan* p, long long c0, long long c1, const double* pc_in, const double* pcg_in) {
+    if (!p || c0 < 0 || c1 > p->Kt || c0 > c1 || !pc_in || (p->need_grad && !pcg_in)) return HSMA_ERR_INVALID_ARG;
+    if (c1 == c0) return HSMA_OK;
+    CU(cudaMemcpyAsync(p->pc + c0, pc_in, (size_t)(c1 - c0) * sizeof(double), cudaMemcpyDeviceToDevice, p->stream));
+    if (p->need_grad) CU(cudaMemcpyAsync(p->pcg + 3 * c0, pcg_in, 3 * (size_t)(c1 - c0) * sizeof(double), cudaMemcpyDeviceToDevice, p->stream));
+    return HSMA_OK;
+}
+extern "C" hsma_status hsma_evaluate_rest_shard(hsma_plan* plan, const double* xyz, const double* q, long long N,
+                                                long long t0, long long t1, double* phi_out, double* force_out,
+                                                double* energy_out) {
+    return evaluate_impl(plan, xyz, q, N, t0, t1, phi_out, energy_out, force_out, kPhaseRest);
+}
+
 extern "C" hsma_status hsma_plan_sync(hsma_plan* plan) {
     if (!plan) return HSMA_ERR_INVALID_ARG;
     int hf[4] = {0, 0, 0, 0};
@@ -721,7 +766,7 @@ extern "C" const char* hsma_status_string(int s) {
 extern "C" hsma_status hsma_plan_info(hsma_plan* p, long long* w) {
     if (!p || !w) return HSMA_ERR_INVALID_ARG;
     w[0] = p->rows; w[1] = p->ncol; w[2] = p->Kt; w[3] = p->C_near; w[4] = p->C_rhs; w[5] = p->d.M; w[6] = p->d.p;
-    w[7] = p->last_launches; w[8] = p->last_images; w[9] = p->n_node_records;
+    w[7] = p->last_launches; w[8] = p->last_images; w[9] = p->n_node_records; w[10] = p->need_grad ? 1 : 0;
     return HSMA_OK;
 }
 

@@ -45,3 +45,67 @@ def all_reduce_energy(U_local: torch.Tensor, group=None) -> torch.Tensor:
     if dist.is_initialized() and dist.get_world_size(group) > 1:
         dist.all_reduce(U_local, op=dist.ReduceOp.SUM, group=group)
     return U_local
+
+
+def all_gather_slices(local: torch.Tensor, total: int, group=None) -> torch.Tensor:
+    """Concatenate per-rank slices along dim 0 (rank r owns shard_bounds(total, world, align=1)[r]); slices are
+    padded to a common length for the equal-size all_gather."""
+    world = dist.get_world_size(group) if dist.is_initialized() else 1
+    if world == 1:
+        return local
+    bounds = shard_bounds(total, world, align=1)
+    width = max(b - a for a, b in bounds)
+    tail = tuple(local.shape[1:])
+    send = torch.zeros((width,) + tail, dtype=local.dtype, device=local.device)
+    send[: local.shape[0]] = local
+    recv = torch.empty((world * width,) + tail, dtype=local.dtype, device=local.device)
+    dist.all_gather_into_tensor(recv, send, group=group)
+    return torch.cat([recv[r * width: r * width + (b - a)] for r, (a, b) in enumerate(bounds)])
+
+
+def evaluate_distributed(plan, xyz: torch.Tensor, q: torch.Tensor, forces: bool = False, group=None):
+    """One HSMA evaluation over all ranks of `group` (every rank holds all N sources and an identical plan):
+      1. this rank's slice of the check-point sums of step (a)      hsma_check_sums_shard
+      2. all-gather of the K_t check sums (one small message)       the only data-path collective before the fit
+      3. fit, mapping and steps (b), (c) for this rank's targets    hsma_evaluate_rest_shard
+      4. all-gather of phi (and F), all-reduce of U                 assembly of the result
+    Returns (phi [N], F [N,3] or None, U [1]) on every rank.  `plan` is a paper_1806_04801_b200.Plan."""
+    from . import binding
+    N = q.numel()
+    rank = dist.get_rank(group) if dist.is_initialized() else 0
+    world = dist.get_world_size(group) if dist.is_initialized() else 1
+    Kt = plan.info["check_targets"]
+    c0, c1 = shard_bounds(Kt, world, align=1)[rank]
+    t0, t1 = shard_bounds(N, world)[rank]
+    need_grad = bool(binding.hsma_plan_needs_check_gradient(plan.handle))
+    binding.hsma_check_sums_shard(plan.handle, xyz, q, c0, c1)
+    pc = torch.empty(c1 - c0, dtype=torch.float64, device=q.device)
+    pcg = torch.empty(c1 - c0, 3, dtype=torch.float64, device=q.device) if need_grad else None
+    binding.hsma_get_check_sums(plan.handle, c0, c1, pc, pcg)
+    if world > 1:
+        pc_all = all_gather_slices(pc, Kt, group)
+        pcg_all = all_gather_slices(pcg, Kt, group) if need_grad else None
+        binding.hsma_set_check_sums(plan.handle, 0, Kt, pc_all.contiguous(), pcg_all.contiguous() if need_grad else None)
+    T = t1 - t0
+    phi = torch.empty(T, dtype=torch.float64, device=q.device)
+    F = torch.empty(T, 3, dtype=torch.float64, device=q.device) if forces else None
+    U = torch.empty(1, dtype=torch.float64, device=q.device)
+    binding.hsma_evaluate_rest_shard(plan.handle, xyz, q, t0, t1, phi, F, U)
+    phi_all = all_gather_phi(phi, N, group)
+    F_all = None
+    if forces:
+        F_all = F if world == 1 else torch.cat([f for f in _gather_rows(F, N, group)])
+    all_reduce_energy(U, group)
+    return phi_all, F_all, U
+
+
+def _gather_rows(local: torch.Tensor, N: int, group=None):
+    """Per-rank [T_r, 3] blocks in rank order (the shards of shard_bounds(N, world))."""
+    world = dist.get_world_size(group)
+    bounds = shard_bounds(N, world)
+    width = max(b - a for a, b in bounds)
+    send = torch.zeros(width, local.shape[1], dtype=local.dtype, device=local.device)
+    send[: local.shape[0]] = local
+    recv = torch.empty(world * width, local.shape[1], dtype=local.dtype, device=local.device)
+    dist.all_gather_into_tensor(recv, send, group=group)
+    return [recv[r * width: r * width + (b - a)] for r, (a, b) in enumerate(bounds)]

@@ -427,6 +427,57 @@ def test_shards_and_host_path_agree(H):
         assert ph_e.numel() == 0 and float(u_e.cpu().numpy()[0]) == 0.0
 
 
+@pytest.mark.parametrize("closure", ["circumsphere", "face_pairs"])
+def test_sharded_check_sums_phases(H, closure):
+    """Multi-GPU path on one GPU: three "ranks" run the phases of DESIGN.md 8 one after the other -- their slice of
+    the check sums, the gathered check sums, then their target shard -- and reproduce the single-call evaluate."""
+    import torch
+    from paper_1806_04801_b200 import shard
+    w = W.config(5, N=7000)
+    if closure == "face_pairs":
+        w = w.with_(closure=W.CLOSURE_FACE_PAIRS, K=900, p=12, M=6000)
+    world = 3
+    with H.Plan.from_workload(w) as plan:
+        xyz, q = dev(w.xyz), dev(w.q)
+        phi_ref, F_ref, U_ref = plan.evaluate_forces(xyz, q, sync=True)
+        Kt = plan.info["check_targets"]
+        need_grad = H.binding.hsma_plan_needs_check_gradient(plan.handle)
+        assert need_grad == (closure == "face_pairs")
+        pcs, pcgs = [], []
+        for a, b in shard.shard_bounds(Kt, world, align=1):
+            H.hsma_check_sums_shard(plan.handle, xyz, q, a, b)
+            pc = torch.empty(b - a, dtype=torch.float64, device="cuda")
+            pcg = torch.empty(b - a, 3, dtype=torch.float64, device="cuda") if need_grad else None
+            H.hsma_get_check_sums(plan.handle, a, b, pc, pcg)
+            pcs.append(pc.clone())
+            pcgs.append(pcg.clone() if need_grad else None)
+        # scramble the plan's copy, then install the gathered sums: the rest phase must use exactly those
+        H.hsma_set_check_sums(plan.handle, 0, Kt, torch.zeros(Kt, dtype=torch.float64, device="cuda"),
+                              torch.zeros(Kt, 3, dtype=torch.float64, device="cuda") if need_grad else None)
+        H.hsma_set_check_sums(plan.handle, 0, Kt, torch.cat(pcs), torch.cat(pcgs) if need_grad else None)
+        phis, Fs, Usum = [], [], 0.0
+        for a, b in shard.shard_bounds(w.N, world):
+            ph = torch.empty(b - a, dtype=torch.float64, device="cuda")
+            F = torch.empty(b - a, 3, dtype=torch.float64, device="cuda")
+            U = torch.empty(1, dtype=torch.float64, device="cuda")
+            H.hsma_evaluate_rest_shard(plan.handle, xyz, q, a, b, ph, F, U)
+            plan.sync()
+            phis.append(ph)
+            Fs.append(F)
+            Usum += float(U)
+        phi, F = torch.cat(phis), torch.cat(Fs)
+        assert float((phi - phi_ref).abs().max()) <= 1e-12 * float(phi_ref.abs().max())
+        assert float((F - F_ref).abs().max()) <= 1e-12 * float(F_ref.abs().max())
+        assert abs(Usum - float(U_ref)) <= 1e-12 * abs(float(U_ref))
+        # the one-call helper with world = 1 is the same path
+        phi1, F1, U1 = shard.evaluate_distributed(plan, xyz, q, forces=True)
+        plan.sync()
+        assert float((phi1 - phi_ref).abs().max()) <= 1e-12 * float(phi_ref.abs().max())
+        assert abs(float(U1) - float(U_ref)) <= 1e-12 * abs(float(U_ref))
+    r = O.hsma(w)
+    assert rel_inf(phi.cpu().numpy(), r.phi) <= PHI_TOL
+
+
 def test_deterministic(H):
     w = W.config(3)
     with H.Plan.from_workload(w) as plan:

@@ -61,6 +61,30 @@ def test_two_ranks_assemble_the_single_rank_result(tmp_path, N):
         assert abs(U - ref.U) <= 1e-14 * abs(ref.U)
 
 
+def _slices_worker(rank, world, port, total, out_dir):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        a, b = shard.shard_bounds(total, world, align=1)[rank]
+        vec = torch.arange(a, b, dtype=torch.float64)
+        mat = torch.stack([vec, 2 * vec, -vec], dim=1)
+        np.save(os.path.join(out_dir, f"v{rank}.npy"), shard.all_gather_slices(vec, total).numpy())
+        np.save(os.path.join(out_dir, f"m{rank}.npy"), shard.all_gather_slices(mat, total).numpy())
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("total", [7, 4000])
+def test_all_gather_slices_reassembles_in_order(tmp_path, total):
+    """The check-point sums of step (a) are sharded with align = 1 and gathered before the fit."""
+    world, port = 2, 31500 + (os.getpid() + total) % 2000
+    mp.spawn(_slices_worker, args=(world, port, total, str(tmp_path)), nprocs=world, join=True)
+    want = np.arange(total, dtype=np.float64)
+    for r in range(world):
+        assert np.array_equal(np.load(tmp_path / f"v{r}.npy"), want)
+        assert np.array_equal(np.load(tmp_path / f"m{r}.npy"), np.stack([want, 2 * want, -want], axis=1))
+
+
 def test_single_process_is_a_no_op():
     x = torch.arange(5, dtype=torch.float64)
     assert shard.all_gather_phi(x, 5) is x
