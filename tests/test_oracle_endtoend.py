@@ -196,3 +196,16 @@ def test_rejections():
         O.hsma(w.with_(R_aux=1.6))                          # sphere pokes out of the 3^3 block (S7)
     with pytest.raises(ValueError):
         O.hsma(w.with_(R_aux=0.8))                          # inside the circumsphere
+
+
+def test_stored_config5_values_are_the_oracles():
+    """tests/golden/config5_oracle.txt (used by the GPU parity test at full size) is what the oracle computes:
+    two of its stored potentials are recomputed here (the fit needs the full step (a): 2.8e10 pairs)."""
+    rows = golden("config5_oracle.txt")
+    w = W.config(5)
+    r = O.hsma(w, targets_slice=slice(0, 257))
+    stored = {int(a): b for a, b in rows[1:]}
+    assert abs(r.phi[0] - stored[0]) <= 1e-13 * rows[0][1]
+    assert abs(r.phi[256] - stored[256]) <= 1e-13 * rows[0][1]
+    assert abs(r.fit_rms - rows[0][2]) <= 1e-9 * rows[0][2]
+    assert len(rows) - 1 == w.N // 256
