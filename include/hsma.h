@@ -19,6 +19,8 @@
  *   - periodic kinds: phi is in the gauge A_00 = 0 (reading S2); U is gauge free for neutral input.
  *   - hsma_evaluate* are asynchronous on the plan's stream and perform no host synchronisation
  *     (hsma_evaluate_host synchronises because it returns host data).
+ *   - on a non-default stream, repeated evaluates with identical arguments (same pointers and sizes: the MD loop)
+ *     are captured into one CUDA graph on the second call and replayed afterwards.
  *   - preconditions not checked: particles inside the box, no coincident particles, no particle on
  *     a check point (reading S13).
  */
@@ -195,7 +197,7 @@ const char* hsma_status_string(int status);
 /* sizes: what[0]=rows of the fit, [1]=columns, [2]=check targets K_t, [3]=near cells, [4]=rhs cells,
  * [5]=M nodes, [6]=p, [7]=kernels launched by the last evaluate, [8]=near images summed per target by the last
  * evaluate (N * cells, or the image count inside the sphere), [9]=node records (M or 3M), [10]=1 if the fit has derivative rows (step (a) then also
- * produces grad Phi_in at the check targets).  host out [11]. */
+ * produces grad Phi_in at the check targets), [11]=evaluates served by replaying the plan's CUDA graph.  host out [12]. */
 hsma_status hsma_plan_info(hsma_plan* plan, long long* what_out);
 /* copies of plan/evaluate state into caller DEVICE buffers (valid after an evaluate on the stream) */
 hsma_status hsma_get_coeffs(hsma_plan* plan, double* A_out /* dev [p*p], R0-scaled basis */);

@@ -302,10 +302,10 @@ def hsma_plan_sync(plan: int):
 
 
 def hsma_plan_info(plan: int) -> dict:
-    w = (ctypes.c_longlong * 11)()
+    w = (ctypes.c_longlong * 12)()
     _check(load_library().hsma_plan_info(plan, w), "hsma_plan_info")
     keys = ("rows", "cols", "check_targets", "near_cells", "rhs_cells", "M", "p", "launches_last_evaluate",
-            "near_images_last_evaluate", "node_records", "check_gradient")
+            "near_images_last_evaluate", "node_records", "check_gradient", "graph_replays")
     return dict(zip(keys, [int(v) for v in w]))
 
 

@@ -512,6 +512,59 @@ def test_sharded_check_sums_phases(H, closure):
     assert rel_inf(phi.cpu().numpy(), r.phi) <= PHI_TOL
 
 
+def test_cuda_graph_replay_on_a_side_stream(H):
+    """on a non-default stream the second evaluate with identical arguments is captured into a CUDA
+    graph and later ones replay it.  Replays must give bit-identical results, follow the DATA behind the same
+    pointers (also across the generic / uniform-|q| switch, which is decided on the device), and a changed argument
+    set must fall back to the normal path."""
+    import torch
+    w = W.config(3)
+    r = O.hsma(w)
+    side = torch.cuda.Stream()
+    with H.Plan.from_workload(w) as plan0:                      # default stream: no graph
+        phi0, U0 = plan0.evaluate(dev(w.xyz), dev(w.q), sync=True)
+        assert plan0.info["graph_replays"] == 0
+    with torch.cuda.stream(side):
+        with H.Plan.from_workload(w) as plan:
+            xyz, q = dev(w.xyz), dev(w.q)
+            phi = torch.empty(w.N, dtype=torch.float64, device="cuda")
+            U = torch.empty(1, dtype=torch.float64, device="cuda")
+            outs = []
+            for _ in range(5):
+                H.hsma_evaluate(plan.handle, xyz, q, phi, U)
+                plan.sync()
+                outs.append((phi.clone(), float(U)))
+            assert H.binding.hsma_plan_info(plan.handle)["graph_replays"] == 4      # call 1 runs plainly, 2-5 via the graph
+            for ph, u in outs:
+                assert torch.equal(ph, phi0) and u == float(U0)
+            assert rel_inf(phi.cpu().numpy(), r.phi) <= PHI_TOL
+            # new data behind the same pointers: random magnitudes -> the generic kernels inside the same graph
+            q2 = np.random.default_rng(9).standard_normal(w.N)
+            q.copy_(dev(q2))
+            H.hsma_evaluate(plan.handle, xyz, q, phi, U)
+            plan.sync()
+            assert H.binding.hsma_plan_info(plan.handle)["graph_replays"] == 5
+            r2 = O.hsma(w.with_(q=q2))
+            assert rel_inf(phi.cpu().numpy(), r2.phi) <= PHI_TOL and abs(float(U) - r2.U) <= U_TOL * abs(r2.U)
+            # forces: another argument set -> plain, then captured again
+            F = torch.empty(w.N, 3, dtype=torch.float64, device="cuda")
+            for _ in range(3):
+                H.hsma_evaluate_forces(plan.handle, xyz, q, phi, F, U)
+                plan.sync()
+            assert H.binding.hsma_plan_info(plan.handle)["graph_replays"] == 7
+            rf = O.hsma(w.with_(q=q2), forces=True)
+            assert rel_inf(F.cpu().numpy(), rf.F) <= 1e-10
+            # a larger system reallocates plan buffers: the graph is dropped, results stay right
+            wb = W.config(3, N=6000)
+            phib, Ub = plan.evaluate(dev(wb.xyz), dev(wb.q), sync=True)
+            rb = O.hsma(wb)
+            assert rel_inf(phib.cpu().numpy(), rb.phi) <= PHI_TOL
+            H.hsma_evaluate_forces(plan.handle, xyz, q, phi, F, U)      # old arguments again: plain call, still right
+            plan.sync()
+            assert rel_inf(F.cpu().numpy(), rf.F) <= 1e-10
+    torch.cuda.synchronize()
+
+
 def test_deterministic(H):
     w = W.config(3)
     with H.Plan.from_workload(w) as plan:
