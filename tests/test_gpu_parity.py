@@ -251,6 +251,21 @@ def test_config5_full_size_sampled(H):
     assert abs(float(U.cpu().numpy()[0]) - Uref) <= U_TOL * abs(Uref)
 
 
+def test_non_cubic_periodic_box(H):
+    """Three different box sides, both closures of the periodic kind, potentials and forces."""
+    L = (1.0, 1.2, 0.9)
+    N = 1800
+    xyz = np.random.default_rng(13).random((N, 3)) * np.asarray(L)
+    w = W.Workload("box", W.BC_PERIODIC, L, (1, 1, 1), 1.0, 1.3, 12, 5000, 800, xyz, W.alternating_charges(N))
+    for ww in (w, w.with_(closure=W.CLOSURE_FACE_PAIRS)):
+        r, phi, U, extra = run_both(H, ww)
+        check_parity(r, phi, U, extra, f"non-cubic box closure={ww.closure}")
+        rf = O.hsma(ww, forces=True)
+        with H.Plan.from_workload(ww) as plan:
+            _, F, _ = plan.evaluate_forces(dev(ww.xyz), dev(ww.q), sync=True)
+        assert rel_inf(F.cpu().numpy(), rf.F) <= 1e-10
+
+
 # ------------------------------------------------------------------ grounded slab (SURVEY.md 8(f) NEXT 3, first part)
 @pytest.mark.parametrize("refine", [1, 2])
 @pytest.mark.parametrize("neutral", [True, False])

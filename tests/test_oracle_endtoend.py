@@ -209,3 +209,17 @@ def test_stored_config5_values_are_the_oracles():
     assert abs(r.phi[256] - stored[256]) <= 1e-13 * rows[0][1]
     assert abs(r.fit_rms - rows[0][2]) <= 1e-9 * rows[0][2]
     assert len(rows) - 1 == w.N // 256
+
+
+def test_non_cubic_periodic_box_matches_ewald():
+    """A box with three different sides (the paper's tests are cubic): both closures of the periodic kind."""
+    L = (1.0, 1.2, 0.9)
+    rng = np.random.default_rng(12)
+    N = 100
+    xyz = rng.random((N, 3)) * np.array(L)
+    q = W.alternating_charges(N)
+    U_e = 0.5 * float(q @ pins.ewald_potentials(xyz, q, np.array(L), alpha=7.0, rcut_cells=1, kmax=12))
+    w = W.Workload("box", W.BC_PERIODIC, L, (1, 1, 1), 1.0, 1.3, 16, 6000, 900, xyz, q)
+    assert abs(O.hsma(w).U - U_e) < 2e-6 * abs(U_e)
+    assert abs(O.hsma(w.with_(closure=W.CLOSURE_FACE_PAIRS)).U - U_e) < 4e-6 * abs(U_e)
+    assert abs(O.hsma(w.with_(p=10, K=500)).U - U_e) < 2e-3 * abs(U_e)
