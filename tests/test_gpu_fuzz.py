@@ -1,0 +1,118 @@
+"""Seeded random sweep of the raw kernels and of whole evaluates against the oracle: sizes around the tile (256),
+block (256 R) and grid boundaries of the persistent decomposition, every boundary kind / closure / mode.  `-m gpu`."""
+import math
+
+import numpy as np
+import pytest
+
+import hsma_workloads as W
+from oracle import hsma_oracle as O
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def H():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    import paper_1806_04801_b200 as H
+    H.binding.load_library()
+    return H
+
+
+def dev(a):
+    import torch
+    return torch.as_tensor(np.ascontiguousarray(a, dtype=np.float64), device="cuda")
+
+
+def rel_inf(a, b):
+    return float(np.max(np.abs(a - b)) / max(np.max(np.abs(b)), 1e-300))
+
+
+SIZES = [1, 2, 31, 255, 256, 257, 511, 512, 513, 1023, 1024, 1025, 2047, 2048, 2049, 3000, 4095, 4097, 9001]
+KINDS = [(W.BC_PERIODIC, (1.0, 1.0, 1.0), (1, 1, 1), 1.0), (W.BC_PERIODIC, (1.0, 0.8, 1.3), (2, 2, 1), 1.0),
+         (W.BC_MIRROR_CAVITY, (1.0, 1.5, 0.7), (1, 1, 1), -1.0), (W.BC_MIRROR_CAVITY, (1.0, 1.0, 1.0), (1, 1, 1), 1.0),
+         (W.BC_SLAB_XY_PERIODIC_Z_MIRROR, (1.0, 1.0, 0.5), (1, 1, 2), 0.5)]
+
+
+@pytest.mark.parametrize("case", range(60))
+def test_raw_sums_random_shapes(H, case):
+    import torch
+    rng = np.random.default_rng(1000 + case)
+    N = int(rng.choice(SIZES))
+    kind, L, shell, gamma = KINDS[case % len(KINDS)]
+    refine = 1 + case % 2
+    Lh = np.asarray(L)
+    src = (rng.random((N, 3)) - 0.5) * Lh
+    pattern = case % 4
+    q = [rng.standard_normal(N), W.alternating_charges(N), np.full(N, -0.5),
+         np.where(rng.random(N) < 0.3, 1.0, -1.0)][pattern]
+    cells = O.cell_table(kind, L, shell, gamma)
+    self_mode = case % 3 == 0
+    if self_mode:
+        t0 = int(rng.integers(0, N))
+        T = int(rng.integers(1, N - t0 + 1))
+        tgt = src[t0:t0 + T]
+        so = t0
+    else:
+        T = int(rng.choice(SIZES[:14]))
+        tgt = (rng.random((T, 3)) - 0.5) * Lh * 1.1
+        so = -1
+    ref = O.near_sum(tgt, src, q, cells, self_offset=so)
+    refg = O.near_grad(tgt, src, q, cells, self_offset=so)
+    out = torch.empty(T, dtype=torch.float64, device="cuda")
+    H.hsma_direct_sum(dev(tgt), dev(src), dev(q), cells.shift, cells.sign, cells.w, cells.central, so, refine, out)
+    scale = max(np.max(np.abs(ref)), np.max(np.abs(q)))          # image terms may cancel: the size of one term counts too
+    tol = 5e-11 if refine == 1 else 1e-12
+    got = out.cpu().numpy()
+    assert np.all(np.isfinite(got)) and np.max(np.abs(got - ref)) <= tol * scale
+    phi = torch.empty(T, dtype=torch.float64, device="cuda")
+    g = torch.empty(T, 3, dtype=torch.float64, device="cuda")
+    H.hsma_direct_field(dev(tgt), dev(src), dev(q), cells.shift, cells.sign, cells.w, cells.central, so, refine, phi, g)
+    assert np.max(np.abs(phi.cpu().numpy() - ref)) <= tol * scale
+    gscale = max(np.max(np.abs(refg)), np.max(np.abs(q)))
+    assert np.max(np.abs(g.cpu().numpy() - refg)) <= 3 * tol * gscale
+
+
+@pytest.mark.parametrize("case", range(24))
+def test_whole_evaluates_random_configurations(H, case):
+    rng = np.random.default_rng(5000 + case)
+    N = 2 * int(rng.integers(1, 1800))
+    which = case % 6
+    p = int(rng.integers(4, 13))
+    M = int(rng.integers(300, 3000))
+    K = int(2 * p * p + rng.integers(20, 300))
+    s32 = math.sqrt(3.0) / 2.0
+    if which == 0:
+        w = W.Workload("f", W.BC_PERIODIC, (1.0, 1.0, 1.0), (1, 1, 1), 1.0, float(rng.uniform(1.05, 1.7)) * s32, p, M, K,
+                       rng.random((N, 3)), W.alternating_charges(N))
+    elif which == 1:
+        w = W.Workload("f", W.BC_PERIODIC, (1.0, 1.0, 1.0), (1, 1, 1), 1.0, 1.5 * s32, p, M, K, rng.random((N, 3)),
+                       W.alternating_charges(N), closure=W.CLOSURE_FACE_PAIRS)
+    elif which == 2:
+        L = (1.0, 1.0, 1.0)
+        w = W.Workload("f", W.BC_MIRROR_CAVITY, L, (1, 1, 1), -1.0, 1.5 * s32, p, M, K, 0.02 + 0.96 * rng.random((N, 3)),
+                       rng.standard_normal(N), check_xyz=W.seeded_face_points(K, L, W.ALL_FACES, seed=case))
+    elif which == 3:
+        L = (1.0, 1.0, 1.0)
+        q = rng.standard_normal(N)
+        w = W.Workload("f", W.BC_MIRROR_CAVITY, L, (1, 1, 1), 1.0, 1.5 * s32, p, M, K, 0.02 + 0.96 * rng.random((N, 3)),
+                       q - q.mean(), check_xyz=W.seeded_face_points(K, L, W.ALL_FACES, seed=case))
+    elif which == 4:
+        L = (1.0, 1.0, 0.5)
+        xyz = rng.random((N, 3)) * np.asarray(L)
+        xyz[:, 2] = 0.02 + 0.92 * xyz[:, 2]
+        w = W.Workload("f", W.BC_SLAB_XY_PERIODIC_Z_MIRROR, L, (1, 1, 2), -1.0, 1.1, p, M, K, xyz, rng.standard_normal(N),
+                       closure=W.CLOSURE_BOUNDARY)
+    else:
+        w = W.Workload("f", W.BC_PERIODIC, (1.0, 1.0, 1.0), (1, 1, 1), 1.0, 1.3 * s32, p, M, K, rng.random((N, 3)),
+                       W.alternating_charges(N), near_mode=W.NEAR_SPHERE)
+    refine = case % 3
+    r = O.hsma(w, forces=True)
+    with H.Plan.from_workload(w, rsqrt_refine=refine) as plan:
+        phi, F, U = plan.evaluate_forces(dev(w.xyz), dev(w.q), sync=True)
+        phi0, U0 = plan.evaluate(dev(w.xyz), dev(w.q), sync=True)
+    assert rel_inf(phi.cpu().numpy(), r.phi) <= 1e-10 and rel_inf(phi0.cpu().numpy(), r.phi) <= 1e-10
+    # random charges can make U = 1/2 sum q phi cancel to almost nothing; its rounding floor is eps sum|q| max|phi|
+    assert abs(float(U) - r.U) <= 1e-11 * abs(r.U) + 1e-13 * float(np.abs(w.q).sum() * np.max(np.abs(r.phi)))
+    assert rel_inf(F.cpu().numpy(), r.F) <= 1e-10
