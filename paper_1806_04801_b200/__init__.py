@@ -117,6 +117,14 @@ class Plan:
     def timing(self) -> dict:
         return binding.hsma_plan_get_timing(self.handle)
 
+    def set_pair_form(self, form: int):
+        """0: automatic (symmetric form of step (b) when it applies); 1: ordered pairs always."""
+        binding.hsma_plan_set_pair_form(self.handle, form)
+
+    @property
+    def last_pair_form(self) -> int:
+        return binding.hsma_plan_last_pair_form(self.handle)
+
     # -- introspection (device tensors) ----------------------------------------------------------
     def _new(self, *shape):
         return torch.empty(*shape, dtype=torch.float64, device="cuda")

@@ -99,6 +99,8 @@ _SIGNATURES = {
                                        ctypes.c_void_p]),
     "hsma_fp64_peak": (ctypes.c_int, [ctypes.c_double, c_double_p, c_double_p]),
     "hsma_plan_set_timing": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int]),
+    "hsma_plan_set_pair_form": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int]),
+    "hsma_plan_last_pair_form": (ctypes.c_int, [ctypes.c_void_p]),
     "hsma_plan_get_timing": (ctypes.c_int, [ctypes.c_void_p, c_double_p]),
     "hsma_launch_count": (ctypes.c_longlong, []),
 }
@@ -386,6 +388,19 @@ TIMING_KEYS = ("prepass", "near_check_kernel", "fit_map", "near_source_kernel", 
 
 def hsma_plan_set_timing(plan: int, enable: bool):
     _check(load_library().hsma_plan_set_timing(plan, 1 if enable else 0), "hsma_plan_set_timing")
+
+
+PAIR_FORM_AUTO, PAIR_FORM_ORDERED, PAIR_FORM_SYMMETRIC = 0, 1, 2
+
+
+def hsma_plan_set_pair_form(plan: int, form: int):
+    """Step (b): 0 = automatic (symmetric form when it applies), 1 = ordered pairs always."""
+    _check(load_library().hsma_plan_set_pair_form(plan, int(form)), "hsma_plan_set_pair_form")
+
+
+def hsma_plan_last_pair_form(plan: int) -> int:
+    """What the last evaluate used for step (b): 1 ordered pairs, 2 symmetric (each unordered pair once)."""
+    return int(load_library().hsma_plan_last_pair_form(plan))
 
 
 def hsma_plan_get_timing(plan: int) -> dict:

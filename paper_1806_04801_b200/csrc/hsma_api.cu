@@ -171,6 +171,35 @@ static Launch choose_near(long long T, long long n_tiles, int C, int refine, boo
     return choose_launch(T, n_tiles * C, field ? 4 : 8, [refine, field](int R) { return near_resident(R, refine, field); });
 }
 
+// Symmetric form of step (b) (sum_kernels.cuh near_sym_kernel): launch shape and buffers.
+struct SymLaunch {
+    int n_blocks, G, rows;
+    long long visits, fine;
+};
+static int sym_resident(int refine) {
+    static int cache[2] = {0, 0};
+    int& c = cache[refine == 1 ? 0 : 1];
+    if (!c) c = refine == 1 ? resident_ctas(near_sym_kernel<1>) : resident_ctas(near_sym_kernel<2>);
+    return c;
+}
+static SymLaunch choose_sym(long long n_tiles, int refine) {
+    SymLaunch L;
+    L.n_blocks = (int)((n_tiles + kSymR - 1) / kSymR);
+    L.visits = sym_visit0(L.n_blocks, n_tiles);
+    L.fine = L.visits * kSymChunks;
+    L.G = (int)std::min<long long>(sym_resident(refine), L.fine);
+    L.rows = 1;
+    for (int I = 0; I < L.n_blocks; ++I) {
+        const int first = cta_of_unit(sym_visit0(I, n_tiles) * kSymChunks, L.fine, L.G);
+        const int last = cta_of_unit(sym_visit0(I + 1, n_tiles) * kSymChunks - 1, L.fine, L.G);
+        L.rows = std::max(L.rows, last - first + 1);
+    }
+    return L;
+}
+// The symmetric form pays when most visits are off the diagonal (a diagonal visit costs 11 instructions per ORDERED
+// pair): from 32 source tiles on, and while the cell table fits its shared-memory copy.
+static bool sym_applies(long long n_tiles, int C) { return n_tiles >= 32 && C <= kSymMaxCells; }
+
 static Launch choose_node(long long T, long long n_tiles, bool field = false) {
     return choose_launch(T, n_tiles, 4, [field](int R) { return node_resident(R, field); });
 }
@@ -237,6 +266,9 @@ struct hsma_plan {
     DevBuf<int> slot_of, tile_np;
     QInfo* qinfo = nullptr;
     DevBuf<double> part_a, part_b, part_c, red, xyz_in, q_in, phi_dev, force_dev;
+    DevBuf<double> sym_col, sym_phi;   // symmetric form of step (b): column sums per visit, phi_near in source order
+    int pair_form = 0;                 // hsma_plan_set_pair_form: 0 = automatic, 1 = ordered pairs only
+    int last_pair_form = 1;            // what the last evaluate used for step (b): 1 ordered, 2 symmetric
     long long last_launches = 0;
     hsma_status sticky = HSMA_OK;
     // CUDA graph of the whole evaluate: captured on the second call with identical arguments,
@@ -275,7 +307,7 @@ static void plan_free(hsma_plan* p) {
     if (p->img_qinfo) cudaFree(p->img_qinfo);
     p->img_counts.release(); p->img_xyz.release(); p->img_q.release(); p->img_stats.release(); p->img_src.release();
     p->img_slot_of.release(); p->img_tile_np.release();
-    p->part_a.release(); p->part_b.release(); p->part_c.release(); p->red.release();
+    p->part_a.release(); p->part_b.release(); p->part_c.release(); p->red.release(); p->sym_col.release(); p->sym_phi.release();
     p->xyz_in.release(); p->q_in.release(); p->phi_dev.release(); p->force_dev.release();
     for (cudaEvent_t e : p->ev) if (e) cudaEventDestroy(e);
     if (p->gexec) cudaGraphExecDestroy(p->gexec);
@@ -626,13 +658,37 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
         const int refine = p->refine ? p->refine : ((double)N * (double)p->last_images < 4294967296.0 ? 2 : 1);
         // rsqrt_refine = 0: the cubic step while (b) is latency-bound anyway (< 2^32 pairs), Newton above
         const size_t comps = field ? 4 : 1;
-        const Launch sb = choose_near(T, n_tiles_near, C_b, refine, field);
-        if (p->part_b.reserve((size_t)sb.rows * T * comps) != cudaSuccess) return HSMA_ERR_ALLOC;
+        const bool sym = !field && !p->sphere && p->pair_form == 0 && t0 == 0 && t1 == N && sym_applies(n_tiles, C_b);
+        p->last_pair_form = sym ? 2 : 1;
+        Launch sb = choose_near(T, n_tiles_near, C_b, refine, field);
+        SymLaunch ss{};
+        if (sym) {
+            ss = choose_sym(n_tiles, refine);
+            if (p->part_b.reserve((size_t)ss.rows * ss.n_blocks * kSymBlock) != cudaSuccess ||
+                p->sym_col.reserve((size_t)ss.visits * kTile) != cudaSuccess || p->sym_phi.reserve((size_t)N) != cudaSuccess)
+                return HSMA_ERR_ALLOC;
+        } else if (p->part_b.reserve((size_t)sb.rows * T * comps) != cudaSuccess) {
+            return HSMA_ERR_ALLOC;
+        }
         const Launch sc = choose_node(T, p->node_tiles, field);
         if (p->part_c.reserve((size_t)sc.rows * T * comps) != cudaSuccess) return HSMA_ERR_ALLOC;
         MARK(3);
-        launch_near(sb, field, reinterpret_cast<const double*>(p->src.p), 4, p->slot_of.p, T, t0, P, cells_b, C_b,
-                    t0, refine, p->part_b.p, st);
+        PartLayout layout_b = sb.layout(p->part_b.p);
+        if (sym) {
+            // every unordered (source, source) pair once: row sums + column sums, then phi_near in source order
+            SymArgs a;
+            a.src = p->src.p; a.n_src = N; a.n_tiles = n_tiles; a.n_blocks = ss.n_blocks; a.cells = cells_b; a.C = C_b;
+            a.fine = ss.fine; a.scale = refine == 1 ? 0.5 : 1.0; a.part = p->part_b.p; a.col = p->sym_col.p;
+            if (refine == 1) near_sym_kernel<1><<<ss.G, kThreads, 0, st>>>(a);
+            else near_sym_kernel<2><<<ss.G, kThreads, 0, st>>>(a);
+            sym_gather_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(p->part_b.p, p->sym_col.p, p->slot_of.p, N, n_tiles,
+                                                                          ss.n_blocks, ss.fine, ss.G, p->sym_phi.p);
+            HSMA_COUNT_LAUNCH(); HSMA_COUNT_LAUNCH();
+            layout_b = PartLayout{p->sym_phi.p, 1, 1, 1, (int)std::min<long long>(T, 2147483647LL)};
+        } else {
+            launch_near(sb, field, reinterpret_cast<const double*>(p->src.p), 4, p->slot_of.p, T, t0, P, cells_b, C_b,
+                        t0, refine, p->part_b.p, st);
+        }
         MARK(4);
         // H6 (c): sphere nodes, charge + dipole
         launch_node(sc, field, reinterpret_cast<const double*>(p->src.p), 4, p->slot_of.p, T, t0, p->nodes, p->node_tiles, p->part_c.p, st);
@@ -643,7 +699,7 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
             finish_field_kernel<<<(unsigned)fb, 256, 0, st>>>(sb.layout(p->part_b.p), sc.layout(p->part_c.p), T, p->src.p, p->slot_of.p, t0,
                                                               phi_out, force_out, energy_out ? p->red.p : nullptr);
         else
-            finish_phi_kernel<<<(unsigned)fb, 256, 0, st>>>(sb.layout(p->part_b.p), sc.layout(p->part_c.p), T, p->src.p, p->slot_of.p, t0, phi_out,
+            finish_phi_kernel<<<(unsigned)fb, 256, 0, st>>>(layout_b, sc.layout(p->part_c.p), T, p->src.p, p->slot_of.p, t0, phi_out,
                                                             energy_out ? p->red.p : nullptr);
         HSMA_COUNT_LAUNCH();
         if (energy_out) {
@@ -1043,6 +1099,15 @@ extern "C" hsma_status hsma_plan_set_timing(hsma_plan* p, int enable) {
     p->ev_valid = false;
     return HSMA_OK;
 }
+
+extern "C" hsma_status hsma_plan_set_pair_form(hsma_plan* p, int form) {
+    if (!p || (form != 0 && form != 1)) return HSMA_ERR_INVALID_ARG;
+    p->pair_form = form;
+    ++g_alloc_epoch;   // a captured evaluate graph holds the other form's launches
+    return HSMA_OK;
+}
+
+extern "C" int hsma_plan_last_pair_form(const hsma_plan* p) { return p ? p->last_pair_form : 0; }
 
 extern "C" hsma_status hsma_plan_get_timing(hsma_plan* p, double* ms_out) {
     if (!p || !ms_out || !p->timing || !p->ev_valid) return HSMA_ERR_INVALID_ARG;

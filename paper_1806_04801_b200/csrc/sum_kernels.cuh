@@ -326,6 +326,223 @@ __global__ void __launch_bounds__(kThreads, near_min_ctas(FIELD ? 2 * R : R)) ne
     if (!fresh) store_block(b);
 }
 
+// ---- step (b), symmetric form (Newton's third law) ---------------------------------------------
+// When the targets ARE the sources (step (b) over all N, Eq.(5) with the self term left out), the
+// image sum is symmetric: the image of source j in cell (k, sigma) lies as far from target i as the image of
+// source i in the partner cell (-sigma o k, sigma), which has the same weight gamma^|k| (the cell
+// table is closed under that map).  So one evaluation y = w / |r_i - img_c(r_j)| serves two sums:
+//     phi_i += q_j y      (row sum, in the registers of the thread that owns target i)
+//     phi_j += q_i y      (column sum: reduced over the 8 targets of a thread, over the cells, then over the lanes)
+// and only the unordered pairs are walked: target block I (kSymBlock packed sources = kSymR tiles) meets source
+// tiles J >= I * kSymR.  The block's own tiles ("diagonal" visits) are done as ordered pairs (row sums only,
+// self term masked in the central cell); every later tile gives both.  Per unordered pair (Newton form):
+// 3 DADD + DMUL + 2 DFMA (r2) + MUFU + DMUL (t) + DFMA (g) + DMUL (y) + 2 DFMA = 11 FP64-pipe instructions, i.e.
+// 5.5 per pair interaction against 9 in near_sum_kernel.  Images are made by moving the SOURCE here
+// (flip + shift of 4 sources per cell), so nothing per-cell lives in registers on the target side and the
+// column sums of a chunk of kSymS sources stay in registers across all cells: one warp reduction per source
+// and tile visit, not per cell.
+// Work decomposition: visits v = (I, J) in block-major order, each cut into kSymChunks chunks of kSymS sources;
+// the fine units f = v * kSymChunks + chunk are dealt to the persistent grid in contiguous ranges exactly as in
+// near_sum_kernel (balance to within one chunk).  Row sums go to part[row][packed index] (row = CTA - first CTA
+// of the block), column sums to col[v][j]; sym_gather_kernel adds both in a fixed order (deterministic).
+constexpr int kSymR = 8;                        // targets per thread
+constexpr int kSymS = 4;                        // sources per chunk
+constexpr int kSymChunks = kTile / kSymS;       // chunks per tile visit
+constexpr int kSymBlock = kThreads * kSymR;     // targets per block
+constexpr int kSymMaxCells = 128;               // cell table entries of this form (static shared memory <= 48 KB)
+// first visit of block I (block I visits tiles I*kSymR .. n_tiles-1)
+__host__ __device__ inline long long sym_visit0(long long I, long long n_tiles) {
+    return I * n_tiles - (long long)kSymR * (I * (I - 1) / 2);
+}
+
+struct SymArgs {
+    const Src4* src;     // packed sources (pack_sources_kernel); targets are the same records
+    long long n_src, n_tiles;
+    int n_blocks;        // ceil(n_tiles / kSymR)
+    const Cell* cells;
+    int C;
+    long long fine;      // F = sym_visit0(n_blocks) * kSymChunks
+    double scale;        // 0.5 for the Newton form (y is twice the reciprocal distance)
+    double* part;        // [rows][n_blocks * kSymBlock]
+    double* col;         // [visits][kTile]
+};
+
+template <int REFINE>
+__device__ __forceinline__ double sym_recip(double dx, double dy, double dz) {
+    const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+    const double y0 = rsqrt_seed(r2);
+    const double t = y0 * y0;
+    if (REFINE == 1) {
+        const double g = fma(-r2, t, kNewton3);
+        return y0 * g;
+    } else {
+        const double e = fma(-r2, t, 1.0);
+        const double h = fma(e, 0.375, 0.5);
+        const double k = fma(e, h, 1.0);
+        return y0 * k;
+    }
+}
+
+template <int REFINE>
+__global__ void __launch_bounds__(kThreads, 1) near_sym_kernel(const SymArgs a) {
+    __shared__ __align__(128) Src4 tile[kStages][kTile];
+    __shared__ __align__(8) uint64_t full[kStages];
+    __shared__ Cell cells[kSymMaxCells];
+    __shared__ double colw[kThreads / 32][kTile];
+
+    constexpr int R = kSymR, S = kSymS;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int G = gridDim.x, k = blockIdx.x;
+    const long long f0 = unit_start(k, a.fine, G), f1 = unit_start(k + 1, a.fine, G);
+    if (f1 <= f0) return;
+    const long long V0 = f0 / kSymChunks, V1 = (f1 - 1) / kSymChunks;
+    const int nt = (int)a.n_tiles;
+    int I = 0;
+    while (sym_visit0(I + 1, nt) <= V0) ++I;
+    int J = I * R + (int)(V0 - sym_visit0(I, nt));
+
+    for (int c = tid; c < a.C; c += kThreads) cells[c] = a.cells[c];
+    if (tid == 0) {
+        for (int s = 0; s < kStages; ++s) mbar_init(&full[s], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    if (tid == 0) {
+        mbar_expect_tx(&full[0], kTile * sizeof(Src4));
+        bulk_g2s(tile[0], a.src + (long long)J * kTile, kTile * sizeof(Src4), &full[0]);
+    }
+
+    double ox[R], oy[R], oz[R], oq[R], tot[R];
+    const int nvis = (int)(V1 - V0) + 1;
+    const int ch_first = (int)(f0 - V0 * kSymChunks), ch_last = (int)(f1 - 1 - V1 * kSymChunks) + 1;
+    const long long Tp = (long long)a.n_blocks * kSymBlock;
+    bool fresh = true;
+    auto store_block = [&](int blk) {
+        const int row = k - cta_of_unit(sym_visit0(blk, nt) * kSymChunks, a.fine, G);
+#pragma unroll
+        for (int r = 0; r < R; ++r) a.part[(long long)row * Tp + (long long)blk * kSymBlock + r * kThreads + tid] = tot[r];
+    };
+
+    for (int it = 0; it < nvis; ++it) {
+        const int st = it & 1;
+        const bool last_of_block = J + 1 == nt;
+        if (tid == 0 && it + 1 < nvis) {
+            const int Jn = last_of_block ? (I + 1) * R : J + 1;
+            mbar_expect_tx(&full[st ^ 1], kTile * sizeof(Src4));
+            bulk_g2s(tile[st ^ 1], a.src + (long long)Jn * kTile, kTile * sizeof(Src4), &full[st ^ 1]);
+        }
+        if (fresh) {
+            fresh = false;
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const int tt = I * R + r;               // tile of these targets; beyond the last tile: phantom, q = 0
+                const Src4 t = a.src[(long long)min(tt, nt - 1) * kTile + tid];
+                ox[r] = t.x; oy[r] = t.y; oz[r] = t.z; oq[r] = tt < nt ? t.q : 0.0;
+                tot[r] = 0.0;
+            }
+        }
+        const int rd = J - I * R;                       // < R: the tile is one of the block's own
+        const bool diag = rd < R;
+        mbar_wait(&full[st], (it >> 1) & 1);
+        const Src4* __restrict__ s = tile[st];
+        const int ch_lo = it == 0 ? ch_first : 0;
+        const int ch_hi = it == nvis - 1 ? ch_last : kSymChunks;
+
+        for (int ch = ch_lo; ch < ch_hi; ++ch) {
+            const int j0 = ch * S;
+            double sx[S], sy[S], sz[S], sq[S], colp[S];
+#pragma unroll
+            for (int i = 0; i < S; ++i) {
+                const double2 xy = *reinterpret_cast<const double2*>(&s[j0 + i].x);
+                const double2 zq = *reinterpret_cast<const double2*>(&s[j0 + i].z);
+                sx[i] = xy.x; sy[i] = xy.y; sz[i] = zq.x; sq[i] = zq.y;
+                colp[i] = 0.0;
+            }
+#pragma unroll 1
+            for (int c = 0; c < a.C; ++c) {
+                const Cell cell = cells[c];
+                const double wc = cell.w * a.scale;
+                if (diag && cell.central) {
+                    // the block's own tile, bare terms: target (r = rd, tid) IS source j = tid; skip that pair
+#pragma unroll 1
+                    for (int i = 0; i < S; ++i) {   // (read from the tile again: no dynamic indexing of registers)
+                        const double2 xy = *reinterpret_cast<const double2*>(&s[j0 + i].x);
+                        const double2 zq = *reinterpret_cast<const double2*>(&s[j0 + i].z);
+                        const double wq = zq.y * wc;
+                        const bool mine = j0 + i == tid;
+#pragma unroll
+                        for (int r = 0; r < R; ++r) {
+                            const bool self = mine && r == rd;
+                            const double y = sym_recip<REFINE>(ox[r] - (self ? ox[r] + 1.0 : xy.x), oy[r] - xy.y, oz[r] - zq.x);
+                            tot[r] = fma(self ? 0.0 : wq, y, tot[r]);
+                        }
+                    }
+                } else {
+#pragma unroll
+                    for (int i = 0; i < S; ++i) {
+                        const double px = flip(sx[i], cell.fx) + cell.sx;
+                        const double py = flip(sy[i], cell.fy) + cell.sy;
+                        const double pz = flip(sz[i], cell.fz) + cell.sz;
+                        const double wq = sq[i] * wc;
+                        double cj = 0.0;
+#pragma unroll
+                        for (int r = 0; r < R; ++r) {
+                            const double y = sym_recip<REFINE>(ox[r] - px, oy[r] - py, oz[r] - pz);
+                            tot[r] = fma(wq, y, tot[r]);
+                            cj = fma(oq[r], y, cj);
+                        }
+                        colp[i] = fma(wc, cj, colp[i]);
+                    }
+                }
+            }
+            if (!diag) {
+#pragma unroll
+                for (int i = 0; i < S; ++i) {
+                    double v = colp[i];
+#pragma unroll
+                    for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+                    if (lane == 0) colw[warp][j0 + i] = v;
+                }
+            }
+        }
+        __syncthreads();  // tile[st] may be refilled; colw is complete
+        if (!diag) {
+            const int j = tid;  // kTile == kThreads
+            if (j >= ch_lo * S && j < ch_hi * S) {
+                double v = 0.0;
+#pragma unroll
+                for (int w = 0; w < kThreads / 32; ++w) v += colw[w][j];
+                a.col[(V0 + it) * kTile + j] = v;
+            }
+            __syncthreads();  // colw is rewritten by the next visit
+        }
+        if (last_of_block) {
+            store_block(I);
+            ++I; J = I * R; fresh = true;
+        } else {
+            ++J;
+        }
+    }
+    if (!fresh) store_block(I);
+}
+
+// phi of step (b) in the ORIGINAL source order: row sums (fixed CTA order) + column sums (blocks in order).
+__global__ void sym_gather_kernel(const double* __restrict__ part, const double* __restrict__ col,
+                                  const int* __restrict__ slot_of, long long N, long long n_tiles, int n_blocks,
+                                  long long fine, int G, double* __restrict__ out) {
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= N) return;
+    const long long p = slot_of[t];
+    const int I = (int)(p / kSymBlock), J = (int)(p / kTile), j = (int)(p % kTile);
+    const long long Tp = (long long)n_blocks * kSymBlock;
+    const int first = cta_of_unit(sym_visit0(I, n_tiles) * kSymChunks, fine, G);
+    const int last = cta_of_unit(sym_visit0(I + 1, n_tiles) * kSymChunks - 1, fine, G);
+    double v = 0.0;
+    for (int r = 0; r <= last - first; ++r) v += part[(long long)r * Tp + p];
+    for (int b = 0; b < I; ++b) v += col[(sym_visit0(b, n_tiles) + (J - b * kSymR)) * kTile + j];
+    out[t] = v;
+}
+
 struct NodeArgs {
     const double* tgt;
     int tstride;
