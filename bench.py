@@ -42,9 +42,30 @@ EXEC_PAIR = {(1, False): (10.0, 14.0), (2, False): (12.0, 18.0), (1, True): (9.0
 # algorithmic: the charge pair (18) + q y^3 (2 mul) + 3 fma = 26 flops
 EXEC_PAIR_FIELD = {(1, False): (16.0, 22.0), (2, False): (18.0, 26.0), (1, True): (15.0, 21.0), (2, True): (17.0, 25.0)}
 FLOPS_PAIR_CHARGE_FIELD = 26.0
+# Symmetric form of step (b) (near_sym_kernel; used when one rank evaluates all N targets): the unit of
+# the kernel is one pair EVALUATION (an unordered source pair in one image cell), which feeds two sums.  Algorithmic
+# flops per evaluation: the 18 of a charge pair + the second accumulation (1 DFMA) = 20.  Executed per evaluation
+# (FP64-pipe instructions, flops): pair 11 / 16 (Newton), 13 / 20 (cubic); + per 8 evaluations the image of the source
+# (3 DFMA), q*w (DMUL) and the column accumulation (DFMA).
+FLOPS_EVAL_SYM = 20.0
+EXEC_EVAL_SYM = {1: (11.0 + 5.0 / 8.0, 16.0 + 9.0 / 8.0), 2: (13.0 + 5.0 / 8.0, 20.0 + 9.0 / 8.0)}
+
+
+def sym_evaluations(N: int, C: int) -> int:
+    """Pair evaluations of one near_sym_kernel launch (csrc/sum_kernels.cuh: visits x tile x block x cells; the
+    diagonal visits and the padding of the last block are evaluated like the rest and counted here)."""
+    nt = -(-N // 256)
+    nb = -(-nt // 8)
+    visits = nb * nt - 8 * (nb * (nb - 1) // 2)
+    return visits * 256 * 2048 * C
+
+
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel from the committed ncu --set full
 # capture (profiles/r01_ncu_near_sum_N262144.md): valid for config 5 at N = 262,144 on one GPU, potential only
 NCU_TRAFFIC_BYTES_CFG5 = 9555200
+NCU_TRAFFIC_BYTES_CFG5_SYM = None   # near_sym_kernel: set from its own capture
+TRAFFIC_SOURCE_SYM = "profiles/r01_ncu_near_sym_N262144.md (dram read+write bytes of one launch)"
+TRAFFIC_SOURCE = "profiles/r01_ncu_near_sum_N262144.md (dram read+write bytes of one launch)"
 # FP64 peak derived from unit counts and clocks (DESIGN.md "Roofline"): SMs x 64 DFMA lanes x 2 x clock
 FP64_LANES_PER_SM = 64
 
@@ -232,6 +253,8 @@ def run_b200(args, w) -> dict:
         torch.cuda.synchronize()
 
     plan = H.Plan.from_workload(w, rsqrt_refine=args.refine)
+    if args.pair_form == "ordered":
+        plan.set_pair_form(1)
     info = plan.info
     refine = args.refine   # 0: resolved after the warm-up (the library decides by the pair count)
     xyz = torch.as_tensor(np.ascontiguousarray(w.xyz), device=dev)
@@ -347,24 +370,47 @@ def run_b200(args, w) -> dict:
     traffic = NCU_TRAFFIC_BYTES_CFG5 if (args.config == 5 and args.size is None and world == 1 and not args.forces
                                          and not args.paper_timing) else None
     issue_peak = sm_count * FP64_LANES_PER_SM * sm_max_mhz * 1e6          # FP64-pipe thread-instructions/s
-    roofline = {"bound": "alu", "kernel": f"near_sum_kernel<R,{refine},{'uniform-|q|' if uniform_q else 'generic'},{'field' if args.forces else 'potential'}> step (b)", "achieved": ach_tf, "peak": peak_tf,
+    symmetric = plan.last_pair_form == 2
+    traffic_source = TRAFFIC_SOURCE
+    if symmetric:
+        traffic = NCU_TRAFFIC_BYTES_CFG5_SYM if traffic else None
+        traffic_source = TRAFFIC_SOURCE_SYM
+        units = sym_evaluations(N, info["near_cells"])
+        alg_flops = FLOPS_EVAL_SYM
+        ex_instr, ex_flops = EXEC_EVAL_SYM[refine]
+        ach_tf = units * alg_flops / (k_ms * 1e-3) * 1e-12 if k_ms > 0 else 0.0
+        kernel_name = f"near_sym_kernel<{refine}> step (b), symmetric form: each unordered pair evaluated once"
+        unit_name = "pair evaluations (one unordered source pair in one image cell, feeding phi_i and phi_j)"
+    else:
+        units = pc_rank["b"]
+        kernel_name = (f"near_sum_kernel<R,{refine},{'uniform-|q|' if uniform_q else 'generic'},"
+                       f"{'field' if args.forces else 'potential'}> step (b)")
+        unit_name = "ordered pair interactions"
+    roofline = {"bound": "alu", "kernel": kernel_name, "achieved": ach_tf, "peak": peak_tf,
                 "unit": "TFLOP/s", "frac": ach_tf / peak_tf, "traffic": traffic,
-                "traffic_source": "profiles/r01_ncu_near_sum_N262144.md (dram read+write bytes of one launch)" if traffic else None,
+                "traffic_source": traffic_source if traffic else None,
                 "peak_source": f"derived: {sm_count} SMs x {FP64_LANES_PER_SM} FP64 lanes x 2 x {sm_max_mhz:.0f} MHz "
                                f"(no FP64 entry in MEASURED_PEAKS.json)",
-                "flops_per_pair_algorithmic": alg_flops, "pairs_per_launch": pc_rank["b"],
+                "units": unit_name, "units_per_launch": units, "flops_per_unit_algorithmic": alg_flops,
+                "pair_interactions_per_launch": pc_rank["b"],
                 "kernel_ms": k_ms, "kernel_pairs_per_s": pc_rank["b"] / (k_ms * 1e-3) if k_ms > 0 else 0.0,
                 "kernel_share_of_step": k_ms / stage_ms["total"] if stage_ms["total"] > 0 else None,
-                "flops_per_pair_executed": ex_flops, "fp64_instr_per_pair_executed": ex_instr,
-                "frac_executed_flops": pc_rank["b"] * ex_flops / (k_ms * 1e-3) * 1e-12 / peak_tf if k_ms > 0 else 0.0,
-                "fp64_pipe_issue_util": pc_rank["b"] * ex_instr / (k_ms * 1e-3) / issue_peak if k_ms > 0 else 0.0,
+                "flops_per_unit_executed": ex_flops, "fp64_instr_per_unit_executed": ex_instr,
+                "frac_executed_flops": units * ex_flops / (k_ms * 1e-3) * 1e-12 / peak_tf if k_ms > 0 else 0.0,
+                "fp64_pipe_issue_util": units * ex_instr / (k_ms * 1e-3) / issue_peak if k_ms > 0 else 0.0,
                 "dfma_microbench_tflops": dfma_tflops, "frac_of_dfma_microbench": ach_tf / dfma_tflops if dfma_tflops else None}
+    if symmetric:
+        # for comparison with the ordered-pair kernel only: the same time charged with 18 flops for every ordered pair
+        # interaction it accounts for.  It may exceed 1: the symmetry removes half of the work, it is not a roofline.
+        roofline["ordered_pair_equivalent_frac"] = pc_rank["b"] * FLOPS_PAIR_CHARGE / (k_ms * 1e-3) * 1e-12 / peak_tf if k_ms > 0 else 0.0
 
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": ms, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64",
            "data": "synthetic",
            "config": {"workload": w.name, "N": N, "near_cells": info["near_cells"], "p": info["p"], "M": info["M"],
                       "check_targets": info["check_targets"], "pairs_per_step": pc_all, "rsqrt_refine": refine, "forces": bool(args.forces),
+                      "pair_form": "symmetric (each unordered source pair evaluated once; value counts the ordered pair interactions it accounts for)"
+                                   if plan.last_pair_form == 2 else "ordered",
                       "parallelism": f"targets and check-point sums sharded over {world} rank(s), sources replicated"
                                      + ("" if world == 1 else "; stage_ms covers the second phase only (step (a) runs in its own call)"),
                       "l2": "256 MiB flush written between iterations"},
@@ -391,6 +437,9 @@ def main():
     ap.add_argument("--face-pairs", action="store_true",
                     help="periodic configs: close by seeded value+derivative pairs on opposite faces instead of the "
                          "paper's circumsphere rule (DESIGN.md 6.10)")
+    ap.add_argument("--pair-form", choices=["auto", "ordered"], default="auto",
+                    help="step (b): auto = symmetric form (each unordered pair once) when one rank evaluates all targets; "
+                         "ordered = always near_sum_kernel")
     ap.add_argument("--forces", action="store_true", help="time hsma_evaluate_forces (potential + forces) instead")
     ap.add_argument("--refine", type=int, default=0, choices=[0, 1, 2], help="hsma_plan_desc.rsqrt_refine")
     ap.add_argument("--e2e-steps", type=int, default=3)

@@ -387,7 +387,8 @@ template <int REFINE>
 __global__ void __launch_bounds__(kThreads, 1) near_sym_kernel(const SymArgs a) {
     __shared__ __align__(128) Src4 tile[kStages][kTile];
     __shared__ __align__(8) uint64_t full[kStages];
-    __shared__ Cell cells[kSymMaxCells];
+    struct SymCell { double sx, sy, sz, w, gx, gy, gz; int central, pad; };  // g = -1 on a reflected axis, else +1
+    __shared__ SymCell cells[kSymMaxCells];
     __shared__ double colw[kThreads / 32][kTile];
 
     constexpr int R = kSymR, S = kSymS;
@@ -401,7 +402,10 @@ __global__ void __launch_bounds__(kThreads, 1) near_sym_kernel(const SymArgs a) 
     while (sym_visit0(I + 1, nt) <= V0) ++I;
     int J = I * R + (int)(V0 - sym_visit0(I, nt));
 
-    for (int c = tid; c < a.C; c += kThreads) cells[c] = a.cells[c];
+    for (int c = tid; c < a.C; c += kThreads) {
+        const Cell g = a.cells[c];
+        cells[c] = SymCell{g.sx, g.sy, g.sz, g.w * a.scale, g.fx ? -1.0 : 1.0, g.fy ? -1.0 : 1.0, g.fz ? -1.0 : 1.0, g.central, 0};
+    }
     if (tid == 0) {
         for (int s = 0; s < kStages; ++s) mbar_init(&full[s], 1);
         mbar_fence_init();
@@ -460,8 +464,8 @@ __global__ void __launch_bounds__(kThreads, 1) near_sym_kernel(const SymArgs a) 
             }
 #pragma unroll 1
             for (int c = 0; c < a.C; ++c) {
-                const Cell cell = cells[c];
-                const double wc = cell.w * a.scale;
+                const SymCell cell = cells[c];
+                const double wc = cell.w;
                 if (diag && cell.central) {
                     // the block's own tile, bare terms: target (r = rd, tid) IS source j = tid; skip that pair
 #pragma unroll 1
@@ -480,9 +484,9 @@ __global__ void __launch_bounds__(kThreads, 1) near_sym_kernel(const SymArgs a) 
                 } else {
 #pragma unroll
                     for (int i = 0; i < S; ++i) {
-                        const double px = flip(sx[i], cell.fx) + cell.sx;
-                        const double py = flip(sy[i], cell.fy) + cell.sy;
-                        const double pz = flip(sz[i], cell.fz) + cell.sz;
+                        const double px = fma(cell.gx, sx[i], cell.sx);   // image = sign o r + shift (exact: g = +-1)
+                        const double py = fma(cell.gy, sy[i], cell.sy);
+                        const double pz = fma(cell.gz, sz[i], cell.sz);
                         const double wq = sq[i] * wc;
                         double cj = 0.0;
 #pragma unroll
