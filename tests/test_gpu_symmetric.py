@@ -1,0 +1,130 @@
+"""The symmetric form of step (b) (near_sym_kernel: each unordered source pair evaluated once,
+PAPER.md:64 Eq.(5) with the image cells of PAPER.md:40-50) against the CPU oracle and against the ordered-pair
+kernel, through the C-ABI.  Bars as in test_gpu_parity.  All `-m gpu`."""
+import numpy as np
+import pytest
+
+import hsma_workloads as W
+from oracle import hsma_oracle as O
+
+pytestmark = pytest.mark.gpu
+
+PHI_TOL = 1e-10
+U_TOL = 1e-11
+ORDERED, SYMMETRIC = 1, 2
+
+
+@pytest.fixture(scope="module")
+def H():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    import paper_1806_04801_b200 as H
+    H.binding.load_library()
+    return H
+
+
+def dev(a):
+    import torch
+    return torch.as_tensor(np.ascontiguousarray(a, dtype=np.float64), device="cuda")
+
+
+def rel_inf(a, b):
+    return float(np.max(np.abs(a - b)) / np.max(np.abs(b)))
+
+
+def both_forms(H, w, **plan_kw):
+    """(phi, U) of the automatic form and of the ordered form, and which form each evaluate used."""
+    with H.Plan.from_workload(w, **plan_kw) as plan:
+        xyz, q = dev(w.xyz), dev(w.q)
+        phi, U = plan.evaluate(xyz, q, sync=True)
+        form = plan.last_pair_form
+        plan.set_pair_form(ORDERED)
+        phi1, U1 = plan.evaluate(xyz, q, sync=True)
+        form1 = plan.last_pair_form
+    return phi.cpu().numpy(), float(U), form, phi1.cpu().numpy(), float(U1), form1
+
+
+# N: 7938 = 32 tiles with a two-source last tile (the smallest case the symmetric form takes); 9000 = 36 tiles, the
+# last block holds 4 tiles (phantom targets) and a ragged tile; 12288 = whole blocks only
+@pytest.mark.parametrize("refine", [1, 2])
+@pytest.mark.parametrize("idx,N", [(2, 7938), (2, 9000), (3, 9000), (4, 9000), (5, 12288)])
+def test_symmetric_form_matches_oracle(H, idx, N, refine):
+    """Periodic, mirror-cavity (reflected images, gamma = -1) and slab (reflected + weighted images, gamma = 0.5)
+    cell tables: every potential and U against the oracle; the ordered kernel agrees to rounding."""
+    w = W.config(idx, N=N)
+    r = O.hsma(w)
+    phi, U, form, phi1, U1, form1 = both_forms(H, w, rsqrt_refine=refine)
+    assert (form, form1) == (SYMMETRIC, ORDERED)
+    assert rel_inf(phi, r.phi) <= PHI_TOL and abs(U - r.U) <= U_TOL * abs(r.U)
+    assert rel_inf(phi1, r.phi) <= PHI_TOL and abs(U1 - r.U) <= U_TOL * abs(r.U)
+    assert rel_inf(phi, phi1) <= 2e-11
+
+
+@pytest.mark.parametrize("refine", [1, 2])
+def test_symmetric_form_random_magnitudes(H, refine):
+    """Charges of any magnitude and sign (the symmetric kernel always multiplies by q): slab table, ragged N."""
+    w = W.config(4, N=8209)
+    q = np.random.default_rng(77).standard_normal(w.N)
+    q -= q.mean()
+    w = w.with_(q=q)
+    r = O.hsma(w)
+    phi, U, form, phi1, U1, form1 = both_forms(H, w, rsqrt_refine=refine)
+    assert (form, form1) == (SYMMETRIC, ORDERED)
+    assert rel_inf(phi, r.phi) <= PHI_TOL and abs(U - r.U) <= U_TOL * abs(r.U)
+    assert rel_inf(phi, phi1) <= 2e-11
+
+
+def test_when_the_symmetric_form_applies(H):
+    """All N targets, potentials only, >= 32 source tiles: symmetric.  Shards, forces, small N: ordered.  The form
+    is not a property of the result: every variant agrees with the full evaluate."""
+    import torch
+    w = W.config(5, N=8192)
+    with H.Plan.from_workload(w) as plan:
+        xyz, q = dev(w.xyz), dev(w.q)
+        phi, U = plan.evaluate(xyz, q, sync=True)
+        assert plan.last_pair_form == SYMMETRIC
+        ref = phi.cpu().numpy()
+        a, _ = plan.evaluate_shard(xyz, q, 0, 5000, sync=True)
+        assert plan.last_pair_form == ORDERED
+        b, _ = plan.evaluate_shard(xyz, q, 5000, w.N, sync=True)
+        assert np.max(np.abs(np.concatenate([a.cpu().numpy(), b.cpu().numpy()]) - ref)) <= 2e-11 * np.max(np.abs(ref))
+        phi_f, F, U_f = plan.evaluate_forces(xyz, q, sync=True)
+        assert plan.last_pair_form == ORDERED
+        assert rel_inf(phi_f.cpu().numpy(), ref) <= 2e-11 and abs(float(U_f) - float(U)) <= 1e-11 * abs(float(U))
+        phi2, U2 = plan.evaluate(xyz, q, sync=True)
+        assert plan.last_pair_form == SYMMETRIC
+        assert torch.equal(phi2, phi) and float(U2) == float(U)     # deterministic: fixed summation order
+        with pytest.raises(Exception):
+            plan.set_pair_form(2)
+    w_small = W.config(5, N=7936)   # 31 tiles
+    with H.Plan.from_workload(w_small) as plan:
+        plan.evaluate(dev(w_small.xyz), dev(w_small.q), sync=True)
+        assert plan.last_pair_form == ORDERED
+
+
+def test_symmetric_form_in_a_replayed_graph(H):
+    """The whole-evaluate CUDA graph (captured on the second identical call on a side stream) holds the symmetric
+    launches; switching the form drops the graph."""
+    import torch
+    w = W.config(5, N=8192)
+    r = O.hsma(w)
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        with H.Plan.from_workload(w) as plan:
+            xyz, q = dev(w.xyz), dev(w.q)
+            phi = torch.empty(w.N, dtype=torch.float64, device="cuda")
+            U = torch.empty(1, dtype=torch.float64, device="cuda")
+            outs = []
+            for _ in range(4):
+                H.hsma_evaluate(plan.handle, xyz, q, phi, U)
+                plan.sync()
+                outs.append((phi.cpu().numpy().copy(), float(U)))
+            assert H.binding.hsma_plan_info(plan.handle)["graph_replays"] >= 1 and plan.last_pair_form == SYMMETRIC
+            for o in outs[1:]:
+                assert np.array_equal(o[0], outs[0][0]) and o[1] == outs[0][1]
+            assert rel_inf(outs[0][0], r.phi) <= PHI_TOL and abs(outs[0][1] - r.U) <= U_TOL * abs(r.U)
+            plan.set_pair_form(ORDERED)
+            H.hsma_evaluate(plan.handle, xyz, q, phi, U)
+            plan.sync()
+            assert plan.last_pair_form == ORDERED
+            assert rel_inf(phi.cpu().numpy(), r.phi) <= PHI_TOL
