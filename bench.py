@@ -63,7 +63,7 @@ def sym_evaluations(N: int, C: int) -> int:
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel from the committed ncu --set full
 # capture (profiles/r01_ncu_near_sum_N262144.md): valid for config 5 at N = 262,144 on one GPU, potential only
 NCU_TRAFFIC_BYTES_CFG5 = 9555200
-NCU_TRAFFIC_BYTES_CFG5_SYM = None   # near_sym_kernel: set from its own capture
+NCU_TRAFFIC_BYTES_CFG5_SYM = 118378496   # near_sym_kernel: 18,231,808 read + 100,146,688 written
 TRAFFIC_SOURCE_SYM = "profiles/r01_ncu_near_sym_N262144.md (dram read+write bytes of one launch)"
 TRAFFIC_SOURCE = "profiles/r01_ncu_near_sum_N262144.md (dram read+write bytes of one launch)"
 # FP64 peak derived from unit counts and clocks: SMs x 64 DFMA lanes x 2 x clock
