@@ -325,9 +325,19 @@ def run_b200(args, w) -> dict:
     xyz_n, q_n, phi_n, U_n = xyz_h.numpy(), q_h.numpy(), phi_h.numpy(), U_h.numpy()
     force_n = torch.empty(max(T, 1), 3, dtype=torch.float64).pin_memory().numpy() if args.forces else None
 
+    phi_all_h = torch.empty(N, dtype=torch.float64).pin_memory() if world > 1 else None
+
     def step_e2e():
         flush.zero_()
-        if args.forces and world == 1:
+        if world > 1:
+            # the distributed call a user makes (shard.evaluate_distributed), fed from pinned host memory
+            xyz.copy_(xyz_h, non_blocking=True)
+            q.copy_(q_h, non_blocking=True)
+            full, _, Uall = shard.evaluate_distributed(plan, xyz, q, forces=args.forces)
+            phi_all_h.copy_(full, non_blocking=True)
+            U_h.copy_(Uall, non_blocking=True)
+            torch.cuda.current_stream().synchronize()
+        elif args.forces:
             H.hsma_evaluate_forces_host(plan.handle, xyz_n, q_n, phi_n, force_n, U_n)
         else:
             H.hsma_evaluate_shard_host(plan.handle, xyz_n, q_n, t0, t1, phi_n, U_n)   # synchronises (returns host data)
@@ -345,9 +355,11 @@ def run_b200(args, w) -> dict:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         ms_e2e = float(t[0])
     e2e = {"value": pairs_step / (ms_e2e * 1e-3), "unit": UNIT, "ms_per_step": ms_e2e, "steps": n_e2e,
-           "h2d_bytes_per_step": int(xyz_n.nbytes + q_n.nbytes), "d2h_bytes_per_step": int(8 * T + 8 + (24 * T if args.forces and world == 1 else 0)),
-           "api": ("hsma_evaluate_forces_host" if args.forces and world == 1 else "hsma_evaluate_shard_host") +
-                  " (pinned host buffers; per rank: all sources in, its phi shard and U out)"}
+           "h2d_bytes_per_step": int(xyz_n.nbytes + q_n.nbytes),
+           "d2h_bytes_per_step": int(8 * N + 8) if world > 1 else int(8 * T + 8 + (24 * T if args.forces else 0)),
+           "api": ("shard.evaluate_distributed fed from pinned host buffers (per rank: all sources in, phi and U out)" if world > 1 else
+                   ("hsma_evaluate_forces_host" if args.forces else "hsma_evaluate_shard_host") +
+                   " (pinned host buffers: all sources in, phi and U out)")}
 
     # roofline of the dominant kernel: near_sum_kernel over the sources, step (b)
     pc_rank = pair_counts(info, N, T)
@@ -375,7 +387,7 @@ def run_b200(args, w) -> dict:
     if symmetric:
         traffic = NCU_TRAFFIC_BYTES_CFG5_SYM if traffic else None
         traffic_source = TRAFFIC_SOURCE_SYM
-        units = sym_evaluations(N, info["near_cells"])
+        units = sym_evaluations(N, info["near_cells"]) // world     # PART form: every rank 1/world of the fine units
         alg_flops = FLOPS_EVAL_SYM
         ex_instr, ex_flops = EXEC_EVAL_SYM[refine]
         ach_tf = units * alg_flops / (k_ms * 1e-3) * 1e-12 if k_ms > 0 else 0.0
@@ -411,7 +423,9 @@ def run_b200(args, w) -> dict:
                       "check_targets": info["check_targets"], "pairs_per_step": pc_all, "rsqrt_refine": refine, "forces": bool(args.forces),
                       "pair_form": "symmetric (each unordered source pair evaluated once; value counts the ordered pair interactions it accounts for)"
                                    if plan.last_pair_form == 2 else "ordered",
-                      "parallelism": f"targets and check-point sums sharded over {world} rank(s), sources replicated"
+                      "parallelism": (f"check-point sums, unordered pairs of (b) and targets of (c) split over {world} rank(s), "
+                                      f"sources replicated; all-reduce of phi and U" if world > 1 and plan.last_pair_form == 2 else
+                                      f"targets and check-point sums sharded over {world} rank(s), sources replicated")
                                      + ("" if world == 1 else "; stage_ms covers the second phase only (step (a) runs in its own call)"),
                       "l2": "256 MiB flush written between iterations"},
            "energy": U_val, "stage_ms": stage_ms, "e2e": e2e, "gpu_launches": int(launches),

@@ -174,7 +174,7 @@ static Launch choose_near(long long T, long long n_tiles, int C, int refine, boo
 // Symmetric form of step (b) (sum_kernels.cuh near_sym_kernel): launch shape and buffers.
 struct SymLaunch {
     int n_blocks, G, rows;
-    long long visits, fine;
+    long long visits, f_begin, fine;
 };
 static int sym_resident(int refine) {
     static int cache[2] = {0, 0};
@@ -182,16 +182,21 @@ static int sym_resident(int refine) {
     if (!c) c = refine == 1 ? resident_ctas(near_sym_kernel<1>) : resident_ctas(near_sym_kernel<2>);
     return c;
 }
-static SymLaunch choose_sym(long long n_tiles, int refine) {
+// part / n_parts: the contiguous share [F * part / n_parts, F * (part + 1) / n_parts) of the F fine units (multi-GPU)
+static SymLaunch choose_sym(long long n_tiles, int refine, int part = 0, int n_parts = 1) {
     SymLaunch L;
     L.n_blocks = (int)((n_tiles + kSymR - 1) / kSymR);
     L.visits = sym_visit0(L.n_blocks, n_tiles);
-    L.fine = L.visits * kSymChunks;
-    L.G = (int)std::min<long long>(sym_resident(refine), L.fine);
+    const long long F = L.visits * kSymChunks;
+    L.f_begin = F * part / n_parts;
+    L.fine = F * (part + 1) / n_parts - L.f_begin;
+    L.G = (int)std::max<long long>(1, std::min<long long>(sym_resident(refine), L.fine));
     L.rows = 1;
-    for (int I = 0; I < L.n_blocks; ++I) {
-        const int first = cta_of_unit(sym_visit0(I, n_tiles) * kSymChunks, L.fine, L.G);
-        const int last = cta_of_unit(sym_visit0(I + 1, n_tiles) * kSymChunks - 1, L.fine, L.G);
+    for (int I = 0; I < L.n_blocks && L.fine > 0; ++I) {
+        const long long lo = std::max(sym_visit0(I, n_tiles) * kSymChunks, L.f_begin);
+        const long long hi = std::min(sym_visit0(I + 1, n_tiles) * kSymChunks, L.f_begin + L.fine);
+        if (lo >= hi) continue;
+        const int first = cta_of_unit(lo - L.f_begin, L.fine, L.G), last = cta_of_unit(hi - 1 - L.f_begin, L.fine, L.G);
         L.rows = std::max(L.rows, last - first + 1);
     }
     return L;
@@ -553,9 +558,11 @@ __global__ void node_positions_kernel(const double* __restrict__ nrm, double R, 
 //   kPhaseCheck   H1 + step (a) for the check targets c0 <= i < c1 only, into the plan's pc (pcg); nothing else
 //   kPhaseRest    H1 + fit + mapping + (b) + (c) + finish with the plan's pc (pcg) AS THEY ARE (hsma_set_check_sums)
 enum { kPhaseAll = 0, kPhaseCheck = 1, kPhaseRest = 2 };
+// part / n_parts (kPhaseRest only, n_parts >= 1 given): the PART form of the multi-GPU path, DESIGN.md 8 -- step (b)
+// in symmetric form over this part's share of the fine units, phi_out [N] = that share + step (c) for t0 <= t < t1.
 static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* q, long long N, long long t0,
                                  long long t1, double* phi_out, double* energy_out, double* force_out = nullptr,
-                                 int phase = kPhaseAll, long long c0 = 0, long long c1 = -1) {
+                                 int phase = kPhaseAll, long long c0 = 0, long long c1 = -1, int part = 0, int n_parts = 0) {
     if (!p || !xyz || !q || N < 1 || t0 < 0 || t1 > N || t0 > t1 ||
         (phase != kPhaseCheck && !phi_out && !force_out && t1 > t0))
         return HSMA_ERR_INVALID_ARG;
@@ -575,7 +582,7 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
     if (p->src.reserve((size_t)Npad) != cudaSuccess || p->slot_of.reserve((size_t)N) != cudaSuccess ||
         p->tile_np.reserve((size_t)n_tiles) != cudaSuccess)
         return HSMA_ERR_ALLOC;
-    if (p->red.reserve((size_t)std::max(4 * n_tiles, (t1 - t0 + 255) / 256 + 1)) != cudaSuccess) return HSMA_ERR_ALLOC;
+    if (p->red.reserve((size_t)std::max(4 * n_tiles, (N + 255) / 256 + 1)) != cudaSuccess) return HSMA_ERR_ALLOC;
     pack_sources_kernel<<<(unsigned)n_tiles, kTile, 0, st>>>(xyz, q, N, p->half[0], p->half[1], p->half[2], p->src.p,
                                                            p->slot_of.p, p->tile_np.p, p->red.p);
     charge_stats_kernel<<<1, 1024, 0, st>>>(p->red.p, n_tiles, p->need_neutral ? 1 : 0, p->scalars + 2, p->qinfo, p->flags);
@@ -653,7 +660,46 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
     HSMA_COUNT_LAUNCH();
 
     const long long T = t1 - t0;
-    if (T > 0) {
+    if (n_parts > 0) {
+        // PART form (multi-GPU): this part's share of the unordered pairs of (b) for ALL targets, (c) for
+        // the targets t0..t1-1; phi_out [N] and U add up over the parts
+        if (field || p->sphere || !sym_applies(n_tiles, C_b) || part < 0 || part >= n_parts || !phi_out) return HSMA_ERR_INVALID_ARG;
+        const int refine = p->refine ? p->refine : ((double)N * (double)p->last_images < 4294967296.0 ? 2 : 1);
+        const SymLaunch ss = choose_sym(n_tiles, refine, part, n_parts);
+        if (p->part_b.reserve((size_t)ss.rows * ss.n_blocks * kSymBlock) != cudaSuccess ||
+            p->sym_col.reserve((size_t)ss.visits * kTile) != cudaSuccess || p->sym_phi.reserve((size_t)N) != cudaSuccess)
+            return HSMA_ERR_ALLOC;
+        Launch sc{};
+        if (T > 0) {
+            sc = choose_node(T, p->node_tiles, false);
+            if (p->part_c.reserve((size_t)sc.rows * T) != cudaSuccess) return HSMA_ERR_ALLOC;
+        }
+        p->last_pair_form = 2;
+        MARK(3);
+        SymArgs a;
+        a.src = p->src.p; a.n_src = N; a.n_tiles = n_tiles; a.n_blocks = ss.n_blocks; a.cells = cells_b; a.C = C_b;
+        a.f_begin = ss.f_begin; a.fine = ss.fine; a.scale = refine == 1 ? 0.5 : 1.0; a.part = p->part_b.p; a.col = p->sym_col.p;
+        if (ss.fine > 0) {
+            if (refine == 1) near_sym_kernel<1><<<ss.G, kThreads, 0, st>>>(a);
+            else near_sym_kernel<2><<<ss.G, kThreads, 0, st>>>(a);
+            HSMA_COUNT_LAUNCH();
+        }
+        sym_gather_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(p->part_b.p, p->sym_col.p, p->slot_of.p, N, n_tiles,
+                                                                      ss.n_blocks, ss.f_begin, ss.fine, ss.G, p->sym_phi.p);
+        HSMA_COUNT_LAUNCH();
+        MARK(4);
+        if (T > 0)
+            launch_node(sc, false, reinterpret_cast<const double*>(p->src.p), 4, p->slot_of.p, T, t0, p->nodes, p->node_tiles, p->part_c.p, st);
+        MARK(5);
+        const long long fb = (N + 255) / 256;
+        finish_part_kernel<<<(unsigned)fb, 256, 0, st>>>(p->sym_phi.p, T > 0 ? sc.layout(p->part_c.p) : PartLayout{nullptr, 1, 1, 1, 1}, N, t0, t1,
+                                                         p->src.p, p->slot_of.p, phi_out, energy_out ? p->red.p : nullptr);
+        HSMA_COUNT_LAUNCH();
+        if (energy_out) {
+            reduce_rows_kernel<<<1, 1024, 0, st>>>(p->red.p, fb, 1, 1, 0.5, energy_out);
+            HSMA_COUNT_LAUNCH();
+        }
+    } else if (T > 0) {
         // H5 (b): near images at the sources, self excluded
         const int refine = p->refine ? p->refine : ((double)N * (double)p->last_images < 4294967296.0 ? 2 : 1);
         // rsqrt_refine = 0: the cubic step while (b) is latency-bound anyway (< 2^32 pairs), Newton above
@@ -678,12 +724,15 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
             // every unordered (source, source) pair once: row sums + column sums, then phi_near in source order
             SymArgs a;
             a.src = p->src.p; a.n_src = N; a.n_tiles = n_tiles; a.n_blocks = ss.n_blocks; a.cells = cells_b; a.C = C_b;
-            a.fine = ss.fine; a.scale = refine == 1 ? 0.5 : 1.0; a.part = p->part_b.p; a.col = p->sym_col.p;
-            if (refine == 1) near_sym_kernel<1><<<ss.G, kThreads, 0, st>>>(a);
-            else near_sym_kernel<2><<<ss.G, kThreads, 0, st>>>(a);
+            a.f_begin = ss.f_begin; a.fine = ss.fine; a.scale = refine == 1 ? 0.5 : 1.0; a.part = p->part_b.p; a.col = p->sym_col.p;
+            if (ss.fine > 0) {
+                if (refine == 1) near_sym_kernel<1><<<ss.G, kThreads, 0, st>>>(a);
+                else near_sym_kernel<2><<<ss.G, kThreads, 0, st>>>(a);
+                HSMA_COUNT_LAUNCH();
+            }
             sym_gather_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(p->part_b.p, p->sym_col.p, p->slot_of.p, N, n_tiles,
-                                                                          ss.n_blocks, ss.fine, ss.G, p->sym_phi.p);
-            HSMA_COUNT_LAUNCH(); HSMA_COUNT_LAUNCH();
+                                                                          ss.n_blocks, ss.f_begin, ss.fine, ss.G, p->sym_phi.p);
+            HSMA_COUNT_LAUNCH();
             layout_b = PartLayout{p->sym_phi.p, 1, 1, 1, (int)std::min<long long>(T, 2147483647LL)};
         } else {
             launch_near(sb, field, reinterpret_cast<const double*>(p->src.p), 4, p->slot_of.p, T, t0, P, cells_b, C_b,
@@ -821,6 +870,17 @@ extern "C" hsma_status hsma_evaluate_rest_shard(hsma_plan* plan, const double* x
                                                 long long t0, long long t1, double* phi_out, double* force_out,
                                                 double* energy_out) {
     return evaluate_impl(plan, xyz, q, N, t0, t1, phi_out, energy_out, force_out, kPhaseRest);
+}
+
+extern "C" hsma_status hsma_evaluate_rest_part(hsma_plan* plan, const double* xyz, const double* q, long long N, int part,
+                                               int n_parts, long long t0, long long t1, double* phi_part_out,
+                                               double* energy_part_out) {
+    if (n_parts < 1) return HSMA_ERR_INVALID_ARG;
+    return evaluate_impl(plan, xyz, q, N, t0, t1, phi_part_out, energy_part_out, nullptr, kPhaseRest, 0, -1, part, n_parts);
+}
+extern "C" int hsma_plan_part_form_applies(const hsma_plan* p, long long N) {
+    if (!p || N < 1) return 0;
+    return !p->sphere && sym_applies((N + kTile - 1) / kTile, p->C_near) ? 1 : 0;
 }
 
 extern "C" hsma_status hsma_plan_sync(hsma_plan* plan) {

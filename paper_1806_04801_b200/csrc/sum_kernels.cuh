@@ -361,7 +361,8 @@ struct SymArgs {
     int n_blocks;        // ceil(n_tiles / kSymR)
     const Cell* cells;
     int C;
-    long long fine;      // F = sym_visit0(n_blocks) * kSymChunks
+    long long f_begin;   // this launch walks the fine units [f_begin, f_begin + fine) of the F = sym_visit0(n_blocks) *
+    long long fine;      // kSymChunks in all (one rank: everything; R ranks: a contiguous 1/R each)
     double scale;        // 0.5 for the Newton form (y is twice the reciprocal distance)
     double* part;        // [rows][n_blocks * kSymBlock]
     double* col;         // [visits][kTile]
@@ -394,7 +395,7 @@ __global__ void __launch_bounds__(kThreads, 1) near_sym_kernel(const SymArgs a) 
     constexpr int R = kSymR, S = kSymS;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int G = gridDim.x, k = blockIdx.x;
-    const long long f0 = unit_start(k, a.fine, G), f1 = unit_start(k + 1, a.fine, G);
+    const long long f0 = a.f_begin + unit_start(k, a.fine, G), f1 = a.f_begin + unit_start(k + 1, a.fine, G);
     if (f1 <= f0) return;
     const long long V0 = f0 / kSymChunks, V1 = (f1 - 1) / kSymChunks;
     const int nt = (int)a.n_tiles;
@@ -422,7 +423,7 @@ __global__ void __launch_bounds__(kThreads, 1) near_sym_kernel(const SymArgs a) 
     const long long Tp = (long long)a.n_blocks * kSymBlock;
     bool fresh = true;
     auto store_block = [&](int blk) {
-        const int row = k - cta_of_unit(sym_visit0(blk, nt) * kSymChunks, a.fine, G);
+        const int row = k - cta_of_unit(max(sym_visit0(blk, nt) * kSymChunks, a.f_begin) - a.f_begin, a.fine, G);
 #pragma unroll
         for (int r = 0; r < R; ++r) a.part[(long long)row * Tp + (long long)blk * kSymBlock + r * kThreads + tid] = tot[r];
     };
@@ -530,20 +531,28 @@ __global__ void __launch_bounds__(kThreads, 1) near_sym_kernel(const SymArgs a) 
     if (!fresh) store_block(I);
 }
 
-// phi of step (b) in the ORIGINAL source order: row sums (fixed CTA order) + column sums (blocks in order).
+// phi of step (b) in the ORIGINAL source order: row sums (fixed CTA order) + column sums (blocks in order), of the
+// fine units [f_begin, f_begin + fine) that the launch walked (all of them on one rank: the whole near sum).
 __global__ void sym_gather_kernel(const double* __restrict__ part, const double* __restrict__ col,
                                   const int* __restrict__ slot_of, long long N, long long n_tiles, int n_blocks,
-                                  long long fine, int G, double* __restrict__ out) {
+                                  long long f_begin, long long fine, int G, double* __restrict__ out) {
     const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= N) return;
     const long long p = slot_of[t];
     const int I = (int)(p / kSymBlock), J = (int)(p / kTile), j = (int)(p % kTile);
     const long long Tp = (long long)n_blocks * kSymBlock;
-    const int first = cta_of_unit(sym_visit0(I, n_tiles) * kSymChunks, fine, G);
-    const int last = cta_of_unit(sym_visit0(I + 1, n_tiles) * kSymChunks - 1, fine, G);
+    const long long f_end = f_begin + fine;
     double v = 0.0;
-    for (int r = 0; r <= last - first; ++r) v += part[(long long)r * Tp + p];
-    for (int b = 0; b < I; ++b) v += col[(sym_visit0(b, n_tiles) + (J - b * kSymR)) * kTile + j];
+    const long long lo = max(sym_visit0(I, n_tiles) * kSymChunks, f_begin), hi = min(sym_visit0(I + 1, n_tiles) * kSymChunks, f_end);
+    if (lo < hi) {
+        const int first = cta_of_unit(lo - f_begin, fine, G), last = cta_of_unit(hi - 1 - f_begin, fine, G);
+        for (int r = 0; r <= last - first; ++r) v += part[(long long)r * Tp + p];
+    }
+    for (int b = 0; b < I; ++b) {
+        const long long vis = sym_visit0(b, n_tiles) + (J - b * kSymR);
+        const long long f = vis * kSymChunks + j / kSymS;
+        if (f >= f_begin && f < f_end) v += col[vis * kTile + j];
+    }
     out[t] = v;
 }
 
@@ -874,6 +883,34 @@ __global__ void finish_phi_kernel(const PartLayout Lb, const PartLayout Lc, long
         const double v = sum_part_rows(Lb, t, T) + sum_part_rows(Lc, t, T);
         phi[t] = v;
         if (src) e = src[slot_of[t_first + t]].q * v;
+    }
+    if (u_part) {
+        __shared__ double sh[32];
+        for (int o = 16; o; o >>= 1) e += __shfl_down_sync(0xffffffffu, e, o);
+        const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+        if (l == 0) sh[w] = e;
+        __syncthreads();
+        if (w == 0) {
+            const int nw = blockDim.x >> 5;
+            e = l < nw ? sh[l] : 0.0;
+            for (int o = 16; o; o >>= 1) e += __shfl_down_sync(0xffffffffu, e, o);
+            if (l == 0) u_part[blockIdx.x] = e;
+        }
+    }
+}
+
+// H7 for a part of the pair work (multi-GPU): phi_part[t] over ALL N targets = this part's share of the
+// near sum + the node sum for the targets t0 <= t < t1 only; U_part = 1/2 sum q phi_part.  Both add up over the parts.
+__global__ void finish_part_kernel(const double* __restrict__ near, const PartLayout Lc, long long N, long long t0,
+                                   long long t1, const Src4* __restrict__ src, const int* __restrict__ slot_of,
+                                   double* __restrict__ phi, double* __restrict__ u_part) {
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    double e = 0.0;
+    if (t < N) {
+        double v = near[t];
+        if (t >= t0 && t < t1) v += sum_part_rows(Lc, t - t0, t1 - t0);
+        phi[t] = v;
+        e = src[slot_of[t]].q * v;
     }
     if (u_part) {
         __shared__ double sh[32];

@@ -47,6 +47,13 @@ def all_reduce_energy(U_local: torch.Tensor, group=None) -> torch.Tensor:
     return U_local
 
 
+def all_reduce_phi(phi_part: torch.Tensor, group=None) -> torch.Tensor:
+    """phi = sum over ranks of the partial potentials of the PART form (in place; [N] doubles, 2 MB at N = 262,144)."""
+    if dist.is_initialized() and dist.get_world_size(group) > 1:
+        dist.all_reduce(phi_part, op=dist.ReduceOp.SUM, group=group)
+    return phi_part
+
+
 def all_gather_slices(local: torch.Tensor, total: int, group=None) -> torch.Tensor:
     """Concatenate per-rank slices along dim 0 (rank r owns shard_bounds(total, world, align=1)[r]); slices are
     padded to a common length for the equal-size all_gather."""
@@ -69,6 +76,9 @@ def evaluate_distributed(plan, xyz: torch.Tensor, q: torch.Tensor, forces: bool 
       2. all-gather of the K_t check sums (one small message)       the only data-path collective before the fit
       3. fit, mapping and steps (b), (c) for this rank's targets    hsma_evaluate_rest_shard
       4. all-gather of phi (and F), all-reduce of U                 assembly of the result
+    or, when the symmetric form of step (b) applies (potentials only, DESIGN.md 6.12 / 8):
+      3'. fit, mapping, this rank's share of the UNORDERED pairs of (b), (c) for its targets    hsma_evaluate_rest_part
+      4'. all-reduce of the partial phi [N] and of the partial U
     Returns (phi [N], F [N,3] or None, U [1]) on every rank.  `plan` is a paper_1806_04801_b200.Plan."""
     from . import binding
     N = q.numel()
@@ -86,6 +96,15 @@ def evaluate_distributed(plan, xyz: torch.Tensor, q: torch.Tensor, forces: bool 
         pc_all = all_gather_slices(pc, Kt, group)
         pcg_all = all_gather_slices(pcg, Kt, group) if need_grad else None
         binding.hsma_set_check_sums(plan.handle, 0, Kt, pc_all.contiguous(), pcg_all.contiguous() if need_grad else None)
+    if not forces and binding.hsma_plan_part_form_applies(plan.handle, N):
+        # PART form: this rank's share of the unordered pairs of (b) for all targets + (c) for its own targets;
+        # phi and U are sums over the ranks (one all-reduce each)
+        phi_part = torch.empty(N, dtype=torch.float64, device=q.device)
+        U = torch.empty(1, dtype=torch.float64, device=q.device)
+        binding.hsma_evaluate_rest_part(plan.handle, xyz, q, rank, world, t0, t1, phi_part, U)
+        all_reduce_phi(phi_part, group)
+        all_reduce_energy(U, group)
+        return phi_part, None, U
     T = t1 - t0
     phi = torch.empty(T, dtype=torch.float64, device=q.device)
     F = torch.empty(T, 3, dtype=torch.float64, device=q.device) if forces else None

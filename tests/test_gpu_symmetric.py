@@ -128,3 +128,55 @@ def test_symmetric_form_in_a_replayed_graph(H):
             plan.sync()
             assert plan.last_pair_form == ORDERED
             assert rel_inf(phi.cpu().numpy(), r.phi) <= PHI_TOL
+
+
+@pytest.mark.parametrize("idx,N", [(5, 8192), (4, 9000), (3, 8200)])
+@pytest.mark.parametrize("n_parts", [1, 2, 3, 7])
+def test_part_form_adds_up_to_the_evaluate(H, idx, N, n_parts):
+    """Multi-GPU PART form with the "ranks" run one after the other on one device: the partial
+    potentials and energies of the parts add up to the one-rank result, for every part count."""
+    import torch
+    from paper_1806_04801_b200 import shard
+    w = W.config(idx, N=N)
+    r = O.hsma(w)
+    with H.Plan.from_workload(w) as plan:
+        xyz, q = dev(w.xyz), dev(w.q)
+        assert H.binding.hsma_plan_part_form_applies(plan.handle, w.N)
+        phi_ref, U_ref = plan.evaluate(xyz, q, sync=True)
+        Kt = plan.info["check_targets"]
+        H.binding.hsma_check_sums_shard(plan.handle, xyz, q, 0, Kt)
+        phi = torch.zeros(w.N, dtype=torch.float64, device="cuda")
+        U = torch.zeros(1, dtype=torch.float64, device="cuda")
+        for part, (t0, t1) in enumerate(shard.shard_bounds(w.N, n_parts)):
+            pp = torch.empty(w.N, dtype=torch.float64, device="cuda")
+            up = torch.empty(1, dtype=torch.float64, device="cuda")
+            H.binding.hsma_evaluate_rest_part(plan.handle, xyz, q, part, n_parts, t0, t1, pp, up)
+            plan.sync()
+            phi += pp
+            U += up
+        assert rel_inf(phi.cpu().numpy(), phi_ref.cpu().numpy()) <= 1e-12
+        assert abs(float(U) - float(U_ref)) <= 1e-12 * abs(float(U_ref))
+        assert rel_inf(phi.cpu().numpy(), r.phi) <= PHI_TOL and abs(float(U) - r.U) <= U_TOL * abs(r.U)
+        # bad part index, forces of a part: refused
+        with pytest.raises(Exception):
+            H.binding.hsma_evaluate_rest_part(plan.handle, xyz, q, n_parts, n_parts, 0, w.N, phi, U)
+
+
+def test_evaluate_distributed_single_process_uses_the_part_form(H):
+    """shard.evaluate_distributed without a process group (world = 1): part 0 of 1 = the whole evaluate."""
+    from paper_1806_04801_b200 import shard
+    w = W.config(5, N=8192)
+    with H.Plan.from_workload(w) as plan:
+        xyz, q = dev(w.xyz), dev(w.q)
+        phi_ref, U_ref = plan.evaluate(xyz, q, sync=True)
+        phi, F, U = shard.evaluate_distributed(plan, xyz, q)
+        plan.sync()
+        assert F is None and plan.last_pair_form == SYMMETRIC
+        assert rel_inf(phi.cpu().numpy(), phi_ref.cpu().numpy()) <= 1e-13 and abs(float(U) - float(U_ref)) <= 1e-13 * abs(float(U_ref))
+        # small systems keep the target-shard path
+        ws = W.config(2)
+        with H.Plan.from_workload(ws) as plan_s:
+            assert not H.binding.hsma_plan_part_form_applies(plan_s.handle, ws.N)
+            ps, _, Us = shard.evaluate_distributed(plan_s, dev(ws.xyz), dev(ws.q))
+            pr, Ur = plan_s.evaluate(dev(ws.xyz), dev(ws.q), sync=True)
+            assert rel_inf(ps.cpu().numpy(), pr.cpu().numpy()) <= 1e-13

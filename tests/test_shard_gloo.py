@@ -85,8 +85,50 @@ def test_all_gather_slices_reassembles_in_order(tmp_path, total):
         assert np.array_equal(np.load(tmp_path / f"m{r}.npy"), np.stack([want, 2 * want, -want], axis=1))
 
 
+def _parts_worker(rank, world, port, N, out_dir):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        import hsma_workloads as W
+        from oracle import hsma_oracle as O
+        w = W.config(2, N=N)
+        cells = O.cell_table(w.kind, w.L, w.near_shell, w.gamma)
+        # stand-in for hsma_evaluate_rest_part: a share of the PAIR work for ALL targets (here: the sources a..b-1;
+        # the self term is left out where the targets are those sources)
+        a, b = shard.shard_bounds(N, world, align=1)[rank]
+        phi_part = np.empty(N)
+        phi_part[a:b] = O.near_sum(w.xyz[a:b], w.xyz[a:b], w.q[a:b], cells, self_offset=0)
+        rest = np.r_[0:a, b:N]
+        phi_part[rest] = O.near_sum(w.xyz[rest], w.xyz[a:b], w.q[a:b], cells)
+        U_part = 0.5 * float(np.dot(w.q, phi_part))
+        phi = shard.all_reduce_phi(torch.from_numpy(phi_part))
+        U = shard.all_reduce_energy(torch.tensor([U_part], dtype=torch.float64))
+        np.save(os.path.join(out_dir, f"p{rank}.npy"), phi.numpy())
+        np.save(os.path.join(out_dir, f"u{rank}.npy"), U.numpy())
+    finally:
+        dist.destroy_process_group()
+
+
+def test_part_form_all_reduce_assembles_the_near_sum(tmp_path):
+    """PART form of the multi-GPU path (DESIGN.md 8): every rank computes a share of the pair work for all targets;
+    one all-reduce of the partial potentials (and of the partial energies) leaves the full sums on every rank."""
+    import hsma_workloads as W
+    from oracle import hsma_oracle as O
+    N, world, port = 601, 2, 33500 + os.getpid() % 2000
+    mp.spawn(_parts_worker, args=(world, port, N, str(tmp_path)), nprocs=world, join=True)
+    w = W.config(2, N=N)
+    cells = O.cell_table(w.kind, w.L, w.near_shell, w.gamma)
+    want = O.near_sum(w.xyz, w.xyz, w.q, cells, self_offset=0)
+    p0, p1 = np.load(tmp_path / "p0.npy"), np.load(tmp_path / "p1.npy")
+    assert np.array_equal(p0, p1)                                   # the all-reduce gives every rank the same bits
+    assert np.max(np.abs(p0 - want)) <= 1e-13 * np.max(np.abs(want))  # = the unsplit sum up to the order of addition
+    u0, u1 = float(np.load(tmp_path / "u0.npy")[0]), float(np.load(tmp_path / "u1.npy")[0])
+    assert u0 == u1 and abs(u0 - 0.5 * float(np.dot(w.q, want))) <= 1e-12 * abs(u0)
+
+
 def test_single_process_is_a_no_op():
     x = torch.arange(5, dtype=torch.float64)
     assert shard.all_gather_phi(x, 5) is x
     u = torch.tensor([1.5], dtype=torch.float64)
     assert shard.all_reduce_energy(u) is u
+    assert shard.all_reduce_phi(x) is x
