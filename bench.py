@@ -49,6 +49,10 @@ FLOPS_PAIR_CHARGE_FIELD = 26.0
 # (3 DFMA), q*w (DMUL) and the column accumulation (DFMA).
 FLOPS_EVAL_SYM = 20.0
 EXEC_EVAL_SYM = {1: (11.0 + 5.0 / 8.0, 16.0 + 9.0 / 8.0), 2: (13.0 + 5.0 / 8.0, 20.0 + 9.0 / 8.0)}
+# the same with the gradient (near_sym_field_kernel): algorithmic = the 26 of a potential+gradient pair + the column side
+# (DFMA + DMUL + 3 DFMA = 9); executed: pair 21 / 33 (Newton), 23 / 37 (cubic) + per 8 evaluations 11 instructions / 18 flops
+FLOPS_EVAL_SYM_FIELD = 35.0
+EXEC_EVAL_SYM_FIELD = {1: (21.0 + 11.0 / 8.0, 33.0 + 18.0 / 8.0), 2: (23.0 + 11.0 / 8.0, 37.0 + 18.0 / 8.0)}
 
 
 def sym_evaluations(N: int, C: int) -> int:
@@ -253,8 +257,8 @@ def run_b200(args, w) -> dict:
         torch.cuda.synchronize()
 
     plan = H.Plan.from_workload(w, rsqrt_refine=args.refine)
-    if args.pair_form == "ordered":
-        plan.set_pair_form(1)
+    if args.pair_form != "auto":
+        plan.set_pair_form(1 if args.pair_form == "ordered" else 2)
     info = plan.info
     refine = args.refine   # 0: resolved after the warm-up (the library decides by the pair count)
     xyz = torch.as_tensor(np.ascontiguousarray(w.xyz), device=dev)
@@ -388,10 +392,11 @@ def run_b200(args, w) -> dict:
         traffic = NCU_TRAFFIC_BYTES_CFG5_SYM if traffic else None
         traffic_source = TRAFFIC_SOURCE_SYM
         units = sym_evaluations(N, info["near_cells"]) // world     # PART form: every rank 1/world of the fine units
-        alg_flops = FLOPS_EVAL_SYM
-        ex_instr, ex_flops = EXEC_EVAL_SYM[refine]
+        alg_flops = FLOPS_EVAL_SYM_FIELD if args.forces else FLOPS_EVAL_SYM
+        ex_instr, ex_flops = (EXEC_EVAL_SYM_FIELD if args.forces else EXEC_EVAL_SYM)[refine]
         ach_tf = units * alg_flops / (k_ms * 1e-3) * 1e-12 if k_ms > 0 else 0.0
-        kernel_name = f"near_sym_kernel<{refine}> step (b), symmetric form: each unordered pair evaluated once"
+        kernel_name = (f"near_sym_field_kernel<{refine}>" if args.forces else f"near_sym_kernel<{refine}>") + \
+            " step (b), symmetric form: each unordered pair evaluated once"
         unit_name = "pair evaluations (one unordered source pair in one image cell, feeding phi_i and phi_j)"
     else:
         units = pc_rank["b"]
@@ -414,7 +419,7 @@ def run_b200(args, w) -> dict:
     if symmetric:
         # for comparison with the ordered-pair kernel only: the same time charged with 18 flops for every ordered pair
         # interaction it accounts for.  It may exceed 1: the symmetry removes half of the work, it is not a roofline.
-        roofline["ordered_pair_equivalent_frac"] = pc_rank["b"] * FLOPS_PAIR_CHARGE / (k_ms * 1e-3) * 1e-12 / peak_tf if k_ms > 0 else 0.0
+        roofline["ordered_pair_equivalent_frac"] = pc_rank["b"] * (FLOPS_PAIR_CHARGE_FIELD if args.forces else FLOPS_PAIR_CHARGE) / (k_ms * 1e-3) * 1e-12 / peak_tf if k_ms > 0 else 0.0
 
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": ms, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64",
@@ -451,9 +456,9 @@ def main():
     ap.add_argument("--face-pairs", action="store_true",
                     help="periodic configs: close by seeded value+derivative pairs on opposite faces instead of the "
                          "paper's circumsphere rule (DESIGN.md 6.10)")
-    ap.add_argument("--pair-form", choices=["auto", "ordered"], default="auto",
-                    help="step (b): auto = symmetric form (each unordered pair once) when one rank evaluates all targets; "
-                         "ordered = always near_sum_kernel")
+    ap.add_argument("--pair-form", choices=["auto", "ordered", "symmetric"], default="auto",
+                    help="step (b): auto = symmetric form (each unordered pair once) when one rank evaluates all targets "
+                         "(forces: from N > 65,280); ordered = always near_sum_kernel; symmetric = wherever it applies")
     ap.add_argument("--forces", action="store_true", help="time hsma_evaluate_forces (potential + forces) instead")
     ap.add_argument("--refine", type=int, default=0, choices=[0, 1, 2], help="hsma_plan_desc.rsqrt_refine")
     ap.add_argument("--e2e-steps", type=int, default=3)

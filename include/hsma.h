@@ -262,13 +262,16 @@ hsma_status hsma_plan_set_timing(hsma_plan* plan, int enable);
 hsma_status hsma_plan_get_timing(hsma_plan* plan, double* ms_out);
 
 /*
- * Form of step (b).  When an evaluate covers all N targets (t0 = 0, t1 = N, potentials only,
- * whole-cell near set, N > 7936, at most 128 near cells) the targets are the sources and the image sum is
- * symmetric (every image cell has a partner of equal weight), so each unordered pair is
- * evaluated once and feeds both phi_i and phi_j ("symmetric" form, near_sym_kernel).  form = 0: choose
- * automatically (default); form = 1: always the ordered-pair kernel (near_sum_kernel), e.g. to compare the two.
- * Shards (t0 > 0 or t1 < N), forces and the sphere-culled near set always use the ordered form.
- * hsma_plan_last_pair_form: what the last evaluate used for step (b): 1 ordered, 2 symmetric (0: null plan).
+ * Form of step (b).  When an evaluate covers all N targets (t0 = 0, t1 = N; whole-cell near set, at
+ * least 32 source tiles = N > 7936, at most 128 near cells) the targets are the sources and the image sum is
+ * symmetric (every image cell has a partner of equal weight), so each unordered pair can be
+ * evaluated once and feed both phi_i and phi_j (and both gradients): the "symmetric" form, near_sym_kernel /
+ * near_sym_field_kernel.  form = 0 (default): automatic -- potentials take it whenever it applies, forces from 256
+ * source tiles on (N > 65,280; below that the ordered gradient kernel is as fast); form = 1: always the ordered-pair
+ * kernel (near_sum_kernel), e.g. to compare the two; form = 2: the symmetric form wherever it applies, forces included.
+ * Shards (t0 > 0 or t1 < N) and the sphere-culled near set always use the ordered form.  Other values:
+ * HSMA_ERR_INVALID_ARG.  hsma_plan_last_pair_form: what the last evaluate used for step (b): 1 ordered, 2 symmetric
+ * (0: null plan).
  */
 hsma_status hsma_plan_set_pair_form(hsma_plan* plan, int form);
 int hsma_plan_last_pair_form(const hsma_plan* plan);

@@ -118,7 +118,7 @@ class Plan:
         return binding.hsma_plan_get_timing(self.handle)
 
     def set_pair_form(self, form: int):
-        """0: automatic (symmetric form of step (b) when it applies); 1: ordered pairs always."""
+        """0: automatic; 1: ordered pairs always; 2: symmetric form of step (b) wherever it applies (forces too)."""
         binding.hsma_plan_set_pair_form(self.handle, form)
 
     @property

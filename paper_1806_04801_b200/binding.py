@@ -411,7 +411,7 @@ PAIR_FORM_AUTO, PAIR_FORM_ORDERED, PAIR_FORM_SYMMETRIC = 0, 1, 2
 
 
 def hsma_plan_set_pair_form(plan: int, form: int):
-    """Step (b): 0 = automatic (symmetric form when it applies), 1 = ordered pairs always."""
+    """Step (b): 0 = automatic, 1 = ordered pairs always, 2 = symmetric form wherever it applies (include/hsma.h)."""
     _check(load_library().hsma_plan_set_pair_form(plan, int(form)), "hsma_plan_set_pair_form")
 
 

@@ -182,19 +182,37 @@ static int sym_resident(int refine) {
     if (!c) c = refine == 1 ? resident_ctas(near_sym_kernel<1>) : resident_ctas(near_sym_kernel<2>);
     return c;
 }
+// the gradient form needs 64 KB of dynamic shared memory: opt in once per instantiation
+template <int REFINE>
+static int sym_field_resident_of() {
+    cudaFuncSetAttribute(near_sym_field_kernel<REFINE>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSymFieldDynSmem);
+    int per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, near_sym_field_kernel<REFINE>, kThreads, kSymFieldDynSmem) != cudaSuccess || per_sm < 1) {
+        cudaGetLastError();
+        per_sm = 1;
+    }
+    return per_sm * num_sm();
+}
+static int sym_field_resident(int refine) {
+    static int cache[2] = {0, 0};
+    int& c = cache[refine == 1 ? 0 : 1];
+    if (!c) c = refine == 1 ? sym_field_resident_of<1>() : sym_field_resident_of<2>();
+    return c;
+}
 // part / n_parts: the contiguous share [F * part / n_parts, F * (part + 1) / n_parts) of the F fine units (multi-GPU)
-static SymLaunch choose_sym(long long n_tiles, int refine, int part = 0, int n_parts = 1) {
+static SymLaunch choose_sym(long long n_tiles, int refine, int part = 0, int n_parts = 1, bool field = false) {
     SymLaunch L;
+    const int chunks = field ? kSymFChunks : kSymChunks;
     L.n_blocks = (int)((n_tiles + kSymR - 1) / kSymR);
     L.visits = sym_visit0(L.n_blocks, n_tiles);
-    const long long F = L.visits * kSymChunks;
+    const long long F = L.visits * chunks;
     L.f_begin = F * part / n_parts;
     L.fine = F * (part + 1) / n_parts - L.f_begin;
-    L.G = (int)std::max<long long>(1, std::min<long long>(sym_resident(refine), L.fine));
+    L.G = (int)std::max<long long>(1, std::min<long long>(field ? sym_field_resident(refine) : sym_resident(refine), L.fine));
     L.rows = 1;
     for (int I = 0; I < L.n_blocks && L.fine > 0; ++I) {
-        const long long lo = std::max(sym_visit0(I, n_tiles) * kSymChunks, L.f_begin);
-        const long long hi = std::min(sym_visit0(I + 1, n_tiles) * kSymChunks, L.f_begin + L.fine);
+        const long long lo = std::max(sym_visit0(I, n_tiles) * chunks, L.f_begin);
+        const long long hi = std::min(sym_visit0(I + 1, n_tiles) * chunks, L.f_begin + L.fine);
         if (lo >= hi) continue;
         const int first = cta_of_unit(lo - L.f_begin, L.fine, L.G), last = cta_of_unit(hi - 1 - L.f_begin, L.fine, L.G);
         L.rows = std::max(L.rows, last - first + 1);
@@ -203,7 +221,11 @@ static SymLaunch choose_sym(long long n_tiles, int refine, int part = 0, int n_p
 }
 // The symmetric form pays when most visits are off the diagonal (a diagonal visit costs 11 instructions per ORDERED
 // pair): from 32 source tiles on, and while the cell table fits its shared-memory copy.
-static bool sym_applies(long long n_tiles, int C) { return n_tiles >= 32 && C <= kSymMaxCells; }
+// The gradient form gains less per evaluation (21 against 15 instructions per ordered pair, at a lower issue rate):
+// it is chosen automatically from 256 tiles on (N > 65,280); hsma_plan_set_pair_form(plan, 2) takes it from 32 tiles.
+static bool sym_applies(long long n_tiles, int C, bool field = false, int form = 0) {
+    return n_tiles >= (field && form != 2 ? 256 : 32) && C <= kSymMaxCells;
+}
 
 static Launch choose_node(long long T, long long n_tiles, bool field = false) {
     return choose_launch(T, n_tiles, 4, [field](int R) { return node_resident(R, field); });
@@ -272,7 +294,7 @@ struct hsma_plan {
     QInfo* qinfo = nullptr;
     DevBuf<double> part_a, part_b, part_c, red, xyz_in, q_in, phi_dev, force_dev;
     DevBuf<double> sym_col, sym_phi;   // symmetric form of step (b): column sums per visit, phi_near in source order
-    int pair_form = 0;                 // hsma_plan_set_pair_form: 0 = automatic, 1 = ordered pairs only
+    int pair_form = 0;                 // hsma_plan_set_pair_form: 0 = automatic, 1 = ordered pairs only, 2 = symmetric wherever possible
     int last_pair_form = 1;            // what the last evaluate used for step (b): 1 ordered, 2 symmetric
     long long last_launches = 0;
     hsma_status sticky = HSMA_OK;
@@ -678,7 +700,7 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
         MARK(3);
         SymArgs a;
         a.src = p->src.p; a.n_src = N; a.n_tiles = n_tiles; a.n_blocks = ss.n_blocks; a.cells = cells_b; a.C = C_b;
-        a.f_begin = ss.f_begin; a.fine = ss.fine; a.scale = refine == 1 ? 0.5 : 1.0; a.part = p->part_b.p; a.col = p->sym_col.p;
+        a.f_begin = ss.f_begin; a.fine = ss.fine; a.scale = refine == 1 ? 0.5 : 1.0; a.scale_grad = 0.0; a.part = p->part_b.p; a.col = p->sym_col.p;
         if (ss.fine > 0) {
             if (refine == 1) near_sym_kernel<1><<<ss.G, kThreads, 0, st>>>(a);
             else near_sym_kernel<2><<<ss.G, kThreads, 0, st>>>(a);
@@ -704,14 +726,14 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
         const int refine = p->refine ? p->refine : ((double)N * (double)p->last_images < 4294967296.0 ? 2 : 1);
         // rsqrt_refine = 0: the cubic step while (b) is latency-bound anyway (< 2^32 pairs), Newton above
         const size_t comps = field ? 4 : 1;
-        const bool sym = !field && !p->sphere && p->pair_form == 0 && t0 == 0 && t1 == N && sym_applies(n_tiles, C_b);
+        const bool sym = !p->sphere && p->pair_form != 1 && t0 == 0 && t1 == N && sym_applies(n_tiles, C_b, field, p->pair_form);
         p->last_pair_form = sym ? 2 : 1;
         Launch sb = choose_near(T, n_tiles_near, C_b, refine, field);
         SymLaunch ss{};
         if (sym) {
-            ss = choose_sym(n_tiles, refine);
-            if (p->part_b.reserve((size_t)ss.rows * ss.n_blocks * kSymBlock) != cudaSuccess ||
-                p->sym_col.reserve((size_t)ss.visits * kTile) != cudaSuccess || p->sym_phi.reserve((size_t)N) != cudaSuccess)
+            ss = choose_sym(n_tiles, refine, 0, 1, field);
+            if (p->part_b.reserve((size_t)ss.rows * ss.n_blocks * kSymBlock * comps) != cudaSuccess ||
+                p->sym_col.reserve((size_t)ss.visits * kTile * comps) != cudaSuccess || p->sym_phi.reserve((size_t)N * comps) != cudaSuccess)
                 return HSMA_ERR_ALLOC;
         } else if (p->part_b.reserve((size_t)sb.rows * T * comps) != cudaSuccess) {
             return HSMA_ERR_ALLOC;
@@ -724,14 +746,24 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
             // every unordered (source, source) pair once: row sums + column sums, then phi_near in source order
             SymArgs a;
             a.src = p->src.p; a.n_src = N; a.n_tiles = n_tiles; a.n_blocks = ss.n_blocks; a.cells = cells_b; a.C = C_b;
-            a.f_begin = ss.f_begin; a.fine = ss.fine; a.scale = refine == 1 ? 0.5 : 1.0; a.part = p->part_b.p; a.col = p->sym_col.p;
+            a.f_begin = ss.f_begin; a.fine = ss.fine; a.scale = refine == 1 ? 0.5 : 1.0; a.scale_grad = refine == 1 ? -0.25 : -1.0;
+            a.part = p->part_b.p; a.col = p->sym_col.p;
             if (ss.fine > 0) {
-                if (refine == 1) near_sym_kernel<1><<<ss.G, kThreads, 0, st>>>(a);
-                else near_sym_kernel<2><<<ss.G, kThreads, 0, st>>>(a);
+                if (field) {
+                    if (refine == 1) near_sym_field_kernel<1><<<ss.G, kThreads, kSymFieldDynSmem, st>>>(a);
+                    else near_sym_field_kernel<2><<<ss.G, kThreads, kSymFieldDynSmem, st>>>(a);
+                } else {
+                    if (refine == 1) near_sym_kernel<1><<<ss.G, kThreads, 0, st>>>(a);
+                    else near_sym_kernel<2><<<ss.G, kThreads, 0, st>>>(a);
+                }
                 HSMA_COUNT_LAUNCH();
             }
-            sym_gather_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(p->part_b.p, p->sym_col.p, p->slot_of.p, N, n_tiles,
-                                                                          ss.n_blocks, ss.f_begin, ss.fine, ss.G, p->sym_phi.p);
+            if (field)
+                sym_gather_field_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(p->part_b.p, p->sym_col.p, p->slot_of.p, N, n_tiles,
+                                                                                    ss.n_blocks, ss.f_begin, ss.fine, ss.G, p->sym_phi.p);
+            else
+                sym_gather_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(p->part_b.p, p->sym_col.p, p->slot_of.p, N, n_tiles,
+                                                                              ss.n_blocks, ss.f_begin, ss.fine, ss.G, p->sym_phi.p);
             HSMA_COUNT_LAUNCH();
             layout_b = PartLayout{p->sym_phi.p, 1, 1, 1, (int)std::min<long long>(T, 2147483647LL)};
         } else {
@@ -745,7 +777,7 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
         // H7: phi (forces) and U
         const long long fb = (T + 255) / 256;
         if (field)
-            finish_field_kernel<<<(unsigned)fb, 256, 0, st>>>(sb.layout(p->part_b.p), sc.layout(p->part_c.p), T, p->src.p, p->slot_of.p, t0,
+            finish_field_kernel<<<(unsigned)fb, 256, 0, st>>>(layout_b, sc.layout(p->part_c.p), T, p->src.p, p->slot_of.p, t0,
                                                               phi_out, force_out, energy_out ? p->red.p : nullptr);
         else
             finish_phi_kernel<<<(unsigned)fb, 256, 0, st>>>(layout_b, sc.layout(p->part_c.p), T, p->src.p, p->slot_of.p, t0, phi_out,
@@ -1161,7 +1193,7 @@ extern "C" hsma_status hsma_plan_set_timing(hsma_plan* p, int enable) {
 }
 
 extern "C" hsma_status hsma_plan_set_pair_form(hsma_plan* p, int form) {
-    if (!p || (form != 0 && form != 1)) return HSMA_ERR_INVALID_ARG;
+    if (!p || form < 0 || form > 2) return HSMA_ERR_INVALID_ARG;
     p->pair_form = form;
     ++g_alloc_epoch;   // a captured evaluate graph holds the other form's launches
     return HSMA_OK;

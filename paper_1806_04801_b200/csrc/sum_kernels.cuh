@@ -364,8 +364,9 @@ struct SymArgs {
     long long f_begin;   // this launch walks the fine units [f_begin, f_begin + fine) of the F = sym_visit0(n_blocks) *
     long long fine;      // kSymChunks in all (one rank: everything; R ranks: a contiguous 1/R each)
     double scale;        // 0.5 for the Newton form (y is twice the reciprocal distance)
-    double* part;        // [rows][n_blocks * kSymBlock]
-    double* col;         // [visits][kTile]
+    double scale_grad;   // gradient form only: -1/4 (Newton), -1 (cubic)
+    double* part;        // [rows][n_blocks * kSymBlock]              (gradient form: [rows][4][...])
+    double* col;         // [visits][kTile]                           (gradient form: [visits][4][kTile])
 };
 
 template <int REFINE>
@@ -529,6 +530,220 @@ __global__ void __launch_bounds__(kThreads, 1) near_sym_kernel(const SymArgs a) 
         }
     }
     if (!fresh) store_block(I);
+}
+
+// ---- step (b), symmetric form with the gradient (forces, Eq.(9)) ------------------------------
+// One evaluation now feeds phi_i, grad phi_i, phi_j and grad phi_j.  With d = r_i - img_c(r_j) and v = w / |d|^3:
+//   grad_i (q_j w / |d|)           = -q_j v d                      (the source is moved, so d is in the original frame)
+//   grad_j (q_i w / |r_j - img'|)  = +q_i v (sigma_c o d)          (partner cell: d' = -sigma_c o d, same |d|)
+// Per evaluation (Newton): 3 DADD + DMUL + 2 DFMA (r2) + MUFU + 3 DMUL (y0^2, y, y^2) + DFMA (g) + DMUL (v)
+// + row: DFMA + DMUL + 3 DFMA + column: DFMA + DMUL + 3 DFMA = 21 FP64-pipe instructions, i.e. 10.5 per pair
+// interaction against 15 in near_sum_kernel<.., FIELD>.  The reflection signs, the cell weight and the powers of
+// two of the Newton form (y = 2/|d|, v = 8/|d|^3) are applied once per (source, cell) and at the stores.
+// Layouts: part[(row * 4 + comp) * Tp + packed index], col[(visit * 4 + comp) * kTile + j], comp 0 = phi,
+// 1..3 = grad phi.  Work decomposition, diagonal visits and determinism as in near_sym_kernel.
+constexpr int kSymFS = 2;                       // sources per chunk of the gradient form (register budget)
+constexpr int kSymFChunks = kTile / kSymFS;
+constexpr int kSymFieldDynSmem = (kThreads / 32) * 4 * kTile * (int)sizeof(double);
+
+template <int REFINE>
+__global__ void __launch_bounds__(kThreads, 1) near_sym_field_kernel(const SymArgs a) {
+    __shared__ __align__(128) Src4 tile[kStages][kTile];
+    __shared__ __align__(8) uint64_t full[kStages];
+    struct SymCell { double sx, sy, sz, w, gx, gy, gz; int central, pad; };
+    __shared__ SymCell cells[kSymMaxCells];
+    extern __shared__ double colw[];   // [kThreads / 32][4][kTile] = 64 KB of dynamic shared memory (kSymFieldDynSmem)
+
+    constexpr int R = kSymR, S = kSymFS;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int G = gridDim.x, k = blockIdx.x;
+    const long long f0 = a.f_begin + unit_start(k, a.fine, G), f1 = a.f_begin + unit_start(k + 1, a.fine, G);
+    if (f1 <= f0) return;
+    const long long V0 = f0 / kSymFChunks, V1 = (f1 - 1) / kSymFChunks;
+    const int nt = (int)a.n_tiles;
+    int I = 0;
+    while (sym_visit0(I + 1, nt) <= V0) ++I;
+    int J = I * R + (int)(V0 - sym_visit0(I, nt));
+
+    for (int c = tid; c < a.C; c += kThreads) {
+        const Cell g = a.cells[c];
+        cells[c] = SymCell{g.sx, g.sy, g.sz, g.w * a.scale, g.fx ? -1.0 : 1.0, g.fy ? -1.0 : 1.0, g.fz ? -1.0 : 1.0, g.central, 0};
+    }
+    if (tid == 0) {
+        for (int s = 0; s < kStages; ++s) mbar_init(&full[s], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    if (tid == 0) {
+        mbar_expect_tx(&full[0], kTile * sizeof(Src4));
+        bulk_g2s(tile[0], a.src + (long long)J * kTile, kTile * sizeof(Src4), &full[0]);
+    }
+
+    double ox[R], oy[R], oz[R], oq[R], tot[R], tgx[R], tgy[R], tgz[R];
+    const int nvis = (int)(V1 - V0) + 1;
+    const int ch_first = (int)(f0 - V0 * kSymFChunks), ch_last = (int)(f1 - 1 - V1 * kSymFChunks) + 1;
+    const long long Tp = (long long)a.n_blocks * kSymBlock;
+    const double sg = a.scale_grad;   // gradient sums -> grad phi: -1/4 (Newton: v = 8/|d|^3 against the 1/2 in w), -1 (cubic)
+    bool fresh = true;
+    auto store_block = [&](int blk) {
+        const int row = k - cta_of_unit(max(sym_visit0(blk, nt) * kSymFChunks, a.f_begin) - a.f_begin, a.fine, G);
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            double* o = a.part + (long long)row * 4 * Tp + (long long)blk * kSymBlock + r * kThreads + tid;
+            o[0] = tot[r]; o[Tp] = sg * tgx[r]; o[2 * Tp] = sg * tgy[r]; o[3 * Tp] = sg * tgz[r];
+        }
+    };
+
+    for (int it = 0; it < nvis; ++it) {
+        const int st = it & 1;
+        const bool last_of_block = J + 1 == nt;
+        if (tid == 0 && it + 1 < nvis) {
+            const int Jn = last_of_block ? (I + 1) * R : J + 1;
+            mbar_expect_tx(&full[st ^ 1], kTile * sizeof(Src4));
+            bulk_g2s(tile[st ^ 1], a.src + (long long)Jn * kTile, kTile * sizeof(Src4), &full[st ^ 1]);
+        }
+        if (fresh) {
+            fresh = false;
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const int tt = I * R + r;
+                const Src4 t = a.src[(long long)min(tt, nt - 1) * kTile + tid];
+                ox[r] = t.x; oy[r] = t.y; oz[r] = t.z; oq[r] = tt < nt ? t.q : 0.0;
+                tot[r] = 0.0; tgx[r] = 0.0; tgy[r] = 0.0; tgz[r] = 0.0;
+            }
+        }
+        const int rd = J - I * R;
+        const bool diag = rd < R;
+        mbar_wait(&full[st], (it >> 1) & 1);
+        const Src4* __restrict__ s = tile[st];
+        const int ch_lo = it == 0 ? ch_first : 0;
+        const int ch_hi = it == nvis - 1 ? ch_last : kSymFChunks;
+        double* colv = a.col + (V0 + it) * 4 * kTile;
+
+        for (int ch = ch_lo; ch < ch_hi; ++ch) {
+            const int j0 = ch * S;
+            double sx[S], sy[S], sz[S], sq[S], cp[S], cx[S], cy[S], cz[S];
+#pragma unroll
+            for (int i = 0; i < S; ++i) {
+                const double2 xy = *reinterpret_cast<const double2*>(&s[j0 + i].x);
+                const double2 zq = *reinterpret_cast<const double2*>(&s[j0 + i].z);
+                sx[i] = xy.x; sy[i] = xy.y; sz[i] = zq.x; sq[i] = zq.y;
+                cp[i] = 0.0; cx[i] = 0.0; cy[i] = 0.0; cz[i] = 0.0;
+            }
+#pragma unroll 1
+            for (int c = 0; c < a.C; ++c) {
+                const SymCell cell = cells[c];
+                const double wc = cell.w;
+                if (diag && cell.central) {
+#pragma unroll 1
+                    for (int i = 0; i < S; ++i) {
+                        const double2 xy = *reinterpret_cast<const double2*>(&s[j0 + i].x);
+                        const double2 zq = *reinterpret_cast<const double2*>(&s[j0 + i].z);
+                        const double wq = zq.y * wc;
+                        const bool mine = j0 + i == tid;
+#pragma unroll
+                        for (int r = 0; r < R; ++r) {
+                            const bool self = mine && r == rd;
+                            const double dx = ox[r] - (self ? ox[r] + 1.0 : xy.x), dy = oy[r] - xy.y, dz = oz[r] - zq.x;
+                            const double y = sym_recip<REFINE>(dx, dy, dz);
+                            const double wm = self ? 0.0 : wq;
+                            const double wv = wm * (y * (y * y));
+                            tot[r] = fma(wm, y, tot[r]);
+                            tgx[r] = fma(wv, dx, tgx[r]); tgy[r] = fma(wv, dy, tgy[r]); tgz[r] = fma(wv, dz, tgz[r]);
+                        }
+                    }
+                } else {
+#pragma unroll
+                    for (int i = 0; i < S; ++i) {
+                        const double px = fma(cell.gx, sx[i], cell.sx);
+                        const double py = fma(cell.gy, sy[i], cell.sy);
+                        const double pz = fma(cell.gz, sz[i], cell.sz);
+                        const double wq = sq[i] * wc;
+                        double cj = 0.0, gx = 0.0, gy = 0.0, gz = 0.0;
+#pragma unroll
+                        for (int r = 0; r < R; ++r) {
+                            const double dx = ox[r] - px, dy = oy[r] - py, dz = oz[r] - pz;
+                            const double y = sym_recip<REFINE>(dx, dy, dz);
+                            const double v = y * (y * y);
+                            const double wv = wq * v, ov = oq[r] * v;
+                            tot[r] = fma(wq, y, tot[r]);
+                            tgx[r] = fma(wv, dx, tgx[r]); tgy[r] = fma(wv, dy, tgy[r]); tgz[r] = fma(wv, dz, tgz[r]);
+                            cj = fma(oq[r], y, cj);
+                            gx = fma(ov, dx, gx); gy = fma(ov, dy, gy); gz = fma(ov, dz, gz);
+                        }
+                        cp[i] = fma(wc, cj, cp[i]);
+                        cx[i] = fma(wc * cell.gx, gx, cx[i]); cy[i] = fma(wc * cell.gy, gy, cy[i]); cz[i] = fma(wc * cell.gz, gz, cz[i]);
+                    }
+                }
+            }
+            if (!diag) {
+#pragma unroll
+                for (int i = 0; i < S; ++i) {
+                    double v0 = cp[i], v1 = cx[i], v2 = cy[i], v3 = cz[i];
+#pragma unroll
+                    for (int o = 16; o; o >>= 1) {
+                        v0 += __shfl_xor_sync(0xffffffffu, v0, o); v1 += __shfl_xor_sync(0xffffffffu, v1, o);
+                        v2 += __shfl_xor_sync(0xffffffffu, v2, o); v3 += __shfl_xor_sync(0xffffffffu, v3, o);
+                    }
+                    if (lane == 0) {
+                        double* o = colw + (warp * 4) * kTile + j0 + i;
+                        o[0] = v0; o[kTile] = v1; o[2 * kTile] = v2; o[3 * kTile] = v3;
+                    }
+                }
+            }
+        }
+        __syncthreads();  // tile[st] may be refilled; colw is complete
+        if (!diag) {
+            // grad_j = +q_i v sigma o d: the factor sg of the row side carries a minus sign, hence -sg here
+            const int j = tid;  // kTile == kThreads
+            if (j >= ch_lo * S && j < ch_hi * S) {
+#pragma unroll
+                for (int comp = 0; comp < 4; ++comp) {
+                    double v = 0.0;
+#pragma unroll
+                    for (int w = 0; w < kThreads / 32; ++w) v += colw[(w * 4 + comp) * kTile + j];
+                    colv[comp * kTile + j] = comp == 0 ? v : -sg * v;
+                }
+            }
+            __syncthreads();  // colw is rewritten by the next visit
+        }
+        if (last_of_block) {
+            store_block(I);
+            ++I; J = I * R; fresh = true;
+        } else {
+            ++J;
+        }
+    }
+    if (!fresh) store_block(I);
+}
+
+// FIELD form of sym_gather_kernel: out[comp * N + t], comp 0 = phi, 1..3 = grad phi, original source order.
+__global__ void sym_gather_field_kernel(const double* __restrict__ part, const double* __restrict__ col,
+                                        const int* __restrict__ slot_of, long long N, long long n_tiles, int n_blocks,
+                                        long long f_begin, long long fine, int G, double* __restrict__ out) {
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= N) return;
+    const long long p = slot_of[t];
+    const int I = (int)(p / kSymBlock), J = (int)(p / kTile), j = (int)(p % kTile);
+    const long long Tp = (long long)n_blocks * kSymBlock;
+    const long long f_end = f_begin + fine;
+    double v[4] = {0.0, 0.0, 0.0, 0.0};
+    const long long lo = max(sym_visit0(I, n_tiles) * kSymFChunks, f_begin), hi = min(sym_visit0(I + 1, n_tiles) * kSymFChunks, f_end);
+    if (lo < hi) {
+        const int first = cta_of_unit(lo - f_begin, fine, G), last = cta_of_unit(hi - 1 - f_begin, fine, G);
+        for (int r = 0; r <= last - first; ++r)
+#pragma unroll
+            for (int c = 0; c < 4; ++c) v[c] += part[((long long)r * 4 + c) * Tp + p];
+    }
+    for (int b = 0; b < I; ++b) {
+        const long long vis = sym_visit0(b, n_tiles) + (J - b * kSymR);
+        const long long f = vis * kSymFChunks + j / kSymFS;
+        if (f >= f_begin && f < f_end)
+#pragma unroll
+            for (int c = 0; c < 4; ++c) v[c] += col[(vis * 4 + c) * kTile + j];
+    }
+#pragma unroll
+    for (int c = 0; c < 4; ++c) out[c * N + t] = v[c];
 }
 
 // phi of step (b) in the ORIGINAL source order: row sums (fixed CTA order) + column sums (blocks in order), of the

@@ -11,7 +11,7 @@ pytestmark = pytest.mark.gpu
 
 PHI_TOL = 1e-10
 U_TOL = 1e-11
-ORDERED, SYMMETRIC = 1, 2
+ORDERED, SYMMETRIC = 1, 2     # also the values of hsma_plan_set_pair_form (0 = automatic)
 
 
 @pytest.fixture(scope="module")
@@ -75,7 +75,7 @@ def test_symmetric_form_random_magnitudes(H, refine):
 
 
 def test_when_the_symmetric_form_applies(H):
-    """All N targets, potentials only, >= 32 source tiles: symmetric.  Shards, forces, small N: ordered.  The form
+    """All N targets, >= 32 source tiles: symmetric (potentials and forces).  Shards, small N: ordered.  The form
     is not a property of the result: every variant agrees with the full evaluate."""
     import torch
     w = W.config(5, N=8192)
@@ -89,13 +89,21 @@ def test_when_the_symmetric_form_applies(H):
         b, _ = plan.evaluate_shard(xyz, q, 5000, w.N, sync=True)
         assert np.max(np.abs(np.concatenate([a.cpu().numpy(), b.cpu().numpy()]) - ref)) <= 2e-11 * np.max(np.abs(ref))
         phi_f, F, U_f = plan.evaluate_forces(xyz, q, sync=True)
-        assert plan.last_pair_form == ORDERED
+        assert plan.last_pair_form == ORDERED                        # forces: automatic only from 256 tiles on
+        plan.set_pair_form(SYMMETRIC)
+        phi_f, F, U_f = plan.evaluate_forces(xyz, q, sync=True)
+        assert plan.last_pair_form == SYMMETRIC                      # ... but available from 32 tiles on request
+        plan.set_pair_form(0)
         assert rel_inf(phi_f.cpu().numpy(), ref) <= 2e-11 and abs(float(U_f) - float(U)) <= 1e-11 * abs(float(U))
+        _, Fs, _ = plan.evaluate_forces_shard(xyz, q, 100, 7000, sync=True)
+        assert plan.last_pair_form == ORDERED
+        Fh = F.cpu().numpy()
+        assert np.max(np.abs(Fs.cpu().numpy() - Fh[100:7000])) <= 2e-11 * np.max(np.abs(Fh))
         phi2, U2 = plan.evaluate(xyz, q, sync=True)
         assert plan.last_pair_form == SYMMETRIC
         assert torch.equal(phi2, phi) and float(U2) == float(U)     # deterministic: fixed summation order
         with pytest.raises(Exception):
-            plan.set_pair_form(2)
+            plan.set_pair_form(3)
     w_small = W.config(5, N=7936)   # 31 tiles
     with H.Plan.from_workload(w_small) as plan:
         plan.evaluate(dev(w_small.xyz), dev(w_small.q), sync=True)
@@ -180,3 +188,45 @@ def test_evaluate_distributed_single_process_uses_the_part_form(H):
             ps, _, Us = shard.evaluate_distributed(plan_s, dev(ws.xyz), dev(ws.q))
             pr, Ur = plan_s.evaluate(dev(ws.xyz), dev(ws.q), sync=True)
             assert rel_inf(ps.cpu().numpy(), pr.cpu().numpy()) <= 1e-13
+
+
+@pytest.mark.parametrize("refine", [1, 2])
+@pytest.mark.parametrize("idx,N", [(2, 7938), (3, 9000), (4, 9000), (5, 12288)])
+def test_symmetric_forces_match_oracle(H, idx, N, refine):
+    """The gradient form of the symmetric kernel (near_sym_field_kernel): forces, potentials and U against the oracle
+    for the periodic, mirror-cavity and slab cell tables (reflected axes flip the column gradient), and against the
+    ordered potential+gradient kernel."""
+    w = W.config(idx, N=N)
+    r = O.hsma(w, forces=True)
+    with H.Plan.from_workload(w, rsqrt_refine=refine) as plan:
+        xyz, q = dev(w.xyz), dev(w.q)
+        plan.set_pair_form(SYMMETRIC)
+        phi, F, U = plan.evaluate_forces(xyz, q, sync=True)
+        assert plan.last_pair_form == SYMMETRIC
+        plan.set_pair_form(ORDERED)
+        phi1, F1, U1 = plan.evaluate_forces(xyz, q, sync=True)
+        assert plan.last_pair_form == ORDERED
+    F, F1, phi = F.cpu().numpy(), F1.cpu().numpy(), phi.cpu().numpy()
+    scale = max(float(np.max(np.abs(r.F))), float(np.max(np.abs(w.q)) * np.max(np.abs(r.phi)) / max(w.L)))
+    assert np.max(np.abs(F - r.F)) <= 1e-10 * scale
+    assert np.max(np.abs(F1 - r.F)) <= 1e-10 * scale
+    assert np.max(np.abs(F - F1)) <= 2e-11 * scale
+    assert rel_inf(phi, r.phi) <= PHI_TOL and abs(float(U) - r.U) <= U_TOL * abs(r.U)
+
+
+def test_symmetric_forces_random_magnitudes_and_momentum(H):
+    """Random-magnitude charges in the periodic box: forces against the oracle; the net force of the near sum
+    vanishes identically in the symmetric form (every pair contributes +f and -f), so the total is at the level of
+    the far field's truncation."""
+    w = W.config(5, N=8300)
+    q = np.random.default_rng(5).standard_normal(w.N)
+    q -= q.mean()
+    w = w.with_(q=q)
+    r = O.hsma(w, forces=True)
+    with H.Plan.from_workload(w) as plan:
+        plan.set_pair_form(SYMMETRIC)
+        phi, F, U = plan.evaluate_forces(dev(w.xyz), dev(w.q), sync=True)
+        assert plan.last_pair_form == SYMMETRIC
+    F = F.cpu().numpy()
+    assert rel_inf(F, r.F) <= 1e-10
+    assert np.abs(F.sum(0)).max() < 1e-3 * np.abs(F).max()
