@@ -458,7 +458,7 @@ def main():
                          "paper's circumsphere rule (DESIGN.md 6.10)")
     ap.add_argument("--pair-form", choices=["auto", "ordered", "symmetric"], default="auto",
                     help="step (b): auto = symmetric form (each unordered pair once) when one rank evaluates all targets "
-                         "(forces: from N > 65,280); ordered = always near_sum_kernel; symmetric = wherever it applies")
+                         "; ordered = always near_sum_kernel; symmetric = wherever it applies")
     ap.add_argument("--forces", action="store_true", help="time hsma_evaluate_forces (potential + forces) instead")
     ap.add_argument("--refine", type=int, default=0, choices=[0, 1, 2], help="hsma_plan_desc.rsqrt_refine")
     ap.add_argument("--e2e-steps", type=int, default=3)

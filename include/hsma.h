@@ -266,9 +266,9 @@ hsma_status hsma_plan_get_timing(hsma_plan* plan, double* ms_out);
  * least 32 source tiles = N > 7936, at most 128 near cells) the targets are the sources and the image sum is
  * symmetric (every image cell has a partner of equal weight), so each unordered pair can be
  * evaluated once and feed both phi_i and phi_j (and both gradients): the "symmetric" form, near_sym_kernel /
- * near_sym_field_kernel.  form = 0 (default): automatic -- potentials take it whenever it applies, forces from 256
- * source tiles on (N > 65,280; below that the ordered gradient kernel is as fast); form = 1: always the ordered-pair
- * kernel (near_sum_kernel), e.g. to compare the two; form = 2: the symmetric form wherever it applies, forces included.
+ * near_sym_field_kernel.  form = 0 (default): automatic -- the symmetric form whenever it applies; form = 1: always
+ * the ordered-pair kernel (near_sum_kernel), e.g. to compare the two; form = 2: the symmetric form wherever it applies
+ * (today the same as 0; kept distinct so that a future cost model in the automatic choice cannot change a caller's request).
  * Shards (t0 > 0 or t1 < N) and the sphere-culled near set always use the ordered form.  Other values:
  * HSMA_ERR_INVALID_ARG.  hsma_plan_last_pair_form: what the last evaluate used for step (b): 1 ordered, 2 symmetric
  * (0: null plan).

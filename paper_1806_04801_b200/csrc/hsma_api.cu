@@ -221,10 +221,10 @@ static SymLaunch choose_sym(long long n_tiles, int refine, int part = 0, int n_p
 }
 // The symmetric form pays when most visits are off the diagonal (a diagonal visit costs 11 instructions per ORDERED
 // pair): from 32 source tiles on, and while the cell table fits its shared-memory copy.
-// The gradient form gains less per evaluation (21 against 15 instructions per ordered pair, at a lower issue rate):
-// it is chosen automatically from 256 tiles on (N > 65,280); hsma_plan_set_pair_form(plan, 2) takes it from 32 tiles.
+// (the gradient form breaks even at 32 tiles too: 1.01x at N = 8192, 1.13x at 16,384, 1.26x at 262,144)
 static bool sym_applies(long long n_tiles, int C, bool field = false, int form = 0) {
-    return n_tiles >= (field && form != 2 ? 256 : 32) && C <= kSymMaxCells;
+    (void)field; (void)form;
+    return n_tiles >= 32 && C <= kSymMaxCells;
 }
 
 static Launch choose_node(long long T, long long n_tiles, bool field = false) {

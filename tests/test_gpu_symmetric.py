@@ -89,11 +89,7 @@ def test_when_the_symmetric_form_applies(H):
         b, _ = plan.evaluate_shard(xyz, q, 5000, w.N, sync=True)
         assert np.max(np.abs(np.concatenate([a.cpu().numpy(), b.cpu().numpy()]) - ref)) <= 2e-11 * np.max(np.abs(ref))
         phi_f, F, U_f = plan.evaluate_forces(xyz, q, sync=True)
-        assert plan.last_pair_form == ORDERED                        # forces: automatic only from 256 tiles on
-        plan.set_pair_form(SYMMETRIC)
-        phi_f, F, U_f = plan.evaluate_forces(xyz, q, sync=True)
-        assert plan.last_pair_form == SYMMETRIC                      # ... but available from 32 tiles on request
-        plan.set_pair_form(0)
+        assert plan.last_pair_form == SYMMETRIC                      # forces over all targets: the gradient form
         assert rel_inf(phi_f.cpu().numpy(), ref) <= 2e-11 and abs(float(U_f) - float(U)) <= 1e-11 * abs(float(U))
         _, Fs, _ = plan.evaluate_forces_shard(xyz, q, 100, 7000, sync=True)
         assert plan.last_pair_form == ORDERED
