@@ -190,16 +190,17 @@ hsma_status hsma_evaluate_rest_shard(hsma_plan* plan, const double* xyz, const d
 /*
  * Step 4 in PART form: instead of a target shard, rank `part` of `n_parts` takes a contiguous
  * 1/n_parts of the UNORDERED source pairs of step (b) (symmetric form: one evaluation feeds phi_i and phi_j) and the
- * node sum (c) for the targets t0 <= i < t1 (the ranks' [t0,t1) must tile 0..N).  phi_part_out dev [N] (all targets)
- * and energy_part_out dev [1] (or NULL) are PARTIAL: their sums over the parts are phi and U -- the caller
- * all-reduces them (2 MB at N = 262,144).  Same arithmetic on every part count; results differ from the one-rank
+ * node sum (c) for the targets t0 <= i < t1 (the ranks' [t0,t1) must tile 0..N).  phi_part_out dev [N] (all targets),
+ * force_part_out dev [N,3] (NULL: potentials only; with forces phi_part_out may be NULL) and energy_part_out dev [1]
+ * (or NULL) are PARTIAL: their sums over the parts are phi, F and U -- the caller all-reduces them (2 MB / 6 MB at
+ * N = 262,144).  Same arithmetic on every part count; results differ from the one-rank
  * evaluate only in the order of the sums.  Needs what the symmetric form needs: hsma_plan_part_form_applies(plan, N)
  * returns 1 if so (whole-cell near set, N > 7936, <= 128 near cells), else 0 (use hsma_evaluate_rest_shard);
- * HSMA_ERR_INVALID_ARG otherwise.  Potentials only.
+ * HSMA_ERR_INVALID_ARG otherwise.
  */
 hsma_status hsma_evaluate_rest_part(hsma_plan* plan, const double* xyz, const double* q, long long N, int part,
                                     int n_parts, long long t0, long long t1, double* phi_part_out,
-                                    double* energy_part_out);
+                                    double* force_part_out, double* energy_part_out);
 int hsma_plan_part_form_applies(const hsma_plan* plan, long long N);
 
 /* Synchronise the plan's stream and return the sticky status of the evaluations since the last

@@ -100,7 +100,7 @@ _SIGNATURES = {
     "hsma_fp64_peak": (ctypes.c_int, [ctypes.c_double, c_double_p, c_double_p]),
     "hsma_evaluate_rest_part": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_longlong,
                                                ctypes.c_int, ctypes.c_int, ctypes.c_longlong, ctypes.c_longlong,
-                                               ctypes.c_void_p, ctypes.c_void_p]),
+                                               ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]),
     "hsma_plan_part_form_applies": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_longlong]),
     "hsma_plan_set_timing": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int]),
     "hsma_plan_set_pair_form": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int]),
@@ -304,11 +304,14 @@ def hsma_evaluate_rest_shard(plan: int, xyz: torch.Tensor, q: torch.Tensor, t0: 
 
 
 def hsma_evaluate_rest_part(plan: int, xyz: torch.Tensor, q: torch.Tensor, part: int, n_parts: int, t0: int, t1: int,
-                            phi_part_out: torch.Tensor, energy_part_out: Optional[torch.Tensor] = None):
-    """PART form of the last multi-GPU step: partial phi over all N targets and partial U (sum over parts = result)."""
+                            phi_part_out: Optional[torch.Tensor], force_part_out: Optional[torch.Tensor] = None,
+                            energy_part_out: Optional[torch.Tensor] = None):
+    """PART form of the last multi-GPU step: partial phi (and F) over all N targets and partial U (sums over the
+    parts = the result)."""
     N = q.numel()
     _check(load_library().hsma_evaluate_rest_part(plan, _dev(xyz, 3 * N, "xyz"), _dev(q, N, "q"), N, int(part), int(n_parts),
                                                   t0, t1, _dev(phi_part_out, N, "phi_part_out"),
+                                                  _dev(force_part_out, 3 * N, "force_part_out"),
                                                   _dev(energy_part_out, 1, "energy_part_out")), "hsma_evaluate_rest_part")
 
 

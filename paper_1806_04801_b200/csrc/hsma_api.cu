@@ -685,37 +685,53 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
     if (n_parts > 0) {
         // PART form (multi-GPU): this part's share of the unordered pairs of (b) for ALL targets, (c) for
         // the targets t0..t1-1; phi_out [N] and U add up over the parts
-        if (field || p->sphere || !sym_applies(n_tiles, C_b) || part < 0 || part >= n_parts || !phi_out) return HSMA_ERR_INVALID_ARG;
+        if (p->sphere || !sym_applies(n_tiles, C_b) || part < 0 || part >= n_parts || (!phi_out && !field)) return HSMA_ERR_INVALID_ARG;
         const int refine = p->refine ? p->refine : ((double)N * (double)p->last_images < 4294967296.0 ? 2 : 1);
-        const SymLaunch ss = choose_sym(n_tiles, refine, part, n_parts);
-        if (p->part_b.reserve((size_t)ss.rows * ss.n_blocks * kSymBlock) != cudaSuccess ||
-            p->sym_col.reserve((size_t)ss.visits * kTile) != cudaSuccess || p->sym_phi.reserve((size_t)N) != cudaSuccess)
+        const size_t comps = field ? 4 : 1;
+        const SymLaunch ss = choose_sym(n_tiles, refine, part, n_parts, field);
+        if (p->part_b.reserve((size_t)ss.rows * ss.n_blocks * kSymBlock * comps) != cudaSuccess ||
+            p->sym_col.reserve((size_t)ss.visits * kTile * comps) != cudaSuccess || p->sym_phi.reserve((size_t)N * comps) != cudaSuccess)
             return HSMA_ERR_ALLOC;
         Launch sc{};
         if (T > 0) {
-            sc = choose_node(T, p->node_tiles, false);
-            if (p->part_c.reserve((size_t)sc.rows * T) != cudaSuccess) return HSMA_ERR_ALLOC;
+            sc = choose_node(T, p->node_tiles, field);
+            if (p->part_c.reserve((size_t)sc.rows * T * comps) != cudaSuccess) return HSMA_ERR_ALLOC;
         }
         p->last_pair_form = 2;
         MARK(3);
         SymArgs a;
         a.src = p->src.p; a.n_src = N; a.n_tiles = n_tiles; a.n_blocks = ss.n_blocks; a.cells = cells_b; a.C = C_b;
-        a.f_begin = ss.f_begin; a.fine = ss.fine; a.scale = refine == 1 ? 0.5 : 1.0; a.scale_grad = 0.0; a.part = p->part_b.p; a.col = p->sym_col.p;
+        a.f_begin = ss.f_begin; a.fine = ss.fine; a.scale = refine == 1 ? 0.5 : 1.0; a.scale_grad = refine == 1 ? -0.25 : -1.0;
+        a.part = p->part_b.p; a.col = p->sym_col.p;
         if (ss.fine > 0) {
-            if (refine == 1) near_sym_kernel<1><<<ss.G, kThreads, 0, st>>>(a);
-            else near_sym_kernel<2><<<ss.G, kThreads, 0, st>>>(a);
+            if (field) {
+                if (refine == 1) near_sym_field_kernel<1><<<ss.G, kThreads, kSymFieldDynSmem, st>>>(a);
+                else near_sym_field_kernel<2><<<ss.G, kThreads, kSymFieldDynSmem, st>>>(a);
+            } else {
+                if (refine == 1) near_sym_kernel<1><<<ss.G, kThreads, 0, st>>>(a);
+                else near_sym_kernel<2><<<ss.G, kThreads, 0, st>>>(a);
+            }
             HSMA_COUNT_LAUNCH();
         }
-        sym_gather_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(p->part_b.p, p->sym_col.p, p->slot_of.p, N, n_tiles,
-                                                                      ss.n_blocks, ss.f_begin, ss.fine, ss.G, p->sym_phi.p);
+        if (field)
+            sym_gather_field_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(p->part_b.p, p->sym_col.p, p->slot_of.p, N, n_tiles,
+                                                                                ss.n_blocks, ss.f_begin, ss.fine, ss.G, p->sym_phi.p);
+        else
+            sym_gather_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(p->part_b.p, p->sym_col.p, p->slot_of.p, N, n_tiles,
+                                                                          ss.n_blocks, ss.f_begin, ss.fine, ss.G, p->sym_phi.p);
         HSMA_COUNT_LAUNCH();
         MARK(4);
         if (T > 0)
-            launch_node(sc, false, reinterpret_cast<const double*>(p->src.p), 4, p->slot_of.p, T, t0, p->nodes, p->node_tiles, p->part_c.p, st);
+            launch_node(sc, field, reinterpret_cast<const double*>(p->src.p), 4, p->slot_of.p, T, t0, p->nodes, p->node_tiles, p->part_c.p, st);
         MARK(5);
         const long long fb = (N + 255) / 256;
-        finish_part_kernel<<<(unsigned)fb, 256, 0, st>>>(p->sym_phi.p, T > 0 ? sc.layout(p->part_c.p) : PartLayout{nullptr, 1, 1, 1, 1}, N, t0, t1,
-                                                         p->src.p, p->slot_of.p, phi_out, energy_out ? p->red.p : nullptr);
+        const PartLayout layout_c = T > 0 ? sc.layout(p->part_c.p) : PartLayout{nullptr, 1, 1, 1, 1};
+        if (field)
+            finish_part_field_kernel<<<(unsigned)fb, 256, 0, st>>>(p->sym_phi.p, layout_c, N, t0, t1, p->src.p, p->slot_of.p, phi_out,
+                                                                   force_out, energy_out ? p->red.p : nullptr);
+        else
+            finish_part_kernel<<<(unsigned)fb, 256, 0, st>>>(p->sym_phi.p, layout_c, N, t0, t1, p->src.p, p->slot_of.p, phi_out,
+                                                             energy_out ? p->red.p : nullptr);
         HSMA_COUNT_LAUNCH();
         if (energy_out) {
             reduce_rows_kernel<<<1, 1024, 0, st>>>(p->red.p, fb, 1, 1, 0.5, energy_out);
@@ -906,9 +922,9 @@ extern "C" hsma_status hsma_evaluate_rest_shard(hsma_plan* plan, const double* x
 
 extern "C" hsma_status hsma_evaluate_rest_part(hsma_plan* plan, const double* xyz, const double* q, long long N, int part,
                                                int n_parts, long long t0, long long t1, double* phi_part_out,
-                                               double* energy_part_out) {
+                                               double* force_part_out, double* energy_part_out) {
     if (n_parts < 1) return HSMA_ERR_INVALID_ARG;
-    return evaluate_impl(plan, xyz, q, N, t0, t1, phi_part_out, energy_part_out, nullptr, kPhaseRest, 0, -1, part, n_parts);
+    return evaluate_impl(plan, xyz, q, N, t0, t1, phi_part_out, energy_part_out, force_part_out, kPhaseRest, 0, -1, part, n_parts);
 }
 extern "C" int hsma_plan_part_form_applies(const hsma_plan* p, long long N) {
     if (!p || N < 1) return 0;

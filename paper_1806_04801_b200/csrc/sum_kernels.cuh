@@ -1151,6 +1151,36 @@ __global__ void finish_part_kernel(const double* __restrict__ near, const PartLa
     }
 }
 
+// The same with forces: near [4][N] (phi, grad phi of this part's share), node sum rows in the FIELD layout for the
+// targets t0..t1-1; phi (may be null) and F = -q grad phi [N,3] are partial sums over the parts.
+__global__ void finish_part_field_kernel(const double* __restrict__ near, const PartLayout Lc, long long N, long long t0,
+                                         long long t1, const Src4* __restrict__ src, const int* __restrict__ slot_of,
+                                         double* __restrict__ phi, double* __restrict__ vec, double* __restrict__ u_part) {
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    double e = 0.0;
+    if (t < N) {
+        double v[4] = {near[t], near[N + t], near[2 * N + t], near[3 * N + t]};
+        if (t >= t0 && t < t1) sum_part_rows4(Lc, t - t0, t1 - t0, v);
+        const double qi = src[slot_of[t]].q;
+        if (phi) phi[t] = v[0];
+        vec[3 * t] = -qi * v[1]; vec[3 * t + 1] = -qi * v[2]; vec[3 * t + 2] = -qi * v[3];
+        e = qi * v[0];
+    }
+    if (u_part) {
+        __shared__ double sh[32];
+        for (int o = 16; o; o >>= 1) e += __shfl_down_sync(0xffffffffu, e, o);
+        const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+        if (l == 0) sh[w] = e;
+        __syncthreads();
+        if (w == 0) {
+            const int nw = blockDim.x >> 5;
+            e = l < nw ? sh[l] : 0.0;
+            for (int o = 16; o; o >>= 1) e += __shfl_down_sync(0xffffffffu, e, o);
+            if (l == 0) u_part[blockIdx.x] = e;
+        }
+    }
+}
+
 // second level of the deterministic reductions: out[k] = scale * sum_i in[i*stride + k], one block
 __global__ void reduce_rows_kernel(const double* __restrict__ in, long long n, int stride, int ncomp, double scale,
                                    double* __restrict__ out) {

@@ -76,9 +76,9 @@ def evaluate_distributed(plan, xyz: torch.Tensor, q: torch.Tensor, forces: bool 
       2. all-gather of the K_t check sums (one small message)       the only data-path collective before the fit
       3. fit, mapping and steps (b), (c) for this rank's targets    hsma_evaluate_rest_shard
       4. all-gather of phi (and F), all-reduce of U                 assembly of the result
-    or, when the symmetric form of step (b) applies (potentials only, DESIGN.md 6.12 / 8):
+    or, when the symmetric form of step (b) applies (DESIGN.md 6.12 / 8):
       3'. fit, mapping, this rank's share of the UNORDERED pairs of (b), (c) for its targets    hsma_evaluate_rest_part
-      4'. all-reduce of the partial phi [N] and of the partial U
+      4'. all-reduce of the partial phi [N] (and F [N,3]) and of the partial U
     Returns (phi [N], F [N,3] or None, U [1]) on every rank.  `plan` is a paper_1806_04801_b200.Plan."""
     from . import binding
     N = q.numel()
@@ -96,15 +96,18 @@ def evaluate_distributed(plan, xyz: torch.Tensor, q: torch.Tensor, forces: bool 
         pc_all = all_gather_slices(pc, Kt, group)
         pcg_all = all_gather_slices(pcg, Kt, group) if need_grad else None
         binding.hsma_set_check_sums(plan.handle, 0, Kt, pc_all.contiguous(), pcg_all.contiguous() if need_grad else None)
-    if not forces and binding.hsma_plan_part_form_applies(plan.handle, N):
+    if binding.hsma_plan_part_form_applies(plan.handle, N):
         # PART form: this rank's share of the unordered pairs of (b) for all targets + (c) for its own targets;
-        # phi and U are sums over the ranks (one all-reduce each)
+        # phi, F and U are sums over the ranks (one all-reduce each)
         phi_part = torch.empty(N, dtype=torch.float64, device=q.device)
+        F_part = torch.empty(N, 3, dtype=torch.float64, device=q.device) if forces else None
         U = torch.empty(1, dtype=torch.float64, device=q.device)
-        binding.hsma_evaluate_rest_part(plan.handle, xyz, q, rank, world, t0, t1, phi_part, U)
+        binding.hsma_evaluate_rest_part(plan.handle, xyz, q, rank, world, t0, t1, phi_part, F_part, U)
         all_reduce_phi(phi_part, group)
+        if forces:
+            all_reduce_phi(F_part, group)
         all_reduce_energy(U, group)
-        return phi_part, None, U
+        return phi_part, F_part, U
     T = t1 - t0
     phi = torch.empty(T, dtype=torch.float64, device=q.device)
     F = torch.empty(T, 3, dtype=torch.float64, device=q.device) if forces else None

@@ -154,16 +154,33 @@ def test_part_form_adds_up_to_the_evaluate(H, idx, N, n_parts):
         for part, (t0, t1) in enumerate(shard.shard_bounds(w.N, n_parts)):
             pp = torch.empty(w.N, dtype=torch.float64, device="cuda")
             up = torch.empty(1, dtype=torch.float64, device="cuda")
-            H.binding.hsma_evaluate_rest_part(plan.handle, xyz, q, part, n_parts, t0, t1, pp, up)
+            H.binding.hsma_evaluate_rest_part(plan.handle, xyz, q, part, n_parts, t0, t1, pp, None, up)
             plan.sync()
             phi += pp
             U += up
         assert rel_inf(phi.cpu().numpy(), phi_ref.cpu().numpy()) <= 1e-12
         assert abs(float(U) - float(U_ref)) <= 1e-12 * abs(float(U_ref))
         assert rel_inf(phi.cpu().numpy(), r.phi) <= PHI_TOL and abs(float(U) - r.U) <= U_TOL * abs(r.U)
-        # bad part index, forces of a part: refused
+        # bad part index: refused
         with pytest.raises(Exception):
-            H.binding.hsma_evaluate_rest_part(plan.handle, xyz, q, n_parts, n_parts, 0, w.N, phi, U)
+            H.binding.hsma_evaluate_rest_part(plan.handle, xyz, q, n_parts, n_parts, 0, w.N, phi, None, U)
+        # the same with forces: partial phi, F and U add up
+        phi_r, F_ref, U_r = plan.evaluate_forces(xyz, q, sync=True)
+        H.binding.hsma_check_sums_shard(plan.handle, xyz, q, 0, Kt)
+        phi.zero_(); U.zero_()
+        F = torch.zeros(w.N, 3, dtype=torch.float64, device="cuda")
+        for part, (t0, t1) in enumerate(shard.shard_bounds(w.N, n_parts)):
+            pp = torch.empty(w.N, dtype=torch.float64, device="cuda")
+            fp = torch.empty(w.N, 3, dtype=torch.float64, device="cuda")
+            up = torch.empty(1, dtype=torch.float64, device="cuda")
+            H.binding.hsma_evaluate_rest_part(plan.handle, xyz, q, part, n_parts, t0, t1, pp, fp, up)
+            plan.sync()
+            phi += pp
+            F += fp
+            U += up
+        assert rel_inf(phi.cpu().numpy(), phi_r.cpu().numpy()) <= 1e-12
+        assert np.max(np.abs((F - F_ref).cpu().numpy())) <= 1e-12 * max(float(F_ref.abs().max()), float(phi_r.abs().max()))
+        assert abs(float(U) - float(U_r)) <= 1e-12 * abs(float(U_r))
 
 
 def test_evaluate_distributed_single_process_uses_the_part_form(H):
@@ -176,6 +193,10 @@ def test_evaluate_distributed_single_process_uses_the_part_form(H):
         phi, F, U = shard.evaluate_distributed(plan, xyz, q)
         plan.sync()
         assert F is None and plan.last_pair_form == SYMMETRIC
+        phi_f, F_f, U_f = shard.evaluate_distributed(plan, xyz, q, forces=True)
+        plan.sync()
+        _, F_ref, _ = plan.evaluate_forces(xyz, q, sync=True)
+        assert float((F_f - F_ref).abs().max()) <= 1e-12 * float(F_ref.abs().max())
         assert rel_inf(phi.cpu().numpy(), phi_ref.cpu().numpy()) <= 1e-13 and abs(float(U) - float(U_ref)) <= 1e-13 * abs(float(U_ref))
         # small systems keep the target-shard path
         ws = W.config(2)
