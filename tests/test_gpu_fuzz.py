@@ -116,3 +116,53 @@ def test_whole_evaluates_random_configurations(H, case):
     # random charges can make U = 1/2 sum q phi cancel to almost nothing; its rounding floor is eps sum|q| max|phi|
     assert abs(float(U) - r.U) <= 1e-11 * abs(r.U) + 1e-13 * float(np.abs(w.q).sum() * np.max(np.abs(r.phi)))
     assert rel_inf(F.cpu().numpy(), r.F) <= 1e-10
+
+
+@pytest.mark.parametrize("case", range(12))
+def test_symmetric_and_part_forms_random_sizes(H, case):
+    """DESIGN.md 6.12 / 8: random sizes between the smallest case the symmetric form takes and 60,000, random cell
+    table, charges, refinement and part count.  The symmetric potential and gradient kernels and the sum over the
+    parts of the multi-GPU PART form must agree with the ordered-pair kernels (which the other tests hold to the
+    oracle) to rounding: these sizes are too large for the oracle in a test, and what is checked here is the work
+    decomposition (visits, chunks, rows, column sums), which does not depend on it."""
+    import torch
+    from paper_1806_04801_b200 import shard
+    rng = np.random.default_rng(7000 + case)
+    idx = int(rng.choice([2, 3, 4, 5]))
+    N = 2 * int(rng.integers(3969, 30000))
+    w = W.config(idx, N=N)
+    if rng.random() < 0.4:
+        q = rng.standard_normal(N)
+        w = w.with_(q=q - q.mean())
+    with H.Plan.from_workload(w, rsqrt_refine=int(rng.choice([1, 2]))) as plan:
+        xyz, q = dev(w.xyz), dev(w.q)
+        phi, U = plan.evaluate(xyz, q, sync=True)
+        assert plan.last_pair_form == 2
+        pf, F, Uf = plan.evaluate_forces(xyz, q, sync=True)
+        assert plan.last_pair_form == 2
+        plan.set_pair_form(1)
+        phi1, U1 = plan.evaluate(xyz, q, sync=True)
+        _, F1, _ = plan.evaluate_forces(xyz, q, sync=True)
+        assert plan.last_pair_form == 1
+        plan.set_pair_form(0)
+        n_parts = int(rng.integers(1, 9))
+        H.binding.hsma_check_sums_shard(plan.handle, xyz, q, 0, plan.info["check_targets"])
+        ps = torch.zeros(N, dtype=torch.float64, device="cuda")
+        Fs = torch.zeros(N, 3, dtype=torch.float64, device="cuda")
+        Us = torch.zeros(1, dtype=torch.float64, device="cuda")
+        for part, (t0, t1) in enumerate(shard.shard_bounds(N, n_parts)):
+            a = torch.empty(N, dtype=torch.float64, device="cuda")
+            b = torch.empty(N, 3, dtype=torch.float64, device="cuda")
+            c = torch.empty(1, dtype=torch.float64, device="cuda")
+            H.binding.hsma_evaluate_rest_part(plan.handle, xyz, q, part, n_parts, t0, t1, a, b, c)
+            plan.sync()
+            ps += a
+            Fs += b
+            Us += c
+    sc = float(phi1.abs().max())
+    fs = max(float(F1.abs().max()), float(np.max(np.abs(w.q))) * sc / max(w.L))
+    tol = 2e-11
+    assert float((phi - phi1).abs().max()) <= tol * sc and float((pf - phi1).abs().max()) <= tol * sc
+    assert float((F - F1).abs().max()) <= tol * fs
+    assert float((ps - phi1).abs().max()) <= tol * sc and float((Fs - F1).abs().max()) <= tol * fs
+    assert abs(float(U) - float(U1)) <= 1e-11 * abs(float(U1)) and abs(float(Us) - float(U1)) <= 1e-11 * abs(float(U1))
