@@ -544,7 +544,7 @@ __global__ void __launch_bounds__(kThreads, 1) near_sym_kernel(const SymArgs a) 
 // 1..3 = grad phi.  Work decomposition, diagonal visits and determinism as in near_sym_kernel.
 constexpr int kSymFS = 2;                       // sources per chunk of the gradient form (register budget)
 constexpr int kSymFChunks = kTile / kSymFS;
-constexpr int kSymFieldDynSmem = ((kThreads / 32) * 4 * kTile + 4 * kSymR * kThreads) * (int)sizeof(double);
+constexpr int kSymFieldDynSmem = ((kThreads / 32) * 4 * kTile + 2 * kSymR * kThreads) * (int)sizeof(double);
 
 template <int REFINE>
 __global__ void __launch_bounds__(kThreads, 1) near_sym_field_kernel(const SymArgs a) {
@@ -552,15 +552,15 @@ __global__ void __launch_bounds__(kThreads, 1) near_sym_field_kernel(const SymAr
     __shared__ __align__(8) uint64_t full[kStages];
     struct SymCell { double sx, sy, sz, w, gx, gy, gz; int central, pad; };
     __shared__ SymCell cells[kSymMaxCells];
-    // dynamic shared memory (kSymFieldDynSmem): colw [kThreads / 32][4][kTile] (64 KB), then the block's targets
-    // txy / tzq [R][kThreads] double2 (32 KB each; slot [r][tid] is written and read by thread tid only).  With phi
-    // and grad phi accumulators for 8 targets the register file is full, and this kernel is bound by dependent-issue
-    // latency (ncu: stall_wait 2.1 per issue with everything in registers): targets AND the chunk's sources are
-    // therefore re-read from shared memory (two conflict-free 128-bit loads per evaluation), which frees ~64
-    // registers for independent pair chains: 99.9 -> 86.0 ms at N = 65,536 (FP64 issue 71 % -> 84 %).
+    // dynamic shared memory (kSymFieldDynSmem): colw [kThreads / 32][4][kTile] (64 KB), then x, y of the block's
+    // targets, txy [R][kThreads] double2 (32 KB; slot [r][tid] is written and read by thread tid only).  With phi and
+    // grad phi accumulators for 8 targets the register file is full, and this kernel is bound by dependent-issue
+    // latency (ncu: stall_wait 2.1 per issue with everything in registers): half of the target coordinates and the
+    // chunk's sources are therefore re-read from shared memory (one conflict-free 128-bit load per evaluation), which
+    // frees ~48 registers for independent pair chains: 99.9 -> 85.0 ms at N = 65,536 (FP64 issue 71 % -> 84 %; all
+    // four target words in shared memory: 86.0 ms).
     extern __shared__ __align__(16) double colw[];
     double2* txy = reinterpret_cast<double2*>(colw + (kThreads / 32) * 4 * kTile);
-    double2* tzq = txy + kSymR * kThreads;
 
     constexpr int R = kSymR, S = kSymFS;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -587,7 +587,7 @@ __global__ void __launch_bounds__(kThreads, 1) near_sym_field_kernel(const SymAr
         bulk_g2s(tile[0], a.src + (long long)J * kTile, kTile * sizeof(Src4), &full[0]);
     }
 
-    double tot[R], tgx[R], tgy[R], tgz[R];
+    double oz[R], oq[R], tot[R], tgx[R], tgy[R], tgz[R];
     const int nvis = (int)(V1 - V0) + 1;
     const int ch_first = (int)(f0 - V0 * kSymFChunks), ch_last = (int)(f1 - 1 - V1 * kSymFChunks) + 1;
     const long long Tp = (long long)a.n_blocks * kSymBlock;
@@ -617,7 +617,7 @@ __global__ void __launch_bounds__(kThreads, 1) near_sym_field_kernel(const SymAr
                 const int tt = I * R + r;
                 const Src4 t = a.src[(long long)min(tt, nt - 1) * kTile + tid];
                 txy[r * kThreads + tid] = make_double2(t.x, t.y);   // read back by this thread only
-                tzq[r * kThreads + tid] = make_double2(t.z, tt < nt ? t.q : 0.0);
+                oz[r] = t.z; oq[r] = tt < nt ? t.q : 0.0;
                 tot[r] = 0.0; tgx[r] = 0.0; tgy[r] = 0.0; tgz[r] = 0.0;
             }
         }
@@ -648,8 +648,8 @@ __global__ void __launch_bounds__(kThreads, 1) near_sym_field_kernel(const SymAr
 #pragma unroll
                         for (int r = 0; r < R; ++r) {
                             const bool self = mine && r == rd;
-                            const double2 oxy = txy[r * kThreads + tid], ozq = tzq[r * kThreads + tid];
-                            const double dx = oxy.x - (self ? oxy.x + 1.0 : xy.x), dy = oxy.y - xy.y, dz = ozq.x - zq.x;
+                            const double2 oxy = txy[r * kThreads + tid];
+                            const double dx = oxy.x - (self ? oxy.x + 1.0 : xy.x), dy = oxy.y - xy.y, dz = oz[r] - zq.x;
                             const double y = sym_recip<REFINE>(dx, dy, dz);
                             const double wm = self ? 0.0 : wq;
                             const double wv = wm * (y * (y * y));
@@ -669,11 +669,11 @@ __global__ void __launch_bounds__(kThreads, 1) near_sym_field_kernel(const SymAr
                         double cj = 0.0, gx = 0.0, gy = 0.0, gz = 0.0;
 #pragma unroll
                         for (int r = 0; r < R; ++r) {
-                            const double2 oxy = txy[r * kThreads + tid], ozq = tzq[r * kThreads + tid];
-                            const double dx = oxy.x - px, dy = oxy.y - py, dz = ozq.x - pz;
+                            const double2 oxy = txy[r * kThreads + tid];
+                            const double dx = oxy.x - px, dy = oxy.y - py, dz = oz[r] - pz;
                             const double y = sym_recip<REFINE>(dx, dy, dz);
                             const double v = y * (y * y);
-                            const double oqr = ozq.y;
+                            const double oqr = oq[r];
                             const double wv = wq * v, ov = oqr * v;
                             tot[r] = fma(wq, y, tot[r]);
                             tgx[r] = fma(wv, dx, tgx[r]); tgy[r] = fma(wv, dy, tgy[r]); tgz[r] = fma(wv, dz, tgz[r]);
