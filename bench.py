@@ -442,6 +442,58 @@ def run_b200(args, w) -> dict:
     return out if rank == 0 else {}
 
 
+def run_parts(args, w) -> dict:
+    """--parts R: the per-rank device time of the R-rank PART form, measured on ONE GPU one rank at a
+    time -- for each part r the two calls rank r makes (its slice of the check sums, then hsma_evaluate_rest_part),
+    bracketed by CUDA events.  No collectives and no concurrency are involved: it measures how evenly the pair work
+    splits and what a rank computes, not a multi-GPU run (that is `--gpus N` under torchrun)."""
+    import torch
+    import paper_1806_04801_b200 as H
+    from paper_1806_04801_b200 import shard
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    stream = torch.cuda.Stream()
+    R, N = args.parts, w.N
+    with torch.cuda.stream(stream):
+        xyz = torch.as_tensor(np.ascontiguousarray(w.xyz), device=dev)
+        q = torch.as_tensor(np.ascontiguousarray(w.q), device=dev)
+        with H.Plan.from_workload(w, rsqrt_refine=args.refine) as plan:
+            if not H.binding.hsma_plan_part_form_applies(plan.handle, N):
+                raise SystemExit("--parts: the PART form does not apply to this workload (needs N > 7936, whole-cell near set)")
+            Kt = plan.info["check_targets"]
+            phi_ref, U_ref = plan.evaluate(xyz, q, sync=True)
+            total = torch.zeros(N, dtype=torch.float64, device=dev)
+            rows = []
+            for part, (t0, t1) in enumerate(shard.shard_bounds(N, R)):
+                c0, c1 = shard.shard_bounds(Kt, R, align=1)[part]
+                a = torch.empty(N, dtype=torch.float64, device=dev)
+                f = torch.empty(N, 3, dtype=torch.float64, device=dev) if args.forces else None
+                u = torch.empty(1, dtype=torch.float64, device=dev)
+                best = None
+                for _ in range(max(1, args.steps)):
+                    e = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+                    plan.sync()
+                    e[0].record()
+                    H.binding.hsma_check_sums_shard(plan.handle, xyz, q, c0, c1)
+                    e[1].record()
+                    H.binding.hsma_evaluate_rest_part(plan.handle, xyz, q, part, R, t0, t1, a, f, u)
+                    e[2].record()
+                    plan.sync()
+                    t = (e[0].elapsed_time(e[1]), e[1].elapsed_time(e[2]))
+                    best = t if best is None or sum(t) < sum(best) else best
+                rows.append({"part": part, "check_sums_ms": best[0], "rest_part_ms": best[1]})
+                # for the check of the sum: the fit needs ALL check sums (the all-gather of the real run)
+                H.binding.hsma_check_sums_shard(plan.handle, xyz, q, 0, Kt)
+                H.binding.hsma_evaluate_rest_part(plan.handle, xyz, q, part, R, t0, t1, a, f, u)
+                plan.sync()
+                total += a
+            err = float((total - phi_ref).abs().max() / phi_ref.abs().max())
+    slowest = max(r["check_sums_ms"] + r["rest_part_ms"] for r in rows)
+    return {"mode": "parts", "note": "per-rank device time of the PART form, one rank at a time on one GPU; collectives not included",
+            "config": {"workload": w.name, "N": N, "forces": bool(args.forces)}, "n_parts": R, "per_part": rows,
+            "slowest_rank_ms": slowest, "sum_of_parts_vs_evaluate_max_rel": err}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -460,6 +512,9 @@ def main():
                     help="step (b): auto = symmetric form (each unordered pair once) when one rank evaluates all targets "
                          "; ordered = always near_sum_kernel; symmetric = wherever it applies")
     ap.add_argument("--forces", action="store_true", help="time hsma_evaluate_forces (potential + forces) instead")
+    ap.add_argument("--parts", type=int, default=0, metavar="R",
+                    help="one GPU: time what each rank of the R-rank PART form computes, one rank at a time (DESIGN.md 8); "
+                         "prints its own JSON line")
     ap.add_argument("--refine", type=int, default=0, choices=[0, 1, 2], help="hsma_plan_desc.rsqrt_refine")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--stage-timing", default="on", choices=["on", "off"],
@@ -479,6 +534,10 @@ def main():
     if args.impl == "reference":
         if rank == 0:
             print(json.dumps(run_reference(args, w)), flush=True)
+        return
+    if args.parts > 0:
+        if rank == 0:
+            print(json.dumps(run_parts(args, w)), flush=True)
         return
     out = run_b200(args, w)
     if rank == 0:
