@@ -222,10 +222,7 @@ static SymLaunch choose_sym(long long n_tiles, int refine, int part = 0, int n_p
 // The symmetric form pays when most visits are off the diagonal (a diagonal visit costs 11 instructions per ORDERED
 // pair): from 32 source tiles on, and while the cell table fits its shared-memory copy.
 // (the gradient form breaks even at 32 tiles too: 1.01x at N = 8192, 1.13x at 16,384, 1.26x at 262,144)
-static bool sym_applies(long long n_tiles, int C, bool field = false, int form = 0) {
-    (void)field; (void)form;
-    return n_tiles >= 32 && C <= kSymMaxCells;
-}
+static bool sym_applies(long long n_tiles, int C) { return n_tiles >= 32 && C <= kSymMaxCells; }
 
 static Launch choose_node(long long T, long long n_tiles, bool field = false) {
     return choose_launch(T, n_tiles, 4, [field](int R) { return node_resident(R, field); });
@@ -580,6 +577,40 @@ __global__ void node_positions_kernel(const double* __restrict__ nrm, double R, 
 //   kPhaseCheck   H1 + step (a) for the check targets c0 <= i < c1 only, into the plan's pc (pcg); nothing else
 //   kPhaseRest    H1 + fit + mapping + (b) + (c) + finish with the plan's pc (pcg) AS THEY ARE (hsma_set_check_sums)
 enum { kPhaseAll = 0, kPhaseCheck = 1, kPhaseRest = 2 };
+// Buffers of the symmetric form (row partials, column sums, near sum in source order); comps = 4 with the gradient.
+static cudaError_t reserve_sym(hsma_plan* p, const SymLaunch& ss, long long N, size_t comps) {
+    cudaError_t e = p->part_b.reserve((size_t)ss.rows * ss.n_blocks * kSymBlock * comps);
+    if (e == cudaSuccess) e = p->sym_col.reserve((size_t)ss.visits * kTile * comps);
+    if (e == cudaSuccess) e = p->sym_phi.reserve((size_t)N * comps);
+    return e;
+}
+// near_sym(_field)_kernel over the fine units of `ss`, then the gather into p->sym_phi ([N], or [4][N] with the gradient).
+static void launch_sym(hsma_plan* p, const SymLaunch& ss, bool field, int refine, const Cell* cells, int C, long long N,
+                       long long n_tiles, cudaStream_t st) {
+    SymArgs a;
+    a.src = p->src.p; a.n_src = N; a.n_tiles = n_tiles; a.n_blocks = ss.n_blocks; a.cells = cells; a.C = C;
+    a.f_begin = ss.f_begin; a.fine = ss.fine; a.scale = refine == 1 ? 0.5 : 1.0; a.scale_grad = refine == 1 ? -0.25 : -1.0;
+    a.part = p->part_b.p; a.col = p->sym_col.p;
+    if (ss.fine > 0) {
+        if (field) {
+            if (refine == 1) near_sym_field_kernel<1><<<ss.G, kThreads, kSymFieldDynSmem, st>>>(a);
+            else near_sym_field_kernel<2><<<ss.G, kThreads, kSymFieldDynSmem, st>>>(a);
+        } else {
+            if (refine == 1) near_sym_kernel<1><<<ss.G, kThreads, 0, st>>>(a);
+            else near_sym_kernel<2><<<ss.G, kThreads, 0, st>>>(a);
+        }
+        HSMA_COUNT_LAUNCH();
+    }
+    const unsigned gb = (unsigned)((N + 255) / 256);
+    if (field)
+        sym_gather_field_kernel<<<gb, 256, 0, st>>>(p->part_b.p, p->sym_col.p, p->slot_of.p, N, n_tiles, ss.n_blocks, ss.f_begin,
+                                                    ss.fine, ss.G, p->sym_phi.p);
+    else
+        sym_gather_kernel<<<gb, 256, 0, st>>>(p->part_b.p, p->sym_col.p, p->slot_of.p, N, n_tiles, ss.n_blocks, ss.f_begin, ss.fine,
+                                              ss.G, p->sym_phi.p);
+    HSMA_COUNT_LAUNCH();
+}
+
 // part / n_parts (kPhaseRest only, n_parts >= 1 given): the PART form of the multi-GPU path, DESIGN.md 8 -- step (b)
 // in symmetric form over this part's share of the fine units, phi_out [N] = that share + step (c) for t0 <= t < t1.
 static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* q, long long N, long long t0,
@@ -689,9 +720,7 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
         const int refine = p->refine ? p->refine : ((double)N * (double)p->last_images < 4294967296.0 ? 2 : 1);
         const size_t comps = field ? 4 : 1;
         const SymLaunch ss = choose_sym(n_tiles, refine, part, n_parts, field);
-        if (p->part_b.reserve((size_t)ss.rows * ss.n_blocks * kSymBlock * comps) != cudaSuccess ||
-            p->sym_col.reserve((size_t)ss.visits * kTile * comps) != cudaSuccess || p->sym_phi.reserve((size_t)N * comps) != cudaSuccess)
-            return HSMA_ERR_ALLOC;
+        if (reserve_sym(p, ss, N, comps) != cudaSuccess) return HSMA_ERR_ALLOC;
         Launch sc{};
         if (T > 0) {
             sc = choose_node(T, p->node_tiles, field);
@@ -699,27 +728,7 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
         }
         p->last_pair_form = 2;
         MARK(3);
-        SymArgs a;
-        a.src = p->src.p; a.n_src = N; a.n_tiles = n_tiles; a.n_blocks = ss.n_blocks; a.cells = cells_b; a.C = C_b;
-        a.f_begin = ss.f_begin; a.fine = ss.fine; a.scale = refine == 1 ? 0.5 : 1.0; a.scale_grad = refine == 1 ? -0.25 : -1.0;
-        a.part = p->part_b.p; a.col = p->sym_col.p;
-        if (ss.fine > 0) {
-            if (field) {
-                if (refine == 1) near_sym_field_kernel<1><<<ss.G, kThreads, kSymFieldDynSmem, st>>>(a);
-                else near_sym_field_kernel<2><<<ss.G, kThreads, kSymFieldDynSmem, st>>>(a);
-            } else {
-                if (refine == 1) near_sym_kernel<1><<<ss.G, kThreads, 0, st>>>(a);
-                else near_sym_kernel<2><<<ss.G, kThreads, 0, st>>>(a);
-            }
-            HSMA_COUNT_LAUNCH();
-        }
-        if (field)
-            sym_gather_field_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(p->part_b.p, p->sym_col.p, p->slot_of.p, N, n_tiles,
-                                                                                ss.n_blocks, ss.f_begin, ss.fine, ss.G, p->sym_phi.p);
-        else
-            sym_gather_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(p->part_b.p, p->sym_col.p, p->slot_of.p, N, n_tiles,
-                                                                          ss.n_blocks, ss.f_begin, ss.fine, ss.G, p->sym_phi.p);
-        HSMA_COUNT_LAUNCH();
+        launch_sym(p, ss, field, refine, cells_b, C_b, N, n_tiles, st);
         MARK(4);
         if (T > 0)
             launch_node(sc, field, reinterpret_cast<const double*>(p->src.p), 4, p->slot_of.p, T, t0, p->nodes, p->node_tiles, p->part_c.p, st);
@@ -742,15 +751,13 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
         const int refine = p->refine ? p->refine : ((double)N * (double)p->last_images < 4294967296.0 ? 2 : 1);
         // rsqrt_refine = 0: the cubic step while (b) is latency-bound anyway (< 2^32 pairs), Newton above
         const size_t comps = field ? 4 : 1;
-        const bool sym = !p->sphere && p->pair_form != 1 && t0 == 0 && t1 == N && sym_applies(n_tiles, C_b, field, p->pair_form);
+        const bool sym = !p->sphere && p->pair_form != 1 && t0 == 0 && t1 == N && sym_applies(n_tiles, C_b);
         p->last_pair_form = sym ? 2 : 1;
         Launch sb = choose_near(T, n_tiles_near, C_b, refine, field);
         SymLaunch ss{};
         if (sym) {
             ss = choose_sym(n_tiles, refine, 0, 1, field);
-            if (p->part_b.reserve((size_t)ss.rows * ss.n_blocks * kSymBlock * comps) != cudaSuccess ||
-                p->sym_col.reserve((size_t)ss.visits * kTile * comps) != cudaSuccess || p->sym_phi.reserve((size_t)N * comps) != cudaSuccess)
-                return HSMA_ERR_ALLOC;
+            if (reserve_sym(p, ss, N, comps) != cudaSuccess) return HSMA_ERR_ALLOC;
         } else if (p->part_b.reserve((size_t)sb.rows * T * comps) != cudaSuccess) {
             return HSMA_ERR_ALLOC;
         }
@@ -760,27 +767,7 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
         PartLayout layout_b = sb.layout(p->part_b.p);
         if (sym) {
             // every unordered (source, source) pair once: row sums + column sums, then phi_near in source order
-            SymArgs a;
-            a.src = p->src.p; a.n_src = N; a.n_tiles = n_tiles; a.n_blocks = ss.n_blocks; a.cells = cells_b; a.C = C_b;
-            a.f_begin = ss.f_begin; a.fine = ss.fine; a.scale = refine == 1 ? 0.5 : 1.0; a.scale_grad = refine == 1 ? -0.25 : -1.0;
-            a.part = p->part_b.p; a.col = p->sym_col.p;
-            if (ss.fine > 0) {
-                if (field) {
-                    if (refine == 1) near_sym_field_kernel<1><<<ss.G, kThreads, kSymFieldDynSmem, st>>>(a);
-                    else near_sym_field_kernel<2><<<ss.G, kThreads, kSymFieldDynSmem, st>>>(a);
-                } else {
-                    if (refine == 1) near_sym_kernel<1><<<ss.G, kThreads, 0, st>>>(a);
-                    else near_sym_kernel<2><<<ss.G, kThreads, 0, st>>>(a);
-                }
-                HSMA_COUNT_LAUNCH();
-            }
-            if (field)
-                sym_gather_field_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(p->part_b.p, p->sym_col.p, p->slot_of.p, N, n_tiles,
-                                                                                    ss.n_blocks, ss.f_begin, ss.fine, ss.G, p->sym_phi.p);
-            else
-                sym_gather_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(p->part_b.p, p->sym_col.p, p->slot_of.p, N, n_tiles,
-                                                                              ss.n_blocks, ss.f_begin, ss.fine, ss.G, p->sym_phi.p);
-            HSMA_COUNT_LAUNCH();
+            launch_sym(p, ss, field, refine, cells_b, C_b, N, n_tiles, st);
             layout_b = PartLayout{p->sym_phi.p, 1, 1, 1, (int)std::min<long long>(T, 2147483647LL)};
         } else {
             launch_near(sb, field, reinterpret_cast<const double*>(p->src.p), 4, p->slot_of.p, T, t0, P, cells_b, C_b,
