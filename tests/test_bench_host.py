@@ -1,0 +1,37 @@
+"""Host-side accounting of bench.py (no GPU): the unit counts its roofline figures are built from.  `-m "not gpu"`."""
+import importlib.util
+import os
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def bench():
+    spec = importlib.util.spec_from_file_location("bench_module", os.path.join(ROOT, "bench.py"))
+    mod = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mod)
+    return mod
+
+
+@pytest.mark.parametrize("N,C", [(7937, 27), (8192, 27), (9000, 45), (20012, 27), (65536, 27), (262144, 27), (1048876, 125)])
+def test_sym_evaluations_counts_the_visits_of_the_symmetric_kernel(bench, N, C):
+    """block I (8 tiles of 256 packed sources) visits the tiles J >= 8 I; every visit is
+    256 x 2048 x C pair evaluations.  bench.sym_evaluations is the closed form of this walk."""
+    n_tiles = -(-N // 256)
+    n_blocks = -(-n_tiles // 8)
+    visits = sum(1 for I in range(n_blocks) for J in range(n_tiles) if J >= 8 * I)
+    assert bench.sym_evaluations(N, C) == visits * 256 * 2048 * C
+    # every ordered pair interaction is covered: evaluations >= N (N - 1) C / 2, and the excess is the diagonal
+    # visits (done as ordered pairs) plus the padding of the last tile and block
+    assert bench.sym_evaluations(N, C) >= N * (N - 1) * C // 2
+    assert bench.sym_evaluations(N, C) <= (n_blocks * 2048) * (n_tiles * 256) * C // 2 + n_blocks * 8 * 256 * 2048 * C
+
+
+def test_executed_instruction_tables_are_consistent(bench):
+    """Per-unit figures quoted in DESIGN.md 6.1 / 6.6 / 6.12 (FP64-pipe instructions, flops with fma = 2)."""
+    assert bench.EXEC_PAIR[(1, True)] == (9.0, 13.0) and bench.EXEC_PAIR[(2, False)] == (12.0, 18.0)
+    assert bench.EXEC_EVAL_SYM[1] == (11.625, 17.125) and bench.EXEC_EVAL_SYM[2] == (13.625, 21.125)
+    assert bench.EXEC_EVAL_SYM_FIELD[1] == (22.375, 35.25)
+    assert bench.FLOPS_EVAL_SYM == bench.FLOPS_PAIR_CHARGE + 2 and bench.FLOPS_EVAL_SYM_FIELD == bench.FLOPS_PAIR_CHARGE_FIELD + 9
