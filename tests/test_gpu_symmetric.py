@@ -247,3 +247,15 @@ def test_symmetric_forces_random_magnitudes_and_momentum(H):
     F = F.cpu().numpy()
     assert rel_inf(F, r.F) <= 1e-10
     assert np.abs(F.sum(0)).max() < 1e-3 * np.abs(F).max()
+
+
+def test_cell_table_sizes_at_the_limit_of_the_symmetric_form(H):
+    """125 near cells (shell 2,2,2) fit the symmetric kernel's shared-memory table (128 entries); 175 (shell 2,2,3) do
+    not and fall back to the ordered kernel.  Both against the oracle."""
+    for shell, cells, form in (((2, 2, 2), 125, SYMMETRIC), ((2, 2, 3), 175, ORDERED)):
+        w = W.config(2, N=8000).with_(near_shell=shell)
+        r = O.hsma(w)
+        with H.Plan.from_workload(w) as plan:
+            phi, U = plan.evaluate(dev(w.xyz), dev(w.q), sync=True)
+            assert plan.info["near_cells"] == cells and plan.last_pair_form == form
+        assert rel_inf(phi.cpu().numpy(), r.phi) <= PHI_TOL and abs(float(U) - r.U) <= U_TOL * abs(r.U)
