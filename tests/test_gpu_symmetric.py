@@ -127,6 +127,18 @@ def test_symmetric_form_in_a_replayed_graph(H):
             for o in outs[1:]:
                 assert np.array_equal(o[0], outs[0][0]) and o[1] == outs[0][1]
             assert rel_inf(outs[0][0], r.phi) <= PHI_TOL and abs(outs[0][1] - r.U) <= U_TOL * abs(r.U)
+            # the gradient form (64 KB + 32 KB of dynamic shared memory) inside a replayed graph
+            rf = O.hsma(w, forces=True)
+            F = torch.empty(w.N, 3, dtype=torch.float64, device="cuda")
+            before = H.binding.hsma_plan_info(plan.handle)["graph_replays"]
+            Fs = []
+            for _ in range(3):
+                H.hsma_evaluate_forces(plan.handle, xyz, q, phi, F, U)
+                plan.sync()
+                Fs.append(F.cpu().numpy().copy())
+            assert H.binding.hsma_plan_info(plan.handle)["graph_replays"] == before + 2 and plan.last_pair_form == SYMMETRIC
+            assert np.array_equal(Fs[0], Fs[1]) and np.array_equal(Fs[0], Fs[2])
+            assert rel_inf(Fs[0], rf.F) <= 1e-10
             plan.set_pair_form(ORDERED)
             H.hsma_evaluate(plan.handle, xyz, q, phi, U)
             plan.sync()
