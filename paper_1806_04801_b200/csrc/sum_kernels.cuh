@@ -337,8 +337,9 @@ __global__ void __launch_bounds__(kThreads, near_min_ctas(FIELD ? 2 * R : R)) ne
 // tiles J >= I * kSymR.  The block's own tiles ("diagonal" visits) are done as ordered pairs (row sums only,
 // self term masked in the central cell); every later tile gives both.  Per unordered pair (Newton form):
 // 3 DADD + DMUL + 2 DFMA (r2) + MUFU + DMUL (t) + DFMA (g) + DMUL (y) + 2 DFMA = 11 FP64-pipe instructions, i.e.
-// 5.5 per pair interaction against 9 in near_sum_kernel.  Images are made by moving the SOURCE here
-// (flip + shift of 4 sources per cell), so nothing per-cell lives in registers on the target side and the
+// 5.5 per pair interaction against 9 in near_sum_kernel (5.8 with the per-source work below).  Images are made
+// by moving the SOURCE here (p = g o s + shift with g = +-1: one DFMA per coordinate, per source and cell, shared
+// by the 8 targets of the thread), so nothing per-cell lives in registers on the target side and the
 // column sums of a chunk of kSymS sources stay in registers across all cells: one warp reduction per source
 // and tile visit, not per cell.
 // Work decomposition: visits v = (I, J) in block-major order, each cut into kSymChunks chunks of kSymS sources;
