@@ -195,7 +195,8 @@ hsma_status hsma_evaluate_rest_shard(hsma_plan* plan, const double* xyz, const d
  * (or NULL) are PARTIAL: their sums over the parts are phi, F and U -- the caller all-reduces them (2 MB / 6 MB at
  * N = 262,144).  Same arithmetic on every part count; results differ from the one-rank
  * evaluate only in the order of the sums.  Needs what the symmetric form needs: hsma_plan_part_form_applies(plan, N)
- * returns 1 if so (whole-cell near set, N > 7936, <= 128 near cells), else 0 (use hsma_evaluate_rest_shard);
+ * returns 1 if so (whole-cell near set, N > 7936, <= 128 near cells, pair form not forced to ordered), else 0 (use
+ * hsma_evaluate_rest_shard);
  * HSMA_ERR_INVALID_ARG otherwise.
  */
 hsma_status hsma_evaluate_rest_part(hsma_plan* plan, const double* xyz, const double* q, long long N, int part,

@@ -915,7 +915,7 @@ extern "C" hsma_status hsma_evaluate_rest_part(hsma_plan* plan, const double* xy
 }
 extern "C" int hsma_plan_part_form_applies(const hsma_plan* p, long long N) {
     if (!p || N < 1) return 0;
-    return !p->sphere && sym_applies((N + kTile - 1) / kTile, p->C_near) ? 1 : 0;
+    return !p->sphere && p->pair_form != 1 && sym_applies((N + kTile - 1) / kTile, p->C_near) ? 1 : 0;
 }
 
 extern "C" hsma_status hsma_plan_sync(hsma_plan* plan) {

@@ -205,6 +205,12 @@ def test_evaluate_distributed_single_process_uses_the_part_form(H):
         phi, F, U = shard.evaluate_distributed(plan, xyz, q)
         plan.sync()
         assert F is None and plan.last_pair_form == SYMMETRIC
+        plan.set_pair_form(ORDERED)             # forced ordered pairs: the distributed call takes the target-shard path
+        assert not H.binding.hsma_plan_part_form_applies(plan.handle, w.N)
+        phi_o, _, U_o = shard.evaluate_distributed(plan, xyz, q)
+        plan.sync()
+        assert plan.last_pair_form == ORDERED and rel_inf(phi_o.cpu().numpy(), phi_ref.cpu().numpy()) <= 2e-11
+        plan.set_pair_form(0)
         phi_f, F_f, U_f = shard.evaluate_distributed(plan, xyz, q, forces=True)
         plan.sync()
         _, F_ref, _ = plan.evaluate_forces(xyz, q, sync=True)
