@@ -278,6 +278,28 @@ hsma_status hsma_plan_get_timing(hsma_plan* plan, double* ms_out);
 hsma_status hsma_plan_set_pair_form(hsma_plan* plan, int form);
 int hsma_plan_last_pair_form(const hsma_plan* plan);
 
+/*
+ * Scratch of the symmetric form.  The unordered pairs of one rank are walked in "waves" (launches);
+ * each wave keeps one column-sum line (2 KB; 8 KB with forces) per (target block, source tile) visit it makes and is
+ * followed by a gather that adds its row and column sums into the near potential in a fixed order.  The number of waves
+ * is chosen so that the column scratch of a wave stays below `bytes` (default and bytes = 0: 64 MiB; a wave never
+ * spans fewer than 2 visits), so the plan's scratch is O(N): sources 32 B, slots 4 B, near sum 8 B (32 B with forces)
+ * per source, a few partial rows, plus this cap -- not the O(N^2 / 10^6) x 2 KB of a single launch.  If the scratch
+ * cannot be allocated, form 0 (automatic) falls back to the ordered-pair kernel; form 2 returns HSMA_ERR_ALLOC.
+ * Results are bit-reproducible for a given (N, cap); two different caps agree to rounding (<= 1e-13 relative).
+ * hsma_plan_scratch_bytes: bytes of per-evaluate scratch the plan holds right now (grown to the largest N seen).
+ */
+hsma_status hsma_plan_set_sym_scratch_cap(hsma_plan* plan, long long bytes);
+long long hsma_plan_scratch_bytes(const hsma_plan* plan);
+
+/*
+ * Thread safety: a plan (and the stream it was created on) must be used by one host thread at a time; different
+ * plans may be driven from different host threads (the only process-wide state, the launch counter and the
+ * allocation epoch that invalidates captured graphs, is atomic).  Host synchronisation: hsma_evaluate* enqueue work
+ * and return, EXCEPT that the first call at a larger N than any before grows the plan's scratch (cudaFree +
+ * cudaMalloc: an implicit device synchronisation), and that the sphere-culled near set reads its image count back.
+ */
+
 /* total number of kernels this library has launched in this process */
 long long hsma_launch_count(void);
 

@@ -121,6 +121,14 @@ class Plan:
         """0: automatic; 1: ordered pairs always; 2: symmetric form of step (b) wherever it applies (forces too)."""
         binding.hsma_plan_set_pair_form(self.handle, form)
 
+    def set_sym_scratch_cap(self, nbytes: int):
+        """Bytes of column-sum scratch per wave of the symmetric form (0: default 64 MiB)."""
+        binding.hsma_plan_set_sym_scratch_cap(self.handle, nbytes)
+
+    @property
+    def scratch_bytes(self) -> int:
+        return binding.hsma_plan_scratch_bytes(self.handle)
+
     @property
     def last_pair_form(self) -> int:
         return binding.hsma_plan_last_pair_form(self.handle)

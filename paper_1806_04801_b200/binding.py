@@ -105,6 +105,8 @@ _SIGNATURES = {
     "hsma_plan_set_timing": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int]),
     "hsma_plan_set_pair_form": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int]),
     "hsma_plan_last_pair_form": (ctypes.c_int, [ctypes.c_void_p]),
+    "hsma_plan_set_sym_scratch_cap": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_longlong]),
+    "hsma_plan_scratch_bytes": (ctypes.c_longlong, [ctypes.c_void_p]),
     "hsma_plan_get_timing": (ctypes.c_int, [ctypes.c_void_p, c_double_p]),
     "hsma_launch_count": (ctypes.c_longlong, []),
 }
@@ -421,6 +423,15 @@ def hsma_plan_set_pair_form(plan: int, form: int):
 def hsma_plan_last_pair_form(plan: int) -> int:
     """What the last evaluate used for step (b): 1 ordered pairs, 2 symmetric (each unordered pair once)."""
     return int(load_library().hsma_plan_last_pair_form(plan))
+
+
+def hsma_plan_set_sym_scratch_cap(plan: int, nbytes: int):
+    """Column-sum scratch per wave of the symmetric form, bytes (0: the default 64 MiB); include/hsma.h."""
+    _check(load_library().hsma_plan_set_sym_scratch_cap(plan, int(nbytes)), "hsma_plan_set_sym_scratch_cap")
+
+
+def hsma_plan_scratch_bytes(plan: int) -> int:
+    return int(load_library().hsma_plan_scratch_bytes(plan))
 
 
 def hsma_plan_get_timing(plan: int) -> dict:

@@ -3,10 +3,12 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <atomic>
+
 namespace hsma {
 
 // ---- launch accounting (hsma_launch_count) --------------------------------------------------
-extern long long g_launches;
+extern std::atomic<long long> g_launches;
 #define HSMA_COUNT_LAUNCH() (++::hsma::g_launches)
 
 // ---- geometry of the all-pairs kernels ------------------------------------------------------

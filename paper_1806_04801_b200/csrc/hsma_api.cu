@@ -2,6 +2,7 @@
 // PAPER.md:142).  Host orchestration only; every arithmetic step of the path is a kernel in
 // sum_kernels.cuh / fit_kernels.cuh.  No CPU fallback exists.
 #include <algorithm>
+#include <atomic>
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -15,14 +16,16 @@
 #include "sum_kernels.cuh"
 
 namespace hsma {
-long long g_launches = 0;
+std::atomic<long long> g_launches{0};
 
 #define CU(x)                                     \
     do {                                          \
         if ((x) != cudaSuccess) return HSMA_ERR_CUDA; \
     } while (0)
 
-static size_t g_alloc_epoch = 0;  // bumped whenever any plan buffer is (re)allocated: captured graphs hold raw pointers
+// bumped whenever any plan buffer is (re)allocated: captured graphs hold raw pointers.  Process-wide and atomic: a bump by
+// another plan (another host thread) only drops this plan's graph, it can never be missed.
+static std::atomic<size_t> g_alloc_epoch{0};
 
 template <class T>
 struct DevBuf {  // growable device buffer owned by the plan
@@ -171,11 +174,18 @@ static Launch choose_near(long long T, long long n_tiles, int C, int refine, boo
     return choose_launch(T, n_tiles * C, field ? 4 : 8, [refine, field](int R) { return near_resident(R, refine, field); });
 }
 
-// Symmetric form of step (b) (sum_kernels.cuh near_sym_kernel): launch shape and buffers.
+// Symmetric form of step (b) (sum_kernels.cuh near_sym_kernel): launch shape and buffers.  The fine units of one rank
+// are walked in `waves` (launches) of at most wave_fine units each, so that the column-sum scratch (one 2 KB line per
+// visit of a wave; 8 KB with the gradient) stays below the plan's cap whatever N is: O(N) memory, DESIGN.md 6.12.
 struct SymLaunch {
-    int n_blocks, G, rows;
+    int n_blocks, rows, chunks;
     long long visits, f_begin, fine;
+    int n_waves, resident;
+    long long wave_fine;       // fine units per wave (the last one takes what is left)
+    long long wave_visits;     // column lines to reserve: max over waves of (last visit - first visit + 1)
+    int wave_blocks;           // row-sum blocks to reserve: max over waves of the blocks a wave touches
 };
+constexpr size_t kSymColCapDefault = 64u << 20;   // bytes of column scratch per wave (fits L2 beside the sources)
 static int sym_resident(int refine) {
     static int cache[2] = {0, 0};
     int& c = cache[refine == 1 ? 0 : 1];
@@ -199,23 +209,56 @@ static int sym_field_resident(int refine) {
     if (!c) c = refine == 1 ? sym_field_resident_of<1>() : sym_field_resident_of<2>();
     return c;
 }
+static int sym_block_of_visit(long long v, long long n_tiles, int n_blocks) {
+    int lo = 0, hi = n_blocks - 1;   // largest I with sym_visit0(I) <= v
+    while (lo < hi) {
+        const int mid = (lo + hi + 1) / 2;
+        if (sym_visit0(mid, n_tiles) <= v) lo = mid; else hi = mid - 1;
+    }
+    return lo;
+}
+// wave w of a launch shape
+static SymWave sym_wave(const SymLaunch& L, long long n_tiles, int w) {
+    SymWave W;
+    W.f_begin = L.f_begin + (long long)w * L.wave_fine;
+    W.fine = std::min(L.wave_fine, L.f_begin + L.fine - W.f_begin);
+    W.v_base = W.f_begin / L.chunks;
+    const long long v_last = (W.f_begin + W.fine - 1) / L.chunks;
+    W.blk_lo = sym_block_of_visit(W.v_base, n_tiles, L.n_blocks);
+    W.blk_hi = sym_block_of_visit(v_last, n_tiles, L.n_blocks);
+    W.G = (int)std::max<long long>(1, std::min<long long>(L.resident, W.fine));
+    W.first = w == 0;
+    return W;
+}
 // part / n_parts: the contiguous share [F * part / n_parts, F * (part + 1) / n_parts) of the F fine units (multi-GPU)
-static SymLaunch choose_sym(long long n_tiles, int refine, int part = 0, int n_parts = 1, bool field = false) {
+static SymLaunch choose_sym(long long n_tiles, int refine, size_t col_cap_bytes, int part = 0, int n_parts = 1, bool field = false) {
     SymLaunch L;
-    const int chunks = field ? kSymFChunks : kSymChunks;
+    L.chunks = field ? kSymFChunks : kSymChunks;
     L.n_blocks = (int)((n_tiles + kSymR - 1) / kSymR);
     L.visits = sym_visit0(L.n_blocks, n_tiles);
-    const long long F = L.visits * chunks;
+    const long long F = L.visits * L.chunks;
     L.f_begin = F * part / n_parts;
     L.fine = F * (part + 1) / n_parts - L.f_begin;
-    L.G = (int)std::max<long long>(1, std::min<long long>(field ? sym_field_resident(refine) : sym_resident(refine), L.fine));
-    L.rows = 1;
-    for (int I = 0; I < L.n_blocks && L.fine > 0; ++I) {
-        const long long lo = std::max(sym_visit0(I, n_tiles) * chunks, L.f_begin);
-        const long long hi = std::min(sym_visit0(I + 1, n_tiles) * chunks, L.f_begin + L.fine);
-        if (lo >= hi) continue;
-        const int first = cta_of_unit(lo - L.f_begin, L.fine, L.G), last = cta_of_unit(hi - 1 - L.f_begin, L.fine, L.G);
-        L.rows = std::max(L.rows, last - first + 1);
+    L.resident = field ? sym_field_resident(refine) : sym_resident(refine);
+    // waves: equal shares of the fine units, each spanning at most cap / line bytes visits (and at least 2 visits)
+    const long long line = (long long)kTile * sizeof(double) * (field ? 4 : 1);
+    const long long cap_visits = std::max<long long>(2, (long long)(col_cap_bytes / (size_t)line));
+    const long long my_visits = L.fine > 0 ? (L.f_begin + L.fine - 1) / L.chunks - L.f_begin / L.chunks + 1 : 0;
+    L.n_waves = (int)std::max<long long>(1, (my_visits + cap_visits - 2) / (cap_visits - 1));
+    L.wave_fine = std::max<long long>(1, (L.fine + L.n_waves - 1) / L.n_waves);
+    L.n_waves = L.fine > 0 ? (int)((L.fine + L.wave_fine - 1) / L.wave_fine) : 0;
+    L.rows = 1; L.wave_visits = 1; L.wave_blocks = 1;
+    for (int w = 0; w < L.n_waves; ++w) {
+        const SymWave W = sym_wave(L, n_tiles, w);
+        L.wave_visits = std::max(L.wave_visits, (W.f_begin + W.fine - 1) / L.chunks - W.v_base + 1);
+        L.wave_blocks = std::max(L.wave_blocks, W.blk_hi - W.blk_lo + 1);
+        for (int I = W.blk_lo; I <= W.blk_hi; ++I) {
+            const long long lo = std::max(sym_visit0(I, n_tiles) * L.chunks, W.f_begin);
+            const long long hi = std::min(sym_visit0(I + 1, n_tiles) * L.chunks, W.f_begin + W.fine);
+            if (lo >= hi) continue;
+            const int first = cta_of_unit(lo - W.f_begin, W.fine, W.G), last = cta_of_unit(hi - 1 - W.f_begin, W.fine, W.G);
+            L.rows = std::max(L.rows, last - first + 1);
+        }
     }
     return L;
 }
@@ -290,7 +333,8 @@ struct hsma_plan {
     DevBuf<int> slot_of, tile_np;
     QInfo* qinfo = nullptr;
     DevBuf<double> part_a, part_b, part_c, red, xyz_in, q_in, phi_dev, force_dev;
-    DevBuf<double> sym_col, sym_phi;   // symmetric form of step (b): column sums per visit, phi_near in source order
+    DevBuf<double> sym_col, sym_phi;   // symmetric form of step (b): column sums per visit of one wave, phi_near in source order
+    size_t sym_col_cap = kSymColCapDefault;   // hsma_plan_set_sym_scratch_cap: bytes of column scratch per wave
     int pair_form = 0;                 // hsma_plan_set_pair_form: 0 = automatic, 1 = ordered pairs only, 2 = symmetric wherever possible
     int last_pair_form = 1;            // what the last evaluate used for step (b): 1 ordered, 2 symmetric
     long long last_launches = 0;
@@ -577,38 +621,43 @@ __global__ void node_positions_kernel(const double* __restrict__ nrm, double R, 
 //   kPhaseCheck   H1 + step (a) for the check targets c0 <= i < c1 only, into the plan's pc (pcg); nothing else
 //   kPhaseRest    H1 + fit + mapping + (b) + (c) + finish with the plan's pc (pcg) AS THEY ARE (hsma_set_check_sums)
 enum { kPhaseAll = 0, kPhaseCheck = 1, kPhaseRest = 2 };
-// Buffers of the symmetric form (row partials, column sums, near sum in source order); comps = 4 with the gradient.
+// Buffers of the symmetric form (row partials and column sums of ONE wave, near sum in source order); comps = 4 with
+// the gradient.  Bounded by the plan's cap on the column scratch: O(N) in all.
 static cudaError_t reserve_sym(hsma_plan* p, const SymLaunch& ss, long long N, size_t comps) {
-    cudaError_t e = p->part_b.reserve((size_t)ss.rows * ss.n_blocks * kSymBlock * comps);
-    if (e == cudaSuccess) e = p->sym_col.reserve((size_t)ss.visits * kTile * comps);
+    cudaError_t e = p->part_b.reserve((size_t)ss.rows * ss.wave_blocks * kSymBlock * comps);
+    if (e == cudaSuccess) e = p->sym_col.reserve((size_t)ss.wave_visits * kTile * comps);
     if (e == cudaSuccess) e = p->sym_phi.reserve((size_t)N * comps);
     return e;
 }
-// near_sym(_field)_kernel over the fine units of `ss`, then the gather into p->sym_phi ([N], or [4][N] with the gradient).
+// near_sym(_field)_kernel over the fine units of `ss`, wave by wave, each followed by its gather into p->sym_phi ([N], or
+// [4][N] with the gradient): the first wave writes, the others add, in wave order (deterministic).
 static void launch_sym(hsma_plan* p, const SymLaunch& ss, bool field, int refine, const Cell* cells, int C, long long N,
                        long long n_tiles, cudaStream_t st) {
     SymArgs a;
     a.src = p->src.p; a.n_src = N; a.n_tiles = n_tiles; a.n_blocks = ss.n_blocks; a.cells = cells; a.C = C;
-    a.f_begin = ss.f_begin; a.fine = ss.fine; a.scale = refine == 1 ? 0.5 : 1.0; a.scale_grad = refine == 1 ? -0.25 : -1.0;
+    a.scale = refine == 1 ? 0.5 : 1.0; a.scale_grad = refine == 1 ? -0.25 : -1.0;
     a.part = p->part_b.p; a.col = p->sym_col.p;
-    if (ss.fine > 0) {
+    const unsigned gb = (unsigned)((N + 255) / 256);
+    if (ss.n_waves == 0) {   // a part with no fine units: its share of the near sum is zero
+        cudaMemsetAsync(p->sym_phi.p, 0, (size_t)N * (field ? 4 : 1) * sizeof(double), st);
+        return;
+    }
+    for (int w = 0; w < ss.n_waves; ++w) {
+        const SymWave W = sym_wave(ss, n_tiles, w);
+        a.f_begin = W.f_begin; a.fine = W.fine; a.v_base = W.v_base; a.blk_base = W.blk_lo; a.part_blocks = W.blk_hi - W.blk_lo + 1;
         if (field) {
-            if (refine == 1) near_sym_field_kernel<1><<<ss.G, kThreads, kSymFieldDynSmem, st>>>(a);
-            else near_sym_field_kernel<2><<<ss.G, kThreads, kSymFieldDynSmem, st>>>(a);
+            if (refine == 1) near_sym_field_kernel<1><<<W.G, kThreads, kSymFieldDynSmem, st>>>(a);
+            else near_sym_field_kernel<2><<<W.G, kThreads, kSymFieldDynSmem, st>>>(a);
+            HSMA_COUNT_LAUNCH();
+            sym_gather_field_kernel<<<gb, 256, 0, st>>>(p->part_b.p, p->sym_col.p, p->slot_of.p, N, n_tiles, W, p->sym_phi.p);
         } else {
-            if (refine == 1) near_sym_kernel<1><<<ss.G, kThreads, 0, st>>>(a);
-            else near_sym_kernel<2><<<ss.G, kThreads, 0, st>>>(a);
+            if (refine == 1) near_sym_kernel<1><<<W.G, kThreads, 0, st>>>(a);
+            else near_sym_kernel<2><<<W.G, kThreads, 0, st>>>(a);
+            HSMA_COUNT_LAUNCH();
+            sym_gather_kernel<<<gb, 256, 0, st>>>(p->part_b.p, p->sym_col.p, p->slot_of.p, N, n_tiles, W, p->sym_phi.p);
         }
         HSMA_COUNT_LAUNCH();
     }
-    const unsigned gb = (unsigned)((N + 255) / 256);
-    if (field)
-        sym_gather_field_kernel<<<gb, 256, 0, st>>>(p->part_b.p, p->sym_col.p, p->slot_of.p, N, n_tiles, ss.n_blocks, ss.f_begin,
-                                                    ss.fine, ss.G, p->sym_phi.p);
-    else
-        sym_gather_kernel<<<gb, 256, 0, st>>>(p->part_b.p, p->sym_col.p, p->slot_of.p, N, n_tiles, ss.n_blocks, ss.f_begin, ss.fine,
-                                              ss.G, p->sym_phi.p);
-    HSMA_COUNT_LAUNCH();
 }
 
 // part / n_parts (kPhaseRest only, n_parts >= 1 given): the PART form of the multi-GPU path, DESIGN.md 8 -- step (b)
@@ -719,7 +768,7 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
         if (p->sphere || !sym_applies(n_tiles, C_b) || part < 0 || part >= n_parts || (!phi_out && !field)) return HSMA_ERR_INVALID_ARG;
         const int refine = p->refine ? p->refine : ((double)N * (double)p->last_images < 4294967296.0 ? 2 : 1);
         const size_t comps = field ? 4 : 1;
-        const SymLaunch ss = choose_sym(n_tiles, refine, part, n_parts, field);
+        const SymLaunch ss = choose_sym(n_tiles, refine, p->sym_col_cap, part, n_parts, field);
         if (reserve_sym(p, ss, N, comps) != cudaSuccess) return HSMA_ERR_ALLOC;
         Launch sc{};
         if (T > 0) {
@@ -751,16 +800,20 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
         const int refine = p->refine ? p->refine : ((double)N * (double)p->last_images < 4294967296.0 ? 2 : 1);
         // rsqrt_refine = 0: the cubic step while (b) is latency-bound anyway (< 2^32 pairs), Newton above
         const size_t comps = field ? 4 : 1;
-        const bool sym = !p->sphere && p->pair_form != 1 && t0 == 0 && t1 == N && sym_applies(n_tiles, C_b);
-        p->last_pair_form = sym ? 2 : 1;
+        bool sym = !p->sphere && p->pair_form != 1 && t0 == 0 && t1 == N && sym_applies(n_tiles, C_b);
         Launch sb = choose_near(T, n_tiles_near, C_b, refine, field);
         SymLaunch ss{};
         if (sym) {
-            ss = choose_sym(n_tiles, refine, 0, 1, field);
-            if (reserve_sym(p, ss, N, comps) != cudaSuccess) return HSMA_ERR_ALLOC;
-        } else if (p->part_b.reserve((size_t)sb.rows * T * comps) != cudaSuccess) {
-            return HSMA_ERR_ALLOC;
+            ss = choose_sym(n_tiles, refine, p->sym_col_cap, 0, 1, field);
+            if (reserve_sym(p, ss, N, comps) != cudaSuccess) {
+                // never fail where the ordered kernel would succeed: in automatic mode fall back to it
+                cudaGetLastError();
+                if (p->pair_form == 2) return HSMA_ERR_ALLOC;
+                sym = false;
+            }
         }
+        if (!sym && p->part_b.reserve((size_t)sb.rows * T * comps) != cudaSuccess) return HSMA_ERR_ALLOC;
+        p->last_pair_form = sym ? 2 : 1;
         const Launch sc = choose_node(T, p->node_tiles, field);
         if (p->part_c.reserve((size_t)sc.rows * T * comps) != cudaSuccess) return HSMA_ERR_ALLOC;
         MARK(3);
@@ -1203,6 +1256,21 @@ extern "C" hsma_status hsma_plan_set_pair_form(hsma_plan* p, int form) {
 }
 
 extern "C" int hsma_plan_last_pair_form(const hsma_plan* p) { return p ? p->last_pair_form : 0; }
+
+extern "C" hsma_status hsma_plan_set_sym_scratch_cap(hsma_plan* p, long long bytes) {
+    if (!p || bytes < 0) return HSMA_ERR_INVALID_ARG;
+    p->sym_col_cap = bytes == 0 ? kSymColCapDefault : (size_t)bytes;
+    ++g_alloc_epoch;   // a captured evaluate graph holds the old wave structure
+    return HSMA_OK;
+}
+extern "C" long long hsma_plan_scratch_bytes(const hsma_plan* p) {
+    if (!p) return 0;
+    size_t b = p->src.cap * sizeof(Src4) + (p->slot_of.cap + p->tile_np.cap) * sizeof(int) +
+               (p->part_a.cap + p->part_b.cap + p->part_c.cap + p->red.cap + p->sym_col.cap + p->sym_phi.cap) * sizeof(double) +
+               p->img_counts.cap * sizeof(long long) + (p->img_xyz.cap + p->img_q.cap + p->img_stats.cap) * sizeof(double) +
+               p->img_src.cap * sizeof(Src4) + (p->img_slot_of.cap + p->img_tile_np.cap) * sizeof(int);
+    return (long long)b;
+}
 
 extern "C" hsma_status hsma_plan_get_timing(hsma_plan* p, double* ms_out) {
     if (!p || !ms_out || !p->timing || !p->ev_valid) return HSMA_ERR_INVALID_ARG;

@@ -366,8 +366,12 @@ struct SymArgs {
     long long fine;      // kSymChunks in all (one rank: everything; R ranks: a contiguous 1/R each)
     double scale;        // 0.5 for the Newton form (y is twice the reciprocal distance)
     double scale_grad;   // gradient form only: -1/4 (Newton), -1 (cubic)
-    double* part;        // [rows][n_blocks * kSymBlock]              (gradient form: [rows][4][...])
-    double* col;         // [visits][kTile]                           (gradient form: [visits][4][kTile])
+    // One launch ("wave") walks a bounded range of fine units, so its scratch is bounded too: the
+    // row sums of the blocks blk_base .. blk_base + part_blocks - 1 and one column line per visit from v_base on.
+    int blk_base, part_blocks;
+    long long v_base;
+    double* part;        // [rows][part_blocks * kSymBlock]           (gradient form: [rows][4][...])
+    double* col;         // [visits of the wave][kTile]               (gradient form: [visits][4][kTile])
 };
 
 template <int REFINE>
@@ -422,12 +426,12 @@ __global__ void __launch_bounds__(kThreads, 1) near_sym_kernel(const SymArgs a) 
     double ox[R], oy[R], oz[R], oq[R], tot[R];
     const int nvis = (int)(V1 - V0) + 1;
     const int ch_first = (int)(f0 - V0 * kSymChunks), ch_last = (int)(f1 - 1 - V1 * kSymChunks) + 1;
-    const long long Tp = (long long)a.n_blocks * kSymBlock;
+    const long long Tp = (long long)a.part_blocks * kSymBlock;
     bool fresh = true;
     auto store_block = [&](int blk) {
         const int row = k - cta_of_unit(max(sym_visit0(blk, nt) * kSymChunks, a.f_begin) - a.f_begin, a.fine, G);
 #pragma unroll
-        for (int r = 0; r < R; ++r) a.part[(long long)row * Tp + (long long)blk * kSymBlock + r * kThreads + tid] = tot[r];
+        for (int r = 0; r < R; ++r) a.part[(long long)row * Tp + (long long)(blk - a.blk_base) * kSymBlock + r * kThreads + tid] = tot[r];
     };
 
     for (int it = 0; it < nvis; ++it) {
@@ -519,7 +523,7 @@ __global__ void __launch_bounds__(kThreads, 1) near_sym_kernel(const SymArgs a) 
                 double v = 0.0;
 #pragma unroll
                 for (int w = 0; w < kThreads / 32; ++w) v += colw[w][j];
-                a.col[(V0 + it) * kTile + j] = v;
+                a.col[(V0 + it - a.v_base) * kTile + j] = v;
             }
             __syncthreads();  // colw is rewritten by the next visit
         }
@@ -591,14 +595,14 @@ __global__ void __launch_bounds__(kThreads, 1) near_sym_field_kernel(const SymAr
     double oz[R], oq[R], tot[R], tgx[R], tgy[R], tgz[R];
     const int nvis = (int)(V1 - V0) + 1;
     const int ch_first = (int)(f0 - V0 * kSymFChunks), ch_last = (int)(f1 - 1 - V1 * kSymFChunks) + 1;
-    const long long Tp = (long long)a.n_blocks * kSymBlock;
+    const long long Tp = (long long)a.part_blocks * kSymBlock;
     const double sg = a.scale_grad;   // gradient sums -> grad phi: -1/4 (Newton: v = 8/|d|^3 against the 1/2 in w), -1 (cubic)
     bool fresh = true;
     auto store_block = [&](int blk) {
         const int row = k - cta_of_unit(max(sym_visit0(blk, nt) * kSymFChunks, a.f_begin) - a.f_begin, a.fine, G);
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            double* o = a.part + (long long)row * 4 * Tp + (long long)blk * kSymBlock + r * kThreads + tid;
+            double* o = a.part + (long long)row * 4 * Tp + (long long)(blk - a.blk_base) * kSymBlock + r * kThreads + tid;
             o[0] = tot[r]; o[Tp] = sg * tgx[r]; o[2 * Tp] = sg * tgy[r]; o[3 * Tp] = sg * tgz[r];
         }
     };
@@ -628,7 +632,7 @@ __global__ void __launch_bounds__(kThreads, 1) near_sym_field_kernel(const SymAr
         const Src4* __restrict__ s = tile[st];
         const int ch_lo = it == 0 ? ch_first : 0;
         const int ch_hi = it == nvis - 1 ? ch_last : kSymFChunks;
-        double* colv = a.col + (V0 + it) * 4 * kTile;
+        double* colv = a.col + (V0 + it - a.v_base) * 4 * kTile;
 
         for (int ch = ch_lo; ch < ch_hi; ++ch) {
             const int j0 = ch * S;
@@ -727,56 +731,71 @@ __global__ void __launch_bounds__(kThreads, 1) near_sym_field_kernel(const SymAr
     if (!fresh) store_block(I);
 }
 
+// What one wave (launch) of the symmetric kernels left behind, for the gathers below.
+struct SymWave {
+    long long f_begin, fine;   // fine units of the wave
+    long long v_base;          // first visit of the wave (column line 0)
+    int blk_lo, blk_hi;        // blocks the wave's visits belong to (row sums: part_blocks = blk_hi - blk_lo + 1)
+    int G;                     // CTAs of the wave
+    int first;                 // 1: the first wave of the evaluate (out is written, not added to)
+};
+
 // FIELD form of sym_gather_kernel: out[comp * N + t], comp 0 = phi, 1..3 = grad phi, original source order.
 __global__ void sym_gather_field_kernel(const double* __restrict__ part, const double* __restrict__ col,
-                                        const int* __restrict__ slot_of, long long N, long long n_tiles, int n_blocks,
-                                        long long f_begin, long long fine, int G, double* __restrict__ out) {
+                                        const int* __restrict__ slot_of, long long N, long long n_tiles, const SymWave w,
+                                        double* __restrict__ out) {
     const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= N) return;
     const long long p = slot_of[t];
     const int I = (int)(p / kSymBlock), J = (int)(p / kTile), j = (int)(p % kTile);
-    const long long Tp = (long long)n_blocks * kSymBlock;
-    const long long f_end = f_begin + fine;
+    const long long Tp = (long long)(w.blk_hi - w.blk_lo + 1) * kSymBlock;
+    const long long f_end = w.f_begin + w.fine;
     double v[4] = {0.0, 0.0, 0.0, 0.0};
-    const long long lo = max(sym_visit0(I, n_tiles) * kSymFChunks, f_begin), hi = min(sym_visit0(I + 1, n_tiles) * kSymFChunks, f_end);
+    if (!w.first) {
+#pragma unroll
+        for (int c = 0; c < 4; ++c) v[c] = out[c * N + t];
+    }
+    const long long lo = max(sym_visit0(I, n_tiles) * kSymFChunks, w.f_begin), hi = min(sym_visit0(I + 1, n_tiles) * kSymFChunks, f_end);
     if (lo < hi) {
-        const int first = cta_of_unit(lo - f_begin, fine, G), last = cta_of_unit(hi - 1 - f_begin, fine, G);
+        const int first = cta_of_unit(lo - w.f_begin, w.fine, w.G), last = cta_of_unit(hi - 1 - w.f_begin, w.fine, w.G);
+        const long long pw = p - (long long)w.blk_lo * kSymBlock;
         for (int r = 0; r <= last - first; ++r)
 #pragma unroll
-            for (int c = 0; c < 4; ++c) v[c] += part[((long long)r * 4 + c) * Tp + p];
+            for (int c = 0; c < 4; ++c) v[c] += part[((long long)r * 4 + c) * Tp + pw];
     }
-    for (int b = 0; b < I; ++b) {
+    for (int b = w.blk_lo; b <= min(w.blk_hi, I - 1); ++b) {
         const long long vis = sym_visit0(b, n_tiles) + (J - b * kSymR);
         const long long f = vis * kSymFChunks + j / kSymFS;
-        if (f >= f_begin && f < f_end)
+        if (f >= w.f_begin && f < f_end)
 #pragma unroll
-            for (int c = 0; c < 4; ++c) v[c] += col[(vis * 4 + c) * kTile + j];
+            for (int c = 0; c < 4; ++c) v[c] += col[((vis - w.v_base) * 4 + c) * kTile + j];
     }
 #pragma unroll
     for (int c = 0; c < 4; ++c) out[c * N + t] = v[c];
 }
 
-// phi of step (b) in the ORIGINAL source order: row sums (fixed CTA order) + column sums (blocks in order), of the
-// fine units [f_begin, f_begin + fine) that the launch walked (all of them on one rank: the whole near sum).
+// phi of step (b) in the ORIGINAL source order: for each wave in turn, row sums (fixed CTA order) + column sums (blocks
+// in order) of the fine units the wave walked; over the waves of one rank this adds up to its share of the near sum.
 __global__ void sym_gather_kernel(const double* __restrict__ part, const double* __restrict__ col,
-                                  const int* __restrict__ slot_of, long long N, long long n_tiles, int n_blocks,
-                                  long long f_begin, long long fine, int G, double* __restrict__ out) {
+                                  const int* __restrict__ slot_of, long long N, long long n_tiles, const SymWave w,
+                                  double* __restrict__ out) {
     const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= N) return;
     const long long p = slot_of[t];
     const int I = (int)(p / kSymBlock), J = (int)(p / kTile), j = (int)(p % kTile);
-    const long long Tp = (long long)n_blocks * kSymBlock;
-    const long long f_end = f_begin + fine;
-    double v = 0.0;
-    const long long lo = max(sym_visit0(I, n_tiles) * kSymChunks, f_begin), hi = min(sym_visit0(I + 1, n_tiles) * kSymChunks, f_end);
+    const long long Tp = (long long)(w.blk_hi - w.blk_lo + 1) * kSymBlock;
+    const long long f_end = w.f_begin + w.fine;
+    double v = w.first ? 0.0 : out[t];
+    const long long lo = max(sym_visit0(I, n_tiles) * kSymChunks, w.f_begin), hi = min(sym_visit0(I + 1, n_tiles) * kSymChunks, f_end);
     if (lo < hi) {
-        const int first = cta_of_unit(lo - f_begin, fine, G), last = cta_of_unit(hi - 1 - f_begin, fine, G);
-        for (int r = 0; r <= last - first; ++r) v += part[(long long)r * Tp + p];
+        const int first = cta_of_unit(lo - w.f_begin, w.fine, w.G), last = cta_of_unit(hi - 1 - w.f_begin, w.fine, w.G);
+        const long long pw = p - (long long)w.blk_lo * kSymBlock;
+        for (int r = 0; r <= last - first; ++r) v += part[(long long)r * Tp + pw];
     }
-    for (int b = 0; b < I; ++b) {
+    for (int b = w.blk_lo; b <= min(w.blk_hi, I - 1); ++b) {
         const long long vis = sym_visit0(b, n_tiles) + (J - b * kSymR);
         const long long f = vis * kSymChunks + j / kSymS;
-        if (f >= f_begin && f < f_end) v += col[vis * kTile + j];
+        if (f >= w.f_begin && f < f_end) v += col[(vis - w.v_base) * kTile + j];
     }
     out[t] = v;
 }

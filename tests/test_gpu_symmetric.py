@@ -277,3 +277,91 @@ def test_cell_table_sizes_at_the_limit_of_the_symmetric_form(H):
             phi, U = plan.evaluate(dev(w.xyz), dev(w.q), sync=True)
             assert plan.info["near_cells"] == cells and plan.last_pair_form == form
         assert rel_inf(phi.cpu().numpy(), r.phi) <= PHI_TOL and abs(float(U) - r.U) <= U_TOL * abs(r.U)
+
+
+# ------------------------------------------------------------------ all-element comparisons at sizes where one CTA of
+# the persistent grid walks many (block, tile) visits and crosses block boundaries (the launch regime of config 5)
+def test_symmetric_every_potential_and_force_at_65536(H):
+    """Config-5 recipe at N = 65,536 (256 tiles, 32 blocks, ~28 visits per CTA of each launch, block boundaries
+    crossed inside a CTA): EVERY potential and EVERY force component of the symmetric potential and gradient kernels
+    against the oracle (1.2e11 pairs on the host cores), default refinement (Newton) and the cubic step."""
+    w = W.config(5, N=65536)
+    r = O.hsma(w, forces=True)
+    fscale = float(np.max(np.abs(r.F)))
+    for refine in (0, 2):
+        with H.Plan.from_workload(w, rsqrt_refine=refine) as plan:
+            xyz, q = dev(w.xyz), dev(w.q)
+            phi, U = plan.evaluate(xyz, q, sync=True)
+            assert plan.last_pair_form == SYMMETRIC
+            phi_f, F, U_f = plan.evaluate_forces(xyz, q, sync=True)
+            assert plan.last_pair_form == SYMMETRIC
+        assert rel_inf(phi.cpu().numpy(), r.phi) <= PHI_TOL and abs(float(U) - r.U) <= U_TOL * abs(r.U)
+        assert rel_inf(phi_f.cpu().numpy(), r.phi) <= PHI_TOL and abs(float(U_f) - r.U) <= U_TOL * abs(r.U)
+        assert np.max(np.abs(F.cpu().numpy() - r.F)) <= 1e-10 * fscale
+
+
+@pytest.mark.parametrize("idx,N", [(3, 40961), (4, 43010)])
+def test_symmetric_every_potential_ragged_mirror_and_slab_tables(H, idx, N):
+    """Mirror-cavity (27 reflected cells, gamma = -1) and slab (45 cells, reflected + weighted) tables at ragged sizes
+    above 40k (161 / 169 tiles: a partly filled last tile and a partly filled last block): every potential, every
+    force component and U against the oracle."""
+    w = W.config(idx, N=N)
+    r = O.hsma(w, forces=True)
+    with H.Plan.from_workload(w) as plan:
+        xyz, q = dev(w.xyz), dev(w.q)
+        phi, U = plan.evaluate(xyz, q, sync=True)
+        assert plan.last_pair_form == SYMMETRIC
+        phi_f, F, U_f = plan.evaluate_forces(xyz, q, sync=True)
+        assert plan.last_pair_form == SYMMETRIC
+    assert rel_inf(phi.cpu().numpy(), r.phi) <= PHI_TOL and abs(float(U) - r.U) <= U_TOL * abs(r.U)
+    assert rel_inf(phi_f.cpu().numpy(), r.phi) <= PHI_TOL and abs(float(U_f) - r.U) <= U_TOL * abs(r.U)
+    assert np.max(np.abs(F.cpu().numpy() - r.F)) <= 1e-10 * float(np.max(np.abs(r.F)))
+
+
+# ------------------------------------------------------------------ bounded scratch: the pairs are walked in waves
+@pytest.mark.parametrize("idx,N", [(5, 12288), (4, 9000), (3, 20011)])
+def test_waves_of_the_symmetric_form(H, idx, N):
+    """hsma_plan_set_sym_scratch_cap: with a tiny cap the unordered pairs are walked in many waves (launch + gather
+    each, wave boundaries inside visits and inside blocks); potentials, forces and the PART form agree with the
+    single-wave result to rounding, meet the oracle bars, stay deterministic, and the scratch shrinks."""
+    import torch
+    w = W.config(idx, N=N)
+    r = O.hsma(w, forces=True)
+    fscale = float(np.max(np.abs(r.F)))
+    with H.Plan.from_workload(w) as plan:
+        xyz, q = dev(w.xyz), dev(w.q)
+        phi0, U0 = plan.evaluate(xyz, q, sync=True)
+        _, F0, _ = plan.evaluate_forces(xyz, q, sync=True)
+        launches_one_wave = plan.launches_last_evaluate()
+        big = plan.scratch_bytes
+    for cap in (2 * 2048, 37 * 2048, 301 * 8192):     # 2 / 37 visits per potential wave, 9 / 301 per force wave
+        with H.Plan.from_workload(w) as plan:
+            plan.set_sym_scratch_cap(cap)
+            xyz, q = dev(w.xyz), dev(w.q)
+            phi, U = plan.evaluate(xyz, q, sync=True)
+            assert plan.last_pair_form == SYMMETRIC
+            phi_f, F, U_f = plan.evaluate_forces(xyz, q, sync=True)
+            assert plan.last_pair_form == SYMMETRIC
+            if cap < 100000:
+                assert plan.launches_last_evaluate() > launches_one_wave and plan.scratch_bytes < big
+            phi2, U2 = plan.evaluate(xyz, q, sync=True)
+            assert torch.equal(phi2, phi) and float(U2) == float(U)
+            # PART form on top of the waves: three "ranks" one after the other
+            tot = torch.zeros(w.N, dtype=torch.float64, device="cuda")
+            Ut = 0.0
+            for part in range(3):
+                t0, t1 = part * w.N // 3, (part + 1) * w.N // 3
+                pp = torch.empty(w.N, dtype=torch.float64, device="cuda")
+                Up = torch.empty(1, dtype=torch.float64, device="cuda")
+                H.hsma_check_sums_shard(plan.handle, xyz, q, 0, plan.info["check_targets"])
+                H.hsma_evaluate_rest_part(plan.handle, xyz, q, part, 3, t0, t1, pp, None, Up)
+                plan.sync()
+                tot += pp
+                Ut += float(Up)
+        for got in (phi, phi_f, tot):
+            assert rel_inf(got.cpu().numpy(), r.phi) <= PHI_TOL
+            assert rel_inf(got.cpu().numpy(), phi0.cpu().numpy()) <= 1e-12
+        for u in (float(U), float(U_f), Ut):
+            assert abs(u - r.U) <= U_TOL * abs(r.U)
+        assert np.max(np.abs(F.cpu().numpy() - r.F)) <= 1e-10 * fscale
+        assert np.max(np.abs((F - F0).cpu().numpy())) <= 1e-12 * fscale

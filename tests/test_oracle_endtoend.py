@@ -200,15 +200,24 @@ def test_rejections():
 
 def test_stored_config5_values_are_the_oracles():
     """tests/golden/config5_oracle.txt (used by the GPU parity test at full size) is what the oracle computes:
-    two of its stored potentials are recomputed here (the fit needs the full step (a): 2.8e10 pairs)."""
+    two of its stored potentials are recomputed here (the fit needs the full step (a): 2.8e10 pairs), and the stored
+    indices follow the rule stated in its header (a sample that reaches every thread position of the CUDA kernels)."""
+    import importlib.util
+    import os
+    spec = importlib.util.spec_from_file_location(
+        "make_config5_golden", os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "make_config5_golden.py"))
+    gen = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(gen)
     rows = golden("config5_oracle.txt")
     w = W.config(5)
-    r = O.hsma(w, targets_slice=slice(0, 257))
+    idx = np.array([int(a) for a, _ in rows[1:]])
+    assert np.array_equal(idx, gen.sample_indices(w.N))
+    assert set(idx % 256) == set(range(256)) and set(idx // 2048) == set(range(w.N // 2048))
+    r = O.hsma(w, targets_slice=slice(0, 252))
     stored = {int(a): b for a, b in rows[1:]}
     assert abs(r.phi[0] - stored[0]) <= 1e-13 * rows[0][1]
-    assert abs(r.phi[256] - stored[256]) <= 1e-13 * rows[0][1]
+    assert abs(r.phi[251] - stored[251]) <= 1e-13 * rows[0][1]
     assert abs(r.fit_rms - rows[0][2]) <= 1e-9 * rows[0][2]
-    assert len(rows) - 1 == w.N // 256
 
 
 def test_non_cubic_periodic_box_matches_ewald():
