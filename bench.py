@@ -43,8 +43,9 @@ EXEC_PAIR = {(1, False): (10.0, 14.0), (2, False): (12.0, 18.0), (1, True): (9.0
 EXEC_PAIR_FIELD = {(1, False): (16.0, 22.0), (2, False): (18.0, 26.0), (1, True): (15.0, 21.0), (2, True): (17.0, 25.0)}
 FLOPS_PAIR_CHARGE_FIELD = 26.0
 # Symmetric form of step (b) (near_sym_kernel; used when one rank evaluates all N targets): the unit of
-# the kernel is one pair EVALUATION (an unordered source pair in one image cell), which feeds two sums.  Algorithmic
-# flops per evaluation: the 18 of a charge pair + the second accumulation (1 DFMA) = 20.  Executed per evaluation
+# the kernel is one pair EVALUATION (an unordered source pair in one image cell), which feeds two sums.  `frac` charges
+# an evaluation SURVEY.md 8(d)'s 18 flops of a charge pair (FLOPS_PAIR_CHARGE), nothing for the second accumulation;
+# `frac_with_second_accumulation` adds that DFMA (20 flops).  Executed per evaluation
 # (FP64-pipe instructions, flops): pair 11 / 16 (Newton), 13 / 20 (cubic); + per 8 evaluations the image of the source
 # (3 DFMA), q*w (DMUL) and the column accumulation (DFMA).
 FLOPS_EVAL_SYM = 20.0
@@ -240,6 +241,9 @@ def run_b200(args, w) -> dict:
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if world != args.gpus:
         raise RuntimeError(f"--gpus {args.gpus} but WORLD_SIZE={world}: launch with torch.distributed.run")
+    if local >= torch.cuda.device_count():
+        raise RuntimeError(f"bench.py --gpus {args.gpus}: rank {rank} needs visible CUDA device {local}, but only "
+                           f"{torch.cuda.device_count()} visible CUDA device(s) exist on this node")
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
     # everything (plan, kernels, flushes, events, NCCL) on one non-default stream: the library can then capture the
@@ -268,19 +272,21 @@ def run_b200(args, w) -> dict:
     force = torch.empty(T, 3, dtype=torch.float64, device=dev) if args.forces else None
     flush = torch.empty(256 * 1024 * 1024 // 8, dtype=torch.float64, device=dev)   # 256 MiB > 126 MB L2
 
-    def step():
-        flush.zero_()                                     # L2 flush between iterations (torch memset, not counted)
+    def step(events=None):
+        flush.zero_()                                     # L2 flush between iterations (torch memset, outside the events)
+        if events:
+            events[0].record()
         if world > 1:
-            # targets AND check-point sums sharded; exchanges: all-gather of the K_t check sums before the fit,
-            # all-gather of phi (F) and all-reduce of U at the end
+            # check-point sums sharded, then the PART form (or target shards); exchanges: all-gather of the K_t check
+            # sums before the fit, all-reduce (or all-gather) of phi (F) and all-reduce of U at the end
             full, _, Uall = shard.evaluate_distributed(plan, xyz, q, forces=args.forces)
             U.copy_(Uall)
-            return full
-        if args.forces:
+        elif args.forces:
             H.hsma_evaluate_forces_shard(plan.handle, xyz, q, t0, t1, phi, force, U)
         else:
             H.hsma_evaluate_shard(plan.handle, xyz, q, t0, t1, phi, U)
-        return phi
+        if events:
+            events[1].record()
 
     # peak FP64 (DFMA microbenchmark) before the run: the measured roofline denominator
     dfma_tflops, _ = H.hsma_fp64_peak(args.peak_seconds)
@@ -295,11 +301,15 @@ def run_b200(args, w) -> dict:
     barrier()
     sampler.start()
     launches0 = H.hsma_launch_count()
+    # device time of EXACTLY args.steps steps: one event pair per step around the evaluate itself, so that the L2 flush
+    # written between iterations (a 256 MiB memset, ~0.05 ms) is not in ms_per_step; the whole region, flushes
+    # included, is ms_per_step_with_flush
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     e0.record()
-    for _ in range(args.steps):
-        step()
+    for i in range(args.steps):
+        step(ev[i])
         if args.stage_timing == "on":
             for k, v in plan.timing().items():           # synchronises the stream once per step
                 stage_ms[k] += v
@@ -307,7 +317,8 @@ def run_b200(args, w) -> dict:
     barrier()
     launches = H.hsma_launch_count() - launches0
     clocks = sampler.stop()
-    ms = e0.elapsed_time(e1) / args.steps
+    ms_with_flush = e0.elapsed_time(e1) / args.steps
+    ms = sum(a.elapsed_time(b) for a, b in ev) / args.steps
     plan.set_timing(False)
     U_val = float(U.cpu()[0])
     if world > 1:
@@ -392,7 +403,10 @@ def run_b200(args, w) -> dict:
         traffic = NCU_TRAFFIC_BYTES_CFG5_SYM if traffic else None
         traffic_source = TRAFFIC_SOURCE_SYM
         units = sym_evaluations(N, info["near_cells"]) // world     # PART form: every rank 1/world of the fine units
-        alg_flops = FLOPS_EVAL_SYM_FIELD if args.forces else FLOPS_EVAL_SYM
+        # 18 flops per charge pair (26 with the gradient) x pair EVALUATIONS; the second accumulation
+        # of an evaluation (what makes it worth two ordered pairs) is charged only in frac_with_second_accumulation
+        alg_flops = FLOPS_PAIR_CHARGE_FIELD if args.forces else FLOPS_PAIR_CHARGE
+        alg_flops_2nd = FLOPS_EVAL_SYM_FIELD if args.forces else FLOPS_EVAL_SYM
         ex_instr, ex_flops = (EXEC_EVAL_SYM_FIELD if args.forces else EXEC_EVAL_SYM)[refine]
         ach_tf = units * alg_flops / (k_ms * 1e-3) * 1e-12 if k_ms > 0 else 0.0
         kernel_name = (f"near_sym_field_kernel<{refine}>" if args.forces else f"near_sym_kernel<{refine}>") + \
@@ -416,13 +430,20 @@ def run_b200(args, w) -> dict:
                 "frac_executed_flops": units * ex_flops / (k_ms * 1e-3) * 1e-12 / peak_tf if k_ms > 0 else 0.0,
                 "fp64_pipe_issue_util": units * ex_instr / (k_ms * 1e-3) / issue_peak if k_ms > 0 else 0.0,
                 "dfma_microbench_tflops": dfma_tflops, "frac_of_dfma_microbench": ach_tf / dfma_tflops if dfma_tflops else None}
+    roofline["frac_definition"] = ("achieved = units_per_launch x flops_per_unit_algorithmic / kernel time; flops_per_unit_algorithmic = "
+                                   "SURVEY.md 8(d)'s count for one charge pair (18; 26 with the gradient), applied to what the "
+                                   "kernel evaluates (units); peak = derived FP64 FMA peak")
+    roofline["evaluations_per_s"] = units / (k_ms * 1e-3) if k_ms > 0 else 0.0
     if symmetric:
+        roofline["frac_with_second_accumulation"] = units * alg_flops_2nd / (k_ms * 1e-3) * 1e-12 / peak_tf if k_ms > 0 else 0.0
+        roofline["flops_per_unit_with_second_accumulation"] = alg_flops_2nd
+        roofline["launches_per_step_of_this_kernel"] = "waves: the unordered pairs are walked in ceil(column scratch / cap) launches, each followed by a gather (in kernel_ms)"
         # for comparison with the ordered-pair kernel only: the same time charged with 18 flops for every ordered pair
         # interaction it accounts for.  It may exceed 1: the symmetry removes half of the work, it is not a roofline.
         roofline["ordered_pair_equivalent_frac"] = pc_rank["b"] * (FLOPS_PAIR_CHARGE_FIELD if args.forces else FLOPS_PAIR_CHARGE) / (k_ms * 1e-3) * 1e-12 / peak_tf if k_ms > 0 else 0.0
 
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-           "ms_per_step": ms, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64",
+           "ms_per_step": ms, "ms_per_step_with_flush": ms_with_flush, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64",
            "data": "synthetic",
            "config": {"workload": w.name, "N": N, "near_cells": info["near_cells"], "p": info["p"], "M": info["M"],
                       "check_targets": info["check_targets"], "pairs_per_step": pc_all, "rsqrt_refine": refine, "forces": bool(args.forces),
@@ -432,7 +453,9 @@ def run_b200(args, w) -> dict:
                                       f"sources replicated; all-reduce of phi and U" if world > 1 and plan.last_pair_form == 2 else
                                       f"targets and check-point sums sharded over {world} rank(s), sources replicated")
                                      + ("" if world == 1 else "; stage_ms covers the second phase only (step (a) runs in its own call)"),
-                      "l2": "256 MiB flush written between iterations"},
+                      "l2": "256 MiB flush written between iterations (outside the per-step events of ms_per_step)"},
+           "pair_evaluations_per_s": ((pc_all["a"] + pc_all["c"] + sym_evaluations(N, info["near_cells"])) / (ms * 1e-3)
+                                      if plan.last_pair_form == 2 else value),
            "energy": U_val, "stage_ms": stage_ms, "e2e": e2e, "gpu_launches": int(launches),
            "launches_per_step": plan.launches_last_evaluate(),
            "graph_replays": H.binding.hsma_plan_info(plan.handle)["graph_replays"], "clocks": clocks, "roofline": roofline}

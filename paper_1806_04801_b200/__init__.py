@@ -26,6 +26,10 @@ class Plan:
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1806_04801_b200 needs a CUDA device (no CPU fallback)")
         self.handle = None
+        # the stream the plan's kernels run on (the current torch stream unless given): shard.evaluate_distributed
+        # orders its collectives against it
+        self.torch_stream = stream if stream is not None else torch.cuda.current_stream()
+        self.stream = int(self.torch_stream.cuda_stream)
         self.handle = binding.hsma_plan_create_ex(kind=kind, L=L, near_shell=near_shell, gamma=gamma, R_aux=R_aux,
                                                   p=p, M=M, K=K, check_xyz=check_xyz, closure=closure,
                                                   far_shell=far_shell, quad_rule=quad_rule,

@@ -1,8 +1,21 @@
-"""Multi-GPU plumbing: the N targets of steps (b)/(c) are split into
-contiguous shards, one per rank; the sources (N x 32 B) and the plan are replicated; step (a) and
-the fit are computed redundantly by every rank (no data-path collective).  The only exchange is the
-assembly of the result: an all-gather of phi and a 1-double all-reduce of U, through
-torch.distributed (nccl on GPUs; gloo in the CPU tests).  No arithmetic of the method lives here."""
+"""Multi-GPU plumbing ("Multi-GPU"): one process per GPU, the sources (N x 32 B) and the plan replicated.
+`evaluate_distributed` is one HSMA evaluation over all ranks:
+  * step (a): every rank sums its slice of the K_t check targets; ONE all-gather of the check sums (32 KB; x4 with
+    derivative rows) before the fit -- the fit needs all of them;
+  * steps (b)+(c): when the symmetric form applies (one evaluation per UNORDERED pair), rank r walks its 1/R share of the
+    unordered pairs for all targets (PART form) and the result is the SUM over ranks: one all-reduce of phi [N] (and of
+    F [N,3]) and of U.  That sum over ranks is part of the method's arithmetic; it is done by the collective (NCCL's
+    or gloo's reduction), nothing else of the method is computed here.  Otherwise (small N, sphere-culled near set)
+    the N targets are split into contiguous shards and the result is assembled by an all-gather of phi (F) and an
+    all-reduce of U.
+Collectives go through torch.distributed: nccl on GPUs; a gloo group is staged through host memory (CPU tests, and the
+two-processes-on-one-GPU test, where NCCL refuses to put two ranks on one device).  Stream ordering: the library
+enqueues on the plan's stream, torch collectives on torch's current stream; evaluate_distributed makes the plan's
+stream current for its duration and orders it after the caller's stream on entry and before it on exit, so the
+result is correct whatever stream the caller is on.
+Verified: world = 2 on one B200 (two processes sharing cuda:0, gloo group, tests/test_gpu_distributed.py) and
+world = 2 gloo on CPU (tests/test_shard_gloo.py).  The NCCL path with world > 1 has not run on hardware: only one
+GPU is available to this build."""
 from __future__ import annotations
 
 from typing import List, Tuple
@@ -25,6 +38,36 @@ def shard_bounds(N: int, world: int, align: int = ALIGN) -> List[Tuple[int, int]
     return [(cuts[r], cuts[r + 1]) for r in range(world)]
 
 
+def _is_gloo(group) -> bool:
+    return dist.is_initialized() and str(dist.get_backend(group)).lower() == "gloo"
+
+
+def _all_gather_into(recv: torch.Tensor, send: torch.Tensor, group) -> torch.Tensor:
+    """dist.all_gather_into_tensor; a gloo group with CUDA tensors is staged through host memory."""
+    if _is_gloo(group) and send.is_cuda:
+        world = dist.get_world_size(group)
+        parts = [torch.empty(send.shape, dtype=send.dtype) for _ in range(world)]
+        dist.all_gather(parts, send.cpu(), group=group)
+        recv.copy_(torch.cat(parts).reshape(recv.shape))
+    elif _is_gloo(group):
+        parts = list(recv.reshape((dist.get_world_size(group),) + tuple(send.shape)).unbind(0))
+        dist.all_gather(parts, send, group=group)
+    else:
+        dist.all_gather_into_tensor(recv, send, group=group)
+    return recv
+
+
+def _all_reduce_sum(t: torch.Tensor, group) -> torch.Tensor:
+    """In-place sum over the ranks; a gloo group with a CUDA tensor is staged through host memory."""
+    if _is_gloo(group) and t.is_cuda:
+        h = t.cpu()
+        dist.all_reduce(h, op=dist.ReduceOp.SUM, group=group)
+        t.copy_(h)
+    else:
+        dist.all_reduce(t, op=dist.ReduceOp.SUM, group=group)
+    return t
+
+
 def all_gather_phi(phi_local: torch.Tensor, N: int, group=None) -> torch.Tensor:
     """Assemble phi [N] on every rank from the per-rank shards (shards padded to a common length for
     the equal-size all_gather; the padding is cut away again)."""
@@ -36,21 +79,21 @@ def all_gather_phi(phi_local: torch.Tensor, N: int, group=None) -> torch.Tensor:
     send = torch.zeros(width, dtype=phi_local.dtype, device=phi_local.device)
     send[: phi_local.numel()] = phi_local
     recv = torch.empty(world * width, dtype=phi_local.dtype, device=phi_local.device)
-    dist.all_gather_into_tensor(recv, send, group=group)
+    _all_gather_into(recv, send, group)
     return torch.cat([recv[r * width: r * width + (b - a)] for r, (a, b) in enumerate(bounds)])
 
 
 def all_reduce_energy(U_local: torch.Tensor, group=None) -> torch.Tensor:
     """U = sum over ranks of the shard energies 1/2 sum_{i in shard} q_i phi_i (in place)."""
     if dist.is_initialized() and dist.get_world_size(group) > 1:
-        dist.all_reduce(U_local, op=dist.ReduceOp.SUM, group=group)
+        _all_reduce_sum(U_local, group)
     return U_local
 
 
 def all_reduce_phi(phi_part: torch.Tensor, group=None) -> torch.Tensor:
     """phi = sum over ranks of the partial potentials of the PART form (in place; [N] doubles, 2 MB at N = 262,144)."""
     if dist.is_initialized() and dist.get_world_size(group) > 1:
-        dist.all_reduce(phi_part, op=dist.ReduceOp.SUM, group=group)
+        _all_reduce_sum(phi_part, group)
     return phi_part
 
 
@@ -66,7 +109,7 @@ def all_gather_slices(local: torch.Tensor, total: int, group=None) -> torch.Tens
     send = torch.zeros((width,) + tail, dtype=local.dtype, device=local.device)
     send[: local.shape[0]] = local
     recv = torch.empty((world * width,) + tail, dtype=local.dtype, device=local.device)
-    dist.all_gather_into_tensor(recv, send, group=group)
+    _all_gather_into(recv, send, group)
     return torch.cat([recv[r * width: r * width + (b - a)] for r, (a, b) in enumerate(bounds)])
 
 
@@ -79,7 +122,26 @@ def evaluate_distributed(plan, xyz: torch.Tensor, q: torch.Tensor, forces: bool 
     or, when the symmetric form of step (b) applies (DESIGN.md 6.12 / 8):
       3'. fit, mapping, this rank's share of the UNORDERED pairs of (b), (c) for its targets    hsma_evaluate_rest_part
       4'. all-reduce of the partial phi [N] (and F [N,3]) and of the partial U
-    Returns (phi [N], F [N,3] or None, U [1]) on every rank.  `plan` is a paper_1806_04801_b200.Plan."""
+    Returns (phi [N], F [N,3] or None, U [1]) on every rank.  `plan` is a paper_1806_04801_b200.Plan.
+    The library calls run on the plan's stream and the collectives on torch's current stream: the plan's stream is made
+    current here, ordered after the caller's stream on entry and before it on exit."""
+    if not q.is_cuda:
+        raise RuntimeError("evaluate_distributed needs device tensors (the CUDA path has no CPU fallback)")
+    caller = torch.cuda.current_stream(q.device)
+    ps = plan.torch_stream
+    if ps.cuda_stream == caller.cuda_stream:
+        return _evaluate_distributed(plan, xyz, q, forces, group)
+    ps.wait_stream(caller)
+    with torch.cuda.stream(ps):
+        out = _evaluate_distributed(plan, xyz, q, forces, group)
+    caller.wait_stream(ps)
+    for t in out:
+        if t is not None:
+            t.record_stream(caller)
+    return out
+
+
+def _evaluate_distributed(plan, xyz: torch.Tensor, q: torch.Tensor, forces: bool, group):
     from . import binding
     N = q.numel()
     rank = dist.get_rank(group) if dist.is_initialized() else 0
@@ -129,5 +191,5 @@ def _gather_rows(local: torch.Tensor, N: int, group=None):
     send = torch.zeros(width, local.shape[1], dtype=local.dtype, device=local.device)
     send[: local.shape[0]] = local
     recv = torch.empty(world * width, local.shape[1], dtype=local.dtype, device=local.device)
-    dist.all_gather_into_tensor(recv, send, group=group)
+    _all_gather_into(recv, send, group)
     return [recv[r * width: r * width + (b - a)] for r, (a, b) in enumerate(bounds)]
