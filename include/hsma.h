@@ -81,6 +81,16 @@ typedef enum {
 } hsma_near_mode;
 
 typedef enum {
+    HSMA_NEAR_ALG_DIRECT = 0,  /* the exact direct sum over all pairs: near_sym_kernel / near_sum_kernel (north_star) */
+    HSMA_NEAR_ALG_FMM = 1      /* SURVEY.md 8(f) NEXT 4, Table I: step (b) by a uniform-grid
+                                  fast multipole method: O(N) instead of O(N^2), the same sum up to the
+                                  truncation of the expansions (<= 1e-12 of max|phi| at the default order 20).  Used when an
+                                  evaluate covers all N targets (potentials; forces and target shards keep the direct
+                                  kernels).  Needs the whole-cell near set and box sides that are integer multiples of
+                                  the smallest one (cubic FMM boxes): HSMA_ERR_INVALID_ARG at plan creation otherwise. */
+} hsma_near_algorithm;
+
+typedef enum {
     HSMA_DIPOLE_EXACT = 0,     /* exact normal dipole on the M nodes (reading S9) */
     HSMA_DIPOLE_FD3 = 1        /* Eq.(12)-(14) PAPER.md:107-120: central difference over three spheres, 3M charges */
 } hsma_dipole_mode;
@@ -112,6 +122,10 @@ typedef struct {
     int near_mode;        /* hsma_near_mode */
     int dipole_mode;      /* hsma_dipole_mode */
     double fd_dr_rel;     /* HSMA_DIPOLE_FD3: Delta r / R_aux (1e-5; 1e-4 for the Dirichlet example); 0 = 1e-5 */
+    /* sub-quadratic near sum; 0 = the direct sum */
+    int near_algorithm;   /* hsma_near_algorithm */
+    int fmm_order;        /* expansion order of the FMM, 2..30; 0 = 20 (truncation <= 1e-12 of max|phi|) */
+    int fmm_levels;       /* leaf level of the FMM box hierarchy, 1..5; 0 = by N (about 500 sources per leaf) */
 } hsma_plan_desc;
 
 /*

@@ -22,7 +22,8 @@ class Plan:
 
     def __init__(self, *, kind: int, L, near_shell, R_aux: float, p: int, M: int, K: int, gamma: float = 1.0,
                  check_xyz=None, closure: int = 0, far_shell=(0, 0, 0), quad_rule: int = 0,
-                 rsqrt_refine: int = 0, near_mode: int = 0, dipole_mode: int = 0, fd_dr_rel: float = 0.0, stream=None):
+                 rsqrt_refine: int = 0, near_mode: int = 0, dipole_mode: int = 0, fd_dr_rel: float = 0.0,
+                 near_algorithm: int = 0, fmm_order: int = 0, fmm_levels: int = 0, stream=None):
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1806_04801_b200 needs a CUDA device (no CPU fallback)")
         self.handle = None
@@ -34,7 +35,9 @@ class Plan:
                                                   p=p, M=M, K=K, check_xyz=check_xyz, closure=closure,
                                                   far_shell=far_shell, quad_rule=quad_rule,
                                                   rsqrt_refine=rsqrt_refine, near_mode=near_mode,
-                                                  dipole_mode=dipole_mode, fd_dr_rel=fd_dr_rel, stream=stream)
+                                                  dipole_mode=dipole_mode, fd_dr_rel=fd_dr_rel,
+                                                  near_algorithm=near_algorithm, fmm_order=fmm_order,
+                                                  fmm_levels=fmm_levels, stream=stream)
         self.info = binding.hsma_plan_info(self.handle)
 
     @classmethod

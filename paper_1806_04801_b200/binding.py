@@ -33,7 +33,8 @@ class hsma_plan_desc(ctypes.Structure):
                 ("p", ctypes.c_int), ("M", ctypes.c_int), ("K", ctypes.c_int), ("check_xyz", c_double_p),
                 ("closure", ctypes.c_int), ("far_shell", ctypes.c_int * 3), ("quad_rule", ctypes.c_int),
                 ("rsqrt_refine", ctypes.c_int), ("near_mode", ctypes.c_int), ("dipole_mode", ctypes.c_int),
-                ("fd_dr_rel", ctypes.c_double)]
+                ("fd_dr_rel", ctypes.c_double), ("near_algorithm", ctypes.c_int), ("fmm_order", ctypes.c_int),
+                ("fmm_levels", ctypes.c_int)]
 
 
 class HsmaError(RuntimeError):
@@ -177,7 +178,8 @@ def hsma_plan_create(L: float, boundary_kind: int, near_shell: int, R_aux: float
 def hsma_plan_create_ex(*, kind: int, L: Sequence[float], near_shell: Sequence[int], gamma: float, R_aux: float,
                         p: int, M: int, K: int, check_xyz=None, closure: int = 0, far_shell=(0, 0, 0),
                         quad_rule: int = 0, rsqrt_refine: int = 0, near_mode: int = 0, dipole_mode: int = 0,
-                        fd_dr_rel: float = 0.0, stream=None) -> int:
+                        fd_dr_rel: float = 0.0, near_algorithm: int = 0, fmm_order: int = 0, fmm_levels: int = 0,
+                        stream=None) -> int:
     d = hsma_plan_desc()
     d.struct_size = ctypes.sizeof(hsma_plan_desc)
     d.kind = kind
@@ -194,6 +196,7 @@ def hsma_plan_create_ex(*, kind: int, L: Sequence[float], near_shell: Sequence[i
     d.far_shell[:] = [int(v) for v in far_shell]
     d.quad_rule, d.rsqrt_refine = int(quad_rule), int(rsqrt_refine)
     d.near_mode, d.dipole_mode, d.fd_dr_rel = int(near_mode), int(dipole_mode), float(fd_dr_rel)
+    d.near_algorithm, d.fmm_order, d.fmm_levels = int(near_algorithm), int(fmm_order), int(fmm_levels)
     h = ctypes.c_void_p()
     _check(load_library().hsma_plan_create_ex(ctypes.byref(d), _stream_ptr(stream), ctypes.byref(h)),
            "hsma_plan_create_ex")
@@ -413,6 +416,8 @@ def hsma_plan_set_timing(plan: int, enable: bool):
 
 
 PAIR_FORM_AUTO, PAIR_FORM_ORDERED, PAIR_FORM_SYMMETRIC = 0, 1, 2
+PAIR_FORM_FMM = 3               # reported by hsma_plan_last_pair_form when step (b) ran as the FMM
+NEAR_ALG_DIRECT, NEAR_ALG_FMM = 0, 1
 
 
 def hsma_plan_set_pair_form(plan: int, form: int):

@@ -1,0 +1,675 @@
+// Sub-quadratic form of step (b) (PAPER.md:144-146 and Table I: "both FMM and
+// GPU accelerations are applied", O(N_s + N_m)): a uniform-grid fast multipole method for the near sum
+//     phi_i = sum_c w_c sum_j' q_j / |r_i - (sigma_c o r_j + k_c L)|            (Eq.(5), whole cells)
+// written from scratch for sm_100a.  It computes the SAME sum as near_sum_kernel / near_sym_kernel up to the truncation
+// of the expansions (order p: measured <= 1e-12 of max|phi| at p = 20); the oracle stays the exact
+// direct sum and the parity bars stay 1e-10 / 1e-11.
+//
+// Expansions (complex solid harmonics, m >= 0 stored, X_n^{-m} = (-1)^m conj X_n^m):
+//     R_n^m(r) = r^n P_n^m(cos th) e^{i m ph} / (n+m)!          regular
+//     S_n^m(r) = (n-m)! P_n^m(cos th) e^{i m ph} / r^{n+1}      singular            (P_n^m without Condon-Shortley phase)
+// with the three addition theorems (checked numerically before this file was written)
+//     1/|a - b|   = sum_{n,m} conj R_n^m(a) S_n^m(b)                                   |a| < |b|
+//     R_n^m(a+b)  = sum_{k,l} R_k^l(a) R_{n-k}^{m-l}(b)
+//     S_n^m(a+b)  = sum_{k,l} (-1)^k conj R_k^l(a) S_{n+k}^{m+l}(b)                    |a| < |b|
+// so that, in units of the box side a_l of each level (M~ = M / a^n, phi = (1/a) sum conj R(x/a) L~):
+//     P2M   M_n^m = sum_j q_j R_n^m((r_j - c)/a)
+//     M2M   M_n^m(parent) = sum_{child} sum_{k,l} R_k^l(s) M_{n-k}^{m-l}(child) 2^{-(n-k)},   s = (c_child - c_parent)/a_parent
+//     M2L   L_k^l(t) = (-1)^k sum_{src} sum_{n,m} conj M_n^m(src) S_{n+k}^{m+l}(d),           d = (c_t - c_src)/a
+//     L2L   L_n^m(child) = 2^{-(n+1)} sum_{k,l} conj R_{k-n}^{l-m}(s) L_k^l(parent)
+//     L2P   phi(x) = (1/a) Re sum_{k,l} conj R_k^l((x - c)/a) L_k^l
+// Well-separated = more than kWs = 2 boxes apart (Chebyshev distance): convergence ratio (sqrt3/2)/2.5 = 0.35 per
+// order instead of 0.58 with one box, which is what makes 1e-12 reachable at p = 20 (one-box separation needs p > 60).
+// Image cells are never materialised here either: a source box in image cell k is the central box (mirrored in a
+// reflecting axis when k_a is odd) shifted by k L; its multipole moments are those of the central box with the
+// reflection signs applied on load (x: (-1)^m conj, y: conj, z: (-1)^{n+m}) and the cell weight gamma^|k|.
+#pragma once
+#include "common.cuh"
+#include "sum_kernels.cuh"
+
+namespace hsma {
+namespace fmm {
+
+constexpr int kWs = 2;                 // boxes within Chebyshev distance kWs are near (P2P)
+constexpr int kOffR = 2 * kWs + 1;     // M2L offsets d in [-5,5]^3 with |d|_inf > kWs
+constexpr int kOffW = 2 * kOffR + 1;   // 11
+constexpr int kOffN = kOffW * kOffW * kOffW;
+constexpr int kMaxOrder = 30;          // P2M runs one lane per order m: p <= 31; shared memory of M2L: p <= 30
+constexpr int kMaxLevels = 6;          // leaf level <= 5 (keys < 2^16: two 8-bit radix passes)
+constexpr int kInvW = kMaxOrder + 2;
+
+__host__ __device__ inline int nc(int p) { return (p + 1) * (p + 2) / 2; }
+__host__ __device__ inline int cidx(int n, int m) { return n * (n + 1) / 2 + m; }
+__host__ __device__ inline int fidx(int n, int m) { return n * n + n + m; }   // full range m = -n..n
+
+struct Geom {
+    int base[3];       // level-0 boxes per cell and axis (cubic boxes of side a0 = L_a / base_a)
+    int levels;        // leaf level (>= 1)
+    int shell[3];      // near cell table: |k_a| <= shell_a
+    int refl[3];       // axis is reflecting: images in odd cells are mirrored
+    int p;             // expansion order
+    double a0;         // level-0 box side
+    double half[3];    // L_a / 2
+    double L[3];
+    const double* w_lut;   // [(2 s_x+1)(2 s_y+1)(2 s_z+1)] cell weights gamma^|k|
+};
+__host__ __device__ inline int grid_n(const Geom& g, int lev, int a) { return g.base[a] << lev; }
+__host__ __device__ inline long long boxes_at(const Geom& g, int lev) {
+    return (long long)grid_n(g, lev, 0) * grid_n(g, lev, 1) * grid_n(g, lev, 2);
+}
+__host__ __device__ inline long long level_offset(const Geom& g, int lev) {   // boxes of the levels above
+    long long o = 0;
+    for (int l = 0; l < lev; ++l) o += boxes_at(g, l);
+    return o;
+}
+__host__ __device__ inline int floor_div(int a, int b) { return a >= 0 ? a / b : -((-a + b - 1) / b); }
+
+// A box with GLOBAL grid coordinates g (any cell) at level lev: the central box it is an image of, its cell's
+// shift, reflection flags and weight.  Returns false if the cell is not in the near table.
+struct ImageBox { int box; int fx, fy, fz; double sx, sy, sz, w; int central; };
+__device__ __forceinline__ bool image_box(const Geom& G, int lev, int gx, int gy, int gz, ImageBox& out) {
+    const int g[3] = {gx, gy, gz};
+    int j[3], f[3], k[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const int n = grid_n(G, lev, a);
+        k[a] = floor_div(g[a], n);
+        if (k[a] < -G.shell[a] || k[a] > G.shell[a]) return false;
+        j[a] = g[a] - k[a] * n;
+        f[a] = G.refl[a] && (k[a] & 1);
+        if (f[a]) j[a] = n - 1 - j[a];
+    }
+    out.box = (j[0] * grid_n(G, lev, 1) + j[1]) * grid_n(G, lev, 2) + j[2];
+    out.fx = f[0]; out.fy = f[1]; out.fz = f[2];
+    out.sx = k[0] * G.L[0]; out.sy = k[1] * G.L[1]; out.sz = k[2] * G.L[2];
+    const int wy = 2 * G.shell[1] + 1, wz = 2 * G.shell[2] + 1;
+    out.w = G.w_lut[((k[0] + G.shell[0]) * wy + (k[1] + G.shell[1])) * wz + (k[2] + G.shell[2])];
+    out.central = (k[0] == 0 && k[1] == 0 && k[2] == 0);
+    return true;
+}
+
+// complex helpers on double2
+__device__ __forceinline__ double2 cmul(double2 a, double2 b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+__device__ __forceinline__ void cfma(double2& acc, double2 a, double2 b) {
+    acc.x = fma(a.x, b.x, acc.x); acc.x = fma(-a.y, b.y, acc.x);
+    acc.y = fma(a.x, b.y, acc.y); acc.y = fma(a.y, b.x, acc.y);
+}
+// X_n^m for any |m| <= n from the m >= 0 storage
+__device__ __forceinline__ double2 cget(const double2* X, int n, int m) {
+    if (m >= 0) return X[cidx(n, m)];
+    const double2 v = X[cidx(n, -m)];
+    return (m & 1) ? make_double2(-v.x, v.y) : make_double2(v.x, -v.y);   // (-1)^m conj
+}
+
+// ---- leaf assignment and a stable two-pass radix sort (8 bits each) of the particles by leaf ------------------------
+__global__ void key_kernel(const double* __restrict__ xyz, long long N, const Geom G, int* __restrict__ key, int* __restrict__ idx) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const double inv = (double)(1 << G.levels) / G.a0;
+    int c[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const int n = grid_n(G, G.levels, a);
+        const int v = (int)floor(xyz[3 * i + a] * inv);     // box coordinates: [0, L_a] -> [0, n]
+        c[a] = v < 0 ? 0 : (v >= n ? n - 1 : v);
+    }
+    key[i] = (c[0] * grid_n(G, G.levels, 1) + c[1]) * grid_n(G, G.levels, 2) + c[2];
+    idx[i] = (int)i;
+}
+__global__ void __launch_bounds__(256) radix_hist_kernel(const int* __restrict__ key, long long N, int shift, long long n_blk,
+                                                         long long* __restrict__ counts) {
+    __shared__ int h[256];
+    h[threadIdx.x] = 0;
+    __syncthreads();
+    const long long i = (long long)blockIdx.x * 256 + threadIdx.x;
+    if (i < N) atomicAdd(&h[(key[i] >> shift) & 255], 1);     // integer counts: order does not matter
+    __syncthreads();
+    counts[(long long)threadIdx.x * n_blk + blockIdx.x] = h[threadIdx.x];
+}
+// stable: items keep their order within a digit (lane order in a warp, warp order in a block, block order)
+__global__ void __launch_bounds__(256) radix_scatter_kernel(const int* __restrict__ key_in, const int* __restrict__ idx_in,
+                                                            long long N, int shift, long long n_blk,
+                                                            const long long* __restrict__ offs, int* __restrict__ key_out,
+                                                            int* __restrict__ idx_out) {
+    __shared__ int cnt[8][256];
+    for (int k = threadIdx.x; k < 8 * 256; k += 256) (&cnt[0][0])[k] = 0;
+    __syncthreads();
+    const long long i = (long long)blockIdx.x * 256 + threadIdx.x;
+    const bool valid = i < N;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int kv = valid ? key_in[i] : 0;
+    const int d = (kv >> shift) & 255;
+    const unsigned peers = __match_any_sync(0xffffffffu, valid ? d : -1 - lane);
+    const int rank = __popc(peers & ((1u << lane) - 1u));
+    if (valid && rank == 0) cnt[warp][d] = __popc(peers);
+    __syncthreads();
+    if (valid) {
+        int before = 0;
+        for (int w = 0; w < warp; ++w) before += cnt[w][d];
+        const long long pos = offs[(long long)d * n_blk + blockIdx.x] + before + rank;
+        key_out[pos] = kv;
+        idx_out[pos] = idx_in[i];
+    }
+}
+// leaf_start[l] = first sorted position with key >= l (l = 0..n_leaves), and the sorted, centred source records
+__global__ void leaf_start_kernel(const int* __restrict__ key, long long N, int n_leaves, int* __restrict__ leaf_start) {
+    const int l = blockIdx.x * blockDim.x + threadIdx.x;
+    if (l > n_leaves) return;
+    long long lo = 0, hi = N;
+    while (lo < hi) {
+        const long long mid = (lo + hi) >> 1;
+        if (key[mid] < l) lo = mid + 1; else hi = mid;
+    }
+    leaf_start[l] = (int)lo;
+}
+__global__ void gather_sorted_kernel(const double* __restrict__ xyz, const double* __restrict__ q, const int* __restrict__ idx,
+                                     long long N, double hx, double hy, double hz, Src4* __restrict__ out) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const long long j = idx[i];
+    out[i] = Src4{xyz[3 * j] - hx, xyz[3 * j + 1] - hy, xyz[3 * j + 2] - hz, q[j]};
+}
+
+// centre of box (ix, iy, iz) of level lev, centred coordinates
+__device__ __forceinline__ void box_centre(const Geom& G, int lev, int box, double c[3], int ic[3]) {
+    const int ny = grid_n(G, lev, 1), nz = grid_n(G, lev, 2);
+    ic[2] = box % nz; ic[1] = (box / nz) % ny; ic[0] = box / (nz * ny);
+    const double a = G.a0 / (double)(1 << lev);
+#pragma unroll
+    for (int k = 0; k < 3; ++k) c[k] = (ic[k] + 0.5) * a - G.half[k];
+}
+
+// inv[n * kInvW + m] = 1 / ((n+m)(n-m)) for n > m (the three-term recurrence of R_n^m in n)
+__device__ __forceinline__ void fill_inv_table(double* inv, int p) {
+    for (int t = threadIdx.x; t < (p + 1) * kInvW; t += blockDim.x) {
+        const int n = t / kInvW, m = t % kInvW;
+        inv[t] = (n > m) ? 1.0 / ((double)(n + m) * (double)(n - m)) : 0.0;
+    }
+}
+
+// ---- P2M: one CTA per leaf, one lane per order m, warps share the particles --------------------------------------------
+// dynamic shared memory: accw [8][nc(p)] double2, inv [(p+1) * kInvW] double
+__global__ void __launch_bounds__(256) p2m_kernel(const Geom G, const Src4* __restrict__ srt, const int* __restrict__ leaf_start,
+                                                  double2* __restrict__ M /* all levels */) {
+    extern __shared__ __align__(16) double2 sm2[];
+    const int p = G.p, NC = nc(p);
+    double2* accw = sm2;
+    double* inv = reinterpret_cast<double*>(sm2 + 8 * NC);
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    for (int t = tid; t < 8 * NC; t += 256) accw[t] = make_double2(0.0, 0.0);
+    fill_inv_table(inv, p);
+    __syncthreads();
+    const int leaf = blockIdx.x;
+    double c[3]; int ic[3];
+    box_centre(G, G.levels, leaf, c, ic);
+    const double ia = (double)(1 << G.levels) / G.a0;
+    const int s0 = leaf_start[leaf], s1 = leaf_start[leaf + 1];
+    double2* acc = accw + warp * NC;
+    for (int j = s0 + warp; j < s1; j += 8) {
+        const Src4 s = srt[j];
+        const double x = (s.x - c[0]) * ia, y = (s.y - c[1]) * ia, z = (s.z - c[2]) * ia;
+        const double r2 = fma(z, z, fma(y, y, x * x));
+        if (lane <= p) {
+            const int m = lane;
+            double rr = 1.0, ri = 0.0;                     // R_m^m = prod_{i<=m} (x + i y) / (2 i)
+            for (int i = 1; i <= m; ++i) {
+                const double f = 0.5 / (double)i;
+                const double t = (rr * x - ri * y) * f;
+                ri = (rr * y + ri * x) * f;
+                rr = t;
+            }
+            double p1r = rr, p1i = ri, p2r = 0.0, p2i = 0.0;
+            double2* a = acc + cidx(m, m);
+            a->x = fma(s.q, rr, a->x); a->y = fma(s.q, ri, a->y);
+            for (int n = m + 1; n <= p; ++n) {
+                const double f = inv[n * kInvW + m], tz = (double)(2 * n - 1) * z;
+                const double cr = (tz * p1r - r2 * p2r) * f, ci = (tz * p1i - r2 * p2i) * f;
+                a = acc + cidx(n, m);
+                a->x = fma(s.q, cr, a->x); a->y = fma(s.q, ci, a->y);
+                p2r = p1r; p2i = p1i; p1r = cr; p1i = ci;
+            }
+        }
+    }
+    __syncthreads();
+    double2* out = M + (level_offset(G, G.levels) + leaf) * NC;
+    for (int t = tid; t < NC; t += 256) {
+        double2 v = make_double2(0.0, 0.0);
+        for (int w = 0; w < 8; ++w) { v.x += accw[w * NC + t].x; v.y += accw[w * NC + t].y; }
+        out[t] = v;
+    }
+}
+
+// ---- plan-time tables ----------------------------------------------------------------------------------------------------
+// Rsh[ch][cidx(n,m)] = R_n^m(s_ch), s_ch = ((cx,cy,cz) - 1/2) / 2 for child ch = 4 cx + 2 cy + cz: the shift from the
+// parent's centre to the child's, in units of the parent's box side (M2M) -- and the same vector for L2L.
+// Stab[off][cidx(N,mu)] = S_N^mu(d), N <= 2p, for the offsets d = (dx,dy,dz) in [-5,5]^3 (off = dense index); entries
+// with |d|_inf <= kWs are never read (left zero).  nm[c] = (n << 8) | m.
+__global__ void tables_kernel(int p, double2* __restrict__ Rsh, double2* __restrict__ Stab, int* __restrict__ nm) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    const int NC = nc(p), NS = nc(2 * p);
+    if (t < NC) {
+        int n = 0;
+        while (cidx(n + 1, 0) <= t) ++n;
+        nm[t] = (n << 8) | (t - cidx(n, 0));
+    }
+    if (t < 8) {
+        const double x = ((t >> 2) & 1) ? 0.25 : -0.25, y = ((t >> 1) & 1) ? 0.25 : -0.25, z = (t & 1) ? 0.25 : -0.25;
+        const double r2 = x * x + y * y + z * z;
+        double2* R = Rsh + t * NC;
+        double rr = 1.0, ri = 0.0;
+        for (int m = 0; m <= p; ++m) {
+            if (m > 0) { const double f = 0.5 / m, u = (rr * x - ri * y) * f; ri = (rr * y + ri * x) * f; rr = u; }
+            double p1r = rr, p1i = ri, p2r = 0.0, p2i = 0.0;
+            R[cidx(m, m)] = make_double2(rr, ri);
+            for (int n = m + 1; n <= p; ++n) {
+                const double f = 1.0 / ((double)(n + m) * (double)(n - m)), tz = (2 * n - 1) * z;
+                const double cr = (tz * p1r - r2 * p2r) * f, ci = (tz * p1i - r2 * p2i) * f;
+                R[cidx(n, m)] = make_double2(cr, ci);
+                p2r = p1r; p2i = p1i; p1r = cr; p1i = ci;
+            }
+        }
+    }
+    if (t < kOffN) {
+        const int dx = t / (kOffW * kOffW) - kOffR, dy = (t / kOffW) % kOffW - kOffR, dz = t % kOffW - kOffR;
+        double2* S = Stab + (long long)t * NS;
+        const int amax = max(abs(dx), max(abs(dy), abs(dz)));
+        if (amax <= kWs) {
+            for (int k = 0; k < NS; ++k) S[k] = make_double2(0.0, 0.0);
+            return;
+        }
+        const double x = dx, y = dy, z = dz, r2 = x * x + y * y + z * z, ir2 = 1.0 / r2;
+        const int P2 = 2 * p;
+        double sr = 1.0 / sqrt(r2), si = 0.0;           // S_m^m = (2m-1) (x + i y) / r^2 S_{m-1}^{m-1}
+        for (int m = 0; m <= P2; ++m) {
+            if (m > 0) { const double f = (2 * m - 1) * ir2, u = (sr * x - si * y) * f; si = (sr * y + si * x) * f; sr = u; }
+            double p1r = sr, p1i = si, p2r = 0.0, p2i = 0.0;
+            S[cidx(m, m)] = make_double2(sr, si);
+            for (int n = m + 1; n <= P2; ++n) {
+                const double tz = (2 * n - 1) * z, g = (double)(n - 1 + m) * (double)(n - 1 - m);
+                const double cr = (tz * p1r - g * p2r) * ir2, ci = (tz * p1i - g * p2i) * ir2;
+                S[cidx(n, m)] = make_double2(cr, ci);
+                p2r = p1r; p2i = p1i; p1r = cr; p1i = ci;
+            }
+        }
+    }
+}
+
+// ---- M2M: one CTA per parent box of level lev, one thread per coefficient ---------------------------------------------
+// dynamic shared memory: Mc [8][NC], Rs [8][NC] double2
+__global__ void __launch_bounds__(256) m2m_kernel(const Geom G, int lev, const double2* __restrict__ Rsh, const int* __restrict__ nm,
+                                                  double2* __restrict__ M) {
+    extern __shared__ __align__(16) double2 sm2[];
+    const int p = G.p, NC = nc(p);
+    double2* Mc = sm2;
+    double2* Rs = sm2 + 8 * NC;
+    const int box = blockIdx.x;
+    const int ny = grid_n(G, lev, 1), nz = grid_n(G, lev, 2);
+    const int iz = box % nz, iy = (box / nz) % ny, ix = box / (nz * ny);
+    const int cy = grid_n(G, lev + 1, 1), cz = grid_n(G, lev + 1, 2);
+    const double2* Mchild = M + level_offset(G, lev + 1) * NC;
+    for (int t = threadIdx.x; t < 8 * NC; t += 256) {
+        const int ch = t / NC, c = t - ch * NC;
+        const int jx = 2 * ix + ((ch >> 2) & 1), jy = 2 * iy + ((ch >> 1) & 1), jz = 2 * iz + (ch & 1);
+        Mc[t] = Mchild[((long long)(jx * cy + jy) * cz + jz) * NC + c];
+        Rs[t] = Rsh[t];
+    }
+    __syncthreads();
+    double2* out = M + (level_offset(G, lev) + box) * NC;
+    for (int c = threadIdx.x; c < NC; c += 256) {
+        const int n = nm[c] >> 8, m = nm[c] & 255;
+        double2 acc = make_double2(0.0, 0.0);
+        for (int ch = 0; ch < 8; ++ch) {
+            const double2* R = Rs + ch * NC;
+            const double2* X = Mc + ch * NC;
+            for (int k = 0; k <= n; ++k) {
+                const int nn = n - k;
+                const double sc = ldexp(1.0, -nn);
+                double2 part = make_double2(0.0, 0.0);
+                const int l_lo = max(-k, m - nn), l_hi = min(k, m + nn);
+                for (int l = l_lo; l <= l_hi; ++l) cfma(part, cget(R, k, l), cget(X, nn, m - l));
+                acc.x = fma(sc, part.x, acc.x); acc.y = fma(sc, part.y, acc.y);
+            }
+        }
+        out[c] = acc;
+    }
+}
+
+// ---- L2L + sum of the M2L partials: one CTA per box of level lev ----------------------------------------------------------
+// L[lev][box] = sum_s Lpart[s][box] (+ the parent's local expansion shifted to this box, lev > 0)
+// dynamic shared memory: Lp [NC], Rs [NC] double2
+__global__ void __launch_bounds__(256) l2l_kernel(const Geom G, int lev, const double2* __restrict__ Rsh, const int* __restrict__ nm,
+                                                  const double2* __restrict__ Lpart, int n_split, double2* __restrict__ L) {
+    extern __shared__ __align__(16) double2 sm2[];
+    const int p = G.p, NC = nc(p);
+    double2* Lp = sm2;
+    double2* Rs = sm2 + NC;
+    const int box = blockIdx.x;
+    const long long nb = boxes_at(G, lev);
+    if (lev > 0) {
+        const int ny = grid_n(G, lev, 1), nz = grid_n(G, lev, 2);
+        const int iz = box % nz, iy = (box / nz) % ny, ix = box / (nz * ny);
+        const int py = grid_n(G, lev - 1, 1), pz = grid_n(G, lev - 1, 2);
+        const long long parent = ((long long)((ix >> 1) * py + (iy >> 1))) * pz + (iz >> 1);
+        const int ch = ((ix & 1) << 2) | ((iy & 1) << 1) | (iz & 1);
+        const double2* Lpar = L + (level_offset(G, lev - 1) + parent) * NC;
+        for (int t = threadIdx.x; t < NC; t += 256) { Lp[t] = Lpar[t]; Rs[t] = Rsh[ch * NC + t]; }
+    }
+    __syncthreads();
+    double2* out = L + (level_offset(G, lev) + box) * NC;
+    for (int c = threadIdx.x; c < NC; c += 256) {
+        const int n = nm[c] >> 8, m = nm[c] & 255;
+        double2 acc = make_double2(0.0, 0.0);
+        for (int s = 0; s < n_split; ++s) {
+            const double2 v = Lpart[((long long)s * nb + box) * NC + c];
+            acc.x += v.x; acc.y += v.y;
+        }
+        if (lev > 0) {
+            double2 sh = make_double2(0.0, 0.0);
+            for (int k = n; k <= p; ++k) {
+                const int dn = k - n;
+                const int l_lo = max(-k, m - dn), l_hi = min(k, m + dn);
+                for (int l = l_lo; l <= l_hi; ++l) {
+                    const double2 r = cget(Rs, dn, l - m);
+                    cfma(sh, make_double2(r.x, -r.y), cget(Lp, k, l));
+                }
+            }
+            const double sc = ldexp(1.0, -(n + 1));
+            acc.x = fma(sc, sh.x, acc.x); acc.y = fma(sc, sh.y, acc.y);
+        }
+        out[c] = acc;
+    }
+}
+
+// ---- M2L: the translation that dominates the far field -----------------------------------------------------------------
+// One CTA = (level, sibling group, split): the <= 8 children of one parent box (level 0: a single box) and a
+// contiguous, weight-balanced share of the offset list.  For an offset d all siblings share S(d) (staged once in shared
+// memory, expanded to -N <= mu <= N) and each valid sibling has its own source box t + d (its conj M, expanded to
+// -n <= m <= n with the image reflection and the cell weight applied, staged too).  Thread (k, l) keeps the 8 local
+// coefficients L_k^l of the siblings in registers: per (n, m) one 128-bit read of S and one broadcast read per sibling
+// feed 4 DFMA per sibling.  The split's partial sums go to Lpart[split][box]; l2l_kernel adds the splits in order.
+struct M2LLevel { int lev, n_groups, n_split, first_cta; long long part_off; };
+struct M2LArgs {
+    M2LLevel lv[kMaxLevels];
+    int n_lv;
+    const int* off_list;      // [n_off] dense offset indices (g - t), |d|_inf > kWs, processing order
+    const int* off_wprefix;   // [n_off + 1] prefix sums of the offset weights (how many of 8 siblings have it)
+    int n_off;
+};
+
+template <int NV>
+__device__ __forceinline__ void m2l_inner(const double2* __restrict__ Sfull, const double2* __restrict__ Mf, int mstride,
+                                          int p, int k, int l, double2 (&tmp)[NV]) {
+    for (int n = 0; n <= p; ++n) {
+        const double2* Srow = Sfull + fidx(n + k, l);
+        const double2* Mrow = Mf + fidx(n, 0);
+#pragma unroll 2
+        for (int m = -n; m <= n; ++m) {
+            const double2 s = Srow[m];
+#pragma unroll
+            for (int i = 0; i < NV; ++i) cfma(tmp[i], Mrow[i * mstride + m], s);
+        }
+    }
+}
+
+__host__ __device__ inline int m2l_smem_bytes(int p) {
+    return (int)sizeof(double2) * ((2 * p + 1) * (2 * p + 1) + 8 * (p + 1) * (p + 1));
+}
+
+__global__ void __launch_bounds__(256) m2l_kernel(const Geom G, const M2LArgs A, const double2* __restrict__ M,
+                                                  const double2* __restrict__ Stab, const int* __restrict__ nm,
+                                                  double2* __restrict__ Lpart) {
+    extern __shared__ __align__(16) double2 sm2[];
+    __shared__ ImageBox sib[8];
+    __shared__ int slot_sib[8];
+    __shared__ int s_nv, s_lo, s_hi;
+    const int p = G.p, NC = nc(p), NS = nc(2 * p), NF = (p + 1) * (p + 1), NSF = (2 * p + 1) * (2 * p + 1);
+    double2* Sfull = sm2;
+    double2* Mfull = sm2 + NSF;
+    const int tid = threadIdx.x;
+    int r = 0;
+    while (r + 1 < A.n_lv && (int)blockIdx.x >= A.lv[r + 1].first_cta) ++r;
+    const M2LLevel lv = A.lv[r];
+    const int local = blockIdx.x - lv.first_cta, group = local / lv.n_split, split = local - group * lv.n_split;
+    const int lev = lv.lev;
+    const int nsib = lev == 0 ? 1 : 8;
+    int P[3];   // parent coordinates (level 0: the box itself)
+    {
+        const int gl = lev == 0 ? 0 : lev - 1;
+        const int ny = grid_n(G, gl, 1), nz = grid_n(G, gl, 2);
+        P[2] = group % nz; P[1] = (group / nz) % ny; P[0] = group / (nz * ny);
+    }
+    if (tid == 0) {   // this split's share of the offsets, by weight
+        const int W = A.off_wprefix[A.n_off];
+        const long long w_lo = (long long)W * split / lv.n_split, w_hi = (long long)W * (split + 1) / lv.n_split;
+        int lo = 0, hi = A.n_off;
+        while (lo < hi) { const int mid = (lo + hi) >> 1; if (A.off_wprefix[mid] < w_lo) lo = mid + 1; else hi = mid; }
+        s_lo = lo;
+        lo = 0; hi = A.n_off;
+        while (lo < hi) { const int mid = (lo + hi) >> 1; if (A.off_wprefix[mid] < w_hi) lo = mid + 1; else hi = mid; }
+        s_hi = lo;
+    }
+    __syncthreads();
+    const int o_lo = s_lo, o_hi = s_hi;
+    const long long nb = boxes_at(G, lev);
+    const double2* Mlev = M + level_offset(G, lev) * NC;
+    const int ny = grid_n(G, lev, 1), nz = grid_n(G, lev, 2);
+
+    for (int c0 = 0; c0 < NC; c0 += 256) {
+        const int c = c0 + tid;
+        const bool have = c < NC;
+        const int k = have ? (nm[c] >> 8) : 0, l = have ? (nm[c] & 255) : 0;
+        double2 acc[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) acc[i] = make_double2(0.0, 0.0);
+        for (int oi = o_lo; oi < o_hi; ++oi) {
+            const int off = A.off_list[oi];
+            const int dx = off / (kOffW * kOffW) - kOffR, dy = (off / kOffW) % kOffW - kOffR, dz = off % kOffW - kOffR;
+            __syncthreads();   // the previous offset's reads of Sfull / Mfull / sib are done
+            if (tid < 32) {
+                bool ok = false;
+                ImageBox ib;
+                if (tid < nsib) {
+                    const int t[3] = {lev == 0 ? P[0] : 2 * P[0] + ((tid >> 2) & 1), lev == 0 ? P[1] : 2 * P[1] + ((tid >> 1) & 1),
+                                      lev == 0 ? P[2] : 2 * P[2] + (tid & 1)};
+                    const int g[3] = {t[0] + dx, t[1] + dy, t[2] + dz};
+                    ok = true;
+                    if (lev > 0)   // the source's parent must be within kWs of the target's parent
+                        for (int a = 0; a < 3; ++a) ok = ok && g[a] >= 2 * (P[a] - kWs) && g[a] <= 2 * (P[a] + kWs) + 1;
+                    ok = ok && image_box(G, lev, g[0], g[1], g[2], ib);
+                }
+                const unsigned mask = __ballot_sync(0xffffffffu, ok);
+                if (ok) {
+                    const int slot = __popc(mask & ((1u << tid) - 1u));
+                    sib[slot] = ib;
+                    slot_sib[slot] = tid;
+                }
+                if (tid == 0) s_nv = __popc(mask);
+            }
+            __syncthreads();
+            const int nv = s_nv;
+            if (nv == 0) continue;
+            // S(t - g) = S(-d), expanded to negative orders
+            const double2* S = Stab + (long long)(((kOffR - dx) * kOffW + (kOffR - dy)) * kOffW + (kOffR - dz)) * NS;
+            for (int t = tid; t < NSF; t += 256) {
+                int N = (int)sqrt((double)t);
+                while (N * N > t) --N;
+                while ((N + 1) * (N + 1) <= t) ++N;
+                const int mu = t - N * N - N;
+                double2 v = S[cidx(N, mu < 0 ? -mu : mu)];
+                if (mu < 0) v = (mu & 1) ? make_double2(-v.x, v.y) : make_double2(v.x, -v.y);
+                Sfull[t] = v;
+            }
+            // conj of the (reflected, weighted) source moments, expanded to negative orders
+            for (int t = tid; t < nv * NC; t += 256) {
+                const int s = t / NC, cc = t - s * NC;
+                const ImageBox ib = sib[s];
+                const int n = nm[cc] >> 8, m = nm[cc] & 255;
+                double2 v = Mlev[(long long)ib.box * NC + cc];
+                if (ib.fx) v = (m & 1) ? make_double2(-v.x, v.y) : make_double2(v.x, -v.y);   // (-1)^m conj
+                if (ib.fy) v.y = -v.y;                                                         // conj
+                if (ib.fz && ((n + m) & 1)) { v.x = -v.x; v.y = -v.y; }
+                v.x *= ib.w; v.y *= ib.w;
+                double2* dst = Mfull + s * NF;
+                dst[fidx(n, m)] = make_double2(v.x, -v.y);
+                if (m > 0) dst[fidx(n, -m)] = (m & 1) ? make_double2(-v.x, -v.y) : v;
+            }
+            __syncthreads();
+            int done = 0;
+            while (done < nv) {
+                const int left = nv - done;
+                const double2* Mf = Mfull + done * NF;
+                if (left >= 8) {
+                    double2 tmp[8];
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) tmp[i] = make_double2(0.0, 0.0);
+                    m2l_inner<8>(Sfull, Mf, NF, p, k, l, tmp);
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        const int sid = slot_sib[done + i];
+#pragma unroll
+                        for (int j = 0; j < 8; ++j) if (j == sid) { acc[j].x += tmp[i].x; acc[j].y += tmp[i].y; }
+                    }
+                    done += 8;
+                } else if (left >= 4) {
+                    double2 tmp[4];
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) tmp[i] = make_double2(0.0, 0.0);
+                    m2l_inner<4>(Sfull, Mf, NF, p, k, l, tmp);
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        const int sid = slot_sib[done + i];
+#pragma unroll
+                        for (int j = 0; j < 8; ++j) if (j == sid) { acc[j].x += tmp[i].x; acc[j].y += tmp[i].y; }
+                    }
+                    done += 4;
+                } else if (left >= 2) {
+                    double2 tmp[2];
+                    tmp[0] = make_double2(0.0, 0.0); tmp[1] = make_double2(0.0, 0.0);
+                    m2l_inner<2>(Sfull, Mf, NF, p, k, l, tmp);
+#pragma unroll
+                    for (int i = 0; i < 2; ++i) {
+                        const int sid = slot_sib[done + i];
+#pragma unroll
+                        for (int j = 0; j < 8; ++j) if (j == sid) { acc[j].x += tmp[i].x; acc[j].y += tmp[i].y; }
+                    }
+                    done += 2;
+                } else {
+                    double2 tmp[1];
+                    tmp[0] = make_double2(0.0, 0.0);
+                    m2l_inner<1>(Sfull, Mf, NF, p, k, l, tmp);
+                    const int sid = slot_sib[done];
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) if (j == sid) { acc[j].x += tmp[0].x; acc[j].y += tmp[0].y; }
+                    done += 1;
+                }
+            }
+        }
+        if (have) {
+            const double sg = (k & 1) ? -1.0 : 1.0;
+#pragma unroll
+            for (int s = 0; s < 8; ++s) {
+                if (s < nsib) {
+                    const int tx = lev == 0 ? P[0] : 2 * P[0] + ((s >> 2) & 1), ty = lev == 0 ? P[1] : 2 * P[1] + ((s >> 1) & 1),
+                              tz = lev == 0 ? P[2] : 2 * P[2] + (s & 1);
+                    const long long box = ((long long)tx * ny + ty) * nz + tz;
+                    Lpart[lv.part_off + ((long long)split * nb + box) * NC + c] = make_double2(sg * acc[s].x, sg * acc[s].y);
+                }
+            }
+        }
+    }
+}
+
+// ---- leaves: L2P + P2P --------------------------------------------------------------------------------------------------
+// One CTA = 256 consecutive particles of the leaf-sorted array (one target per thread); the leaves it spans are worked
+// through one after the other (threads of other leaves idle).  For a leaf: its local expansion is evaluated at the
+// targets (L2P), then the 5^3 neighbour boxes -- images through the near cell table, never materialised -- are summed
+// directly (P2P) from 256-source tiles in shared memory with the pair arithmetic of near_sum_kernel: the target is
+// moved into the image's frame, sigma o (t - kL); only the bare self term (central cell, same particle) is masked.
+// dynamic shared memory: Ls [NC] double2, inv [(p+1) * kInvW] double
+template <int REFINE>
+__global__ void __launch_bounds__(256) leaf_kernel(const Geom G, const Src4* __restrict__ srt, const int* __restrict__ key,
+                                                   const int* __restrict__ idx, const int* __restrict__ leaf_start, long long N,
+                                                   const double2* __restrict__ L, double* __restrict__ phi_out) {
+    extern __shared__ __align__(16) double2 sm2[];
+    __shared__ __align__(16) Src4 tile[256];
+    const int p = G.p, NC = nc(p), lev = G.levels;
+    double2* Ls = sm2;
+    double* inv = reinterpret_cast<double*>(sm2 + NC);
+    const int tid = threadIdx.x;
+    fill_inv_table(inv, p);
+    const long long pos = (long long)blockIdx.x * 256 + tid;
+    const bool valid = pos < N;
+    const Src4 me = valid ? srt[pos] : Src4{0.0, 0.0, 0.0, 0.0};
+    const int my_leaf = valid ? key[pos] : -1;
+    const int leaf_lo = key[(long long)blockIdx.x * 256];
+    const int leaf_hi = key[min(N - 1, (long long)blockIdx.x * 256 + 255)];
+    const double a = G.a0 / (double)(1 << lev), ia = 1.0 / a;
+    const double2* Llev = L + level_offset(G, lev) * NC;
+    const double scale = REFINE == 1 ? 0.5 : 1.0;
+    double total = 0.0;
+
+    for (int leaf = leaf_lo; leaf <= leaf_hi; ++leaf) {
+        if (leaf_start[leaf] == leaf_start[leaf + 1]) continue;
+        const bool active = my_leaf == leaf;
+        double c[3]; int ic[3];
+        box_centre(G, lev, leaf, c, ic);
+        __syncthreads();
+        for (int t = tid; t < NC; t += 256) Ls[t] = Llev[(long long)leaf * NC + t];
+        __syncthreads();
+        if (active) {   // L2P: (1/a) Re sum conj R_n^m L_n^m, m < 0 folded in (factor 2)
+            const double x = (me.x - c[0]) * ia, y = (me.y - c[1]) * ia, z = (me.z - c[2]) * ia;
+            const double r2 = fma(z, z, fma(y, y, x * x));
+            double rr = 1.0, ri = 0.0, far = 0.0;
+            for (int m = 0; m <= p; ++m) {
+                if (m > 0) { const double f = 0.5 / (double)m, u = (rr * x - ri * y) * f; ri = (rr * y + ri * x) * f; rr = u; }
+                double p1r = rr, p1i = ri, p2r = 0.0, p2i = 0.0;
+                double2 lc = Ls[cidx(m, m)];
+                double s = fma(rr, lc.x, ri * lc.y);
+                for (int n = m + 1; n <= p; ++n) {
+                    const double f = inv[n * kInvW + m], tz = (double)(2 * n - 1) * z;
+                    const double cr = (tz * p1r - r2 * p2r) * f, ci = (tz * p1i - r2 * p2i) * f;
+                    lc = Ls[cidx(n, m)];
+                    s = fma(cr, lc.x, s); s = fma(ci, lc.y, s);
+                    p2r = p1r; p2i = p1i; p1r = cr; p1i = ci;
+                }
+                far += m == 0 ? s : 2.0 * s;
+            }
+            total += far * ia;
+        }
+        for (int dx = -kWs; dx <= kWs; ++dx)
+            for (int dy = -kWs; dy <= kWs; ++dy)
+                for (int dz = -kWs; dz <= kWs; ++dz) {
+                    ImageBox ib;
+                    if (!image_box(G, lev, ic[0] + dx, ic[1] + dy, ic[2] + dz, ib)) continue;
+                    const int s0 = leaf_start[ib.box], s1 = leaf_start[ib.box + 1];
+                    if (s0 == s1) continue;
+                    const double tx = flip(me.x - ib.sx, ib.fx), ty = flip(me.y - ib.sy, ib.fy), tz = flip(me.z - ib.sz, ib.fz);
+                    const bool self_here = ib.central && dx == 0 && dy == 0 && dz == 0;
+                    double acc = 0.0;
+                    for (int base = s0; base < s1; base += 256) {
+                        __syncthreads();
+                        tile[tid] = base + tid < s1 ? srt[base + tid] : Src4{kFar, kFar, kFar, 0.0};
+                        __syncthreads();
+                        if (!active) continue;
+                        const int cnt = min(256, s1 - base);
+                        if (self_here) {
+                            const long long sj = pos - base;
+#pragma unroll 2
+                            for (int j = 0; j < cnt; ++j) {
+                                const bool self = j == sj;
+                                pair<REFINE>(tx, ty, tz, self ? tx + 1.0 : tile[j].x, self ? ty : tile[j].y, self ? tz : tile[j].z,
+                                             self ? 0.0 : tile[j].q, acc);
+                            }
+                        } else {
+#pragma unroll 4
+                            for (int j = 0; j < cnt; ++j) pair<REFINE>(tx, ty, tz, tile[j].x, tile[j].y, tile[j].z, tile[j].q, acc);
+                        }
+                    }
+                    total = fma(ib.w * scale, acc, total);
+                }
+    }
+    if (valid) phi_out[idx[pos]] = total;
+}
+
+}  // namespace fmm
+}  // namespace hsma

@@ -10,6 +10,7 @@
 
 #include "common.cuh"
 #include "fit_kernels.cuh"
+#include "fmm_host.cuh"
 #include "geometry.h"
 #include "hsma.h"
 #include "peak.cuh"
@@ -335,6 +336,7 @@ struct hsma_plan {
     DevBuf<double> part_a, part_b, part_c, red, xyz_in, q_in, phi_dev, force_dev;
     DevBuf<double> sym_col, sym_phi;   // symmetric form of step (b): column sums per visit of one wave, phi_near in source order
     size_t sym_col_cap = kSymColCapDefault;   // hsma_plan_set_sym_scratch_cap: bytes of column scratch per wave
+    hsma::fmm::State fmm;              // near_algorithm = FMM: tables and scratch of the sub-quadratic form of step (b)
     int pair_form = 0;                 // hsma_plan_set_pair_form: 0 = automatic, 1 = ordered pairs only, 2 = symmetric wherever possible
     int last_pair_form = 1;            // what the last evaluate used for step (b): 1 ordered, 2 symmetric
     long long last_launches = 0;
@@ -377,6 +379,7 @@ static void plan_free(hsma_plan* p) {
     p->img_slot_of.release(); p->img_tile_np.release();
     p->part_a.release(); p->part_b.release(); p->part_c.release(); p->red.release(); p->sym_col.release(); p->sym_phi.release();
     p->xyz_in.release(); p->q_in.release(); p->phi_dev.release(); p->force_dev.release();
+    p->fmm.release();
     for (cudaEvent_t e : p->ev) if (e) cudaEventDestroy(e);
     if (p->gexec) cudaGraphExecDestroy(p->gexec);
     delete p;
@@ -401,6 +404,7 @@ extern "C" hsma_status hsma_plan_create_ex(const hsma_plan_desc* desc, void* cud
     if (d.dipole_mode != HSMA_DIPOLE_EXACT && d.dipole_mode != HSMA_DIPOLE_FD3) return HSMA_ERR_INVALID_ARG;
     if (d.near_mode == HSMA_NEAR_SPHERE && d.closure == HSMA_CLOSURE_FAR_DATA) return HSMA_ERR_INVALID_ARG;
     if (d.fd_dr_rel < 0.0 || d.fd_dr_rel > 0.1) return HSMA_ERR_INVALID_ARG;
+    if (d.near_algorithm != HSMA_NEAR_ALG_DIRECT && d.near_algorithm != HSMA_NEAR_ALG_FMM) return HSMA_ERR_INVALID_ARG;
     for (int a = 0; a < 3; ++a)
         if (!(d.L[a] > 0.0) || d.near_shell[a] < 0 || d.near_shell[a] > 8) return HSMA_ERR_INVALID_ARG;
     if (d.kind == HSMA_BC_PERIODIC && d.closure == HSMA_CLOSURE_FAR_DATA) return HSMA_ERR_INVALID_ARG;
@@ -451,6 +455,12 @@ extern "C" hsma_status hsma_plan_create_ex(const hsma_plan_desc* desc, void* cud
         for (int c = 0; c < (int)near.size(); ++c) if (!near[c].central) order.push_back(c);
         PCU(upload(&p->cell_order, order, st));
         PCU(cudaMalloc(&p->img_qinfo, sizeof(QInfo)));
+    }
+    if (d.near_algorithm == HSMA_NEAR_ALG_FMM) {
+        bool refl[3];
+        reflecting_axes(d.kind, refl);
+        const hsma_status fs = fmm::setup(p->fmm, d, refl, st);
+        if (fs != HSMA_OK) { plan_free(p); return fs; }
     }
     if (rhsc.empty()) { p->cells_rhs = p->cells_near; p->C_rhs = p->C_near; }
     else { p->C_rhs = (int)rhsc.size(); PCU(upload(&p->cells_rhs, rhsc, st)); }
@@ -800,8 +810,11 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
         const int refine = p->refine ? p->refine : ((double)N * (double)p->last_images < 4294967296.0 ? 2 : 1);
         // rsqrt_refine = 0: the cubic step while (b) is latency-bound anyway (< 2^32 pairs), Newton above
         const size_t comps = field ? 4 : 1;
-        bool sym = !p->sphere && p->pair_form != 1 && t0 == 0 && t1 == N && sym_applies(n_tiles, C_b);
+        // near_algorithm = FMM: step (b) over all N targets (potentials) by the fast multipole method, DESIGN.md 6.13
+        const bool use_fmm = p->fmm.enabled && !field && t0 == 0 && t1 == N && p->pair_form == 0;
+        bool sym = !use_fmm && !p->sphere && p->pair_form != 1 && t0 == 0 && t1 == N && sym_applies(n_tiles, C_b);
         Launch sb = choose_near(T, n_tiles_near, C_b, refine, field);
+        if (use_fmm && p->sym_phi.reserve((size_t)N) != cudaSuccess) return HSMA_ERR_ALLOC;
         SymLaunch ss{};
         if (sym) {
             ss = choose_sym(n_tiles, refine, p->sym_col_cap, 0, 1, field);
@@ -812,13 +825,17 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
                 sym = false;
             }
         }
-        if (!sym && p->part_b.reserve((size_t)sb.rows * T * comps) != cudaSuccess) return HSMA_ERR_ALLOC;
-        p->last_pair_form = sym ? 2 : 1;
+        if (!sym && !use_fmm && p->part_b.reserve((size_t)sb.rows * T * comps) != cudaSuccess) return HSMA_ERR_ALLOC;
+        p->last_pair_form = use_fmm ? 3 : (sym ? 2 : 1);
         const Launch sc = choose_node(T, p->node_tiles, field);
         if (p->part_c.reserve((size_t)sc.rows * T * comps) != cudaSuccess) return HSMA_ERR_ALLOC;
         MARK(3);
         PartLayout layout_b = sb.layout(p->part_b.p);
-        if (sym) {
+        if (use_fmm) {
+            const hsma_status fs = fmm::near_sum(p->fmm, xyz, q, N, p->half, refine, p->sym_phi.p, g_alloc_epoch, st);
+            if (fs != HSMA_OK) return fs;
+            layout_b = PartLayout{p->sym_phi.p, 1, 1, 1, (int)std::min<long long>(T, 2147483647LL)};
+        } else if (sym) {
             // every unordered (source, source) pair once: row sums + column sums, then phi_near in source order
             launch_sym(p, ss, field, refine, cells_b, C_b, N, n_tiles, st);
             layout_b = PartLayout{p->sym_phi.p, 1, 1, 1, (int)std::min<long long>(T, 2147483647LL)};
@@ -1268,7 +1285,7 @@ extern "C" long long hsma_plan_scratch_bytes(const hsma_plan* p) {
     size_t b = p->src.cap * sizeof(Src4) + (p->slot_of.cap + p->tile_np.cap) * sizeof(int) +
                (p->part_a.cap + p->part_b.cap + p->part_c.cap + p->red.cap + p->sym_col.cap + p->sym_phi.cap) * sizeof(double) +
                p->img_counts.cap * sizeof(long long) + (p->img_xyz.cap + p->img_q.cap + p->img_stats.cap) * sizeof(double) +
-               p->img_src.cap * sizeof(Src4) + (p->img_slot_of.cap + p->img_tile_np.cap) * sizeof(int);
+               p->img_src.cap * sizeof(Src4) + (p->img_slot_of.cap + p->img_tile_np.cap) * sizeof(int) + p->fmm.scratch_bytes();
     return (long long)b;
 }
 
