@@ -36,21 +36,21 @@ struct State {
     double a0 = 0.0, L[3] = {0, 0, 0};
     double* w_lut = nullptr;
     double2 *Rsh = nullptr, *Stab = nullptr;
-    int *nm = nullptr, *off_list = nullptr, *off_wprefix = nullptr;
-    int n_off = 0;
-    Buf<int> key_a, key_b, idx_a, idx_b, leaf_start;
+    int *nm = nullptr, *pm = nullptr, *sfmap = nullptr, *off_list = nullptr, *off_wprefix = nullptr;
+    int n_off = 0, W = 0;      // offsets of the M2L list and their total weight
+    Buf<int> key_a, key_b, idx_a, idx_b, leaf_start, chunk_start;
     Buf<long long> counts;
     Buf<Src4> srt;
     Buf<double2> Mx, Lx, Lpart;   // multipole / local expansions of all levels, M2L partial sums
     double* phi = nullptr;     // not owned: the plan's sym_phi buffer
     void release() {
-        for (void* q : {(void*)w_lut, (void*)Rsh, (void*)Stab, (void*)nm, (void*)off_list, (void*)off_wprefix}) if (q) cudaFree(q);
-        w_lut = nullptr; Rsh = Stab = nullptr; nm = off_list = off_wprefix = nullptr;
-        key_a.release(); key_b.release(); idx_a.release(); idx_b.release(); leaf_start.release(); counts.release();
+        for (void* q : {(void*)w_lut, (void*)Rsh, (void*)Stab, (void*)nm, (void*)pm, (void*)sfmap, (void*)off_list, (void*)off_wprefix}) if (q) cudaFree(q);
+        w_lut = nullptr; Rsh = Stab = nullptr; nm = pm = sfmap = off_list = off_wprefix = nullptr;
+        key_a.release(); key_b.release(); idx_a.release(); idx_b.release(); leaf_start.release(); chunk_start.release(); counts.release();
         srt.release(); Mx.release(); Lx.release(); Lpart.release();
     }
     size_t scratch_bytes() const {
-        return (key_a.cap + key_b.cap + idx_a.cap + idx_b.cap + leaf_start.cap) * sizeof(int) + counts.cap * sizeof(long long) +
+        return (key_a.cap + key_b.cap + idx_a.cap + idx_b.cap + leaf_start.cap + chunk_start.cap) * sizeof(int) + counts.cap * sizeof(long long) +
                srt.cap * sizeof(Src4) + (Mx.cap + Lx.cap + Lpart.cap) * sizeof(double2);
     }
 };
@@ -97,6 +97,7 @@ inline hsma_status setup(State& S, const hsma_plan_desc& d, const bool refl[3], 
                 wpre.push_back(wpre.back() + w);
             }
     S.n_off = (int)off.size();
+    S.W = wpre.back();
     const int NC = nc(S.p), NS = nc(2 * S.p);
 #define FCU(x) do { if ((x) != cudaSuccess) return HSMA_ERR_CUDA; } while (0)
     FCU(cudaMalloc(&S.w_lut, lut.size() * sizeof(double)));
@@ -108,7 +109,10 @@ inline hsma_status setup(State& S, const hsma_plan_desc& d, const bool refl[3], 
     FCU(cudaMalloc(&S.Rsh, 8 * (size_t)NC * sizeof(double2)));
     FCU(cudaMalloc(&S.Stab, (size_t)kOffN * NS * sizeof(double2)));
     FCU(cudaMalloc(&S.nm, NC * sizeof(int)));
-    tables_kernel<<<(std::max(kOffN, NC) + 127) / 128, 128, 0, st>>>(S.p, S.Rsh, S.Stab, S.nm);
+    FCU(cudaMalloc(&S.pm, m2l_pairs(S.p) * sizeof(int)));
+    const int NSF = (2 * S.p + 1) * (2 * S.p + 1);
+    FCU(cudaMalloc(&S.sfmap, NSF * sizeof(int)));
+    tables_kernel<<<(std::max({kOffN, NC, NSF}) + 127) / 128, 128, 0, st>>>(S.p, S.Rsh, S.Stab, S.nm, S.pm, S.sfmap);
     HSMA_COUNT_LAUNCH();
     FCU(cudaStreamSynchronize(st));   // the host vectors above go out of scope
     FCU(cudaFuncSetAttribute(m2l_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, m2l_smem_bytes(S.p)));
@@ -134,7 +138,7 @@ inline int resident_m2l(int p) {
     int per_sm = 0, dev = 0, sms = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, m2l_kernel, 256, m2l_smem_bytes(p)) != cudaSuccess || per_sm < 1) {
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, m2l_kernel, kM2LThreads, m2l_smem_bytes(p)) != cudaSuccess || per_sm < 1) {
         cudaGetLastError();
         per_sm = 1;
     }
@@ -155,31 +159,32 @@ inline hsma_status near_sum(State& S, const double* xyz, const double* q, long l
     const long long n_leaves = boxes_at(G, G.levels), n_boxes = level_offset(G, G.levels + 1);
     if (n_leaves >= 65536) return HSMA_ERR_INVALID_ARG;
     const long long n_blk = (N + 255) / 256;
-    // M2L launch shape: per level, groups x splits CTAs; splits fill about two waves of the resident CTAs
+    // M2L launch shape: one persistent wave over the units (group, offset weight), deepest level first
     M2LArgs A;
     A.n_lv = 0;
-    const int slots = resident_m2l(S.p);
-    int ctas = 0;
-    long long part_elems = 0;
-    int split_of[kMaxLevels];
-    for (int lev = 0; lev <= G.levels; ++lev) {
+    A.W = S.W;
+    int n_groups_total = 0;
+    for (int lev = G.levels; lev >= 0; --lev) {
         M2LLevel& r = A.lv[A.n_lv++];
         r.lev = lev;
         r.n_groups = (int)(lev == 0 ? boxes_at(G, 0) : boxes_at(G, lev - 1));
-        r.n_split = (int)std::max<long long>(1, std::min<long long>(64, (2LL * slots + r.n_groups - 1) / r.n_groups));
-        if (lev == 0) r.n_split = std::min(r.n_split, 8);
-        r.first_cta = ctas;
-        r.part_off = part_elems;
-        ctas += r.n_groups * r.n_split;
-        part_elems += (long long)r.n_split * boxes_at(G, lev) * NC;
-        split_of[lev] = r.n_split;
+        r.first_group = n_groups_total;
+        n_groups_total += r.n_groups;
+    }
+    A.units = (long long)n_groups_total * A.W;
+    const int Gm2l = (int)std::min<long long>(resident_m2l(S.p), A.units);
+    A.rows = part_rows(A.units, A.W, Gm2l);
+    long long part_elems = 0;
+    for (int r = 0; r < A.n_lv; ++r) {
+        A.lv[r].part_off = part_elems;
+        part_elems += (long long)A.rows * boxes_at(G, A.lv[r].lev) * NC;
     }
     A.off_list = S.off_list; A.off_wprefix = S.off_wprefix; A.n_off = S.n_off;
 #define FR(x) do { if ((x) != cudaSuccess) return HSMA_ERR_ALLOC; } while (0)
     FR(S.key_a.reserve((size_t)N, epoch)); FR(S.key_b.reserve((size_t)N, epoch));
     FR(S.idx_a.reserve((size_t)N, epoch)); FR(S.idx_b.reserve((size_t)N, epoch));
-    FR(S.leaf_start.reserve((size_t)n_leaves + 1, epoch));
-    FR(S.counts.reserve((size_t)(256 * n_blk + 1), epoch));
+    FR(S.leaf_start.reserve((size_t)n_leaves + 1, epoch)); FR(S.chunk_start.reserve((size_t)n_leaves + 1, epoch));
+    FR(S.counts.reserve((size_t)(256 * n_blk + 256), epoch));
     FR(S.srt.reserve((size_t)N, epoch));
     FR(S.Mx.reserve((size_t)n_boxes * NC, epoch)); FR(S.Lx.reserve((size_t)n_boxes * NC, epoch));
     FR(S.Lpart.reserve((size_t)part_elems, epoch));
@@ -194,9 +199,10 @@ inline hsma_status near_sum(State& S, const double* xyz, const double* q, long l
         int* kout = pass == 0 ? S.key_b.p : S.key_a.p;
         int* iout = pass == 0 ? S.idx_b.p : S.idx_a.p;
         radix_hist_kernel<<<gN, 256, 0, st>>>(kin, N, 8 * pass, n_blk, S.counts.p);
-        scan_counts_kernel<<<1, 1024, 0, st>>>(S.counts.p, 256 * n_blk);
-        radix_scatter_kernel<<<gN, 256, 0, st>>>(kin, iin, N, 8 * pass, n_blk, S.counts.p, kout, iout);
-        HSMA_COUNT_LAUNCH(); HSMA_COUNT_LAUNCH(); HSMA_COUNT_LAUNCH();
+        radix_rowscan_kernel<<<256, 1024, 0, st>>>(S.counts.p, n_blk, S.counts.p + 256 * n_blk);
+        radix_base_kernel<<<1, 256, 0, st>>>(S.counts.p + 256 * n_blk);
+        radix_scatter_kernel<<<gN, 256, 0, st>>>(kin, iin, N, 8 * pass, n_blk, S.counts.p, S.counts.p + 256 * n_blk, kout, iout);
+        HSMA_COUNT_LAUNCH(); HSMA_COUNT_LAUNCH(); HSMA_COUNT_LAUNCH(); HSMA_COUNT_LAUNCH();
     }
     leaf_start_kernel<<<(unsigned)((n_leaves + 1 + 255) / 256), 256, 0, st>>>(S.key_a.p, N, (int)n_leaves, S.leaf_start.p);
     gather_sorted_kernel<<<gN, 256, 0, st>>>(xyz, q, S.idx_a.p, N, half[0], half[1], half[2], S.srt.p);
@@ -210,16 +216,18 @@ inline hsma_status near_sum(State& S, const double* xyz, const double* q, long l
         HSMA_COUNT_LAUNCH();
     }
     // far field: M2L at every level, then down
-    m2l_kernel<<<(unsigned)ctas, 256, m2l_smem_bytes(S.p), st>>>(G, A, S.Mx.p, S.Stab, S.nm, S.Lpart.p);
+    m2l_kernel<<<(unsigned)Gm2l, kM2LThreads, m2l_smem_bytes(S.p), st>>>(G, A, S.Mx.p, S.Stab, S.nm, S.pm, S.sfmap, S.Lpart.p);
     HSMA_COUNT_LAUNCH();
     for (int lev = 0; lev <= G.levels; ++lev) {
-        l2l_kernel<<<(unsigned)boxes_at(G, lev), 256, 2 * NC * sizeof(double2), st>>>(G, lev, S.Rsh, S.nm, S.Lpart.p + A.lv[lev].part_off,
-                                                                                  split_of[lev], S.Lx.p);
+        l2l_kernel<<<(unsigned)boxes_at(G, lev), 256, 2 * NC * sizeof(double2), st>>>(G, lev, S.Rsh, S.nm, S.Lpart.p, A, Gm2l, S.Lx.p);
         HSMA_COUNT_LAUNCH();
     }
     const size_t leaf_smem = NC * sizeof(double2) + inv_bytes;
-    if (refine == 1) leaf_kernel<1><<<gN, 256, leaf_smem, st>>>(G, S.srt.p, S.key_a.p, S.idx_a.p, S.leaf_start.p, N, S.Lx.p, phi_out);
-    else leaf_kernel<2><<<gN, 256, leaf_smem, st>>>(G, S.srt.p, S.key_a.p, S.idx_a.p, S.leaf_start.p, N, S.Lx.p, phi_out);
+    leaf_chunks_kernel<<<1, 1024, 0, st>>>(S.leaf_start.p, (int)n_leaves, S.chunk_start.p);
+    HSMA_COUNT_LAUNCH();
+    const unsigned gl = (unsigned)(N / (kLeafThreads * kLeafR) + n_leaves);
+    if (refine == 1) leaf_kernel<1><<<gl, kLeafThreads, leaf_smem, st>>>(G, S.srt.p, S.idx_a.p, S.leaf_start.p, S.chunk_start.p, (int)n_leaves, S.Lx.p, phi_out);
+    else leaf_kernel<2><<<gl, kLeafThreads, leaf_smem, st>>>(G, S.srt.p, S.idx_a.p, S.leaf_start.p, S.chunk_start.p, (int)n_leaves, S.Lx.p, phi_out);
     HSMA_COUNT_LAUNCH();
     return HSMA_OK;
 }

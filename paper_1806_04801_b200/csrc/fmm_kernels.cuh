@@ -126,11 +126,52 @@ __global__ void __launch_bounds__(256) radix_hist_kernel(const int* __restrict__
     __syncthreads();
     counts[(long long)threadIdx.x * n_blk + blockIdx.x] = h[threadIdx.x];
 }
+// counts[d][b] (digit-major) -> exclusive prefix over the blocks b of row d; tot[d] = row total.  One CTA per digit.
+__global__ void __launch_bounds__(1024) radix_rowscan_kernel(long long* __restrict__ counts, long long n_blk, long long* __restrict__ tot) {
+    __shared__ long long wsum[32];
+    __shared__ long long carry;
+    long long* row = counts + (long long)blockIdx.x * n_blk;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (threadIdx.x == 0) carry = 0;
+    __syncthreads();
+    for (long long base = 0; base < n_blk; base += 1024) {
+        const long long i = base + threadIdx.x;
+        const long long v = i < n_blk ? row[i] : 0;
+        long long x = v;
+        for (int o = 1; o < 32; o <<= 1) { const long long y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+        if (lane == 31) wsum[warp] = x;
+        __syncthreads();
+        if (warp == 0) {
+            long long w = wsum[lane];
+            for (int o = 1; o < 32; o <<= 1) { const long long y = __shfl_up_sync(0xffffffffu, w, o); if (lane >= o) w += y; }
+            wsum[lane] = w;
+        }
+        __syncthreads();
+        const long long before = carry + (warp > 0 ? wsum[warp - 1] : 0);
+        if (i < n_blk) row[i] = before + x - v;
+        __syncthreads();
+        if (threadIdx.x == 0) carry += wsum[31];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) tot[blockIdx.x] = carry;
+}
+// tot[256] -> exclusive prefix (digit bases), in place.  One warp-scan per 32, single block of 256.
+__global__ void __launch_bounds__(256) radix_base_kernel(long long* __restrict__ tot) {
+    __shared__ long long sh[256];
+    sh[threadIdx.x] = tot[threadIdx.x];
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        long long run = 0;
+        for (int d = 0; d < 256; ++d) { const long long v = sh[d]; sh[d] = run; run += v; }
+    }
+    __syncthreads();
+    tot[threadIdx.x] = sh[threadIdx.x];
+}
 // stable: items keep their order within a digit (lane order in a warp, warp order in a block, block order)
 __global__ void __launch_bounds__(256) radix_scatter_kernel(const int* __restrict__ key_in, const int* __restrict__ idx_in,
                                                             long long N, int shift, long long n_blk,
-                                                            const long long* __restrict__ offs, int* __restrict__ key_out,
-                                                            int* __restrict__ idx_out) {
+                                                            const long long* __restrict__ offs, const long long* __restrict__ dbase,
+                                                            int* __restrict__ key_out, int* __restrict__ idx_out) {
     __shared__ int cnt[8][256];
     for (int k = threadIdx.x; k < 8 * 256; k += 256) (&cnt[0][0])[k] = 0;
     __syncthreads();
@@ -146,7 +187,7 @@ __global__ void __launch_bounds__(256) radix_scatter_kernel(const int* __restric
     if (valid) {
         int before = 0;
         for (int w = 0; w < warp; ++w) before += cnt[w][d];
-        const long long pos = offs[(long long)d * n_blk + blockIdx.x] + before + rank;
+        const long long pos = dbase[d] + offs[(long long)d * n_blk + blockIdx.x] + before + rank;
         key_out[pos] = kv;
         idx_out[pos] = idx_in[i];
     }
@@ -239,14 +280,46 @@ __global__ void __launch_bounds__(256) p2m_kernel(const Geom G, const Src4* __re
     }
 }
 
+// ---- M2L work decomposition (used by m2l_kernel and by l2l_kernel, which adds its partial rows) -----------------------
+// Work decomposition as in the pair kernels (sum_kernels.cuh "persistent work decomposition"): the linear sequence of
+// units u = group * W + w -- groups of all levels, deepest level first; W = total offset weight of a group -- is dealt
+// to a persistent grid in contiguous ranges, so every CTA gets the same weight to within one offset.  A CTA writes
+// one partial row per group it touches, row = CTA - first CTA of the group; l2l_kernel adds the rows in that order.
+struct M2LLevel { int lev, n_groups, first_group; long long part_off; };   // part_off: this level's rows in Lpart (double2)
+struct M2LArgs {
+    M2LLevel lv[kMaxLevels];  // deepest level first
+    int n_lv;
+    int rows;                 // partial rows per group
+    long long units;          // n_groups_total * W
+    const int* off_list;      // [n_off] dense offset indices (g - t), |d|_inf > kWs, processing order
+    const int* off_wprefix;   // [n_off + 1] prefix sums of the offset weights (how many of 8 siblings have it)
+    int n_off, W;
+};
+__host__ __device__ inline int m2l_level_record(const M2LArgs& A, int lev) {
+    for (int r = 0; r < A.n_lv; ++r) if (A.lv[r].lev == lev) return r;
+    return 0;
+}
+
 // ---- plan-time tables ----------------------------------------------------------------------------------------------------
 // Rsh[ch][cidx(n,m)] = R_n^m(s_ch), s_ch = ((cx,cy,cz) - 1/2) / 2 for child ch = 4 cx + 2 cy + cz: the shift from the
 // parent's centre to the child's, in units of the parent's box side (M2M) -- and the same vector for L2L.
 // Stab[off][cidx(N,mu)] = S_N^mu(d), N <= 2p, for the offsets d = (dx,dy,dz) in [-5,5]^3 (off = dense index); entries
 // with |d|_inf <= kWs are never read (left zero).  nm[c] = (n << 8) | m.
-__global__ void tables_kernel(int p, double2* __restrict__ Rsh, double2* __restrict__ Stab, int* __restrict__ nm) {
+__global__ void tables_kernel(int p, double2* __restrict__ Rsh, double2* __restrict__ Stab, int* __restrict__ nm,
+                              int* __restrict__ pm, int* __restrict__ sfmap) {
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
     const int NC = nc(p), NS = nc(2 * p);
+    if (t < (2 * p + 1) * (2 * p + 1)) {   // expanded S table entry t = fidx(N, mu)
+        int N = 0;
+        while ((N + 1) * (N + 1) <= t) ++N;
+        const int mu = t - N * N - N;
+        sfmap[t] = (cidx(N, mu < 0 ? -mu : mu) << 2) | (mu < 0 ? ((mu & 1) ? 2 : 1) : 0);
+    }
+    if (t == 0) {   // output pairs (k, l0), l0 even
+        int c = 0;
+        for (int k = 0; k <= p; ++k)
+            for (int l0 = 0; l0 <= k; l0 += 2) pm[c++] = (k << 8) | l0;
+    }
     if (t < NC) {
         int n = 0;
         while (cidx(n + 1, 0) <= t) ++n;
@@ -338,29 +411,36 @@ __global__ void __launch_bounds__(256) m2m_kernel(const Geom G, int lev, const d
 // L[lev][box] = sum_s Lpart[s][box] (+ the parent's local expansion shifted to this box, lev > 0)
 // dynamic shared memory: Lp [NC], Rs [NC] double2
 __global__ void __launch_bounds__(256) l2l_kernel(const Geom G, int lev, const double2* __restrict__ Rsh, const int* __restrict__ nm,
-                                                  const double2* __restrict__ Lpart, int n_split, double2* __restrict__ L) {
+                                                  const double2* __restrict__ Lpart, const M2LArgs A, int Gm2l,
+                                                  double2* __restrict__ L) {
     extern __shared__ __align__(16) double2 sm2[];
     const int p = G.p, NC = nc(p);
     double2* Lp = sm2;
     double2* Rs = sm2 + NC;
     const int box = blockIdx.x;
     const long long nb = boxes_at(G, lev);
+    long long parent = box;   // level 0: the box is its own group
     if (lev > 0) {
         const int ny = grid_n(G, lev, 1), nz = grid_n(G, lev, 2);
         const int iz = box % nz, iy = (box / nz) % ny, ix = box / (nz * ny);
         const int py = grid_n(G, lev - 1, 1), pz = grid_n(G, lev - 1, 2);
-        const long long parent = ((long long)((ix >> 1) * py + (iy >> 1))) * pz + (iz >> 1);
+        parent = ((long long)((ix >> 1) * py + (iy >> 1))) * pz + (iz >> 1);
         const int ch = ((ix & 1) << 2) | ((iy & 1) << 1) | (iz & 1);
         const double2* Lpar = L + (level_offset(G, lev - 1) + parent) * NC;
         for (int t = threadIdx.x; t < NC; t += 256) { Lp[t] = Lpar[t]; Rs[t] = Rsh[ch * NC + t]; }
     }
     __syncthreads();
+    // the M2L partial rows of this box's group: the CTAs of m2l_kernel that worked on it, in CTA order
+    const M2LLevel lvr = A.lv[m2l_level_record(A, lev)];
+    const long long grp = lvr.first_group + parent;
+    const int n_rows = cta_of_unit((grp + 1) * A.W - 1, A.units, Gm2l) - cta_of_unit(grp * A.W, A.units, Gm2l) + 1;
+    const double2* Lrows = Lpart + lvr.part_off;
     double2* out = L + (level_offset(G, lev) + box) * NC;
     for (int c = threadIdx.x; c < NC; c += 256) {
         const int n = nm[c] >> 8, m = nm[c] & 255;
         double2 acc = make_double2(0.0, 0.0);
-        for (int s = 0; s < n_split; ++s) {
-            const double2 v = Lpart[((long long)s * nb + box) * NC + c];
+        for (int s = 0; s < n_rows; ++s) {
+            const double2 v = Lrows[((long long)s * nb + box) * NC + c];
             acc.x += v.x; acc.y += v.y;
         }
         if (lev > 0) {
@@ -381,294 +461,385 @@ __global__ void __launch_bounds__(256) l2l_kernel(const Geom G, int lev, const d
 }
 
 // ---- M2L: the translation that dominates the far field -----------------------------------------------------------------
-// One CTA = (level, sibling group, split): the <= 8 children of one parent box (level 0: a single box) and a
-// contiguous, weight-balanced share of the offset list.  For an offset d all siblings share S(d) (staged once in shared
+// Unit of work = (sibling group, offset): the <= 8 children of one parent box (level 0: a single box) and one offset;
+// a CTA walks a contiguous, weight-balanced range of them.  For an offset d all siblings share S(d) (staged once in shared
 // memory, expanded to -N <= mu <= N) and each valid sibling has its own source box t + d (its conj M, expanded to
 // -n <= m <= n with the image reflection and the cell weight applied, staged too).  Thread (k, l) keeps the 8 local
 // coefficients L_k^l of the siblings in registers: per (n, m) one 128-bit read of S and one broadcast read per sibling
-// feed 4 DFMA per sibling.  The split's partial sums go to Lpart[split][box]; l2l_kernel adds the splits in order.
-struct M2LLevel { int lev, n_groups, n_split, first_cta; long long part_off; };
-struct M2LArgs {
-    M2LLevel lv[kMaxLevels];
-    int n_lv;
-    const int* off_list;      // [n_off] dense offset indices (g - t), |d|_inf > kWs, processing order
-    const int* off_wprefix;   // [n_off + 1] prefix sums of the offset weights (how many of 8 siblings have it)
-    int n_off;
-};
-
+// feed 4 DFMA per sibling.  The CTA's partial sums go to Lpart[row][box]; l2l_kernel adds the rows in CTA order.
+// Thread = two neighbouring outputs (k, l0) and (k, l0 + 1), l0 even: S_{n+k}^{m+l0+1} of one step is S_{n+k}^{(m+1)+l0}
+// of the next, so a sliding window needs ONE new S value per step for both outputs, and every broadcast read of a
+// sibling's moment feeds 8 DFMA.  Per step and 8 siblings: 1 + 8 shared-memory reads, 64 DFMA.
 template <int NV>
 __device__ __forceinline__ void m2l_inner(const double2* __restrict__ Sfull, const double2* __restrict__ Mf, int mstride,
-                                          int p, int k, int l, double2 (&tmp)[NV]) {
+                                          int p, int k, int l0, double2 (&a0)[NV], double2 (&a1)[NV]) {
     for (int n = 0; n <= p; ++n) {
-        const double2* Srow = Sfull + fidx(n + k, l);
+        const double2* Srow = Sfull + fidx(n + k, l0);
         const double2* Mrow = Mf + fidx(n, 0);
+        double2 s0 = Srow[-n];
 #pragma unroll 2
         for (int m = -n; m <= n; ++m) {
-            const double2 s = Srow[m];
+            const double2 s1 = Srow[m + 1];   // (for the half pair l0 = k this runs one element past the row: unused)
 #pragma unroll
-            for (int i = 0; i < NV; ++i) cfma(tmp[i], Mrow[i * mstride + m], s);
+            for (int i = 0; i < NV; ++i) {
+                const double2 mv = Mrow[i * mstride + m];
+                cfma(a0[i], mv, s0);
+                cfma(a1[i], mv, s1);
+            }
+            s0 = s1;
         }
     }
 }
 
+constexpr int kM2LThreads = 128;
+__host__ __device__ inline int m2l_pairs(int p) {   // sum_k ceil((k+1)/2)
+    int s = 0;
+    for (int k = 0; k <= p; ++k) s += (k + 2) / 2;
+    return s;
+}
 __host__ __device__ inline int m2l_smem_bytes(int p) {
-    return (int)sizeof(double2) * ((2 * p + 1) * (2 * p + 1) + 8 * (p + 1) * (p + 1));
+    return (int)sizeof(double2) * ((2 * p + 1) * (2 * p + 1) + 1 + 8 * (p + 1) * (p + 1));
 }
 
-__global__ void __launch_bounds__(256) m2l_kernel(const Geom G, const M2LArgs A, const double2* __restrict__ M,
-                                                  const double2* __restrict__ Stab, const int* __restrict__ nm,
-                                                  double2* __restrict__ Lpart) {
-    extern __shared__ __align__(16) double2 sm2[];
-    __shared__ ImageBox sib[8];
-    __shared__ int slot_sib[8];
-    __shared__ int s_nv, s_lo, s_hi;
-    const int p = G.p, NC = nc(p), NS = nc(2 * p), NF = (p + 1) * (p + 1), NSF = (2 * p + 1) * (2 * p + 1);
-    double2* Sfull = sm2;
-    double2* Mfull = sm2 + NSF;
-    const int tid = threadIdx.x;
-    int r = 0;
-    while (r + 1 < A.n_lv && (int)blockIdx.x >= A.lv[r + 1].first_cta) ++r;
-    const M2LLevel lv = A.lv[r];
-    const int local = blockIdx.x - lv.first_cta, group = local / lv.n_split, split = local - group * lv.n_split;
-    const int lev = lv.lev;
-    const int nsib = lev == 0 ? 1 : 8;
-    int P[3];   // parent coordinates (level 0: the box itself)
-    {
-        const int gl = lev == 0 ? 0 : lev - 1;
-        const int ny = grid_n(G, gl, 1), nz = grid_n(G, gl, 2);
-        P[2] = group % nz; P[1] = (group / nz) % ny; P[0] = group / (nz * ny);
+// pm[t] = (k << 8) | l0 of output pair t; sfmap[t] = (cidx(N, |mu|) << 2) | op for the expanded S table entry t =
+// fidx(N, mu): op 0 as stored, 1 conj (mu < 0 even), 2 -conj (mu < 0 odd)
+template <int NV>
+__device__ __forceinline__ void m2l_add(double2 (&acc)[8], const double2 (&tmp)[NV], const int* slot_sib, int done) {
+#pragma unroll
+    for (int i = 0; i < NV; ++i) {
+        const int sid = slot_sib[done + i];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) if (j == sid) { acc[j].x += tmp[i].x; acc[j].y += tmp[i].y; }
     }
-    if (tid == 0) {   // this split's share of the offsets, by weight
-        const int W = A.off_wprefix[A.n_off];
-        const long long w_lo = (long long)W * split / lv.n_split, w_hi = (long long)W * (split + 1) / lv.n_split;
-        int lo = 0, hi = A.n_off;
-        while (lo < hi) { const int mid = (lo + hi) >> 1; if (A.off_wprefix[mid] < w_lo) lo = mid + 1; else hi = mid; }
-        s_lo = lo;
-        lo = 0; hi = A.n_off;
-        while (lo < hi) { const int mid = (lo + hi) >> 1; if (A.off_wprefix[mid] < w_hi) lo = mid + 1; else hi = mid; }
-        s_hi = lo;
-    }
-    __syncthreads();
-    const int o_lo = s_lo, o_hi = s_hi;
-    const long long nb = boxes_at(G, lev);
-    const double2* Mlev = M + level_offset(G, lev) * NC;
-    const int ny = grid_n(G, lev, 1), nz = grid_n(G, lev, 2);
+}
 
-    for (int c0 = 0; c0 < NC; c0 += 256) {
-        const int c = c0 + tid;
-        const bool have = c < NC;
-        const int k = have ? (nm[c] >> 8) : 0, l = have ? (nm[c] & 255) : 0;
-        double2 acc[8];
+__global__ void __launch_bounds__(kM2LThreads) m2l_kernel(const Geom G, const M2LArgs A, const double2* __restrict__ M,
+                                                          const double2* __restrict__ Stab, const int* __restrict__ nm,
+                                                          const int* __restrict__ pm, const int* __restrict__ sfmap,
+                                                          double2* __restrict__ Lpart) {
+    extern __shared__ __align__(16) double2 sm2[];
+    __shared__ int sib_box[8], sib_flip[8], slot_sib[8];
+    __shared__ double sib_w[8];
+    __shared__ int s_nv, s_lo, s_hi;
+    const int p = G.p, NC = nc(p), NS = nc(2 * p), NF = (p + 1) * (p + 1), NSF = (2 * p + 1) * (2 * p + 1), NP = m2l_pairs(p);
+    double2* Sfull = sm2;
+    double2* Mfull = sm2 + NSF + 1;
+    const int tid = threadIdx.x;
+    const int Gc = gridDim.x, kc = blockIdx.x;
+    const long long u0 = unit_start(kc, A.units, Gc), u1 = unit_start(kc + 1, A.units, Gc);
+    if (u1 <= u0) return;
+    if (tid == 0) Sfull[NSF] = make_double2(0.0, 0.0);
+    for (long long grp = u0 / A.W; grp <= (u1 - 1) / A.W; ++grp) {
+        int r = 0;
+        while (r + 1 < A.n_lv && grp >= A.lv[r + 1].first_group) ++r;
+        const M2LLevel lv = A.lv[r];
+        const int group = (int)(grp - lv.first_group);
+        const int row = kc - cta_of_unit(grp * A.W, A.units, Gc);
+        const int lev = lv.lev;
+        const int nsib = lev == 0 ? 1 : 8;
+        int P[3];   // parent coordinates (level 0: the box itself)
+        {
+            const int gl = lev == 0 ? 0 : lev - 1;
+            const int gy = grid_n(G, gl, 1), gz = grid_n(G, gl, 2);
+            P[2] = group % gz; P[1] = (group / gz) % gy; P[0] = group / (gz * gy);
+        }
+        __syncthreads();
+        if (tid == 0) {   // this CTA's share of the group's offsets, by weight: offsets whose prefix start lies in [w_lo, w_hi)
+            const long long w_lo = max(u0, grp * A.W) - grp * A.W, w_hi = min(u1, (grp + 1) * A.W) - grp * A.W;
+            int lo = 0, hi = A.n_off;
+            while (lo < hi) { const int mid = (lo + hi) >> 1; if (A.off_wprefix[mid] < w_lo) lo = mid + 1; else hi = mid; }
+            s_lo = lo;
+            lo = 0; hi = A.n_off;
+            while (lo < hi) { const int mid = (lo + hi) >> 1; if (A.off_wprefix[mid] < w_hi) lo = mid + 1; else hi = mid; }
+            s_hi = lo;
+        }
+        __syncthreads();
+        const int o_lo = s_lo, o_hi = s_hi;
+        const long long nb = boxes_at(G, lev);
+        const double2* Mlev = M + level_offset(G, lev) * NC;
+        const int ny = grid_n(G, lev, 1), nz = grid_n(G, lev, 2);
+
+        for (int c0 = 0; c0 < NP; c0 += kM2LThreads) {
+            const int c = c0 + tid;
+            const bool have = c < NP;
+            const int k = have ? (pm[c] >> 8) : 0, l0 = have ? (pm[c] & 255) : 0;
+            double2 acc0[8], acc1[8];
 #pragma unroll
-        for (int i = 0; i < 8; ++i) acc[i] = make_double2(0.0, 0.0);
-        for (int oi = o_lo; oi < o_hi; ++oi) {
-            const int off = A.off_list[oi];
-            const int dx = off / (kOffW * kOffW) - kOffR, dy = (off / kOffW) % kOffW - kOffR, dz = off % kOffW - kOffR;
-            __syncthreads();   // the previous offset's reads of Sfull / Mfull / sib are done
-            if (tid < 32) {
-                bool ok = false;
-                ImageBox ib;
-                if (tid < nsib) {
-                    const int t[3] = {lev == 0 ? P[0] : 2 * P[0] + ((tid >> 2) & 1), lev == 0 ? P[1] : 2 * P[1] + ((tid >> 1) & 1),
-                                      lev == 0 ? P[2] : 2 * P[2] + (tid & 1)};
-                    const int g[3] = {t[0] + dx, t[1] + dy, t[2] + dz};
-                    ok = true;
-                    if (lev > 0)   // the source's parent must be within kWs of the target's parent
-                        for (int a = 0; a < 3; ++a) ok = ok && g[a] >= 2 * (P[a] - kWs) && g[a] <= 2 * (P[a] + kWs) + 1;
-                    ok = ok && image_box(G, lev, g[0], g[1], g[2], ib);
+            for (int i = 0; i < 8; ++i) { acc0[i] = make_double2(0.0, 0.0); acc1[i] = make_double2(0.0, 0.0); }
+            for (int oi = o_lo; oi < o_hi; ++oi) {
+                const int off = A.off_list[oi];
+                const int dx = off / (kOffW * kOffW) - kOffR, dy = (off / kOffW) % kOffW - kOffR, dz = off % kOffW - kOffR;
+                __syncthreads();   // the previous offset's reads of Sfull / Mfull / sib_* are done
+                if (tid < 32) {
+                    bool ok = false;
+                    ImageBox ib;
+                    if (tid < nsib) {
+                        const int t[3] = {lev == 0 ? P[0] : 2 * P[0] + ((tid >> 2) & 1), lev == 0 ? P[1] : 2 * P[1] + ((tid >> 1) & 1),
+                                          lev == 0 ? P[2] : 2 * P[2] + (tid & 1)};
+                        const int g[3] = {t[0] + dx, t[1] + dy, t[2] + dz};
+                        ok = true;
+                        if (lev > 0)   // the source's parent must be within kWs of the target's parent
+                            for (int a = 0; a < 3; ++a) ok = ok && g[a] >= 2 * (P[a] - kWs) && g[a] <= 2 * (P[a] + kWs) + 1;
+                        ok = ok && image_box(G, lev, g[0], g[1], g[2], ib);
+                    }
+                    const unsigned mask = __ballot_sync(0xffffffffu, ok);
+                    if (ok) {
+                        const int slot = __popc(mask & ((1u << tid) - 1u));
+                        sib_box[slot] = ib.box; sib_flip[slot] = ib.fx | (ib.fy << 1) | (ib.fz << 2); sib_w[slot] = ib.w;
+                        slot_sib[slot] = tid;
+                    }
+                    if (tid == 0) s_nv = __popc(mask);
                 }
-                const unsigned mask = __ballot_sync(0xffffffffu, ok);
-                if (ok) {
-                    const int slot = __popc(mask & ((1u << tid) - 1u));
-                    sib[slot] = ib;
-                    slot_sib[slot] = tid;
+                __syncthreads();
+                const int nv = s_nv;
+                if (nv == 0) continue;
+                // S(t - g) = S(-d), expanded to negative orders
+                const double2* S = Stab + (long long)(((kOffR - dx) * kOffW + (kOffR - dy)) * kOffW + (kOffR - dz)) * NS;
+                for (int t = tid; t < NSF; t += kM2LThreads) {
+                    const int e = sfmap[t];
+                    double2 v = S[e >> 2];
+                    if (e & 1) v.y = -v.y;
+                    if (e & 2) { v.x = -v.x; }
+                    Sfull[t] = v;
                 }
-                if (tid == 0) s_nv = __popc(mask);
-            }
-            __syncthreads();
-            const int nv = s_nv;
-            if (nv == 0) continue;
-            // S(t - g) = S(-d), expanded to negative orders
-            const double2* S = Stab + (long long)(((kOffR - dx) * kOffW + (kOffR - dy)) * kOffW + (kOffR - dz)) * NS;
-            for (int t = tid; t < NSF; t += 256) {
-                int N = (int)sqrt((double)t);
-                while (N * N > t) --N;
-                while ((N + 1) * (N + 1) <= t) ++N;
-                const int mu = t - N * N - N;
-                double2 v = S[cidx(N, mu < 0 ? -mu : mu)];
-                if (mu < 0) v = (mu & 1) ? make_double2(-v.x, v.y) : make_double2(v.x, -v.y);
-                Sfull[t] = v;
-            }
-            // conj of the (reflected, weighted) source moments, expanded to negative orders
-            for (int t = tid; t < nv * NC; t += 256) {
-                const int s = t / NC, cc = t - s * NC;
-                const ImageBox ib = sib[s];
-                const int n = nm[cc] >> 8, m = nm[cc] & 255;
-                double2 v = Mlev[(long long)ib.box * NC + cc];
-                if (ib.fx) v = (m & 1) ? make_double2(-v.x, v.y) : make_double2(v.x, -v.y);   // (-1)^m conj
-                if (ib.fy) v.y = -v.y;                                                         // conj
-                if (ib.fz && ((n + m) & 1)) { v.x = -v.x; v.y = -v.y; }
-                v.x *= ib.w; v.y *= ib.w;
-                double2* dst = Mfull + s * NF;
-                dst[fidx(n, m)] = make_double2(v.x, -v.y);
-                if (m > 0) dst[fidx(n, -m)] = (m & 1) ? make_double2(-v.x, -v.y) : v;
-            }
-            __syncthreads();
-            int done = 0;
-            while (done < nv) {
-                const int left = nv - done;
-                const double2* Mf = Mfull + done * NF;
-                if (left >= 8) {
-                    double2 tmp[8];
+                // conj of the (reflected, weighted) source moments, expanded to negative orders
+                for (int t = tid; t < nv * NC; t += kM2LThreads) {
+                    const int sl = t / NC, cc = t - sl * NC;
+                    const int fl = sib_flip[sl];
+                    const double w = sib_w[sl];
+                    const int n = nm[cc] >> 8, m = nm[cc] & 255;
+                    double2 v = Mlev[(long long)sib_box[sl] * NC + cc];
+                    if (fl & 1) v = (m & 1) ? make_double2(-v.x, v.y) : make_double2(v.x, -v.y);   // x: (-1)^m conj
+                    if (fl & 2) v.y = -v.y;                                                         // y: conj
+                    if ((fl & 4) && ((n + m) & 1)) { v.x = -v.x; v.y = -v.y; }                      // z: (-1)^(n+m)
+                    v.x *= w; v.y *= w;
+                    double2* dst = Mfull + sl * NF;
+                    dst[fidx(n, m)] = make_double2(v.x, -v.y);
+                    if (m > 0) dst[fidx(n, -m)] = (m & 1) ? make_double2(-v.x, -v.y) : v;
+                }
+                __syncthreads();
+                int done = 0;
+                while (done < nv) {
+                    const int left = nv - done;
+                    const double2* Mf = Mfull + done * NF;
+                    if (left >= 8) {
+                        m2l_inner<8>(Sfull, Mf, NF, p, k, l0, acc0, acc1);   // all eight siblings: slot i is sibling i
+                        done += 8;
+                    } else if (left >= 4) {
+                        double2 t0[4], t1[4];
 #pragma unroll
-                    for (int i = 0; i < 8; ++i) tmp[i] = make_double2(0.0, 0.0);
-                    m2l_inner<8>(Sfull, Mf, NF, p, k, l, tmp);
+                        for (int i = 0; i < 4; ++i) { t0[i] = make_double2(0.0, 0.0); t1[i] = make_double2(0.0, 0.0); }
+                        m2l_inner<4>(Sfull, Mf, NF, p, k, l0, t0, t1);
+                        m2l_add<4>(acc0, t0, slot_sib, done); m2l_add<4>(acc1, t1, slot_sib, done);
+                        done += 4;
+                    } else if (left >= 2) {
+                        double2 t0[2], t1[2];
 #pragma unroll
-                    for (int i = 0; i < 8; ++i) {
-                        const int sid = slot_sib[done + i];
-#pragma unroll
-                        for (int j = 0; j < 8; ++j) if (j == sid) { acc[j].x += tmp[i].x; acc[j].y += tmp[i].y; }
+                        for (int i = 0; i < 2; ++i) { t0[i] = make_double2(0.0, 0.0); t1[i] = make_double2(0.0, 0.0); }
+                        m2l_inner<2>(Sfull, Mf, NF, p, k, l0, t0, t1);
+                        m2l_add<2>(acc0, t0, slot_sib, done); m2l_add<2>(acc1, t1, slot_sib, done);
+                        done += 2;
+                    } else {
+                        double2 t0[1], t1[1];
+                        t0[0] = make_double2(0.0, 0.0); t1[0] = make_double2(0.0, 0.0);
+                        m2l_inner<1>(Sfull, Mf, NF, p, k, l0, t0, t1);
+                        m2l_add<1>(acc0, t0, slot_sib, done); m2l_add<1>(acc1, t1, slot_sib, done);
+                        done += 1;
                     }
-                    done += 8;
-                } else if (left >= 4) {
-                    double2 tmp[4];
+                }
+            }
+            if (have) {
+                const double sg = (k & 1) ? -1.0 : 1.0;
+                const int cc = cidx(k, l0);
 #pragma unroll
-                    for (int i = 0; i < 4; ++i) tmp[i] = make_double2(0.0, 0.0);
-                    m2l_inner<4>(Sfull, Mf, NF, p, k, l, tmp);
-#pragma unroll
-                    for (int i = 0; i < 4; ++i) {
-                        const int sid = slot_sib[done + i];
-#pragma unroll
-                        for (int j = 0; j < 8; ++j) if (j == sid) { acc[j].x += tmp[i].x; acc[j].y += tmp[i].y; }
+                for (int sI = 0; sI < 8; ++sI) {
+                    if (sI < nsib) {
+                        const int tx = lev == 0 ? P[0] : 2 * P[0] + ((sI >> 2) & 1), ty = lev == 0 ? P[1] : 2 * P[1] + ((sI >> 1) & 1),
+                                  tz = lev == 0 ? P[2] : 2 * P[2] + (sI & 1);
+                        const long long box = ((long long)tx * ny + ty) * nz + tz;
+                        double2* o = Lpart + lv.part_off + ((long long)row * nb + box) * NC + cc;
+                        o[0] = make_double2(sg * acc0[sI].x, sg * acc0[sI].y);
+                        if (l0 + 1 <= k) o[1] = make_double2(sg * acc1[sI].x, sg * acc1[sI].y);
                     }
-                    done += 4;
-                } else if (left >= 2) {
-                    double2 tmp[2];
-                    tmp[0] = make_double2(0.0, 0.0); tmp[1] = make_double2(0.0, 0.0);
-                    m2l_inner<2>(Sfull, Mf, NF, p, k, l, tmp);
-#pragma unroll
-                    for (int i = 0; i < 2; ++i) {
-                        const int sid = slot_sib[done + i];
-#pragma unroll
-                        for (int j = 0; j < 8; ++j) if (j == sid) { acc[j].x += tmp[i].x; acc[j].y += tmp[i].y; }
-                    }
-                    done += 2;
-                } else {
-                    double2 tmp[1];
-                    tmp[0] = make_double2(0.0, 0.0);
-                    m2l_inner<1>(Sfull, Mf, NF, p, k, l, tmp);
-                    const int sid = slot_sib[done];
-#pragma unroll
-                    for (int j = 0; j < 8; ++j) if (j == sid) { acc[j].x += tmp[0].x; acc[j].y += tmp[0].y; }
-                    done += 1;
                 }
             }
         }
-        if (have) {
-            const double sg = (k & 1) ? -1.0 : 1.0;
-#pragma unroll
-            for (int s = 0; s < 8; ++s) {
-                if (s < nsib) {
-                    const int tx = lev == 0 ? P[0] : 2 * P[0] + ((s >> 2) & 1), ty = lev == 0 ? P[1] : 2 * P[1] + ((s >> 1) & 1),
-                              tz = lev == 0 ? P[2] : 2 * P[2] + (s & 1);
-                    const long long box = ((long long)tx * ny + ty) * nz + tz;
-                    Lpart[lv.part_off + ((long long)split * nb + box) * NC + c] = make_double2(sg * acc[s].x, sg * acc[s].y);
-                }
-            }
-        }
-    }
+    }   // groups of this CTA
 }
 
 // ---- leaves: L2P + P2P --------------------------------------------------------------------------------------------------
-// One CTA = 256 consecutive particles of the leaf-sorted array (one target per thread); the leaves it spans are worked
-// through one after the other (threads of other leaves idle).  For a leaf: its local expansion is evaluated at the
-// targets (L2P), then the 5^3 neighbour boxes -- images through the near cell table, never materialised -- are summed
-// directly (P2P) from 256-source tiles in shared memory with the pair arithmetic of near_sum_kernel: the target is
-// moved into the image's frame, sigma o (t - kL); only the bare self term (central cell, same particle) is masked.
+// One CTA of 64 threads per chunk of a leaf: up to 4 rows of 64 targets, i.e. a thread owns R <= 4 targets of ONE leaf
+// in registers (every smem read of a source feeds R pairs), and the number of rows follows the leaf population, so
+// the lanes are full whatever it is (534 targets = 9 rows = chunks of 4 + 4 + 1).  The leaf's
+// local expansion is evaluated at the targets (L2P), then the 5^3 neighbour boxes -- images through the near cell table,
+// never materialised -- are summed directly (P2P) from 256-source tiles in shared memory with the pair arithmetic of
+// near_sum_kernel: the target is moved into the image's frame, sigma o (t - kL); only the bare self term (central
+// cell, same particle) is masked.
 // dynamic shared memory: Ls [NC] double2, inv [(p+1) * kInvW] double
+constexpr int kLeafThreads = 64;
+constexpr int kLeafTile = 128;
+constexpr int kLeafR = 4;      // rows of kLeafThreads targets per chunk (targets per thread)
+
+template <int REFINE, int R>
+__device__ __forceinline__ void leaf_round(const Geom& G, const int ic[3], const double c[3], const Src4* __restrict__ srt,
+                                           const int* __restrict__ idx, const int* __restrict__ leaf_start, int t0, int t1,
+                                           Src4* tile, const double2* Ls, const double* inv, double* __restrict__ phi_out) {
+    const int p = G.p, lev = G.levels, tid = threadIdx.x;
+    const double ia = (double)(1 << lev) / G.a0;
+    const double scale = REFINE == 1 ? 0.5 : 1.0;
+    double total[R];
+    // L2P: (1/a) Re sum conj R_n^m L_n^m, m < 0 folded in (factor 2)
+#pragma unroll 1
+    for (int r = 0; r < R; ++r) {
+        const Src4 t = srt[min(t0 + r * kLeafThreads + tid, t1 - 1)];
+        const double x = (t.x - c[0]) * ia, y = (t.y - c[1]) * ia, z = (t.z - c[2]) * ia;
+        const double r2 = fma(z, z, fma(y, y, x * x));
+        double rr = 1.0, ri = 0.0, far = 0.0;
+        for (int m = 0; m <= p; ++m) {
+            if (m > 0) { const double f = 0.5 / (double)m, u = (rr * x - ri * y) * f; ri = (rr * y + ri * x) * f; rr = u; }
+            double p1r = rr, p1i = ri, p2r = 0.0, p2i = 0.0;
+            double2 lc = Ls[cidx(m, m)];
+            double s = fma(rr, lc.x, ri * lc.y);
+            for (int n = m + 1; n <= p; ++n) {
+                const double f = inv[n * kInvW + m], tz = (double)(2 * n - 1) * z;
+                const double cr = (tz * p1r - r2 * p2r) * f, ci = (tz * p1i - r2 * p2i) * f;
+                lc = Ls[cidx(n, m)];
+                s = fma(cr, lc.x, s); s = fma(ci, lc.y, s);
+                p2r = p1r; p2i = p1i; p1r = cr; p1i = ci;
+            }
+            far += m == 0 ? s : 2.0 * s;
+        }
+        // (dynamic index into a register array would spill: select)
+#pragma unroll
+        for (int k = 0; k < R; ++k) if (k == r) total[k] = far * ia;
+    }
+    Src4 me[R];
+    int pos[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        pos[r] = min(t0 + r * kLeafThreads + tid, t1 - 1);   // slots past the end repeat the last target and do not store
+        me[r] = srt[pos[r]];
+    }
+    for (int dx = -kWs; dx <= kWs; ++dx)
+        for (int dy = -kWs; dy <= kWs; ++dy)
+            for (int dz = -kWs; dz <= kWs; ++dz) {
+                ImageBox ib;
+                if (!image_box(G, lev, ic[0] + dx, ic[1] + dy, ic[2] + dz, ib)) continue;
+                const int s0 = leaf_start[ib.box], s1 = leaf_start[ib.box + 1];
+                if (s0 == s1) continue;
+                double tx[R], ty[R], tz[R], acc[R];
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    tx[r] = flip(me[r].x - ib.sx, ib.fx); ty[r] = flip(me[r].y - ib.sy, ib.fy); tz[r] = flip(me[r].z - ib.sz, ib.fz);
+                    acc[r] = 0.0;
+                }
+                const bool self_here = ib.central && dx == 0 && dy == 0 && dz == 0;
+                for (int base = s0; base < s1; base += kLeafTile) {
+                    __syncthreads();
+#pragma unroll
+                    for (int h = 0; h < kLeafTile / kLeafThreads; ++h) {
+                        const int j = base + h * kLeafThreads + tid;
+                        tile[h * kLeafThreads + tid] = j < s1 ? srt[j] : Src4{kFar, kFar, kFar, 0.0};
+                    }
+                    __syncthreads();
+                    const int cnt = min(kLeafTile, s1 - base);
+                    if (self_here) {
+#pragma unroll 1
+                        for (int j = 0; j < cnt; ++j) {
+                            const double2 xy = *reinterpret_cast<const double2*>(&tile[j].x);
+                            const double2 zq = *reinterpret_cast<const double2*>(&tile[j].z);
+#pragma unroll
+                            for (int r = 0; r < R; ++r) {
+                                const bool self = base + j == pos[r];
+                                pair<REFINE>(tx[r], ty[r], tz[r], self ? tx[r] + 1.0 : xy.x, self ? ty[r] : xy.y, self ? tz[r] : zq.x,
+                                             self ? 0.0 : zq.y, acc[r]);
+                            }
+                        }
+                    } else {
+#pragma unroll 2
+                        for (int j = 0; j < cnt; ++j) {
+                            const double2 xy = *reinterpret_cast<const double2*>(&tile[j].x);
+                            const double2 zq = *reinterpret_cast<const double2*>(&tile[j].z);
+#pragma unroll
+                            for (int r = 0; r < R; ++r) pair<REFINE>(tx[r], ty[r], tz[r], xy.x, xy.y, zq.x, zq.y, acc[r]);
+                        }
+                    }
+                }
+                const double w = ib.w * scale;
+#pragma unroll
+                for (int r = 0; r < R; ++r) total[r] = fma(w, acc[r], total[r]);
+            }
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const int t = t0 + r * kLeafThreads + tid;
+        if (t < t1) phi_out[idx[t]] = total[r];
+    }
+}
+
+// chunk_start[l] = number of chunks of the leaves before l (a chunk = up to kLeafR rows of kLeafThreads targets of one
+// leaf); chunk_start[n_leaves] = total.  Single block.
+__global__ void __launch_bounds__(1024) leaf_chunks_kernel(const int* __restrict__ leaf_start, int n_leaves, int* __restrict__ chunk_start) {
+    __shared__ int wsum[32];
+    __shared__ int carry;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (threadIdx.x == 0) carry = 0;
+    __syncthreads();
+    for (int base = 0; base < n_leaves; base += 1024) {
+        const int l = base + threadIdx.x;
+        const int n = l < n_leaves ? leaf_start[l + 1] - leaf_start[l] : 0;
+        const int v = (n + kLeafThreads * kLeafR - 1) / (kLeafThreads * kLeafR);
+        int x = v;
+        for (int o = 1; o < 32; o <<= 1) { const int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+        if (lane == 31) wsum[warp] = x;
+        __syncthreads();
+        if (warp == 0) {
+            int w = wsum[lane];
+            for (int o = 1; o < 32; o <<= 1) { const int y = __shfl_up_sync(0xffffffffu, w, o); if (lane >= o) w += y; }
+            wsum[lane] = w;
+        }
+        __syncthreads();
+        if (l < n_leaves) chunk_start[l] = carry + (warp > 0 ? wsum[warp - 1] : 0) + x - v;
+        __syncthreads();
+        if (threadIdx.x == 0) carry += wsum[31];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) chunk_start[n_leaves] = carry;
+}
+
+// grid: an upper bound of the number of chunks (N / (kLeafThreads * kLeafR) + n_leaves); surplus CTAs return
 template <int REFINE>
-__global__ void __launch_bounds__(256) leaf_kernel(const Geom G, const Src4* __restrict__ srt, const int* __restrict__ key,
-                                                   const int* __restrict__ idx, const int* __restrict__ leaf_start, long long N,
-                                                   const double2* __restrict__ L, double* __restrict__ phi_out) {
+__global__ void __launch_bounds__(kLeafThreads) leaf_kernel(const Geom G, const Src4* __restrict__ srt, const int* __restrict__ idx,
+                                                            const int* __restrict__ leaf_start, const int* __restrict__ chunk_start,
+                                                            int n_leaves, const double2* __restrict__ L, double* __restrict__ phi_out) {
     extern __shared__ __align__(16) double2 sm2[];
-    __shared__ __align__(16) Src4 tile[256];
+    __shared__ __align__(16) Src4 tile[kLeafTile];
     const int p = G.p, NC = nc(p), lev = G.levels;
     double2* Ls = sm2;
     double* inv = reinterpret_cast<double*>(sm2 + NC);
-    const int tid = threadIdx.x;
-    fill_inv_table(inv, p);
-    const long long pos = (long long)blockIdx.x * 256 + tid;
-    const bool valid = pos < N;
-    const Src4 me = valid ? srt[pos] : Src4{0.0, 0.0, 0.0, 0.0};
-    const int my_leaf = valid ? key[pos] : -1;
-    const int leaf_lo = key[(long long)blockIdx.x * 256];
-    const int leaf_hi = key[min(N - 1, (long long)blockIdx.x * 256 + 255)];
-    const double a = G.a0 / (double)(1 << lev), ia = 1.0 / a;
-    const double2* Llev = L + level_offset(G, lev) * NC;
-    const double scale = REFINE == 1 ? 0.5 : 1.0;
-    double total = 0.0;
-
-    for (int leaf = leaf_lo; leaf <= leaf_hi; ++leaf) {
-        if (leaf_start[leaf] == leaf_start[leaf + 1]) continue;
-        const bool active = my_leaf == leaf;
-        double c[3]; int ic[3];
-        box_centre(G, lev, leaf, c, ic);
-        __syncthreads();
-        for (int t = tid; t < NC; t += 256) Ls[t] = Llev[(long long)leaf * NC + t];
-        __syncthreads();
-        if (active) {   // L2P: (1/a) Re sum conj R_n^m L_n^m, m < 0 folded in (factor 2)
-            const double x = (me.x - c[0]) * ia, y = (me.y - c[1]) * ia, z = (me.z - c[2]) * ia;
-            const double r2 = fma(z, z, fma(y, y, x * x));
-            double rr = 1.0, ri = 0.0, far = 0.0;
-            for (int m = 0; m <= p; ++m) {
-                if (m > 0) { const double f = 0.5 / (double)m, u = (rr * x - ri * y) * f; ri = (rr * y + ri * x) * f; rr = u; }
-                double p1r = rr, p1i = ri, p2r = 0.0, p2i = 0.0;
-                double2 lc = Ls[cidx(m, m)];
-                double s = fma(rr, lc.x, ri * lc.y);
-                for (int n = m + 1; n <= p; ++n) {
-                    const double f = inv[n * kInvW + m], tz = (double)(2 * n - 1) * z;
-                    const double cr = (tz * p1r - r2 * p2r) * f, ci = (tz * p1i - r2 * p2i) * f;
-                    lc = Ls[cidx(n, m)];
-                    s = fma(cr, lc.x, s); s = fma(ci, lc.y, s);
-                    p2r = p1r; p2i = p1i; p1r = cr; p1i = ci;
-                }
-                far += m == 0 ? s : 2.0 * s;
-            }
-            total += far * ia;
-        }
-        for (int dx = -kWs; dx <= kWs; ++dx)
-            for (int dy = -kWs; dy <= kWs; ++dy)
-                for (int dz = -kWs; dz <= kWs; ++dz) {
-                    ImageBox ib;
-                    if (!image_box(G, lev, ic[0] + dx, ic[1] + dy, ic[2] + dz, ib)) continue;
-                    const int s0 = leaf_start[ib.box], s1 = leaf_start[ib.box + 1];
-                    if (s0 == s1) continue;
-                    const double tx = flip(me.x - ib.sx, ib.fx), ty = flip(me.y - ib.sy, ib.fy), tz = flip(me.z - ib.sz, ib.fz);
-                    const bool self_here = ib.central && dx == 0 && dy == 0 && dz == 0;
-                    double acc = 0.0;
-                    for (int base = s0; base < s1; base += 256) {
-                        __syncthreads();
-                        tile[tid] = base + tid < s1 ? srt[base + tid] : Src4{kFar, kFar, kFar, 0.0};
-                        __syncthreads();
-                        if (!active) continue;
-                        const int cnt = min(256, s1 - base);
-                        if (self_here) {
-                            const long long sj = pos - base;
-#pragma unroll 2
-                            for (int j = 0; j < cnt; ++j) {
-                                const bool self = j == sj;
-                                pair<REFINE>(tx, ty, tz, self ? tx + 1.0 : tile[j].x, self ? ty : tile[j].y, self ? tz : tile[j].z,
-                                             self ? 0.0 : tile[j].q, acc);
-                            }
-                        } else {
-#pragma unroll 4
-                            for (int j = 0; j < cnt; ++j) pair<REFINE>(tx, ty, tz, tile[j].x, tile[j].y, tile[j].z, tile[j].q, acc);
-                        }
-                    }
-                    total = fma(ib.w * scale, acc, total);
-                }
+    const int b = blockIdx.x;
+    if (b >= chunk_start[n_leaves]) return;
+    int lo = 0, hi = n_leaves - 1;   // the leaf with chunk_start[leaf] <= b < chunk_start[leaf + 1]
+    while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if (chunk_start[mid] <= b) lo = mid; else hi = mid - 1;
     }
-    if (valid) phi_out[idx[pos]] = total;
+    const int leaf = lo;
+    const int s1 = leaf_start[leaf + 1];
+    const int t0 = leaf_start[leaf] + (b - chunk_start[leaf]) * (kLeafThreads * kLeafR);
+    const int t1 = min(s1, t0 + kLeafThreads * kLeafR);
+    fill_inv_table(inv, p);
+    const double2* Lleaf = L + (level_offset(G, lev) + leaf) * NC;
+    for (int t = threadIdx.x; t < NC; t += kLeafThreads) Ls[t] = Lleaf[t];
+    double c[3]; int ic[3];
+    box_centre(G, lev, leaf, c, ic);
+    __syncthreads();
+    const int R = (t1 - t0 + kLeafThreads - 1) / kLeafThreads;
+    switch (R) {
+        case 1: leaf_round<REFINE, 1>(G, ic, c, srt, idx, leaf_start, t0, t1, tile, Ls, inv, phi_out); break;
+        case 2: leaf_round<REFINE, 2>(G, ic, c, srt, idx, leaf_start, t0, t1, tile, Ls, inv, phi_out); break;
+        case 3: leaf_round<REFINE, 3>(G, ic, c, srt, idx, leaf_start, t0, t1, tile, Ls, inv, phi_out); break;
+        default: leaf_round<REFINE, 4>(G, ic, c, srt, idx, leaf_start, t0, t1, tile, Ls, inv, phi_out); break;
+    }
 }
 
 }  // namespace fmm
