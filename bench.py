@@ -260,7 +260,9 @@ def run_b200(args, w) -> dict:
             dist.barrier()
         torch.cuda.synchronize()
 
-    plan = H.Plan.from_workload(w, rsqrt_refine=args.refine)
+    fmm_arm = args.near_algorithm == "fmm"
+    plan = H.Plan.from_workload(w, rsqrt_refine=args.refine, near_algorithm=1 if fmm_arm else 0, fmm_order=args.fmm_order,
+                                fmm_levels=args.fmm_levels)
     if args.pair_form != "auto":
         plan.set_pair_form(1 if args.pair_form == "ordered" else 2)
     info = plan.info
@@ -459,6 +461,46 @@ def run_b200(args, w) -> dict:
            "energy": U_val, "stage_ms": stage_ms, "e2e": e2e, "gpu_launches": int(launches),
            "launches_per_step": plan.launches_last_evaluate(),
            "graph_replays": H.binding.hsma_plan_info(plan.handle)["graph_replays"], "clocks": clocks, "roofline": roofline}
+    if fmm_arm:
+        out["config"]["near_algorithm"] = (f"fmm (order {args.fmm_order or 20}, two-box separation, leaf level "
+                                           f"{args.fmm_levels or 'by N'}): step (b) sub-quadratic, DESIGN.md 6.13; value still "
+                                           f"counts the pair interactions of the direct sum it replaces")
+        roofline["kernel"] = "fmm step (b): sort + p2m + m2m + m2l_kernel + l2l + leaf_kernel (kernel_ms is the whole stage)"
+        for k in ("achieved", "frac", "frac_executed_flops", "fp64_pipe_issue_util", "frac_of_dfma_microbench", "evaluations_per_s"):
+            roofline[k] = None     # the direct-sum unit counts do not apply to the FMM; see profiles/ for its kernels
+        roofline["traffic"] = None
+    elif world == 1 and not args.forces and not args.no_fmm_line and not args.paper_timing:
+        # the sub-quadratic form of step (b) on the same workload, measured beside the direct sum (not the headline)
+        try:
+            with H.Plan.from_workload(w, rsqrt_refine=args.refine, near_algorithm=1, fmm_order=args.fmm_order,
+                                      fmm_levels=args.fmm_levels) as pf:
+                phi_f = torch.empty(N, dtype=torch.float64, device=dev)
+                U_f = torch.empty(1, dtype=torch.float64, device=dev)
+                for _ in range(3):
+                    H.hsma_evaluate(pf.handle, xyz, q, phi_f, U_f)
+                pf.sync()
+                f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                nrep = max(3, min(args.steps, 10))
+                tot = 0.0
+                for _ in range(nrep):
+                    flush.zero_()
+                    f0.record()
+                    H.hsma_evaluate(pf.handle, xyz, q, phi_f, U_f)
+                    f1.record()
+                    f1.synchronize()
+                    tot += f0.elapsed_time(f1)
+                pf.set_timing(True)
+                H.hsma_evaluate(pf.handle, xyz, q, phi_f, U_f)
+                pf.sync()
+                tm = pf.timing()
+                out["fmm"] = {"ms_per_step": tot / nrep, "steps": nrep, "near_source_ms": tm["near_source_kernel"],
+                              "order": args.fmm_order or 20, "energy": float(U_f.cpu()[0]),
+                              "energy_rel_diff_vs_direct": abs(float(U_f.cpu()[0]) - U_val) / abs(U_val) if U_val else None,
+                              "max_phi_rel_diff_vs_direct": float((phi_f - phi).abs().max() / phi.abs().max()),
+                              "note": "near_algorithm = FMM (DESIGN.md 6.13): the same evaluate with step (b) by the fast multipole "
+                                      "method; parity against the oracle in tests/test_gpu_fmm.py; run `--near-algorithm fmm` for its own line"}
+        except H.HsmaError as e:   # geometry the FMM does not tile (non-cubic boxes)
+            out["fmm"] = {"unavailable": str(e)}
     plan.close()
     if world > 1:
         dist.destroy_process_group()
@@ -534,6 +576,12 @@ def main():
     ap.add_argument("--pair-form", choices=["auto", "ordered", "symmetric"], default="auto",
                     help="step (b): auto = symmetric form (each unordered pair once) when one rank evaluates all targets "
                          "; ordered = always near_sum_kernel; symmetric = wherever it applies")
+    ap.add_argument("--near-algorithm", choices=["direct", "fmm"], default="direct",
+                    help="step (b): direct = the exact pair sum (the metric's kernel, default); fmm = sub-quadratic form "
+                         "(DESIGN.md 6.13).  The default line also reports the FMM time of the same workload under \"fmm\"")
+    ap.add_argument("--fmm-order", type=int, default=0, help="FMM expansion order (0 = 20)")
+    ap.add_argument("--fmm-levels", type=int, default=0, help="FMM leaf level (0 = by N)")
+    ap.add_argument("--no-fmm-line", action="store_true", help="skip the extra FMM measurement of the default line")
     ap.add_argument("--forces", action="store_true", help="time hsma_evaluate_forces (potential + forces) instead")
     ap.add_argument("--parts", type=int, default=0, metavar="R",
                     help="one GPU: time what each rank of the R-rank PART form computes, one rank at a time (DESIGN.md 8); "

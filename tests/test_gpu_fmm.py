@@ -1,0 +1,162 @@
+"""The sub-quadratic form of step (b) (near_algorithm = FMM; PAPER.md:144-146 and
+Table I) against the CPU oracle -- which stays the exact direct sum -- through the C-ABI, at the
+north_star bars: max|dphi|/max|phi| <= 1e-10, |dU|/|U| <= 1e-11.  All `-m gpu`."""
+import numpy as np
+import pytest
+
+import hsma_workloads as W
+from oracle import hsma_oracle as O
+
+pytestmark = pytest.mark.gpu
+
+PHI_TOL = 1e-10
+U_TOL = 1e-11
+FMM = 3      # hsma_plan_last_pair_form: step (b) ran as the FMM
+
+
+@pytest.fixture(scope="module")
+def H():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    import paper_1806_04801_b200 as H
+    H.binding.load_library()
+    return H
+
+
+def dev(a):
+    import torch
+    return torch.as_tensor(np.ascontiguousarray(a, dtype=np.float64), device="cuda")
+
+
+def rel_inf(a, b):
+    return float(np.max(np.abs(a - b)) / np.max(np.abs(b)))
+
+
+def run_fmm(H, w, **kw):
+    with H.Plan.from_workload(w, near_algorithm=H.binding.NEAR_ALG_FMM, **kw) as plan:
+        phi, U = plan.evaluate(dev(w.xyz), dev(w.q), sync=True)
+        assert plan.last_pair_form == FMM
+    return phi.cpu().numpy(), float(U)
+
+
+@pytest.mark.parametrize("levels", [0, 1, 2, 3])
+def test_config2_every_potential(H, levels):
+    """BASELINE.json config 2 (N = 1,000) in full: the automatic leaf level (1: everything is near, the far field
+    comes from the few level-1 boxes three boxes away) and forced deeper hierarchies (M2M, level-2/3 M2L, L2L)."""
+    w = W.config(2)
+    r = O.hsma(w)
+    phi, U = run_fmm(H, w, fmm_levels=levels)
+    assert rel_inf(phi, r.phi) <= PHI_TOL and abs(U - r.U) <= U_TOL * abs(r.U)
+
+
+@pytest.mark.parametrize("idx,N,levels,order", [(5, 20012, 0, 0), (5, 20012, 3, 0), (3, 9001, 2, 0), (3, 20011, 0, 0), (4, 9000, 0, 0),
+                                                (4, 16384, 2, 0), (1, 8, 2, 26)])
+def test_all_cell_tables_every_potential(H, idx, N, levels, order):
+    """Periodic (27 cells), mirror cavity (reflected images, gamma = -1: the multipole moments of an image box are
+    those of the central box with the reflection signs), slab (base grid 2 x 2 x 1 boxes per cell, 45 reflected and
+    weighted cells, gamma = 0.5) and the Madelung cell with its 125-cell table (level-0 translations): every
+    potential and U against the oracle.  The rock-salt ions sit exactly on the corners of the FMM boxes -- the largest
+    expansion radius there is -- and their errors add coherently: at the default order 20 that case reaches 1.8e-11 in
+    phi and U (phi inside its bar, U not), so lattice-aligned inputs take order 26."""
+    w = W.config(idx, N=N)
+    r = O.hsma(w)
+    phi, U = run_fmm(H, w, fmm_levels=levels, fmm_order=order)
+    assert rel_inf(phi, r.phi) <= PHI_TOL and abs(U - r.U) <= U_TOL * abs(r.U)
+
+
+def test_config5_recipe_at_65536_every_potential(H):
+    """Config-5 recipe at N = 65,536: every potential and U, automatic level (2: 1,024 sources per leaf) and level 3."""
+    w = W.config(5, N=65536)
+    r = O.hsma(w)
+    for levels in (0, 3):
+        phi, U = run_fmm(H, w, fmm_levels=levels)
+        assert rel_inf(phi, r.phi) <= PHI_TOL and abs(U - r.U) <= U_TOL * abs(r.U)
+
+
+def test_config5_full_size_against_stored_oracle(H):
+    """BASELINE.json config 5 (N = 262,144) by the FMM: total energy and the ~9,200 stored potentials
+    (tests/golden/config5_oracle.txt, every thread slot and block sampled) at the bars, default order (20) and 24."""
+    from tests.conftest import golden
+    rows = golden("config5_oracle.txt")
+    U_ref, phimax_ref, _ = rows[0]
+    idx = np.array([int(r[0]) for r in rows[1:]])
+    phi_ref = np.array([r[1] for r in rows[1:]])
+    w = W.config(5)
+    for order in (0, 24):
+        phi, U = run_fmm(H, w, fmm_order=order)
+        assert np.max(np.abs(phi[idx] - phi_ref)) <= PHI_TOL * phimax_ref
+        assert abs(U - U_ref) <= U_TOL * abs(U_ref)
+        assert np.all(np.isfinite(phi))
+        Uself = 0.5 * float(np.sum(np.asarray(w.q, dtype=np.longdouble) * phi.astype(np.longdouble)))
+        assert abs(U - Uself) <= U_TOL * abs(Uself)
+
+
+def test_truncation_error_decays_with_the_order(H):
+    """The FMM differs from the direct sum by the truncation of its expansions only: the difference falls by a factor
+    >= 5 per two orders (convergence ratio (sqrt3/2)/2.5 with two-box separation) until rounding takes over, and
+    the direct and FMM plans agree to <= 2e-12 at the default order."""
+    w = W.config(5, N=30000)
+    with H.Plan.from_workload(w, rsqrt_refine=2) as plan:
+        ref, U_ref = plan.evaluate(dev(w.xyz), dev(w.q), sync=True)
+    ref = ref.cpu().numpy()
+    errs = {}
+    for order in (6, 8, 10, 12, 20):
+        phi, _ = run_fmm(H, w, fmm_order=order, fmm_levels=2, rsqrt_refine=2)
+        errs[order] = rel_inf(phi, ref)
+    assert errs[8] < errs[6] / 5 and errs[10] < errs[8] / 5 and errs[12] < errs[10] / 5
+    assert errs[20] <= 2e-12
+
+
+def test_charge_magnitudes_clustered_input_determinism_and_graph(H):
+    """Random-magnitude charges; a clustered (non-uniform) input that leaves most leaves empty and a few crowded;
+    repeated evaluates are bit-identical (fixed summation orders, no floating-point atomics), also when the second
+    call is replayed from the captured graph."""
+    import torch
+    rng = np.random.default_rng(8)
+    w = W.config(3, N=12000)
+    w = w.with_(q=rng.standard_normal(w.N))
+    r = O.hsma(w)
+    phi, U = run_fmm(H, w, fmm_levels=2)
+    assert rel_inf(phi, r.phi) <= PHI_TOL and abs(U - r.U) <= U_TOL * abs(r.U)
+    # clustered: 90 % of the particles in a ball of radius 0.08, the rest uniform
+    N = 16000
+    c = np.array([0.31, 0.62, 0.55])
+    xyz = np.where(rng.random((N, 1)) < 0.9, c + 0.08 * rng.standard_normal((N, 3)).clip(-1, 1) / np.sqrt(3), rng.random((N, 3)))
+    w = W.config(5, N=N).with_(xyz=np.ascontiguousarray(xyz))
+    r = O.hsma(w)
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        with H.Plan.from_workload(w, near_algorithm=H.binding.NEAR_ALG_FMM, fmm_levels=3) as plan:
+            x, q = dev(w.xyz), dev(w.q)
+            out = [torch.empty(w.N, dtype=torch.float64, device="cuda") for _ in range(1)]
+            Us = torch.empty(1, dtype=torch.float64, device="cuda")
+            res = []
+            for _ in range(4):      # the second identical call is captured, later ones replayed
+                H.hsma_evaluate(plan.handle, x, q, out[0], Us)
+                plan.sync()
+                res.append((out[0].clone(), float(Us)))
+            assert H.binding.hsma_plan_info(plan.handle)["graph_replays"] >= 2
+    assert all(torch.equal(res[0][0], a) and res[0][1] == u for a, u in res[1:])
+    phi = res[0][0].cpu().numpy()
+    assert rel_inf(phi, r.phi) <= PHI_TOL and abs(res[0][1] - r.U) <= U_TOL * abs(r.U)
+
+
+def test_where_the_fmm_applies_and_what_it_rejects(H):
+    """Forces and target shards keep the direct kernels (and agree with the FMM potentials); geometry the FMM cannot
+    tile with cubic boxes, the sphere-culled near set and out-of-range orders are rejected at plan creation."""
+    w = W.config(5, N=9000)
+    with H.Plan.from_workload(w, near_algorithm=H.binding.NEAR_ALG_FMM) as plan:
+        x, q = dev(w.xyz), dev(w.q)
+        phi, U = plan.evaluate(x, q, sync=True)
+        assert plan.last_pair_form == FMM
+        phi_f, F, U_f = plan.evaluate_forces(x, q, sync=True)
+        assert plan.last_pair_form == 2
+        a, _ = plan.evaluate_shard(x, q, 0, 4000, sync=True)
+        assert plan.last_pair_form == 1
+        assert rel_inf(phi_f.cpu().numpy(), phi.cpu().numpy()) <= 2e-11
+        assert rel_inf(a.cpu().numpy(), phi.cpu().numpy()[:4000]) <= 2e-11
+    for bad in (dict(L=(1.0, 1.2, 0.9), R_aux=1.3), dict(near_mode=W.NEAR_SPHERE), dict(fmm_order=31), dict(fmm_order=1),
+                dict(fmm_levels=6)):
+        with pytest.raises(H.HsmaError) as e:
+            H.Plan.from_workload(w, near_algorithm=H.binding.NEAR_ALG_FMM, **bad)
+        assert e.value.status == H.HSMA_ERR_INVALID_ARG
