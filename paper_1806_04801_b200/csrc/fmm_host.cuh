@@ -145,20 +145,78 @@ inline int resident_m2l(int p) {
     return per_sm * sms;
 }
 
-// The near sum of step (b) at all N sources, original order, into phi_out [N] (device).  scal_refine as in the
-// direct kernels (1 Newton, 2 cubic) for the P2P part.
-inline hsma_status near_sum(State& S, const double* xyz, const double* q, long long N, const double half[3], int refine,
-                            double* phi_out, std::atomic<size_t>& epoch, cudaStream_t st) {
-    if (N > 2000000000LL) return HSMA_ERR_INVALID_ARG;
+inline Geom make_geom(const State& S, long long N, const double half[3]) {
     Geom G;
     for (int a = 0; a < 3; ++a) { G.base[a] = S.base[a]; G.shell[a] = S.shell[a]; G.refl[a] = S.refl[a]; G.half[a] = half[a]; G.L[a] = S.L[a]; }
     G.levels = choose_levels(S, N);
     G.p = S.p; G.a0 = S.a0; G.w_lut = S.w_lut;
+    return G;
+}
+
+// Upward pass of one evaluate: leaf sort, sorted source records, P2M, M2M.  Afterwards the multipoles of all levels
+// are in S.Mx (used by step (a) through `points` and by step (b) through `downward`).
+inline hsma_status upward(State& S, const double* xyz, const double* q, long long N, const double half[3],
+                          std::atomic<size_t>& epoch, cudaStream_t st) {
+    if (N > 2000000000LL) return HSMA_ERR_INVALID_ARG;
+    const Geom G = make_geom(S, N, half);
     S.last_levels = G.levels;
     const int NC = nc(S.p);
     const long long n_leaves = boxes_at(G, G.levels), n_boxes = level_offset(G, G.levels + 1);
     if (n_leaves >= 65536) return HSMA_ERR_INVALID_ARG;
     const long long n_blk = (N + 255) / 256;
+#define FR(x) do { if ((x) != cudaSuccess) return HSMA_ERR_ALLOC; } while (0)
+    FR(S.key_a.reserve((size_t)N, epoch)); FR(S.key_b.reserve((size_t)N, epoch));
+    FR(S.idx_a.reserve((size_t)N, epoch)); FR(S.idx_b.reserve((size_t)N, epoch));
+    FR(S.leaf_start.reserve((size_t)n_leaves + 1, epoch)); FR(S.chunk_start.reserve((size_t)n_leaves + 1, epoch));
+    FR(S.counts.reserve((size_t)(256 * n_blk + 256), epoch));
+    FR(S.srt.reserve((size_t)N, epoch));
+    FR(S.Mx.reserve((size_t)n_boxes * NC, epoch)); FR(S.Lx.reserve((size_t)n_boxes * NC, epoch));
+#undef FR
+    const unsigned gN = (unsigned)n_blk;
+    key_kernel<<<gN, 256, 0, st>>>(xyz, N, G, S.key_a.p, S.idx_a.p);
+    HSMA_COUNT_LAUNCH();
+    // two stable 8-bit passes: a -> b -> a
+    for (int pass = 0; pass < 2; ++pass) {
+        const int* kin = pass == 0 ? S.key_a.p : S.key_b.p;
+        const int* iin = pass == 0 ? S.idx_a.p : S.idx_b.p;
+        int* kout = pass == 0 ? S.key_b.p : S.key_a.p;
+        int* iout = pass == 0 ? S.idx_b.p : S.idx_a.p;
+        radix_hist_kernel<<<gN, 256, 0, st>>>(kin, N, 8 * pass, n_blk, S.counts.p);
+        radix_rowscan_kernel<<<256, 1024, 0, st>>>(S.counts.p, n_blk, S.counts.p + 256 * n_blk);
+        radix_base_kernel<<<1, 256, 0, st>>>(S.counts.p + 256 * n_blk);
+        radix_scatter_kernel<<<gN, 256, 0, st>>>(kin, iin, N, 8 * pass, n_blk, S.counts.p, S.counts.p + 256 * n_blk, kout, iout);
+        HSMA_COUNT_LAUNCH(); HSMA_COUNT_LAUNCH(); HSMA_COUNT_LAUNCH(); HSMA_COUNT_LAUNCH();
+    }
+    leaf_start_kernel<<<(unsigned)((n_leaves + 1 + 255) / 256), 256, 0, st>>>(S.key_a.p, N, (int)n_leaves, S.leaf_start.p);
+    gather_sorted_kernel<<<gN, 256, 0, st>>>(xyz, q, S.idx_a.p, N, half[0], half[1], half[2], S.srt.p);
+    HSMA_COUNT_LAUNCH(); HSMA_COUNT_LAUNCH();
+    const int inv_bytes = (S.p + 1) * kInvW * (int)sizeof(double);
+    p2m_kernel<<<(unsigned)n_leaves, 256, 8 * NC * sizeof(double2) + inv_bytes, st>>>(G, S.srt.p, S.leaf_start.p, S.Mx.p);
+    HSMA_COUNT_LAUNCH();
+    for (int lev = G.levels - 1; lev >= 0; --lev) {
+        m2m_kernel<<<(unsigned)boxes_at(G, lev), 256, 16 * NC * sizeof(double2), st>>>(G, lev, S.Rsh, S.nm, S.Mx.p);
+        HSMA_COUNT_LAUNCH();
+    }
+    return HSMA_OK;
+}
+
+// Step (a) from the hierarchy built by `upward`: the near sum at T arbitrary points (centred coordinates, device).
+inline hsma_status points(State& S, const double* tgt, long long T, long long N, const double half[3], double* phi_out,
+                          cudaStream_t st) {
+    if (T < 1) return HSMA_OK;
+    const Geom G = make_geom(S, N, half);
+    m2p_points_kernel<<<(unsigned)T, kM2PThreads, 0, st>>>(G, tgt, S.srt.p, S.leaf_start.p, S.Mx.p, phi_out);
+    HSMA_COUNT_LAUNCH();
+    return HSMA_OK;
+}
+
+// Step (b) at all N sources, original order, into phi_out [N] (device): M2L at every level, L2L down, leaves
+// (L2P + P2P).  refine as in the direct kernels (1 Newton, 2 cubic) for the P2P part.
+inline hsma_status downward(State& S, long long N, const double half[3], int refine, double* phi_out,
+                            std::atomic<size_t>& epoch, cudaStream_t st) {
+    const Geom G = make_geom(S, N, half);
+    const int NC = nc(S.p);
+    const long long n_leaves = boxes_at(G, G.levels);
     // M2L launch shape: one persistent wave over the units (group, offset weight), deepest level first
     M2LArgs A;
     A.n_lv = 0;
@@ -180,48 +238,14 @@ inline hsma_status near_sum(State& S, const double* xyz, const double* q, long l
         part_elems += (long long)A.rows * boxes_at(G, A.lv[r].lev) * NC;
     }
     A.off_list = S.off_list; A.off_wprefix = S.off_wprefix; A.n_off = S.n_off;
-#define FR(x) do { if ((x) != cudaSuccess) return HSMA_ERR_ALLOC; } while (0)
-    FR(S.key_a.reserve((size_t)N, epoch)); FR(S.key_b.reserve((size_t)N, epoch));
-    FR(S.idx_a.reserve((size_t)N, epoch)); FR(S.idx_b.reserve((size_t)N, epoch));
-    FR(S.leaf_start.reserve((size_t)n_leaves + 1, epoch)); FR(S.chunk_start.reserve((size_t)n_leaves + 1, epoch));
-    FR(S.counts.reserve((size_t)(256 * n_blk + 256), epoch));
-    FR(S.srt.reserve((size_t)N, epoch));
-    FR(S.Mx.reserve((size_t)n_boxes * NC, epoch)); FR(S.Lx.reserve((size_t)n_boxes * NC, epoch));
-    FR(S.Lpart.reserve((size_t)part_elems, epoch));
-#undef FR
-    const unsigned gN = (unsigned)n_blk;
-    key_kernel<<<gN, 256, 0, st>>>(xyz, N, G, S.key_a.p, S.idx_a.p);
-    HSMA_COUNT_LAUNCH();
-    // two stable 8-bit passes: a -> b -> a
-    for (int pass = 0; pass < 2; ++pass) {
-        const int* kin = pass == 0 ? S.key_a.p : S.key_b.p;
-        const int* iin = pass == 0 ? S.idx_a.p : S.idx_b.p;
-        int* kout = pass == 0 ? S.key_b.p : S.key_a.p;
-        int* iout = pass == 0 ? S.idx_b.p : S.idx_a.p;
-        radix_hist_kernel<<<gN, 256, 0, st>>>(kin, N, 8 * pass, n_blk, S.counts.p);
-        radix_rowscan_kernel<<<256, 1024, 0, st>>>(S.counts.p, n_blk, S.counts.p + 256 * n_blk);
-        radix_base_kernel<<<1, 256, 0, st>>>(S.counts.p + 256 * n_blk);
-        radix_scatter_kernel<<<gN, 256, 0, st>>>(kin, iin, N, 8 * pass, n_blk, S.counts.p, S.counts.p + 256 * n_blk, kout, iout);
-        HSMA_COUNT_LAUNCH(); HSMA_COUNT_LAUNCH(); HSMA_COUNT_LAUNCH(); HSMA_COUNT_LAUNCH();
-    }
-    leaf_start_kernel<<<(unsigned)((n_leaves + 1 + 255) / 256), 256, 0, st>>>(S.key_a.p, N, (int)n_leaves, S.leaf_start.p);
-    gather_sorted_kernel<<<gN, 256, 0, st>>>(xyz, q, S.idx_a.p, N, half[0], half[1], half[2], S.srt.p);
-    HSMA_COUNT_LAUNCH(); HSMA_COUNT_LAUNCH();
-    // upward pass
-    const int inv_bytes = (S.p + 1) * kInvW * (int)sizeof(double);
-    p2m_kernel<<<(unsigned)n_leaves, 256, 8 * NC * sizeof(double2) + inv_bytes, st>>>(G, S.srt.p, S.leaf_start.p, S.Mx.p);
-    HSMA_COUNT_LAUNCH();
-    for (int lev = G.levels - 1; lev >= 0; --lev) {
-        m2m_kernel<<<(unsigned)boxes_at(G, lev), 256, 16 * NC * sizeof(double2), st>>>(G, lev, S.Rsh, S.nm, S.Mx.p);
-        HSMA_COUNT_LAUNCH();
-    }
-    // far field: M2L at every level, then down
+    if (S.Lpart.reserve((size_t)part_elems, epoch) != cudaSuccess) return HSMA_ERR_ALLOC;
     m2l_kernel<<<(unsigned)Gm2l, kM2LThreads, m2l_smem_bytes(S.p), st>>>(G, A, S.Mx.p, S.Stab, S.nm, S.pm, S.sfmap, S.Lpart.p);
     HSMA_COUNT_LAUNCH();
     for (int lev = 0; lev <= G.levels; ++lev) {
         l2l_kernel<<<(unsigned)boxes_at(G, lev), 256, 2 * NC * sizeof(double2), st>>>(G, lev, S.Rsh, S.nm, S.Lpart.p, A, Gm2l, S.Lx.p);
         HSMA_COUNT_LAUNCH();
     }
+    const int inv_bytes = (S.p + 1) * kInvW * (int)sizeof(double);
     const size_t leaf_smem = NC * sizeof(double2) + inv_bytes;
     leaf_chunks_kernel<<<1, 1024, 0, st>>>(S.leaf_start.p, (int)n_leaves, S.chunk_start.p);
     HSMA_COUNT_LAUNCH();

@@ -842,5 +842,95 @@ __global__ void __launch_bounds__(kLeafThreads) leaf_kernel(const Geom G, const 
     }
 }
 
+// ---- step (a) from the same hierarchy: the near sum at arbitrary points (the check targets) --------------------------------
+// A check target x may lie outside the central cell (the circumsphere points of PAPER.md:80-82), where no local
+// expansion exists; it is served by the MULTIPOLES directly (M2P): with b_l the box of level l that contains x (global
+// grid coordinates, any cell), the boxes of b_l's interaction list -- parent within kWs of b_l's parent, more than
+// kWs away from b_l; at level 0 every box of the cell table more than kWs away -- are evaluated as
+//     phi += (1/a) Re sum_{n,m} conj M_n^m S_n^m((x' - c)/a),      x' = sigma o (x - kL)
+// (the target is moved into the frame of the image, as in the pair kernels, so the central box's moments serve
+// unreflected), and the leaf boxes within kWs of b_lmax are summed directly.  Same separation and order as M2L, hence
+// the same truncation error.  One CTA per target; the threads share the boxes; fixed-order tree reduction.
+constexpr int kM2PThreads = 128;
+
+__global__ void __launch_bounds__(kM2PThreads) m2p_points_kernel(const Geom G, const double* __restrict__ tgt /* [T,3] centred */,
+                                                                 const Src4* __restrict__ srt, const int* __restrict__ leaf_start,
+                                                                 const double2* __restrict__ M, double* __restrict__ phi_out) {
+    __shared__ double red[kM2PThreads];
+    const int p = G.p, NC = nc(p), lmax = G.levels, tid = threadIdx.x;
+    const double x = tgt[3 * (size_t)blockIdx.x], y = tgt[3 * (size_t)blockIdx.x + 1], z = tgt[3 * (size_t)blockIdx.x + 2];
+    const double xc[3] = {x, y, z};
+    int gl[3];   // leaf-level box of the target, global coordinates
+#pragma unroll
+    for (int a = 0; a < 3; ++a) gl[a] = (int)floor((xc[a] + G.half[a]) * (double)(1 << lmax) / G.a0);
+    double acc = 0.0;
+    // far field: multipoles of the interaction lists, all levels
+    for (int lev = lmax; lev >= 0; --lev) {
+        const int sh = lmax - lev;
+        const int b[3] = {gl[0] >> sh, gl[1] >> sh, gl[2] >> sh};
+        int R[3];   // candidate offsets |d_a| <= R_a
+#pragma unroll
+        for (int a = 0; a < 3; ++a) R[a] = lev > 0 ? kOffR : (2 * G.shell[a] + 1) * G.base[a] - 1;
+        const int wx = 2 * R[0] + 1, wy = 2 * R[1] + 1, wz = 2 * R[2] + 1;
+        const double al = G.a0 / (double)(1 << lev), ial = 1.0 / al;
+        const double2* Mlev = M + level_offset(G, lev) * NC;
+        for (int o = tid; o < wx * wy * wz; o += kM2PThreads) {
+            const int dx = o / (wy * wz) - R[0], dy = (o / wz) % wy - R[1], dz = o % wz - R[2];
+            if (max(abs(dx), max(abs(dy), abs(dz))) <= kWs) continue;
+            const int g[3] = {b[0] + dx, b[1] + dy, b[2] + dz};
+            bool ok = true;
+            if (lev > 0)
+#pragma unroll
+                for (int a = 0; a < 3; ++a) { const int P = b[a] >> 1; ok = ok && g[a] >= 2 * (P - kWs) && g[a] <= 2 * (P + kWs) + 1; }
+            ImageBox ib;
+            if (!ok || !image_box(G, lev, g[0], g[1], g[2], ib)) continue;
+            double c[3]; int ic[3];
+            box_centre(G, lev, ib.box, c, ic);
+            // target in the image's frame, relative to the central box's centre, in box units
+            const double rx = (flip(x - ib.sx, ib.fx) - c[0]) * ial, ry = (flip(y - ib.sy, ib.fy) - c[1]) * ial,
+                         rz = (flip(z - ib.sz, ib.fz) - c[2]) * ial;
+            const double r2 = fma(rz, rz, fma(ry, ry, rx * rx)), ir2 = 1.0 / r2;
+            const double2* Mb = Mlev + (long long)ib.box * NC;
+            double sr = rsqrt_cubic(r2), si = 0.0, sum = 0.0;      // S_0^0 = 1/r
+            for (int m = 0; m <= p; ++m) {
+                if (m > 0) { const double f = (double)(2 * m - 1) * ir2, u = (sr * rx - si * ry) * f; si = (sr * ry + si * rx) * f; sr = u; }
+                double p1r = sr, p1i = si, p2r = 0.0, p2i = 0.0;
+                double2 mc = Mb[cidx(m, m)];
+                double s = fma(mc.x, sr, mc.y * si);
+                for (int n = m + 1; n <= p; ++n) {
+                    const double tz = (double)(2 * n - 1) * rz, gg = (double)(n - 1 + m) * (double)(n - 1 - m);
+                    const double cr = (tz * p1r - gg * p2r) * ir2, ci = (tz * p1i - gg * p2i) * ir2;
+                    mc = Mb[cidx(n, m)];
+                    s = fma(mc.x, cr, s); s = fma(mc.y, ci, s);
+                    p2r = p1r; p2i = p1i; p1r = cr; p1i = ci;
+                }
+                sum += m == 0 ? s : 2.0 * s;
+            }
+            acc = fma(ib.w * ial, sum, acc);
+        }
+    }
+    // near field: the leaf boxes within kWs, pair by pair (cubic refinement: step (a) feeds the fit)
+    for (int o = 0; o < (2 * kWs + 1) * (2 * kWs + 1) * (2 * kWs + 1); ++o) {
+        const int dx = o / 25 - kWs, dy = (o / 5) % 5 - kWs, dz = o % 5 - kWs;
+        ImageBox ib;
+        if (!image_box(G, lmax, gl[0] + dx, gl[1] + dy, gl[2] + dz, ib)) continue;
+        const int s0 = leaf_start[ib.box], s1 = leaf_start[ib.box + 1];
+        const double tx = flip(x - ib.sx, ib.fx), ty = flip(y - ib.sy, ib.fy), tz = flip(z - ib.sz, ib.fz);
+        double a2 = 0.0;
+        for (int j = s0 + tid; j < s1; j += kM2PThreads) {
+            const Src4 s = srt[j];
+            pair<2>(tx, ty, tz, s.x, s.y, s.z, s.q, a2);
+        }
+        acc = fma(ib.w, a2, acc);
+    }
+    red[tid] = acc;
+    __syncthreads();
+    for (int o = kM2PThreads / 2; o > 0; o >>= 1) {
+        if (tid < o) red[tid] += red[tid + o];
+        __syncthreads();
+    }
+    if (tid == 0) phi_out[blockIdx.x] = red[0];
+}
+
 }  // namespace fmm
 }  // namespace hsma

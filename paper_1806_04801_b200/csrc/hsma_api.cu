@@ -738,8 +738,21 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
         p->last_images = Ns;
     }
 
+    // near_algorithm = FMM: step (b) over all N targets (potentials) by the fast multipole method; its
+    // upward pass (leaf sort, P2M, M2M) comes first because step (a) can use the multipoles too
+    const bool use_fmm = p->fmm.enabled && phase == kPhaseAll && n_parts == 0 && !field && t0 == 0 && t1 == N && p->pair_form == 0;
+    if (use_fmm) {
+        const hsma_status fs = fmm::upward(p->fmm, xyz, q, N, p->half, g_alloc_epoch, st);
+        if (fs != HSMA_OK) return fs;
+    }
     // H2 (a): Phi_in (or the far-cell data) at the monitoring points c0..c1-1 -> pc [Kt]
-    if (phase != kPhaseRest && c1 > c0) {
+    if (use_fmm && p->cells_rhs == p->cells_near && !p->need_grad && c1 > c0) {
+        // the check targets from the same hierarchy: multipoles of the interaction lists + direct sum over the near leaves
+        MARK(1);
+        const hsma_status fs = fmm::points(p->fmm, p->chk + 3 * c0, c1 - c0, N, p->half, p->pc + c0, st);
+        if (fs != HSMA_OK) return fs;
+        MARK(2);
+    } else if (phase != kPhaseRest && c1 > c0) {
         const long long Tc = c1 - c0;
         const bool fa = p->need_grad;   // derivative rows need grad Phi_in at the check targets: the FIELD form of (a)
         const Launch s = choose_near(Tc, n_tiles_near, C_a, 2, fa);
@@ -810,8 +823,6 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
         const int refine = p->refine ? p->refine : ((double)N * (double)p->last_images < 4294967296.0 ? 2 : 1);
         // rsqrt_refine = 0: the cubic step while (b) is latency-bound anyway (< 2^32 pairs), Newton above
         const size_t comps = field ? 4 : 1;
-        // near_algorithm = FMM: step (b) over all N targets (potentials) by the fast multipole method, DESIGN.md 6.13
-        const bool use_fmm = p->fmm.enabled && !field && t0 == 0 && t1 == N && p->pair_form == 0;
         bool sym = !use_fmm && !p->sphere && p->pair_form != 1 && t0 == 0 && t1 == N && sym_applies(n_tiles, C_b);
         Launch sb = choose_near(T, n_tiles_near, C_b, refine, field);
         if (use_fmm && p->sym_phi.reserve((size_t)N) != cudaSuccess) return HSMA_ERR_ALLOC;
@@ -832,7 +843,7 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
         MARK(3);
         PartLayout layout_b = sb.layout(p->part_b.p);
         if (use_fmm) {
-            const hsma_status fs = fmm::near_sum(p->fmm, xyz, q, N, p->half, refine, p->sym_phi.p, g_alloc_epoch, st);
+            const hsma_status fs = fmm::downward(p->fmm, N, p->half, refine, p->sym_phi.p, g_alloc_epoch, st);
             if (fs != HSMA_OK) return fs;
             layout_b = PartLayout{p->sym_phi.p, 1, 1, 1, (int)std::min<long long>(T, 2147483647LL)};
         } else if (sym) {

@@ -32,10 +32,15 @@ def rel_inf(a, b):
     return float(np.max(np.abs(a - b)) / np.max(np.abs(b)))
 
 
-def run_fmm(H, w, **kw):
+def run_fmm(H, w, oracle=None, **kw):
+    """Evaluate with near_algorithm = FMM.  With an oracle result: also the right-hand side of the fit, i.e. step (a) --
+    which the FMM plan computes from the same multipoles (m2p_points_kernel) -- and the coefficients against it."""
     with H.Plan.from_workload(w, near_algorithm=H.binding.NEAR_ALG_FMM, **kw) as plan:
         phi, U = plan.evaluate(dev(w.xyz), dev(w.q), sync=True)
         assert plan.last_pair_form == FMM
+        if oracle is not None:
+            assert rel_inf(plan.rhs().cpu().numpy(), oracle.rhs) <= 1e-10
+            assert rel_inf(plan.coeffs().cpu().numpy(), oracle.A) <= 1e-9
     return phi.cpu().numpy(), float(U)
 
 
@@ -45,7 +50,7 @@ def test_config2_every_potential(H, levels):
     comes from the few level-1 boxes three boxes away) and forced deeper hierarchies (M2M, level-2/3 M2L, L2L)."""
     w = W.config(2)
     r = O.hsma(w)
-    phi, U = run_fmm(H, w, fmm_levels=levels)
+    phi, U = run_fmm(H, w, oracle=r, fmm_levels=levels)
     assert rel_inf(phi, r.phi) <= PHI_TOL and abs(U - r.U) <= U_TOL * abs(r.U)
 
 
@@ -60,7 +65,7 @@ def test_all_cell_tables_every_potential(H, idx, N, levels, order):
     phi and U (phi inside its bar, U not), so lattice-aligned inputs take order 26."""
     w = W.config(idx, N=N)
     r = O.hsma(w)
-    phi, U = run_fmm(H, w, fmm_levels=levels, fmm_order=order)
+    phi, U = run_fmm(H, w, oracle=r, fmm_levels=levels, fmm_order=order)
     assert rel_inf(phi, r.phi) <= PHI_TOL and abs(U - r.U) <= U_TOL * abs(r.U)
 
 
@@ -118,10 +123,10 @@ def test_charge_magnitudes_clustered_input_determinism_and_graph(H):
     r = O.hsma(w)
     phi, U = run_fmm(H, w, fmm_levels=2)
     assert rel_inf(phi, r.phi) <= PHI_TOL and abs(U - r.U) <= U_TOL * abs(r.U)
-    # clustered: 90 % of the particles in a ball of radius 0.08, the rest uniform
+    # clustered: 90 % of the particles in a Gaussian blob of width 0.03, the rest uniform
     N = 16000
     c = np.array([0.31, 0.62, 0.55])
-    xyz = np.where(rng.random((N, 1)) < 0.9, c + 0.08 * rng.standard_normal((N, 3)).clip(-1, 1) / np.sqrt(3), rng.random((N, 3)))
+    xyz = np.where(rng.random((N, 1)) < 0.9, np.mod(c + 0.03 * rng.standard_normal((N, 3)), 1.0), rng.random((N, 3)))
     w = W.config(5, N=N).with_(xyz=np.ascontiguousarray(xyz))
     r = O.hsma(w)
     side = torch.cuda.Stream()
