@@ -22,7 +22,7 @@ import math
 import os
 import subprocess
 from dataclasses import dataclass
-from typing import Optional
+from typing import Callable, Optional
 
 import numpy as np
 
@@ -481,9 +481,149 @@ def validate_geometry(L, shell, R_aux):
     return R0
 
 
+# ---- the fit of Eq.(7), one routine per closure --------------------------------------------------------------------
+# A closure says WHERE Phi_in is sampled (check_targets), WHICH linear functionals of the harmonic series are matched
+# there (the rows of the fitting matrix F) and WHAT they are matched to (the right-hand side, built from the sums of
+# Phi_in -- and, for derivative rows, of grad Phi_in -- at the check targets).  hsma() below is the same for all of them.
+@dataclass
+class Closure:
+    F: np.ndarray                  # [rows, unknowns] fitting matrix, Eq.(7)
+    check_targets: np.ndarray      # [K_t, 3] where Phi_in is summed
+    drop_constant: bool            # no row sees the constant harmonic: column (0,0) dropped, A00 = 0 (reading S2)
+    rhs: Callable                  # rhs(phi_check [K_t], grad_check() -> [K_t, 3]) -> [rows]
+    far_cells: Optional["CellTable"] = None   # far-data closure: the cells whose field is fitted (else the near set)
+
+
+def _wall_axes(xf, L, kind):
+    """The reflecting axis whose face each wall point lies on (cavity: any axis; slab: z)."""
+    return np.argmax(np.isclose(np.abs(xf), 0.5 * L, rtol=0, atol=1e-12 * L.max()) &
+                     np.array([kind == BC_MIRROR_CAVITY, kind == BC_MIRROR_CAVITY, True]), axis=1)
+
+
+def closure_periodic_circumsphere(w, L, R0, p) -> Closure:
+    """K points x_i on the circumsphere |x| = R0 (Fibonacci grid) and their partners x~_i wrapped into
+    the box; v_i = Phi(x_i) - Phi(x~_i) = 0.  Rows B(x_i) - B(x~_i); the constant cancels (reading S2)."""
+    x = fibonacci_sphere_checkpoints(w.K, R0) if w.check_xyz is None else np.asarray(w.check_xyz, float)
+    xt = wrap_into_box(x, L)
+    keep = np.any(np.abs(x - xt) > 0, axis=1)       # rows with x~ = x carry no information
+    x, xt = x[keep], xt[keep]
+    Bx = real_solid_harmonics(x, p, R0)
+    Bt = real_solid_harmonics(xt, p, R0)
+    K = x.shape[0]
+    return Closure((Bx - Bt)[:, 1:], np.concatenate([x, xt], axis=0), True,
+                   lambda phi, grad: -(phi[:K] - phi[K:]))
+
+
+def closure_periodic_face_pairs(w, L, R0, p) -> Closure:
+    """BASELINE.json: "check-point pairs on opposite faces".  Matching the values alone is rank deficient (every
+    harmonic even in x, y and z is invisible, reading S15); periodicity of Phi AND of its normal derivative across the
+    faces is the complete condition: K points on the lower faces x_a = -L_a/2, partners x + L_a e_a, one value row and
+    one derivative row per pair.  The constant is dropped (reading S2)."""
+    x = default_lower_face_points(w.K, L) if w.check_xyz is None else np.asarray(w.check_xyz, float)
+    on = np.isclose(x, -0.5 * L, rtol=0, atol=1e-12 * L.max())
+    if not on.any(axis=1).all():
+        raise ValueError("face-pair check points must lie on the lower faces x_a = -L_a/2")
+    pair_axes = np.argmax(on, axis=1)
+    xt = x.copy()
+    xt[np.arange(x.shape[0]), pair_axes] += L[pair_axes]
+    idx = np.arange(x.shape[0])
+    Fv = real_solid_harmonics(x, p, R0) - real_solid_harmonics(xt, p, R0)
+    Fd = (real_solid_harmonics_grad(x, p, R0)[idx, :, pair_axes]
+          - real_solid_harmonics_grad(xt, p, R0)[idx, :, pair_axes])
+    K = x.shape[0]
+
+    def rhs(phi, grad):
+        g = grad()[np.arange(2 * K), np.tile(pair_axes, 2)]
+        return np.concatenate([-(phi[:K] - phi[K:]), -(g[:K] - g[K:])])
+
+    return Closure(np.concatenate([Fv, Fd], axis=0)[:, 1:], np.concatenate([x, xt], axis=0), True, rhs)
+
+
+def closure_slab_boundary(w, L, R0, p, neumann) -> Closure:
+    """Slab closed by its own boundary conditions: two families of rows ("boundary
+    conditions", 80-82 for the periodic directions):
+      pairs    K Fibonacci points on the circumsphere and their partners wrapped in x and y only,
+               Phi(x_i) - Phi(x~_i) = 0 (the image system is xy-periodic at every height, also beyond the plates);
+      plates   K points on the two faces z = +-H/2: Phi = 0 for gamma = -1 ("DBC"), d Phi/dz = 0
+               for gamma = +1.
+    Dirichlet plate rows see the constant harmonic (no column dropped); Neumann rows do not (A00 = 0)."""
+    xs = fibonacci_sphere_checkpoints(w.K, R0)
+    xt = wrap_into_box(xs, L, periodic_axes=(True, True, False))
+    keep = np.any(np.abs(xs - xt) > 0, axis=1)
+    xs, xt = xs[keep], xt[keep]
+    xf = default_face_points(w.K, L, (2,)) if w.check_xyz is None else np.asarray(w.check_xyz, float)
+    n_pair = xs.shape[0]
+    if neumann:
+        axes = _wall_axes(xf, L, w.kind)
+        Fw = real_solid_harmonics_grad(xf, p, R0)[np.arange(xf.shape[0]), :, axes]
+    else:
+        axes, Fw = None, real_solid_harmonics(xf, p, R0)
+    F = np.concatenate([real_solid_harmonics(xs, p, R0) - real_solid_harmonics(xt, p, R0), Fw], axis=0)
+
+    def rhs(phi, grad):
+        if neumann:
+            wall = -grad()[2 * n_pair:][np.arange(xf.shape[0]), axes]
+        else:
+            wall = -phi[2 * n_pair:]
+        return np.concatenate([-(phi[:n_pair] - phi[n_pair:2 * n_pair]), wall])
+
+    return Closure(F[:, 1:] if neumann else F, np.concatenate([xs, xt, xf], axis=0), neumann, rhs)
+
+
+def closure_walls(w, L, R0, p, neumann) -> Closure:
+    """Reflecting walls closed by the wall condition at K wall points: gamma = -1 is a conductor,
+    Phi_in + Phi_out = 0 (Dirichlet rows B(x), "DBC"); gamma = +1 the insulating / symmetric wall,
+    d(Phi_in + Phi_out)/d x_a = 0 with a the axis of the wall the point lies on (Neumann rows)."""
+    if w.check_xyz is not None:
+        x = np.asarray(w.check_xyz, float)
+    else:
+        x = default_face_points(w.K, L, (0, 1, 2) if w.kind == BC_MIRROR_CAVITY else (2,))
+    if neumann:
+        axes = _wall_axes(x, L, w.kind)
+        F = real_solid_harmonics_grad(x, p, R0)[np.arange(x.shape[0]), :, axes][:, 1:]
+        return Closure(F, x, True, lambda phi, grad: -grad()[np.arange(x.shape[0]), axes])
+    return Closure(real_solid_harmonics(x, p, R0), x, False, lambda phi, grad: -phi)
+
+
+def closure_far_data(w, L, R0, p) -> Closure:
+    """Reading S16 (config 4): Phi_out := the field of the far cells (far_shell minus near_shell), fitted from its
+    directly summed values at K points on the six faces.  Rows B(x), right-hand side +Phi_far(x)."""
+    x = np.asarray(w.check_xyz, float) if w.check_xyz is not None else default_face_points(w.K, L, (0, 1, 2))
+    far = cell_table(w.kind, L, w.far_shell, w.gamma, exclude_shell=w.near_shell)
+    return Closure(real_solid_harmonics(x, p, R0), x, False, lambda phi, grad: phi.copy(), far_cells=far)
+
+
+def make_closure(w, L, R0, p) -> Closure:
+    periodic = w.kind == BC_PERIODIC
+    if periodic:
+        if w.closure == CLOSURE_FACE_PAIRS:
+            return closure_periodic_face_pairs(w, L, R0, p)
+        if w.closure != CLOSURE_BOUNDARY:
+            raise ValueError("periodic kind uses the boundary or the face-pair closure")
+        return closure_periodic_circumsphere(w, L, R0, p)
+    if w.closure == CLOSURE_FAR_DATA:
+        return closure_far_data(w, L, R0, p)
+    # wall rows of the boundary closure on reflecting axes (PAPER.md:52, 74)
+    if w.gamma not in (-1.0, 1.0):
+        raise ValueError("the boundary closure on reflecting walls is defined for gamma = -1 (Dirichlet) or +1 (Neumann)")
+    neumann = w.gamma == 1.0
+    if w.kind == BC_SLAB:
+        return closure_slab_boundary(w, L, R0, p, neumann)
+    return closure_walls(w, L, R0, p, neumann)
+
+
+def must_be_neutral(w) -> bool:
+    """Periodic axes without a screening conductor, and Neumann walls, admit no solution for a net charge (S17)."""
+    slab_bc = w.kind == BC_SLAB and w.closure == CLOSURE_BOUNDARY
+    neumann = w.kind != BC_PERIODIC and w.closure == CLOSURE_BOUNDARY and w.gamma == 1.0
+    return w.kind == BC_PERIODIC or (w.kind == BC_SLAB and not slab_bc) or neumann
+
+
 def hsma(w, targets_slice: Optional[slice] = None, dipole: str = "exact", dr_rel: float = 1e-5,
          p: Optional[int] = None, M: Optional[int] = None, forces: bool = False) -> OracleResult:
-    """One HSMA evaluation of workload `w` (an hsma_workloads.Workload).
+    """One HSMA evaluation of workload `w` (an hsma_workloads.Workload), PAPER.md:140-142 in order:
+    cells -> closure (check points, fitting matrix) -> nodes -> Phi_in at the check points -> least squares ->
+    surface mapping -> sums at the sources -> energy.
     `targets_slice`: evaluate phi only at that slice of the sources (sampled parity at full size);
     U is then the partial sum over the slice.  `dipole`: "exact" (reading S9, primary) or "fd3"
     (the paper's three-sphere central difference, Eq.12-14, cross-check)."""
@@ -497,29 +637,10 @@ def hsma(w, targets_slice: Optional[slice] = None, dipole: str = "exact", dr_rel
     src = np.asarray(w.xyz, dtype=np.float64) - 0.5 * L
     q = np.asarray(w.q, dtype=np.float64)
     N = src.shape[0]
-    periodic = w.kind == BC_PERIODIC
-    # grounded slab: x,y periodic, conducting plates at z = +-H/2
-    # (gamma = -1), closed by the boundary conditions themselves instead of far-cell data
-    slab_bc = w.kind == BC_SLAB and w.closure == CLOSURE_BOUNDARY
-    n_pair = 0
-    # wall rows of the boundary closure on reflecting axes: gamma = -1 is a conductor, Phi = 0
-    # (Dirichlet rows); gamma = +1 is the insulating / symmetric wall, d Phi/d n = 0 (Neumann rows)
-    neumann = w.kind != BC_PERIODIC and w.closure == CLOSURE_BOUNDARY and w.gamma == 1.0
     if w.kind != BC_PERIODIC and w.closure == CLOSURE_BOUNDARY and w.gamma not in (-1.0, 1.0):
         raise ValueError("the boundary closure on reflecting walls is defined for gamma = -1 (Dirichlet) or +1 (Neumann)")
-    if periodic or (w.kind == BC_SLAB and not slab_bc) or neumann:
-        if abs(q.sum()) > 1e-12 * np.abs(q).sum():
-            raise ValueError("periodic / Neumann system must be neutral (reading S17)")
-
-    def wall_rows(xf):
-        """Rows of the fitting matrix at wall points: B(x) (Dirichlet) or dB/dx_a (Neumann), a = the axis whose
-        face the point lies on; returns (rows, axes)."""
-        if not neumann:
-            return real_solid_harmonics(xf, p, R0), None
-        axes = np.argmax(np.isclose(np.abs(xf), 0.5 * L, rtol=0, atol=1e-12 * L.max()) &
-                         np.array([w.kind == BC_MIRROR_CAVITY, w.kind == BC_MIRROR_CAVITY, True]), axis=1)
-        G = real_solid_harmonics_grad(xf, p, R0)
-        return G[np.arange(xf.shape[0]), :, axes], axes
+    if must_be_neutral(w) and abs(q.sum()) > 1e-12 * np.abs(q).sum():
+        raise ValueError("periodic / Neumann system must be neutral (reading S17)")
 
     # -- preparation step, PAPER.md:140 ----------------------------------------------------
     near = cell_table(w.kind, L, w.near_shell, w.gamma)
@@ -532,101 +653,25 @@ def hsma(w, targets_slice: Optional[slice] = None, dipole: str = "exact", dr_rel
         near_src, near_q, near_cells = (*images_inside_sphere(src, q, near, w.R_aux), identity_cell())
     else:
         near_src, near_q, near_cells = src, q, near
-    face_pairs = periodic and w.closure == CLOSURE_FACE_PAIRS
-    if face_pairs:
-        # BASELINE.json: "check-point pairs on opposite faces".  Matching the values alone is rank deficient (every
-        # harmonic even in x, y and z is invisible, reading S15); periodicity of Phi AND of its normal derivative
-        # across the faces is the complete condition: K points on the lower faces x_a = -L_a/2, partners x + L_a e_a,
-        # one value row and one derivative row per pair.  The constant is dropped (reading S2).
-        x = default_lower_face_points(w.K, L) if w.check_xyz is None else np.asarray(w.check_xyz, float)
-        on = np.isclose(x, -0.5 * L, rtol=0, atol=1e-12 * L.max())
-        if not on.any(axis=1).all():
-            raise ValueError("face-pair check points must lie on the lower faces x_a = -L_a/2")
-        pair_axes = np.argmax(on, axis=1)
-        xt = x.copy()
-        xt[np.arange(x.shape[0]), pair_axes] += L[pair_axes]
-        idx = np.arange(x.shape[0])
-        Fv = real_solid_harmonics(x, p, R0) - real_solid_harmonics(xt, p, R0)
-        Fd = (real_solid_harmonics_grad(x, p, R0)[idx, :, pair_axes]
-              - real_solid_harmonics_grad(xt, p, R0)[idx, :, pair_axes])
-        F = np.concatenate([Fv, Fd], axis=0)[:, 1:]
-        check_targets = np.concatenate([x, xt], axis=0)
-        n_pair = x.shape[0]
-    elif periodic:
-        if w.closure != CLOSURE_BOUNDARY:
-            raise ValueError("periodic kind uses the boundary or the face-pair closure")
-        x = fibonacci_sphere_checkpoints(w.K, R0) if w.check_xyz is None else np.asarray(w.check_xyz, float)
-        xt = wrap_into_box(x, L)
-        keep = np.any(np.abs(x - xt) > 0, axis=1)       # rows with x~ = x carry no information
-        x, xt = x[keep], xt[keep]
-        Bx = real_solid_harmonics(x, p, R0)
-        Bt = real_solid_harmonics(xt, p, R0)
-        F = (Bx - Bt)[:, 1:]                              # reading S2: drop the constant, A00 = 0
-        check_targets = np.concatenate([x, xt], axis=0)
-        n_pair = x.shape[0]
-    elif slab_bc:
-        # Two families of rows ("boundary conditions", 80-82 for the periodic directions):
-        #   pairs    K Fibonacci points on the circumsphere and their partners wrapped in x and y only,
-        #            Phi(x_i) - Phi(x~_i) = 0 (the image system is xy-periodic at every height, also beyond the plates);
-        #   plates   K points on the two faces z = +-H/2, Phi = 0 ("DBC").
-        # The constant harmonic is seen by the plate rows, so no column is dropped.
-        xs = fibonacci_sphere_checkpoints(w.K, R0)
-        xt = wrap_into_box(xs, L, periodic_axes=(True, True, False))
-        keep = np.any(np.abs(xs - xt) > 0, axis=1)
-        xs, xt = xs[keep], xt[keep]
-        xf = default_face_points(w.K, L, (2,)) if w.check_xyz is None else np.asarray(w.check_xyz, float)
-        Fw, wall_axes = wall_rows(xf)
-        F = np.concatenate([real_solid_harmonics(xs, p, R0) - real_solid_harmonics(xt, p, R0), Fw], axis=0)
-        if neumann:
-            F = F[:, 1:]                                  # neither family of rows sees the constant: A00 = 0
-        check_targets = np.concatenate([xs, xt, xf], axis=0)
-        n_pair = xs.shape[0]
-    else:
-        if w.check_xyz is not None:
-            x = np.asarray(w.check_xyz, float)
-        elif w.closure == CLOSURE_FAR_DATA:
-            x = default_face_points(w.K, L, (0, 1, 2))
-        else:
-            x = default_face_points(w.K, L, (0, 1, 2) if w.kind == BC_MIRROR_CAVITY else (2,))
-        if w.closure == CLOSURE_FAR_DATA:
-            F, wall_axes = real_solid_harmonics(x, p, R0), None
-        else:
-            F, wall_axes = wall_rows(x)
-            if neumann:
-                F = F[:, 1:]
-        check_targets = x
+    cl = make_closure(w, L, R0, p)
+    F, check_targets = cl.F, cl.check_targets
     nodes, nrm, wq = make_nodes(M, w.R_aux, w.quad_rule)
     Ynodes = real_solid_harmonics(nodes, p, w.R_aux)      # = Y_nm at the node directions (r = a)
 
     # -- update step, PAPER.md:142 ---------------------------------------------------------
     # right-hand side: Phi_in at the monitoring points, Eq.(5), cost O(N_s N_m) PAPER.md:78
-    if w.closure == CLOSURE_FAR_DATA:
-        far = cell_table(w.kind, L, w.far_shell, w.gamma, exclude_shell=w.near_shell)
-        phi_check = near_sum(check_targets, src, q, far)
-        rhs = phi_check.copy()                            # Phi_out := field of the far cells (S16)
-        n_check_cells = far.w.shape[0]
+    if cl.far_cells is not None:
+        phi_check = near_sum(check_targets, src, q, cl.far_cells)   # Phi_out := field of the far cells (S16)
+        n_check_cells = cl.far_cells.w.shape[0]
+        rhs = cl.rhs(phi_check, None)
     else:
         phi_check = near_sum(check_targets, near_src, near_q, near_cells)
         n_check_cells = near.w.shape[0]
-        if face_pairs:
-            K = x.shape[0]
-            g = near_grad(check_targets, near_src, near_q, near_cells)[np.arange(2 * K), np.tile(pair_axes, 2)]
-            rhs = np.concatenate([-(phi_check[:K] - phi_check[K:]), -(g[:K] - g[K:])])
-        elif periodic:
-            K = x.shape[0]
-            rhs = -(phi_check[:K] - phi_check[K:])        # v_i = Phi(x_i) - Phi(x~_i) = 0
-        else:
-            xw = check_targets[2 * n_pair:]               # the wall points (all of them in the cavity)
-            if neumann:                                   # d(Phi_in + Phi_out)/d x_a = 0 on the wall
-                gw = near_grad(xw, near_src, near_q, near_cells)
-                wall_rhs = -gw[np.arange(xw.shape[0]), wall_axes]
-            else:                                         # grounded wall: Phi_in + Phi_out = 0
-                wall_rhs = -phi_check[2 * n_pair:]
-            rhs = np.concatenate([-(phi_check[:n_pair] - phi_check[n_pair:2 * n_pair]), wall_rhs])
+        rhs = cl.rhs(phi_check, lambda: near_grad(check_targets, near_src, near_q, near_cells))
     # least squares, Eq.(7)
     sol, *_ = np.linalg.lstsq(F, rhs, rcond=None)
     sv = np.linalg.svd(F, compute_uv=False)
-    A = np.concatenate([[0.0], sol]) if (periodic or neumann) else sol
+    A = np.concatenate([[0.0], sol]) if cl.drop_constant else sol
     fit_rms = float(np.linalg.norm(F @ sol - rhs) / math.sqrt(F.shape[0]))
 
     # harmonic surface mapping, Eq.(10),(11) PAPER.md:99-105: on |r'| = R_aux
