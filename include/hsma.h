@@ -85,8 +85,9 @@ typedef enum {
     HSMA_NEAR_ALG_FMM = 1      /* SURVEY.md 8(f) NEXT 4, Table I: step (b) by a uniform-grid
                                   fast multipole method: O(N) instead of O(N^2), the same sum up to the
                                   truncation of the expansions (<= 1e-12 of max|phi| at the default order 20).  Used when an
-                                  evaluate covers all N targets (potentials; forces and target shards keep the direct
-                                  kernels).  Needs the whole-cell near set and box sides that are integer multiples of
+                                  evaluate covers all N targets (potentials and forces; target shards and the multi-GPU
+                                  phases keep the direct kernels); step (a) at the check targets is then served by the
+                                  same multipoles (boundary closures without derivative rows).  Needs the whole-cell near set and box sides that are integer multiples of
                                   the smallest one (cubic FMM boxes): HSMA_ERR_INVALID_ARG at plan creation otherwise. */
 } hsma_near_algorithm;
 

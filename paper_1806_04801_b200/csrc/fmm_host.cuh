@@ -1,6 +1,6 @@
 // Host orchestration of the FMM form of step (b) (fmm_kernels.cuh).  Plan time: geometry checks and
 // the translation tables.  Evaluate time: sort by leaf -> P2M -> M2M up -> M2L (all levels, one launch) -> L2L down
-// (+ sum of the M2L splits) -> leaves (L2P + P2P).  No host synchronisation, no atomics in floating point: a given
+// (+ sum of the M2L partial rows) -> leaves (L2P + P2P; with forces also their gradients).  No host synchronisation, no atomics in floating point: a given
 // (N, plan) is bit-reproducible.
 #pragma once
 #include <algorithm>
@@ -212,7 +212,7 @@ inline hsma_status points(State& S, const double* tgt, long long T, long long N,
 
 // Step (b) at all N sources, original order, into phi_out [N] (device): M2L at every level, L2L down, leaves
 // (L2P + P2P).  refine as in the direct kernels (1 Newton, 2 cubic) for the P2P part.
-inline hsma_status downward(State& S, long long N, const double half[3], int refine, double* phi_out,
+inline hsma_status downward(State& S, long long N, const double half[3], int refine, bool field, double* phi_out,
                             std::atomic<size_t>& epoch, cudaStream_t st) {
     const Geom G = make_geom(S, N, half);
     const int NC = nc(S.p);
@@ -250,8 +250,11 @@ inline hsma_status downward(State& S, long long N, const double half[3], int ref
     leaf_chunks_kernel<<<1, 1024, 0, st>>>(S.leaf_start.p, (int)n_leaves, S.chunk_start.p);
     HSMA_COUNT_LAUNCH();
     const unsigned gl = (unsigned)(N / (kLeafThreads * kLeafR) + n_leaves);
-    if (refine == 1) leaf_kernel<1><<<gl, kLeafThreads, leaf_smem, st>>>(G, S.srt.p, S.idx_a.p, S.leaf_start.p, S.chunk_start.p, (int)n_leaves, S.Lx.p, phi_out);
-    else leaf_kernel<2><<<gl, kLeafThreads, leaf_smem, st>>>(G, S.srt.p, S.idx_a.p, S.leaf_start.p, S.chunk_start.p, (int)n_leaves, S.Lx.p, phi_out);
+    // field: phi_out is [4][N]: phi, grad phi (forces)
+#define LEAF(RF, FL) leaf_kernel<RF, FL><<<gl, kLeafThreads, leaf_smem, st>>>(G, S.srt.p, S.idx_a.p, S.leaf_start.p, S.chunk_start.p, (int)n_leaves, S.Lx.p, N, phi_out)
+    if (field) { if (refine == 1) LEAF(1, true); else LEAF(2, true); }
+    else { if (refine == 1) LEAF(1, false); else LEAF(2, false); }
+#undef LEAF
     HSMA_COUNT_LAUNCH();
     return HSMA_OK;
 }

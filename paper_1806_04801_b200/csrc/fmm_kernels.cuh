@@ -467,26 +467,44 @@ __global__ void __launch_bounds__(256) l2l_kernel(const Geom G, int lev, const d
 // -n <= m <= n with the image reflection and the cell weight applied, staged too).  Thread (k, l) keeps the 8 local
 // coefficients L_k^l of the siblings in registers: per (n, m) one 128-bit read of S and one broadcast read per sibling
 // feed 4 DFMA per sibling.  The CTA's partial sums go to Lpart[row][box]; l2l_kernel adds the rows in CTA order.
-// Thread = two neighbouring outputs (k, l0) and (k, l0 + 1), l0 even: S_{n+k}^{m+l0+1} of one step is S_{n+k}^{(m+1)+l0}
-// of the next, so a sliding window needs ONE new S value per step for both outputs, and every broadcast read of a
-// sibling's moment feeds 8 DFMA.  Per step and 8 siblings: 1 + 8 shared-memory reads, 64 DFMA.
+// Thread = two neighbouring outputs (k, l0) and (k, l0 + 1), l0 even, of all 8 siblings.  The terms m and -m of a source
+// moment M_n^m = a + ib are taken together (M_n^{-m} = (-1)^m conj M_n^m):
+//     conj(M_n^m) S^{l+m} + conj(M_n^{-m}) S^{l-m} = a P + b Q,   P = S^{l+m} + (-1)^m S^{l-m},  Q = -i (S^{l+m} - (-1)^m S^{l-m})
+// P and Q do not depend on the sibling: 4 real FMA per sibling, output and (m, -m) pair instead of 8, and only the m >= 0
+// moments are staged.  S_{n+k}^{l0+1+m} of one step is S_{n+k}^{l0+(m+1)} of the next (and the same downwards), so two
+// sliding windows need two new S values per step for both outputs.  Per step and 8 siblings: 2 + 8 shared-memory
+// reads, 64 DFMA.
 template <int NV>
 __device__ __forceinline__ void m2l_inner(const double2* __restrict__ Sfull, const double2* __restrict__ Mf, int mstride,
                                           int p, int k, int l0, double2 (&a0)[NV], double2 (&a1)[NV]) {
     for (int n = 0; n <= p; ++n) {
-        const double2* Srow = Sfull + fidx(n + k, l0);
-        const double2* Mrow = Mf + fidx(n, 0);
-        double2 s0 = Srow[-n];
-#pragma unroll 2
-        for (int m = -n; m <= n; ++m) {
-            const double2 s1 = Srow[m + 1];   // (for the half pair l0 = k this runs one element past the row: unused)
+        const double2* Srow = Sfull + fidx(n + k, l0);   // Srow[j] = S_{n+k}^{l0 + j}
+        const double2* Mrow = Mf + cidx(n, 0);
+        double2 up0 = Srow[0], up1 = Srow[1];            // (for the half pair l0 = k, up1 / dn1 may leave the row: unused)
+        double2 dn0 = up0, dn1 = up1;
+#pragma unroll
+        for (int i = 0; i < NV; ++i) {                   // m = 0: M_n^0 is real
+            const double a = Mrow[i * mstride].x;
+            a0[i].x = fma(a, up0.x, a0[i].x); a0[i].y = fma(a, up0.y, a0[i].y);
+            a1[i].x = fma(a, up1.x, a1[i].x); a1[i].y = fma(a, up1.y, a1[i].y);
+        }
+        double sgn = -1.0;
+        for (int m = 1; m <= n; ++m) {
+            up0 = up1; up1 = Srow[m + 1];
+            dn1 = dn0; dn0 = Srow[-m];
+            const double2 P0 = make_double2(fma(sgn, dn0.x, up0.x), fma(sgn, dn0.y, up0.y));
+            const double2 P1 = make_double2(fma(sgn, dn1.x, up1.x), fma(sgn, dn1.y, up1.y));
+            const double2 Q0 = make_double2(fma(-sgn, dn0.y, up0.y), fma(sgn, dn0.x, -up0.x));   // -i (up - sgn dn)
+            const double2 Q1 = make_double2(fma(-sgn, dn1.y, up1.y), fma(sgn, dn1.x, -up1.x));
 #pragma unroll
             for (int i = 0; i < NV; ++i) {
                 const double2 mv = Mrow[i * mstride + m];
-                cfma(a0[i], mv, s0);
-                cfma(a1[i], mv, s1);
+                a0[i].x = fma(mv.x, P0.x, a0[i].x); a0[i].x = fma(mv.y, Q0.x, a0[i].x);
+                a0[i].y = fma(mv.x, P0.y, a0[i].y); a0[i].y = fma(mv.y, Q0.y, a0[i].y);
+                a1[i].x = fma(mv.x, P1.x, a1[i].x); a1[i].x = fma(mv.y, Q1.x, a1[i].x);
+                a1[i].y = fma(mv.x, P1.y, a1[i].y); a1[i].y = fma(mv.y, Q1.y, a1[i].y);
             }
-            s0 = s1;
+            sgn = -sgn;
         }
     }
 }
@@ -498,7 +516,7 @@ __host__ __device__ inline int m2l_pairs(int p) {   // sum_k ceil((k+1)/2)
     return s;
 }
 __host__ __device__ inline int m2l_smem_bytes(int p) {
-    return (int)sizeof(double2) * ((2 * p + 1) * (2 * p + 1) + 1 + 8 * (p + 1) * (p + 1));
+    return (int)sizeof(double2) * ((2 * p + 1) * (2 * p + 1) + 1 + 8 * nc(p));
 }
 
 // pm[t] = (k << 8) | l0 of output pair t; sfmap[t] = (cidx(N, |mu|) << 2) | op for the expanded S table entry t =
@@ -602,7 +620,7 @@ __global__ void __launch_bounds__(kM2LThreads) m2l_kernel(const Geom G, const M2
                     if (e & 2) { v.x = -v.x; }
                     Sfull[t] = v;
                 }
-                // conj of the (reflected, weighted) source moments, expanded to negative orders
+                // the (reflected, weighted) source moments of the valid siblings, m >= 0
                 for (int t = tid; t < nv * NC; t += kM2LThreads) {
                     const int sl = t / NC, cc = t - sl * NC;
                     const int fl = sib_flip[sl];
@@ -612,37 +630,34 @@ __global__ void __launch_bounds__(kM2LThreads) m2l_kernel(const Geom G, const M2
                     if (fl & 1) v = (m & 1) ? make_double2(-v.x, v.y) : make_double2(v.x, -v.y);   // x: (-1)^m conj
                     if (fl & 2) v.y = -v.y;                                                         // y: conj
                     if ((fl & 4) && ((n + m) & 1)) { v.x = -v.x; v.y = -v.y; }                      // z: (-1)^(n+m)
-                    v.x *= w; v.y *= w;
-                    double2* dst = Mfull + sl * NF;
-                    dst[fidx(n, m)] = make_double2(v.x, -v.y);
-                    if (m > 0) dst[fidx(n, -m)] = (m & 1) ? make_double2(-v.x, -v.y) : v;
+                    Mfull[t] = make_double2(v.x * w, v.y * w);
                 }
                 __syncthreads();
                 int done = 0;
                 while (done < nv) {
                     const int left = nv - done;
-                    const double2* Mf = Mfull + done * NF;
+                    const double2* Mf = Mfull + done * NC;
                     if (left >= 8) {
-                        m2l_inner<8>(Sfull, Mf, NF, p, k, l0, acc0, acc1);   // all eight siblings: slot i is sibling i
+                        m2l_inner<8>(Sfull, Mf, NC, p, k, l0, acc0, acc1);   // all eight siblings: slot i is sibling i
                         done += 8;
                     } else if (left >= 4) {
                         double2 t0[4], t1[4];
 #pragma unroll
                         for (int i = 0; i < 4; ++i) { t0[i] = make_double2(0.0, 0.0); t1[i] = make_double2(0.0, 0.0); }
-                        m2l_inner<4>(Sfull, Mf, NF, p, k, l0, t0, t1);
+                        m2l_inner<4>(Sfull, Mf, NC, p, k, l0, t0, t1);
                         m2l_add<4>(acc0, t0, slot_sib, done); m2l_add<4>(acc1, t1, slot_sib, done);
                         done += 4;
                     } else if (left >= 2) {
                         double2 t0[2], t1[2];
 #pragma unroll
                         for (int i = 0; i < 2; ++i) { t0[i] = make_double2(0.0, 0.0); t1[i] = make_double2(0.0, 0.0); }
-                        m2l_inner<2>(Sfull, Mf, NF, p, k, l0, t0, t1);
+                        m2l_inner<2>(Sfull, Mf, NC, p, k, l0, t0, t1);
                         m2l_add<2>(acc0, t0, slot_sib, done); m2l_add<2>(acc1, t1, slot_sib, done);
                         done += 2;
                     } else {
                         double2 t0[1], t1[1];
                         t0[0] = make_double2(0.0, 0.0); t1[0] = make_double2(0.0, 0.0);
-                        m2l_inner<1>(Sfull, Mf, NF, p, k, l0, t0, t1);
+                        m2l_inner<1>(Sfull, Mf, NC, p, k, l0, t0, t1);
                         m2l_add<1>(acc0, t0, slot_sib, done); m2l_add<1>(acc1, t1, slot_sib, done);
                         done += 1;
                     }
@@ -680,38 +695,62 @@ constexpr int kLeafThreads = 64;
 constexpr int kLeafTile = 128;
 constexpr int kLeafR = 4;      // rows of kLeafThreads targets per chunk (targets per thread)
 
-template <int REFINE, int R>
+// FIELD: also the gradient (forces): out[comp * N + i], comp 0 = phi, 1..3 = grad phi.  The gradient of
+// the local expansion uses d/dz R_n^m = R_{n-1}^m, (d/dx + i d/dy) conj R_n^m = conj R_{n-1}^{m-1}:
+//   dPsi/dz = sum_k [R_k^0 L_{k+1}^0 + 2 Re sum_{j>=1} conj R_k^j L_{k+1}^j]
+//   dPsi/dx + i dPsi/dy = sum_k [sum_{j>=0} conj R_k^j L_{k+1}^{j+1} - sum_{j>=1} R_k^j conj L_{k+1}^{j-1}]
+// (checked against finite differences before this was written); the P2P part uses pair_field of sum_kernels.cuh.
+template <int REFINE, int R, bool FIELD>
 __device__ __forceinline__ void leaf_round(const Geom& G, const int ic[3], const double c[3], const Src4* __restrict__ srt,
                                            const int* __restrict__ idx, const int* __restrict__ leaf_start, int t0, int t1,
-                                           Src4* tile, const double2* Ls, const double* inv, double* __restrict__ phi_out) {
+                                           Src4* tile, const double2* Ls, const double* inv, long long N, double* __restrict__ phi_out) {
+    constexpr int RG = FIELD ? R : 1;
     const int p = G.p, lev = G.levels, tid = threadIdx.x;
     const double ia = (double)(1 << lev) / G.a0;
-    const double scale = REFINE == 1 ? 0.5 : 1.0;
-    double total[R];
+    const double scale = REFINE == 1 ? 0.5 : 1.0, scale_grad = REFINE == 1 ? -0.125 : -1.0;
+    double total[R], totx[RG], toty[RG], totz[RG];
     // L2P: (1/a) Re sum conj R_n^m L_n^m, m < 0 folded in (factor 2)
 #pragma unroll 1
     for (int r = 0; r < R; ++r) {
         const Src4 t = srt[min(t0 + r * kLeafThreads + tid, t1 - 1)];
         const double x = (t.x - c[0]) * ia, y = (t.y - c[1]) * ia, z = (t.z - c[2]) * ia;
         const double r2 = fma(z, z, fma(y, y, x * x));
-        double rr = 1.0, ri = 0.0, far = 0.0;
+        double rr = 1.0, ri = 0.0, far = 0.0, gpr = 0.0, gpi = 0.0, gz = 0.0;
         for (int m = 0; m <= p; ++m) {
             if (m > 0) { const double f = 0.5 / (double)m, u = (rr * x - ri * y) * f; ri = (rr * y + ri * x) * f; rr = u; }
             double p1r = rr, p1i = ri, p2r = 0.0, p2i = 0.0;
-            double2 lc = Ls[cidx(m, m)];
-            double s = fma(rr, lc.x, ri * lc.y);
-            for (int n = m + 1; n <= p; ++n) {
-                const double f = inv[n * kInvW + m], tz = (double)(2 * n - 1) * z;
-                const double cr = (tz * p1r - r2 * p2r) * f, ci = (tz * p1i - r2 * p2i) * f;
-                lc = Ls[cidx(n, m)];
+            double s = 0.0, sz = 0.0;
+            for (int n = m; n <= p; ++n) {
+                double cr, ci;
+                if (n == m) { cr = rr; ci = ri; }
+                else {
+                    const double f = inv[n * kInvW + m], tz = (double)(2 * n - 1) * z;
+                    cr = (tz * p1r - r2 * p2r) * f; ci = (tz * p1i - r2 * p2i) * f;
+                    p2r = p1r; p2i = p1i; p1r = cr; p1i = ci;
+                }
+                const double2 lc = Ls[cidx(n, m)];
                 s = fma(cr, lc.x, s); s = fma(ci, lc.y, s);
-                p2r = p1r; p2i = p1i; p1r = cr; p1i = ci;
+                if (FIELD && n < p) {
+                    const double2 lz = Ls[cidx(n + 1, m)], lp = Ls[cidx(n + 1, m + 1)];
+                    sz = fma(cr, lz.x, sz); sz = fma(ci, lz.y, sz);
+                    gpr = fma(cr, lp.x, gpr); gpr = fma(ci, lp.y, gpr);      // conj(R) L^{m+1}
+                    gpi = fma(cr, lp.y, gpi); gpi = fma(-ci, lp.x, gpi);
+                    if (m >= 1) {                                            // - R conj(L^{m-1})
+                        const double2 lm = Ls[cidx(n + 1, m - 1)];
+                        gpr = fma(-cr, lm.x, gpr); gpr = fma(-ci, lm.y, gpr);
+                        gpi = fma(-ci, lm.x, gpi); gpi = fma(cr, lm.y, gpi);
+                    }
+                }
             }
             far += m == 0 ? s : 2.0 * s;
+            if (FIELD) gz += m == 0 ? sz : 2.0 * sz;
         }
         // (dynamic index into a register array would spill: select)
 #pragma unroll
-        for (int k = 0; k < R; ++k) if (k == r) total[k] = far * ia;
+        for (int k = 0; k < R; ++k) if (k == r) {
+            total[k] = far * ia;
+            if (FIELD) { totx[k % RG] = gpr * ia * ia; toty[k % RG] = gpi * ia * ia; totz[k % RG] = gz * ia * ia; }
+        }
     }
     Src4 me[R];
     int pos[R];
@@ -727,11 +766,12 @@ __device__ __forceinline__ void leaf_round(const Geom& G, const int ic[3], const
                 if (!image_box(G, lev, ic[0] + dx, ic[1] + dy, ic[2] + dz, ib)) continue;
                 const int s0 = leaf_start[ib.box], s1 = leaf_start[ib.box + 1];
                 if (s0 == s1) continue;
-                double tx[R], ty[R], tz[R], acc[R];
+                double tx[R], ty[R], tz[R], acc[R], gx[RG], gy[RG], gz[RG];
 #pragma unroll
                 for (int r = 0; r < R; ++r) {
                     tx[r] = flip(me[r].x - ib.sx, ib.fx); ty[r] = flip(me[r].y - ib.sy, ib.fy); tz[r] = flip(me[r].z - ib.sz, ib.fz);
                     acc[r] = 0.0;
+                    if (FIELD) { gx[r % RG] = 0.0; gy[r % RG] = 0.0; gz[r % RG] = 0.0; }
                 }
                 const bool self_here = ib.central && dx == 0 && dy == 0 && dz == 0;
                 for (int base = s0; base < s1; base += kLeafTile) {
@@ -751,8 +791,12 @@ __device__ __forceinline__ void leaf_round(const Geom& G, const int ic[3], const
 #pragma unroll
                             for (int r = 0; r < R; ++r) {
                                 const bool self = base + j == pos[r];
-                                pair<REFINE>(tx[r], ty[r], tz[r], self ? tx[r] + 1.0 : xy.x, self ? ty[r] : xy.y, self ? tz[r] : zq.x,
-                                             self ? 0.0 : zq.y, acc[r]);
+                                if (FIELD)
+                                    pair_field<REFINE, 0>(tx[r], ty[r], tz[r], self ? tx[r] + 1.0 : xy.x, self ? ty[r] : xy.y,
+                                                          self ? tz[r] : zq.x, self ? 0.0 : zq.y, acc[r], gx[r % RG], gy[r % RG], gz[r % RG]);
+                                else
+                                    pair<REFINE>(tx[r], ty[r], tz[r], self ? tx[r] + 1.0 : xy.x, self ? ty[r] : xy.y, self ? tz[r] : zq.x,
+                                                 self ? 0.0 : zq.y, acc[r]);
                             }
                         }
                     } else {
@@ -761,18 +805,32 @@ __device__ __forceinline__ void leaf_round(const Geom& G, const int ic[3], const
                             const double2 xy = *reinterpret_cast<const double2*>(&tile[j].x);
                             const double2 zq = *reinterpret_cast<const double2*>(&tile[j].z);
 #pragma unroll
-                            for (int r = 0; r < R; ++r) pair<REFINE>(tx[r], ty[r], tz[r], xy.x, xy.y, zq.x, zq.y, acc[r]);
+                            for (int r = 0; r < R; ++r) {
+                                if (FIELD) pair_field<REFINE, 0>(tx[r], ty[r], tz[r], xy.x, xy.y, zq.x, zq.y, acc[r], gx[r % RG], gy[r % RG], gz[r % RG]);
+                                else pair<REFINE>(tx[r], ty[r], tz[r], xy.x, xy.y, zq.x, zq.y, acc[r]);
+                            }
                         }
                     }
                 }
-                const double w = ib.w * scale;
+                const double w = ib.w * scale, wg = ib.w * scale_grad;
 #pragma unroll
-                for (int r = 0; r < R; ++r) total[r] = fma(w, acc[r], total[r]);
+                for (int r = 0; r < R; ++r) {
+                    total[r] = fma(w, acc[r], total[r]);
+                    if (FIELD) {   // the pair loop ran in the frame of the transformed target: a reflected axis flips back
+                        totx[r % RG] = fma(wg, flip(gx[r % RG], ib.fx), totx[r % RG]);
+                        toty[r % RG] = fma(wg, flip(gy[r % RG], ib.fy), toty[r % RG]);
+                        totz[r % RG] = fma(wg, flip(gz[r % RG], ib.fz), totz[r % RG]);
+                    }
+                }
             }
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         const int t = t0 + r * kLeafThreads + tid;
-        if (t < t1) phi_out[idx[t]] = total[r];
+        if (t < t1) {
+            const long long i = idx[t];
+            phi_out[i] = total[r];
+            if (FIELD) { phi_out[N + i] = totx[r % RG]; phi_out[2 * N + i] = toty[r % RG]; phi_out[3 * N + i] = totz[r % RG]; }
+        }
     }
 }
 
@@ -807,10 +865,11 @@ __global__ void __launch_bounds__(1024) leaf_chunks_kernel(const int* __restrict
 }
 
 // grid: an upper bound of the number of chunks (N / (kLeafThreads * kLeafR) + n_leaves); surplus CTAs return
-template <int REFINE>
+template <int REFINE, bool FIELD>
 __global__ void __launch_bounds__(kLeafThreads) leaf_kernel(const Geom G, const Src4* __restrict__ srt, const int* __restrict__ idx,
                                                             const int* __restrict__ leaf_start, const int* __restrict__ chunk_start,
-                                                            int n_leaves, const double2* __restrict__ L, double* __restrict__ phi_out) {
+                                                            int n_leaves, const double2* __restrict__ L, long long N,
+                                                            double* __restrict__ phi_out) {
     extern __shared__ __align__(16) double2 sm2[];
     __shared__ __align__(16) Src4 tile[kLeafTile];
     const int p = G.p, NC = nc(p), lev = G.levels;
@@ -835,10 +894,10 @@ __global__ void __launch_bounds__(kLeafThreads) leaf_kernel(const Geom G, const 
     __syncthreads();
     const int R = (t1 - t0 + kLeafThreads - 1) / kLeafThreads;
     switch (R) {
-        case 1: leaf_round<REFINE, 1>(G, ic, c, srt, idx, leaf_start, t0, t1, tile, Ls, inv, phi_out); break;
-        case 2: leaf_round<REFINE, 2>(G, ic, c, srt, idx, leaf_start, t0, t1, tile, Ls, inv, phi_out); break;
-        case 3: leaf_round<REFINE, 3>(G, ic, c, srt, idx, leaf_start, t0, t1, tile, Ls, inv, phi_out); break;
-        default: leaf_round<REFINE, 4>(G, ic, c, srt, idx, leaf_start, t0, t1, tile, Ls, inv, phi_out); break;
+        case 1: leaf_round<REFINE, 1, FIELD>(G, ic, c, srt, idx, leaf_start, t0, t1, tile, Ls, inv, N, phi_out); break;
+        case 2: leaf_round<REFINE, 2, FIELD>(G, ic, c, srt, idx, leaf_start, t0, t1, tile, Ls, inv, N, phi_out); break;
+        case 3: leaf_round<REFINE, 3, FIELD>(G, ic, c, srt, idx, leaf_start, t0, t1, tile, Ls, inv, N, phi_out); break;
+        default: leaf_round<REFINE, 4, FIELD>(G, ic, c, srt, idx, leaf_start, t0, t1, tile, Ls, inv, N, phi_out); break;
     }
 }
 

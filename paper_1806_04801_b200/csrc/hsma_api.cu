@@ -740,7 +740,7 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
 
     // near_algorithm = FMM: step (b) over all N targets (potentials) by the fast multipole method; its
     // upward pass (leaf sort, P2M, M2M) comes first because step (a) can use the multipoles too
-    const bool use_fmm = p->fmm.enabled && phase == kPhaseAll && n_parts == 0 && !field && t0 == 0 && t1 == N && p->pair_form == 0;
+    const bool use_fmm = p->fmm.enabled && phase == kPhaseAll && n_parts == 0 && t0 == 0 && t1 == N && p->pair_form == 0;
     if (use_fmm) {
         const hsma_status fs = fmm::upward(p->fmm, xyz, q, N, p->half, g_alloc_epoch, st);
         if (fs != HSMA_OK) return fs;
@@ -825,7 +825,7 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
         const size_t comps = field ? 4 : 1;
         bool sym = !use_fmm && !p->sphere && p->pair_form != 1 && t0 == 0 && t1 == N && sym_applies(n_tiles, C_b);
         Launch sb = choose_near(T, n_tiles_near, C_b, refine, field);
-        if (use_fmm && p->sym_phi.reserve((size_t)N) != cudaSuccess) return HSMA_ERR_ALLOC;
+        if (use_fmm && p->sym_phi.reserve((size_t)N * comps) != cudaSuccess) return HSMA_ERR_ALLOC;
         SymLaunch ss{};
         if (sym) {
             ss = choose_sym(n_tiles, refine, p->sym_col_cap, 0, 1, field);
@@ -843,7 +843,7 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
         MARK(3);
         PartLayout layout_b = sb.layout(p->part_b.p);
         if (use_fmm) {
-            const hsma_status fs = fmm::downward(p->fmm, N, p->half, refine, p->sym_phi.p, g_alloc_epoch, st);
+            const hsma_status fs = fmm::downward(p->fmm, N, p->half, refine, field, p->sym_phi.p, g_alloc_epoch, st);
             if (fs != HSMA_OK) return fs;
             layout_b = PartLayout{p->sym_phi.p, 1, 1, 1, (int)std::min<long long>(T, 2147483647LL)};
         } else if (sym) {

@@ -69,6 +69,19 @@ def test_all_cell_tables_every_potential(H, idx, N, levels, order):
     assert rel_inf(phi, r.phi) <= PHI_TOL and abs(U - r.U) <= U_TOL * abs(r.U)
 
 
+@pytest.mark.parametrize("idx,N,levels", [(5, 20012, 0), (5, 20012, 3), (3, 9001, 2), (4, 9000, 0), (2, 1000, 2)])
+def test_forces_every_component(H, idx, N, levels):
+    """Forces by the FMM (gradient of the local expansions + gradient pair sums over the near leaves):
+    every force component, potential and U against the oracle for the three cell tables."""
+    w = W.config(idx, N=N)
+    r = O.hsma(w, forces=True)
+    with H.Plan.from_workload(w, near_algorithm=H.binding.NEAR_ALG_FMM, fmm_levels=levels) as plan:
+        phi, F, U = plan.evaluate_forces(dev(w.xyz), dev(w.q), sync=True)
+        assert plan.last_pair_form == FMM
+    assert np.max(np.abs(F.cpu().numpy() - r.F)) <= 1e-10 * float(np.max(np.abs(r.F)))
+    assert rel_inf(phi.cpu().numpy(), r.phi) <= PHI_TOL and abs(float(U) - r.U) <= U_TOL * abs(r.U)
+
+
 def test_config5_recipe_at_65536_every_potential(H):
     """Config-5 recipe at N = 65,536: every potential and U, automatic level (2: 1,024 sources per leaf) and level 3."""
     w = W.config(5, N=65536)
@@ -147,7 +160,7 @@ def test_charge_magnitudes_clustered_input_determinism_and_graph(H):
 
 
 def test_where_the_fmm_applies_and_what_it_rejects(H):
-    """Forces and target shards keep the direct kernels (and agree with the FMM potentials); geometry the FMM cannot
+    """Target shards keep the direct kernels (and agree with the FMM potentials); geometry the FMM cannot
     tile with cubic boxes, the sphere-culled near set and out-of-range orders are rejected at plan creation."""
     w = W.config(5, N=9000)
     with H.Plan.from_workload(w, near_algorithm=H.binding.NEAR_ALG_FMM) as plan:
@@ -155,7 +168,7 @@ def test_where_the_fmm_applies_and_what_it_rejects(H):
         phi, U = plan.evaluate(x, q, sync=True)
         assert plan.last_pair_form == FMM
         phi_f, F, U_f = plan.evaluate_forces(x, q, sync=True)
-        assert plan.last_pair_form == 2
+        assert plan.last_pair_form == FMM
         a, _ = plan.evaluate_shard(x, q, 0, 4000, sync=True)
         assert plan.last_pair_form == 1
         assert rel_inf(phi_f.cpu().numpy(), phi.cpu().numpy()) <= 2e-11
