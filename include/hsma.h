@@ -76,8 +76,12 @@ typedef enum {
     HSMA_NEAR_WHOLE_CELLS = 0, /* every image of the cells |k_a| <= near_shell[a], generated on the fly (reading S7) */
     HSMA_NEAR_SPHERE = 1       /* only the images inside the sphere |r| <= R_aux.  Each evaluate builds
                                   the explicit image list on the device (count, scan, scatter), packs it and sums it
-                                  with the identity cell; the image count is read back, so hsma_evaluate* SYNCHRONISES
-                                  the stream once in this mode.  Boundary closure only. */
+                                  with the identity cell.  The length of the list never visits the host (buffers are
+                                  sized for the whole cell table, the kernels read the count themselves): no host
+                                  synchronisation, CUDA-graph replay as in the other modes.  A source outside the
+                                  sphere is detected on the device and surfaces as HSMA_ERR_GEOMETRY at
+                                  hsma_plan_sync.  Boundary closures only.  Ordered-pair kernels only: an image inside
+                                  the sphere need not have its partner inside, so the symmetric form does not apply. */
 } hsma_near_mode;
 
 typedef enum {
@@ -312,7 +316,7 @@ long long hsma_plan_scratch_bytes(const hsma_plan* plan);
  * plans may be driven from different host threads (the only process-wide state, the launch counter and the
  * allocation epoch that invalidates captured graphs, is atomic).  Host synchronisation: hsma_evaluate* enqueue work
  * and return, EXCEPT that the first call at a larger N than any before grows the plan's scratch (cudaFree +
- * cudaMalloc: an implicit device synchronisation), and that the sphere-culled near set reads its image count back.
+ * cudaMalloc: an implicit device synchronisation).
  */
 
 /* total number of kernels this library has launched in this process */

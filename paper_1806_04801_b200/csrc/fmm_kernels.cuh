@@ -539,7 +539,7 @@ __global__ void __launch_bounds__(kM2LThreads) m2l_kernel(const Geom G, const M2
     __shared__ int sib_box[8], sib_flip[8], slot_sib[8];
     __shared__ double sib_w[8];
     __shared__ int s_nv, s_lo, s_hi;
-    const int p = G.p, NC = nc(p), NS = nc(2 * p), NF = (p + 1) * (p + 1), NSF = (2 * p + 1) * (2 * p + 1), NP = m2l_pairs(p);
+    const int p = G.p, NC = nc(p), NS = nc(2 * p), NSF = (2 * p + 1) * (2 * p + 1), NP = m2l_pairs(p);
     double2* Sfull = sm2;
     double2* Mfull = sm2 + NSF + 1;
     const int tid = threadIdx.x;

@@ -62,7 +62,11 @@ struct Launch {
     long long Ub, U;  // units per block / in all
     int G;            // CTAs = min(resident CTAs, U)
     int rows;         // rows of the partial-sum buffer
-    PartLayout layout(const double* part) const { return PartLayout{part, U, Ub, G, kThreads * R}; }
+    PartLayout layout(const double* part, const long long* dyn = nullptr, int cells = 1) const {
+        PartLayout L{part, U, Ub, G, kThreads * R};
+        L.dyn = dyn; L.cells = cells;
+        return L;
+    }
 };
 
 template <class K>
@@ -134,6 +138,7 @@ static Launch choose_launch(long long T, long long units_per_block, int Rmax, Re
 // The packed sources of one evaluate (pack_sources_kernel) as the pair kernels need them.
 struct Packed {
     const Src4* src; long long n_src, n_tiles; const int* tile_np; const int* slot_of; const QInfo* qinfo;
+    const long long* dyn = nullptr;   // sphere-culled near set: device-resident {n_src, n_tiles} (n_src, n_tiles above are estimates)
 };
 
 template <bool UNIFORM, bool FIELD>
@@ -159,7 +164,7 @@ static void launch_near(const Launch& L, bool field, const double* tgt, int tstr
     NearArgs a;
     a.tgt = tgt; a.tstride = tstride; a.tgt_index = tgt_index; a.T = T; a.t_first = t_first;
     a.src = P.src; a.n_src = P.n_src; a.n_tiles = P.n_tiles; a.tile_np = P.tile_np; a.slot_of = P.slot_of; a.qinfo = P.qinfo;
-    a.cells = cells; a.C = C; a.units = L.U; a.self_offset = self_offset;
+    a.cells = cells; a.C = C; a.units = L.U; a.self_offset = self_offset; a.dyn = P.dyn; a.ntb = L.ntb;
     a.scale = refine == 1 ? 0.5 : 1.0; a.scale_grad = refine == 1 ? -0.125 : -1.0; a.part = part;
     // generic form always; the uniform-|q| form too when the charge statistics are available (each returns at
     // once unless QInfo.uniform selects it)
@@ -321,6 +326,7 @@ struct hsma_plan {
     DevBuf<Src4> img_src;
     DevBuf<int> img_slot_of, img_tile_np;
     QInfo* img_qinfo = nullptr;
+    long long* img_dyn = nullptr;    // device {images inside the sphere, their tiles} of the last evaluate
     Cell* cells_rhs = nullptr;   // == cells_near for the boundary closure
     double* chk = nullptr;       // [Kt,3]
     double* nrm = nullptr;       // [M,3]
@@ -375,6 +381,7 @@ static void plan_free(hsma_plan* p) {
     if (p->pcg) cudaFree(p->pcg);
     if (p->cell_order) cudaFree(p->cell_order);
     if (p->img_qinfo) cudaFree(p->img_qinfo);
+    if (p->img_dyn) cudaFree(p->img_dyn);
     p->img_counts.release(); p->img_xyz.release(); p->img_q.release(); p->img_stats.release(); p->img_src.release();
     p->img_slot_of.release(); p->img_tile_np.release();
     p->part_a.release(); p->part_b.release(); p->part_c.release(); p->red.release(); p->sym_col.release(); p->sym_phi.release();
@@ -455,6 +462,8 @@ extern "C" hsma_status hsma_plan_create_ex(const hsma_plan_desc* desc, void* cud
         for (int c = 0; c < (int)near.size(); ++c) if (!near[c].central) order.push_back(c);
         PCU(upload(&p->cell_order, order, st));
         PCU(cudaMalloc(&p->img_qinfo, sizeof(QInfo)));
+        PCU(cudaMalloc(&p->img_dyn, 2 * sizeof(long long)));
+        PCU(cudaMemsetAsync(p->img_dyn, 0, 2 * sizeof(long long), st));
     }
     if (d.near_algorithm == HSMA_NEAR_ALG_FMM) {
         bool refl[3];
@@ -704,39 +713,57 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
     int C_a = p->C_rhs, C_b = p->C_near;
     long long n_tiles_near = n_tiles;
     p->last_images = N * (long long)p->C_near;
+    const long long* dyn = nullptr;   // sphere-culled near set: device-resident source count of the pair kernels
+    long long nt_lo = n_tiles, nt_hi = n_tiles;   // bounds of the source tiles (partial-row allocation)
     if (p->sphere) {
         // paper-literal near set: explicit list of the images inside the sphere, central cell first
-        // (image i < N is source i), packed like a source array and summed with the identity cell
+        // (image i < N is source i), packed like a source array and summed with the identity cell.  The length of the
+        // list stays on the device (img_dyn): buffers are sized for the whole cell table, grids for the worst case
+        // (surplus CTAs return), the persistent pair kernels and the finish read the count themselves -- no host
+        // synchronisation, so the evaluate can be captured and replayed as a CUDA graph like the other modes.
         const long long entries = (long long)p->C_near * N, blocks = (entries + kTile - 1) / kTile;
         const double R2 = d.R_aux * d.R_aux;
-        if (p->img_counts.reserve((size_t)blocks + 1) != cudaSuccess) return HSMA_ERR_ALLOC;
+        if (entries > 2000000000LL) return HSMA_ERR_INVALID_ARG;
+        const long long nt_max = blocks;
+        if (p->img_counts.reserve((size_t)blocks + 1) != cudaSuccess || p->img_xyz.reserve(3 * (size_t)entries) != cudaSuccess ||
+            p->img_q.reserve((size_t)entries) != cudaSuccess || p->img_src.reserve((size_t)nt_max * kTile) != cudaSuccess ||
+            p->img_slot_of.reserve((size_t)entries) != cudaSuccess || p->img_tile_np.reserve((size_t)nt_max) != cudaSuccess ||
+            p->img_stats.reserve(4 * (size_t)nt_max + 2) != cudaSuccess)
+            return HSMA_ERR_ALLOC;
         image_count_kernel<<<(unsigned)blocks, kTile, 0, st>>>(xyz, q, N, p->half[0], p->half[1], p->half[2], p->cells_near,
                                                               p->cell_order, p->C_near, R2, p->img_counts.p);
         scan_counts_kernel<<<1, 1024, 0, st>>>(p->img_counts.p, blocks);
-        HSMA_COUNT_LAUNCH(); HSMA_COUNT_LAUNCH();
-        long long Ns = 0;   // the launch shapes below depend on it: the one host synchronisation of this mode
-        if (cudaMemcpyAsync(&Ns, p->img_counts.p + blocks, sizeof(long long), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
-            cudaStreamSynchronize(st) != cudaSuccess)
-            return HSMA_ERR_CUDA;
-        if (Ns < N || Ns > 2000000000LL) return HSMA_ERR_GEOMETRY;   // a source outside the sphere / index overflow
-        const long long nt_img = (Ns + kTile - 1) / kTile;
-        if (p->img_xyz.reserve(3 * (size_t)Ns) != cudaSuccess || p->img_q.reserve((size_t)Ns) != cudaSuccess ||
-            p->img_src.reserve((size_t)nt_img * kTile) != cudaSuccess || p->img_slot_of.reserve((size_t)Ns) != cudaSuccess ||
-            p->img_tile_np.reserve((size_t)nt_img) != cudaSuccess || p->img_stats.reserve(4 * (size_t)nt_img + 2) != cudaSuccess)
-            return HSMA_ERR_ALLOC;
+        image_finalize_kernel<<<1, 1, 0, st>>>(p->img_counts.p + blocks, N, p->img_dyn, p->flags);
         image_scatter_kernel<<<(unsigned)blocks, kTile, 0, st>>>(xyz, q, N, p->half[0], p->half[1], p->half[2], p->cells_near,
                                                                 p->cell_order, p->C_near, R2, p->img_counts.p, p->img_xyz.p,
                                                                 p->img_q.p);
-        pack_sources_kernel<<<(unsigned)nt_img, kTile, 0, st>>>(p->img_xyz.p, p->img_q.p, Ns, 0.0, 0.0, 0.0, p->img_src.p,
-                                                               p->img_slot_of.p, p->img_tile_np.p, p->img_stats.p);
-        charge_stats_kernel<<<1, 1024, 0, st>>>(p->img_stats.p, nt_img, 0, p->img_stats.p + 4 * nt_img, p->img_qinfo, p->flags);
-        HSMA_COUNT_LAUNCH(); HSMA_COUNT_LAUNCH(); HSMA_COUNT_LAUNCH();
-        P = Packed{p->img_src.p, Ns, nt_img, p->img_tile_np.p, p->img_slot_of.p, p->img_qinfo};
+        pack_sources_kernel<<<(unsigned)nt_max, kTile, 0, st>>>(p->img_xyz.p, p->img_q.p, entries, 0.0, 0.0, 0.0, p->img_src.p,
+                                                               p->img_slot_of.p, p->img_tile_np.p, p->img_stats.p, p->img_dyn);
+        charge_stats_kernel<<<1, 1024, 0, st>>>(p->img_stats.p, nt_max, 0, p->img_stats.p + 4 * nt_max, p->img_qinfo, p->flags,
+                                                p->img_dyn);
+        for (int i = 0; i < 6; ++i) HSMA_COUNT_LAUNCH();
+        // host-side ESTIMATE of the list (launch shapes only): the sphere's share of the cell block
+        const double vol = 4.18879020478639098 * d.R_aux * d.R_aux * d.R_aux / (d.L[0] * d.L[1] * d.L[2]);
+        const long long Ns_est = std::max<long long>(N, std::min<long long>(entries, (long long)(vol * (double)N)));
+        const long long nt_img = (Ns_est + kTile - 1) / kTile;
+        P = Packed{p->img_src.p, Ns_est, nt_img, p->img_tile_np.p, p->img_slot_of.p, p->img_qinfo, p->img_dyn};
         cells_a = cells_b = p->cell_identity;
         C_a = C_b = 1;
         n_tiles_near = nt_img;
-        p->last_images = Ns;
+        p->last_images = Ns_est;
+        dyn = p->img_dyn;
+        nt_lo = n_tiles; nt_hi = nt_max;
     }
+    // rows of a partial-sum buffer when the source tiles are only known to lie in [nt_lo, nt_hi] (sphere-culled set)
+    auto rows_for = [&](const Launch& L, int C) {
+        int r = L.rows;
+        if (dyn)
+            for (long long nt : {nt_lo, nt_hi, n_tiles_near}) {
+                const long long Ub = nt * C, U = (long long)L.ntb * Ub;
+                r = std::max(r, part_rows(U, Ub, L.G) + 1);
+            }
+        return r;
+    };
 
     // near_algorithm = FMM: step (b) over all N targets (potentials) by the fast multipole method; its
     // upward pass (leaf sort, P2M, M2M) comes first because step (a) can use the multipoles too
@@ -756,14 +783,14 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
         const long long Tc = c1 - c0;
         const bool fa = p->need_grad;   // derivative rows need grad Phi_in at the check targets: the FIELD form of (a)
         const Launch s = choose_near(Tc, n_tiles_near, C_a, 2, fa);
-        if (p->part_a.reserve((size_t)s.rows * Tc * (fa ? 4 : 1)) != cudaSuccess) return HSMA_ERR_ALLOC;
+        if (p->part_a.reserve((size_t)rows_for(s, C_a) * Tc * (fa ? 4 : 1)) != cudaSuccess) return HSMA_ERR_ALLOC;
         MARK(1);
         launch_near(s, fa, p->chk, 3, nullptr, Tc, c0, P, cells_a, C_a, -1, 2, p->part_a.p, st);  // (a) always cubic: it feeds the fit
         MARK(2);
         if (fa)
-            finish_field_kernel<<<(unsigned)((Tc + 255) / 256), 256, 0, st>>>(s.layout(p->part_a.p), PartLayout{nullptr, 1, 1, 1, 1}, Tc, nullptr, nullptr, 0, p->pc + c0, p->pcg + 3 * c0, nullptr);
+            finish_field_kernel<<<(unsigned)((Tc + 255) / 256), 256, 0, st>>>(s.layout(p->part_a.p, dyn, C_a), PartLayout{nullptr, 1, 1, 1, 1}, Tc, nullptr, nullptr, 0, p->pc + c0, p->pcg + 3 * c0, nullptr);
         else
-            finish_phi_kernel<<<(unsigned)((Tc + 255) / 256), 256, 0, st>>>(s.layout(p->part_a.p), PartLayout{nullptr, 1, 1, 1, 1}, Tc, nullptr, nullptr, 0, p->pc + c0, nullptr);
+            finish_phi_kernel<<<(unsigned)((Tc + 255) / 256), 256, 0, st>>>(s.layout(p->part_a.p, dyn, C_a), PartLayout{nullptr, 1, 1, 1, 1}, Tc, nullptr, nullptr, 0, p->pc + c0, nullptr);
         HSMA_COUNT_LAUNCH();
     } else {
         MARK(1); MARK(2);
@@ -836,12 +863,12 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
                 sym = false;
             }
         }
-        if (!sym && !use_fmm && p->part_b.reserve((size_t)sb.rows * T * comps) != cudaSuccess) return HSMA_ERR_ALLOC;
+        if (!sym && !use_fmm && p->part_b.reserve((size_t)rows_for(sb, C_b) * T * comps) != cudaSuccess) return HSMA_ERR_ALLOC;
         p->last_pair_form = use_fmm ? 3 : (sym ? 2 : 1);
         const Launch sc = choose_node(T, p->node_tiles, field);
         if (p->part_c.reserve((size_t)sc.rows * T * comps) != cudaSuccess) return HSMA_ERR_ALLOC;
         MARK(3);
-        PartLayout layout_b = sb.layout(p->part_b.p);
+        PartLayout layout_b = sb.layout(p->part_b.p, dyn, C_b);
         if (use_fmm) {
             const hsma_status fs = fmm::downward(p->fmm, N, p->half, refine, field, p->sym_phi.p, g_alloc_epoch, st);
             if (fs != HSMA_OK) return fs;
@@ -893,7 +920,7 @@ static hsma_status evaluate_graphed(hsma_plan* p, const double* xyz, const doubl
                                     long long t1, double* phi_out, double* energy_out, double* force_out) {
     if (!p) return HSMA_ERR_INVALID_ARG;
     cudaStream_t st = p->stream;
-    if (st == nullptr || p->timing || p->sphere) return evaluate_impl(p, xyz, q, N, t0, t1, phi_out, energy_out, force_out);
+    if (st == nullptr || p->timing) return evaluate_impl(p, xyz, q, N, t0, t1, phi_out, energy_out, force_out);
     hsma_plan::GraphKey key;
     key.xyz = xyz; key.q = q; key.phi = phi_out; key.U = energy_out; key.F = force_out; key.N = N; key.t0 = t0; key.t1 = t1;
     if (p->gexec && key == p->gkey && p->gepoch == g_alloc_epoch) {
@@ -1011,6 +1038,10 @@ extern "C" hsma_status hsma_plan_sync(hsma_plan* plan) {
         cudaMemsetAsync(plan->flags + 1, 0, sizeof(int), plan->stream);
         if (s == HSMA_OK) s = HSMA_ERR_NOT_NEUTRAL;
     }
+    if (hf[2]) {   // sphere-culled near set: a source outside the auxiliary sphere (found on the device)
+        cudaMemsetAsync(plan->flags + 2, 0, sizeof(int), plan->stream);
+        if (s == HSMA_OK) s = HSMA_ERR_GEOMETRY;
+    }
     return s;
 }
 
@@ -1070,6 +1101,12 @@ extern "C" const char* hsma_status_string(int s) {
 
 extern "C" hsma_status hsma_plan_info(hsma_plan* p, long long* w) {
     if (!p || !w) return HSMA_ERR_INVALID_ARG;
+    if (p->sphere && p->img_dyn) {   // the image count lives on the device: fetch it for the caller (synchronises)
+        long long h[2] = {0, 0};
+        if (cudaMemcpyAsync(h, p->img_dyn, sizeof(h), cudaMemcpyDeviceToHost, p->stream) == cudaSuccess &&
+            cudaStreamSynchronize(p->stream) == cudaSuccess && h[0] > 0)
+            p->last_images = h[0];
+    }
     w[0] = p->rows; w[1] = p->ncol; w[2] = p->Kt; w[3] = p->C_near; w[4] = p->C_rhs; w[5] = p->d.M; w[6] = p->d.p;
     w[7] = p->last_launches; w[8] = p->last_images; w[9] = p->n_node_records; w[10] = p->need_grad ? 1 : 0; w[11] = p->greplays;
     return HSMA_OK;

@@ -36,7 +36,18 @@ struct PartLayout {      // how finish_phi_kernel finds the partial rows of one 
     long long U, Ub;     // units in all / per target block
     int G;               // CTAs of the launch
     int block_targets;   // targets per block (kThreads * R)
+    // sphere-culled near set: the source count lives on the device (dyn[1] = source tiles), Ub = dyn[1] * cells
+    const long long* dyn = nullptr;
+    int cells = 1;
 };
+// units per block / in all of a layout whose source count is device-resident
+__device__ __forceinline__ void layout_units(const PartLayout& L, long long T, long long& U, long long& Ub) {
+    U = L.U; Ub = L.Ub;
+    if (L.dyn) {
+        Ub = L.dyn[1] * L.cells;
+        U = ((T + L.block_targets - 1) / L.block_targets) * Ub;
+    }
+}
 
 struct QInfo { double qmag; int uniform; int pad; };  // all |q| equal to qmag (charge_stats_kernel)
 
@@ -55,6 +66,10 @@ struct NearArgs {
     const Cell* cells;   // [C]
     int C;
     long long units;     // U = ntb * n_tiles * C
+    // sphere-culled near set: the image list is built on the device and its length never visits the host.  dyn[0] =
+    // sources, dyn[1] = source tiles replace n_src / n_tiles, and units = ntb * dyn[1] * C (null: the values above)
+    const long long* dyn;
+    long long ntb;
     long long self_offset;  // >= 0: target t is source (self_offset + t); its bare term is skipped
     double scale;        // applied to the cell weights (0.5 for the Newton form, see below)
     double scale_grad;   // FIELD: weight of the gradient sums (-1/8 Newton, -1 cubic)
@@ -158,9 +173,11 @@ __global__ void __launch_bounds__(kThreads, near_min_ctas(FIELD ? 2 * R : R)) ne
     if ((a.qinfo != nullptr && a.qinfo->uniform != 0) != UNIFORM) return;
     const int tid = threadIdx.x;
     const int G = gridDim.x, k = blockIdx.x;
-    const long long u0 = unit_start(k, a.units, G), u1 = unit_start(k + 1, a.units, G);
-    if (u1 <= u0) return;  // (never: the host launches G <= U CTAs)
-    const long long Ub = a.n_tiles * a.C;
+    const long long a_n_src = a.dyn ? a.dyn[0] : a.n_src, a_n_tiles = a.dyn ? a.dyn[1] : a.n_tiles;
+    const long long a_units = a.dyn ? a.ntb * a_n_tiles * a.C : a.units;
+    const long long u0 = unit_start(k, a_units, G), u1 = unit_start(k + 1, a_units, G);
+    if (u1 <= u0) return;  // (G <= U, except with a device-resident source count smaller than the host's estimate)
+    const long long Ub = a_n_tiles * a.C;
     const long long V0 = u0 / a.C, V1 = (u1 - 1) / a.C;  // visits v = b * n_tiles + t of this CTA
 
     for (int c = tid; c < a.C; c += kThreads) cells[c] = a.cells[c];
@@ -171,7 +188,7 @@ __global__ void __launch_bounds__(kThreads, near_min_ctas(FIELD ? 2 * R : R)) ne
     __syncthreads();
     if (tid == 0) {
         mbar_expect_tx(&full[0], kTile * sizeof(Src4));
-        bulk_g2s(tile[0], a.src + (V0 % a.n_tiles) * kTile, kTile * sizeof(Src4), &full[0]);
+        bulk_g2s(tile[0], a.src + (V0 % a_n_tiles) * kTile, kTile * sizeof(Src4), &full[0]);
     }
     const double qmag = UNIFORM ? a.qinfo->qmag : 1.0;
 
@@ -180,13 +197,13 @@ __global__ void __launch_bounds__(kThreads, near_min_ctas(FIELD ? 2 * R : R)) ne
     double totx[RG], toty[RG], totz[RG];
     // visits are walked with 32-bit state: block b, tile tl inside the block
     const int nvis = (int)(V1 - V0) + 1;
-    const int nt = (int)a.n_tiles;
-    int b = (int)(V0 / a.n_tiles), tl = (int)(V0 - (long long)b * a.n_tiles);
+    const int nt = (int)a_n_tiles;
+    int b = (int)(V0 / a_n_tiles), tl = (int)(V0 - (long long)b * a_n_tiles);
     const int c_first = (int)(u0 - V0 * a.C), c_last = (int)(u1 - 1 - V1 * a.C) + 1;
     bool fresh = true;  // targets of block b not loaded yet
     // partial sums of block b go to row (k - first CTA that works on b)
     auto store_block = [&](int blk) {
-        const int row = k - cta_of_unit(blk * Ub, a.units, G);
+        const int row = k - cta_of_unit(blk * Ub, a_units, G);
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const long long t = (long long)blk * (kThreads * R) + r * kThreads + tid;
@@ -223,7 +240,7 @@ __global__ void __launch_bounds__(kThreads, near_min_ctas(FIELD ? 2 * R : R)) ne
             }
         }
         const int np = a.tile_np[tl];
-        const int nv = (int)min((long long)kTile, a.n_src - (long long)tl * kTile);
+        const int nv = (int)min((long long)kTile, a_n_src - (long long)tl * kTile);
         mbar_wait(&full[st], (it >> 1) & 1);
         const Src4* __restrict__ s = tile[st];
         // self: target t is source self_offset + t (same tile after the in-tile sort).  Block-uniform test
@@ -916,7 +933,9 @@ __global__ void __launch_bounds__(kThreads, near_min_ctas(FIELD ? 2 * R : R)) no
 __global__ void __launch_bounds__(kTile) pack_sources_kernel(const double* __restrict__ xyz, const double* __restrict__ q,
                                                            long long N, double hx, double hy, double hz,
                                                            Src4* __restrict__ out, int* __restrict__ slot_of,
-                                                           int* __restrict__ tile_np, double* __restrict__ stats /* [gridDim.x][4] */) {
+                                                           int* __restrict__ tile_np, double* __restrict__ stats /* [gridDim.x][4] */,
+                                                           const long long* __restrict__ dynN = nullptr /* device-resident N */) {
+    if (dynN) { N = dynN[0]; if ((long long)blockIdx.x * kTile >= N) return; }
     __shared__ int wpos[kTile / 32], wneg[kTile / 32];
     __shared__ double sh[4][kTile / 32];
     const int tid = threadIdx.x, w = tid >> 5, l = tid & 31;
@@ -1019,6 +1038,15 @@ __global__ void __launch_bounds__(1024) scan_counts_kernel(long long* __restrict
     }
     if (threadIdx.x == 0) counts[n] = carry;
 }
+// dyn[0] = images inside the sphere, dyn[1] = their tiles; flags[2] = 1 if a source itself lies outside the sphere
+// (fewer images than sources) or the list would overflow the 32-bit packed indices
+__global__ void image_finalize_kernel(const long long* __restrict__ counts_total, long long N, long long* __restrict__ dyn,
+                                      int* __restrict__ flags) {
+    const long long Ns = counts_total[0];
+    dyn[0] = Ns;
+    dyn[1] = (Ns + kTile - 1) / kTile;
+    if (Ns < N || Ns > 2000000000LL) flags[2] = 1;
+}
 __global__ void __launch_bounds__(kTile) image_scatter_kernel(const double* __restrict__ xyz, const double* __restrict__ q,
                                                             long long N, double hx, double hy, double hz,
                                                             const Cell* __restrict__ cells, const int* __restrict__ order,
@@ -1044,7 +1072,9 @@ __global__ void __launch_bounds__(kTile) image_scatter_kernel(const double* __re
 // Single block: sum q, sum |q| -> scal[0..1]; neutrality flag (reading S17); QInfo (all |q| equal, bit for bit).
 __global__ void __launch_bounds__(1024) charge_stats_kernel(const double* __restrict__ stats, long long nblocks,
                                                             int need_neutral, double* __restrict__ scal,
-                                                            QInfo* __restrict__ qi, int* __restrict__ flags) {
+                                                            QInfo* __restrict__ qi, int* __restrict__ flags,
+                                                            const long long* __restrict__ dyn = nullptr /* dyn[1] = blocks */) {
+    if (dyn) nblocks = dyn[1];
     __shared__ double sh[4][32];
     double a = 0.0, b = 0.0, mn = 1e300, mx = 0.0;
     for (long long i = threadIdx.x; i < nblocks; i += blockDim.x) {
@@ -1073,7 +1103,9 @@ __global__ void __launch_bounds__(1024) charge_stats_kernel(const double* __rest
 __device__ __forceinline__ double sum_part_rows(const PartLayout& L, long long t, long long T) {
     if (!L.part) return 0.0;
     const long long b = t / L.block_targets;
-    const int first = cta_of_unit(b * L.Ub, L.U, L.G), last = cta_of_unit((b + 1) * L.Ub - 1, L.U, L.G);
+    long long U, Ub;
+    layout_units(L, T, U, Ub);
+    const int first = cta_of_unit(b * Ub, U, L.G), last = cta_of_unit((b + 1) * Ub - 1, U, L.G);
     double s = 0.0;
     for (int k = 0; k <= last - first; ++k) s += L.part[(long long)k * T + t];
     return s;
@@ -1082,7 +1114,9 @@ __device__ __forceinline__ double sum_part_rows(const PartLayout& L, long long t
 __device__ __forceinline__ void sum_part_rows4(const PartLayout& L, long long t, long long T, double out[4]) {
     if (!L.part) return;
     const long long b = t / L.block_targets;
-    const int first = cta_of_unit(b * L.Ub, L.U, L.G), last = cta_of_unit((b + 1) * L.Ub - 1, L.U, L.G);
+    long long U, Ub;
+    layout_units(L, T, U, Ub);
+    const int first = cta_of_unit(b * Ub, U, L.G), last = cta_of_unit((b + 1) * Ub - 1, U, L.G);
     for (int k = 0; k <= last - first; ++k)
 #pragma unroll
         for (int c = 0; c < 4; ++c) out[c] += L.part[((long long)k * 4 + c) * T + t];

@@ -106,3 +106,37 @@ def test_sphere_mode_rejects_a_sphere_beyond_the_cell_block(H):
     with pytest.raises(H.HsmaError) as e:
         H.Plan(kind=0, L=(1, 1, 1), near_shell=(1, 1, 1), R_aux=1.6, p=8, M=400, K=200, near_mode=W.NEAR_SPHERE)
     assert e.value.status == H.HSMA_ERR_GEOMETRY
+
+
+def test_sphere_mode_keeps_the_image_count_on_the_device_and_replays_as_a_graph(H):
+    """The sphere-culled near set no longer reads its image count back (the count stays in device memory and the
+    kernels size themselves from it), so the evaluate is captured on the second identical call and replayed like the
+    other modes; replays are bit-identical to the plain call, follow new data behind the same pointers (a different
+    image count!), and meet the oracle."""
+    import torch
+    w = W.paper_timing(4096)
+    r = O.hsma(w)
+    xyz2 = np.mod(np.asarray(w.xyz) + 0.013, 1.0)            # shifted lattice: other images fall inside the sphere
+    r2 = O.hsma(w.with_(xyz=xyz2))
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        with H.Plan.from_workload(w) as plan:
+            x, q = dev(w.xyz), dev(w.q)
+            phi = torch.empty(w.N, dtype=torch.float64, device="cuda")
+            U = torch.empty(1, dtype=torch.float64, device="cuda")
+            outs = []
+            for _ in range(4):
+                H.hsma_evaluate(plan.handle, x, q, phi, U)
+                plan.sync()
+                outs.append((phi.clone(), float(U)))
+            assert H.binding.hsma_plan_info(plan.handle)["graph_replays"] >= 2
+            n1 = plan.near_images_last_evaluate()
+            x.copy_(dev(xyz2))
+            H.hsma_evaluate(plan.handle, x, q, phi, U)      # replay on new data
+            plan.sync()
+            n2 = plan.near_images_last_evaluate()
+            phi2, U2 = phi.cpu().numpy(), float(U)
+    assert all(torch.equal(outs[0][0], a) and outs[0][1] == u for a, u in outs[1:])
+    assert rel_inf(outs[0][0].cpu().numpy(), r.phi) <= PHI_TOL and abs(outs[0][1] - r.U) <= U_TOL_FD3 * abs(r.U)
+    assert rel_inf(phi2, r2.phi) <= PHI_TOL and abs(U2 - r2.U) <= U_TOL_FD3 * abs(r2.U)
+    assert n1 == r.pairs["b"] // w.N and n2 == r2.pairs["b"] // w.N
