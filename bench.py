@@ -458,6 +458,7 @@ def run_b200(args, w) -> dict:
                       "l2": "256 MiB flush written between iterations (outside the per-step events of ms_per_step)"},
            "pair_evaluations_per_s": ((pc_all["a"] + pc_all["c"] + sym_evaluations(N, info["near_cells"])) / (ms * 1e-3)
                                       if plan.last_pair_form == 2 else value),
+           "plan_scratch_bytes": plan.scratch_bytes,
            "energy": U_val, "stage_ms": stage_ms, "e2e": e2e, "gpu_launches": int(launches),
            "launches_per_step": plan.launches_last_evaluate(),
            "graph_replays": H.binding.hsma_plan_info(plan.handle)["graph_replays"], "clocks": clocks, "roofline": roofline}

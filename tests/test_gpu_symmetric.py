@@ -364,3 +364,26 @@ def test_waves_of_the_symmetric_form(H, idx, N):
             assert abs(u - r.U) <= U_TOL * abs(r.U)
         assert np.max(np.abs(F.cpu().numpy() - r.F)) <= 1e-10 * fscale
         assert np.max(np.abs((F - F0).cpu().numpy())) <= 1e-12 * fscale
+
+
+def test_scratch_stays_linear_in_N_at_one_million(H):
+    """N = 2^20 (config-5 recipe), potentials and forces in the symmetric form: the column scratch of a single launch
+    would be 2.1 GB (8.6 GB with forces); walked in waves the whole per-evaluate scratch of the plan stays below
+    0.5 GB, and a slice of potentials and forces straddling a block boundary meets the oracle at the bars."""
+    w = W.config(5, N=1 << 20)
+    sl = slice(524288 - 32, 524288 + 32)
+    r = O.hsma(w, targets_slice=sl, forces=True)
+    with H.Plan.from_workload(w) as plan:
+        xyz, q = dev(w.xyz), dev(w.q)
+        phi, U = plan.evaluate(xyz, q, sync=True)
+        assert plan.last_pair_form == SYMMETRIC
+        phi_f, F, U_f = plan.evaluate_forces(xyz, q, sync=True)
+        assert plan.last_pair_form == SYMMETRIC
+        assert plan.scratch_bytes < 500e6
+    phi, phi_f, F = phi.cpu().numpy(), phi_f.cpu().numpy(), F.cpu().numpy()
+    scale = float(np.max(np.abs(phi)))
+    assert np.max(np.abs(phi[sl] - r.phi)) <= PHI_TOL * scale and np.max(np.abs(phi_f[sl] - r.phi)) <= PHI_TOL * scale
+    assert np.max(np.abs(F[sl] - r.F)) <= 1e-10 * float(np.max(np.abs(F)))
+    assert abs(float(U) - float(U_f)) <= U_TOL * abs(float(U))
+    Uself = 0.5 * float(np.sum(np.asarray(w.q, dtype=np.longdouble) * phi.astype(np.longdouble)))
+    assert abs(float(U) - Uself) <= U_TOL * abs(Uself)
