@@ -41,17 +41,18 @@ struct State {
     Buf<int> key_a, key_b, idx_a, idx_b, leaf_start, chunk_start;
     Buf<long long> counts;
     Buf<Src4> srt;
+    Buf<double> slab;             // leaf kernel: one partial row per slab of neighbour boxes
     Buf<double2> Mx, Lx, Lpart;   // multipole / local expansions of all levels, M2L partial sums
     double* phi = nullptr;     // not owned: the plan's sym_phi buffer
     void release() {
         for (void* q : {(void*)w_lut, (void*)Rsh, (void*)Stab, (void*)nm, (void*)pm, (void*)sfmap, (void*)off_list, (void*)off_wprefix}) if (q) cudaFree(q);
         w_lut = nullptr; Rsh = Stab = nullptr; nm = pm = sfmap = off_list = off_wprefix = nullptr;
         key_a.release(); key_b.release(); idx_a.release(); idx_b.release(); leaf_start.release(); chunk_start.release(); counts.release();
-        srt.release(); Mx.release(); Lx.release(); Lpart.release();
+        srt.release(); Mx.release(); Lx.release(); Lpart.release(); slab.release();
     }
     size_t scratch_bytes() const {
         return (key_a.cap + key_b.cap + idx_a.cap + idx_b.cap + leaf_start.cap + chunk_start.cap) * sizeof(int) + counts.cap * sizeof(long long) +
-               srt.cap * sizeof(Src4) + (Mx.cap + Lx.cap + Lpart.cap) * sizeof(double2);
+               srt.cap * sizeof(Src4) + (Mx.cap + Lx.cap + Lpart.cap) * sizeof(double2) + slab.cap * sizeof(double);
     }
 };
 
@@ -251,10 +252,15 @@ inline hsma_status downward(State& S, long long N, const double half[3], int ref
     HSMA_COUNT_LAUNCH();
     const unsigned gl = (unsigned)(N / (kLeafThreads * kLeafR) + n_leaves);
     // field: phi_out is [4][N]: phi, grad phi (forces)
-#define LEAF(RF, FL) leaf_kernel<RF, FL><<<gl, kLeafThreads, leaf_smem, st>>>(G, S.srt.p, S.idx_a.p, S.leaf_start.p, S.chunk_start.p, (int)n_leaves, S.Lx.p, N, phi_out)
+    const long long comps_n = (field ? 4 : 1) * N;
+    if (S.slab.reserve((size_t)(2 * kWs + 1) * comps_n, epoch) != cudaSuccess) return HSMA_ERR_ALLOC;
+    const dim3 gl3(gl, 2 * kWs + 1);
+#define LEAF(RF, FL) leaf_kernel<RF, FL><<<gl3, kLeafThreads, leaf_smem, st>>>(G, S.srt.p, S.idx_a.p, S.leaf_start.p, S.chunk_start.p, (int)n_leaves, S.Lx.p, N, S.slab.p)
     if (field) { if (refine == 1) LEAF(1, true); else LEAF(2, true); }
     else { if (refine == 1) LEAF(1, false); else LEAF(2, false); }
 #undef LEAF
+    HSMA_COUNT_LAUNCH();
+    leaf_sum_kernel<<<(unsigned)((comps_n + 255) / 256), 256, 0, st>>>(S.slab.p, comps_n, phi_out);
     HSMA_COUNT_LAUNCH();
     return HSMA_OK;
 }

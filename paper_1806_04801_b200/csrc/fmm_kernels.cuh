@@ -703,15 +703,18 @@ constexpr int kLeafR = 4;      // rows of kLeafThreads targets per chunk (target
 template <int REFINE, int R, bool FIELD>
 __device__ __forceinline__ void leaf_round(const Geom& G, const int ic[3], const double c[3], const Src4* __restrict__ srt,
                                            const int* __restrict__ idx, const int* __restrict__ leaf_start, int t0, int t1,
-                                           Src4* tile, const double2* Ls, const double* inv, long long N, double* __restrict__ phi_out) {
+                                           Src4* tile, const double2* Ls, const double* inv, long long N, int dx_slab,
+                                           double* __restrict__ phi_out /* this slab's [comps][N] */) {
     constexpr int RG = FIELD ? R : 1;
     const int p = G.p, lev = G.levels, tid = threadIdx.x;
     const double ia = (double)(1 << lev) / G.a0;
     const double scale = REFINE == 1 ? 0.5 : 1.0, scale_grad = REFINE == 1 ? -0.125 : -1.0;
     double total[R], totx[RG], toty[RG], totz[RG];
-    // L2P: (1/a) Re sum conj R_n^m L_n^m, m < 0 folded in (factor 2)
+#pragma unroll
+    for (int r = 0; r < R; ++r) { total[r] = 0.0; if (FIELD) { totx[r % RG] = 0.0; toty[r % RG] = 0.0; totz[r % RG] = 0.0; } }
+    // L2P: (1/a) Re sum conj R_n^m L_n^m, m < 0 folded in (factor 2) -- by the slab dx = 0 only
 #pragma unroll 1
-    for (int r = 0; r < R; ++r) {
+    for (int r = 0; r < (dx_slab == 0 ? R : 0); ++r) {
         const Src4 t = srt[min(t0 + r * kLeafThreads + tid, t1 - 1)];
         const double x = (t.x - c[0]) * ia, y = (t.y - c[1]) * ia, z = (t.z - c[2]) * ia;
         const double r2 = fma(z, z, fma(y, y, x * x));
@@ -759,7 +762,8 @@ __device__ __forceinline__ void leaf_round(const Geom& G, const int ic[3], const
         pos[r] = min(t0 + r * kLeafThreads + tid, t1 - 1);   // slots past the end repeat the last target and do not store
         me[r] = srt[pos[r]];
     }
-    for (int dx = -kWs; dx <= kWs; ++dx)
+    {
+        const int dx = dx_slab;
         for (int dy = -kWs; dy <= kWs; ++dy)
             for (int dz = -kWs; dz <= kWs; ++dz) {
                 ImageBox ib;
@@ -823,6 +827,7 @@ __device__ __forceinline__ void leaf_round(const Geom& G, const int ic[3], const
                     }
                 }
             }
+    }
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         const int t = t0 + r * kLeafThreads + tid;
@@ -869,7 +874,7 @@ template <int REFINE, bool FIELD>
 __global__ void __launch_bounds__(kLeafThreads) leaf_kernel(const Geom G, const Src4* __restrict__ srt, const int* __restrict__ idx,
                                                             const int* __restrict__ leaf_start, const int* __restrict__ chunk_start,
                                                             int n_leaves, const double2* __restrict__ L, long long N,
-                                                            double* __restrict__ phi_out) {
+                                                            double* __restrict__ slab_out /* [2 kWs + 1][comps][N] */) {
     extern __shared__ __align__(16) double2 sm2[];
     __shared__ __align__(16) Src4 tile[kLeafTile];
     const int p = G.p, NC = nc(p), lev = G.levels;
@@ -892,13 +897,27 @@ __global__ void __launch_bounds__(kLeafThreads) leaf_kernel(const Geom G, const 
     double c[3]; int ic[3];
     box_centre(G, lev, leaf, c, ic);
     __syncthreads();
+    // blockIdx.y = the slab dx of the 5 x 5 x 5 neighbour boxes this CTA sums (five times more, five times shorter CTAs:
+    // the tail of the launch shrinks accordingly); each slab writes its own partial row, leaf_sum_kernel adds them in order
+    const int dx_slab = (int)blockIdx.y - kWs;
+    double* phi_out = slab_out + (long long)blockIdx.y * (FIELD ? 4 : 1) * N;
     const int R = (t1 - t0 + kLeafThreads - 1) / kLeafThreads;
     switch (R) {
-        case 1: leaf_round<REFINE, 1, FIELD>(G, ic, c, srt, idx, leaf_start, t0, t1, tile, Ls, inv, N, phi_out); break;
-        case 2: leaf_round<REFINE, 2, FIELD>(G, ic, c, srt, idx, leaf_start, t0, t1, tile, Ls, inv, N, phi_out); break;
-        case 3: leaf_round<REFINE, 3, FIELD>(G, ic, c, srt, idx, leaf_start, t0, t1, tile, Ls, inv, N, phi_out); break;
-        default: leaf_round<REFINE, 4, FIELD>(G, ic, c, srt, idx, leaf_start, t0, t1, tile, Ls, inv, N, phi_out); break;
+        case 1: leaf_round<REFINE, 1, FIELD>(G, ic, c, srt, idx, leaf_start, t0, t1, tile, Ls, inv, N, dx_slab, phi_out); break;
+        case 2: leaf_round<REFINE, 2, FIELD>(G, ic, c, srt, idx, leaf_start, t0, t1, tile, Ls, inv, N, dx_slab, phi_out); break;
+        case 3: leaf_round<REFINE, 3, FIELD>(G, ic, c, srt, idx, leaf_start, t0, t1, tile, Ls, inv, N, dx_slab, phi_out); break;
+        default: leaf_round<REFINE, 4, FIELD>(G, ic, c, srt, idx, leaf_start, t0, t1, tile, Ls, inv, N, dx_slab, phi_out); break;
     }
+}
+
+// out[c][i] = sum over the slabs, in slab order
+__global__ void leaf_sum_kernel(const double* __restrict__ slab, long long n /* comps * N */, double* __restrict__ out) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    double v = 0.0;
+#pragma unroll
+    for (int sl = 0; sl < 2 * kWs + 1; ++sl) v += slab[(long long)sl * n + i];
+    out[i] = v;
 }
 
 // ---- step (a) from the same hierarchy: the near sum at arbitrary points (the check targets) --------------------------------

@@ -170,3 +170,62 @@ def test_symmetric_and_part_forms_random_sizes(H, case):
     assert float((F - F1).abs().max()) <= tol * fs
     assert float((ps - phi1).abs().max()) <= tol * sc and float((Fs - F1).abs().max()) <= tol * fs
     assert abs(float(U) - float(U1)) <= 1e-11 * abs(float(U1)) and abs(float(Us) - float(U1)) <= 1e-11 * abs(float(U1))
+
+
+@pytest.mark.parametrize("case", range(12))
+def test_fmm_random_configurations(H, case):
+    """near_algorithm = FMM on random sizes, box shapes the FMM can tile (cubic, 2:1:1, 1:1:0.5, 2x2x1
+    boxes per cell), cell tables (periodic; Dirichlet, Neumann and dielectric mirrors; grounded slab), shells, leaf
+    levels, charges of any magnitude and box scales far from 1: potentials, forces and U against the oracle at the bars."""
+    rng = np.random.default_rng(9100 + case)
+    N = 2 * int(rng.integers(50, 9000))
+    p = int(rng.integers(5, 12))
+    M = int(rng.integers(400, 2500))
+    K = int(2 * p * p + rng.integers(20, 300))
+    scale = float(10.0 ** rng.uniform(-2, 2))          # box size 0.01 .. 100: the FMM works in box units at every level
+    which = case % 6
+    levels = int(rng.integers(0, 4))
+    if which == 0:
+        L = (scale, scale, scale)
+        R0 = 0.5 * math.sqrt(3.0) * scale
+        w = W.Workload("f", W.BC_PERIODIC, L, (1, 1, 1), 1.0, float(rng.uniform(1.05, 1.7)) * R0, p, M, K,
+                       rng.random((N, 3)) * scale, W.alternating_charges(N))
+    elif which == 1:                                   # non-cubic cell, cubic FMM boxes: 2 x 1 x 1 per cell
+        L = (2.0 * scale, scale, scale)
+        R0 = 0.5 * math.sqrt(6.0) * scale
+        q = rng.standard_normal(N)
+        w = W.Workload("f", W.BC_PERIODIC, L, (1, 1, 1), 1.0, 1.15 * R0, p, M, K, rng.random((N, 3)) * np.asarray(L), q - q.mean())
+    elif which == 2:
+        L = (scale, scale, scale)
+        R0 = 0.5 * math.sqrt(3.0) * scale
+        w = W.Workload("f", W.BC_MIRROR_CAVITY, L, (1, 1, 1), -1.0, 1.5 * R0, p, M, K, (0.02 + 0.96 * rng.random((N, 3))) * scale,
+                       rng.standard_normal(N), check_xyz=W.seeded_face_points(K, L, W.ALL_FACES, seed=case))
+    elif which == 3:                                   # Neumann cavity: derivative rows -> step (a) keeps its direct FIELD form
+        L = (scale, scale, scale)
+        R0 = 0.5 * math.sqrt(3.0) * scale
+        q = rng.standard_normal(N)
+        w = W.Workload("f", W.BC_MIRROR_CAVITY, L, (1, 1, 1), 1.0, 1.5 * R0, p, M, K, (0.02 + 0.96 * rng.random((N, 3))) * scale,
+                       q - q.mean(), check_xyz=W.seeded_face_points(K, L, W.ALL_FACES, seed=case))
+    elif which == 4:                                   # grounded slab, boundary closure, 2 x 2 x 1 boxes per cell
+        L = (scale, scale, 0.5 * scale)
+        xyz = rng.random((N, 3)) * np.asarray(L)
+        xyz[:, 2] = (0.02 + 0.92 * xyz[:, 2] / L[2]) * L[2]
+        w = W.Workload("f", W.BC_SLAB_XY_PERIODIC_Z_MIRROR, L, (1, 1, 2), -1.0, 1.1 * scale, p, M, K, xyz, rng.standard_normal(N),
+                       closure=W.CLOSURE_BOUNDARY)
+    else:                                              # dielectric slab, far-data closure (step (a) over the far table: direct)
+        L = (scale, scale, 0.5 * scale)
+        q = rng.standard_normal(N)
+        w = W.Workload("f", W.BC_SLAB_XY_PERIODIC_Z_MIRROR, L, (1, 1, 2), float(rng.uniform(-0.9, 0.9)), 1.1 * scale, p, M, K,
+                       rng.random((N, 3)) * np.asarray(L), q - q.mean(), closure=W.CLOSURE_FAR_DATA, far_shell=(2, 2, 3),
+                       check_xyz=W.seeded_face_points(K, L, W.ALL_FACES, seed=case))
+    r = O.hsma(w, forces=True)
+    with H.Plan.from_workload(w, near_algorithm=H.binding.NEAR_ALG_FMM, fmm_levels=levels) as plan:
+        phi, F, U = plan.evaluate_forces(dev(w.xyz), dev(w.q), sync=True)
+        assert plan.last_pair_form == 3
+        phi0, U0 = plan.evaluate(dev(w.xyz), dev(w.q), sync=True)
+        assert plan.last_pair_form == 3
+    assert rel_inf(phi.cpu().numpy(), r.phi) <= 1e-10 and rel_inf(phi0.cpu().numpy(), r.phi) <= 1e-10
+    S = 0.5 * float(np.sum(np.abs(w.q * r.phi)))
+    for u in (float(U), float(U0)):
+        assert abs(u - r.U) <= (1e-11 * abs(r.U) if abs(r.U) >= 0.01 * S else 1e-13 * S)
+    assert rel_inf(F.cpu().numpy(), r.F) <= 1e-10
