@@ -41,6 +41,14 @@ constexpr int kInvW = kMaxOrder + 2;
 __host__ __device__ inline int nc(int p) { return (p + 1) * (p + 2) / 2; }
 __host__ __device__ inline int cidx(int n, int m) { return n * (n + 1) / 2 + m; }
 __host__ __device__ inline int fidx(int n, int m) { return n * n + n + m; }   // full range m = -n..n
+// Shared-memory layout of the expanded S table: row N (N = 0..2p) at N (N + 1), split by the parity of mu -- even orders
+// first, odd orders N + 1 slots later -- so that the threads of a row (l0 = 0, 2, 4, ...: orders of one parity at every
+// step) read CONSECUTIVE 16-byte slots (the plain layout had them 32 bytes apart: two-way bank conflicts on every read).
+__host__ __device__ inline int sp_size(int p) { return (2 * p + 1) * (2 * p + 2) + 2; }
+__host__ __device__ inline int sp_index(int N, int mu) {
+    const int par = mu & 1;
+    return N * (N + 1) + par * (N + 1) + ((mu + N + ((N + par) & 1)) >> 1);
+}
 
 struct Geom {
     int base[3];       // level-0 boxes per cell and axis (cubic boxes of side a0 = L_a / base_a)
@@ -313,7 +321,7 @@ __global__ void tables_kernel(int p, double2* __restrict__ Rsh, double2* __restr
         int N = 0;
         while ((N + 1) * (N + 1) <= t) ++N;
         const int mu = t - N * N - N;
-        sfmap[t] = (cidx(N, mu < 0 ? -mu : mu) << 2) | (mu < 0 ? ((mu & 1) ? 2 : 1) : 0);
+        sfmap[t] = (sp_index(N, mu) << 14) | (cidx(N, mu < 0 ? -mu : mu) << 2) | (mu < 0 ? ((mu & 1) ? 2 : 1) : 0);
     }
     if (t == 0) {   // output pairs (k, l0), l0 even
         int c = 0;
@@ -475,12 +483,31 @@ __global__ void __launch_bounds__(256) l2l_kernel(const Geom G, int lev, const d
 // sliding windows need two new S values per step for both outputs.  Per step and 8 siblings: 2 + 8 shared-memory
 // reads, 64 DFMA.
 template <int NV>
+__device__ __forceinline__ void m2l_step(const double2* __restrict__ Mrow, int mstride, int m, double sgn, double2 up0, double2 up1,
+                                         double2 dn0, double2 dn1, double2 (&a0)[NV], double2 (&a1)[NV]) {
+    const double2 P0 = make_double2(fma(sgn, dn0.x, up0.x), fma(sgn, dn0.y, up0.y));
+    const double2 P1 = make_double2(fma(sgn, dn1.x, up1.x), fma(sgn, dn1.y, up1.y));
+    const double2 Q0 = make_double2(fma(-sgn, dn0.y, up0.y), fma(sgn, dn0.x, -up0.x));   // -i (up - sgn dn)
+    const double2 Q1 = make_double2(fma(-sgn, dn1.y, up1.y), fma(sgn, dn1.x, -up1.x));
+#pragma unroll
+    for (int i = 0; i < NV; ++i) {
+        const double2 mv = Mrow[i * mstride + m];
+        a0[i].x = fma(mv.x, P0.x, a0[i].x); a0[i].x = fma(mv.y, Q0.x, a0[i].x);
+        a0[i].y = fma(mv.x, P0.y, a0[i].y); a0[i].y = fma(mv.y, Q0.y, a0[i].y);
+        a1[i].x = fma(mv.x, P1.x, a1[i].x); a1[i].x = fma(mv.y, Q1.x, a1[i].x);
+        a1[i].y = fma(mv.x, P1.y, a1[i].y); a1[i].y = fma(mv.y, Q1.y, a1[i].y);
+    }
+}
+template <int NV>
 __device__ __forceinline__ void m2l_inner(const double2* __restrict__ Sfull, const double2* __restrict__ Mf, int mstride,
                                           int p, int k, int l0, double2 (&a0)[NV], double2 (&a1)[NV]) {
     for (int n = 0; n <= p; ++n) {
-        const double2* Srow = Sfull + fidx(n + k, l0);   // Srow[j] = S_{n+k}^{l0 + j}
+        const int N = n + k;
+        // S_N^{l0 + j}: even j at E[j / 2], odd j at O[(j + 1) / 2]   (parity-split rows, sp_index)
+        const double2* E = Sfull + N * (N + 1) + ((l0 + N + (N & 1)) >> 1);
+        const double2* O = Sfull + N * (N + 1) + (N + 1) + ((l0 + N + ((N + 1) & 1) - 1) >> 1);
         const double2* Mrow = Mf + cidx(n, 0);
-        double2 up0 = Srow[0], up1 = Srow[1];            // (for the half pair l0 = k, up1 / dn1 may leave the row: unused)
+        double2 up0 = E[0], up1 = O[1];                  // (for the half pair l0 = k, up1 / dn1 may leave the row: unused)
         double2 dn0 = up0, dn1 = up1;
 #pragma unroll
         for (int i = 0; i < NV; ++i) {                   // m = 0: M_n^0 is real
@@ -488,23 +515,12 @@ __device__ __forceinline__ void m2l_inner(const double2* __restrict__ Sfull, con
             a0[i].x = fma(a, up0.x, a0[i].x); a0[i].y = fma(a, up0.y, a0[i].y);
             a1[i].x = fma(a, up1.x, a1[i].x); a1[i].y = fma(a, up1.y, a1[i].y);
         }
-        double sgn = -1.0;
-        for (int m = 1; m <= n; ++m) {
-            up0 = up1; up1 = Srow[m + 1];
-            dn1 = dn0; dn0 = Srow[-m];
-            const double2 P0 = make_double2(fma(sgn, dn0.x, up0.x), fma(sgn, dn0.y, up0.y));
-            const double2 P1 = make_double2(fma(sgn, dn1.x, up1.x), fma(sgn, dn1.y, up1.y));
-            const double2 Q0 = make_double2(fma(-sgn, dn0.y, up0.y), fma(sgn, dn0.x, -up0.x));   // -i (up - sgn dn)
-            const double2 Q1 = make_double2(fma(-sgn, dn1.y, up1.y), fma(sgn, dn1.x, -up1.x));
-#pragma unroll
-            for (int i = 0; i < NV; ++i) {
-                const double2 mv = Mrow[i * mstride + m];
-                a0[i].x = fma(mv.x, P0.x, a0[i].x); a0[i].x = fma(mv.y, Q0.x, a0[i].x);
-                a0[i].y = fma(mv.x, P0.y, a0[i].y); a0[i].y = fma(mv.y, Q0.y, a0[i].y);
-                a1[i].x = fma(mv.x, P1.x, a1[i].x); a1[i].x = fma(mv.y, Q1.x, a1[i].x);
-                a1[i].y = fma(mv.x, P1.y, a1[i].y); a1[i].y = fma(mv.y, Q1.y, a1[i].y);
-            }
-            sgn = -sgn;
+        for (int m = 1; m <= n; m += 2) {
+            up0 = up1; up1 = E[(m + 1) >> 1]; dn1 = dn0; dn0 = O[-((m - 1) >> 1)];        // odd m
+            m2l_step<NV>(Mrow, mstride, m, -1.0, up0, up1, dn0, dn1, a0, a1);
+            if (m + 1 > n) break;
+            up0 = up1; up1 = O[(m + 3) >> 1]; dn1 = dn0; dn0 = E[-((m + 1) >> 1)];        // even m + 1
+            m2l_step<NV>(Mrow, mstride, m + 1, 1.0, up0, up1, dn0, dn1, a0, a1);
         }
     }
 }
@@ -516,7 +532,7 @@ __host__ __device__ inline int m2l_pairs(int p) {   // sum_k ceil((k+1)/2)
     return s;
 }
 __host__ __device__ inline int m2l_smem_bytes(int p) {
-    return (int)sizeof(double2) * ((2 * p + 1) * (2 * p + 1) + 1 + 8 * nc(p));
+    return (int)sizeof(double2) * (sp_size(p) + 8 * nc(p));
 }
 
 // pm[t] = (k << 8) | l0 of output pair t; sfmap[t] = (cidx(N, |mu|) << 2) | op for the expanded S table entry t =
@@ -541,12 +557,12 @@ __global__ void __launch_bounds__(kM2LThreads) m2l_kernel(const Geom G, const M2
     __shared__ int s_nv, s_lo, s_hi;
     const int p = G.p, NC = nc(p), NS = nc(2 * p), NSF = (2 * p + 1) * (2 * p + 1), NP = m2l_pairs(p);
     double2* Sfull = sm2;
-    double2* Mfull = sm2 + NSF + 1;
+    double2* Mfull = sm2 + sp_size(p);
     const int tid = threadIdx.x;
     const int Gc = gridDim.x, kc = blockIdx.x;
     const long long u0 = unit_start(kc, A.units, Gc), u1 = unit_start(kc + 1, A.units, Gc);
     if (u1 <= u0) return;
-    if (tid == 0) Sfull[NSF] = make_double2(0.0, 0.0);
+    for (int t = tid; t < sp_size(p); t += kM2LThreads) Sfull[t] = make_double2(0.0, 0.0);   // (pads and unused slots)
     for (long long grp = u0 / A.W; grp <= (u1 - 1) / A.W; ++grp) {
         int r = 0;
         while (r + 1 < A.n_lv && grp >= A.lv[r + 1].first_group) ++r;
@@ -615,10 +631,10 @@ __global__ void __launch_bounds__(kM2LThreads) m2l_kernel(const Geom G, const M2
                 const double2* S = Stab + (long long)(((kOffR - dx) * kOffW + (kOffR - dy)) * kOffW + (kOffR - dz)) * NS;
                 for (int t = tid; t < NSF; t += kM2LThreads) {
                     const int e = sfmap[t];
-                    double2 v = S[e >> 2];
+                    double2 v = S[(e >> 2) & 4095];
                     if (e & 1) v.y = -v.y;
                     if (e & 2) { v.x = -v.x; }
-                    Sfull[t] = v;
+                    Sfull[e >> 14] = v;
                 }
                 // the (reflected, weighted) source moments of the valid siblings, m >= 0
                 for (int t = tid; t < nv * NC; t += kM2LThreads) {
