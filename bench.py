@@ -68,8 +68,8 @@ def sym_evaluations(N: int, C: int) -> int:
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel from the committed ncu --set full
 # capture (profiles/r01_ncu_near_sum_N262144.md): valid for config 5 at N = 262,144 on one GPU, potential only
 NCU_TRAFFIC_BYTES_CFG5 = 9555200
-NCU_TRAFFIC_BYTES_CFG5_SYM = 118378496   # near_sym_kernel: 18,231,808 read + 100,146,688 written
-TRAFFIC_SOURCE_SYM = "profiles/r01_ncu_near_sym_N262144.md (dram read+write bytes of one launch)"
+NCU_TRAFFIC_BYTES_CFG5_SYM = 28873728    # near_sym_kernel, 3 waves per evaluate: 3 x (8,463,872 read + 1,160,704 written)
+TRAFFIC_SOURCE_SYM = "profiles/r02_ncu_near_sym_waves_N262144.md (dram read+write bytes of one wave x 3 waves per evaluate)"
 TRAFFIC_SOURCE = "profiles/r01_ncu_near_sum_N262144.md (dram read+write bytes of one launch)"
 # FP64 peak derived from unit counts and clocks: SMs x 64 DFMA lanes x 2 x clock
 FP64_LANES_PER_SM = 64
