@@ -990,13 +990,11 @@ __global__ void __launch_bounds__(kM2PThreads) m2p_points_kernel(const Geom G, c
                 if (m > 0) { const double f = (double)(2 * m - 1) * ir2, u = (sr * rx - si * ry) * f; si = (sr * ry + si * rx) * f; sr = u; }
                 double p1r = sr, p1i = si, p2r = 0.0, p2i = 0.0;
                 double2 mc = Mb[cidx(m, m)];
-                double2 mn = m < p ? Mb[cidx(m + 1, m)] : mc;          // the moment of the next step is fetched one step ahead
                 double s = fma(mc.x, sr, mc.y * si);
                 for (int n = m + 1; n <= p; ++n) {
-                    mc = mn;
-                    if (n < p) mn = Mb[cidx(n + 1, m)];
                     const double tz = (double)(2 * n - 1) * rz, gg = (double)(n - 1 + m) * (double)(n - 1 - m);
                     const double cr = (tz * p1r - gg * p2r) * ir2, ci = (tz * p1i - gg * p2i) * ir2;
+                    mc = Mb[cidx(n, m)];
                     s = fma(mc.x, cr, s); s = fma(mc.y, ci, s);
                     p2r = p1r; p2i = p1i; p1r = cr; p1i = ci;
                 }

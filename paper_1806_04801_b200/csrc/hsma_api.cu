@@ -99,10 +99,10 @@ static int near_resident(int R, int refine, bool field) {
     return c;
 }
 static int node_resident(int R, bool field) {
-    static int cache[3][2] = {};
-    int& c = cache[R == 4 ? 2 : (R == 2 ? 1 : 0)][field ? 1 : 0];
+    static int cache[4][2] = {};
+    int& c = cache[R == 8 ? 3 : R == 4 ? 2 : (R == 2 ? 1 : 0)][field ? 1 : 0];
     if (!c) {
-        if (!field) c = R == 4 ? resident_ctas(node_sum_kernel<4, false>) : R == 2 ? resident_ctas(node_sum_kernel<2, false>) : resident_ctas(node_sum_kernel<1, false>);
+        if (!field) c = R == 8 ? resident_ctas(node_sum_kernel<8, false>) : R == 4 ? resident_ctas(node_sum_kernel<4, false>) : R == 2 ? resident_ctas(node_sum_kernel<2, false>) : resident_ctas(node_sum_kernel<1, false>);
         else c = R == 4 ? resident_ctas(node_sum_kernel<4, true>) : R == 2 ? resident_ctas(node_sum_kernel<2, true>) : resident_ctas(node_sum_kernel<1, true>);
     }
     return c;
@@ -274,7 +274,7 @@ static SymLaunch choose_sym(long long n_tiles, int refine, size_t col_cap_bytes,
 static bool sym_applies(long long n_tiles, int C) { return n_tiles >= 32 && C <= kSymMaxCells; }
 
 static Launch choose_node(long long T, long long n_tiles, bool field = false) {
-    return choose_launch(T, n_tiles, 4, [field](int R) { return node_resident(R, field); });
+    return choose_launch(T, n_tiles, field ? 4 : 8, [field](int R) { return node_resident(R, field); });
 }
 static void launch_node(const Launch& L, bool field, const double* tgt, int tstride, const int* tgt_index, long long T,
                         long long t_first, const Node8* nodes, long long n_tiles, double* part, cudaStream_t st) {
@@ -286,7 +286,8 @@ static void launch_node(const Launch& L, bool field, const double* tgt, int tstr
         else if (L.R == 2) node_sum_kernel<2, true><<<L.G, kThreads, 0, st>>>(a);
         else node_sum_kernel<1, true><<<L.G, kThreads, 0, st>>>(a);
     } else {
-        if (L.R == 4) node_sum_kernel<4, false><<<L.G, kThreads, 0, st>>>(a);
+        if (L.R == 8) node_sum_kernel<8, false><<<L.G, kThreads, 0, st>>>(a);
+        else if (L.R == 4) node_sum_kernel<4, false><<<L.G, kThreads, 0, st>>>(a);
         else if (L.R == 2) node_sum_kernel<2, false><<<L.G, kThreads, 0, st>>>(a);
         else node_sum_kernel<1, false><<<L.G, kThreads, 0, st>>>(a);
     }
