@@ -463,8 +463,9 @@ def run_b200(args, w) -> dict:
            "launches_per_step": plan.launches_last_evaluate(),
            "graph_replays": H.binding.hsma_plan_info(plan.handle)["graph_replays"], "clocks": clocks, "roofline": roofline}
     if fmm_arm:
-        out["config"]["near_algorithm"] = (f"fmm (order {args.fmm_order or 20}, two-box separation, leaf level "
-                                           f"{args.fmm_levels or 'by N'}): step (b) sub-quadratic, DESIGN.md 6.13; value still "
+        fi = H.binding.hsma_plan_fmm_info(plan.handle)
+        out["config"]["near_algorithm"] = (f"fmm (order {fi['order']}, two-box separation, leaf level {fi['leaf_level']} = "
+                                           f"{fi['leaves']} leaves): steps (a), (b) sub-quadratic, DESIGN.md 6.13; value still "
                                            f"counts the pair interactions of the direct sum it replaces")
         roofline["kernel"] = "fmm step (b): sort + p2m + m2m + m2l_kernel + l2l + leaf_kernel (kernel_ms is the whole stage)"
         for k in ("achieved", "frac", "frac_executed_flops", "fp64_pipe_issue_util", "frac_of_dfma_microbench", "evaluations_per_s"):
@@ -494,8 +495,9 @@ def run_b200(args, w) -> dict:
                 H.hsma_evaluate(pf.handle, xyz, q, phi_f, U_f)
                 pf.sync()
                 tm = pf.timing()
+                fi = H.binding.hsma_plan_fmm_info(pf.handle)
                 out["fmm"] = {"ms_per_step": tot / nrep, "steps": nrep, "near_source_ms": tm["near_source_kernel"],
-                              "order": args.fmm_order or 20, "energy": float(U_f.cpu()[0]),
+                              "order": fi["order"], "leaf_level": fi["leaf_level"], "leaves": fi["leaves"], "energy": float(U_f.cpu()[0]),
                               "energy_rel_diff_vs_direct": abs(float(U_f.cpu()[0]) - U_val) / abs(U_val) if U_val else None,
                               "max_phi_rel_diff_vs_direct": float((phi_f - phi).abs().max() / phi.abs().max()),
                               "note": "near_algorithm = FMM (DESIGN.md 6.13): the same evaluate with step (b) by the fast multipole "

@@ -295,7 +295,12 @@ hsma_status hsma_plan_get_timing(hsma_plan* plan, double* ms_out);
  * (0: null plan).
  */
 hsma_status hsma_plan_set_pair_form(hsma_plan* plan, int form);
-int hsma_plan_last_pair_form(const hsma_plan* plan);
+int hsma_plan_last_pair_form(const hsma_plan* plan);   /* also 3: step (b) ran as the FMM (near_algorithm = HSMA_NEAR_ALG_FMM) */
+
+/* near_algorithm = FMM: what[0] = expansion order, [1] = leaf level of the last evaluate (0 before the first), [2] = leaf
+ * boxes of that level, [3] = 1 if the plan's geometry lets step (a) use the multipoles too.  host out [4].
+ * HSMA_ERR_INVALID_ARG for a plan created with the direct algorithm. */
+hsma_status hsma_plan_fmm_info(hsma_plan* plan, long long* what_out);
 
 /*
  * Scratch of the symmetric form.  The unordered pairs of one rank are walked in "waves" (launches);

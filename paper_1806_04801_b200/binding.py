@@ -108,6 +108,7 @@ _SIGNATURES = {
     "hsma_plan_last_pair_form": (ctypes.c_int, [ctypes.c_void_p]),
     "hsma_plan_set_sym_scratch_cap": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_longlong]),
     "hsma_plan_scratch_bytes": (ctypes.c_longlong, [ctypes.c_void_p]),
+    "hsma_plan_fmm_info": (ctypes.c_int, [ctypes.c_void_p, ctypes.POINTER(ctypes.c_longlong)]),
     "hsma_plan_get_timing": (ctypes.c_int, [ctypes.c_void_p, c_double_p]),
     "hsma_launch_count": (ctypes.c_longlong, []),
 }
@@ -433,6 +434,13 @@ def hsma_plan_last_pair_form(plan: int) -> int:
 def hsma_plan_set_sym_scratch_cap(plan: int, nbytes: int):
     """Column-sum scratch per wave of the symmetric form, bytes (0: the default 64 MiB); include/hsma.h."""
     _check(load_library().hsma_plan_set_sym_scratch_cap(plan, int(nbytes)), "hsma_plan_set_sym_scratch_cap")
+
+
+def hsma_plan_fmm_info(plan: int) -> dict:
+    """near_algorithm = FMM: expansion order, leaf level and leaf count of the last evaluate, whether step (a) uses the multipoles."""
+    w = (ctypes.c_longlong * 4)()
+    _check(load_library().hsma_plan_fmm_info(plan, w), "hsma_plan_fmm_info")
+    return dict(zip(("order", "leaf_level", "leaves", "check_points_by_m2p"), [int(v) for v in w]))
 
 
 def hsma_plan_scratch_bytes(plan: int) -> int:

@@ -1323,6 +1323,14 @@ extern "C" hsma_status hsma_plan_set_pair_form(hsma_plan* p, int form) {
 
 extern "C" int hsma_plan_last_pair_form(const hsma_plan* p) { return p ? p->last_pair_form : 0; }
 
+extern "C" hsma_status hsma_plan_fmm_info(hsma_plan* p, long long* w) {
+    if (!p || !w || !p->fmm.enabled) return HSMA_ERR_INVALID_ARG;
+    w[0] = p->fmm.p; w[1] = p->fmm.last_levels;
+    w[2] = p->fmm.last_levels > 0 ? ((long long)p->fmm.base[0] * p->fmm.base[1] * p->fmm.base[2]) << (3 * p->fmm.last_levels) : 0;
+    w[3] = (p->cells_rhs == p->cells_near && !p->need_grad) ? 1 : 0;
+    return HSMA_OK;
+}
+
 extern "C" hsma_status hsma_plan_set_sym_scratch_cap(hsma_plan* p, long long bytes) {
     if (!p || bytes < 0) return HSMA_ERR_INVALID_ARG;
     p->sym_col_cap = bytes == 0 ? kSymColCapDefault : (size_t)bytes;
