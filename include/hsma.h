@@ -277,7 +277,9 @@ hsma_status hsma_fp64_peak(double seconds, double* tflops_out, double* sm_clock_
  * milliseconds to host ms_out [8]:
  *   [0] H1 pre-pass (+ neutrality)   [1] H2 near_sum_kernel over the check targets, kernel only
  *   [2] H2 finish + H3 fit + H4 map  [3] H5 near_sum_kernel over the sources, kernel only (the hot loop)
- *   [4] H6 node_sum_kernel, kernel only   [5] H7 finish + energy   [6] whole evaluate   [7] 0
+ *   [4] H6 node_sum_kernel, kernel only   [5] H7 finish + energy   [6] whole evaluate
+ *   [7] near_algorithm = FMM: the far field of step (b) (M2L + L2L), which runs before step (a) and is NOT in [0] or [3]
+ *       ([0] then holds the leaf sort, P2M and M2M; [3] the leaf kernel); 0 otherwise
  */
 hsma_status hsma_plan_set_timing(hsma_plan* plan, int enable);
 hsma_status hsma_plan_get_timing(hsma_plan* plan, double* ms_out);

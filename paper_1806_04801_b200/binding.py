@@ -409,7 +409,7 @@ def hsma_fp64_peak(seconds: float = 1.0):
     return t.value, c.value
 
 
-TIMING_KEYS = ("prepass", "near_check_kernel", "fit_map", "near_source_kernel", "node_kernel", "finish", "total")
+TIMING_KEYS = ("prepass", "near_check_kernel", "fit_map", "near_source_kernel", "node_kernel", "finish", "total", "fmm_far_field")
 
 
 def hsma_plan_set_timing(plan: int, enable: bool):

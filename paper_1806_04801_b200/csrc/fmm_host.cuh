@@ -201,23 +201,22 @@ inline hsma_status upward(State& S, const double* xyz, const double* q, long lon
     return HSMA_OK;
 }
 
-// Step (a) from the hierarchy built by `upward`: the near sum at T arbitrary points (centred coordinates, device).
+// Step (a) from the hierarchy built by `upward` and `far_field`: the near sum at T arbitrary points (centred coordinates, device).
 inline hsma_status points(State& S, const double* tgt, long long T, long long N, const double half[3], double* phi_out,
                           cudaStream_t st) {
     if (T < 1) return HSMA_OK;
     const Geom G = make_geom(S, N, half);
-    m2p_points_kernel<<<(unsigned)T, kM2PThreads, 0, st>>>(G, tgt, S.srt.p, S.leaf_start.p, S.Mx.p, phi_out);
+    const size_t smem = nc(S.p) * sizeof(double2) + (S.p + 1) * kInvW * sizeof(double);
+    m2p_points_kernel<<<(unsigned)T, kM2PThreads, smem, st>>>(G, tgt, S.srt.p, S.leaf_start.p, S.Mx.p, S.Lx.p, phi_out);
     HSMA_COUNT_LAUNCH();
     return HSMA_OK;
 }
 
-// Step (b) at all N sources, original order, into phi_out [N] (device): M2L at every level, L2L down, leaves
-// (L2P + P2P).  refine as in the direct kernels (1 Newton, 2 cubic) for the P2P part.
-inline hsma_status downward(State& S, long long N, const double half[3], int refine, bool field, double* phi_out,
-                            std::atomic<size_t>& epoch, cudaStream_t st) {
+// Far field of step (b): M2L at every level, L2L down.  Afterwards the local expansions of all boxes are in S.Lx (used by
+// step (a) for check targets inside the central cell, and by `leaves`).
+inline hsma_status far_field(State& S, long long N, const double half[3], std::atomic<size_t>& epoch, cudaStream_t st) {
     const Geom G = make_geom(S, N, half);
     const int NC = nc(S.p);
-    const long long n_leaves = boxes_at(G, G.levels);
     // M2L launch shape: one persistent wave over the units (group, offset weight), deepest level first
     M2LArgs A;
     A.n_lv = 0;
@@ -246,6 +245,16 @@ inline hsma_status downward(State& S, long long N, const double half[3], int ref
         l2l_kernel<<<(unsigned)boxes_at(G, lev), 256, 2 * NC * sizeof(double2), st>>>(G, lev, S.Rsh, S.nm, S.Lpart.p, A, Gm2l, S.Lx.p);
         HSMA_COUNT_LAUNCH();
     }
+    return HSMA_OK;
+}
+
+// Step (b) at all N sources, original order, into phi_out [N] ([4][N] with forces): the leaves (L2P + P2P) after
+// `far_field`.  refine as in the direct kernels (1 Newton, 2 cubic) for the P2P part.
+inline hsma_status leaves(State& S, long long N, const double half[3], int refine, bool field, double* phi_out,
+                          std::atomic<size_t>& epoch, cudaStream_t st) {
+    const Geom G = make_geom(S, N, half);
+    const int NC = nc(S.p);
+    const long long n_leaves = boxes_at(G, G.levels);
     const int inv_bytes = (S.p + 1) * kInvW * (int)sizeof(double);
     const size_t leaf_smem = NC * sizeof(double2) + inv_bytes;
     leaf_chunks_kernel<<<1, 1024, 0, st>>>(S.leaf_start.p, (int)n_leaves, S.chunk_start.p);

@@ -947,10 +947,15 @@ __global__ void leaf_sum_kernel(const double* __restrict__ slab, long long n /* 
 // the same truncation error.  One CTA per target; the threads share the boxes; fixed-order tree reduction.
 constexpr int kM2PThreads = 128;
 
+// A target INSIDE the central cell has a leaf with a local expansion: its far field is one L2P (231 terms, the orders m
+// shared among the threads) instead of ~2,700 M2P.
+// dynamic shared memory: Ls [NC] double2, inv [(p+1) * kInvW] double
 __global__ void __launch_bounds__(kM2PThreads) m2p_points_kernel(const Geom G, const double* __restrict__ tgt /* [T,3] centred */,
                                                                  const Src4* __restrict__ srt, const int* __restrict__ leaf_start,
-                                                                 const double2* __restrict__ M, double* __restrict__ phi_out) {
+                                                                 const double2* __restrict__ M, const double2* __restrict__ L,
+                                                                 double* __restrict__ phi_out) {
     __shared__ double red[kM2PThreads];
+    extern __shared__ __align__(16) double2 sm2[];
     const int p = G.p, NC = nc(p), lmax = G.levels, tid = threadIdx.x;
     const double x = tgt[3 * (size_t)blockIdx.x], y = tgt[3 * (size_t)blockIdx.x + 1], z = tgt[3 * (size_t)blockIdx.x + 2];
     const double xc[3] = {x, y, z};
@@ -958,8 +963,41 @@ __global__ void __launch_bounds__(kM2PThreads) m2p_points_kernel(const Geom G, c
 #pragma unroll
     for (int a = 0; a < 3; ++a) gl[a] = (int)floor((xc[a] + G.half[a]) * (double)(1 << lmax) / G.a0);
     double acc = 0.0;
-    // far field: multipoles of the interaction lists, all levels
-    for (int lev = lmax; lev >= 0; --lev) {
+    bool inside = true;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) inside = inside && gl[a] >= 0 && gl[a] < grid_n(G, lmax, a);
+    if (inside) {   // far field = the leaf's local expansion: thread m takes the order m
+        double2* Ls = sm2;
+        double* inv = reinterpret_cast<double*>(sm2 + NC);
+        const int leaf = (gl[0] * grid_n(G, lmax, 1) + gl[1]) * grid_n(G, lmax, 2) + gl[2];
+        const double2* Lleaf = L + (level_offset(G, lmax) + leaf) * NC;
+        for (int t = tid; t < NC; t += kM2PThreads) Ls[t] = Lleaf[t];
+        fill_inv_table(inv, p);
+        __syncthreads();
+        if (tid <= p) {
+            double c[3]; int ic[3];
+            box_centre(G, lmax, leaf, c, ic);
+            const double ia = (double)(1 << lmax) / G.a0;
+            const double rx = (x - c[0]) * ia, ry = (y - c[1]) * ia, rz = (z - c[2]) * ia;
+            const double r2 = fma(rz, rz, fma(ry, ry, rx * rx));
+            const int m = tid;
+            double rr = 1.0, ri = 0.0;
+            for (int i = 1; i <= m; ++i) { const double f = 0.5 / (double)i, u = (rr * rx - ri * ry) * f; ri = (rr * ry + ri * rx) * f; rr = u; }
+            double p1r = rr, p1i = ri, p2r = 0.0, p2i = 0.0;
+            double2 lc = Ls[cidx(m, m)];
+            double s = fma(rr, lc.x, ri * lc.y);
+            for (int n = m + 1; n <= p; ++n) {
+                const double f = inv[n * kInvW + m], tz = (double)(2 * n - 1) * rz;
+                const double cr = (tz * p1r - r2 * p2r) * f, ci = (tz * p1i - r2 * p2i) * f;
+                lc = Ls[cidx(n, m)];
+                s = fma(cr, lc.x, s); s = fma(ci, lc.y, s);
+                p2r = p1r; p2i = p1i; p1r = cr; p1i = ci;
+            }
+            acc = (m == 0 ? s : 2.0 * s) * ia;
+        }
+    }
+    // far field of a target outside the central cell: multipoles of the interaction lists, all levels
+    for (int lev = inside ? -1 : lmax; lev >= 0; --lev) {
         const int sh = lmax - lev;
         const int b[3] = {gl[0] >> sh, gl[1] >> sh, gl[2] >> sh};
         int R[3];   // candidate offsets |d_a| <= R_a
