@@ -143,17 +143,23 @@ struct Packed {
 
 template <bool UNIFORM, bool FIELD>
 static void launch_near_form(const Launch& L, int refine, const NearArgs& a, cudaStream_t st) {
-    if (refine == 1) {
-        if (L.R == 8) { if (!FIELD) near_sum_kernel<8, 1, UNIFORM, false><<<L.G, kThreads, 0, st>>>(a); }
-        else if (L.R == 4) near_sum_kernel<4, 1, UNIFORM, FIELD><<<L.G, kThreads, 0, st>>>(a);
-        else if (L.R == 2) near_sum_kernel<2, 1, UNIFORM, FIELD><<<L.G, kThreads, 0, st>>>(a);
-        else near_sum_kernel<1, 1, UNIFORM, FIELD><<<L.G, kThreads, 0, st>>>(a);
-    } else {
-        if (L.R == 8) { if (!FIELD) near_sum_kernel<8, 2, UNIFORM, false><<<L.G, kThreads, 0, st>>>(a); }
-        else if (L.R == 4) near_sum_kernel<4, 2, UNIFORM, FIELD><<<L.G, kThreads, 0, st>>>(a);
-        else if (L.R == 2) near_sum_kernel<2, 2, UNIFORM, FIELD><<<L.G, kThreads, 0, st>>>(a);
-        else near_sum_kernel<1, 2, UNIFORM, FIELD><<<L.G, kThreads, 0, st>>>(a);
-    }
+#define NEAR_LAUNCH(K)                                                                                   \
+    do {                                                                                                 \
+        if (refine == 1) {                                                                               \
+            if (L.R == 8) { if (!FIELD) K<8, 1, UNIFORM, false><<<L.G, kThreads, 0, st>>>(a); }          \
+            else if (L.R == 4) K<4, 1, UNIFORM, FIELD><<<L.G, kThreads, 0, st>>>(a);                     \
+            else if (L.R == 2) K<2, 1, UNIFORM, FIELD><<<L.G, kThreads, 0, st>>>(a);                     \
+            else K<1, 1, UNIFORM, FIELD><<<L.G, kThreads, 0, st>>>(a);                                   \
+        } else {                                                                                         \
+            if (L.R == 8) { if (!FIELD) K<8, 2, UNIFORM, false><<<L.G, kThreads, 0, st>>>(a); }          \
+            else if (L.R == 4) K<4, 2, UNIFORM, FIELD><<<L.G, kThreads, 0, st>>>(a);                     \
+            else if (L.R == 2) K<2, 2, UNIFORM, FIELD><<<L.G, kThreads, 0, st>>>(a);                     \
+            else K<1, 2, UNIFORM, FIELD><<<L.G, kThreads, 0, st>>>(a);                                   \
+        }                                                                                                \
+    } while (0)
+    if (a.dyn) NEAR_LAUNCH(near_sum_dyn_kernel);   // sphere-culled near set: device-resident source count
+    else NEAR_LAUNCH(near_sum_kernel);
+#undef NEAR_LAUNCH
     HSMA_COUNT_LAUNCH();
 }
 

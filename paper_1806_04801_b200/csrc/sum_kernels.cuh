@@ -163,8 +163,8 @@ constexpr int near_min_ctas(int R) { return R >= 8 ? 1 : (R == 4 ? 2 : (R == 2 ?
 // and each instantiation keeps only its own loops: fewer live registers, better schedules).
 // FIELD: also accumulate the gradient; partial rows then hold 4 components per target, part[(row*4 + comp)*T + t],
 // comp 0 = phi, 1..3 = grad phi (in the frame of the ORIGINAL target: a reflected axis flips its component back).
-template <int R, int REFINE, bool UNIFORM, bool FIELD = false>
-__global__ void __launch_bounds__(kThreads, near_min_ctas(FIELD ? 2 * R : R)) near_sum_kernel(const NearArgs a) {
+template <int R, int REFINE, bool UNIFORM, bool FIELD>
+__device__ __forceinline__ void near_sum_body(const NearArgs& a) {
     __shared__ __align__(128) Src4 tile[kStages][kTile];
     __shared__ __align__(8) uint64_t full[kStages];
     __shared__ Cell cells[kMaxCells];
@@ -173,11 +173,9 @@ __global__ void __launch_bounds__(kThreads, near_min_ctas(FIELD ? 2 * R : R)) ne
     if ((a.qinfo != nullptr && a.qinfo->uniform != 0) != UNIFORM) return;
     const int tid = threadIdx.x;
     const int G = gridDim.x, k = blockIdx.x;
-    const long long a_n_src = a.dyn ? a.dyn[0] : a.n_src, a_n_tiles = a.dyn ? a.dyn[1] : a.n_tiles;
-    const long long a_units = a.dyn ? a.ntb * a_n_tiles * a.C : a.units;
-    const long long u0 = unit_start(k, a_units, G), u1 = unit_start(k + 1, a_units, G);
-    if (u1 <= u0) return;  // (G <= U, except with a device-resident source count smaller than the host's estimate)
-    const long long Ub = a_n_tiles * a.C;
+    const long long u0 = unit_start(k, a.units, G), u1 = unit_start(k + 1, a.units, G);
+    if (u1 <= u0) return;  // (never: the host launches G <= U CTAs)
+    const long long Ub = a.n_tiles * a.C;
     const long long V0 = u0 / a.C, V1 = (u1 - 1) / a.C;  // visits v = b * n_tiles + t of this CTA
 
     for (int c = tid; c < a.C; c += kThreads) cells[c] = a.cells[c];
@@ -188,7 +186,7 @@ __global__ void __launch_bounds__(kThreads, near_min_ctas(FIELD ? 2 * R : R)) ne
     __syncthreads();
     if (tid == 0) {
         mbar_expect_tx(&full[0], kTile * sizeof(Src4));
-        bulk_g2s(tile[0], a.src + (V0 % a_n_tiles) * kTile, kTile * sizeof(Src4), &full[0]);
+        bulk_g2s(tile[0], a.src + (V0 % a.n_tiles) * kTile, kTile * sizeof(Src4), &full[0]);
     }
     const double qmag = UNIFORM ? a.qinfo->qmag : 1.0;
 
@@ -197,13 +195,13 @@ __global__ void __launch_bounds__(kThreads, near_min_ctas(FIELD ? 2 * R : R)) ne
     double totx[RG], toty[RG], totz[RG];
     // visits are walked with 32-bit state: block b, tile tl inside the block
     const int nvis = (int)(V1 - V0) + 1;
-    const int nt = (int)a_n_tiles;
-    int b = (int)(V0 / a_n_tiles), tl = (int)(V0 - (long long)b * a_n_tiles);
+    const int nt = (int)a.n_tiles;
+    int b = (int)(V0 / a.n_tiles), tl = (int)(V0 - (long long)b * a.n_tiles);
     const int c_first = (int)(u0 - V0 * a.C), c_last = (int)(u1 - 1 - V1 * a.C) + 1;
     bool fresh = true;  // targets of block b not loaded yet
     // partial sums of block b go to row (k - first CTA that works on b)
     auto store_block = [&](int blk) {
-        const int row = k - cta_of_unit(blk * Ub, a_units, G);
+        const int row = k - cta_of_unit(blk * Ub, a.units, G);
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const long long t = (long long)blk * (kThreads * R) + r * kThreads + tid;
@@ -240,7 +238,7 @@ __global__ void __launch_bounds__(kThreads, near_min_ctas(FIELD ? 2 * R : R)) ne
             }
         }
         const int np = a.tile_np[tl];
-        const int nv = (int)min((long long)kTile, a_n_src - (long long)tl * kTile);
+        const int nv = (int)min((long long)kTile, a.n_src - (long long)tl * kTile);
         mbar_wait(&full[st], (it >> 1) & 1);
         const Src4* __restrict__ s = tile[st];
         // self: target t is source self_offset + t (same tile after the in-tile sort).  Block-uniform test
@@ -341,6 +339,23 @@ __global__ void __launch_bounds__(kThreads, near_min_ctas(FIELD ? 2 * R : R)) ne
         }
     }
     if (!fresh) store_block(b);
+}
+
+template <int R, int REFINE, bool UNIFORM, bool FIELD = false>
+__global__ void __launch_bounds__(kThreads, near_min_ctas(FIELD ? 2 * R : R)) near_sum_kernel(const NearArgs a) {
+    near_sum_body<R, REFINE, UNIFORM, FIELD>(a);
+}
+// The same with the source count read from device memory (sphere-culled near set: the image list is built on the device
+// and its length never visits the host): dyn[0] = sources, dyn[1] = source tiles replace n_src / n_tiles, and
+// units = ntb * dyn[1] * C.  A separate instantiation, so that the kernel above keeps exactly its register allocation
+// (folding the choice into it cost the R = 8 loop 2.7 % at 244 registers).
+template <int R, int REFINE, bool UNIFORM, bool FIELD = false>
+__global__ void __launch_bounds__(kThreads, near_min_ctas(FIELD ? 2 * R : R)) near_sum_dyn_kernel(const NearArgs a) {
+    NearArgs b = a;
+    b.n_src = a.dyn[0];
+    b.n_tiles = a.dyn[1];
+    b.units = a.ntb * b.n_tiles * a.C;
+    near_sum_body<R, REFINE, UNIFORM, FIELD>(b);
 }
 
 // ---- step (b), symmetric form (Newton's third law) ---------------------------------------------
