@@ -43,7 +43,6 @@ struct State {
     Buf<Src4> srt;
     Buf<double> slab;             // leaf kernel: one partial row per slab of neighbour boxes
     Buf<double2> Mx, Lx, Lpart;   // multipole / local expansions of all levels, M2L partial sums
-    double* phi = nullptr;     // not owned: the plan's sym_phi buffer
     void release() {
         for (void* q : {(void*)w_lut, (void*)Rsh, (void*)Stab, (void*)nm, (void*)pm, (void*)sfmap, (void*)off_list, (void*)off_wprefix}) if (q) cudaFree(q);
         w_lut = nullptr; Rsh = Stab = nullptr; nm = pm = sfmap = off_list = off_wprefix = nullptr;
