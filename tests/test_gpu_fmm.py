@@ -178,3 +178,15 @@ def test_where_the_fmm_applies_and_what_it_rejects(H):
         with pytest.raises(H.HsmaError) as e:
             H.Plan.from_workload(w, near_algorithm=H.binding.NEAR_ALG_FMM, **bad)
         assert e.value.status == H.HSMA_ERR_INVALID_ARG
+
+
+def test_paper_lattice_site_workload(H):
+    """The paper's own large-scale workload (charges on lattice sites with random signs): 32^3 sites fall
+    on the faces and corners of the FMM boxes, the geometry with the largest expansion radii -- unlike the ordered rock
+    salt of config 1 the random signs do not add the errors coherently, and the default order meets the bars."""
+    w = W.paper_timing(32768).with_(near_mode=W.NEAR_WHOLE_CELLS, R_aux=1.5 * np.sqrt(3) / 2, p=12, K=400, M=2000,
+                                    quad_rule=W.QUAD_SPIRAL, dipole_mode=W.DIPOLE_EXACT)
+    r = O.hsma(w)
+    for levels in (0, 3):
+        phi, U = run_fmm(H, w, oracle=r, fmm_levels=levels)
+        assert rel_inf(phi, r.phi) <= PHI_TOL and abs(U - r.U) <= U_TOL * abs(r.U)
