@@ -18,7 +18,8 @@
  *     the library centres them (reading G10).
  *   - periodic kinds: phi is in the gauge A_00 = 0 (reading S2); U is gauge free for neutral input.
  *   - hsma_evaluate* are asynchronous on the plan's stream and perform no host synchronisation
- *     (hsma_evaluate_host synchronises because it returns host data).
+ *     (hsma_evaluate_host synchronises because it returns host data; the first evaluate at a larger N than before grows
+ *     the plan's scratch with cudaFree/cudaMalloc, an implicit device synchronisation -- see "Thread safety" below).
  *   - on a non-default stream, repeated evaluates with identical arguments (same pointers and sizes: the MD loop)
  *     are captured into one CUDA graph on the second call and replayed afterwards.
  *   - preconditions not checked: particles inside the box, no coincident particles, no particle on
