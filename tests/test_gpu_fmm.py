@@ -190,3 +190,17 @@ def test_paper_lattice_site_workload(H):
     for levels in (0, 3):
         phi, U = run_fmm(H, w, oracle=r, fmm_levels=levels)
         assert rel_inf(phi, r.phi) <= PHI_TOL and abs(U - r.U) <= U_TOL * abs(r.U)
+
+
+@pytest.mark.parametrize("order", [2, 7, 30])
+def test_extreme_orders_run_and_converge(H, order):
+    """The smallest and the largest supported expansion orders (30: two passes over the output pairs in m2l_kernel, one
+    CTA per SM) and an odd one: the result is finite and its distance from the oracle is what the order allows."""
+    w = W.config(2, N=3000)
+    r = O.hsma(w)
+    phi, U = run_fmm(H, w, fmm_order=order, fmm_levels=2)
+    err = rel_inf(phi, r.phi)
+    assert np.all(np.isfinite(phi))
+    assert err <= {2: 3e-2, 7: 1e-4, 30: PHI_TOL}[order]
+    if order == 30:
+        assert abs(U - r.U) <= U_TOL * abs(r.U)
