@@ -418,7 +418,7 @@ def hsma_plan_set_timing(plan: int, enable: bool):
 
 PAIR_FORM_AUTO, PAIR_FORM_ORDERED, PAIR_FORM_SYMMETRIC = 0, 1, 2
 PAIR_FORM_FMM = 3               # reported by hsma_plan_last_pair_form when step (b) ran as the FMM
-NEAR_ALG_DIRECT, NEAR_ALG_FMM = 0, 1
+NEAR_ALG_DIRECT, NEAR_ALG_FMM, NEAR_ALG_AUTO = 0, 1, 2
 
 
 def hsma_plan_set_pair_form(plan: int, form: int):

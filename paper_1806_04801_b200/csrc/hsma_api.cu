@@ -350,6 +350,7 @@ struct hsma_plan {
     DevBuf<double> sym_col, sym_phi;   // symmetric form of step (b): column sums per visit of one wave, phi_near in source order
     size_t sym_col_cap = kSymColCapDefault;   // hsma_plan_set_sym_scratch_cap: bytes of column scratch per wave
     hsma::fmm::State fmm;              // near_algorithm = FMM: tables and scratch of the sub-quadratic form of step (b)
+    long long fmm_min_N = 0;           // near_algorithm = AUTO: the FMM from this N on
     int pair_form = 0;                 // hsma_plan_set_pair_form: 0 = automatic, 1 = ordered pairs only, 2 = symmetric wherever possible
     int last_pair_form = 1;            // what the last evaluate used for step (b): 1 ordered, 2 symmetric
     long long last_launches = 0;
@@ -419,7 +420,8 @@ extern "C" hsma_status hsma_plan_create_ex(const hsma_plan_desc* desc, void* cud
     if (d.dipole_mode != HSMA_DIPOLE_EXACT && d.dipole_mode != HSMA_DIPOLE_FD3) return HSMA_ERR_INVALID_ARG;
     if (d.near_mode == HSMA_NEAR_SPHERE && d.closure == HSMA_CLOSURE_FAR_DATA) return HSMA_ERR_INVALID_ARG;
     if (d.fd_dr_rel < 0.0 || d.fd_dr_rel > 0.1) return HSMA_ERR_INVALID_ARG;
-    if (d.near_algorithm != HSMA_NEAR_ALG_DIRECT && d.near_algorithm != HSMA_NEAR_ALG_FMM) return HSMA_ERR_INVALID_ARG;
+    if (d.near_algorithm != HSMA_NEAR_ALG_DIRECT && d.near_algorithm != HSMA_NEAR_ALG_FMM && d.near_algorithm != HSMA_NEAR_ALG_AUTO)
+        return HSMA_ERR_INVALID_ARG;
     for (int a = 0; a < 3; ++a)
         if (!(d.L[a] > 0.0) || d.near_shell[a] < 0 || d.near_shell[a] > 8) return HSMA_ERR_INVALID_ARG;
     if (d.kind == HSMA_BC_PERIODIC && d.closure == HSMA_CLOSURE_FAR_DATA) return HSMA_ERR_INVALID_ARG;
@@ -473,11 +475,13 @@ extern "C" hsma_status hsma_plan_create_ex(const hsma_plan_desc* desc, void* cud
         PCU(cudaMalloc(&p->img_dyn, 2 * sizeof(long long)));
         PCU(cudaMemsetAsync(p->img_dyn, 0, 2 * sizeof(long long), st));
     }
-    if (d.near_algorithm == HSMA_NEAR_ALG_FMM) {
+    if (d.near_algorithm == HSMA_NEAR_ALG_FMM || d.near_algorithm == HSMA_NEAR_ALG_AUTO) {
         bool refl[3];
         reflecting_axes(d.kind, refl);
         const hsma_status fs = fmm::setup(p->fmm, d, refl, st);
-        if (fs != HSMA_OK) { plan_free(p); return fs; }
+        if (fs != HSMA_OK && d.near_algorithm == HSMA_NEAR_ALG_FMM) { plan_free(p); return fs; }
+        if (fs != HSMA_OK) { p->fmm.release(); p->fmm.enabled = false; cudaGetLastError(); }   // AUTO: the direct sum serves this geometry
+        p->fmm_min_N = d.near_algorithm == HSMA_NEAR_ALG_AUTO ? 24576 : 0;
     }
     if (rhsc.empty()) { p->cells_rhs = p->cells_near; p->C_rhs = p->C_near; }
     else { p->C_rhs = (int)rhsc.size(); PCU(upload(&p->cells_rhs, rhsc, st)); }
@@ -775,7 +779,7 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
 
     // near_algorithm = FMM: step (b) over all N targets (potentials) by the fast multipole method; its
     // upward pass (leaf sort, P2M, M2M) comes first because step (a) can use the multipoles too
-    const bool use_fmm = p->fmm.enabled && phase == kPhaseAll && n_parts == 0 && t0 == 0 && t1 == N && p->pair_form == 0;
+    const bool use_fmm = p->fmm.enabled && N >= p->fmm_min_N && phase == kPhaseAll && n_parts == 0 && t0 == 0 && t1 == N && p->pair_form == 0;
     if (use_fmm) {
         hsma_status fs = fmm::upward(p->fmm, xyz, q, N, p->half, g_alloc_epoch, st);
         if (fs != HSMA_OK) return fs;
