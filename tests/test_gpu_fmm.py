@@ -219,3 +219,14 @@ def test_automatic_choice_of_the_near_algorithm(H):
     with H.Plan.from_workload(w, near_algorithm=H.binding.NEAR_ALG_AUTO) as plan:      # no cubic boxes: direct, not an error
         phi, U = plan.evaluate(dev(w.xyz), dev(w.q), sync=True)
         assert plan.last_pair_form == 2 and np.all(np.isfinite(phi.cpu().numpy()))
+
+
+@pytest.mark.parametrize("idx,N", [(2, 2), (3, 1), (3, 7), (2, 256), (3, 257)])
+def test_tiny_inputs(H, idx, N):
+    """One, two, seven sources (most leaves empty, a tile boundary at 256/257): the FMM path still meets the oracle."""
+    w = W.config(idx, N=N)
+    r = O.hsma(w)
+    for levels in (0, 2):
+        phi, U = run_fmm(H, w, oracle=r, fmm_levels=levels)
+        scale = max(np.max(np.abs(r.phi)), 1e-300)
+        assert np.max(np.abs(phi - r.phi)) <= PHI_TOL * scale and abs(U - r.U) <= U_TOL * abs(r.U)
