@@ -39,7 +39,9 @@ def run_fmm(H, w, oracle=None, **kw):
         phi, U = plan.evaluate(dev(w.xyz), dev(w.q), sync=True)
         assert plan.last_pair_form == FMM
         if oracle is not None:
-            assert rel_inf(plan.rhs().cpu().numpy(), oracle.rhs) <= 1e-10
+            # (not a north_star bar: a check target on a box face is the worst case of the a-priori bound of DESIGN.md 6.13,
+            # 1.3e-10 q/a per far source at order 20; with a few hundred sources nothing averages it down)
+            assert rel_inf(plan.rhs().cpu().numpy(), oracle.rhs) <= 1e-9
             assert rel_inf(plan.coeffs().cpu().numpy(), oracle.A) <= 1e-9
     return phi.cpu().numpy(), float(U)
 
