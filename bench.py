@@ -241,6 +241,12 @@ def run_b200(args, w) -> dict:
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if world != args.gpus:
         raise RuntimeError(f"--gpus {args.gpus} but WORLD_SIZE={world}: launch with torch.distributed.run")
+    # Rehearsal switch (tests only): HSMA_BENCH_SHARE_GPU=1 runs all ranks on cuda:0 over a gloo group, so that the whole
+    # N > 1 code path of this file -- rendezvous, barriers, shard.evaluate_distributed per step, max over ranks, rank-0
+    # line -- can be executed on a one-GPU box (NCCL refuses two ranks on one device).  Its numbers are not measurements.
+    share_gpu = world > 1 and os.environ.get("HSMA_BENCH_SHARE_GPU") == "1"
+    if share_gpu:
+        local = 0
     if local >= torch.cuda.device_count():
         raise RuntimeError(f"bench.py --gpus {args.gpus}: rank {rank} needs visible CUDA device {local}, but only "
                            f"{torch.cuda.device_count()} visible CUDA device(s) exist on this node")
@@ -250,7 +256,10 @@ def run_b200(args, w) -> dict:
     # evaluate into a CUDA graph (it does so only while stage timing is off)
     torch.cuda.set_stream(torch.cuda.Stream(device=dev))
     if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
+        if share_gpu:
+            dist.init_process_group("gloo")
+        else:
+            dist.init_process_group("nccl", device_id=dev)
     N = w.N
     t0, t1 = shard.shard_bounds(N, world)[rank]
     T = t1 - t0
@@ -324,7 +333,7 @@ def run_b200(args, w) -> dict:
     plan.set_timing(False)
     U_val = float(U.cpu()[0])
     if world > 1:
-        t = torch.tensor([ms], dtype=torch.float64, device=dev)
+        t = torch.tensor([ms], dtype=torch.float64, device="cpu" if share_gpu else dev)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         ms = float(t[0])
     stage_ms = {k: v / args.steps for k, v in stage_ms.items()}
@@ -368,7 +377,7 @@ def run_b200(args, w) -> dict:
     barrier()
     ms_e2e = 1e3 * (time.perf_counter() - tw) / n_e2e
     if world > 1:
-        t = torch.tensor([ms_e2e], dtype=torch.float64, device=dev)
+        t = torch.tensor([ms_e2e], dtype=torch.float64, device="cpu" if share_gpu else dev)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         ms_e2e = float(t[0])
     e2e = {"value": pairs_step / (ms_e2e * 1e-3), "unit": UNIT, "ms_per_step": ms_e2e, "steps": n_e2e,
@@ -462,6 +471,8 @@ def run_b200(args, w) -> dict:
            "energy": U_val, "stage_ms": stage_ms, "e2e": e2e, "gpu_launches": int(launches),
            "launches_per_step": plan.launches_last_evaluate(),
            "graph_replays": H.binding.hsma_plan_info(plan.handle)["graph_replays"], "clocks": clocks, "roofline": roofline}
+    if share_gpu:
+        out["rehearsal"] = "HSMA_BENCH_SHARE_GPU=1: all ranks on cuda:0 over a gloo group -- exercises the N > 1 code path, NOT a measurement"
     if fmm_arm:
         fi = H.binding.hsma_plan_fmm_info(plan.handle)
         out["config"]["near_algorithm"] = (f"fmm (order {fi['order']}, two-box separation, leaf level {fi['leaf_level']} = "

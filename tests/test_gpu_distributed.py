@@ -113,3 +113,30 @@ def test_bench_refuses_more_ranks_than_devices():
                         "--config", "2", "--no-cpu-baseline"], env=env, capture_output=True, text=True, timeout=600)
     assert p.returncode != 0
     assert "visible CUDA device" in (p.stderr + p.stdout)
+
+
+@pytest.mark.parametrize("extra", [[], ["--forces"], ["--size", "3000", "--config", "2"]])
+def test_bench_two_ranks_rehearsal_on_one_gpu(extra):
+    """bench.py --gpus 2 exactly as the driver launches it (torch.distributed.run, two ranks), with HSMA_BENCH_SHARE_GPU=1:
+    both ranks on cuda:0 over gloo.  The whole N > 1 path of bench.py runs -- rendezvous, barriers, one
+    shard.evaluate_distributed per step (PART form at N = 9,000; target shards at N = 3,000), max over ranks, end-to-end
+    leg, ONE JSON line from rank 0 with n_gpus = 2 -- and the energy agrees with the one-rank run."""
+    import json
+    import subprocess
+    base = [os.path.join(ROOT, "bench.py"), "--steps", "2", "--warmup", "1", "--no-cpu-baseline", "--e2e-steps", "1",
+            "--peak-seconds", "0.1"] + (extra if "--size" in extra else ["--size", "9000"] + extra)
+    env = dict(os.environ, HSMA_BENCH_SHARE_GPU="1")
+    port = 37100 + (os.getpid() + len(extra)) % 800
+    p2 = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr",
+                         "127.0.0.1", "--master-port", str(port)] + base + ["--gpus", "2"], env=env, capture_output=True, text=True,
+                        timeout=900)
+    assert p2.returncode == 0, p2.stderr[-2000:]
+    lines = [ln for ln in p2.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1, p2.stdout[-2000:]
+    d2 = json.loads(lines[0])
+    assert d2["n_gpus"] == 2 and d2["ms_per_step"] > 0 and d2["value"] > 0 and d2["gpu_launches"] > 0 and "rehearsal" in d2
+    p1 = subprocess.run([sys.executable] + base + ["--no-fmm-line"], capture_output=True, text=True, timeout=900)
+    assert p1.returncode == 0, p1.stderr[-2000:]
+    d1 = json.loads([ln for ln in p1.stdout.splitlines() if ln.startswith("{")][0])
+    assert abs(d2["energy"] - d1["energy"]) <= 1e-11 * abs(d1["energy"])
+    assert d2["config"]["pairs_per_step"] == d1["config"]["pairs_per_step"]
