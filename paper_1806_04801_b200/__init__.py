@@ -132,6 +132,14 @@ class Plan:
         """Bytes of column-sum scratch per wave of the symmetric form (0: default 64 MiB)."""
         binding.hsma_plan_set_sym_scratch_cap(self.handle, nbytes)
 
+    def set_image_factoring(self, on: bool):
+        """Lattice-factored image sums on (default) / off."""
+        binding.hsma_plan_set_image_factoring(self.handle, on)
+
+    @property
+    def image_factoring(self) -> bool:
+        return binding.hsma_plan_image_factoring(self.handle)
+
     @property
     def scratch_bytes(self) -> int:
         return binding.hsma_plan_scratch_bytes(self.handle)

@@ -108,6 +108,8 @@ _SIGNATURES = {
     "hsma_plan_last_pair_form": (ctypes.c_int, [ctypes.c_void_p]),
     "hsma_plan_set_sym_scratch_cap": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_longlong]),
     "hsma_plan_scratch_bytes": (ctypes.c_longlong, [ctypes.c_void_p]),
+    "hsma_plan_set_image_factoring": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int]),
+    "hsma_plan_image_factoring": (ctypes.c_int, [ctypes.c_void_p]),
     "hsma_plan_fmm_info": (ctypes.c_int, [ctypes.c_void_p, ctypes.POINTER(ctypes.c_longlong)]),
     "hsma_plan_get_timing": (ctypes.c_int, [ctypes.c_void_p, c_double_p]),
     "hsma_launch_count": (ctypes.c_longlong, []),
@@ -434,6 +436,16 @@ def hsma_plan_last_pair_form(plan: int) -> int:
 def hsma_plan_set_sym_scratch_cap(plan: int, nbytes: int):
     """Column-sum scratch per wave of the symmetric form, bytes (0: the default 64 MiB); include/hsma.h."""
     _check(load_library().hsma_plan_set_sym_scratch_cap(plan, int(nbytes)), "hsma_plan_set_sym_scratch_cap")
+
+
+def hsma_plan_set_image_factoring(plan: int, on: bool):
+    """Lattice-factored image sums on (default) / off; include/hsma.h."""
+    _check(load_library().hsma_plan_set_image_factoring(plan, 1 if on else 0), "hsma_plan_set_image_factoring")
+
+
+def hsma_plan_image_factoring(plan: int) -> bool:
+    """True if the lattice-factored kernels are in use for this plan."""
+    return bool(load_library().hsma_plan_image_factoring(plan))
 
 
 def hsma_plan_fmm_info(plan: int) -> dict:

@@ -14,7 +14,7 @@ ROOT = os.path.dirname(PKG)
 CSRC = os.path.join(PKG, "csrc")
 LIB = os.path.join(PKG, "libhsma_b200.so")
 SOURCES = ["hsma_api.cu"]
-HEADERS = ["common.cuh", "sum_kernels.cuh", "fit_kernels.cuh", "fmm_kernels.cuh", "fmm_host.cuh", "geometry.h", "peak.cuh"]
+HEADERS = ["common.cuh", "sum_kernels.cuh", "lattice_kernels.cuh", "fit_kernels.cuh", "fmm_kernels.cuh", "fmm_host.cuh", "geometry.h", "peak.cuh"]
 
 
 def nvcc_path() -> str:

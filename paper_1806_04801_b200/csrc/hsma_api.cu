@@ -15,6 +15,7 @@
 #include "hsma.h"
 #include "peak.cuh"
 #include "sum_kernels.cuh"
+#include "lattice_kernels.cuh"
 
 namespace hsma {
 std::atomic<long long> g_launches{0};
@@ -304,6 +305,15 @@ static void launch_node(const Launch& L, bool field, const double* tgt, int tstr
 
 using namespace hsma;
 
+// Lattice-factored kernels (lattice_kernels.cuh): the shapes instantiated, by (near_shell, reflecting axes).
+static int lat_shape_of(const int shell[3], const bool refl[3]) {
+    const int mask = (refl[0] ? 1 : 0) | (refl[1] ? 2 : 0) | (refl[2] ? 4 : 0);
+    if (shell[0] == 1 && shell[1] == 1 && shell[2] == 1 && mask == 0) return 1;
+    if (shell[0] == 1 && shell[1] == 1 && shell[2] == 1 && mask == 7) return 2;
+    if (shell[0] == 1 && shell[1] == 1 && shell[2] == 2 && mask == 4) return 3;
+    return 0;
+}
+
 struct hsma_plan {
     hsma_plan_desc d;
     cudaStream_t stream = nullptr;
@@ -348,6 +358,9 @@ struct hsma_plan {
     QInfo* qinfo = nullptr;
     DevBuf<double> part_a, part_b, part_c, red, xyz_in, q_in, phi_dev, force_dev;
     DevBuf<double> sym_col, sym_phi;   // symmetric form of step (b): column sums per visit of one wave, phi_near in source order
+    int lat_shape = 0;           // lattice-factored kernels (lattice_kernels.cuh): 0 none, else index into the instantiated shapes
+    bool lat_on = true;          // hsma_plan_set_image_factoring
+    LatGeom lat;                 // shifts k L_a and gamma^m (unscaled)
     size_t sym_col_cap = kSymColCapDefault;   // hsma_plan_set_sym_scratch_cap: bytes of column scratch per wave
     hsma::fmm::State fmm;              // near_algorithm = FMM: tables and scratch of the sub-quadratic form of step (b)
     long long fmm_min_N = 0;           // near_algorithm = AUTO: the FMM from this N on
@@ -463,6 +476,14 @@ extern "C" hsma_status hsma_plan_create_ex(const hsma_plan_desc* desc, void* cud
     if ((int)near.size() > kMaxCells || (int)rhsc.size() > kMaxCells) { plan_free(p); return HSMA_ERR_INVALID_ARG; }
     p->C_near = (int)near.size();
     PCU(upload(&p->cells_near, near, st));
+    {
+        bool refl[3];
+        reflecting_axes(d.kind, refl);
+        p->lat_shape = p->sphere ? 0 : lat_shape_of(d.near_shell, refl);
+        for (int a = 0; a < 3; ++a)
+            for (int k = -2; k <= 2; ++k) p->lat.sh[a][k + 2] = k * d.L[a];
+        for (int m = 0; m < 8; ++m) p->lat.wpow[m] = m == 0 ? 1.0 : std::pow(d.gamma, (double)m);
+    }
     if (p->sphere) {
         Cell id;
         id.sx = id.sy = id.sz = 0.0; id.w = 1.0; id.fx = id.fy = id.fz = 0; id.central = 1;
@@ -652,6 +673,19 @@ __global__ void node_positions_kernel(const double* __restrict__ nrm, double R, 
 //   kPhaseCheck   H1 + step (a) for the check targets c0 <= i < c1 only, into the plan's pc (pcg); nothing else
 //   kPhaseRest    H1 + fit + mapping + (b) + (c) + finish with the plan's pc (pcg) AS THEY ARE (hsma_set_check_sums)
 enum { kPhaseAll = 0, kPhaseCheck = 1, kPhaseRest = 2 };
+static bool lat_applies(const hsma_plan* p, const Cell* cells) { return p->lat_on && p->lat_shape != 0 && cells == p->cells_near; }
+static void launch_lat_sym(int shape, int refine, int G, const SymArgs& a, const LatGeom& g, cudaStream_t st) {
+#define HSMA_LAT_SYM(SX, SY, SZ, MASK)                                                              \
+    do {                                                                                            \
+        if (refine == 1) near_lat_sym_kernel<1, SX, SY, SZ, MASK><<<G, kThreads, 0, st>>>(a, g);    \
+        else near_lat_sym_kernel<2, SX, SY, SZ, MASK><<<G, kThreads, 0, st>>>(a, g);                \
+    } while (0)
+    if (shape == 1) HSMA_LAT_SYM(1, 1, 1, 0);
+    else if (shape == 2) HSMA_LAT_SYM(1, 1, 1, 7);
+    else HSMA_LAT_SYM(1, 1, 2, 4);
+#undef HSMA_LAT_SYM
+}
+
 // Buffers of the symmetric form (row partials and column sums of ONE wave, near sum in source order); comps = 4 with
 // the gradient.  Bounded by the plan's cap on the column scratch: O(N) in all.
 static cudaError_t reserve_sym(hsma_plan* p, const SymLaunch& ss, long long N, size_t comps) {
@@ -669,6 +703,9 @@ static void launch_sym(hsma_plan* p, const SymLaunch& ss, bool field, int refine
     a.scale = refine == 1 ? 0.5 : 1.0; a.scale_grad = refine == 1 ? -0.25 : -1.0;
     a.part = p->part_b.p; a.col = p->sym_col.p;
     const unsigned gb = (unsigned)((N + 255) / 256);
+    const bool lat = !field && lat_applies(p, cells);
+    LatGeom lg = p->lat;
+    for (int m = 0; m < 8; ++m) lg.wpow[m] *= a.scale;
     if (ss.n_waves == 0) {   // a part with no fine units: its share of the near sum is zero
         cudaMemsetAsync(p->sym_phi.p, 0, (size_t)N * (field ? 4 : 1) * sizeof(double), st);
         return;
@@ -682,7 +719,8 @@ static void launch_sym(hsma_plan* p, const SymLaunch& ss, bool field, int refine
             HSMA_COUNT_LAUNCH();
             sym_gather_field_kernel<<<gb, 256, 0, st>>>(p->part_b.p, p->sym_col.p, p->slot_of.p, N, n_tiles, W, p->sym_phi.p);
         } else {
-            if (refine == 1) near_sym_kernel<1><<<W.G, kThreads, 0, st>>>(a);
+            if (lat) launch_lat_sym(p->lat_shape, refine, W.G, a, lg, st);
+            else if (refine == 1) near_sym_kernel<1><<<W.G, kThreads, 0, st>>>(a);
             else near_sym_kernel<2><<<W.G, kThreads, 0, st>>>(a);
             HSMA_COUNT_LAUNCH();
             sym_gather_kernel<<<gb, 256, 0, st>>>(p->part_b.p, p->sym_col.p, p->slot_of.p, N, n_tiles, W, p->sym_phi.p);
@@ -1355,6 +1393,13 @@ extern "C" hsma_status hsma_plan_set_sym_scratch_cap(hsma_plan* p, long long byt
     ++g_alloc_epoch;   // a captured evaluate graph holds the old wave structure
     return HSMA_OK;
 }
+extern "C" hsma_status hsma_plan_set_image_factoring(hsma_plan* p, int on) {
+    if (!p || on < 0 || on > 1) return HSMA_ERR_INVALID_ARG;
+    p->lat_on = on != 0;
+    ++g_alloc_epoch;   // a captured evaluate graph holds the other kernels
+    return HSMA_OK;
+}
+extern "C" int hsma_plan_image_factoring(const hsma_plan* p) { return p && p->lat_on && p->lat_shape != 0 ? 1 : 0; }
 extern "C" long long hsma_plan_scratch_bytes(const hsma_plan* p) {
     if (!p) return 0;
     size_t b = p->src.cap * sizeof(Src4) + (p->slot_of.cap + p->tile_np.cap) * sizeof(int) +
