@@ -483,6 +483,11 @@ extern "C" hsma_status hsma_plan_create_ex(const hsma_plan_desc* desc, void* cud
         for (int a = 0; a < 3; ++a)
             for (int k = -2; k <= 2; ++k) p->lat.sh[a][k + 2] = k * d.L[a];
         for (int m = 0; m < 8; ++m) p->lat.wpow[m] = m == 0 ? 1.0 : std::pow(d.gamma, (double)m);
+        for (int a = 0; a < 3; ++a)
+            for (int k = -2; k <= 2; ++k) p->lat.wa[a][k + 2] = (refl[a] && k != 0) ? std::pow(d.gamma, (double)std::abs(k)) : 1.0;
+        for (int i = 0; i < 5; ++i)
+            for (int j = 0; j < 5; ++j) p->lat.wxy[i][j] = p->lat.wa[0][i] * p->lat.wa[1][j];
+        p->lat.cgrad = 1.0;
     }
     if (p->sphere) {
         Cell id;
@@ -685,6 +690,26 @@ static void launch_lat_sym(int shape, int refine, int G, const SymArgs& a, const
     else HSMA_LAT_SYM(1, 1, 2, 4);
 #undef HSMA_LAT_SYM
 }
+template <int REFINE, int SX, int SY, int SZ, int MASK>
+static void launch_lat_sym_field_of(int G, const SymArgs& a, const LatGeom& g, cudaStream_t st) {
+    static bool opted = false;   // > 48 KB of dynamic shared memory: opt in once per instantiation
+    if (!opted) {
+        cudaFuncSetAttribute(near_lat_sym_field_kernel<REFINE, SX, SY, SZ, MASK>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLatFieldDynSmem);
+        opted = true;
+    }
+    near_lat_sym_field_kernel<REFINE, SX, SY, SZ, MASK><<<G, kThreads, kLatFieldDynSmem, st>>>(a, g);
+}
+static void launch_lat_sym_field(int shape, int refine, int G, const SymArgs& a, const LatGeom& g, cudaStream_t st) {
+#define HSMA_LAT_SYMF(SX, SY, SZ, MASK)                                                 \
+    do {                                                                                \
+        if (refine == 1) launch_lat_sym_field_of<1, SX, SY, SZ, MASK>(G, a, g, st);     \
+        else launch_lat_sym_field_of<2, SX, SY, SZ, MASK>(G, a, g, st);                 \
+    } while (0)
+    if (shape == 1) HSMA_LAT_SYMF(1, 1, 1, 0);
+    else if (shape == 2) HSMA_LAT_SYMF(1, 1, 1, 7);
+    else HSMA_LAT_SYMF(1, 1, 2, 4);
+#undef HSMA_LAT_SYMF
+}
 
 // Buffers of the symmetric form (row partials and column sums of ONE wave, near sum in source order); comps = 4 with
 // the gradient.  Bounded by the plan's cap on the column scratch: O(N) in all.
@@ -703,9 +728,10 @@ static void launch_sym(hsma_plan* p, const SymLaunch& ss, bool field, int refine
     a.scale = refine == 1 ? 0.5 : 1.0; a.scale_grad = refine == 1 ? -0.25 : -1.0;
     a.part = p->part_b.p; a.col = p->sym_col.p;
     const unsigned gb = (unsigned)((N + 255) / 256);
-    const bool lat = !field && lat_applies(p, cells);
+    const bool lat = lat_applies(p, cells);
     LatGeom lg = p->lat;
     for (int m = 0; m < 8; ++m) lg.wpow[m] *= a.scale;
+    lg.cgrad = refine == 1 ? 0.125 : 1.0;
     if (ss.n_waves == 0) {   // a part with no fine units: its share of the near sum is zero
         cudaMemsetAsync(p->sym_phi.p, 0, (size_t)N * (field ? 4 : 1) * sizeof(double), st);
         return;
@@ -714,7 +740,8 @@ static void launch_sym(hsma_plan* p, const SymLaunch& ss, bool field, int refine
         const SymWave W = sym_wave(ss, n_tiles, w);
         a.f_begin = W.f_begin; a.fine = W.fine; a.v_base = W.v_base; a.blk_base = W.blk_lo; a.part_blocks = W.blk_hi - W.blk_lo + 1;
         if (field) {
-            if (refine == 1) near_sym_field_kernel<1><<<W.G, kThreads, kSymFieldDynSmem, st>>>(a);
+            if (lat) launch_lat_sym_field(p->lat_shape, refine, W.G, a, lg, st);
+            else if (refine == 1) near_sym_field_kernel<1><<<W.G, kThreads, kSymFieldDynSmem, st>>>(a);
             else near_sym_field_kernel<2><<<W.G, kThreads, kSymFieldDynSmem, st>>>(a);
             HSMA_COUNT_LAUNCH();
             sym_gather_field_kernel<<<gb, 256, 0, st>>>(p->part_b.p, p->sym_col.p, p->slot_of.p, N, n_tiles, W, p->sym_phi.p);
