@@ -183,6 +183,44 @@ static void launch_near(const Launch& L, bool field, const double* tgt, int tstr
         if (a.qinfo) launch_near_form<true, false>(L, refine, a, st);
     }
 }
+// Ordered pairs, lattice-factored (lattice_kernels.cuh near_lat_sum_kernel): R in {2, 1} -- the 27+ image chains of one
+// pair already fill the FP64 pipe, so more targets per thread buy nothing -- and units of kLatChunk sources.
+using LatNearFn = void (*)(const NearArgs, const LatGeom);
+static LatNearFn lat_near_fn(int R, int refine, bool field, int shape) {
+#define HSMA_LAT_SHAPE(RR, RF, FD)                                                          \
+    (shape == 1 ? (LatNearFn)near_lat_sum_kernel<RR, RF, FD, 1, 1, 1, 0>                    \
+                : shape == 2 ? (LatNearFn)near_lat_sum_kernel<RR, RF, FD, 1, 1, 1, 7>       \
+                             : (LatNearFn)near_lat_sum_kernel<RR, RF, FD, 1, 1, 2, 4>)
+    if (R == 2) {
+        if (refine == 1) return field ? HSMA_LAT_SHAPE(2, 1, true) : HSMA_LAT_SHAPE(2, 1, false);
+        return field ? HSMA_LAT_SHAPE(2, 2, true) : HSMA_LAT_SHAPE(2, 2, false);
+    }
+    if (refine == 1) return field ? HSMA_LAT_SHAPE(1, 1, true) : HSMA_LAT_SHAPE(1, 1, false);
+    return field ? HSMA_LAT_SHAPE(1, 2, true) : HSMA_LAT_SHAPE(1, 2, false);
+#undef HSMA_LAT_SHAPE
+}
+static int lat_near_resident(int R, int refine, bool field, int shape) {
+    static int cache[2][2][2][4] = {};
+    int& c = cache[R == 2 ? 1 : 0][refine == 1 ? 0 : 1][field ? 1 : 0][shape];
+    if (!c) c = resident_ctas(lat_near_fn(R, refine, field, shape));
+    return c;
+}
+static Launch choose_near_lat(long long T, long long n_tiles, int refine, bool field, int shape) {
+    return choose_launch(T, n_tiles * kLatChunks, 2, [=](int R) { return lat_near_resident(R, refine, field, shape); });
+}
+static void launch_near_lat(const Launch& L, bool field, const double* tgt, int tstride, const int* tgt_index, long long T,
+                            long long t_first, const Packed& P, long long self_offset, int refine, int shape, LatGeom g,
+                            double* part, cudaStream_t st) {
+    NearArgs a;
+    a.tgt = tgt; a.tstride = tstride; a.tgt_index = tgt_index; a.T = T; a.t_first = t_first;
+    a.src = P.src; a.n_src = P.n_src; a.n_tiles = P.n_tiles; a.tile_np = P.tile_np; a.slot_of = P.slot_of; a.qinfo = nullptr;
+    a.cells = nullptr; a.C = kLatChunks; a.units = L.U; a.self_offset = self_offset; a.dyn = nullptr; a.ntb = L.ntb;
+    a.scale = refine == 1 ? 0.5 : 1.0; a.scale_grad = 0.0; a.part = part;
+    for (int m = 0; m < 8; ++m) g.wpow[m] *= a.scale;
+    g.cgrad = refine == 1 ? 0.125 : 1.0;
+    lat_near_fn(L.R, refine, field, shape)<<<L.G, kThreads, 0, st>>>(a, g);
+    HSMA_COUNT_LAUNCH();
+}
 static Launch choose_near(long long T, long long n_tiles, int C, int refine, bool field = false) {
     return choose_launch(T, n_tiles * C, field ? 4 : 8, [refine, field](int R) { return near_resident(R, refine, field); });
 }
@@ -866,10 +904,13 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
     } else if (phase != kPhaseRest && c1 > c0) {
         const long long Tc = c1 - c0;
         const bool fa = p->need_grad;   // derivative rows need grad Phi_in at the check targets: the FIELD form of (a)
-        const Launch s = choose_near(Tc, n_tiles_near, C_a, 2, fa);
+        const bool lat_a = lat_applies(p, cells_a);
+        const Launch s = lat_a ? choose_near_lat(Tc, n_tiles_near, 2, fa, p->lat_shape) : choose_near(Tc, n_tiles_near, C_a, 2, fa);
         if (p->part_a.reserve((size_t)rows_for(s, C_a) * Tc * (fa ? 4 : 1)) != cudaSuccess) return HSMA_ERR_ALLOC;
         MARK(1);
-        launch_near(s, fa, p->chk, 3, nullptr, Tc, c0, P, cells_a, C_a, -1, 2, p->part_a.p, st);  // (a) always cubic: it feeds the fit
+        // (a) always cubic: it feeds the fit
+        if (lat_a) launch_near_lat(s, fa, p->chk, 3, nullptr, Tc, c0, P, -1, 2, p->lat_shape, p->lat, p->part_a.p, st);
+        else launch_near(s, fa, p->chk, 3, nullptr, Tc, c0, P, cells_a, C_a, -1, 2, p->part_a.p, st);
         MARK(2);
         if (fa)
             finish_field_kernel<<<(unsigned)((Tc + 255) / 256), 256, 0, st>>>(s.layout(p->part_a.p, dyn, C_a), PartLayout{nullptr, 1, 1, 1, 1}, Tc, nullptr, nullptr, 0, p->pc + c0, p->pcg + 3 * c0, nullptr);
@@ -935,7 +976,8 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
         // rsqrt_refine = 0: the cubic step while (b) is latency-bound anyway (< 2^32 pairs), Newton above
         const size_t comps = field ? 4 : 1;
         bool sym = !use_fmm && !p->sphere && p->pair_form != 1 && t0 == 0 && t1 == N && sym_applies(n_tiles, C_b);
-        Launch sb = choose_near(T, n_tiles_near, C_b, refine, field);
+        const bool lat_b = lat_applies(p, cells_b);
+        Launch sb = lat_b ? choose_near_lat(T, n_tiles_near, refine, field, p->lat_shape) : choose_near(T, n_tiles_near, C_b, refine, field);
         if (use_fmm && p->sym_phi.reserve((size_t)N * comps) != cudaSuccess) return HSMA_ERR_ALLOC;
         SymLaunch ss{};
         if (sym) {
@@ -961,6 +1003,9 @@ static hsma_status evaluate_impl(hsma_plan* p, const double* xyz, const double* 
             // every unordered (source, source) pair once: row sums + column sums, then phi_near in source order
             launch_sym(p, ss, field, refine, cells_b, C_b, N, n_tiles, st);
             layout_b = PartLayout{p->sym_phi.p, 1, 1, 1, (int)std::min<long long>(T, 2147483647LL)};
+        } else if (lat_b) {
+            launch_near_lat(sb, field, reinterpret_cast<const double*>(p->src.p), 4, p->slot_of.p, T, t0, P, t0, refine,
+                            p->lat_shape, p->lat, p->part_b.p, st);
         } else {
             launch_near(sb, field, reinterpret_cast<const double*>(p->src.p), 4, p->slot_of.p, T, t0, P, cells_b, C_b,
                         t0, refine, p->part_b.p, st);

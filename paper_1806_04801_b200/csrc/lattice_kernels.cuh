@@ -445,4 +445,136 @@ __global__ void __launch_bounds__(kThreads, 1) near_lat_sym_field_kernel(const S
     if (!fresh) store_block(I);
 }
 
+// ---- ordered pairs (steps (a) and (b) of near_sum_kernel), lattice-factored ---------------------------------------
+// Same targets, partial-row layout and grid logic as near_sum_kernel (sum_kernels.cuh), with one difference: a unit is
+// (target block, source tile, chunk of kLatChunk sources) -- all cells of the chunk -- instead of (block, tile, cell),
+// so the host passes a.C = kLatChunks.  a.cells, a.qinfo and a.tile_np are not read (the charges enter once per pair,
+// so there is nothing to gain from the sign-sorted tiles here).
+constexpr int kLatChunk = 8;
+constexpr int kLatChunks = kTile / kLatChunk;
+
+template <int R, int REFINE, bool FIELD, int SX, int SY, int SZ, int MASK>
+__global__ void __launch_bounds__(kThreads, 1) near_lat_sum_kernel(const NearArgs a, const LatGeom g) {
+    __shared__ __align__(128) Src4 tile[kStages][kTile];
+    __shared__ __align__(8) uint64_t full[kStages];
+
+    const int tid = threadIdx.x;
+    const int G = gridDim.x, k = blockIdx.x;
+    const long long u0 = unit_start(k, a.units, G), u1 = unit_start(k + 1, a.units, G);
+    if (u1 <= u0) return;
+    const long long Ub = a.n_tiles * kLatChunks;
+    const long long V0 = u0 / kLatChunks, V1 = (u1 - 1) / kLatChunks;
+
+    if (tid == 0) {
+        for (int s = 0; s < kStages; ++s) mbar_init(&full[s], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    if (tid == 0) {
+        mbar_expect_tx(&full[0], kTile * sizeof(Src4));
+        bulk_g2s(tile[0], a.src + (V0 % a.n_tiles) * kTile, kTile * sizeof(Src4), &full[0]);
+    }
+
+    constexpr int RG = FIELD ? R : 1;
+    double ox[R], oy[R], oz[R], tot[R];
+    double totx[RG], toty[RG], totz[RG];
+    const int nvis = (int)(V1 - V0) + 1;
+    const int nt = (int)a.n_tiles;
+    int b = (int)(V0 / a.n_tiles), tl = (int)(V0 - (long long)b * a.n_tiles);
+    const int c_first = (int)(u0 - V0 * kLatChunks), c_last = (int)(u1 - 1 - V1 * kLatChunks) + 1;
+    const double cphi = a.scale, cg = -g.cgrad;
+    bool fresh = true;
+    auto store_block = [&](int blk) {
+        const int row = k - cta_of_unit(blk * Ub, a.units, G);
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const long long t = (long long)blk * (kThreads * R) + r * kThreads + tid;
+            if (t < a.T) {
+                if (FIELD) {
+                    double* o = a.part + (long long)row * 4 * a.T + t;
+                    o[0] = cphi * tot[r]; o[a.T] = cg * totx[r % RG]; o[2 * a.T] = cg * toty[r % RG]; o[3 * a.T] = cg * totz[r % RG];
+                } else {
+                    a.part[(long long)row * a.T + t] = tot[r];
+                }
+            }
+        }
+    };
+
+    for (int it = 0; it < nvis; ++it) {
+        const int st = it & 1;
+        if (tid == 0 && it + 1 < nvis) {
+            const int tn = tl + 1 == nt ? 0 : tl + 1;
+            mbar_expect_tx(&full[st ^ 1], kTile * sizeof(Src4));
+            bulk_g2s(tile[st ^ 1], a.src + (long long)tn * kTile, kTile * sizeof(Src4), &full[st ^ 1]);
+        }
+        const long long tb = (long long)b * (kThreads * R);
+        if (fresh) {
+            fresh = false;
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                long long t = a.t_first + min(tb + r * kThreads + tid, a.T - 1);
+                if (a.tgt_index) t = a.tgt_index[t];
+                const double* p = a.tgt + t * a.tstride;
+                ox[r] = p[0]; oy[r] = p[1]; oz[r] = p[2];
+                tot[r] = 0.0;
+                if (FIELD) { totx[r % RG] = 0.0; toty[r % RG] = 0.0; totz[r % RG] = 0.0; }
+            }
+        }
+        mbar_wait(&full[st], (it >> 1) & 1);
+        const Src4* __restrict__ s = tile[st];
+        const long long j0 = (long long)tl * kTile;
+        const long long self_lo = a.self_offset + tb, self_hi = a.self_offset + min(a.T, tb + (long long)kThreads * R);
+        const bool tile_has_self = a.self_offset >= 0 && j0 < self_hi && j0 + kTile > self_lo;
+        const int j_lo = (it == 0 ? c_first : 0) * kLatChunk;
+        const int j_hi = (it == nvis - 1 ? c_last : kLatChunks) * kLatChunk;
+
+        if (tile_has_self) {
+            int sj[R];
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const long long i = a.self_offset + min(tb + r * kThreads + tid, a.T - 1);
+                const long long slot = a.slot_of ? (long long)a.slot_of[i] : i;
+                sj[r] = (int)max(-1LL, min((long long)kTile, slot - j0));
+            }
+#pragma unroll 1
+            for (int j = j_lo; j < j_hi; ++j) {
+                const double2 xy = *reinterpret_cast<const double2*>(&s[j].x);
+                const double2 zq = *reinterpret_cast<const double2*>(&s[j].z);
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    if (FIELD) {
+                        const LatField f = lat_sum_field<REFINE, SX, SY, SZ, MASK, true>(g, ox[r], oy[r], oz[r], xy.x, xy.y, zq.x, j == sj[r]);
+                        tot[r] = fma(zq.y, f.p, tot[r]);
+                        totx[r % RG] = fma(zq.y, f.tx, totx[r % RG]); toty[r % RG] = fma(zq.y, f.ty, toty[r % RG]); totz[r % RG] = fma(zq.y, f.tz, totz[r % RG]);
+                    } else {
+                        tot[r] = fma(zq.y, lat_sum<REFINE, SX, SY, SZ, MASK, true>(g, ox[r], oy[r], oz[r], xy.x, xy.y, zq.x, j == sj[r]), tot[r]);
+                    }
+                }
+            }
+        } else {
+#pragma unroll 1
+            for (int j = j_lo; j < j_hi; ++j) {
+                const double2 xy = *reinterpret_cast<const double2*>(&s[j].x);
+                const double2 zq = *reinterpret_cast<const double2*>(&s[j].z);
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    if (FIELD) {
+                        const LatField f = lat_sum_field<REFINE, SX, SY, SZ, MASK, false>(g, ox[r], oy[r], oz[r], xy.x, xy.y, zq.x, false);
+                        tot[r] = fma(zq.y, f.p, tot[r]);
+                        totx[r % RG] = fma(zq.y, f.tx, totx[r % RG]); toty[r % RG] = fma(zq.y, f.ty, toty[r % RG]); totz[r % RG] = fma(zq.y, f.tz, totz[r % RG]);
+                    } else {
+                        tot[r] = fma(zq.y, lat_sum<REFINE, SX, SY, SZ, MASK, false>(g, ox[r], oy[r], oz[r], xy.x, xy.y, zq.x, false), tot[r]);
+                    }
+                }
+            }
+        }
+        __syncthreads();  // everyone is done with tile[st] before it is refilled
+        if (++tl == nt) {
+            store_block(b);
+            tl = 0; ++b; fresh = true;
+        }
+    }
+    if (!fresh) store_block(b);
+}
+
 }  // namespace hsma
