@@ -56,6 +56,31 @@ FLOPS_EVAL_SYM_FIELD = 35.0
 EXEC_EVAL_SYM_FIELD = {1: (21.0 + 11.0 / 8.0, 33.0 + 18.0 / 8.0), 2: (23.0 + 11.0 / 8.0, 37.0 + 18.0 / 8.0)}
 
 
+# Lattice-factored kernels (csrc/lattice_kernels.cuh): the unit is still one image-pair evaluation, but
+# its r^2 comes from per-axis squares shared by all images of the (target, source) pair and the charges enter once per
+# pair.  Counted from the formulation (and checked against the SASS of the inner loop, profiles/r02_sass_opcodes.md):
+#   per image   : r^2 = z-square + (x-square + y-square) [DFMA], y0^2 [DMUL], Newton factor [DFMA], accumulate [DFMA]
+#                 (+ 2 DFMA for the cubic step)
+#   per pair    : offsets (1 + 2 s_a [+ 1 on a reflecting axis] DADD per axis), x squares (2 s_x + 1 DMUL),
+#                 x-square + y-square (DFMA per (kx, ky)), weight classes (1 DMUL + DFMA per further class),
+#                 row and column accumulation (2 DFMA; 1 for ordered pairs)
+# Gradient forms: measured on the 27-cell periodic shape (10.22 instructions / 15.15 flops per image, Newton).
+def lat_counts(shell, reflecting, refine: int, field: bool, symmetric: bool):
+    """(FP64-pipe instructions, flops) executed per image-pair evaluation by the lattice-factored kernels."""
+    sx, sy, sz = shell
+    images = (2 * sx + 1) * (2 * sy + 1) * (2 * sz + 1)
+    if field:
+        instr, flops = 10.22, 15.15
+        return (instr + (2.0 if refine == 2 else 0.0), flops + (4.0 if refine == 2 else 0.0))
+    classes = 1 + sum(s for s, r in zip(shell, reflecting) if r)
+    dadd = sum(1 + 2 * s + (1 if r else 0) for s, r in zip(shell, reflecting))
+    dmul = (2 * sx + 1) + 1
+    dfma = (2 * sx + 1) * (2 * sy + 1) + (classes - 1) + (2 if symmetric else 1)
+    per_img_instr = 4 + (2 if refine == 2 else 0)
+    per_img_flops = 7 + (4 if refine == 2 else 0)
+    return (per_img_instr + (dadd + dmul + dfma) / images, per_img_flops + (dadd + dmul + 2 * dfma) / images)
+
+
 def sym_evaluations(N: int, C: int) -> int:
     """Pair evaluations of one near_sym_kernel launch (csrc/sum_kernels.cuh: visits x tile x block x cells; the
     diagonal visits and the padding of the last block are evaluated like the rest and counted here)."""
@@ -274,6 +299,8 @@ def run_b200(args, w) -> dict:
                                 fmm_levels=args.fmm_levels)
     if args.pair_form != "auto":
         plan.set_pair_form(1 if args.pair_form == "ordered" else 2)
+    if args.image_factoring == "off":
+        plan.set_image_factoring(False)
     info = plan.info
     refine = args.refine   # 0: resolved after the warm-up (the library decides by the pair count)
     xyz = torch.as_tensor(np.ascontiguousarray(w.xyz), device=dev)
@@ -428,6 +455,22 @@ def run_b200(args, w) -> dict:
         kernel_name = (f"near_sum_kernel<R,{refine},{'uniform-|q|' if uniform_q else 'generic'},"
                        f"{'field' if args.forces else 'potential'}> step (b)")
         unit_name = "ordered pair interactions"
+    lattice = bool(plan.image_factoring) and plan.last_pair_form in (1, 2)
+    frac_survey = None
+    if lattice:
+        # the factored form needs fewer flops per image pair than SURVEY.md 8(d)'s per-pair count, so 18 x units / time can
+        # exceed the FP64 peak: that figure is kept as frac_survey_8d_count (a comparison with the cell-by-cell kernels, not
+        # a roofline); `frac` charges the factored formulation's own count
+        refl = {W.BC_PERIODIC: (False, False, False), W.BC_MIRROR_CAVITY: (True, True, True),
+                W.BC_SLAB_XY_PERIODIC_Z_MIRROR: (False, False, True)}[int(w.kind)]
+        frac_survey = ach_tf / peak_tf
+        ex_instr, ex_flops = lat_counts(tuple(int(x) for x in w.near_shell), refl, refine, bool(args.forces), symmetric)
+        alg_flops = ex_flops
+        ach_tf = units * alg_flops / (k_ms * 1e-3) * 1e-12 if k_ms > 0 else 0.0
+        kernel_name = (("near_lat_sym_field_kernel" if args.forces else "near_lat_sym_kernel") if symmetric else "near_lat_sum_kernel") + \
+            f"<refine {refine}, shell {tuple(int(x) for x in w.near_shell)}> step (b), lattice-factored image sums" + \
+            (", symmetric form: each unordered pair evaluated once" if symmetric else "")
+        unit_name = ("image-pair evaluations (one source pair in one image cell" + (", feeding phi_i and phi_j)" if symmetric else ")"))
     roofline = {"bound": "alu", "kernel": kernel_name, "achieved": ach_tf, "peak": peak_tf,
                 "unit": "TFLOP/s", "frac": ach_tf / peak_tf, "traffic": traffic,
                 "traffic_source": traffic_source if traffic else None,
@@ -445,7 +488,17 @@ def run_b200(args, w) -> dict:
                                    "SURVEY.md 8(d)'s count for one charge pair (18; 26 with the gradient), applied to what the "
                                    "kernel evaluates (units); peak = derived FP64 FMA peak")
     roofline["evaluations_per_s"] = units / (k_ms * 1e-3) if k_ms > 0 else 0.0
-    if symmetric:
+    if lattice:
+        roofline["frac_definition"] = ("achieved = units_per_launch x flops_per_unit_algorithmic / kernel time; the lattice-factored "
+                                       "formulation (DESIGN.md 6.14) shares the per-axis squares between all images of a pair, so its "
+                                       "algorithmic count per image pair is what it executes (flops_per_unit_algorithmic = "
+                                       "flops_per_unit_executed); peak = derived FP64 FMA peak.  fp64_pipe_issue_util is the measure of "
+                                       "kernel quality: FP64 instructions issued / (SMs x 64 lanes x clock)")
+        roofline["frac_survey_8d_count"] = frac_survey
+        roofline["frac_survey_8d_count_note"] = ("SURVEY.md 8(d)'s 18 flops (26 with the gradient) x units / time / peak: what the "
+                                                 "cell-by-cell kernels were charged; above 1 here because the factoring removes "
+                                                 "work, not a roofline")
+    if symmetric and not lattice:
         roofline["frac_with_second_accumulation"] = units * alg_flops_2nd / (k_ms * 1e-3) * 1e-12 / peak_tf if k_ms > 0 else 0.0
         roofline["flops_per_unit_with_second_accumulation"] = alg_flops_2nd
         roofline["launches_per_step_of_this_kernel"] = "waves: the unordered pairs are walked in ceil(column scratch / cap) launches, each followed by a gather (in kernel_ms)"
@@ -458,6 +511,7 @@ def run_b200(args, w) -> dict:
            "data": "synthetic",
            "config": {"workload": w.name, "N": N, "near_cells": info["near_cells"], "p": info["p"], "M": info["M"],
                       "check_targets": info["check_targets"], "pairs_per_step": pc_all, "rsqrt_refine": refine, "forces": bool(args.forces),
+                      "image_factoring": bool(plan.image_factoring),
                       "pair_form": "symmetric (each unordered source pair evaluated once; value counts the ordered pair interactions it accounts for)"
                                    if plan.last_pair_form == 2 else "ordered",
                       "parallelism": (f"check-point sums, unordered pairs of (b) and targets of (c) split over {world} rank(s), "
@@ -588,6 +642,9 @@ def main():
     ap.add_argument("--face-pairs", action="store_true",
                     help="periodic configs: close by seeded value+derivative pairs on opposite faces instead of the "
                          "paper's circumsphere rule (DESIGN.md 6.10)")
+    ap.add_argument("--image-factoring", choices=["on", "off"], default="on",
+                    help="off: the cell-by-cell pair kernels everywhere (DESIGN.md 6.1, 6.12) instead of the lattice-factored "
+                         "ones (6.14) -- for comparison")
     ap.add_argument("--pair-form", choices=["auto", "ordered", "symmetric"], default="auto",
                     help="step (b): auto = symmetric form (each unordered pair once) when one rank evaluates all targets "
                          "; ordered = always near_sum_kernel; symmetric = wherever it applies")

@@ -1,0 +1,140 @@
+"""Lattice-factored image sums (csrc/lattice_kernels.cuh: |r_i - img_k(r_j)|^2 = X[k_x] + Y[k_y] + Z[k_z]
+for the full box of image cells of PAPER.md:40-50 Eq.(3)/(4); one add per image for r^2, charges and cell weights once
+per pair) against the CPU oracle and against the cell-by-cell kernels they replace, through the C-ABI.  Every shape that
+is instantiated -- 27 periodic cells, 27 reflected cells (gamma = -1 and +1), 45 slab cells (3 x 3 periodic x 5 reflected,
+gamma = 0.5 and -1) -- in the ordered form (small N, target shards, step (a)), the symmetric form (N >= 7,937) and their
+gradient forms; both refinements; and the geometries that must keep the cell-by-cell kernels.  Bars as in
+test_gpu_parity (north_star).  All `-m gpu`."""
+import math
+
+import numpy as np
+import pytest
+
+import hsma_workloads as W
+from oracle import hsma_oracle as O
+
+pytestmark = pytest.mark.gpu
+
+PHI_TOL, U_TOL, F_TOL = 1e-10, 1e-11, 1e-10
+AGREE = 2e-12          # the two kernel families differ only in the rounding of r^2 and of the sums
+
+
+@pytest.fixture(scope="module")
+def H():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    import paper_1806_04801_b200 as H
+    H.binding.load_library()
+    return H
+
+
+def dev(a):
+    import torch
+    return torch.as_tensor(np.ascontiguousarray(a, dtype=np.float64), device="cuda")
+
+
+def rel_inf(a, b):
+    return float(np.max(np.abs(a - b)) / np.max(np.abs(b)))
+
+
+def on_and_off(H, w, forces, **plan_kw):
+    """Results with the factored kernels (default) and with the cell-by-cell ones, from ONE plan."""
+    out = []
+    with H.Plan.from_workload(w, **plan_kw) as plan:
+        xyz, q = dev(w.xyz), dev(w.q)
+        assert plan.image_factoring
+        for on in (True, False):
+            plan.set_image_factoring(on)
+            assert plan.image_factoring == on
+            if forces:
+                phi, F, U = plan.evaluate_forces(xyz, q, sync=True)
+                out.append((phi.cpu().numpy(), F.cpu().numpy(), float(U), plan.last_pair_form))
+            else:
+                phi, U = plan.evaluate(xyz, q, sync=True)
+                out.append((phi.cpu().numpy(), None, float(U), plan.last_pair_form))
+    return out
+
+
+def check(w, r, got, forces):
+    (phi, F, U, form), (phi0, F0, U0, form0) = got
+    assert form == form0
+    for p, f, u in ((phi, F, U), (phi0, F0, U0)):
+        assert rel_inf(p, r.phi) <= PHI_TOL and abs(u - r.U) <= U_TOL * abs(r.U)
+        if forces:
+            assert np.max(np.abs(f - r.F)) <= F_TOL * np.max(np.abs(r.F))
+    assert rel_inf(phi, phi0) <= AGREE and abs(U - U0) <= AGREE * abs(U0)
+    if forces:
+        assert np.max(np.abs(F - F0)) <= AGREE * np.max(np.abs(F0))
+    return form
+
+
+# (config, N): 2 / 5 = 27 periodic cells, 3 = 27 reflected cells gamma = -1, 4 = 45 slab cells gamma = 0.5 with the far-data
+# closure (step (a) keeps the cell-by-cell kernel there: its table is the 396 far cells).  N < 7,937: ordered pairs
+# (R = 1 and 2 targets per thread, ragged last block and tile); N >= 7,937: symmetric form, ragged last block.
+CASES = [(2, 700), (2, 3000), (3, 1501), (4, 2500), (5, 9000), (3, 9001), (4, 8210)]
+
+
+@pytest.mark.parametrize("forces", [False, True])
+@pytest.mark.parametrize("refine", [1, 2])
+@pytest.mark.parametrize("idx,N", CASES)
+def test_factored_kernels_match_oracle_and_cell_by_cell(H, idx, N, refine, forces):
+    w = W.config(idx, N=N)
+    r = O.hsma(w, forces=forces)
+    form = check(w, r, on_and_off(H, w, forces, rsqrt_refine=refine), forces)
+    assert form == (2 if N >= 7937 else 1)
+
+
+@pytest.mark.parametrize("forces", [False, True])
+def test_generic_charges_and_weights(H, forces):
+    """Charges of any magnitude (the factored kernels multiply by q once per pair) with the weighted slab images."""
+    w = W.config(4, N=3001)
+    q = np.random.default_rng(5).standard_normal(w.N)
+    w = w.with_(q=q - q.mean())
+    check(w, O.hsma(w, forces=forces), on_and_off(H, w, forces), forces)
+
+
+@pytest.mark.parametrize("closure", ["walls", "slab_boundary", "face_pairs"])
+def test_other_closures(H, closure):
+    """Neumann walls (27 reflected cells with gamma = +1: every weight class has weight 1), the grounded slab by its own
+    boundary conditions (gamma = -1 on the 45-cell table) and the face-pair closure, whose derivative rows take
+    step (a) in its gradient form (near_lat_sum_kernel<.., FIELD> at the check targets)."""
+    rng = np.random.default_rng(8)
+    if closure == "walls":
+        N, L = 1200, (1.0, 1.0, 1.0)
+        w = W.Workload("neumann_cavity", W.BC_MIRROR_CAVITY, L, (1, 1, 1), 1.0, 1.5 * math.sqrt(3) / 2, 12, 4000, 900,
+                       0.03 + 0.94 * rng.random((N, 3)), W.alternating_charges(N),
+                       check_xyz=W.seeded_face_points(900, L, W.ALL_FACES, seed=9))
+    elif closure == "slab_boundary":
+        N, L = 1500, (1.0, 1.0, 0.5)
+        xyz = rng.random((N, 3)) * np.asarray(L)
+        xyz[:, 2] = 0.02 + 0.92 * xyz[:, 2]
+        w = W.Workload("slab_grounded", W.BC_SLAB_XY_PERIODIC_Z_MIRROR, L, (1, 1, 2), -1.0, 1.1, 12, 6000, 1000, xyz,
+                       rng.standard_normal(N) + 0.2, closure=W.CLOSURE_BOUNDARY)
+    else:
+        w = W.config(2, N=1100)
+        w = w.with_(closure=W.CLOSURE_FACE_PAIRS, check_xyz=W.seeded_face_points(w.K, w.L, W.LOWER_FACES, seed=3))
+    check(w, O.hsma(w, forces=True), on_and_off(H, w, True), True)
+
+
+def test_target_shards(H):
+    """Target shards (ordered pairs, self term found by slot) with the factored kernels: the pieces add up to the one-call
+    evaluate (symmetric form).  The PART form runs in tests/test_gpu_distributed.py."""
+    import torch
+    w = W.config(5, N=9000)
+    xyz, q = dev(w.xyz), dev(w.q)
+    with H.Plan.from_workload(w) as plan:
+        phi, U = plan.evaluate(xyz, q, sync=True)
+        cuts = [0, 2999, 3000, 7000, w.N]
+        pieces = [plan.evaluate_shard(xyz, q, a, b, sync=True)[0] for a, b in zip(cuts[:-1], cuts[1:])]
+        assert plan.last_pair_form == 1
+        got = torch.cat(pieces)
+        assert float((got - phi).abs().max() / phi.abs().max()) <= AGREE
+
+
+def test_where_the_cell_by_cell_kernels_stay(H):
+    """Shell 2 (config 1: 125 cells) and the sphere-culled near set are not instantiated / not a full box."""
+    with H.Plan.from_workload(W.config(1)) as plan:
+        assert not plan.image_factoring
+    w = W.config(2, N=800).with_(near_mode=W.NEAR_SPHERE)
+    with H.Plan.from_workload(w) as plan:
+        assert not plan.image_factoring
