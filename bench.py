@@ -94,6 +94,8 @@ def sym_evaluations(N: int, C: int) -> int:
 # capture (profiles/r01_ncu_near_sum_N262144.md): valid for config 5 at N = 262,144 on one GPU, potential only
 NCU_TRAFFIC_BYTES_CFG5 = 9555200
 NCU_TRAFFIC_BYTES_CFG5_SYM = 28873728    # near_sym_kernel, 3 waves per evaluate: 3 x (8,463,872 read + 1,160,704 written)
+NCU_TRAFFIC_BYTES_CFG5_LAT_SYM = 27668736   # near_lat_sym_kernel, 3 waves per evaluate: 3 x (8,527,360 read + 695,552 written)
+TRAFFIC_SOURCE_LAT_SYM = "profiles/r02_ncu_lat_sym_N262144.md (dram read+write bytes of one wave x 3 waves per evaluate)"
 TRAFFIC_SOURCE_SYM = "profiles/r02_ncu_near_sym_waves_N262144.md (dram read+write bytes of one wave x 3 waves per evaluate)"
 TRAFFIC_SOURCE = "profiles/r01_ncu_near_sum_N262144.md (dram read+write bytes of one launch)"
 # FP64 peak derived from unit counts and clocks: SMs x 64 DFMA lanes x 2 x clock
@@ -464,6 +466,11 @@ def run_b200(args, w) -> dict:
         refl = {W.BC_PERIODIC: (False, False, False), W.BC_MIRROR_CAVITY: (True, True, True),
                 W.BC_SLAB_XY_PERIODIC_Z_MIRROR: (False, False, True)}[int(w.kind)]
         frac_survey = ach_tf / peak_tf
+        if symmetric:
+            traffic = NCU_TRAFFIC_BYTES_CFG5_LAT_SYM if traffic else None
+            traffic_source = TRAFFIC_SOURCE_LAT_SYM
+        else:
+            traffic = None     # no capture of the ordered factored kernel at this size
         ex_instr, ex_flops = lat_counts(tuple(int(x) for x in w.near_shell), refl, refine, bool(args.forces), symmetric)
         alg_flops = ex_flops
         ach_tf = units * alg_flops / (k_ms * 1e-3) * 1e-12 if k_ms > 0 else 0.0
