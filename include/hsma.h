@@ -94,7 +94,7 @@ typedef enum {
                                   phases keep the direct kernels); step (a) at the check targets is then served by the
                                   same multipoles (boundary closures without derivative rows).  Needs the whole-cell near set and box sides that are integer multiples of
                                   the smallest one (cubic FMM boxes): HSMA_ERR_INVALID_ARG at plan creation otherwise. */
-    , HSMA_NEAR_ALG_AUTO = 2   /* the FMM from N = 24,576 sources on (the measured crossover is N ~ 22k) where the
+    , HSMA_NEAR_ALG_AUTO = 2   /* the FMM from N = 36,864 sources on (the measured crossover is N ~ 35k) where the
                                   geometry allows it, the direct sum below and wherever the FMM does not apply; never an error */
 } hsma_near_algorithm;
 

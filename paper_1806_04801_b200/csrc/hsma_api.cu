@@ -545,7 +545,7 @@ extern "C" hsma_status hsma_plan_create_ex(const hsma_plan_desc* desc, void* cud
         const hsma_status fs = fmm::setup(p->fmm, d, refl, st);
         if (fs != HSMA_OK && d.near_algorithm == HSMA_NEAR_ALG_FMM) { plan_free(p); return fs; }
         if (fs != HSMA_OK) { p->fmm.release(); p->fmm.enabled = false; cudaGetLastError(); }   // AUTO: the direct sum serves this geometry
-        p->fmm_min_N = d.near_algorithm == HSMA_NEAR_ALG_AUTO ? 24576 : 0;
+        p->fmm_min_N = d.near_algorithm == HSMA_NEAR_ALG_AUTO ? 36864 : 0;
     }
     if (rhsc.empty()) { p->cells_rhs = p->cells_near; p->C_rhs = p->C_near; }
     else { p->C_rhs = (int)rhsc.size(); PCU(upload(&p->cells_rhs, rhsc, st)); }

@@ -210,12 +210,12 @@ def test_extreme_orders_run_and_converge(H, order):
 
 def test_automatic_choice_of_the_near_algorithm(H):
     """near_algorithm = AUTO: the direct sum below the crossover and wherever the FMM cannot tile the box, the FMM above."""
-    for N, form in ((9000, 2), (30000, FMM)):
+    for N, form in ((9000, 2), (30000, 2), (40000, FMM)):
         w = W.config(5, N=N)
         with H.Plan.from_workload(w, near_algorithm=H.binding.NEAR_ALG_AUTO) as plan:
             plan.evaluate(dev(w.xyz), dev(w.q), sync=True)
             assert plan.last_pair_form == form
-    w = W.config(5, N=30000)
+    w = W.config(5, N=40000)
     L = (1.0, 1.2, 0.9)
     w = w.with_(L=L, R_aux=1.3, xyz=np.asarray(w.xyz) * np.asarray(L))
     with H.Plan.from_workload(w, near_algorithm=H.binding.NEAR_ALG_AUTO) as plan:      # no cubic boxes: direct, not an error
