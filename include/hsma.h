@@ -43,7 +43,8 @@ typedef enum {
     HSMA_ERR_NOT_NEUTRAL = -3,    /* periodic axes need sum q = 0             (reading S17) */
     HSMA_ERR_CUDA = -4,
     HSMA_ERR_ALLOC = -5,
-    HSMA_ERR_RANK_DEFICIENT = -6  /* fitting matrix lost rank in the Householder QR */
+    HSMA_ERR_RANK_DEFICIENT = -6, /* fitting matrix lost rank in the Householder QR */
+    HSMA_ERR_TOO_LARGE = -7       /* hsma_direct_sum_static only: sizes beyond its fixed scratch */
 } hsma_status;
 
 typedef enum {
@@ -256,6 +257,29 @@ hsma_status hsma_direct_sum(const double* tgt, long long T, const double* src, c
                             long long N, const double* shift_host, const double* sign_host,
                             const double* w_host, int C, int central_cell, long long self_offset,
                             int refine, double* phi_out, void* cuda_stream);
+/*
+ * The same raw kernel for callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): hsma_direct_sum_static calls no cudaMalloc / cudaFree / allocating library routine and
+ * copies nothing from host memory (the cell table travels as a kernel argument).  All of its scratch -- cell table, packed
+ * sources, slots, tile statistics, partial rows -- lives in ONE file-scope `static __device__` array of 16 MiB inside the
+ * library (hsma_static_scratch_bytes), which every GPU that loads the library holds until the process exits.
+ *   Arguments, layouts and result as hsma_direct_sum (Eq.(5)), with these limits: N <= 65,536 sources,
+ *   T <= 65,536 targets, C <= 32 cells, and 16 MiB of scratch in all for the launch shape chosen (checked per call); beyond
+ *   any of them the call returns HSMA_ERR_TOO_LARGE and launches nothing.  Other errors as hsma_direct_sum.
+ *   Asynchronous: it enqueues 6 kernels on `cuda_stream` and returns without synchronising; phi_out is valid once the
+ *   stream has passed them.  shift/sign/w are read before the call returns.
+ *   EVERY call on a device shares the one array, which keeps the last call's contents (the call clears what must start at
+ *   zero itself).  Calls on the same stream are ordered and safe; calls that can overlap on the GPU (different streams,
+ *   different host threads; another process has its own copy) RACE on the scratch: serialise them.
+ * hsma_static_scratch_setup: looks up the array's device address for the CURRENT device (cudaGetSymbolAddress; done once
+ * per device, also lazily by the first hsma_direct_sum_static on that device) -- call it before starting a graph capture.
+ */
+hsma_status hsma_direct_sum_static(const double* tgt, long long T, const double* src, const double* q,
+                                   long long N, const double* shift_host, const double* sign_host,
+                                   const double* w_host, int C, int central_cell, long long self_offset,
+                                   int refine, double* phi_out, void* cuda_stream);
+hsma_status hsma_static_scratch_setup(void);
+long long hsma_static_scratch_bytes(void);
 /* Raw kernel (c): phi[t] = sum_j Q_j/rho - P_j.(t - R_j)/rho^3.  All dev pointers; R [M,3], P [M,3]. */
 hsma_status hsma_node_sum(const double* tgt, long long T, const double* R, const double* Q,
                           const double* P, long long M, double* phi_out, void* cuda_stream);

@@ -20,6 +20,7 @@ c_double_p = ctypes.POINTER(ctypes.c_double)
 HSMA_OK = 0
 HSMA_ERR_INVALID_ARG, HSMA_ERR_GEOMETRY, HSMA_ERR_NOT_NEUTRAL = -1, -2, -3
 HSMA_ERR_CUDA, HSMA_ERR_ALLOC, HSMA_ERR_RANK_DEFICIENT = -4, -5, -6
+HSMA_ERR_TOO_LARGE = -7
 HSMA_BC_PERIODIC, HSMA_BC_MIRROR_CAVITY, HSMA_BC_SLAB_XY_PERIODIC_Z_MIRROR = 0, 1, 2
 HSMA_CLOSURE_BOUNDARY, HSMA_CLOSURE_FAR_DATA, HSMA_CLOSURE_FACE_PAIRS = 0, 1, 2
 HSMA_QUAD_SPIRAL, HSMA_QUAD_LATTICE = 0, 1
@@ -89,6 +90,12 @@ _SIGNATURES = {
                                        ctypes.c_longlong, c_double_p, c_double_p, c_double_p, ctypes.c_int,
                                        ctypes.c_int, ctypes.c_longlong, ctypes.c_int, ctypes.c_void_p,
                                        ctypes.c_void_p]),
+    "hsma_direct_sum_static": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p,
+                                              ctypes.c_longlong, c_double_p, c_double_p, c_double_p, ctypes.c_int,
+                                              ctypes.c_int, ctypes.c_longlong, ctypes.c_int, ctypes.c_void_p,
+                                              ctypes.c_void_p]),
+    "hsma_static_scratch_setup": (ctypes.c_int, []),
+    "hsma_static_scratch_bytes": (ctypes.c_longlong, []),
     "hsma_node_sum": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p,
                                      ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p]),
     "hsma_direct_field": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p,
@@ -377,6 +384,26 @@ def hsma_direct_sum(tgt: torch.Tensor, src: torch.Tensor, q: torch.Tensor, shift
     _check(load_library().hsma_direct_sum(_dev(tgt, 3 * T, "tgt"), T, _dev(src, 3 * N, "src"), _dev(q, N, "q"), N,
                                           _hp(shift), _hp(sign), _hp(w), C, central_cell, self_offset, refine,
                                           _dev(phi_out, T, "phi_out"), _stream_ptr(stream)), "hsma_direct_sum")
+
+
+def hsma_direct_sum_static(tgt: torch.Tensor, src: torch.Tensor, q: torch.Tensor, shift, sign, w, central_cell: int,
+                           self_offset: int, refine: int, phi_out: torch.Tensor, stream=None):
+    """hsma_direct_sum without any device allocation: scratch in the library's fixed 16 MiB device array (N, T <= 65,536,
+    C <= 32; HSMA_ERR_TOO_LARGE beyond).  Asynchronous on `stream`; overlapping calls race on the scratch.  include/hsma.h."""
+    shift, sign, w = _host(shift), _host(sign), _host(w)
+    T, N, C = tgt.shape[0], q.numel(), w.shape[0]
+    _check(load_library().hsma_direct_sum_static(_dev(tgt, 3 * T, "tgt"), T, _dev(src, 3 * N, "src"), _dev(q, N, "q"), N,
+                                                 _hp(shift), _hp(sign), _hp(w), C, central_cell, self_offset, refine,
+                                                 _dev(phi_out, T, "phi_out"), _stream_ptr(stream)), "hsma_direct_sum_static")
+
+
+def hsma_static_scratch_setup():
+    """Look up the fixed scratch array's address on the current device (once per device; e.g. before a graph capture)."""
+    _check(load_library().hsma_static_scratch_setup(), "hsma_static_scratch_setup")
+
+
+def hsma_static_scratch_bytes() -> int:
+    return int(load_library().hsma_static_scratch_bytes())
 
 
 def hsma_node_sum(tgt: torch.Tensor, R: torch.Tensor, Q: torch.Tensor, P: torch.Tensor, phi_out: torch.Tensor,

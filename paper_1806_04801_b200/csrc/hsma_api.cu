@@ -5,6 +5,7 @@
 #include <atomic>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -1224,6 +1225,7 @@ extern "C" const char* hsma_status_string(int s) {
         case HSMA_ERR_CUDA: return "HSMA_ERR_CUDA";
         case HSMA_ERR_ALLOC: return "HSMA_ERR_ALLOC";
         case HSMA_ERR_RANK_DEFICIENT: return "HSMA_ERR_RANK_DEFICIENT";
+        case HSMA_ERR_TOO_LARGE: return "HSMA_ERR_TOO_LARGE: sizes beyond the fixed scratch of hsma_direct_sum_static (N, T <= 65,536, C <= 32, 16 MiB in all)";
         default: return "HSMA_ERR_UNKNOWN";
     }
 }
@@ -1504,3 +1506,101 @@ extern "C" hsma_status hsma_plan_get_timing(hsma_plan* p, double* ms_out) {
 }
 
 extern "C" long long hsma_launch_count(void) { return g_launches; }
+
+// ---- allocation-free raw direct sum: hsma_direct_sum_static (include/hsma.h) ---------------------------------------
+// The same launches as hsma_direct_sum (pack_sources_kernel, charge_stats_kernel, near_sum_kernel, finish_phi_kernel)
+// with every scratch buffer -- cell table, packed sources, slots, tile statistics, partial rows -- carved out of ONE
+// file-scope device array of fixed size, for callers that cannot call cudaMalloc (CUDA graph capture, serving loops).
+// Every GPU that loads the library holds the array until the process exits.  In host code `g_static_scratch` is a
+// host-side stand-in for the symbol, NOT a device address: the address comes from cudaGetSymbolAddress, once per device,
+// with that device current.
+namespace hsma {
+constexpr size_t kStaticScratchBytes = 16u << 20;      // 16 MiB
+constexpr long long kStaticMaxN = 65536, kStaticMaxT = 65536;
+constexpr int kStaticMaxC = 32;
+constexpr int kStaticMaxDevices = 64;
+struct StaticCells { Cell c[kStaticMaxC]; };           // 1536 B: travels as a kernel argument, no host-to-device copy
+__global__ void static_cells_kernel(const StaticCells t, int C, Cell* __restrict__ out, int* __restrict__ flags) {
+    const int i = threadIdx.x;
+    if (i < C) out[i] = t.c[i];
+    if (i < 4) flags[i] = 0;                           // what must start at zero (the array keeps the last call's contents)
+}
+}  // namespace hsma
+
+static __device__ __align__(256) unsigned char g_static_scratch[hsma::kStaticScratchBytes];
+
+static std::mutex g_static_mu;
+static unsigned char* g_static_ptr[hsma::kStaticMaxDevices] = {};
+
+// device address of the scratch array on the CURRENT device (looked up once per device)
+static hsma_status static_scratch_address(unsigned char** out) {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kStaticMaxDevices) { cudaGetLastError(); return HSMA_ERR_CUDA; }
+    std::lock_guard<std::mutex> lk(g_static_mu);
+    if (!g_static_ptr[dev]) {
+        void* ptr = nullptr;
+        if (cudaGetSymbolAddress(&ptr, g_static_scratch) != cudaSuccess || !ptr) { cudaGetLastError(); return HSMA_ERR_CUDA; }
+        g_static_ptr[dev] = static_cast<unsigned char*>(ptr);
+    }
+    *out = g_static_ptr[dev];
+    return HSMA_OK;
+}
+
+extern "C" hsma_status hsma_static_scratch_setup(void) {
+    unsigned char* p = nullptr;
+    return static_scratch_address(&p);
+}
+extern "C" long long hsma_static_scratch_bytes(void) { return (long long)kStaticScratchBytes; }
+
+extern "C" hsma_status hsma_direct_sum_static(const double* tgt, long long T, const double* src, const double* q, long long N,
+                                              const double* shift_host, const double* sign_host, const double* w_host, int C,
+                                              int central_cell, long long self_offset, int refine, double* phi_out,
+                                              void* cuda_stream) {
+    if (!tgt || !src || !q || !shift_host || !sign_host || !w_host || !phi_out) return HSMA_ERR_INVALID_ARG;
+    if (T < 1 || N < 1 || C < 1 || (refine != 1 && refine != 2)) return HSMA_ERR_INVALID_ARG;
+    if (T > kStaticMaxT || N > kStaticMaxN || C > kStaticMaxC) return HSMA_ERR_TOO_LARGE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    StaticCells cells;
+    for (int c = 0; c < kStaticMaxC; ++c) {
+        Cell& k = cells.c[c];
+        k.sx = k.sy = k.sz = 0.0; k.w = 0.0; k.fx = k.fy = k.fz = 0; k.central = 0;
+        if (c >= C) continue;
+        k.sx = shift_host[3 * c]; k.sy = shift_host[3 * c + 1]; k.sz = shift_host[3 * c + 2];
+        k.w = w_host[c];
+        k.fx = sign_host[3 * c] < 0; k.fy = sign_host[3 * c + 1] < 0; k.fz = sign_host[3 * c + 2] < 0;
+        k.central = (c == central_cell);
+    }
+    const long long n_tiles = (N + kTile - 1) / kTile, Npad = n_tiles * kTile;
+    const Launch s = choose_near(T, n_tiles, C, refine, false);
+    // carve the array: every piece 256-byte aligned
+    auto up = [](size_t b) { return (b + 255) & ~(size_t)255; };
+    size_t off = 0;
+    const size_t o_cells = off; off += up(kStaticMaxC * sizeof(Cell));
+    const size_t o_qi = off;    off += up(sizeof(QInfo));
+    const size_t o_flags = off; off += up(4 * sizeof(int));
+    const size_t o_src = off;   off += up((size_t)Npad * sizeof(Src4));
+    const size_t o_idx = off;   off += up((size_t)(N + n_tiles) * sizeof(int));       // slot_of [N] then tile_np [n_tiles]
+    const size_t o_stats = off; off += up((size_t)(4 * n_tiles + 2) * sizeof(double)); // per tile [4] then scalars [2]
+    const size_t o_part = off;  off += up((size_t)s.rows * T * sizeof(double));
+    if (off > kStaticScratchBytes) return HSMA_ERR_TOO_LARGE;
+    unsigned char* base = nullptr;
+    const hsma_status rs = static_scratch_address(&base);
+    if (rs != HSMA_OK) return rs;
+    Cell* dc = reinterpret_cast<Cell*>(base + o_cells);
+    QInfo* qi = reinterpret_cast<QInfo*>(base + o_qi);
+    int* flags = reinterpret_cast<int*>(base + o_flags);
+    Src4* ds = reinterpret_cast<Src4*>(base + o_src);
+    int* idx = reinterpret_cast<int*>(base + o_idx);
+    double* stats = reinterpret_cast<double*>(base + o_stats);
+    double* part = reinterpret_cast<double*>(base + o_part);
+    static_cells_kernel<<<1, 32, 0, st>>>(cells, C, dc, flags);
+    pack_sources_kernel<<<(unsigned)n_tiles, kTile, 0, st>>>(src, q, N, 0.0, 0.0, 0.0, ds, idx, idx + N, stats);
+    charge_stats_kernel<<<1, 1024, 0, st>>>(stats, n_tiles, 0, stats + 4 * n_tiles, qi, flags);
+    HSMA_COUNT_LAUNCH(); HSMA_COUNT_LAUNCH(); HSMA_COUNT_LAUNCH();
+    const Packed P{ds, N, n_tiles, idx + N, idx, qi};
+    launch_near(s, false, tgt, 3, nullptr, T, 0, P, dc, C, central_cell >= 0 ? self_offset : -1, refine, part, st);
+    finish_phi_kernel<<<(unsigned)((T + 255) / 256), 256, 0, st>>>(s.layout(part), PartLayout{nullptr, 1, 1, 1, 1}, T, nullptr, nullptr, 0, phi_out, nullptr);
+    HSMA_COUNT_LAUNCH();
+    if (cudaPeekAtLastError() != cudaSuccess) { cudaGetLastError(); return HSMA_ERR_CUDA; }
+    return HSMA_OK;
+}
