@@ -273,6 +273,8 @@ hsma_status hsma_direct_sum(const double* tgt, long long T, const double* src, c
  *   different host threads; another process has its own copy) RACE on the scratch: serialise them.
  * hsma_static_scratch_setup: looks up the array's device address for the CURRENT device (cudaGetSymbolAddress; done once
  * per device, also lazily by the first hsma_direct_sum_static on that device) -- call it before starting a graph capture.
+ * The first launch of a kernel on a device makes the CUDA runtime load it (lazy module loading, which may allocate inside the
+ * driver): make one warm-up call of hsma_direct_sum_static with the same refine before a capture.
  */
 hsma_status hsma_direct_sum_static(const double* tgt, long long T, const double* src, const double* q,
                                    long long N, const double* shift_host, const double* sign_host,
