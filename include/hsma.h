@@ -282,6 +282,9 @@ hsma_status hsma_direct_sum_static(const double* tgt, long long T, const double*
                                    int refine, double* phi_out, void* cuda_stream);
 hsma_status hsma_static_scratch_setup(void);
 long long hsma_static_scratch_bytes(void);
+/* test hook: fill the whole scratch array with `byte` on `cuda_stream` (0xFF makes every double a NaN): a call that follows must
+ * still give the right answer, i.e. it reads nothing that it has not written itself. */
+hsma_status hsma_static_scratch_fill(int byte, void* cuda_stream);
 /* Raw kernel (c): phi[t] = sum_j Q_j/rho - P_j.(t - R_j)/rho^3.  All dev pointers; R [M,3], P [M,3]. */
 hsma_status hsma_node_sum(const double* tgt, long long T, const double* R, const double* Q,
                           const double* P, long long M, double* phi_out, void* cuda_stream);

@@ -96,6 +96,7 @@ _SIGNATURES = {
                                               ctypes.c_void_p]),
     "hsma_static_scratch_setup": (ctypes.c_int, []),
     "hsma_static_scratch_bytes": (ctypes.c_longlong, []),
+    "hsma_static_scratch_fill": (ctypes.c_int, [ctypes.c_int, ctypes.c_void_p]),
     "hsma_node_sum": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p,
                                      ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p]),
     "hsma_direct_field": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p,
@@ -404,6 +405,11 @@ def hsma_static_scratch_setup():
 
 def hsma_static_scratch_bytes() -> int:
     return int(load_library().hsma_static_scratch_bytes())
+
+
+def hsma_static_scratch_fill(byte: int, stream=None):
+    """Test hook: overwrite the fixed scratch array with `byte` (0xFF: NaNs) on `stream`."""
+    _check(load_library().hsma_static_scratch_fill(int(byte), _stream_ptr(stream)), "hsma_static_scratch_fill")
 
 
 def hsma_node_sum(tgt: torch.Tensor, R: torch.Tensor, Q: torch.Tensor, P: torch.Tensor, phi_out: torch.Tensor,

@@ -1551,6 +1551,15 @@ extern "C" hsma_status hsma_static_scratch_setup(void) {
     return static_scratch_address(&p);
 }
 extern "C" long long hsma_static_scratch_bytes(void) { return (long long)kStaticScratchBytes; }
+// test hook: overwrite the whole array with `byte` (0xFF: every double a NaN) on `cuda_stream`, so that a test can show
+// that a call reads nothing a previous call (or nobody) left behind
+extern "C" hsma_status hsma_static_scratch_fill(int byte, void* cuda_stream) {
+    unsigned char* p = nullptr;
+    const hsma_status rs = static_scratch_address(&p);
+    if (rs != HSMA_OK) return rs;
+    if (cudaMemsetAsync(p, byte, kStaticScratchBytes, (cudaStream_t)cuda_stream) != cudaSuccess) { cudaGetLastError(); return HSMA_ERR_CUDA; }
+    return HSMA_OK;
+}
 
 extern "C" hsma_status hsma_direct_sum_static(const double* tgt, long long T, const double* src, const double* q, long long N,
                                               const double* shift_host, const double* sign_host, const double* w_host, int C,

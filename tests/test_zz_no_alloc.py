@@ -92,6 +92,23 @@ def test_self_exclusion_and_uniform_charges(H):
         assert rel_inf(out.cpu().numpy(), ref) < 1e-12
 
 
+@pytest.mark.parametrize("byte", [0xFF, 0x00, 0x7F])
+def test_reads_nothing_left_behind_in_the_scratch(H, byte):
+    """The array keeps whatever the last call (or the fill hook) left: poisoned with NaN bytes, zeros or large finite
+    garbage, the next call still equals the allocating path bit for bit -- every scratch word it reads, it wrote."""
+    import torch
+    for seed, N, T in ((21, 2311, 77), (22, 256, 4000)):
+        src, q, tgt, c = problem(seed, N, T, W.BC_SLAB_XY_PERIODIC_Z_MIRROR, (1.0, 1.0, 0.5), (1, 1, 1), 0.5)
+        t, s_, q_ = dev(tgt), dev(src), dev(q)
+        out, old = torch.empty(T, dtype=torch.float64, device="cuda"), torch.empty(T, dtype=torch.float64, device="cuda")
+        H.hsma_static_scratch_fill(byte)
+        H.hsma_direct_sum_static(t, s_, q_, c.shift, c.sign, c.w, c.central, -1, 2, out)
+        torch.cuda.synchronize()
+        H.hsma_direct_sum(t, s_, q_, c.shift, c.sign, c.w, c.central, -1, 2, old)
+        assert torch.equal(out, old) and bool(torch.isfinite(out).all())
+        assert rel_inf(out.cpu().numpy(), O.near_sum(tgt, src, q, c)) < 1e-12
+
+
 def test_limits_are_rejected_with_a_clear_error(H):
     """N, T > 65,536 or C > 32: HSMA_ERR_TOO_LARGE, nothing launched, output untouched; the maximum itself runs."""
     import torch
