@@ -138,3 +138,28 @@ def test_where_the_cell_by_cell_kernels_stay(H):
     w = W.config(2, N=800).with_(near_mode=W.NEAR_SPHERE)
     with H.Plan.from_workload(w) as plan:
         assert not plan.image_factoring
+
+
+@pytest.mark.parametrize("idx,N", [(5, 30010), (4, 20500)])
+def test_both_families_over_many_blocks_and_waves(H, idx, N):
+    """Many target blocks and several waves (column scratch capped at 4 MiB): the factored kernels against the oracle, and the
+    cell-by-cell kernels -- now only the fallback for cell tables that are not instantiated -- against them, potentials and
+    forces, every element."""
+    w = W.config(idx, N=N)
+    r = O.hsma(w, forces=True)
+    res = []
+    with H.Plan.from_workload(w) as plan:
+        plan.set_sym_scratch_cap(4 << 20)
+        xyz, q = dev(w.xyz), dev(w.q)
+        for on in (True, False):
+            plan.set_image_factoring(on)
+            phi, F, U = plan.evaluate_forces(xyz, q, sync=True)
+            phi2, U2 = plan.evaluate(xyz, q, sync=True)
+            assert plan.last_pair_form == 2
+            res.append((phi.cpu().numpy(), F.cpu().numpy(), float(U), phi2.cpu().numpy(), float(U2)))
+    for phi, F, U, phi2, U2 in res:
+        assert rel_inf(phi, r.phi) <= PHI_TOL and rel_inf(phi2, r.phi) <= PHI_TOL
+        assert abs(U - r.U) <= U_TOL * abs(r.U) and abs(U2 - r.U) <= U_TOL * abs(r.U)
+        assert np.max(np.abs(F - r.F)) <= F_TOL * np.max(np.abs(r.F))
+    assert rel_inf(res[0][0], res[1][0]) <= AGREE and rel_inf(res[0][3], res[1][3]) <= AGREE
+    assert np.max(np.abs(res[0][1] - res[1][1])) <= AGREE * np.max(np.abs(res[1][1]))
