@@ -718,11 +718,20 @@ __global__ void node_positions_kernel(const double* __restrict__ nrm, double R, 
 //   kPhaseRest    H1 + fit + mapping + (b) + (c) + finish with the plan's pc (pcg) AS THEY ARE (hsma_set_check_sums)
 enum { kPhaseAll = 0, kPhaseCheck = 1, kPhaseRest = 2 };
 static bool lat_applies(const hsma_plan* p, const Cell* cells) { return p->lat_on && p->lat_shape != 0 && cells == p->cells_near; }
+template <int REFINE, int SX, int SY, int SZ, int MASK>
+static void launch_lat_sym_of(int G, const SymArgs& a, const LatGeom& g, cudaStream_t st) {
+    static bool opted = false;   // dynamic shared memory of this instantiation: set the limit once
+    if (!opted) {
+        cudaFuncSetAttribute(near_lat_sym_kernel<REFINE, SX, SY, SZ, MASK>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSymWideDynSmem);
+        opted = true;
+    }
+    near_lat_sym_kernel<REFINE, SX, SY, SZ, MASK><<<G, kSymWideThreads, kSymWideDynSmem, st>>>(a, g);
+}
 static void launch_lat_sym(int shape, int refine, int G, const SymArgs& a, const LatGeom& g, cudaStream_t st) {
-#define HSMA_LAT_SYM(SX, SY, SZ, MASK)                                                              \
-    do {                                                                                            \
-        if (refine == 1) near_lat_sym_kernel<1, SX, SY, SZ, MASK><<<G, kThreads, 0, st>>>(a, g);    \
-        else near_lat_sym_kernel<2, SX, SY, SZ, MASK><<<G, kThreads, 0, st>>>(a, g);                \
+#define HSMA_LAT_SYM(SX, SY, SZ, MASK)                                              \
+    do {                                                                            \
+        if (refine == 1) launch_lat_sym_of<1, SX, SY, SZ, MASK>(G, a, g, st);       \
+        else launch_lat_sym_of<2, SX, SY, SZ, MASK>(G, a, g, st);                   \
     } while (0)
     if (shape == 1) HSMA_LAT_SYM(1, 1, 1, 0);
     else if (shape == 2) HSMA_LAT_SYM(1, 1, 1, 7);

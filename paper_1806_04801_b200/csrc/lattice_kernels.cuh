@@ -90,13 +90,22 @@ __device__ __forceinline__ double lat_sum(const LatGeom& g, double xi, double yi
 
 // ---- step (b), symmetric form, lattice-factored: same work decomposition, arguments, scratch layout and gathers as
 // near_sym_kernel (sum_kernels.cuh; a.cells / a.C are not read), so launch_sym's waves and the PART form carry over.
+// 512 threads per CTA and 4 targets per thread (16 warps per SM under a 128-register cap; the image chains of one pair
+// are all the instruction-level parallelism a thread needs, so the wider CTA buys latency hiding: 312.4 -> 303.5 ms at
+// config 5 against 256 threads x 8 targets, 10-13 % on the reflecting shapes).  Thread t owns the block's targets
+// r * 512 + t, r < 4, i.e. tile 2r + (t >> 8), slot t & 255 -- the same linear index as near_sym_kernel's r * 256 + t.
+// colw [16][kTile] lives in dynamic shared memory.
+constexpr int kSymWideThreads = 512;
+constexpr int kSymWideR = kSymBlock / kSymWideThreads;
+constexpr int kSymWideDynSmem = (kSymWideThreads / 32) * kTile * (int)sizeof(double);
+
 template <int REFINE, int SX, int SY, int SZ, int MASK>
-__global__ void __launch_bounds__(kThreads, 1) near_lat_sym_kernel(const SymArgs a, const LatGeom g) {
+__global__ void __launch_bounds__(kSymWideThreads, 1) near_lat_sym_kernel(const SymArgs a, const LatGeom g) {
     __shared__ __align__(128) Src4 tile[kStages][kTile];
     __shared__ __align__(8) uint64_t full[kStages];
-    __shared__ double colw[kThreads / 32][kTile];
+    extern __shared__ __align__(16) double colw_dyn[];     // [kSymWideThreads / 32][kTile]
 
-    constexpr int R = kSymR, S = kSymS;
+    constexpr int R = kSymWideR, TH = kSymWideThreads, S = kSymS, RB = kSymR;   // RB: tiles per block
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int G = gridDim.x, k = blockIdx.x;
     const long long f0 = a.f_begin + unit_start(k, a.fine, G), f1 = a.f_begin + unit_start(k + 1, a.fine, G);
@@ -105,7 +114,7 @@ __global__ void __launch_bounds__(kThreads, 1) near_lat_sym_kernel(const SymArgs
     const int nt = (int)a.n_tiles;
     int I = 0;
     while (sym_visit0(I + 1, nt) <= V0) ++I;
-    int J = I * R + (int)(V0 - sym_visit0(I, nt));
+    int J = I * RB + (int)(V0 - sym_visit0(I, nt));
 
     if (tid == 0) {
         for (int s = 0; s < kStages; ++s) mbar_init(&full[s], 1);
@@ -121,18 +130,19 @@ __global__ void __launch_bounds__(kThreads, 1) near_lat_sym_kernel(const SymArgs
     const int nvis = (int)(V1 - V0) + 1;
     const int ch_first = (int)(f0 - V0 * kSymChunks), ch_last = (int)(f1 - 1 - V1 * kSymChunks) + 1;
     const long long Tp = (long long)a.part_blocks * kSymBlock;
+    const int my_tile = tid >> 8, my_slot = tid & (kTile - 1);   // tile (within a pair of tiles) and slot of this thread's targets
     bool fresh = true;
     auto store_block = [&](int blk) {
         const int row = k - cta_of_unit(max(sym_visit0(blk, nt) * kSymChunks, a.f_begin) - a.f_begin, a.fine, G);
 #pragma unroll
-        for (int r = 0; r < R; ++r) a.part[(long long)row * Tp + (long long)(blk - a.blk_base) * kSymBlock + r * kThreads + tid] = tot[r];
+        for (int r = 0; r < R; ++r) a.part[(long long)row * Tp + (long long)(blk - a.blk_base) * kSymBlock + r * TH + tid] = tot[r];
     };
 
     for (int it = 0; it < nvis; ++it) {
         const int st = it & 1;
         const bool last_of_block = J + 1 == nt;
         if (tid == 0 && it + 1 < nvis) {
-            const int Jn = last_of_block ? (I + 1) * R : J + 1;
+            const int Jn = last_of_block ? (I + 1) * RB : J + 1;
             mbar_expect_tx(&full[st ^ 1], kTile * sizeof(Src4));
             bulk_g2s(tile[st ^ 1], a.src + (long long)Jn * kTile, kTile * sizeof(Src4), &full[st ^ 1]);
         }
@@ -140,29 +150,29 @@ __global__ void __launch_bounds__(kThreads, 1) near_lat_sym_kernel(const SymArgs
             fresh = false;
 #pragma unroll
             for (int r = 0; r < R; ++r) {
-                const int tt = I * R + r;               // tile of these targets; beyond the last tile: phantom, q = 0
-                const Src4 t = a.src[(long long)min(tt, nt - 1) * kTile + tid];
+                const int tt = I * RB + 2 * r + my_tile;
+                const Src4 t = a.src[(long long)min(tt, nt - 1) * kTile + my_slot];
                 ox[r] = t.x; oy[r] = t.y; oz[r] = t.z; oq[r] = tt < nt ? t.q : 0.0;
                 tot[r] = 0.0;
             }
         }
-        const int rd = J - I * R;                       // < R: the tile is one of the block's own
-        const bool diag = rd < R;
+        const int rd = J - I * RB;                      // < RB: the tile is one of the block's own
+        const bool diag = rd < RB;
         mbar_wait(&full[st], (it >> 1) & 1);
         const Src4* __restrict__ s = tile[st];
         const int j_lo = (it == 0 ? ch_first : 0) * S;
         const int j_hi = (it == nvis - 1 ? ch_last : kSymChunks) * S;
 
         if (diag) {
-            // the block's own tile: ordered pairs, row sums only; target (r = rd, tid) IS source j = tid
+            const int r_self = (rd - my_tile) >= 0 && ((rd - my_tile) & 1) == 0 ? (rd - my_tile) >> 1 : -1;   // my target that lives in tile rd
 #pragma unroll 1
             for (int j = j_lo; j < j_hi; ++j) {
                 const double2 xy = *reinterpret_cast<const double2*>(&s[j].x);
                 const double2 zq = *reinterpret_cast<const double2*>(&s[j].z);
-                const bool mine = j == tid;
+                const bool mine = j == my_slot;
 #pragma unroll
                 for (int r = 0; r < R; ++r) {
-                    const double v = lat_sum<REFINE, SX, SY, SZ, MASK, true>(g, ox[r], oy[r], oz[r], xy.x, xy.y, zq.x, mine && r == rd);
+                    const double v = lat_sum<REFINE, SX, SY, SZ, MASK, true>(g, ox[r], oy[r], oz[r], xy.x, xy.y, zq.x, mine && r == r_self);
                     tot[r] = fma(zq.y, v, tot[r]);
                 }
             }
@@ -180,23 +190,23 @@ __global__ void __launch_bounds__(kThreads, 1) near_lat_sym_kernel(const SymArgs
                 }
 #pragma unroll
                 for (int o = 16; o; o >>= 1) cj += __shfl_xor_sync(0xffffffffu, cj, o);
-                if (lane == 0) colw[warp][j] = cj;
+                if (lane == 0) colw_dyn[warp * kTile + j] = cj;
             }
         }
         __syncthreads();  // tile[st] may be refilled; colw is complete
         if (!diag) {
-            const int j = tid;  // kTile == kThreads
-            if (j >= j_lo && j < j_hi) {
+            const int j = tid;
+            if (j < kTile && j >= j_lo && j < j_hi) {
                 double v = 0.0;
 #pragma unroll
-                for (int w = 0; w < kThreads / 32; ++w) v += colw[w][j];
+                for (int w = 0; w < TH / 32; ++w) v += colw_dyn[w * kTile + j];
                 a.col[(V0 + it - a.v_base) * kTile + j] = v;
             }
             __syncthreads();  // colw is rewritten by the next visit
         }
         if (last_of_block) {
             store_block(I);
-            ++I; J = I * R; fresh = true;
+            ++I; J = I * RB; fresh = true;
         } else {
             ++J;
         }
@@ -454,7 +464,7 @@ constexpr int kLatChunk = 8;
 constexpr int kLatChunks = kTile / kLatChunk;
 
 template <int R, int REFINE, bool FIELD, int SX, int SY, int SZ, int MASK>
-__global__ void __launch_bounds__(kThreads, 1) near_lat_sum_kernel(const NearArgs a, const LatGeom g) {
+__global__ void __launch_bounds__(kThreads, FIELD ? 1 : 2) near_lat_sum_kernel(const NearArgs a, const LatGeom g) {
     __shared__ __align__(128) Src4 tile[kStages][kTile];
     __shared__ __align__(8) uint64_t full[kStages];
 
