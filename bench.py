@@ -63,7 +63,8 @@ EXEC_EVAL_SYM_FIELD = {1: (21.0 + 11.0 / 8.0, 33.0 + 18.0 / 8.0), 2: (23.0 + 11.
 #                 (+ 2 DFMA for the cubic step)
 #   per pair    : offsets (1 + 2 s_a [+ 1 on a reflecting axis] DADD per axis), x squares (2 s_x + 1 DMUL),
 #                 x-square + y-square (DFMA per (kx, ky)), weight classes (1 DMUL + DFMA per further class),
-#                 row and column accumulation (2 DFMA; 1 for ordered pairs)
+#                 row and column accumulation (2 DFMA; 1 for ordered pairs), symmetric form: 5/4 DADD (warp reduction of the
+#                 column sum of a source, once per 4 targets)
 # Gradient forms: measured on the 27-cell periodic shape (10.22 instructions / 15.15 flops per image, Newton).
 def lat_counts(shell, reflecting, refine: int, field: bool, symmetric: bool):
     """(FP64-pipe instructions, flops) executed per image-pair evaluation by the lattice-factored kernels."""
@@ -78,7 +79,8 @@ def lat_counts(shell, reflecting, refine: int, field: bool, symmetric: bool):
     dfma = (2 * sx + 1) * (2 * sy + 1) + (classes - 1) + (2 if symmetric else 1)
     per_img_instr = 4 + (2 if refine == 2 else 0)
     per_img_flops = 7 + (4 if refine == 2 else 0)
-    return (per_img_instr + (dadd + dmul + dfma) / images, per_img_flops + (dadd + dmul + 2 * dfma) / images)
+    red = 5.0 / 4.0 if symmetric else 0.0     # symmetric form: 5 DADD of the warp reduction of a source's column sum, per 4 pairs
+    return (per_img_instr + (dadd + dmul + dfma + red) / images, per_img_flops + (dadd + dmul + 2 * dfma + red) / images)
 
 
 def sym_evaluations(N: int, C: int) -> int:
@@ -94,8 +96,8 @@ def sym_evaluations(N: int, C: int) -> int:
 # capture (profiles/r01_ncu_near_sum_N262144.md): valid for config 5 at N = 262,144 on one GPU, potential only
 NCU_TRAFFIC_BYTES_CFG5 = 9555200
 NCU_TRAFFIC_BYTES_CFG5_SYM = 28873728    # near_sym_kernel, 3 waves per evaluate: 3 x (8,463,872 read + 1,160,704 written)
-NCU_TRAFFIC_BYTES_CFG5_LAT_SYM = 27668736   # near_lat_sym_kernel, 3 waves per evaluate: 3 x (8,527,360 read + 695,552 written)
-TRAFFIC_SOURCE_LAT_SYM = "profiles/r02_ncu_lat_sym_N262144.md (dram read+write bytes of one wave x 3 waves per evaluate)"
+NCU_TRAFFIC_BYTES_CFG5_LAT_SYM = 29011968   # near_lat_sym_kernel, 3 waves per evaluate: 3 x (8,478,464 read + 1,192,192 written)
+TRAFFIC_SOURCE_LAT_SYM = "profiles/r02c_ncu_lat_sym_N262144.md (dram read+write bytes of one wave x 3 waves per evaluate)"
 TRAFFIC_SOURCE_SYM = "profiles/r02_ncu_near_sym_waves_N262144.md (dram read+write bytes of one wave x 3 waves per evaluate)"
 TRAFFIC_SOURCE = "profiles/r01_ncu_near_sum_N262144.md (dram read+write bytes of one launch)"
 # FP64 peak derived from unit counts and clocks: SMs x 64 DFMA lanes x 2 x clock

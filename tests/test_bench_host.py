@@ -41,16 +41,16 @@ def test_lattice_factored_counts(bench):
     """DESIGN.md 6.14 / csrc/lattice_kernels.cuh: FP64-pipe instructions and flops per image-pair evaluation of the
     lattice-factored kernels, counted from the formulation (per image: r^2 DFMA, y0^2 DMUL, Newton DFMA, accumulate DFMA;
     per pair: offsets, x squares, x^2 + y^2, weight classes, row/column accumulation).  The SASS of the 27-cell periodic
-    inner loop has 1061 FP64 instructions for 216 images = 4.91 (profiles/r02_sass_lattice.md; +0.02 warp reduction)."""
+    inner loop has 533 FP64 instructions for 108 images = 4.935 (profiles/r02c_ncu_lat_sym_N262144.md)."""
     p = (False, False, False)
     i, f = bench.lat_counts((1, 1, 1), p, 1, False, True)
-    assert abs(i - (4 + (9 + 4 + 11) / 27)) < 1e-12 and abs(f - (7 + (9 + 4 + 22) / 27)) < 1e-12
-    assert abs(i - 1061 / 216) < 0.03
+    assert abs(i - (4 + (9 + 4 + 11 + 1.25) / 27)) < 1e-12 and abs(f - (7 + (9 + 4 + 22 + 1.25) / 27)) < 1e-12
+    assert abs(i - 533 / 108) < 1e-3          # SASS of the inner loop, profiles/r02c_ncu_lat_sym_N262144.md
     # cubic refinement: two more DFMA per image; ordered pairs: one accumulation less per pair
     i2, f2 = bench.lat_counts((1, 1, 1), p, 2, False, True)
     assert abs(i2 - i - 2) < 1e-12 and abs(f2 - f - 4) < 1e-12
     io, fo = bench.lat_counts((1, 1, 1), p, 1, False, False)
-    assert abs(i - io - 1 / 27) < 1e-12 and abs(f - fo - 2 / 27) < 1e-12
+    assert abs(i - io - 2.25 / 27) < 1e-12 and abs(f - fo - 3.25 / 27) < 1e-12
     # reflecting axes: one more offset per axis (x_i + x_j) and one DFMA per further weight class
     im, _ = bench.lat_counts((1, 1, 1), (True, True, True), 1, False, True)
     assert abs(im - i - (3 + 3) / 27) < 1e-12
