@@ -244,10 +244,26 @@ static int sym_resident(int refine) {
     if (!c) c = refine == 1 ? resident_ctas(near_sym_kernel<1>) : resident_ctas(near_sym_kernel<2>);
     return c;
 }
-// the gradient form needs 64 KB of dynamic shared memory: opt in once per instantiation
+// Kernels with more than 48 KB of shared memory: raise the limit once per kernel AND per device (a function attribute
+// belongs to the device that was current when it was set; one mask per call site, bit = device ordinal mod 64).
+template <class K>
+static void ensure_dyn_smem(K kernel, int bytes, std::atomic<unsigned long long>& done) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); dev = 0; }
+    const unsigned long long bit = 1ull << (dev & 63);
+    if (done.load(std::memory_order_relaxed) & bit) return;
+    if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes) != cudaSuccess) cudaGetLastError();
+    done.fetch_or(bit, std::memory_order_relaxed);
+}
+template <int REFINE>
+static void ensure_sym_field_smem() {
+    static std::atomic<unsigned long long> done{0};
+    ensure_dyn_smem(near_sym_field_kernel<REFINE>, kSymFieldDynSmem, done);
+}
+// the gradient form needs 64 KB of dynamic shared memory
 template <int REFINE>
 static int sym_field_resident_of() {
-    cudaFuncSetAttribute(near_sym_field_kernel<REFINE>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSymFieldDynSmem);
+    ensure_sym_field_smem<REFINE>();
     int per_sm = 0;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, near_sym_field_kernel<REFINE>, kThreads, kSymFieldDynSmem) != cudaSuccess || per_sm < 1) {
         cudaGetLastError();
@@ -720,11 +736,8 @@ enum { kPhaseAll = 0, kPhaseCheck = 1, kPhaseRest = 2 };
 static bool lat_applies(const hsma_plan* p, const Cell* cells) { return p->lat_on && p->lat_shape != 0 && cells == p->cells_near; }
 template <int REFINE, int SX, int SY, int SZ, int MASK>
 static void launch_lat_sym_of(int G, const SymArgs& a, const LatGeom& g, cudaStream_t st) {
-    static bool opted = false;   // dynamic shared memory of this instantiation: set the limit once
-    if (!opted) {
-        cudaFuncSetAttribute(near_lat_sym_kernel<REFINE, SX, SY, SZ, MASK>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSymWideDynSmem);
-        opted = true;
-    }
+    static std::atomic<unsigned long long> done{0};
+    ensure_dyn_smem(near_lat_sym_kernel<REFINE, SX, SY, SZ, MASK>, kSymWideDynSmem, done);
     near_lat_sym_kernel<REFINE, SX, SY, SZ, MASK><<<G, kSymWideThreads, kSymWideDynSmem, st>>>(a, g);
 }
 static void launch_lat_sym(int shape, int refine, int G, const SymArgs& a, const LatGeom& g, cudaStream_t st) {
@@ -740,11 +753,8 @@ static void launch_lat_sym(int shape, int refine, int G, const SymArgs& a, const
 }
 template <int REFINE, int SX, int SY, int SZ, int MASK>
 static void launch_lat_sym_field_of(int G, const SymArgs& a, const LatGeom& g, cudaStream_t st) {
-    static bool opted = false;   // > 48 KB of dynamic shared memory: opt in once per instantiation
-    if (!opted) {
-        cudaFuncSetAttribute(near_lat_sym_field_kernel<REFINE, SX, SY, SZ, MASK>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLatFieldDynSmem);
-        opted = true;
-    }
+    static std::atomic<unsigned long long> done{0};
+    ensure_dyn_smem(near_lat_sym_field_kernel<REFINE, SX, SY, SZ, MASK>, kLatFieldDynSmem, done);
     near_lat_sym_field_kernel<REFINE, SX, SY, SZ, MASK><<<G, kThreads, kLatFieldDynSmem, st>>>(a, g);
 }
 static void launch_lat_sym_field(int shape, int refine, int G, const SymArgs& a, const LatGeom& g, cudaStream_t st) {
@@ -789,8 +799,8 @@ static void launch_sym(hsma_plan* p, const SymLaunch& ss, bool field, int refine
         a.f_begin = W.f_begin; a.fine = W.fine; a.v_base = W.v_base; a.blk_base = W.blk_lo; a.part_blocks = W.blk_hi - W.blk_lo + 1;
         if (field) {
             if (lat) launch_lat_sym_field(p->lat_shape, refine, W.G, a, lg, st);
-            else if (refine == 1) near_sym_field_kernel<1><<<W.G, kThreads, kSymFieldDynSmem, st>>>(a);
-            else near_sym_field_kernel<2><<<W.G, kThreads, kSymFieldDynSmem, st>>>(a);
+            else if (refine == 1) { ensure_sym_field_smem<1>(); near_sym_field_kernel<1><<<W.G, kThreads, kSymFieldDynSmem, st>>>(a); }
+            else { ensure_sym_field_smem<2>(); near_sym_field_kernel<2><<<W.G, kThreads, kSymFieldDynSmem, st>>>(a); }
             HSMA_COUNT_LAUNCH();
             sym_gather_field_kernel<<<gb, 256, 0, st>>>(p->part_b.p, p->sym_col.p, p->slot_of.p, N, n_tiles, W, p->sym_phi.p);
         } else {
