@@ -163,3 +163,53 @@ def test_both_families_over_many_blocks_and_waves(H, idx, N):
         assert np.max(np.abs(F - r.F)) <= F_TOL * np.max(np.abs(r.F))
     assert rel_inf(res[0][0], res[1][0]) <= AGREE and rel_inf(res[0][3], res[1][3]) <= AGREE
     assert np.max(np.abs(res[0][1] - res[1][1])) <= AGREE * np.max(np.abs(res[1][1]))
+
+
+@pytest.mark.parametrize("seed", [1, 2, 3])
+def test_fuzz_both_families_agree(H, seed):
+    """40 random cases per seed -- boundary kind, box, N from 1 to 40,000 (ordered and symmetric forms, ragged tiles, phantom
+    targets of a last block), charges (alternating, scaled, random), refinement, potentials or forces, column-scratch cap
+    (waves) -- evaluated by the factored and by the cell-by-cell kernels from one plan: finite and equal to rounding.  (The
+    oracle comparisons are the tests above; this one hunts index errors at sizes no fixed case names.)"""
+    rng = np.random.default_rng(seed)
+    for case in range(40):
+        kind = int(rng.integers(0, 3))
+        N = int(rng.integers(7937, 40000)) if rng.random() < 0.6 else int(rng.integers(1, 7937))
+        if kind == 0:
+            L = (1.0, 1.0, 1.0) if rng.random() < 0.5 else (1.0, 1.1, 0.9)
+            N += N % 2
+            q = W.alternating_charges(N) * (1.0 if rng.random() < 0.5 else 0.37)
+            if rng.random() < 0.4:
+                q = rng.standard_normal(N)
+                q -= q.mean()
+            R = min(1.3 * 0.5 * math.sqrt(sum(x * x for x in L)), 1.45 * min(L))
+            w = W.Workload("f", W.BC_PERIODIC, L, (1, 1, 1), 1.0, R, 8, 1500, 400, rng.random((N, 3)) * np.asarray(L), q)
+        elif kind == 1:
+            q = rng.standard_normal(N) if rng.random() < 0.5 else W.alternating_charges(N + N % 2)[:N]
+            w = W.Workload("f", W.BC_MIRROR_CAVITY, (1.0, 1.0, 1.0), (1, 1, 1), -1.0, 1.5 * math.sqrt(3) / 2, 8, 1500, 400,
+                           0.02 + 0.96 * rng.random((N, 3)), q)
+        else:
+            L = (1.0, 1.0, 0.5)
+            xyz = rng.random((N, 3)) * np.asarray(L)
+            xyz[:, 2] = 0.02 + 0.92 * xyz[:, 2]
+            w = W.Workload("f", W.BC_SLAB_XY_PERIODIC_Z_MIRROR, L, (1, 1, 2), -1.0, 1.1, 8, 2000, 500, xyz, rng.standard_normal(N),
+                           closure=W.CLOSURE_BOUNDARY)
+        refine, forces = int(rng.integers(0, 3)), bool(rng.random() < 0.5)
+        res = []
+        with H.Plan.from_workload(w, rsqrt_refine=refine) as plan:
+            if rng.random() < 0.3:
+                plan.set_sym_scratch_cap(int(rng.integers(1, 16)) << 20)
+            xyz, q = dev(w.xyz), dev(w.q)
+            for on in (True, False):
+                plan.set_image_factoring(on)
+                if forces:
+                    phi, F, U = plan.evaluate_forces(xyz, q, sync=True)
+                    res.append((phi.cpu().numpy(), F.cpu().numpy()))
+                else:
+                    phi, U = plan.evaluate(xyz, q, sync=True)
+                    res.append((phi.cpu().numpy(), None))
+        tag = f"seed {seed} case {case}: kind {kind} N {N} refine {refine} forces {forces}"
+        assert np.all(np.isfinite(res[0][0])), tag
+        assert rel_inf(res[0][0], res[1][0]) <= AGREE, tag
+        if forces:
+            assert np.max(np.abs(res[0][1] - res[1][1])) <= AGREE * np.max(np.abs(res[1][1])), tag
