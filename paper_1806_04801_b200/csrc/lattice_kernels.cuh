@@ -8,8 +8,9 @@
 // reflecting axes of |k_a| (weight gamma^m, Eq.(4)), the weight, so the reciprocal distances are accumulated per class
 // with one DFMA (seed * Newton factor, never multiplied out) and the charges enter once per PAIR:
 //     S_ij = sum_m gamma^m sum_{k in class m} 1 / |r_i - img_k(r_j)|,     phi_i += q_j S_ij,   phi_j += q_i S_ij.
-// Per image (Newton form): DADD (r^2) + MUFU.RSQ64H + DMUL (y0^2) + DFMA (3 - r^2 y0^2) + DFMA (accumulate) = 4 FP64
-// instructions + 1/3 + (15 + 3) / 27 per-pair ones = 5.0, against 11 in near_sym_kernel and 9 in near_sum_kernel.
+// Per image (Newton form): DFMA (r^2 = e_z^2 + (X + Y)) + MUFU.RSQ64H + DMUL (y0^2) + DFMA (3 - r^2 y0^2) + DFMA (accumulate)
+// = 4 FP64 instructions, + per pair (9 offsets, 3 x-squares, 9 X + Y, scale, row and column sums) / 27 = 0.89: 4.9, against
+// 11.6 in near_sym_kernel and 9 in near_sum_kernel (SASS counts: profiles/r02c_ncu_lat_sym_N262144.md).
 // Instantiated for the shapes the configurations use; any other cell table keeps the cell-by-cell kernels.
 #pragma once
 #include "sum_kernels.cuh"
