@@ -354,8 +354,8 @@ long long hsma_plan_scratch_bytes(const hsma_plan* plan);
  * Lattice-factored image sums (Eq.(3)/(4): the near set is a full box of image cells).
  * For one (target, source) pair the squared distances to all images separate over the axes, |d_k|^2 = X[k_x] + Y[k_y] +
  * Z[k_z], so the direct sums of steps (a) and (b) cost one add per image for r^2 and the charges and cell weights enter
- * once per pair.  On by default wherever it applies: whole-cell near sets of shape (1,1,1) periodic, (1,1,1) reflecting
- * and (1,1,2) xy-periodic / z-reflecting; any other cell table, the sphere-culled near set and the far-data table keep
+ * once per pair.  On by default wherever it applies: whole-cell near sets of shape (1,1,1) periodic, (1,1,1) reflecting,
+ * (1,1,1) and (1,1,2) xy-periodic / z-reflecting; any other cell table, the sphere-culled near set and the far-data table keep
  * the cell-by-cell kernels.  on = 0 restores those everywhere (same results to rounding: the two forms differ only in
  * the rounding of r^2).  hsma_plan_image_factoring: 1 if the factored kernels are in use for this plan.
  */

@@ -191,6 +191,7 @@ static LatNearFn lat_near_fn(int R, int refine, bool field, int shape) {
 #define HSMA_LAT_SHAPE(RR, RF, FD)                                                          \
     (shape == 1 ? (LatNearFn)near_lat_sum_kernel<RR, RF, FD, 1, 1, 1, 0>                    \
                 : shape == 2 ? (LatNearFn)near_lat_sum_kernel<RR, RF, FD, 1, 1, 1, 7>       \
+                : shape == 4 ? (LatNearFn)near_lat_sum_kernel<RR, RF, FD, 1, 1, 1, 4>       \
                              : (LatNearFn)near_lat_sum_kernel<RR, RF, FD, 1, 1, 2, 4>)
     if (R == 2) {
         if (refine == 1) return field ? HSMA_LAT_SHAPE(2, 1, true) : HSMA_LAT_SHAPE(2, 1, false);
@@ -201,7 +202,7 @@ static LatNearFn lat_near_fn(int R, int refine, bool field, int shape) {
 #undef HSMA_LAT_SHAPE
 }
 static int lat_near_resident(int R, int refine, bool field, int shape) {
-    static int cache[2][2][2][4] = {};
+    static int cache[2][2][2][5] = {};
     int& c = cache[R == 2 ? 1 : 0][refine == 1 ? 0 : 1][field ? 1 : 0][shape];
     if (!c) c = resident_ctas(lat_near_fn(R, refine, field, shape));
     return c;
@@ -366,6 +367,7 @@ static int lat_shape_of(const int shell[3], const bool refl[3]) {
     if (shell[0] == 1 && shell[1] == 1 && shell[2] == 1 && mask == 0) return 1;
     if (shell[0] == 1 && shell[1] == 1 && shell[2] == 1 && mask == 7) return 2;
     if (shell[0] == 1 && shell[1] == 1 && shell[2] == 2 && mask == 4) return 3;
+    if (shell[0] == 1 && shell[1] == 1 && shell[2] == 1 && mask == 4) return 4;
     return 0;
 }
 
@@ -748,6 +750,7 @@ static void launch_lat_sym(int shape, int refine, int G, const SymArgs& a, const
     } while (0)
     if (shape == 1) HSMA_LAT_SYM(1, 1, 1, 0);
     else if (shape == 2) HSMA_LAT_SYM(1, 1, 1, 7);
+    else if (shape == 4) HSMA_LAT_SYM(1, 1, 1, 4);
     else HSMA_LAT_SYM(1, 1, 2, 4);
 #undef HSMA_LAT_SYM
 }
@@ -765,6 +768,7 @@ static void launch_lat_sym_field(int shape, int refine, int G, const SymArgs& a,
     } while (0)
     if (shape == 1) HSMA_LAT_SYMF(1, 1, 1, 0);
     else if (shape == 2) HSMA_LAT_SYMF(1, 1, 1, 7);
+    else if (shape == 4) HSMA_LAT_SYMF(1, 1, 1, 4);
     else HSMA_LAT_SYMF(1, 1, 2, 4);
 #undef HSMA_LAT_SYMF
 }

@@ -2,7 +2,7 @@
 for the full box of image cells of PAPER.md:40-50 Eq.(3)/(4); one add per image for r^2, charges and cell weights once
 per pair) against the CPU oracle and against the cell-by-cell kernels they replace, through the C-ABI.  Every shape that
 is instantiated -- 27 periodic cells, 27 reflected cells (gamma = -1 and +1), 45 slab cells (3 x 3 periodic x 5 reflected,
-gamma = 0.5 and -1) -- in the ordered form (small N, target shards, step (a)), the symmetric form (N >= 7,937) and their
+gamma = 0.5 and -1), 27 slab cells (3 x 3 periodic x 3 reflected) -- in the ordered form (small N, target shards, step (a)), the symmetric form (N >= 7,937) and their
 gradient forms; both refinements; and the geometries that must keep the cell-by-cell kernels.  Bars as in
 test_gpu_parity (north_star).  All `-m gpu`."""
 import math
@@ -114,6 +114,21 @@ def test_other_closures(H, closure):
         w = W.config(2, N=1100)
         w = w.with_(closure=W.CLOSURE_FACE_PAIRS, check_xyz=W.seeded_face_points(w.K, w.L, W.LOWER_FACES, seed=3))
     check(w, O.hsma(w, forces=True), on_and_off(H, w, True), True)
+
+
+@pytest.mark.parametrize("forces", [False, True])
+@pytest.mark.parametrize("N", [2501, 9003])
+def test_slab_with_one_shell(H, N, forces):
+    """The slab kind with near shell (1,1,1) -- what hsma_plan_create(L, SLAB, near_shell = 1, ...) builds: 27 cells, z
+    reflecting (weights gamma^|k_z|), grounded plates closed by their own boundary conditions.  Ordered and symmetric forms."""
+    rng = np.random.default_rng(17)
+    L = (1.0, 1.0, 0.8)
+    xyz = rng.random((N, 3)) * np.asarray(L)
+    xyz[:, 2] = 0.02 * L[2] + 0.96 * xyz[:, 2]
+    w = W.Workload("slab_one_shell", W.BC_SLAB_XY_PERIODIC_Z_MIRROR, L, (1, 1, 1), -1.0, 1.0, 10, 3000, 700, xyz,
+                   rng.standard_normal(N) + 0.1, closure=W.CLOSURE_BOUNDARY)
+    form = check(w, O.hsma(w, forces=forces), on_and_off(H, w, forces), forces)
+    assert form == (2 if N >= 7937 else 1)
 
 
 def test_target_shards(H):
